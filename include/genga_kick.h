@@ -1,0 +1,156 @@
+/*
+ * genga_kick.h -- C ABI of the B200-native GENGA kick + close-encounter pre-check.
+ *
+ * The one operation behind this boundary is the interaction part H_B of the hybrid symplectic
+ * integrator of arXiv 2201.10058 (eq. 3; App. A PAPER.md:986-992 "Kick(dt/2),
+ * close-encounter pre-check"):
+ *
+ *   a_i = sum_{j in [0, n_massive), j != i}  G m_j W_L(r_ij) (x_j - x_i) / r_ij^3
+ *
+ *   W_0 = K(r; rc0_ij)
+ *   W_L = prod_{k<L} [1 - K(r; rck_ij)] * K(r; rcL_ij)         eq. 62-63
+ *   K(r; rc): y = (r - 0.1 rc)/(0.9 rc); 0 for y <= 0; 1 for y >= 1; else y^2/(2y^2 - 2y + 1)
+ *   rck_ij = max(rcrit[k][i], rcrit[k][j])                     eq. 5
+ *   pre-check: (i, j) is an encounter pair iff r_ij^2 < (enc_factor * rcL_ij)^2   (strict)
+ *
+ * Bodies [0, n_massive) interact fully; bodies [n_massive, n_massive + n_test) are semi-active
+ * test particles: they feel the massive bodies and not each other, and exert no force on this
+ * path (sec. 8.1).  Readings of the paper where it is silent: DESIGN.md.
+ *
+ * All functions return 0 on success or a negative genga_kick_error.  Nothing throws, aborts or
+ * prints.  Nothing falls back to the CPU: without a usable CUDA device genga_kick_init fails.
+ */
+#ifndef GENGA_KICK_H
+#define GENGA_KICK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GENGA_KICK_OK        =  0,
+    GENGA_KICK_E_NULL    = -1,   /* a required pointer is NULL                                   */
+    GENGA_KICK_E_ALIGN   = -2,   /* a device pointer is not 16-byte aligned                      */
+    GENGA_KICK_E_SIZE    = -3,   /* n_massive < 0, n_test < 0, N == 0 or N > 2^30, capacity < 0  */
+    GENGA_KICK_E_LEVEL   = -4,   /* changeover_level outside [0, max_level]                      */
+    GENGA_KICK_E_CUDA    = -5,   /* a CUDA call failed; genga_kick_last_cuda_error() has the text */
+    GENGA_KICK_E_NOMEM   = -6    /* host allocation failed                                       */
+} genga_kick_error;
+
+/* bits of the device status word (genga_kick_status) */
+#define GENGA_KICK_STATUS_COINCIDENT 1   /* two distinct bodies at the same position were met
+                                            (outside the domain; that pair was skipped)          */
+
+typedef struct genga_kick_ctx genga_kick_ctx;   /* opaque; owned by the library */
+
+typedef struct {
+    int32_t n_massive;      /* fully interacting bodies: indices [0, n_massive)                    */
+    int32_t n_test;         /* semi-active test particles: [n_massive, n_massive + n_test)         */
+    int32_t max_level;      /* largest changeover_level that will be passed (0 = original K only)  */
+    int32_t device;         /* CUDA device ordinal                                                 */
+    int64_t pair_capacity;  /* rows available in out_pairs                                         */
+    double  G;              /* gravitational constant; k^2, k = 0.01720209895 in AU / day / Msun   */
+    double  enc_factor;     /* f in r_ij < f * rcL_ij; 1.0                                         */
+} genga_kick_config;
+
+/*
+ * How one call is cut into CTAs (host logic, no CUDA call; exported so it can be tested on a
+ * machine without a GPU).  The kick is a grid of tiles (i-block x j-tile), i-major; CTA c owns
+ * the contiguous tile range [c*T/n_ctas, (c+1)*T/n_ctas) and writes one partial-sum segment per
+ * i-block it touches; a second pass adds the segments of each i-block in ascending CTA order
+ * (fixed order => bit-reproducible).
+ */
+typedef struct {
+    int32_t threads;        /* threads per CTA                                                     */
+    int32_t i_per_thread;   /* i-bodies owned by one thread                                        */
+    int32_t i_block;        /* = threads * i_per_thread                                            */
+    int32_t j_tile;         /* j-bodies per shared-memory tile                                     */
+    int32_t m_pad;          /* records [0, m_pad): massive bodies + padding; test particles follow  */
+    int32_t n_i_blocks;     /* ceil(n_i / i_block), n_i = n_test ? m_pad + n_test : n_massive      */
+    int32_t n_j_tiles;      /* ceil(n_massive / j_tile)                                            */
+    int64_t n_tiles;        /* T = n_i_blocks * n_j_tiles                                          */
+    int32_t n_ctas;         /* CTAs launched (a multiple of the SM count unless T is smaller)      */
+    int32_t max_segs;       /* most i-blocks any CTA touches                                       */
+    int64_t n_rec;          /* records allocated (n_i rounded up to a multiple of 1024)            */
+    int64_t partial_doubles;/* doubles of scratch for the partial sums                             */
+} genga_kick_plan;
+
+/* Fill *plan for a problem of n_massive + n_test bodies at changeover level `level` on a device
+ * with num_sms multiprocessors.  Errors: E_NULL, E_SIZE, E_LEVEL (level < 0). */
+int genga_kick_make_plan(int32_t n_massive, int32_t n_test, int32_t level, int32_t num_sms,
+                         genga_kick_plan* plan);
+/* Tile range [*t0, *t1) of CTA `cta` under *plan.  Errors: E_NULL, E_SIZE. */
+int genga_kick_plan_cta_range(const genga_kick_plan* plan, int32_t cta, int64_t* t0, int64_t* t1);
+/* First and last CTA whose range meets i-block `ib`.  Errors: E_NULL, E_SIZE. */
+int genga_kick_plan_iblock_ctas(const genga_kick_plan* plan, int32_t ib, int32_t* c_first, int32_t* c_last);
+
+/* Create a context on cfg->device: allocates the library's scratch (packed j-bodies, partial
+ * sums, host-call staging is allocated lazily).  *out_ctx is written only on success.
+ * Errors: E_NULL, E_SIZE, E_LEVEL, E_CUDA (no device, wrong device, out of memory). */
+int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** out_ctx);
+
+/* Stream the following genga_kick calls enqueue on (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream; NULL = the default stream).  Not owned. */
+int genga_kick_set_stream(genga_kick_ctx* ctx, void* cuda_stream);
+
+/*
+ * One kick + pre-check.  N = n_massive + n_test.  Every array is DEVICE memory owned by the
+ * caller, 16-byte aligned, and must stay valid until the stream has run the call.  The call only
+ * enqueues kernels on the context's stream; it never synchronises.
+ *
+ *   pos        [3][N] SoA (x[0..N), y[0..N), z[0..N)), heliocentric positions        (read)
+ *   vel        [3][N] SoA or NULL; if non-NULL, v += dt * a in place (what Kick(dt/2) of
+ *              App. A does with dt = half the step)                                   (read/write)
+ *   mass       [N]                                                                    (read)
+ *   rcrit      [changeover_level + 1][N]: row k = r_crit,i at time step dt / s^k      (read)
+ *   out_acc    [3][N] SoA accelerations; NULL allowed only if vel is non-NULL         (write)
+ *   out_pairs  [pair_capacity][2] int32, each unordered encounter pair once as (lo, hi),
+ *              rows in arbitrary order; may be NULL if pair_capacity == 0 (write)
+ *   out_npairs [N + 1] int32: [i] = number of encounter partners of body i (a massive body also
+ *              counts its test-particle partners); [N] = TRUE number of pairs found.  If
+ *              [N] > pair_capacity the rows beyond capacity were dropped (never written out of
+ *              bounds) and the caller re-calls with a larger buffer.                  (write)
+ *
+ * out_acc and out_npairs are bit-reproducible from call to call; out_pairs is a set.
+ * Errors: E_NULL, E_ALIGN, E_LEVEL, E_CUDA.
+ */
+int genga_kick(genga_kick_ctx* ctx,
+               const double* pos, double* vel, const double* mass, const double* rcrit,
+               int32_t changeover_level, double dt,
+               double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
+
+/*
+ * The same call with HOST arrays (same shapes; any alignment; vel and out_acc may be NULL as
+ * above, out_pairs may be NULL): copies the inputs to library-owned device buffers, runs
+ * genga_kick, copies the results back and synchronises the stream before returning.  At most
+ * min([N], pair_capacity) pair rows are copied back.  Errors: as genga_kick.
+ */
+int genga_kick_host(genga_kick_ctx* ctx,
+                    const double* pos, double* vel, const double* mass, const double* rcrit,
+                    int32_t changeover_level, double dt,
+                    double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
+
+/* Plan the context uses at `changeover_level` (what genga_kick will launch). */
+int genga_kick_get_plan(const genga_kick_ctx* ctx, int32_t changeover_level, genga_kick_plan* plan);
+
+/* Synchronise the stream and read the device status word (GENGA_KICK_STATUS_* bits, OR-ed over
+ * all calls since init) into *status. */
+int genga_kick_status(genga_kick_ctx* ctx, int32_t* status);
+
+/* Kernel launches enqueued by the context since init (for the bench's launch count). */
+int64_t genga_kick_launch_count(const genga_kick_ctx* ctx);
+
+/* Free the context and its scratch.  NULL is allowed. */
+int genga_kick_free(genga_kick_ctx* ctx);
+
+/* Static text for an error code. */
+const char* genga_kick_strerror(int code);
+/* Text of the last CUDA error seen by this context ("" if none); valid until the next call. */
+const char* genga_kick_last_cuda_error(const genga_kick_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GENGA_KICK_H */

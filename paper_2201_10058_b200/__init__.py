@@ -1,0 +1,11 @@
+"""B200-native GENGA kick + close-encounter pre-check (arXiv 2201.10058, eq. 3 / eq. 62-63 / App. A).
+
+The product is the C-ABI library libgenga_kick.so (include/genga_kick.h, csrc/); this package is
+its thin ctypes binding.  It never imports oracle/ and has no CPU fallback."""
+from .binding import (GengaKick, GengaKickConfig, GengaKickPlan, GengaKickError, lib, make_plan, plan_cta_range,
+                      plan_iblock_ctas, strerror, EXPORTS, LIB_PATH, STATUS_COINCIDENT,
+                      OK, E_NULL, E_ALIGN, E_SIZE, E_LEVEL, E_CUDA, E_NOMEM)
+
+__all__ = ["GengaKick", "GengaKickConfig", "GengaKickPlan", "GengaKickError", "lib", "make_plan", "plan_cta_range",
+           "plan_iblock_ctas", "strerror", "EXPORTS", "LIB_PATH", "STATUS_COINCIDENT",
+           "OK", "E_NULL", "E_ALIGN", "E_SIZE", "E_LEVEL", "E_CUDA", "E_NOMEM"]

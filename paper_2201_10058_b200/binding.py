@@ -1,0 +1,163 @@
+"""Thin ctypes binding of libgenga_kick.so (include/genga_kick.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the library's CUDA
+kernels.  There is no CPU fallback: if the library is missing or no sm_100 device is present the
+calls raise."""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libgenga_kick.so")
+
+OK, E_NULL, E_ALIGN, E_SIZE, E_LEVEL, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4, -5, -6
+STATUS_COINCIDENT = 1
+
+EXPORTS = (
+    "genga_kick_make_plan", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
+    "genga_kick_set_stream", "genga_kick", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
+    "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
+)
+
+
+class GengaKickConfig(C.Structure):
+    _fields_ = [("n_massive", C.c_int32), ("n_test", C.c_int32), ("max_level", C.c_int32), ("device", C.c_int32),
+                ("pair_capacity", C.c_int64), ("G", C.c_double), ("enc_factor", C.c_double)]
+
+
+class GengaKickPlan(C.Structure):
+    _fields_ = [("threads", C.c_int32), ("i_per_thread", C.c_int32), ("i_block", C.c_int32), ("j_tile", C.c_int32),
+                ("m_pad", C.c_int32), ("n_i_blocks", C.c_int32), ("n_j_tiles", C.c_int32), ("n_tiles", C.c_int64),
+                ("n_ctas", C.c_int32), ("max_segs", C.c_int32), ("n_rec", C.c_int64), ("partial_doubles", C.c_int64)]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+class GengaKickError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"genga_kick error {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built (python -m paper_2201_10058_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2201_10058_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, d = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        L.genga_kick_make_plan.argtypes = [i32, i32, i32, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_plan_cta_range.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i64), C.POINTER(i64)]
+        L.genga_kick_plan_iblock_ctas.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i32), C.POINTER(i32)]
+        L.genga_kick_init.argtypes = [C.POINTER(GengaKickConfig), C.POINTER(vp)]
+        L.genga_kick_set_stream.argtypes = [vp, vp]
+        L.genga_kick.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, vp]
+        L.genga_kick_host.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, vp]
+        L.genga_kick_get_plan.argtypes = [vp, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_status.argtypes = [vp, C.POINTER(i32)]
+        L.genga_kick_launch_count.argtypes = [vp]
+        L.genga_kick_launch_count.restype = i64
+        L.genga_kick_free.argtypes = [vp]
+        L.genga_kick_strerror.argtypes = [C.c_int]
+        L.genga_kick_strerror.restype = C.c_char_p
+        L.genga_kick_last_cuda_error.argtypes = [vp]
+        L.genga_kick_last_cuda_error.restype = C.c_char_p
+        for name in EXPORTS:
+            if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().genga_kick_strerror(int(code)).decode()
+
+
+def make_plan(n_massive: int, n_test: int, level: int, num_sms: int) -> GengaKickPlan:
+    plan = GengaKickPlan()
+    rc = lib().genga_kick_make_plan(n_massive, n_test, level, num_sms, C.byref(plan))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
+    return plan
+
+
+def plan_cta_range(plan: GengaKickPlan, cta: int):
+    t0, t1 = C.c_int64(), C.c_int64()
+    rc = lib().genga_kick_plan_cta_range(C.byref(plan), cta, C.byref(t0), C.byref(t1))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
+    return t0.value, t1.value
+
+
+def plan_iblock_ctas(plan: GengaKickPlan, ib: int):
+    a, b = C.c_int32(), C.c_int32()
+    rc = lib().genga_kick_plan_iblock_ctas(C.byref(plan), ib, C.byref(a), C.byref(b))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
+    return a.value, b.value
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class GengaKick:
+    """A genga_kick context.  Arrays are torch tensors (device tensors for kick(), CPU tensors for
+    kick_host()), float64 / int32, C-contiguous, laid out as include/genga_kick.h states."""
+
+    def __init__(self, n_massive, n_test=0, max_level=0, pair_capacity=1 << 20, G=1.0, enc_factor=1.0, device=0):
+        self.cfg = GengaKickConfig(int(n_massive), int(n_test), int(max_level), int(device), int(pair_capacity),
+                                   float(G), float(enc_factor))
+        self.n = int(n_massive) + int(n_test)
+        self._ctx = C.c_void_p()
+        rc = lib().genga_kick_init(C.byref(self.cfg), C.byref(self._ctx))
+        if rc != OK:
+            raise GengaKickError(rc, strerror(rc))
+
+    def _check(self, rc):
+        if rc != OK:
+            text = strerror(rc)
+            if rc == E_CUDA:
+                text += ": " + lib().genga_kick_last_cuda_error(self._ctx).decode()
+            raise GengaKickError(rc, text)
+
+    def set_stream(self, cuda_stream: int):
+        self._check(lib().genga_kick_set_stream(self._ctx, C.c_void_p(int(cuda_stream))))
+
+    def kick(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
+        self._check(lib().genga_kick(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit), int(changeover_level),
+                                     float(dt), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs)))
+
+    def kick_host(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
+        self._check(lib().genga_kick_host(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit),
+                                          int(changeover_level), float(dt), _ptr(out_acc), _ptr(out_pairs),
+                                          _ptr(out_npairs)))
+
+    def plan(self, changeover_level=0) -> GengaKickPlan:
+        plan = GengaKickPlan()
+        self._check(lib().genga_kick_get_plan(self._ctx, int(changeover_level), C.byref(plan)))
+        return plan
+
+    def status(self) -> int:
+        s = C.c_int32()
+        self._check(lib().genga_kick_status(self._ctx, C.byref(s)))
+        return s.value
+
+    def launch_count(self) -> int:
+        return int(lib().genga_kick_launch_count(self._ctx))
+
+    def free(self):
+        if self._ctx:
+            lib().genga_kick_free(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass

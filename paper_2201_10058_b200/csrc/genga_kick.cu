@@ -1,0 +1,264 @@
+// C ABI of the B200-native GENGA kick + close-encounter pre-check (include/genga_kick.h).
+// Host side only: argument checks, scratch ownership, kernel launches on the caller's stream.
+// Every step of the path runs in the kernels of genga_kick_kernels.cuh; there is no CPU fallback.
+#include "../../include/genga_kick.h"
+#include "genga_kick_variants.h"
+#include "genga_kick_kernels.cuh"
+
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+struct genga_kick_ctx {
+    genga_kick_config cfg;
+    int64_t N;
+    int num_sms;
+    cudaStream_t stream;
+    genga_kick_plan* plans;        // one per level 0..max_level
+    // scratch (device)
+    double2* rxy;
+    double2* rzm;
+    int* rfw;
+    int* ridx;
+    int* cfw;
+    double* partial;
+    int* status;
+    int64_t n_rec_alloc;
+    // staging for genga_kick_host (device, lazily allocated)
+    double* h_pos; double* h_vel; double* h_mass; double* h_rcrit; double* h_acc;
+    int32_t* h_pairs; int32_t* h_npairs;
+    int64_t launches;
+    std::string cuda_err;
+};
+
+namespace {
+
+int cuda_fail(genga_kick_ctx* ctx, cudaError_t e)
+{
+    if (ctx) ctx->cuda_err = cudaGetErrorString(e);
+    return GENGA_KICK_E_CUDA;
+}
+#define GK_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_); } while (0)
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+template <int THREADS, int IPT, int JT, int CTAS, bool DENSE>
+cudaError_t launch_kick(const genga::KickParams& kp, cudaStream_t st)
+{
+    genga::kick_kernel<THREADS, IPT, JT, CTAS, DENSE><<<kp.n_ctas, THREADS, 0, st>>>(kp);
+    return cudaGetLastError();
+}
+
+// the compiled shapes: must list every entry of GENGA_DENSE_VARIANTS / GENGA_SPARSE_VARIANTS
+cudaError_t dispatch_kick(const genga_kick_plan& pl, bool dense, const genga::KickParams& kp, cudaStream_t st)
+{
+#define GK_SHAPE(T, I, J, C)                                                          \
+    if (pl.threads == T && pl.i_per_thread == I && pl.j_tile == J)                    \
+        return dense ? launch_kick<T, I, J, C, true>(kp, st) : launch_kick<T, I, J, C, false>(kp, st);
+    GK_SHAPE(256, 2, 256, 2)
+    GK_SHAPE(128, 2, 128, 4)
+    GK_SHAPE(128, 1, 64, 4)
+#undef GK_SHAPE
+    return cudaErrorInvalidConfiguration;
+}
+
+}  // namespace
+
+extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** out_ctx)
+{
+    if (!cfg || !out_ctx) return GENGA_KICK_E_NULL;
+    const int64_t N = (int64_t)cfg->n_massive + (int64_t)cfg->n_test;
+    if (cfg->n_massive < 0 || cfg->n_test < 0 || N <= 0 || N > GENGA_MAX_BODIES || cfg->pair_capacity < 0)
+        return GENGA_KICK_E_SIZE;
+    if (cfg->max_level < 0 || cfg->max_level > 62) return GENGA_KICK_E_LEVEL;
+
+    genga_kick_ctx* ctx = new (std::nothrow) genga_kick_ctx();
+    if (!ctx) return GENGA_KICK_E_NOMEM;
+    ctx->cfg = *cfg;
+    ctx->N = N;
+    ctx->stream = nullptr;
+    ctx->launches = 0;
+
+    int rc = GENGA_KICK_OK;
+    cudaError_t e;
+    int ndev = 0;
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceCount(&ndev)) != cudaSuccess) goto cuda_error;
+    if (cfg->device < 0 || cfg->device >= ndev) { e = cudaErrorInvalidDevice; goto cuda_error; }
+    if ((e = cudaSetDevice(cfg->device)) != cudaSuccess) goto cuda_error;
+    if ((e = cudaGetDeviceProperties(&prop, cfg->device)) != cudaSuccess) goto cuda_error;
+    if (prop.major != 10) { e = cudaErrorNoKernelImageForDevice; goto cuda_error; }   // sm_100a only
+    ctx->num_sms = prop.multiProcessorCount;
+
+    ctx->plans = static_cast<genga_kick_plan*>(std::calloc((size_t)cfg->max_level + 1, sizeof(genga_kick_plan)));
+    if (!ctx->plans) { rc = GENGA_KICK_E_NOMEM; goto fail; }
+    {
+        int64_t max_partial = 1;
+        for (int l = 0; l <= cfg->max_level; l++) {
+            rc = genga_kick_make_plan(cfg->n_massive, cfg->n_test, l, ctx->num_sms, &ctx->plans[l]);
+            if (rc != GENGA_KICK_OK) goto fail;
+            if (ctx->plans[l].partial_doubles > max_partial) max_partial = ctx->plans[l].partial_doubles;
+        }
+        const int64_t nr = ctx->plans[0].n_rec;
+        ctx->n_rec_alloc = nr;
+        if ((e = cudaMalloc(&ctx->rxy, (size_t)nr * sizeof(double2))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->rzm, (size_t)nr * sizeof(double2))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->rfw, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->ridx, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->cfw, (size_t)(nr / GENGA_CHUNK) * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->partial, (size_t)max_partial * sizeof(double))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->status, sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMemset(ctx->status, 0, sizeof(int))) != cudaSuccess) goto cuda_error;
+    }
+    *out_ctx = ctx;
+    return GENGA_KICK_OK;
+
+cuda_error:
+    (void)e;
+    rc = GENGA_KICK_E_CUDA;
+fail:
+    genga_kick_free(ctx);
+    return rc;
+}
+
+extern "C" int genga_kick_set_stream(genga_kick_ctx* ctx, void* cuda_stream)
+{
+    if (!ctx) return GENGA_KICK_E_NULL;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
+                          int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs)
+{
+    if (!ctx || !pos || !mass || !rcrit || !out_npairs) return GENGA_KICK_E_NULL;
+    if (!out_acc && !vel) return GENGA_KICK_E_NULL;
+    if (!out_pairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
+    if (misaligned(pos) || misaligned(vel) || misaligned(mass) || misaligned(rcrit) || misaligned(out_acc) ||
+        misaligned(out_pairs) || misaligned(out_npairs))
+        return GENGA_KICK_E_ALIGN;
+    if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
+
+    const genga_kick_plan& pl = ctx->plans[changeover_level];
+    const int N = (int)ctx->N;
+    const int n_rec = (int)pl.n_rec;
+    cudaStream_t st = ctx->stream;
+
+    {
+        const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
+        genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, nullptr, N, ctx->cfg.n_massive, pl.m_pad, n_rec,
+                                                   changeover_level, ctx->cfg.G, ctx->cfg.enc_factor, ctx->rxy, ctx->rzm,
+                                                   ctx->rfw, ctx->ridx, ctx->cfw, out_npairs);
+        GK_CUDA(ctx, cudaGetLastError());
+        ctx->launches++;
+    }
+    if (pl.n_ctas > 0) {
+        genga::KickParams kp;
+        kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx; kp.cfw = ctx->cfw;
+        kp.rcrit = rcrit;
+        kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
+        kp.n_j_tiles = pl.n_j_tiles; kp.n_ctas = pl.n_ctas; kp.max_segs = pl.max_segs; kp.n_tiles = pl.n_tiles;
+        kp.partial = ctx->partial;
+        kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
+        kp.status = ctx->status;
+        GK_CUDA(ctx, dispatch_kick(pl, changeover_level == 0, kp, st));
+        ctx->launches++;
+    }
+    {
+        genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(ctx->partial, ctx->ridx, n_rec, N, pl.i_block, pl.n_j_tiles,
+                                                                  pl.n_tiles, pl.n_ctas, pl.max_segs, dt, out_acc, vel);
+        GK_CUDA(ctx, cudaGetLastError());
+        ctx->launches++;
+    }
+    return GENGA_KICK_OK;
+}
+
+namespace {
+template <typename T>
+int ensure(genga_kick_ctx* ctx, T** p, size_t count)
+{
+    if (*p) return GENGA_KICK_OK;
+    GK_CUDA(ctx, cudaMalloc(p, count * sizeof(T) + 16));
+    return GENGA_KICK_OK;
+}
+}  // namespace
+
+extern "C" int genga_kick_host(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass,
+                               const double* rcrit, int32_t changeover_level, double dt, double* out_acc,
+                               int32_t* out_pairs, int32_t* out_npairs)
+{
+    if (!ctx || !pos || !mass || !rcrit || !out_npairs) return GENGA_KICK_E_NULL;
+    if (!out_acc && !vel) return GENGA_KICK_E_NULL;
+    if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
+    const size_t N = (size_t)ctx->N;
+    const size_t cap = (size_t)ctx->cfg.pair_capacity;
+    const size_t rows = (size_t)ctx->cfg.max_level + 1;
+    cudaStream_t st = ctx->stream;
+    int rc;
+    if ((rc = ensure(ctx, &ctx->h_pos, 3 * N))) return rc;
+    if ((rc = ensure(ctx, &ctx->h_mass, N))) return rc;
+    if ((rc = ensure(ctx, &ctx->h_rcrit, rows * N))) return rc;
+    if ((rc = ensure(ctx, &ctx->h_acc, 3 * N))) return rc;
+    if ((rc = ensure(ctx, &ctx->h_npairs, N + 1))) return rc;
+    if ((rc = ensure(ctx, &ctx->h_pairs, 2 * cap + 4))) return rc;
+    if (vel && (rc = ensure(ctx, &ctx->h_vel, 3 * N))) return rc;
+
+    GK_CUDA(ctx, cudaMemcpyAsync(ctx->h_pos, pos, 3 * N * sizeof(double), cudaMemcpyHostToDevice, st));
+    GK_CUDA(ctx, cudaMemcpyAsync(ctx->h_mass, mass, N * sizeof(double), cudaMemcpyHostToDevice, st));
+    GK_CUDA(ctx, cudaMemcpyAsync(ctx->h_rcrit, rcrit, ((size_t)changeover_level + 1) * N * sizeof(double),
+                                 cudaMemcpyHostToDevice, st));
+    if (vel) GK_CUDA(ctx, cudaMemcpyAsync(ctx->h_vel, vel, 3 * N * sizeof(double), cudaMemcpyHostToDevice, st));
+
+    rc = genga_kick(ctx, ctx->h_pos, vel ? ctx->h_vel : nullptr, ctx->h_mass, ctx->h_rcrit, changeover_level, dt,
+                    ctx->h_acc, cap ? ctx->h_pairs : nullptr, ctx->h_npairs);
+    if (rc != GENGA_KICK_OK) return rc;
+
+    if (out_acc) GK_CUDA(ctx, cudaMemcpyAsync(out_acc, ctx->h_acc, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (vel) GK_CUDA(ctx, cudaMemcpyAsync(vel, ctx->h_vel, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    GK_CUDA(ctx, cudaMemcpyAsync(out_npairs, ctx->h_npairs, (N + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    GK_CUDA(ctx, cudaStreamSynchronize(st));
+    if (out_pairs && cap) {
+        size_t got = (size_t)out_npairs[N];
+        if (got > cap) got = cap;
+        if (got) GK_CUDA(ctx, cudaMemcpyAsync(out_pairs, ctx->h_pairs, 2 * got * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        GK_CUDA(ctx, cudaStreamSynchronize(st));
+    }
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_get_plan(const genga_kick_ctx* ctx, int32_t changeover_level, genga_kick_plan* plan)
+{
+    if (!ctx || !plan) return GENGA_KICK_E_NULL;
+    if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
+    *plan = ctx->plans[changeover_level];
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_status(genga_kick_ctx* ctx, int32_t* status)
+{
+    if (!ctx || !status) return GENGA_KICK_E_NULL;
+    GK_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    GK_CUDA(ctx, cudaMemcpy(status, ctx->status, sizeof(int), cudaMemcpyDeviceToHost));
+    return GENGA_KICK_OK;
+}
+
+extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int genga_kick_free(genga_kick_ctx* ctx)
+{
+    if (!ctx) return GENGA_KICK_OK;
+    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->partial, ctx->status, ctx->h_pos,
+                    ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs};
+    for (void* b : bufs)
+        if (b) cudaFree(b);
+    std::free(ctx->plans);
+    delete ctx;
+    return GENGA_KICK_OK;
+}
+
+extern "C" const char* genga_kick_last_cuda_error(const genga_kick_ctx* ctx)
+{
+    return ctx ? ctx->cuda_err.c_str() : "";
+}

@@ -1,0 +1,421 @@
+// sm_100a kernels of the GENGA kick + close-encounter pre-check.
+//
+//   pack_kernel    O(N): writes the body RECORDS the pair loop reads (positions, G m, filter word,
+//                  caller's index) in the library's internal order, the per-chunk filter maxima,
+//                  and clears the encounter counters.
+//   kick_kernel    O(N * n_massive): the pair loop (eq. 3 PAPER.md:63-64 with the weights of
+//                  eq. 62-63, fused with the pre-check of App. A).
+//   reduce_kernel  O(N): fixed-order sum of the partial accelerations, scatter to
+//                  the caller's order, optional v += dt * a (the Kick of App. A).
+//
+// No code, header, table or helper is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace genga {
+
+#define GENGA_STATUS_COINCIDENT 1
+// Padding records sit far from every real body; records used as i-bodies and as j-bodies share
+// one array, so a padding i meets a padding j at distance 0 -- its lanes are never stored.
+#define GENGA_SENTINEL_POS 1.0e30
+#define GENGA_CHUNK 8              // j-records per filter chunk (one warp vote per chunk)
+#define GENGA_PAD 1024             // record arrays are padded to multiples of this
+
+struct KickParams {
+    // records (library scratch), internal order: massive bodies in [0, m_pad), semi-active test
+    // particles from m_pad on; padding records have idx = -1, G m = 0, filter word = -1
+    const double2* __restrict__ rxy;   // (x, y)
+    const double2* __restrict__ rzm;   // (z, G m)
+    const int* __restrict__ rfw;       // filter word (see filter_word)
+    const int* __restrict__ ridx;      // caller's body index, -1 for padding
+    const int* __restrict__ cfw;       // max filter word of each chunk of GENGA_CHUNK records
+    // the caller's arrays (read by the exact per-pair path only)
+    const double* __restrict__ rcrit;  // [L+1][N]
+    int N, n_massive, L;
+    double f;                          // enc_factor
+    // decomposition (genga_kick_plan)
+    int n_j_tiles, n_ctas, max_segs;
+    long long n_tiles;
+    double* __restrict__ partial;      // [n_ctas][max_segs][3][i_block]
+    // encounter output
+    int* __restrict__ out_pairs;       // [capacity][2]
+    long long capacity;
+    int* __restrict__ out_npairs;      // [N + 1]
+    int* __restrict__ status;
+};
+
+// ---------------------------------------------------------------------------------------------
+// Filter word of a body.  With R_b = max(rc0_b, f rcL_b), a pair (i, j) can only have W != 1
+// (level 0), W != 0 (level >= 1: the factor 1 - K_0 of eq. 63 PAPER.md:627-632 vanishes for
+// r >= rc0_ij) or be an encounter pair (r < f rcL_ij) if r < max(R_i, R_j).  Positive doubles
+// order like their bit patterns, so the test is done on the HIGH WORDS on the integer pipe
+// (DSETP runs at a quarter of the DFMA rate); the + 1 covers the truncated low word, the one-ulp
+// difference between the fused r^2 of the pair loop and the unfused r^2 of the exact path, and
+// the rounding of y = (r - 0.1 rc)/(0.9 rc) near 1: a pair that passes the filter has
+// r^2 >= R^2 (1 + 2^-20).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int filter_word(double rc0, double rcL, double f)
+{
+    const double m = fmax(rc0, __dmul_rn(f, rcL));
+    return __double2hiint(__dmul_rn(m, m)) + 1;
+}
+
+// perm == nullptr: internal order = caller's order.
+__global__ void __launch_bounds__(256)
+pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, const double* __restrict__ rcrit,
+            const int* __restrict__ perm, int N, int n_massive, int m_pad, int n_rec, int L, double G, double f,
+            double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
+            int* __restrict__ cfw, int* __restrict__ out_npairs)
+{
+    const int stride = gridDim.x * blockDim.x;       // a multiple of 32
+    const int top = max(n_rec, ((N + 1 + 31) / 32) * 32);
+    for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < top; r += stride) {
+        int fw = -1;
+        if (r < n_rec) {
+            int b = -1;                               // caller's index of record r
+            if (r < m_pad) { if (r < n_massive) b = r; }
+            else if (r - m_pad < N - n_massive) b = n_massive + (r - m_pad);
+            if (b >= 0 && perm) b = perm[b];
+            if (b >= 0) {
+                rxy[r] = make_double2(pos[b], pos[(size_t)N + b]);
+                rzm[r] = make_double2(pos[2 * (size_t)N + b], __dmul_rn(G, mass[b]));
+                fw = filter_word(rcrit[b], rcrit[(size_t)L * N + b], f);
+            } else {
+                rxy[r] = make_double2(GENGA_SENTINEL_POS, GENGA_SENTINEL_POS);
+                rzm[r] = make_double2(GENGA_SENTINEL_POS, 0.0);
+            }
+            rfw[r] = fw;
+            ridx[r] = b;
+        }
+        // chunk maximum over GENGA_CHUNK consecutive records (= consecutive lanes)
+        int m = fw;
+        m = max(m, __shfl_xor_sync(0xffffffffu, m, 1));
+        m = max(m, __shfl_xor_sync(0xffffffffu, m, 2));
+        m = max(m, __shfl_xor_sync(0xffffffffu, m, 4));
+        if (r < n_rec && (r % GENGA_CHUNK) == 0) cfw[r / GENGA_CHUNK] = m;
+        if (r <= N) out_npairs[r] = 0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The changeover function K (form of Chambers 1999 eq. 10, reading G1 of
+// DESIGN.md), evaluated with IEEE operations in a fixed order and no contraction.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double changeover_K(double r, double rc)
+{
+    const double y = __ddiv_rn(__dsub_rn(r, __dmul_rn(0.1, rc)), __dmul_rn(0.9, rc));
+    if (y <= 0.0) return 0.0;
+    if (y >= 1.0) return 1.0;
+    const double yy = __dmul_rn(y, y);
+    const double twoy = __dmul_rn(2.0, y);
+    const double den = __dadd_rn(__dsub_rn(__dmul_rn(twoy, y), twoy), 1.0);
+    return __ddiv_rn(yy, den);
+}
+
+struct ExactResult {
+    double s;     // G m_j W_L / r^3 (0 if the pair contributes nothing)
+    int enc;      // 1 if (i, j) is an encounter pair
+};
+
+// The exact per-pair evaluation for the few pairs the filter lets through: the level weight W_L
+// and the pre-check, in unfused IEEE arithmetic (so the strict comparison r^2 < (f rcL)^2 is taken
+// on the bits a plain left-to-right evaluation gives).  Out of line: it runs for ~1e-4 of the
+// pairs and must not cost the pair loop registers.  bi, bj are the caller's indices.
+__device__ __noinline__ ExactResult exact_pair(const double* __restrict__ rcrit, int N, int L, double f, int* status,
+                                               int bi, int bj, double dx, double dy, double dz, double gmj)
+{
+    ExactResult out;
+    out.s = 0.0;
+    out.enc = 0;
+    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    if (!(r2 > 0.0)) {                                             // coincident distinct bodies
+        atomicOr(status, GENGA_STATUS_COINCIDENT);
+        return out;
+    }
+    const double r = __dsqrt_rn(r2);
+    const size_t n = (size_t)N;
+    const double rcL = fmax(rcrit[L * n + bi], rcrit[L * n + bj]);
+    const double thr = __dmul_rn(f, rcL);
+    out.enc = r2 < __dmul_rn(thr, thr) ? 1 : 0;
+    double W = 1.0;
+    for (int k = 0; k < L; k++) {
+        const double rck = fmax(rcrit[k * n + bi], rcrit[k * n + bj]);
+        W = __dmul_rn(W, __dsub_rn(1.0, changeover_K(r, rck)));
+    }
+    W = __dmul_rn(W, changeover_K(r, rcL));
+    if (W != 0.0) out.s = __ddiv_rn(__dmul_rn(gmj, W), __dmul_rn(r2, r));
+    return out;
+}
+
+// One warp-wide emission step: lanes with `hit` append (lo, hi) to the pair list with one atomic
+// per warp (ballot + popc); rows beyond capacity are dropped but counted.
+__device__ __forceinline__ void emit_pairs(const KickParams& p, bool hit, int lo, int hi)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (m == 0) return;
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(m) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(p.out_npairs + p.N, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (hit) {
+        const long long slot = (long long)base + __popc(m & ((1u << lane) - 1u));
+        if (slot < p.capacity) reinterpret_cast<int2*>(p.out_pairs)[slot] = make_int2(lo, hi);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// mbarrier + 1-D TMA bulk copy (cp.async.bulk, SASS UBLKCP) for the j-tile staging
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra WAIT_%=;\n\t}"
+        ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// MUFU.RSQ64H: 1/sqrt to ~2^-20 from the high word only (low word of the result is 0); runs on
+// the SFU pipe, not the FP64 pipe.  Skipped (result 0) for pairs the filter catches, so that they
+// add exactly 0 in the pair loop and r2 = 0 (the self pair) never makes an infinity.
+__device__ __forceinline__ double rsqrt_seed_unless(double x, bool skip)
+{
+    double y = 0.0;
+    asm("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %2, 0;\n\t@!q rsqrt.approx.ftz.f64 %0, %1;\n\t}"
+        : "+d"(y) : "d"(x), "r"((int)skip));
+    return y;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The pair loop's arithmetic for one (i, j) -- ROW a2-a4 of SURVEY.md section 8(a).
+//   d = x_j - x_i, r2 = d.d                         3 DADD, 1 DMUL, 2 DFMA
+//   trig = hi(r2) < thr  (integer pipe)             the pair goes to the exact path instead
+//   DENSE (level 0, W = K = 1 for every pair that passes the filter):
+//     y0 = MUFU.RSQ64H(r2) ~ r^-1 (1 + O(2^-20));  e = 1 - r2 y0^2
+//     G m_j r^-3 = y0^2 (G m_j y0) (1 + e (3/2 + 15/8 e))  + O(e^3)      4 DMUL, 3 DFMA
+//     a += s d                                       3 DFMA
+//   16 FP64-pipe instructions, 24 flops.  Every DFMA but the three accumulations has at most two
+//   distinct register operands (a third costs a register-file cycle on this part).
+//   SPARSE (level >= 1): a pair that passes the filter has W_L = 0 exactly; nothing is added.
+// ---------------------------------------------------------------------------------------------
+template <bool DENSE>
+__device__ __forceinline__ void pair_fast(double xj, double yj, double zj, double gmj,
+                                          double xi, double yi, double zi, int thr,
+                                          double& ax, double& ay, double& az, bool& any)
+{
+    const double dx = __dsub_rn(xj, xi), dy = __dsub_rn(yj, yi), dz = __dsub_rn(zj, zi);
+    const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
+    const bool trig = __double2hiint(r2) < thr;
+    any |= trig;
+    if (DENSE) {
+        const double y0 = rsqrt_seed_unless(r2, trig);
+        const double t = __dmul_rn(y0, y0);
+        const double e = fma(-r2, t, 1.0);
+        const double g = __dmul_rn(gmj, y0);
+        const double u = __dmul_rn(t, g);
+        const double c = fma(1.875, e, 1.5);
+        const double q = fma(e, c, 1.0);
+        const double s = __dmul_rn(u, q);
+        ax = fma(s, dx, ax);
+        ay = fma(s, dy, ay);
+        az = fma(s, dz, az);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// kick_kernel.  CTA c owns the tiles [c T / C, (c+1) T / C) of the i-major (i-block x j-tile)
+// grid (genga_kick_plan); thread `tid` owns the IPT i-records ib * IB + k * THREADS + tid.
+// j-tiles are staged by TMA bulk copies into a two-stage shared-memory ring; every lane reads
+// the same j-record (LDS broadcast).  Per chunk of GENGA_CHUNK j-records one warp vote decides
+// whether any pair of the chunk needs the exact path.
+// ---------------------------------------------------------------------------------------------
+template <int JT>
+struct alignas(128) TileStage {
+    double2 xy[JT];
+    double2 zm[JT];
+    int cf[JT / GENGA_CHUNK];
+};
+
+template <int THREADS, int IPT, int JT, int CTAS, bool DENSE>
+__global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
+{
+    constexpr int IB = THREADS * IPT;
+    constexpr int NCH = JT / GENGA_CHUNK;
+    constexpr uint32_t TILE_BYTES = JT * 32 + NCH * 4;
+    __shared__ TileStage<JT> st[2];
+    __shared__ __align__(8) uint64_t full[2];
+
+    const int tid = threadIdx.x;
+    const long long t0 = plan_tile_begin(blockIdx.x, p.n_tiles, p.n_ctas);
+    const long long t1 = plan_tile_begin(blockIdx.x + 1, p.n_tiles, p.n_ctas);
+    if (t0 >= t1) return;
+
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    auto issue = [&](long long t, int s) {
+        const int jt = (int)(t % p.n_j_tiles);
+        mbar_expect_tx(&full[s], TILE_BYTES);
+        bulk_g2s(st[s].xy, p.rxy + (size_t)jt * JT, JT * 16, &full[s]);
+        bulk_g2s(st[s].zm, p.rzm + (size_t)jt * JT, JT * 16, &full[s]);
+        bulk_g2s(st[s].cf, p.cfw + (size_t)jt * NCH, NCH * 4, &full[s]);
+    };
+    if (tid == 0) {
+        issue(t0, 0);
+        if (t0 + 1 < t1) issue(t0 + 1, 1);
+    }
+
+    double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT];
+    int fi[IPT], bi[IPT], cnt[IPT];
+    const int first_ib = (int)(t0 / p.n_j_tiles);
+    int cur_ib = -1;
+
+    auto flush = [&]() {
+        const size_t base = ((size_t)blockIdx.x * p.max_segs + (cur_ib - first_ib)) * 3 * IB;
+#pragma unroll
+        for (int k = 0; k < IPT; k++) {
+            const int off = k * THREADS + tid;
+            p.partial[base + off] = ax[k];
+            p.partial[base + IB + off] = ay[k];
+            p.partial[base + 2 * IB + off] = az[k];
+            if (cnt[k] > 0 && bi[k] >= 0) atomicAdd(p.out_npairs + bi[k], cnt[k]);
+        }
+    };
+
+    for (long long t = t0; t < t1; ++t) {
+        const int it = (int)(t - t0);
+        const int s = it & 1;
+        const int ib = (int)(t / p.n_j_tiles);
+        const int jt = (int)(t - (long long)ib * p.n_j_tiles);
+        if (ib != cur_ib) {
+            if (cur_ib >= 0) flush();
+            cur_ib = ib;
+#pragma unroll
+            for (int k = 0; k < IPT; k++) {
+                const size_t r = (size_t)ib * IB + k * THREADS + tid;
+                const double2 a = p.rxy[r], b = p.rzm[r];
+                xi[k] = a.x; yi[k] = a.y; zi[k] = b.x;
+                fi[k] = p.rfw[r];
+                bi[k] = p.ridx[r];
+                ax[k] = ay[k] = az[k] = 0.0;
+                cnt[k] = 0;
+            }
+        }
+        mbar_wait(&full[s], (uint32_t)((it >> 1) & 1));
+        const TileStage<JT>& S = st[s];
+
+#pragma unroll 1
+        for (int jj = 0; jj < JT; jj += GENGA_CHUNK) {
+            const int cm = S.cf[jj / GENGA_CHUNK];
+            int thr[IPT];
+#pragma unroll
+            for (int k = 0; k < IPT; k++) thr[k] = max(fi[k], cm);
+            bool any = false;
+#pragma unroll
+            for (int u = 0; u < GENGA_CHUNK; u++) {
+                const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
+#pragma unroll
+                for (int k = 0; k < IPT; k++)
+                    pair_fast<DENSE>(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], any);
+            }
+            if (__any_sync(0xffffffffu, any)) {
+                // exact path: the pairs of this chunk that the filter caught (a3, a5, a6)
+#pragma unroll 1
+                for (int u = 0; u < GENGA_CHUNK; u++) {
+                    const int jrec = jt * JT + jj + u;
+                    const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
+#pragma unroll
+                    for (int k = 0; k < IPT; k++) {
+                        const double dx = __dsub_rn(xy.x, xi[k]), dy = __dsub_rn(xy.y, yi[k]), dz = __dsub_rn(zm.x, zi[k]);
+                        const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
+                        bool hit = false;
+                        int lo = 0, hi = 0;
+                        if (__double2hiint(r2) < thr[k] && ib * IB + k * THREADS + tid != jrec) {
+                            const int bj = p.ridx[jrec];
+                            if (bj >= 0 && bi[k] >= 0) {
+                                const ExactResult e = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi[k], bj, dx, dy, dz, zm.y);
+                                ax[k] = fma(e.s, dx, ax[k]);
+                                ay[k] = fma(e.s, dy, ay[k]);
+                                az[k] = fma(e.s, dz, az[k]);
+                                if (e.enc) {
+                                    cnt[k]++;
+                                    if (bi[k] >= p.n_massive) {          // test particle i, massive j
+                                        atomicAdd(p.out_npairs + bj, 1);
+                                        hit = true; lo = bj; hi = bi[k];
+                                    } else if (bi[k] < bj) {
+                                        hit = true; lo = bi[k]; hi = bj;
+                                    }
+                                }
+                            }
+                        }
+                        emit_pairs(p, hit, lo, hi);
+                    }
+                }
+            }
+        }
+        __syncthreads();                                   // every warp is done with stage s
+        if (tid == 0 && t + 2 < t1) issue(t + 2, s);
+    }
+    flush();
+}
+
+// ---------------------------------------------------------------------------------------------
+// reduce_kernel (row a8 + a7): record r sums the partial accelerations of the CTAs whose tile
+// range met its i-block, in ascending CTA order, and writes the caller's arrays.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, int n_rec, int N, int IB,
+              int n_j_tiles, long long n_tiles, int n_ctas, int max_segs, double dt,
+              double* __restrict__ out_acc, double* __restrict__ vel)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_rec) return;
+    const int b = ridx[r];
+    if (b < 0) return;
+    const int ib = r / IB, off = r - ib * IB;
+    const long long ta = (long long)ib * n_j_tiles, tb = ta + n_j_tiles - 1;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    const int c_first = n_ctas > 0 ? plan_tile_owner(ta, n_tiles, n_ctas) : 0;
+    const int c_last = n_ctas > 0 ? plan_tile_owner(tb, n_tiles, n_ctas) : -1;    // no massive body: a = 0
+    for (int c = c_first; c <= c_last; c++) {
+        const int seg = ib - (int)(plan_tile_begin(c, n_tiles, n_ctas) / n_j_tiles);
+        const double* q = partial + ((size_t)c * max_segs + seg) * 3 * IB + off;
+        a0 = __dadd_rn(a0, q[0]);
+        a1 = __dadd_rn(a1, q[IB]);
+        a2 = __dadd_rn(a2, q[2 * (size_t)IB]);
+    }
+    if (out_acc) {
+        out_acc[b] = a0;
+        out_acc[(size_t)N + b] = a1;
+        out_acc[2 * (size_t)N + b] = a2;
+    }
+    if (vel) {
+        vel[b] = fma(dt, a0, vel[b]);
+        vel[(size_t)N + b] = fma(dt, a1, vel[(size_t)N + b]);
+        vel[2 * (size_t)N + b] = fma(dt, a2, vel[2 * (size_t)N + b]);
+    }
+}
+
+}  // namespace genga

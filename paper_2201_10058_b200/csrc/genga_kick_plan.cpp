@@ -1,0 +1,97 @@
+// Host-side work decomposition of one kick (no CUDA here; see include/genga_kick.h).
+//
+// The pair matrix is cut into tiles: i-blocks of `i_block` bodies (all N bodies: massive first,
+// then the semi-active test particles, sec. 8.1) times j-tiles of `j_tile`
+// massive bodies.  Tiles are numbered i-major, t = ib * n_j_tiles + jt, and CTA c owns
+// [floor(c T / C), floor((c+1) T / C)).  This splits the j-range across CTAs when N is too small
+// to fill the SMs with whole i-blocks and balances to within one tile for any N.  Each CTA writes
+// one partial-sum segment per i-block it touches; the reduction pass adds the segments of an
+// i-block in ascending CTA order, a fixed order ("parallel reductions have a well
+// defined order").
+#include "../../include/genga_kick.h"
+#include "genga_kick_variants.h"
+
+static int64_t cta_t0(const genga_kick_plan* p, int64_t c)
+{
+    return plan_tile_begin(c, p->n_tiles, p->n_ctas);
+}
+
+extern "C" int genga_kick_make_plan(int32_t n_massive, int32_t n_test, int32_t level, int32_t num_sms,
+                                    genga_kick_plan* plan)
+{
+    if (!plan) return GENGA_KICK_E_NULL;
+    if (level < 0) return GENGA_KICK_E_LEVEL;
+    const int64_t N = (int64_t)n_massive + (int64_t)n_test;
+    if (n_massive < 0 || n_test < 0 || N <= 0 || N > GENGA_MAX_BODIES || num_sms <= 0) return GENGA_KICK_E_SIZE;
+
+    const genga_variant* vars = level == 0 ? GENGA_DENSE_VARIANTS : GENGA_SPARSE_VARIANTS;
+    genga_kick_plan p;
+    for (int v = 0; v < GENGA_N_VARIANTS; v++) {
+        p.threads = vars[v].threads;
+        p.i_per_thread = vars[v].i_per_thread;
+        p.i_block = p.threads * p.i_per_thread;
+        p.j_tile = vars[v].j_tile;
+        // records: massive bodies padded to a multiple of GENGA_M_ALIGN, then the test particles
+        p.m_pad = (int32_t)(((int64_t)n_massive + GENGA_M_ALIGN - 1) / GENGA_M_ALIGN * GENGA_M_ALIGN);
+        const int64_t n_i = n_test > 0 ? (int64_t)p.m_pad + n_test : (int64_t)n_massive;
+        p.n_rec = (n_i + GENGA_REC_ALIGN - 1) / GENGA_REC_ALIGN * GENGA_REC_ALIGN;
+        if (p.n_rec < p.m_pad) p.n_rec = (p.m_pad + GENGA_REC_ALIGN - 1) / GENGA_REC_ALIGN * GENGA_REC_ALIGN;
+        p.n_i_blocks = (int32_t)((n_i + p.i_block - 1) / p.i_block);
+        p.n_j_tiles = (n_massive + p.j_tile - 1) / p.j_tile;
+        p.n_tiles = (int64_t)p.n_i_blocks * p.n_j_tiles;
+        p.n_ctas = num_sms * vars[v].ctas_per_sm;
+        if (p.n_tiles >= (int64_t)GENGA_MIN_TILES_PER_CTA * p.n_ctas) break;
+    }
+    if (p.n_tiles < p.n_ctas) p.n_ctas = (int32_t)p.n_tiles;      // 0 CTAs when there is no massive body
+
+    // most i-blocks any CTA touches
+    int32_t max_segs = 1;
+    if (p.n_j_tiles > 0) {
+        for (int64_t c = 0; c < p.n_ctas; c++) {
+            const int64_t t0 = cta_t0(&p, c), t1 = cta_t0(&p, c + 1);
+            if (t1 <= t0) continue;
+            const int32_t segs = (int32_t)((t1 - 1) / p.n_j_tiles - t0 / p.n_j_tiles + 1);
+            if (segs > max_segs) max_segs = segs;
+        }
+    }
+    p.max_segs = max_segs;
+    p.partial_doubles = (int64_t)p.n_ctas * p.max_segs * 3 * p.i_block;
+    *plan = p;
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_plan_cta_range(const genga_kick_plan* plan, int32_t cta, int64_t* t0, int64_t* t1)
+{
+    if (!plan || !t0 || !t1) return GENGA_KICK_E_NULL;
+    if (cta < 0 || cta >= plan->n_ctas) return GENGA_KICK_E_SIZE;
+    *t0 = cta_t0(plan, cta);
+    *t1 = cta_t0(plan, (int64_t)cta + 1);
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_plan_iblock_ctas(const genga_kick_plan* plan, int32_t ib, int32_t* c_first, int32_t* c_last)
+{
+    if (!plan || !c_first || !c_last) return GENGA_KICK_E_NULL;
+    if (ib < 0 || ib >= plan->n_i_blocks || plan->n_j_tiles <= 0) return GENGA_KICK_E_SIZE;
+    // the CTA that owns tile t is the largest c with floor(c T / C) <= t,
+    // i.e. c = floor(((t + 1) C - 1) / T)
+    const int64_t T = plan->n_tiles, C = plan->n_ctas;
+    const int64_t ta = (int64_t)ib * plan->n_j_tiles, tb = ta + plan->n_j_tiles - 1;
+    *c_first = plan_tile_owner(ta, T, C);
+    *c_last = plan_tile_owner(tb, T, C);
+    return GENGA_KICK_OK;
+}
+
+extern "C" const char* genga_kick_strerror(int code)
+{
+    switch (code) {
+    case GENGA_KICK_OK: return "ok";
+    case GENGA_KICK_E_NULL: return "a required pointer is NULL";
+    case GENGA_KICK_E_ALIGN: return "a device pointer is not 16-byte aligned";
+    case GENGA_KICK_E_SIZE: return "a size is out of range";
+    case GENGA_KICK_E_LEVEL: return "changeover_level is outside [0, max_level]";
+    case GENGA_KICK_E_CUDA: return "a CUDA call failed";
+    case GENGA_KICK_E_NOMEM: return "host allocation failed";
+    default: return "unknown genga_kick error code";
+    }
+}

@@ -1,0 +1,48 @@
+// Kernel shapes the library is compiled for, shared by the host planner (genga_kick_plan.cpp)
+// and the launcher (genga_kick.cu).  A variant fixes threads per CTA, i-bodies per thread, the
+// j-tile length and the CTAs per SM the kernel is bounded for (__launch_bounds__).
+//
+// Two families:
+//   dense  (changeover_level == 0): every pair contributes; ~16 FP64-pipe instructions per pair.
+//   sparse (changeover_level >= 1): W_L = 0 exactly for r >= rc0_ij (factor 1 - K_0 of eq. 63,
+//          PAPER.md:627-632), so a far pair costs r^2 + an integer compare; more i-bodies per
+//          thread to amortise the shared-memory loads.
+#pragma once
+#include <stdint.h>
+
+#if defined(__CUDACC__)
+#define GENGA_HD __host__ __device__ __forceinline__
+#else
+#define GENGA_HD static inline
+#endif
+
+// Tile ranges of the decomposition (genga_kick_plan): CTA c of C owns tiles [c T / C, (c+1) T / C).
+GENGA_HD long long plan_tile_begin(long long c, long long T, long long C) { return (c * T) / C; }
+// The CTA that owns tile t: the largest c with floor(c T / C) <= t.
+GENGA_HD int plan_tile_owner(long long t, long long T, long long C) { return (int)(((t + 1) * C - 1) / T); }
+
+struct genga_variant {
+    int32_t threads;
+    int32_t i_per_thread;
+    int32_t j_tile;
+    int32_t ctas_per_sm;
+};
+
+static const int GENGA_N_VARIANTS = 3;
+
+// ordered from the large-N shape to the small-N shape; the planner takes the first one that
+// gives every CTA at least GENGA_MIN_TILES_PER_CTA tiles, else the last
+static const genga_variant GENGA_DENSE_VARIANTS[GENGA_N_VARIANTS] = {
+    {256, 2, 256, 2},
+    {128, 2, 128, 4},
+    {128, 1, 64, 4},
+};
+static const genga_variant GENGA_SPARSE_VARIANTS[GENGA_N_VARIANTS] = {
+    {256, 2, 256, 2},
+    {128, 2, 128, 4},
+    {128, 1, 64, 4},
+};
+static const int GENGA_MIN_TILES_PER_CTA = 4;
+static const int GENGA_M_ALIGN = 256;      // every j_tile divides it
+static const int GENGA_REC_ALIGN = 1024;   // every i_block divides it
+static const int64_t GENGA_MAX_BODIES = (int64_t)1 << 30;

@@ -1,0 +1,175 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Acceptance (BASELINE.json north_star): |a_gpu - a_oracle| <= 1e-13 * sum_j |term_ij| per component;
+the encounter pair list equal as a sorted set except pairs within 1e-12 (relative) of the
+threshold, which are counted; per-body counts equal (same exception)."""
+import numpy as np
+import pytest
+
+import genga_inputs as gi
+from tests.gpu_harness import run_gpu, compare, sorted_pairs
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-13
+
+
+def _full(ki, oracle_mod, level=None, **kw):
+    level = ki.level if level is None else level
+    gpu = run_gpu(ki, level=level, **kw)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=level, G=ki.G,
+                          enc_factor=ki.enc_factor)
+    assert not orc.coincident and gpu.status == 0
+    d = compare(gpu, orc, ki.n_massive, tol=TOL)
+    assert gpu.total == len(gpu.pairs)
+    return gpu, orc, d
+
+
+def test_config0_full(oracle_mod):
+    ki = gi.make_config(0)
+    gpu, orc, d = _full(ki, oracle_mod)
+    assert gpu.total > 50                        # the recipe gives ~2e2 pairs
+    assert int(gpu.counts.sum()) == 2 * gpu.total
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 33, 127, 129, 257, 1000, 2047, 2049, 5000])
+def test_ragged_sizes_level0(oracle_mod, n):
+    ki = gi.make_config(0, n=n)
+    _full(ki, oracle_mod)
+
+
+@pytest.mark.parametrize("level", [0, 1, 2])
+def test_config2_giants_levels(oracle_mod, level):
+    ki = gi.make_config(2, n=6000, level=2)
+    gpu, orc, d = _full(ki, oracle_mod, level=level)
+    assert gpu.total > 0
+
+
+@pytest.mark.parametrize("level", [0, 1])
+def test_config3_reduced(oracle_mod, level):
+    ki = gi.make_config(3, n=9001, level=1)
+    gpu, orc, d = _full(ki, oracle_mod, level=level)
+    assert gpu.total > 0
+
+
+def test_config1_single_kick(oracle_mod):
+    ki = gi.make_config(1)
+    _full(ki, oracle_mod)
+
+
+@pytest.mark.parametrize("nm,nt", [(300, 5000), (2048, 20000), (1, 100), (257, 1)])
+def test_config4_test_particles_reduced(oracle_mod, nm, nt):
+    ki = gi.make_config(4, n=nm, n_test=nt)
+    gpu, orc, d = _full(ki, oracle_mod)
+    # test particles exert no force and do not meet each other
+    assert all(p[0] < ki.n_massive for p in gpu.pairs.tolist())
+
+
+def test_no_massive_bodies(oracle_mod):
+    ki = gi.make_config(4, n=0, n_test=500)
+    gpu = run_gpu(ki)
+    assert gpu.total == 0 and not gpu.counts.any() and not gpu.acc.any()
+
+
+@pytest.mark.parametrize("n", [16, 64, 1024, 4096])
+def test_ring_eight_partners(oracle_mod, n):
+    ki = gi.make_ring(n)
+    gpu = run_gpu(ki)
+    assert (gpu.counts == 8).all() and gpu.total == 4 * n
+
+
+def test_close_pairs_and_band(oracle_mod):
+    """Pairs all through the changeover band, incl. r < 0.1 rc (K = 0) and bodies 1e-9 AU apart."""
+    ki = gi.make_config(0, n=1024)
+    pos = ki.pos.copy()
+    rng = np.random.RandomState(5)
+    for q, frac in enumerate(np.concatenate([np.linspace(0.02, 1.2, 200), [1e-7, 1e-5, 0.0999, 0.1, 0.1001, 0.9999, 1.0, 1.0001]])):
+        i, j = 2 * q, 2 * q + 1
+        rc = max(ki.rcrit[0, i], ki.rcrit[0, j])
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        pos[:, j] = pos[:, i] + frac * rc * u
+    ki.pos = np.ascontiguousarray(pos)
+    _full(ki, oracle_mod)
+
+
+def test_levels_with_substeps_10(oracle_mod):
+    ki = gi.make_disk(3000, 77, level=3, substeps=10, total_mass=5 * gi.M_EARTH)
+    for level in range(4):
+        _full(ki, oracle_mod, level=level)
+
+
+def test_enc_factor(oracle_mod):
+    ki = gi.make_config(0, n=3000)
+    ki.enc_factor = 1.7
+    gpu, orc, d = _full(ki, oracle_mod)
+    ki.enc_factor = 0.5
+    _full(ki, oracle_mod)
+
+
+def test_bit_reproducible_and_vel_update(oracle_mod):
+    ki = gi.make_config(3, n=5000, level=1)
+    a = run_gpu(ki, level=0, with_vel=True)
+    b = run_gpu(ki, level=0, with_vel=True)
+    assert np.array_equal(a.acc, b.acc) and np.array_equal(a.counts, b.counts) and a.total == b.total
+    assert np.array_equal(sorted_pairs(a.pairs), sorted_pairs(b.pairs))
+    want = ki.vel + ki.dt * a.acc
+    assert np.allclose(a.vel, want, rtol=0, atol=4e-16 * np.abs(want).max())
+    assert np.max(np.abs(a.vel - want) / (np.abs(ki.vel) + np.abs(ki.dt * a.acc))) < 3e-16
+
+
+def test_pair_capacity_overflow(oracle_mod):
+    ki = gi.make_config(0)
+    full = run_gpu(ki)
+    small = run_gpu(ki, capacity=16)
+    assert small.total == full.total and len(small.pairs) == 16
+    allp = {tuple(p) for p in full.pairs.tolist()}
+    assert all(tuple(p) in allp for p in small.pairs.tolist())
+    zero = run_gpu(ki, capacity=0)
+    assert zero.total == full.total and np.array_equal(zero.counts, full.counts)
+
+
+def test_host_entry_point(oracle_mod):
+    ki = gi.make_config(0, n=1500)
+    h = run_gpu(ki, host=True, with_vel=True)
+    d = run_gpu(ki, with_vel=True)
+    assert np.array_equal(h.acc, d.acc) and np.array_equal(h.vel, d.vel)
+    assert np.array_equal(sorted_pairs(h.pairs), sorted_pairs(d.pairs)) and np.array_equal(h.counts, d.counts)
+
+
+def test_momentum(oracle_mod):
+    ki = gi.make_config(1, n=4096)
+    gpu = run_gpu(ki)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, level=0, G=ki.G)
+    p = (ki.mass * gpu.acc).sum(axis=1)
+    scale = (ki.mass * orc.S).sum(axis=1)
+    assert np.all(np.abs(p) <= 1e-13 * scale)
+
+
+def test_coincident_bodies_flagged():
+    ki = gi.make_config(0, n=100)
+    ki.pos[:, 7] = ki.pos[:, 3]
+    gpu = run_gpu(ki)
+    assert gpu.status & 1 and np.isfinite(gpu.acc).all()
+
+
+def test_error_codes():
+    import torch
+    import paper_2201_10058_b200 as g
+    with pytest.raises(g.GengaKickError) as e:
+        g.GengaKick(0, 0)
+    assert e.value.code == g.E_SIZE
+    k = g.GengaKick(64, 0, max_level=0, pair_capacity=8)
+    x = torch.zeros(3 * 64 + 1, dtype=torch.float64, device="cuda")
+    m = torch.ones(64, dtype=torch.float64, device="cuda")
+    acc = torch.zeros(3, 64, dtype=torch.float64, device="cuda")
+    pr = torch.zeros(8, 2, dtype=torch.int32, device="cuda")
+    npr = torch.zeros(65, dtype=torch.int32, device="cuda")
+    with pytest.raises(g.GengaKickError) as e:
+        k.kick(x[1:], None, m, m, 0, 1.0, acc, pr, npr)
+    assert e.value.code == g.E_ALIGN
+    with pytest.raises(g.GengaKickError) as e:
+        k.kick(x, None, m, m, 1, 1.0, acc, pr, npr)
+    assert e.value.code == g.E_LEVEL
+    with pytest.raises(g.GengaKickError) as e:
+        k.kick(x, None, m, m, 0, 1.0, None, pr, npr)
+    assert e.value.code == g.E_NULL
+    k.free()
