@@ -53,7 +53,14 @@ typedef struct {
     int64_t pair_capacity;  /* rows available in out_pairs                                         */
     double  G;              /* gravitational constant; k^2, k = 0.01720209895 in AU / day / Msun   */
     double  enc_factor;     /* f in r_ij < f * rcL_ij; 1.0                                         */
+    int32_t order_mode;     /* GENGA_KICK_ORDER_*: the library's INTERNAL body order (never visible
+                               in the outputs; changes speed and summation order, not the contract) */
+    int32_t reserved;       /* 0                                                                   */
 } genga_kick_config;
+
+#define GENGA_KICK_ORDER_AUTO    0   /* spatially sorted copy when N >= 4096, caller's order below  */
+#define GENGA_KICK_ORDER_CALLER  1   /* always the caller's order                                   */
+#define GENGA_KICK_ORDER_SORTED  2   /* always the spatially sorted copy                            */
 
 /*
  * How one call is cut into CTAs (host logic, no CUDA call; exported so it can be tested on a

@@ -11,6 +11,7 @@ LIB_PATH = os.path.join(HERE, "libgenga_kick.so")
 
 OK, E_NULL, E_ALIGN, E_SIZE, E_LEVEL, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4, -5, -6
 STATUS_COINCIDENT = 1
+ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 
 EXPORTS = (
     "genga_kick_make_plan", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
@@ -21,7 +22,8 @@ EXPORTS = (
 
 class GengaKickConfig(C.Structure):
     _fields_ = [("n_massive", C.c_int32), ("n_test", C.c_int32), ("max_level", C.c_int32), ("device", C.c_int32),
-                ("pair_capacity", C.c_int64), ("G", C.c_double), ("enc_factor", C.c_double)]
+                ("pair_capacity", C.c_int64), ("G", C.c_double), ("enc_factor", C.c_double),
+                ("order_mode", C.c_int32), ("reserved", C.c_int32)]
 
 
 class GengaKickPlan(C.Structure):
@@ -110,9 +112,10 @@ class GengaKick:
     """A genga_kick context.  Arrays are torch tensors (device tensors for kick(), CPU tensors for
     kick_host()), float64 / int32, C-contiguous, laid out as include/genga_kick.h states."""
 
-    def __init__(self, n_massive, n_test=0, max_level=0, pair_capacity=1 << 20, G=1.0, enc_factor=1.0, device=0):
+    def __init__(self, n_massive, n_test=0, max_level=0, pair_capacity=1 << 20, G=1.0, enc_factor=1.0, device=0,
+                 order_mode=0):
         self.cfg = GengaKickConfig(int(n_massive), int(n_test), int(max_level), int(device), int(pair_capacity),
-                                   float(G), float(enc_factor))
+                                   float(G), float(enc_factor), int(order_mode), 0)
         self.n = int(n_massive) + int(n_test)
         self._ctx = C.c_void_p()
         rc = lib().genga_kick_init(C.byref(self.cfg), C.byref(self._ctx))

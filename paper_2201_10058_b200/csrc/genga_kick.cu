@@ -4,6 +4,7 @@
 #include "../../include/genga_kick.h"
 #include "genga_kick_variants.h"
 #include "genga_kick_kernels.cuh"
+#include "genga_kick_sort.cuh"
 
 #include <algorithm>
 #include <cstdlib>
@@ -23,6 +24,17 @@ struct genga_kick_ctx {
     int* rfw;
     int* ridx;
     int* cfw;
+    float4* cblo;
+    float4* cbhi;
+    // internal order (genga_kick_sort.cuh); sorted == false: caller's order
+    bool sorted;
+    int sort_blocks;
+    unsigned* bbox;
+    unsigned* keys_a;
+    unsigned* keys_b;
+    int* vals_a;                   // ends up holding the permutation
+    int* vals_b;
+    int* counts;
     double* partial;
     int* status;
     int64_t n_rec_alloc;
@@ -73,6 +85,7 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
     if (cfg->n_massive < 0 || cfg->n_test < 0 || N <= 0 || N > GENGA_MAX_BODIES || cfg->pair_capacity < 0)
         return GENGA_KICK_E_SIZE;
     if (cfg->max_level < 0 || cfg->max_level > 62) return GENGA_KICK_E_LEVEL;
+    if (cfg->order_mode < GENGA_KICK_ORDER_AUTO || cfg->order_mode > GENGA_KICK_ORDER_SORTED) return GENGA_KICK_E_SIZE;
 
     genga_kick_ctx* ctx = new (std::nothrow) genga_kick_ctx();
     if (!ctx) return GENGA_KICK_E_NOMEM;
@@ -108,6 +121,20 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
         if ((e = cudaMalloc(&ctx->rfw, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->ridx, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->cfw, (size_t)(nr / GENGA_CHUNK) * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->cblo, (size_t)(nr / GENGA_GROUP) * sizeof(float4))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->cbhi, (size_t)(nr / GENGA_GROUP) * sizeof(float4))) != cudaSuccess) goto cuda_error;
+        ctx->sorted = cfg->order_mode == GENGA_KICK_ORDER_SORTED ||
+                      (cfg->order_mode == GENGA_KICK_ORDER_AUTO && N >= GENGA_SORT_MIN_BODIES);
+        if (ctx->sorted) {
+            ctx->sort_blocks = (int)((N + GENGA_SORT_BLOCK - 1) / GENGA_SORT_BLOCK);
+            const size_t nc = (size_t)GENGA_SORT_MAXDIGITS * ctx->sort_blocks;
+            if ((e = cudaMalloc(&ctx->bbox, 4 * sizeof(unsigned))) != cudaSuccess) goto cuda_error;
+            if ((e = cudaMalloc(&ctx->keys_a, (size_t)N * sizeof(unsigned))) != cudaSuccess) goto cuda_error;
+            if ((e = cudaMalloc(&ctx->keys_b, (size_t)N * sizeof(unsigned))) != cudaSuccess) goto cuda_error;
+            if ((e = cudaMalloc(&ctx->vals_a, (size_t)N * sizeof(int))) != cudaSuccess) goto cuda_error;
+            if ((e = cudaMalloc(&ctx->vals_b, (size_t)N * sizeof(int))) != cudaSuccess) goto cuda_error;
+            if ((e = cudaMalloc(&ctx->counts, nc * sizeof(int))) != cudaSuccess) goto cuda_error;
+        }
         if ((e = cudaMalloc(&ctx->partial, (size_t)max_partial * sizeof(double))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->status, sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMemset(ctx->status, 0, sizeof(int))) != cudaSuccess) goto cuda_error;
@@ -146,17 +173,36 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
     const int n_rec = (int)pl.n_rec;
     cudaStream_t st = ctx->stream;
 
+    if (ctx->sorted) {
+        // stable LSD radix sort of the 17-bit keys: digits of 8 and 9 bits
+        const int nb = ctx->sort_blocks;
+        genga::sort_init_kernel<<<1, 32, 0, st>>>(ctx->bbox);
+        genga::bbox_kernel<<<std::min((N + 255) / 256, 8 * ctx->num_sms), 256, 0, st>>>(pos, N, ctx->bbox);
+        genga::key_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(pos, N, ctx->cfg.n_massive, ctx->bbox, ctx->keys_a,
+                                                                  ctx->vals_a, 8, nb, ctx->counts);
+        genga::scan_kernel<<<1, 1024, 0, st>>>(ctx->counts, 256 * nb);
+        genga::radix_scatter_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_a, ctx->vals_a, N, 0, 8, nb, ctx->counts,
+                                                                       ctx->keys_b, ctx->vals_b);
+        genga::radix_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_b, N, 8, 9, nb, ctx->counts);
+        genga::scan_kernel<<<1, 1024, 0, st>>>(ctx->counts, 512 * nb);
+        genga::radix_scatter_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_b, ctx->vals_b, N, 8, 9, nb, ctx->counts,
+                                                                       nullptr, ctx->vals_a);
+        GK_CUDA(ctx, cudaGetLastError());
+        ctx->launches += 8;
+    }
     {
         const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
-        genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, nullptr, N, ctx->cfg.n_massive, pl.m_pad, n_rec,
-                                                   changeover_level, ctx->cfg.G, ctx->cfg.enc_factor, ctx->rxy, ctx->rzm,
-                                                   ctx->rfw, ctx->ridx, ctx->cfw, out_npairs);
+        genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
+                                                   ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
+                                                   ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw,
+                                                   ctx->cblo, ctx->cbhi, out_npairs);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
     }
     if (pl.n_ctas > 0) {
         genga::KickParams kp;
         kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx; kp.cfw = ctx->cfw;
+        kp.cblo = ctx->cblo; kp.cbhi = ctx->cbhi;
         kp.rcrit = rcrit;
         kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
         kp.n_j_tiles = pl.n_j_tiles; kp.n_ctas = pl.n_ctas; kp.max_segs = pl.max_segs; kp.n_tiles = pl.n_tiles;
@@ -249,7 +295,8 @@ extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return c
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)
 {
     if (!ctx) return GENGA_KICK_OK;
-    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->partial, ctx->status, ctx->h_pos,
+    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
+                    ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->status, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs};
     for (void* b : bufs)
         if (b) cudaFree(b);

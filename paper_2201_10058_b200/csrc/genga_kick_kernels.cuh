@@ -18,8 +18,9 @@ namespace genga {
 #define GENGA_STATUS_COINCIDENT 1
 // Padding records sit far from every real body; records used as i-bodies and as j-bodies share
 // one array, so a padding i meets a padding j at distance 0 -- its lanes are never stored.
-#define GENGA_SENTINEL_POS 1.0e30
+#define GENGA_SENTINEL_POS 1.0e15   // its square fits a float (group boxes are kept in FP32)
 #define GENGA_CHUNK 8              // j-records per filter chunk (one warp vote per chunk)
+#define GENGA_GROUP 32             // j-records per culling group (one box per group)
 #define GENGA_PAD 1024             // record arrays are padded to multiples of this
 
 struct KickParams {
@@ -30,6 +31,8 @@ struct KickParams {
     const int* __restrict__ rfw;       // filter word (see filter_word)
     const int* __restrict__ ridx;      // caller's body index, -1 for padding
     const int* __restrict__ cfw;       // max filter word of each chunk of GENGA_CHUNK records
+    const float4* __restrict__ cblo;   // box of each group of GENGA_GROUP records: (lo x, lo y, lo z, max filter word)
+    const float4* __restrict__ cbhi;   //                                            (hi x, hi y, hi z, -)
     // the caller's arrays (read by the exact per-pair path only)
     const double* __restrict__ rcrit;  // [L+1][N]
     int N, n_massive, L;
@@ -61,30 +64,32 @@ __device__ __forceinline__ int filter_word(double rc0, double rcL, double f)
     return __double2hiint(__dmul_rn(m, m)) + 1;
 }
 
-// perm == nullptr: internal order = caller's order.
+// perm == nullptr: internal order = caller's order; else perm[s] = caller's index of the body at
+// sorted position s (massive bodies first).  One warp writes one group of GENGA_GROUP records and
+// its bounding box (FP32, rounded outwards).
 __global__ void __launch_bounds__(256)
 pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, const double* __restrict__ rcrit,
             const int* __restrict__ perm, int N, int n_massive, int m_pad, int n_rec, int L, double G, double f,
             double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
-            int* __restrict__ cfw, int* __restrict__ out_npairs)
+            int* __restrict__ cfw, float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs)
 {
     const int stride = gridDim.x * blockDim.x;       // a multiple of 32
     const int top = max(n_rec, ((N + 1 + 31) / 32) * 32);
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < top; r += stride) {
         int fw = -1;
+        double x = GENGA_SENTINEL_POS, y = GENGA_SENTINEL_POS, z = GENGA_SENTINEL_POS, gm = 0.0;
         if (r < n_rec) {
             int b = -1;                               // caller's index of record r
             if (r < m_pad) { if (r < n_massive) b = r; }
             else if (r - m_pad < N - n_massive) b = n_massive + (r - m_pad);
             if (b >= 0 && perm) b = perm[b];
             if (b >= 0) {
-                rxy[r] = make_double2(pos[b], pos[(size_t)N + b]);
-                rzm[r] = make_double2(pos[2 * (size_t)N + b], __dmul_rn(G, mass[b]));
+                x = pos[b]; y = pos[(size_t)N + b]; z = pos[2 * (size_t)N + b];
+                gm = __dmul_rn(G, mass[b]);
                 fw = filter_word(rcrit[b], rcrit[(size_t)L * N + b], f);
-            } else {
-                rxy[r] = make_double2(GENGA_SENTINEL_POS, GENGA_SENTINEL_POS);
-                rzm[r] = make_double2(GENGA_SENTINEL_POS, 0.0);
             }
+            rxy[r] = make_double2(x, y);
+            rzm[r] = make_double2(z, gm);
             rfw[r] = fw;
             ridx[r] = b;
         }
@@ -94,6 +99,21 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
         m = max(m, __shfl_xor_sync(0xffffffffu, m, 2));
         m = max(m, __shfl_xor_sync(0xffffffffu, m, 4));
         if (r < n_rec && (r % GENGA_CHUNK) == 0) cfw[r / GENGA_CHUNK] = m;
+        // group box
+        float lx = __double2float_rd(x), ly = __double2float_rd(y), lz = __double2float_rd(z);
+        float hx = __double2float_ru(x), hy = __double2float_ru(y), hz = __double2float_ru(z);
+#pragma unroll
+        for (int o = 8; o < 32; o <<= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            lx = fminf(lx, __shfl_xor_sync(0xffffffffu, lx, o)); hx = fmaxf(hx, __shfl_xor_sync(0xffffffffu, hx, o));
+            ly = fminf(ly, __shfl_xor_sync(0xffffffffu, ly, o)); hy = fmaxf(hy, __shfl_xor_sync(0xffffffffu, hy, o));
+            lz = fminf(lz, __shfl_xor_sync(0xffffffffu, lz, o)); hz = fmaxf(hz, __shfl_xor_sync(0xffffffffu, hz, o));
+        }
+        if (r < n_rec && (r % GENGA_GROUP) == 0) {
+            cblo[r / GENGA_GROUP] = make_float4(lx, ly, lz, __int_as_float(m));
+            cbhi[r / GENGA_GROUP] = make_float4(hx, hy, hz, 0.0f);
+        }
         if (r <= N) out_npairs[r] = 0;
     }
 }
@@ -216,6 +236,26 @@ __device__ __forceinline__ double rsqrt_seed_unless(double x, bool skip)
 //   distinct register operands (a third costs a register-file cycle on this part).
 //   SPARSE (level >= 1): a pair that passes the filter has W_L = 0 exactly; nothing is added.
 // ---------------------------------------------------------------------------------------------
+// The same arithmetic without the filter, for groups the box test has cleared.
+__device__ __forceinline__ void pair_bare(double xj, double yj, double zj, double gmj,
+                                          double xi, double yi, double zi, double& ax, double& ay, double& az)
+{
+    const double dx = __dsub_rn(xj, xi), dy = __dsub_rn(yj, yi), dz = __dsub_rn(zj, zi);
+    const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
+    const double t = __dmul_rn(y0, y0);
+    const double e = fma(-r2, t, 1.0);
+    const double g = __dmul_rn(gmj, y0);
+    const double u = __dmul_rn(t, g);
+    const double c = fma(1.875, e, 1.5);
+    const double q = fma(e, c, 1.0);
+    const double s = __dmul_rn(u, q);
+    ax = fma(s, dx, ax);
+    ay = fma(s, dy, ay);
+    az = fma(s, dz, az);
+}
+
 template <bool DENSE>
 __device__ __forceinline__ void pair_fast(double xj, double yj, double zj, double gmj,
                                           double xi, double yi, double zi, int thr,
@@ -242,28 +282,57 @@ __device__ __forceinline__ void pair_fast(double xj, double yj, double zj, doubl
 
 // ---------------------------------------------------------------------------------------------
 // kick_kernel.  CTA c owns the tiles [c T / C, (c+1) T / C) of the i-major (i-block x j-tile)
-// grid (genga_kick_plan); thread `tid` owns the IPT i-records ib * IB + k * THREADS + tid.
+// grid (genga_kick_plan); warp w owns the 32 * IPT consecutive i-records
+// ib * IB + w * 32 * IPT + [0, 32 * IPT), lane l the records k * 32 + l of them.
 // j-tiles are staged by TMA bulk copies into a two-stage shared-memory ring; every lane reads
-// the same j-record (LDS broadcast).  Per chunk of GENGA_CHUNK j-records one warp vote decides
-// whether any pair of the chunk needs the exact path.
+// the same j-record (LDS broadcast).
+//
+// Culling: per tile, lane g tests the box of the warp's i-records against the box of j-group g
+// (GENGA_GROUP records).  If the boxes are further apart than the largest filter radius of either
+// side, no pair of the (warp, group) combination can trip the filter, and the group runs
+//   DENSE : the bare pair loop (no compare, no vote) -- same arithmetic, same order, same bits as
+//           the checked loop would give;
+//   SPARSE: not at all (every W_L is exactly 0, nothing is an encounter).
+// Otherwise the group runs the checked loop: per chunk of GENGA_CHUNK j-records one warp vote
+// decides whether any pair of the chunk needs the exact path.
 // ---------------------------------------------------------------------------------------------
 template <int JT>
 struct alignas(128) TileStage {
     double2 xy[JT];
     double2 zm[JT];
+    float4 blo[JT / GENGA_GROUP];
+    float4 bhi[JT / GENGA_GROUP];
     int cf[JT / GENGA_CHUNK];
 };
+
+// lower bound of the squared distance between two boxes against the upper bound of the squared
+// filter radius: true if some pair might trip the filter
+__device__ __forceinline__ bool boxes_near(float4 alo, float4 ahi, int afw, float4 blo, float4 bhi)
+{
+    const float gx = fmaxf(fmaxf(__fsub_rd(alo.x, bhi.x), __fsub_rd(blo.x, ahi.x)), 0.0f);
+    const float gy = fmaxf(fmaxf(__fsub_rd(alo.y, bhi.y), __fsub_rd(blo.y, ahi.y)), 0.0f);
+    const float gz = fmaxf(fmaxf(__fsub_rd(alo.z, bhi.z), __fsub_rd(blo.z, ahi.z)), 0.0f);
+    const float d2 = __fmaf_rd(gx, gx, __fmaf_rd(gy, gy, __fmul_rd(gz, gz)));
+    const int fw = max(max(afw, __float_as_int(blo.w)), 0);
+    // the filter trips iff hi(r2) < fw, so r2 >= double(fw, 0) is safe; 1.0001 covers the FP32
+    // roundings here and the ulp between the true and the computed r2
+    const float R2 = __fmul_ru(__double2float_ru(__hiloint2double(fw, 0)), 1.0001f);
+    return !(d2 >= R2);
+}
 
 template <int THREADS, int IPT, int JT, int CTAS, bool DENSE>
 __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
     constexpr int IB = THREADS * IPT;
     constexpr int NCH = JT / GENGA_CHUNK;
-    constexpr uint32_t TILE_BYTES = JT * 32 + NCH * 4;
+    constexpr int NG = JT / GENGA_GROUP;
+    constexpr uint32_t TILE_BYTES = JT * 32 + NG * 32 + NCH * 4;
+    static_assert(NG <= 32 && JT % GENGA_GROUP == 0, "one lane per group");
     __shared__ TileStage<JT> st[2];
     __shared__ __align__(8) uint64_t full[2];
 
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int woff = (tid >> 5) * (32 * IPT) + lane;        // offset of the thread's first record in the i-block
     const long long t0 = plan_tile_begin(blockIdx.x, p.n_tiles, p.n_ctas);
     const long long t1 = plan_tile_begin(blockIdx.x + 1, p.n_tiles, p.n_ctas);
     if (t0 >= t1) return;
@@ -280,6 +349,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         mbar_expect_tx(&full[s], TILE_BYTES);
         bulk_g2s(st[s].xy, p.rxy + (size_t)jt * JT, JT * 16, &full[s]);
         bulk_g2s(st[s].zm, p.rzm + (size_t)jt * JT, JT * 16, &full[s]);
+        bulk_g2s(st[s].blo, p.cblo + (size_t)jt * NG, NG * 16, &full[s]);
+        bulk_g2s(st[s].bhi, p.cbhi + (size_t)jt * NG, NG * 16, &full[s]);
         bulk_g2s(st[s].cf, p.cfw + (size_t)jt * NCH, NCH * 4, &full[s]);
     };
     if (tid == 0) {
@@ -289,6 +360,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 
     double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT];
     int fi[IPT], bi[IPT], cnt[IPT];
+    float4 wlo, whi;                                        // box of the warp's i-records
+    int wfw = -1;
     const int first_ib = (int)(t0 / p.n_j_tiles);
     int cur_ib = -1;
 
@@ -296,7 +369,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         const size_t base = ((size_t)blockIdx.x * p.max_segs + (cur_ib - first_ib)) * 3 * IB;
 #pragma unroll
         for (int k = 0; k < IPT; k++) {
-            const int off = k * THREADS + tid;
+            const int off = woff + k * 32;
             p.partial[base + off] = ax[k];
             p.partial[base + IB + off] = ay[k];
             p.partial[base + 2 * IB + off] = az[k];
@@ -312,65 +385,92 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         if (ib != cur_ib) {
             if (cur_ib >= 0) flush();
             cur_ib = ib;
+            wlo = make_float4(3.0e38f, 3.0e38f, 3.0e38f, 0.0f);
+            whi = make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
+            wfw = -1;
 #pragma unroll
             for (int k = 0; k < IPT; k++) {
-                const size_t r = (size_t)ib * IB + k * THREADS + tid;
+                const size_t r = (size_t)ib * IB + woff + k * 32;
                 const double2 a = p.rxy[r], b = p.rzm[r];
                 xi[k] = a.x; yi[k] = a.y; zi[k] = b.x;
                 fi[k] = p.rfw[r];
                 bi[k] = p.ridx[r];
                 ax[k] = ay[k] = az[k] = 0.0;
                 cnt[k] = 0;
+                // the groups of GENGA_GROUP records are aligned with the warp's k-slices
+                const float4 glo = p.cblo[r / GENGA_GROUP], ghi = p.cbhi[r / GENGA_GROUP];
+                wlo.x = fminf(wlo.x, glo.x); wlo.y = fminf(wlo.y, glo.y); wlo.z = fminf(wlo.z, glo.z);
+                whi.x = fmaxf(whi.x, ghi.x); whi.y = fmaxf(whi.y, ghi.y); whi.z = fmaxf(whi.z, ghi.z);
+                wfw = max(wfw, __float_as_int(glo.w));
             }
         }
         mbar_wait(&full[s], (uint32_t)((it >> 1) & 1));
         const TileStage<JT>& S = st[s];
 
+        const bool mine_near = lane < NG ? boxes_near(wlo, whi, wfw, S.blo[lane], S.bhi[lane]) : false;
+        const unsigned nearmask = __ballot_sync(0xffffffffu, mine_near);
+
 #pragma unroll 1
-        for (int jj = 0; jj < JT; jj += GENGA_CHUNK) {
-            const int cm = S.cf[jj / GENGA_CHUNK];
-            int thr[IPT];
+        for (int g = 0; g < NG; g++) {
+            const int j0 = g * GENGA_GROUP;
+            if (!((nearmask >> g) & 1u)) {
+                if (DENSE) {
+#pragma unroll 4
+                    for (int u = 0; u < GENGA_GROUP; u++) {
+                        const double2 xy = S.xy[j0 + u], zm = S.zm[j0 + u];
 #pragma unroll
-            for (int k = 0; k < IPT; k++) thr[k] = max(fi[k], cm);
-            bool any = false;
-#pragma unroll
-            for (int u = 0; u < GENGA_CHUNK; u++) {
-                const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
-#pragma unroll
-                for (int k = 0; k < IPT; k++)
-                    pair_fast<DENSE>(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], any);
+                        for (int k = 0; k < IPT; k++)
+                            pair_bare(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], ax[k], ay[k], az[k]);
+                    }
+                }
+                continue;
             }
-            if (__any_sync(0xffffffffu, any)) {
-                // exact path: the pairs of this chunk that the filter caught (a3, a5, a6)
 #pragma unroll 1
+            for (int jj = j0; jj < j0 + GENGA_GROUP; jj += GENGA_CHUNK) {
+                const int cm = S.cf[jj / GENGA_CHUNK];
+                int thr[IPT];
+#pragma unroll
+                for (int k = 0; k < IPT; k++) thr[k] = max(fi[k], cm);
+                bool any = false;
+#pragma unroll
                 for (int u = 0; u < GENGA_CHUNK; u++) {
-                    const int jrec = jt * JT + jj + u;
                     const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
 #pragma unroll
-                    for (int k = 0; k < IPT; k++) {
-                        const double dx = __dsub_rn(xy.x, xi[k]), dy = __dsub_rn(xy.y, yi[k]), dz = __dsub_rn(zm.x, zi[k]);
-                        const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
-                        bool hit = false;
-                        int lo = 0, hi = 0;
-                        if (__double2hiint(r2) < thr[k] && ib * IB + k * THREADS + tid != jrec) {
-                            const int bj = p.ridx[jrec];
-                            if (bj >= 0 && bi[k] >= 0) {
-                                const ExactResult e = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi[k], bj, dx, dy, dz, zm.y);
-                                ax[k] = fma(e.s, dx, ax[k]);
-                                ay[k] = fma(e.s, dy, ay[k]);
-                                az[k] = fma(e.s, dz, az[k]);
-                                if (e.enc) {
-                                    cnt[k]++;
-                                    if (bi[k] >= p.n_massive) {          // test particle i, massive j
-                                        atomicAdd(p.out_npairs + bj, 1);
-                                        hit = true; lo = bj; hi = bi[k];
-                                    } else if (bi[k] < bj) {
-                                        hit = true; lo = bi[k]; hi = bj;
+                    for (int k = 0; k < IPT; k++)
+                        pair_fast<DENSE>(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], any);
+                }
+                if (__any_sync(0xffffffffu, any)) {
+                    // exact path: the pairs of this chunk that the filter caught (a3, a5, a6)
+#pragma unroll 1
+                    for (int u = 0; u < GENGA_CHUNK; u++) {
+                        const int jrec = jt * JT + jj + u;
+                        const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
+#pragma unroll
+                        for (int k = 0; k < IPT; k++) {
+                            const double dx = __dsub_rn(xy.x, xi[k]), dy = __dsub_rn(xy.y, yi[k]), dz = __dsub_rn(zm.x, zi[k]);
+                            const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
+                            bool hit = false;
+                            int lo = 0, hi = 0;
+                            if (__double2hiint(r2) < thr[k] && ib * IB + woff + k * 32 != jrec) {
+                                const int bj = p.ridx[jrec];
+                                if (bj >= 0 && bi[k] >= 0) {
+                                    const ExactResult e = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi[k], bj, dx, dy, dz, zm.y);
+                                    ax[k] = fma(e.s, dx, ax[k]);
+                                    ay[k] = fma(e.s, dy, ay[k]);
+                                    az[k] = fma(e.s, dz, az[k]);
+                                    if (e.enc) {
+                                        cnt[k]++;
+                                        if (bi[k] >= p.n_massive) {          // test particle i, massive j
+                                            atomicAdd(p.out_npairs + bj, 1);
+                                            hit = true; lo = bj; hi = bi[k];
+                                        } else if (bi[k] < bj) {
+                                            hit = true; lo = bi[k]; hi = bj;
+                                        }
                                     }
                                 }
                             }
+                            emit_pairs(p, hit, lo, hi);
                         }
-                        emit_pairs(p, hit, lo, hi);
                     }
                 }
             }

@@ -13,6 +13,17 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-13
 
 
+@pytest.fixture(params=[1, 2], ids=["caller_order", "sorted_order"], autouse=True)
+def order_mode(request, monkeypatch):
+    """Every test runs with both internal body orders (GENGA_KICK_ORDER_CALLER / _SORTED)."""
+    import tests.gpu_harness as h
+    orig = h.run_gpu
+    monkeypatch.setattr(h, "run_gpu", lambda *a, **k: orig(*a, **{"order_mode": request.param, **k}))
+    globals()["run_gpu"] = h.run_gpu
+    yield request.param
+    globals()["run_gpu"] = orig
+
+
 def _full(ki, oracle_mod, level=None, **kw):
     level = ki.level if level is None else level
     gpu = run_gpu(ki, level=level, **kw)
@@ -173,3 +184,17 @@ def test_error_codes():
         k.kick(x, None, m, m, 0, 1.0, None, pr, npr)
     assert e.value.code == g.E_NULL
     k.free()
+
+
+def test_internal_order_is_invisible(oracle_mod):
+    """Caller's order, sorted order and auto give the same pair set and counts; accelerations agree
+    to the rounding of a different summation order."""
+    ki = gi.make_config(3, n=7000, level=1)
+    for level in (0, 1):
+        a = run_gpu(ki, level=level, order_mode=1)
+        b = run_gpu(ki, level=level, order_mode=2)
+        c = run_gpu(ki, level=level, order_mode=0)
+        assert np.array_equal(sorted_pairs(a.pairs), sorted_pairs(b.pairs)) and np.array_equal(a.counts, b.counts)
+        assert np.array_equal(b.acc, c.acc)                      # auto sorts at this size
+        orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, level=level, G=ki.G)
+        assert np.all(np.abs(a.acc - b.acc) <= 2e-13 * orc.S)
