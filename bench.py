@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- FP64 pair interactions/s of the GENGA kick + close-encounter pre-check on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference]
+
+Workload (BASELINE.json configs[3], the one `metric` is quoted on): N = 65,536 fully interactive
+planetesimals, a in [0.5, 4] AU with surface density ~ a^-1.5, masses log-uniform in
+[1e-4, 1e-2] Earth masses, r_crit rows at dt = 6 d and dt/2, seeded synthetic (genga_inputs).
+
+One STEP = one pass of the whole hot path over that disk with the paper's two-level changeover
+weights of eq. 63: the all-pairs kick with W_0 = K(r, dt) and the all-pairs kick
+with W_1 = (1 - K(r, dt)) K(r, dt/2), each fused with its encounter pre-check, pair list, per-body
+counts and the velocity update v += dt a (rows a1-a8 of SURVEY.md 8(a)).
+A step is 2 N (N - 1) ordered pair interactions.  The per-level numbers are reported beside the
+aggregate (`levels`): the level-0 kick is the dense one (every pair contributes) and is the kernel
+the `roofline` object describes.
+
+N > 1 GPUs (torchrun, one rank per GPU): the path runs on one GPU (north_star); ranks are
+independent replicas on independently seeded disks, no data-path collective ("scaling": "weak").
+
+--impl reference times the CPU oracle (oracle/, plain C, as it stands) on the host cores on a
+bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import genga_inputs as gi  # noqa: E402
+
+METRIC = "FP64 pair interactions/s (kick+encounter) at N=65,536"
+UNIT = "pair interactions/s"
+N_BODIES = 65536
+LEVELS = (0, 1)
+PAIR_CAPACITY = 1 << 20
+# FP64-pipe instructions and flops of one far pair in the dense (level-0) pair loop, read off the
+# committed SASS (profiles/sass_pair_loop_r01.md): 3 DADD + 5 DMUL + 8 DFMA; kept in ONE place.
+FP64_INSTR_PER_PAIR = 16
+FLOPS_PER_PAIR = 24
+FP64_LANES_PER_SM = 64           # 148 SMs x 64 lanes x 2 flops x clocks.max.sm
+# dram__bytes_read.sum + dram__bytes_write.sum of one level-0 kick_kernel launch, from the ncu
+# --set full capture summarised in profiles/ (None until that capture exists)
+NCU_DRAM_BYTES_PER_LAUNCH = None
+
+
+def workload(rank: int):
+    """configs[3]; rank r > 0 draws an independent disk of the same recipe."""
+    if rank == 0:
+        return gi.make_config(3)
+    ki = gi.make_disk(N_BODIES, 1003 + 7919 * rank, a_law="sigma_a^-1.5",
+                      mass_law="loguniform_1e-4_1e-2_mearth", level=1)
+    ki.meta["config"] = gi.CONFIG_NAMES[3] + f"_replica{rank}"
+    return ki
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU while the timed region runs (NVML)."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons = index, period_s, [], set()
+        self.max_mhz, self._stop_evt, self.err = None, threading.Event(), None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            names = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                     "sw_power_cap": 0x4, "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10,
+                     "applications_clocks_setting": 0x2}
+            while not self._stop_evt.is_set():
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                self.reasons |= {k for k, bit in names.items() if mask & bit}
+                time.sleep(self.period)
+        except Exception as e:  # NVML missing: the line says so instead of inventing clocks
+            self.err = repr(e)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        d = {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+             "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        if self.err:
+            d["error"] = self.err
+        return d
+
+
+def physical_gpu_index(local_index: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        ids = [v.strip() for v in vis.split(",") if v.strip()]
+        if local_index < len(ids) and ids[local_index].isdigit():
+            return int(ids[local_index])
+    return local_index
+
+
+def oracle_sample(ki, rows_per_level: int, oracle):
+    """The oracle, as it stands, on `rows_per_level` evenly spaced i-rows (all j) at both levels.
+    Returns (seconds, ordered pair interactions)."""
+    rows = np.linspace(0, ki.n - 1, rows_per_level).astype(np.int32)
+    t0 = time.perf_counter()
+    for level in LEVELS:
+        oracle.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=level, G=ki.G,
+                    enc_factor=ki.enc_factor, rows=rows)
+    dt = time.perf_counter() - t0
+    return dt, len(LEVELS) * rows_per_level * (ki.n_massive - 1)
+
+
+def calibrate_rows(ki, oracle, target_s: float) -> int:
+    probe = 64
+    t, _ = oracle_sample(ki, probe, oracle)
+    return int(max(probe, min(ki.n, probe * target_s / max(t, 1e-6))))
+
+
+def run_reference(args, rank: int, world: int):
+    if rank != 0:
+        return
+    import oracle
+    ki = workload(0)
+    cores = oracle.num_threads()
+    rows = calibrate_rows(ki, oracle, target_s=2.0)          # ~2 s per step => K=20, W=5: under a minute
+    for _ in range(args.warmup):
+        oracle_sample(ki, rows, oracle)
+    t_tot, pairs_tot = 0.0, 0
+    for _ in range(args.steps):
+        t, p = oracle_sample(ki, rows, oracle)
+        t_tot += t
+        pairs_tot += p
+    value = pairs_tot / t_tot
+    sample = (f"{rows} evenly spaced i-rows x all {ki.n_massive} j, levels 0 and 1, per step "
+              f"(full step = {ki.n} rows); wall clock")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[3]: N=65536 planetesimal disk, two-level changeover (L=0 and L=1)",
+                       "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_b200(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+    from paper_2201_10058_b200 import GengaKick        # raises if the CUDA library is missing
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    ki = workload(rank)
+    n = ki.n
+    kick = GengaKick(ki.n_massive, ki.n_test, max_level=max(LEVELS), pair_capacity=PAIR_CAPACITY, G=ki.G,
+                     enc_factor=ki.enc_factor, device=local_rank)
+    stream = torch.cuda.current_stream()
+    kick.set_stream(stream.cuda_stream)
+    kick.enable_timing(True)
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    pos, mass, rcrit = to_dev(ki.pos), to_dev(ki.mass), to_dev(ki.rcrit)
+    vel = to_dev(ki.vel)
+    acc = torch.empty(3, n, dtype=torch.float64, device=dev)
+    pairs = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev)
+    npairs = torch.empty(n + 1, dtype=torch.int32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 256 MiB > 126 MB of L2
+
+    def step():
+        for level in LEVELS:
+            kick.kick(pos, vel, mass, rcrit, level, 0.5 * ki.dt, acc, pairs, npairs)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # FP64 ALU roofline of this device, measured before the timed region
+    dfma_rate = kick.measure_dfma_rate(iters=8192, reps=5)
+    for _ in range(args.warmup):
+        step()
+        flush.fill_(1)
+    torch.cuda.synchronize()
+    enc_pairs = {}
+
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    launches0 = kick.launch_count()
+    barrier()
+    sampler.start()
+    e0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    e1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    loop_ms = {level: [] for level in LEVELS}
+    for s in range(args.steps):
+        e0[s].record(stream)
+        step()
+        e1[s].record(stream)
+        flush.fill_(s & 0xff)                      # L2 flush between timed iterations (outside the events)
+        e1[s].synchronize()
+        for level in LEVELS:
+            loop_ms[level].append(kick.last_pair_loop_ms(level))
+    barrier()
+    clocks = sampler.stop()
+    launches = kick.launch_count() - launches0
+    step_ms = [a.elapsed_time(b) for a, b in zip(e0, e1)]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    pairs_per_kick = ki.n_massive * (ki.n_massive - 1) + ki.n_test * ki.n_massive
+    pairs_per_step = len(LEVELS) * pairs_per_kick
+    value = world * pairs_per_step * args.steps / (total_ms * 1e-3)
+
+    # per-level numbers: one more kick each, timed alone (after the timed region)
+    levels = {}
+    for level in LEVELS:
+        ts = []
+        for _ in range(5):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            flush.fill_(3)
+            a.record(stream)
+            kick.kick(pos, vel, mass, rcrit, level, 0.5 * ki.dt, acc, pairs, npairs)
+            b.record(stream)
+            b.synchronize()
+            ts.append(a.elapsed_time(b))
+        enc_pairs[level] = int(npairs[n].item())
+        ms = float(np.median(ts))
+        levels[str(level)] = {"ms_per_kick": ms, "pairs_per_s": pairs_per_kick / (ms * 1e-3),
+                              "pair_loop_ms": float(np.mean(loop_ms[level])), "encounter_pairs": enc_pairs[level]}
+
+    # end to end through the host entry point: pinned host arrays in, results back, every step
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
+    h_acc = torch.empty(3, n, dtype=torch.float64).pin_memory()
+    h_pairs = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32).pin_memory()
+    h_np = torch.empty(n + 1, dtype=torch.int32).pin_memory()
+
+    def host_step():
+        for level in LEVELS:
+            kick.kick_host(h_pos, h_vel, h_mass, h_rc, level, 0.5 * ki.dt, h_acc, h_pairs, h_np)
+
+    for _ in range(max(args.warmup, 3)):
+        host_step()
+    e2e_steps = args.steps
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        host_step()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = sum(8 * n * (3 + 3 + 1 + (level + 1)) for level in LEVELS)
+    d2h = sum(8 * n * (3 + 3) + 4 * (n + 1) + 8 * min(enc_pairs[level], PAIR_CAPACITY) for level in LEVELS)
+    e2e_value = world * pairs_per_step * e2e_steps / e2e_s
+
+    if rank == 0:
+        props = torch.cuda.get_device_properties(local_rank)
+        sm_max_mhz = clocks.get("sm_max_mhz") or 1965
+        peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+        peak_dfma = 2.0 * dfma_rate / 1e12
+        k0_ms = float(np.mean(loop_ms[0]))
+        achieved = FLOPS_PER_PAIR * pairs_per_kick / (k0_ms * 1e-3) / 1e12
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[3]: N=65536 planetesimal disk (sigma ~ a^-1.5, log-uniform masses), "
+                                   "step = level-0 kick + level-1 kick (two-level changeover, eq. 63), each "
+                                   "with encounter pre-check, pair list, counts and v += dt a",
+                       "n_massive": ki.n_massive, "n_test": ki.n_test, "levels": list(LEVELS),
+                       "pairs_per_step": pairs_per_step, "pair_capacity": PAIR_CAPACITY,
+                       "l2": "256 MiB buffer written between timed iterations (working set 3 MB is L2-resident)",
+                       "parallelism": "replicas" if world > 1 else "single GPU"},
+            "levels": levels,
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
+                    "api": "genga_kick_host (pinned host arrays, copies and synchronisation inside the call)"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "kernel": "kick_kernel<dense> (level 0)", "achieved": achieved,
+                         "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
+                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+                         "peak_source": f"nominal: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes "
+                                        f"x 2 x {sm_max_mhz} MHz (no FP64 figure in MEASURED_PEAKS.json)",
+                         "peak_measured_dfma": peak_dfma, "frac_of_measured_dfma": achieved / peak_dfma,
+                         "flops_per_pair": FLOPS_PER_PAIR, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR,
+                         "fp64_pipe_issue_frac": FP64_INSTR_PER_PAIR * pairs_per_kick / (k0_ms * 1e-3) /
+                                                 (props.multi_processor_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
+                         "kernel_ms": k0_ms, "pairs_per_launch": pairs_per_kick},
+        }
+        import oracle                                   # cpu_baseline leg: rank 0, N=1 only
+        if world == 1 and not args.no_cpu_baseline:
+            rows = calibrate_rows(ki, oracle, target_s=12.0)
+            t, p = oracle_sample(ki, rows, oracle)
+            line["cpu_baseline"] = {"value": p / t, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                                    "sample": f"{rows} evenly spaced i-rows x all {ki.n_massive} j at levels 0 and 1 "
+                                              f"({t:.1f} s wall clock)"}
+        print(json.dumps(line), flush=True)
+    kick.free()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3                                  # timing rule: W >= 3
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus > 1 and world == 1:
+        # convenience: re-launch under torchrun as the driver would
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                   f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+                                   "--master-port", os.environ.get("MASTER_PORT", "29541"), os.path.abspath(__file__),
+                                   *sys.argv[1:]])
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_b200(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

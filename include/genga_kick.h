@@ -149,6 +149,21 @@ int genga_kick_status(genga_kick_ctx* ctx, int32_t* status);
 /* Kernel launches enqueued by the context since init (for the bench's launch count). */
 int64_t genga_kick_launch_count(const genga_kick_ctx* ctx);
 
+/* Measurement aid: with on != 0 every following genga_kick records a CUDA event pair around its
+ * pair-loop kernel (the N^2 part, rows a1-a6 of SURVEY.md 8(a)) on the context's stream.
+ * genga_kick_last_pair_loop_ms waits for the pair of the most recent call at `changeover_level`
+ * and returns that kernel's duration in *ms (it synchronises on the event, like
+ * genga_kick_status / genga_kick_host synchronise on the stream).
+ * Errors: E_NULL, E_LEVEL, E_NOMEM, E_CUDA; E_SIZE if timing is off or no such call was made. */
+int genga_kick_enable_timing(genga_kick_ctx* ctx, int32_t on);
+int genga_kick_last_pair_loop_ms(genga_kick_ctx* ctx, int32_t changeover_level, float* ms);
+
+/* Measurement aid: the plain FP64 ALU roofline of the device.  Runs `reps` launches of a kernel
+ * of independent DFMA chains (8 chains per thread, `iters` x 8 DFMAs each, 1024 threads x 2 CTAs
+ * per SM) on the context's stream and returns the best launch's rate in *dfma_per_s (one DFMA =
+ * 2 flops).  Synchronises.  Errors: E_NULL, E_SIZE (iters or reps < 1), E_CUDA. */
+int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, int32_t reps, double* dfma_per_s);
+
 /* Free the context and its scratch.  NULL is allowed. */
 int genga_kick_free(genga_kick_ctx* ctx);
 

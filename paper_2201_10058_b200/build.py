@@ -8,6 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgenga_kick.so")
 SOURCES = [os.path.join(CSRC, "genga_kick.cu"), os.path.join(CSRC, "genga_kick_plan.cpp")]
 DEPENDS = SOURCES + [os.path.join(CSRC, "genga_kick_kernels.cuh"), os.path.join(CSRC, "genga_kick_variants.h"),
+                     os.path.join(CSRC, "genga_kick_sort.cuh"),
                      os.path.join(os.path.dirname(HERE), "include", "genga_kick.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # --fmad=false: no contraction the source does not spell out (the kernels write every fma() themselves)

@@ -42,6 +42,10 @@ struct genga_kick_ctx {
     double* h_pos; double* h_vel; double* h_mass; double* h_rcrit; double* h_acc;
     int32_t* h_pairs; int32_t* h_npairs;
     int64_t launches;
+    // measurement aids (genga_kick_enable_timing)
+    bool timing;
+    cudaEvent_t* ev;               // [max_level + 1][2], created by genga_kick_enable_timing
+    bool* ev_set;                  // [max_level + 1]
     std::string cuda_err;
 };
 
@@ -143,7 +147,7 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
     return GENGA_KICK_OK;
 
 cuda_error:
-    (void)e;
+    (void)e;                       // the context is freed below: the text of e cannot be kept
     rc = GENGA_KICK_E_CUDA;
 fail:
     genga_kick_free(ctx);
@@ -209,7 +213,12 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
         kp.partial = ctx->partial;
         kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
         kp.status = ctx->status;
+        if (ctx->timing) GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level], st));
         GK_CUDA(ctx, dispatch_kick(pl, changeover_level == 0, kp, st));
+        if (ctx->timing) {
+            GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level + 1], st));
+            ctx->ev_set[changeover_level] = true;
+        }
         ctx->launches++;
     }
     {
@@ -290,6 +299,89 @@ extern "C" int genga_kick_status(genga_kick_ctx* ctx, int32_t* status)
     return GENGA_KICK_OK;
 }
 
+extern "C" int genga_kick_enable_timing(genga_kick_ctx* ctx, int32_t on)
+{
+    if (!ctx) return GENGA_KICK_E_NULL;
+    const int nl = ctx->cfg.max_level + 1;
+    if (on && !ctx->ev) {
+        ctx->ev = static_cast<cudaEvent_t*>(std::calloc((size_t)2 * nl, sizeof(cudaEvent_t)));
+        ctx->ev_set = static_cast<bool*>(std::calloc((size_t)nl, sizeof(bool)));
+        if (!ctx->ev || !ctx->ev_set) return GENGA_KICK_E_NOMEM;
+        for (int k = 0; k < 2 * nl; k++) GK_CUDA(ctx, cudaEventCreate(&ctx->ev[k]));
+    }
+    ctx->timing = on != 0;
+    if (ctx->ev_set) std::memset(ctx->ev_set, 0, (size_t)nl * sizeof(bool));
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_last_pair_loop_ms(genga_kick_ctx* ctx, int32_t changeover_level, float* ms)
+{
+    if (!ctx || !ms) return GENGA_KICK_E_NULL;
+    if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
+    if (!ctx->timing || !ctx->ev_set[changeover_level]) return GENGA_KICK_E_SIZE;
+    GK_CUDA(ctx, cudaEventSynchronize(ctx->ev[2 * changeover_level + 1]));
+    GK_CUDA(ctx, cudaEventElapsedTime(ms, ctx->ev[2 * changeover_level], ctx->ev[2 * changeover_level + 1]));
+    return GENGA_KICK_OK;
+}
+
+namespace genga {
+// Independent DFMA chains: the plain FP64 ALU roofline (include/genga_kick.h).  The operands come
+// from memory so that nothing folds; the result is stored so that nothing is dropped.
+__global__ void __launch_bounds__(1024, 2) dfma_rate_kernel(const double* __restrict__ in, double* __restrict__ out, int iters)
+{
+    const double m = in[0], c = in[1];
+    double a[8];
+#pragma unroll
+    for (int k = 0; k < 8; k++) a[k] = in[2] * (double)(threadIdx.x + k);
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+#pragma unroll
+            for (int k = 0; k < 8; k++) a[k] = fma(a[k], m, c);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; k++) s += a[k];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace genga
+
+extern "C" int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, int32_t reps, double* dfma_per_s)
+{
+    if (!ctx || !dfma_per_s) return GENGA_KICK_E_NULL;
+    if (iters < 1 || reps < 1) return GENGA_KICK_E_SIZE;
+    const int blocks = 2 * ctx->num_sms, threads = 1024;
+    double* buf = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaStream_t st = ctx->stream;
+    const double host_in[3] = {0.999999, 1.0e-6, 1.0e-3};
+    cudaError_t e;
+    float best = 0.0f;
+    if ((e = cudaMalloc(&buf, ((size_t)blocks * threads + 4) * sizeof(double))) != cudaSuccess) goto done;
+    if ((e = cudaMemcpyAsync(buf, host_in, sizeof(host_in), cudaMemcpyHostToDevice, st)) != cudaSuccess) goto done;
+    if ((e = cudaEventCreate(&e0)) != cudaSuccess) goto done;
+    if ((e = cudaEventCreate(&e1)) != cudaSuccess) goto done;
+    for (int r = 0; r <= reps; r++) {                              // launch 0 is the warm-up
+        if ((e = cudaEventRecord(e0, st)) != cudaSuccess) goto done;
+        genga::dfma_rate_kernel<<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
+        if ((e = cudaGetLastError()) != cudaSuccess) goto done;
+        if ((e = cudaEventRecord(e1, st)) != cudaSuccess) goto done;
+        if ((e = cudaEventSynchronize(e1)) != cudaSuccess) goto done;
+        float ms = 0.0f;
+        if ((e = cudaEventElapsedTime(&ms, e0, e1)) != cudaSuccess) goto done;
+        if (r > 0 && (best == 0.0f || ms < best)) best = ms;
+        ctx->launches++;
+    }
+    *dfma_per_s = (double)blocks * threads * 64.0 * (double)iters / ((double)best * 1.0e-3);
+done:
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (buf) cudaFree(buf);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return GENGA_KICK_OK;
+}
+
 extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)
@@ -300,6 +392,11 @@ extern "C" int genga_kick_free(genga_kick_ctx* ctx)
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs};
     for (void* b : bufs)
         if (b) cudaFree(b);
+    if (ctx->ev)
+        for (int k = 0; k < 2 * (ctx->cfg.max_level + 1); k++)
+            if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+    std::free(ctx->ev);
+    std::free(ctx->ev_set);
     std::free(ctx->plans);
     delete ctx;
     return GENGA_KICK_OK;

@@ -1,0 +1,120 @@
+"""-m "not gpu": the C-ABI library loads, exports every symbol include/genga_kick.h declares, and its
+host-side logic (work decomposition, argument checks that need no device) behaves as documented.
+No compute call is made here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2201_10058_b200 as g
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def built():
+    from paper_2201_10058_b200 import build
+    return build.build()
+
+
+def test_every_declared_symbol_is_exported(built):
+    header = open(os.path.join(ROOT, "include", "genga_kick.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(genga_kick\w*)\s*\(", header))
+    assert declared, "no declarations found in include/genga_kick.h"
+    lib = ctypes.CDLL(built)
+    missing = [name for name in sorted(declared) if not hasattr(lib, name)]
+    assert not missing, f"declared but not exported: {missing}"
+    assert declared == set(g.EXPORTS), f"binding and header disagree: {declared ^ set(g.EXPORTS)}"
+
+
+def test_strerror_texts(built):
+    for code in (g.OK, g.E_NULL, g.E_ALIGN, g.E_SIZE, g.E_LEVEL, g.E_CUDA, g.E_NOMEM):
+        assert g.strerror(code) and "unknown" not in g.strerror(code)
+    assert "unknown" in g.strerror(-99)
+
+
+def test_init_without_device_fails_loudly(built):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(g.GengaKickError) as e:
+        g.GengaKick(128, 0)
+    assert e.value.code == g.E_CUDA                  # no CPU fallback
+
+
+def test_init_argument_checks(built):
+    for nm, nt, lvl in [(-1, 0, 0), (0, 0, 0), (5, -2, 0)]:
+        with pytest.raises(g.GengaKickError) as e:
+            g.GengaKick(nm, nt, max_level=lvl)
+        assert e.value.code == g.E_SIZE
+    with pytest.raises(g.GengaKickError) as e:
+        g.GengaKick(10, 0, max_level=-1)
+    assert e.value.code == g.E_LEVEL
+
+
+@pytest.mark.parametrize("nm,nt,level", [(1, 0, 0), (2048, 0, 0), (8192, 0, 0), (32770, 0, 1), (65536, 0, 0),
+                                         (65536, 0, 1), (2048, 1048576, 0), (0, 500, 0), (257, 1, 0), (5000, 0, 2)])
+def test_plan_covers_every_tile_once(built, nm, nt, level):
+    sms = 148
+    p = g.make_plan(nm, nt, level, sms)
+    d = p.as_dict()
+    assert d["i_block"] == d["threads"] * d["i_per_thread"]
+    assert d["m_pad"] >= nm and d["m_pad"] % d["j_tile"] == 0
+    n_i = d["m_pad"] + nt if nt else nm
+    assert d["n_i_blocks"] * d["i_block"] >= n_i and d["n_rec"] >= n_i and d["n_rec"] % d["i_block"] == 0
+    assert d["n_j_tiles"] * d["j_tile"] >= nm and d["n_tiles"] == d["n_i_blocks"] * d["n_j_tiles"]
+    assert d["n_ctas"] <= max(d["n_tiles"], 0) or d["n_tiles"] == 0
+    if d["n_tiles"] > d["n_ctas"]:
+        assert d["n_ctas"] % sms == 0                # whole waves unless there are fewer tiles than that
+    # ranges are contiguous, disjoint, cover [0, T), balanced to one tile
+    prev, sizes, segs = 0, [], 1
+    for c in range(d["n_ctas"]):
+        t0, t1 = g.plan_cta_range(p, c)
+        assert t0 == prev and t1 >= t0
+        prev = t1
+        sizes.append(t1 - t0)
+        if t1 > t0:
+            segs = max(segs, (t1 - 1) // d["n_j_tiles"] - t0 // d["n_j_tiles"] + 1)
+    assert prev == d["n_tiles"]
+    if sizes:
+        assert max(sizes) - min(sizes) <= 1
+    assert d["max_segs"] == segs
+    assert d["partial_doubles"] == d["n_ctas"] * d["max_segs"] * 3 * d["i_block"]
+    # the reduction pass visits exactly the CTAs whose range meets the i-block
+    for ib in sorted({0, d["n_i_blocks"] // 2, d["n_i_blocks"] - 1}):
+        if d["n_j_tiles"] == 0 or ib < 0:
+            continue
+        a, b = g.plan_iblock_ctas(p, ib)
+        ta, tb = ib * d["n_j_tiles"], (ib + 1) * d["n_j_tiles"]
+        meets = [c for c in range(d["n_ctas"]) if (lambda r: r[0] < tb and r[1] > ta and r[1] > r[0])(g.plan_cta_range(p, c))]
+        assert meets == list(range(a, b + 1))
+
+
+def test_plan_errors(built):
+    with pytest.raises(g.GengaKickError) as e:
+        g.make_plan(0, 0, 0, 148)
+    assert e.value.code == g.E_SIZE
+    with pytest.raises(g.GengaKickError) as e:
+        g.make_plan(10, 0, -1, 148)
+    assert e.value.code == g.E_LEVEL
+    with pytest.raises(g.GengaKickError) as e:
+        g.make_plan(10, 0, 0, 0)
+    assert e.value.code == g.E_SIZE
+
+
+def test_product_does_not_touch_the_oracle():
+    """The product path may not import, link or read oracle/ (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_2201_10058_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
+                assert "oracle/" not in text.replace("shared with oracle/", "").replace("imports oracle/", ""), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2201_10058_b200" not in text.replace("paper_2201_10058_b200/csrc/", "") or f.endswith(".c")
+            assert not re.search(r"^\s*(from|import)\s+paper_2201_10058_b200\b", text, flags=re.M), f
