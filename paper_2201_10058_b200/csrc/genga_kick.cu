@@ -63,7 +63,7 @@ bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) !
 template <int THREADS, int IPT, int JT, int CTAS, bool DENSE>
 cudaError_t launch_kick(const genga::KickParams& kp, cudaStream_t st)
 {
-    genga::kick_kernel<THREADS, IPT, JT, CTAS, DENSE><<<kp.n_ctas, THREADS, 0, st>>>(kp);
+    genga::kick_kernel<THREADS, IPT, JT, CTAS, DENSE, GENGA_STAGES><<<kp.n_ctas, THREADS, 0, st>>>(kp);
     return cudaGetLastError();
 }
 

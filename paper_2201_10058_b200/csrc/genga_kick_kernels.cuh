@@ -100,8 +100,13 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
         m = max(m, __shfl_xor_sync(0xffffffffu, m, 4));
         if (r < n_rec && (r % GENGA_CHUNK) == 0) cfw[r / GENGA_CHUNK] = m;
         // group box
-        float lx = __double2float_rd(x), ly = __double2float_rd(y), lz = __double2float_rd(z);
-        float hx = __double2float_ru(x), hy = __double2float_ru(y), hz = __double2float_ru(z);
+        // ... over the real bodies of the group only: a padding record (fw = -1) cannot trip the
+        // filter, and a group without real bodies gets an empty box that is near to nothing
+        const bool real = fw >= 0;
+        float lx = real ? __double2float_rd(x) : 3.0e38f, ly = real ? __double2float_rd(y) : 3.0e38f,
+              lz = real ? __double2float_rd(z) : 3.0e38f;
+        float hx = real ? __double2float_ru(x) : -3.0e38f, hy = real ? __double2float_ru(y) : -3.0e38f,
+              hz = real ? __double2float_ru(z) : -3.0e38f;
 #pragma unroll
         for (int o = 8; o < 32; o <<= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
 #pragma unroll
@@ -320,32 +325,108 @@ __device__ __forceinline__ bool boxes_near(float4 alo, float4 ahi, int afw, floa
     return !(d2 >= R2);
 }
 
-template <int THREADS, int IPT, int JT, int CTAS, bool DENSE>
+// ---------------------------------------------------------------------------------------------
+// Exact path, lane-parallel.  Pairs the filter catches are not evaluated where they are found (one
+// lane at a time): the warp appends (i-record, j-record) to its candidate queue in shared memory
+// and, whenever 32 candidates are waiting (and before its accumulators are flushed), DRAINS them:
+// lane e evaluates candidate e with exact_pair -- weight, pre-check, pair emission with one atomic
+// per drain -- and the terms are then handed to the lanes that own the i-bodies in queue order
+// (shuffles), so the summation order is a fixed function of the inputs.
+// ---------------------------------------------------------------------------------------------
+#define GENGA_QCAP 64              // entries per warp queue (a push adds <= 32 to < 32 waiting)
+
+template <int IPT>
+__device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __restrict__ q, int head, int n,
+                                            double (&ax)[IPT], double (&ay)[IPT], double (&az)[IPT], int (&cnt)[IPT])
+{
+    const int lane = threadIdx.x & 31;
+    double s = 0.0, dx = 0.0, dy = 0.0, dz = 0.0;
+    int info = -1;                                         // enc << 8 | k << 5 | owner lane; -1: nothing to add
+    bool hit = false;
+    int lo = 0, hi = 0;
+    if (lane < n) {
+        const int2 e = q[(head + lane) & (GENGA_QCAP - 1)];
+        const int ir = e.x, jr = e.y;
+        const int bi = p.ridx[ir], bj = p.ridx[jr];
+        if (ir != jr && bi >= 0 && bj >= 0) {
+            const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
+            dx = __dsub_rn(jxy.x, ixy.x); dy = __dsub_rn(jxy.y, ixy.y); dz = __dsub_rn(jzm.x, izm.x);
+            const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
+            s = r.s;
+            info = (r.enc << 8) | (((ir >> 5) % IPT) << 5) | (ir & 31);
+            if (r.enc) {
+                if (bi >= p.n_massive) {                   // test particle i, massive j
+                    atomicAdd(p.out_npairs + bj, 1);
+                    hit = true; lo = bj; hi = bi;
+                } else if (bi < bj) {
+                    hit = true; lo = bi; hi = bj;
+                }
+            }
+        }
+    }
+    emit_pairs(p, hit, lo, hi);
+    for (int e = 0; e < n; e++) {
+        const int inf = __shfl_sync(0xffffffffu, info, e);
+        if (inf < 0) continue;                             // warp-uniform
+        const double se = __shfl_sync(0xffffffffu, s, e);
+        const double dxe = __shfl_sync(0xffffffffu, dx, e), dye = __shfl_sync(0xffffffffu, dy, e),
+                     dze = __shfl_sync(0xffffffffu, dz, e);
+        if (lane == (inf & 31)) {
+            const int k = (inf >> 5) & 7;
+#pragma unroll
+            for (int kk = 0; kk < IPT; kk++)
+                if (kk == k) {
+                    ax[kk] = fma(se, dxe, ax[kk]);
+                    ay[kk] = fma(se, dye, ay[kk]);
+                    az[kk] = fma(se, dze, az[kk]);
+                    cnt[kk] += inf >> 8;
+                }
+        }
+    }
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+template <int THREADS, int IPT, int JT, int CTAS, bool DENSE, int STAGES>
 __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
     constexpr int IB = THREADS * IPT;
+    constexpr int WARPS = THREADS / 32;
     constexpr int NCH = JT / GENGA_CHUNK;
     constexpr int NG = JT / GENGA_GROUP;
     constexpr uint32_t TILE_BYTES = JT * 32 + NG * 32 + NCH * 4;
     static_assert(NG <= 32 && JT % GENGA_GROUP == 0, "one lane per group");
-    __shared__ TileStage<JT> st[2];
-    __shared__ __align__(8) uint64_t full[2];
+    static_assert(GENGA_CHUNK * IPT <= 32, "one trigger bit per pair of a chunk");
+    __shared__ TileStage<JT> st[STAGES];
+    __shared__ int2 queue[WARPS][GENGA_QCAP];
+    __shared__ __align__(8) uint64_t full[STAGES];
+    __shared__ __align__(8) uint64_t empty[STAGES];
 
-    const int tid = threadIdx.x, lane = tid & 31;
-    const int woff = (tid >> 5) * (32 * IPT) + lane;        // offset of the thread's first record in the i-block
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int woff = warp * (32 * IPT) + lane;              // offset of the thread's first record in the i-block
     const long long t0 = plan_tile_begin(blockIdx.x, p.n_tiles, p.n_ctas);
     const long long t1 = plan_tile_begin(blockIdx.x + 1, p.n_tiles, p.n_ctas);
     if (t0 >= t1) return;
 
     if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
+#pragma unroll
+        for (int s = 0; s < STAGES; s++) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], WARPS);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    auto issue = [&](long long t, int s) {
-        const int jt = (int)(t % p.n_j_tiles);
+    // tile t0 + g goes to stage g % STAGES; the stage is free once every warp has arrived on its
+    // `empty` barrier for the tile that used it before (g - STAGES)
+    auto issue = [&](int g) {
+        const int s = g % STAGES;
+        if (g >= STAGES) mbar_wait(&empty[s], (uint32_t)((g / STAGES - 1) & 1));
+        const int jt = (int)((t0 + g) % p.n_j_tiles);
         mbar_expect_tx(&full[s], TILE_BYTES);
         bulk_g2s(st[s].xy, p.rxy + (size_t)jt * JT, JT * 16, &full[s]);
         bulk_g2s(st[s].zm, p.rzm + (size_t)jt * JT, JT * 16, &full[s]);
@@ -353,10 +434,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         bulk_g2s(st[s].bhi, p.cbhi + (size_t)jt * NG, NG * 16, &full[s]);
         bulk_g2s(st[s].cf, p.cfw + (size_t)jt * NCH, NCH * 4, &full[s]);
     };
-    if (tid == 0) {
-        issue(t0, 0);
-        if (t0 + 1 < t1) issue(t0 + 1, 1);
-    }
+    const int n_it = (int)(t1 - t0);
+    if (tid == 0)
+        for (int g = 0; g < STAGES && g < n_it; g++) issue(g);
 
     double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT];
     int fi[IPT], bi[IPT], cnt[IPT];
@@ -364,8 +444,14 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
     int wfw = -1;
     const int first_ib = (int)(t0 / p.n_j_tiles);
     int cur_ib = -1;
+    int2* const q = queue[warp];
+    int qhead = 0, qtail = 0;                               // warp-uniform; entries [qhead, qtail) wait
 
     auto flush = [&]() {
+        __syncwarp();
+        if (qtail != qhead) drain_queue<IPT>(p, q, qhead, qtail - qhead, ax, ay, az, cnt);
+        qhead = qtail;
+        __syncwarp();
         const size_t base = ((size_t)blockIdx.x * p.max_segs + (cur_ib - first_ib)) * 3 * IB;
 #pragma unroll
         for (int k = 0; k < IPT; k++) {
@@ -377,9 +463,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         }
     };
 
-    for (long long t = t0; t < t1; ++t) {
-        const int it = (int)(t - t0);
-        const int s = it & 1;
+    for (int it = 0; it < n_it; ++it) {
+        const long long t = t0 + it;
+        const int s = it % STAGES;
         const int ib = (int)(t / p.n_j_tiles);
         const int jt = (int)(t - (long long)ib * p.n_j_tiles);
         if (ib != cur_ib) {
@@ -404,7 +490,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                 wfw = max(wfw, __float_as_int(glo.w));
             }
         }
-        mbar_wait(&full[s], (uint32_t)((it >> 1) & 1));
+        mbar_wait(&full[s], (uint32_t)((it / STAGES) & 1));
         const TileStage<JT>& S = st[s];
 
         const bool mine_near = lane < NG ? boxes_near(wlo, whi, wfw, S.blo[lane], S.bhi[lane]) : false;
@@ -431,52 +517,40 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                 int thr[IPT];
 #pragma unroll
                 for (int k = 0; k < IPT; k++) thr[k] = max(fi[k], cm);
-                bool any = false;
+                unsigned tm = 0;                            // bit u * IPT + k: pair (k, jj + u) tripped the filter
 #pragma unroll
                 for (int u = 0; u < GENGA_CHUNK; u++) {
                     const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
 #pragma unroll
-                    for (int k = 0; k < IPT; k++)
-                        pair_fast<DENSE>(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], any);
+                    for (int k = 0; k < IPT; k++) {
+                        bool trig = false;
+                        pair_fast<DENSE>(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], trig);
+                        tm |= (trig ? 1u : 0u) << (u * IPT + k);
+                    }
                 }
-                if (__any_sync(0xffffffffu, any)) {
-                    // exact path: the pairs of this chunk that the filter caught (a3, a5, a6)
-#pragma unroll 1
-                    for (int u = 0; u < GENGA_CHUNK; u++) {
-                        const int jrec = jt * JT + jj + u;
-                        const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
-#pragma unroll
-                        for (int k = 0; k < IPT; k++) {
-                            const double dx = __dsub_rn(xy.x, xi[k]), dy = __dsub_rn(xy.y, yi[k]), dz = __dsub_rn(zm.x, zi[k]);
-                            const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
-                            bool hit = false;
-                            int lo = 0, hi = 0;
-                            if (__double2hiint(r2) < thr[k] && ib * IB + woff + k * 32 != jrec) {
-                                const int bj = p.ridx[jrec];
-                                if (bj >= 0 && bi[k] >= 0) {
-                                    const ExactResult e = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi[k], bj, dx, dy, dz, zm.y);
-                                    ax[k] = fma(e.s, dx, ax[k]);
-                                    ay[k] = fma(e.s, dy, ay[k]);
-                                    az[k] = fma(e.s, dz, az[k]);
-                                    if (e.enc) {
-                                        cnt[k]++;
-                                        if (bi[k] >= p.n_massive) {          // test particle i, massive j
-                                            atomicAdd(p.out_npairs + bj, 1);
-                                            hit = true; lo = bj; hi = bi[k];
-                                        } else if (bi[k] < bj) {
-                                            hit = true; lo = bi[k]; hi = bj;
-                                        }
-                                    }
-                                }
-                            }
-                            emit_pairs(p, hit, lo, hi);
-                        }
+                unsigned todo = __reduce_or_sync(0xffffffffu, tm);
+                while (todo) {                              // warp-uniform: the (u, k) some lane tripped
+                    const int b = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    const bool mine = (tm >> b) & 1u;
+                    const unsigned m = __ballot_sync(0xffffffffu, mine);
+                    if (mine) {
+                        const int slot = qtail + __popc(m & ((1u << lane) - 1u));
+                        q[slot & (GENGA_QCAP - 1)] = make_int2(ib * IB + woff + (b % IPT) * 32, jt * JT + jj + b / IPT);
+                    }
+                    qtail += __popc(m);
+                    if (qtail - qhead >= 32) {
+                        __syncwarp();
+                        drain_queue<IPT>(p, q, qhead, 32, ax, ay, az, cnt);
+                        qhead += 32;
+                        __syncwarp();
                     }
                 }
             }
         }
-        __syncthreads();                                   // every warp is done with stage s
-        if (tid == 0 && t + 2 < t1) issue(t + 2, s);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]);              // this warp is done with stage s
+        if (tid == 0 && it >= 1 && it - 1 + STAGES < n_it) issue(it - 1 + STAGES);
     }
     flush();
 }

@@ -3,8 +3,8 @@
 // The pair loop is fastest when a warp's i-bodies and a chunk's j-bodies are neighbours in space:
 // then almost every (warp, chunk) combination is provably out of range of every critical radius
 // and runs without any per-pair check.  The library therefore works on a spatially sorted copy
-// of the bodies: key = class bit (massive / test particle) | 16-bit Morton code of the (x, y)
-// cell in a 256 x 256 grid over the bounding box.  The caller never sees this order (indices in
+// of the bodies: key = class bit (massive / test particle) | 16-bit Hilbert-curve index of the
+// (x, y) cell in a 256 x 256 grid over the bounding box.  The caller never sees this order (indices in
 // the outputs are the caller's).
 //
 // The sort is a least-significant-digit radix sort (8 + 9 bits), STABLE, hence a fixed function
@@ -60,12 +60,23 @@ bbox_kernel(const double* __restrict__ pos, int N, unsigned* __restrict__ bbox)
     }
 }
 
-__device__ __forceinline__ unsigned spread8(unsigned v)      // 8 bits -> even bit positions
+// Position of cell (x, y) of a 2^GENGA_GRID_BITS-square grid along the Hilbert curve.  Unlike the
+// Morton (Z) order the curve never jumps: cells with consecutive indices share an edge, so any
+// run of consecutive bodies is spatially compact -- which is what keeps the culling boxes small.
+__device__ __forceinline__ unsigned hilbert_index(unsigned x, unsigned y)
 {
-    v = (v | (v << 4)) & 0x0f0fu;
-    v = (v | (v << 2)) & 0x3333u;
-    v = (v | (v << 1)) & 0x5555u;
-    return v;
+    constexpr unsigned n = 1u << GENGA_GRID_BITS;
+    unsigned d = 0;
+#pragma unroll
+    for (unsigned s = n >> 1; s > 0; s >>= 1) {
+        const unsigned rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
+        d += s * s * ((3u * rx) ^ ry);
+        if (ry == 0) {                                        // rotate / reflect the quadrant
+            if (rx) { x = (n - 1u) - x; y = (n - 1u) - y; }
+            const unsigned t = x; x = y; y = t;
+        }
+    }
+    return d;
 }
 
 // key of body b; counts of the first digit per sort block
@@ -88,7 +99,7 @@ key_hist_kernel(const double* __restrict__ pos, int N, int n_massive, const unsi
             // NaN or out-of-box values land in cell 0 / the last cell; any key gives a correct kick
             const unsigned ix = (unsigned)min(max((int)fx, 0), (1 << GENGA_GRID_BITS) - 1);
             const unsigned iy = (unsigned)min(max((int)fy, 0), (1 << GENGA_GRID_BITS) - 1);
-            const unsigned key = (b >= n_massive ? 0x10000u : 0u) | spread8(ix) | (spread8(iy) << 1);
+            const unsigned key = (b >= n_massive ? 0x10000u : 0u) | hilbert_index(ix, iy);
             keys[b] = key;
             vals[b] = b;
             atomicAdd(&hist[key & (nd - 1)], 1);              // a count: order-free

@@ -43,6 +43,7 @@ static const genga_variant GENGA_SPARSE_VARIANTS[GENGA_N_VARIANTS] = {
     {128, 1, 64, 4},
 };
 static const int GENGA_MIN_TILES_PER_CTA = 4;
+static const int GENGA_STAGES = 4;          // depth of the j-tile ring in shared memory
 static const int GENGA_M_ALIGN = 256;      // every j_tile divides it
 static const int GENGA_SORT_MIN_BODIES = 4096;   // GENGA_KICK_ORDER_AUTO sorts from here on
 static const int GENGA_REC_ALIGN = 1024;   // every i_block divides it
