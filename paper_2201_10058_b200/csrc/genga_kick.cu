@@ -382,6 +382,13 @@ done:
     return GENGA_KICK_OK;
 }
 
+#ifdef GENGA_TRACE
+extern "C" int genga_kick_debug_trace(long long* host, long long n)
+{
+    return (int)cudaMemcpyFromSymbol(host, genga::g_trace, (size_t)n * sizeof(long long));
+}
+#endif
+
 extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)

@@ -336,7 +336,8 @@ __device__ __forceinline__ bool boxes_near(float4 alo, float4 ahi, int afw, floa
 #define GENGA_QCAP 64              // entries per warp queue (a push adds <= 32 to < 32 waiting)
 
 template <int IPT>
-__device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __restrict__ q, int head, int n,
+__device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __restrict__ q, int* __restrict__ own,
+                                            int head, int n,
                                             double (&ax)[IPT], double (&ay)[IPT], double (&az)[IPT], int (&cnt)[IPT])
 {
     const int lane = threadIdx.x & 31;
@@ -344,6 +345,7 @@ __device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __r
     int info = -1;                                         // enc << 8 | k << 5 | owner lane; -1: nothing to add
     bool hit = false;
     int lo = 0, hi = 0;
+    own[lane] = 0;
     if (lane < n) {
         const int2 e = q[(head + lane) & (GENGA_QCAP - 1)];
         const int ir = e.x, jr = e.y;
@@ -365,13 +367,23 @@ __device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __r
         }
     }
     emit_pairs(p, hit, lo, hi);
-    for (int e = 0; e < n; e++) {
+    // hand the terms to the lanes that own the i-bodies: own[l] = mask of the entries lane l owns;
+    // every lane then adds its entries in ascending queue order (a fixed order)
+    __syncwarp();
+    const int owner = info >= 0 ? (info & 31) : 32 + lane;   // 32 + lane: a group of its own, unused
+    const unsigned peers = __match_any_sync(0xffffffffu, owner);
+    if (info >= 0 && lane == __ffs(peers) - 1) own[owner] = (int)peers;
+    __syncwarp();
+    unsigned mine = (unsigned)own[lane];
+    while (__any_sync(0xffffffffu, mine != 0)) {
+        const bool have = mine != 0;
+        const int e = have ? __ffs(mine) - 1 : lane;
+        mine &= mine - 1;
         const int inf = __shfl_sync(0xffffffffu, info, e);
-        if (inf < 0) continue;                             // warp-uniform
         const double se = __shfl_sync(0xffffffffu, s, e);
         const double dxe = __shfl_sync(0xffffffffu, dx, e), dye = __shfl_sync(0xffffffffu, dy, e),
                      dze = __shfl_sync(0xffffffffu, dz, e);
-        if (lane == (inf & 31)) {
+        if (have) {
             const int k = (inf >> 5) & 7;
 #pragma unroll
             for (int kk = 0; kk < IPT; kk++)
@@ -383,6 +395,7 @@ __device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __r
                 }
         }
     }
+    __syncwarp();
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
@@ -390,9 +403,25 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+#ifdef GENGA_TRACE
+// Working aid (never compiled into the product library): per-warp start / end times, SM id and
+// counters of the last kick_kernel launch.
+__device__ long long g_trace[1 << 18];
+__device__ __forceinline__ long long trace_now()
+{
+    long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#endif
+
 template <int THREADS, int IPT, int JT, int CTAS, bool DENSE, int STAGES>
 __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
+#ifdef GENGA_TRACE
+    const long long tr_start = trace_now();
+    int tr_near = 0, tr_cand = 0, tr_drain = 0;
+#endif
     constexpr int IB = THREADS * IPT;
     constexpr int WARPS = THREADS / 32;
     constexpr int NCH = JT / GENGA_CHUNK;
@@ -402,6 +431,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
     static_assert(GENGA_CHUNK * IPT <= 32, "one trigger bit per pair of a chunk");
     __shared__ TileStage<JT> st[STAGES];
     __shared__ int2 queue[WARPS][GENGA_QCAP];
+    __shared__ int qown[WARPS][32];
     __shared__ __align__(8) uint64_t full[STAGES];
     __shared__ __align__(8) uint64_t empty[STAGES];
 
@@ -449,7 +479,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 
     auto flush = [&]() {
         __syncwarp();
-        if (qtail != qhead) drain_queue<IPT>(p, q, qhead, qtail - qhead, ax, ay, az, cnt);
+        if (qtail != qhead) drain_queue<IPT>(p, q, qown[warp], qhead, qtail - qhead, ax, ay, az, cnt);
         qhead = qtail;
         __syncwarp();
         const size_t base = ((size_t)blockIdx.x * p.max_segs + (cur_ib - first_ib)) * 3 * IB;
@@ -495,6 +525,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 
         const bool mine_near = lane < NG ? boxes_near(wlo, whi, wfw, S.blo[lane], S.bhi[lane]) : false;
         const unsigned nearmask = __ballot_sync(0xffffffffu, mine_near);
+#ifdef GENGA_TRACE
+        tr_near += __popc(nearmask);
+#endif
 
 #pragma unroll 1
         for (int g = 0; g < NG; g++) {
@@ -539,9 +572,13 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                         q[slot & (GENGA_QCAP - 1)] = make_int2(ib * IB + woff + (b % IPT) * 32, jt * JT + jj + b / IPT);
                     }
                     qtail += __popc(m);
+#ifdef GENGA_TRACE
+                    tr_cand += __popc(m);
+                    tr_drain += (qtail - qhead >= 32);
+#endif
                     if (qtail - qhead >= 32) {
                         __syncwarp();
-                        drain_queue<IPT>(p, q, qhead, 32, ax, ay, az, cnt);
+                        drain_queue<IPT>(p, q, qown[warp], qhead, 32, ax, ay, az, cnt);
                         qhead += 32;
                         __syncwarp();
                     }
@@ -553,6 +590,14 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         if (tid == 0 && it >= 1 && it - 1 + STAGES < n_it) issue(it - 1 + STAGES);
     }
     flush();
+#ifdef GENGA_TRACE
+    if (lane == 0) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        long long* o = g_trace + ((size_t)blockIdx.x * WARPS + warp) * 8;
+        o[0] = tr_start; o[1] = trace_now(); o[2] = smid; o[3] = tr_near; o[4] = tr_cand; o[5] = tr_drain;
+    }
+#endif
 }
 
 // ---------------------------------------------------------------------------------------------
