@@ -42,6 +42,11 @@ typedef enum {
 /* bits of the device status word (genga_kick_status) */
 #define GENGA_KICK_STATUS_COINCIDENT 1   /* two distinct bodies at the same position were met
                                             (outside the domain; that pair was skipped)          */
+#define GENGA_KICK_STATUS_CAND_OVERFLOW 2 /* more pairs inside a critical radius than the library's
+                                            candidate list holds (64 per body): the excess pairs
+                                            were dropped, out_acc / out_pairs are incomplete      */
+#define GENGA_KICK_STATUS_FX_RANGE 4     /* a changeover-weighted term outside [7e-43, 4.5e15]
+                                            (or not finite) was met and left out of out_acc       */
 
 typedef struct genga_kick_ctx genga_kick_ctx;   /* opaque; owned by the library */
 

@@ -37,6 +37,12 @@ struct genga_kick_ctx {
     int* counts;
     double* partial;
     int* status;
+    // exact path: candidate list, fixed-point accumulators (genga_kick_kernels.cuh)
+    int2* cand;
+    int64_t cand_capacity;
+    int* ncand;
+    unsigned long long* fx;
+    int* touched;
     int64_t n_rec_alloc;
     // staging for genga_kick_host (device, lazily allocated)
     double* h_pos; double* h_vel; double* h_mass; double* h_rcrit; double* h_acc;
@@ -140,6 +146,13 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
             if ((e = cudaMalloc(&ctx->counts, nc * sizeof(int))) != cudaSuccess) goto cuda_error;
         }
         if ((e = cudaMalloc(&ctx->partial, (size_t)max_partial * sizeof(double))) != cudaSuccess) goto cuda_error;
+        ctx->cand_capacity = std::min<int64_t>(std::max<int64_t>(GENGA_CAND_PER_BODY * N, GENGA_CAND_MIN), GENGA_CAND_MAX);
+        if ((e = cudaMalloc(&ctx->cand, (size_t)ctx->cand_capacity * sizeof(int2))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->ncand, sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->fx, (size_t)nr * 3 * GENGA_FX_LIMBS * sizeof(unsigned long long))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMemset(ctx->fx, 0, (size_t)nr * 3 * GENGA_FX_LIMBS * sizeof(unsigned long long))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->touched, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMemset(ctx->touched, 0, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->status, sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMemset(ctx->status, 0, sizeof(int))) != cudaSuccess) goto cuda_error;
     }
@@ -199,7 +212,7 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
         genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
                                                    ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
                                                    ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw,
-                                                   ctx->cblo, ctx->cbhi, out_npairs);
+                                                   ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
     }
@@ -213,6 +226,8 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
         kp.partial = ctx->partial;
         kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
         kp.status = ctx->status;
+        kp.cand = ctx->cand; kp.cand_capacity = ctx->cand_capacity; kp.ncand = ctx->ncand;
+        kp.fx = ctx->fx; kp.touched = ctx->touched;
         if (ctx->timing) GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level], st));
         GK_CUDA(ctx, dispatch_kick(pl, changeover_level == 0, kp, st));
         if (ctx->timing) {
@@ -220,10 +235,15 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
             ctx->ev_set[changeover_level] = true;
         }
         ctx->launches++;
+        // exact path: one candidate per thread, grid-stride over the list the pair loop has written
+        genga::exact_kernel<<<4 * ctx->num_sms, 256, 0, st>>>(kp);
+        GK_CUDA(ctx, cudaGetLastError());
+        ctx->launches++;
     }
     {
         genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(ctx->partial, ctx->ridx, n_rec, N, pl.i_block, pl.n_j_tiles,
-                                                                  pl.n_tiles, pl.n_ctas, pl.max_segs, dt, out_acc, vel);
+                                                                  pl.n_tiles, pl.n_ctas, pl.max_segs, dt, ctx->fx,
+                                                                  ctx->touched, ctx->status, out_acc, vel);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
     }
@@ -395,7 +415,7 @@ extern "C" int genga_kick_free(genga_kick_ctx* ctx)
 {
     if (!ctx) return GENGA_KICK_OK;
     void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
-                    ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->status, ctx->h_pos,
+                    ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs};
     for (void* b : bufs)
         if (b) cudaFree(b);

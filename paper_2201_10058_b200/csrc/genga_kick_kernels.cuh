@@ -46,6 +46,12 @@ struct KickParams {
     long long capacity;
     int* __restrict__ out_npairs;      // [N + 1]
     int* __restrict__ status;
+    // exact path (candidate list, fixed-point accumulators)
+    int2* __restrict__ cand;           // [cand_capacity] (i-record, j-record)
+    long long cand_capacity;
+    int* __restrict__ ncand;           // candidates appended (may exceed the capacity: status bit)
+    unsigned long long* __restrict__ fx;   // [n_rec][3][GENGA_FX_LIMBS], all zero between calls
+    int* __restrict__ touched;         // [n_rec] != 0: the record's accumulators were added to
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -71,8 +77,10 @@ __global__ void __launch_bounds__(256)
 pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, const double* __restrict__ rcrit,
             const int* __restrict__ perm, int N, int n_massive, int m_pad, int n_rec, int L, double G, double f,
             double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
-            int* __restrict__ cfw, float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs)
+            int* __restrict__ cfw, float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs,
+            int* __restrict__ ncand)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0) *ncand = 0;
     const int stride = gridDim.x * blockDim.x;       // a multiple of 32
     const int top = max(n_rec, ((N + 1 + 31) / 32) * 32);
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < top; r += stride) {
@@ -326,76 +334,172 @@ __device__ __forceinline__ bool boxes_near(float4 alo, float4 ahi, int afw, floa
 }
 
 // ---------------------------------------------------------------------------------------------
-// Exact path, lane-parallel.  Pairs the filter catches are not evaluated where they are found (one
-// lane at a time): the warp appends (i-record, j-record) to its candidate queue in shared memory
-// and, whenever 32 candidates are waiting (and before its accumulators are flushed), DRAINS them:
-// lane e evaluates candidate e with exact_pair -- weight, pre-check, pair emission with one atomic
-// per drain -- and the terms are then handed to the lanes that own the i-bodies in queue order
-// (shuffles), so the summation order is a fixed function of the inputs.
+// Exact path, decoupled from the pair loop.  kick_kernel only APPENDS the pairs the filter catches
+// to a global candidate list (ordered pairs (i-record, j-record); one atomic per warp and push);
+// exact_kernel then evaluates one candidate per thread -- weight, pre-check, pair emission, counts.
+// The candidates cluster where the disk is dense (inner edge: > 100 partners per body against a
+// mean of 15), so evaluating them where they are found serialises a few warps; as a list they
+// spread over the whole device.
+//
+// The candidates' terms G m_j W d / r^3 are added to body i in FIXED POINT: integer addition is
+// associative, so the sum does not depend on the (arbitrary) order of the list and every output
+// bit stays a fixed function of the inputs.  A body's accumulator is, per
+// component, GENGA_FX_LIMBS 64-bit integers; limb l counts units of 2^(GENGA_FX_E0 + 32 l).  A
+// double is cut into three 32-bit pieces on that grid (exactly, unless bits fall below
+// 2^GENGA_FX_E0: those are truncated towards zero) and each piece is added with one 64-bit
+// integer atomic; a limb has room for 2^31 pieces.  reduce_kernel propagates the carries,
+// rounds the 96 leading bits to a double and adds it to the far-field sum.
+// Window: [2^-140, 2^52) = [7e-43, 4.5e15] AU/day^2.
 // ---------------------------------------------------------------------------------------------
-#define GENGA_QCAP 64              // entries per warp queue (a push adds <= 32 to < 32 waiting)
+#define GENGA_FX_LIMBS 6
+#define GENGA_FX_E0 (-140)
+#define GENGA_STATUS_CAND_OVERFLOW 2
+#define GENGA_STATUS_FX_RANGE 4
 
-template <int IPT>
-__device__ __forceinline__ void drain_queue(const KickParams& p, const int2* __restrict__ q, int* __restrict__ own,
-                                            int head, int n,
-                                            double (&ax)[IPT], double (&ay)[IPT], double (&az)[IPT], int (&cnt)[IPT])
+__device__ __forceinline__ void fx_add(unsigned long long* __restrict__ acc, double x, int* status)
+{
+    const long long bits = __double_as_longlong(x);
+    const int ex = (int)((bits >> 52) & 0x7ff);
+    unsigned long long m = (unsigned long long)bits & 0xfffffffffffffULL;
+    if (ex == 0x7ff) { atomicOr(status, GENGA_STATUS_FX_RANGE); return; }      // inf / nan
+    int e = -1074;                                                              // x = +- m 2^e
+    if (ex) { m |= 1ULL << 52; e = ex - 1075; }
+    int pos = e - GENGA_FX_E0;                                                  // grid position of m's lowest bit
+    if (pos < 0) {
+        if (pos <= -53) return;
+        m >>= -pos;
+        pos = 0;
+    }
+    if (m == 0) return;
+    const int l0 = pos >> 5, r = pos & 31;
+    const unsigned long long lo = m << r;
+    const unsigned long long q0 = lo & 0xffffffffULL, q1 = lo >> 32, q2 = r ? (m >> (64 - r)) : 0ULL;
+    const bool neg = bits < 0;
+    if ((q0 && l0 >= GENGA_FX_LIMBS) || (q1 && l0 + 1 >= GENGA_FX_LIMBS) || (q2 && l0 + 2 >= GENGA_FX_LIMBS)) {
+        atomicOr(status, GENGA_STATUS_FX_RANGE);
+        return;
+    }
+    if (q0) atomicAdd(acc + l0, neg ? 0ULL - q0 : q0);
+    if (q1) atomicAdd(acc + l0 + 1, neg ? 0ULL - q1 : q1);
+    if (q2) atomicAdd(acc + l0 + 2, neg ? 0ULL - q2 : q2);
+}
+
+// value of one accumulator; clears it for the next call
+__device__ __forceinline__ double fx_take(unsigned long long* __restrict__ acc, int* status)
+{
+    unsigned w[GENGA_FX_LIMBS];
+    long long carry = 0;
+#pragma unroll
+    for (int l = 0; l < GENGA_FX_LIMBS; l++) {
+        const long long v = (long long)acc[l] + carry;
+        acc[l] = 0ULL;
+        w[l] = (unsigned)((unsigned long long)v & 0xffffffffULL);
+        carry = v >> 32;                                   // arithmetic: the sign travels upwards
+    }
+    if (carry != 0 && carry != -1) atomicOr(status, GENGA_STATUS_FX_RANGE);
+    const bool neg = carry < 0;
+    if (neg) {                                             // two's complement -> magnitude
+        unsigned c = 1u;
+#pragma unroll
+        for (int l = 0; l < GENGA_FX_LIMBS; l++) {
+            const unsigned t = ~w[l];
+            w[l] = t + c;
+            c = (c && t == 0xffffffffu) ? 1u : 0u;
+        }
+    }
+    int h = -1;
+#pragma unroll
+    for (int l = 0; l < GENGA_FX_LIMBS; l++)
+        if (w[l]) h = l;
+    if (h < 0) return 0.0;
+    double v = 0.0;                                        // the three leading limbs
+#pragma unroll
+    for (int l = GENGA_FX_LIMBS - 1; l >= 0; l--)
+        if (l <= h && l >= h - 2) v = __dadd_rn(__dmul_rn(v, 4294967296.0), (double)w[l]);
+    const int lowest = h >= 2 ? h - 2 : 0;
+    v = scalbn(v, GENGA_FX_E0 + 32 * lowest);
+    return neg ? -v : v;
+}
+
+// Append the warp's tripped pairs (i-record, j-record) to the candidate list.  A warp reserves the
+// list GENGA_CAND_BLOCK slots at a time (one atomic per block, not per push: the counter is a
+// single hot address) and fills its block with a private cursor; the slots of a block it does
+// not use are closed with the empty entry (-1, -1), which exact_kernel skips.
+#define GENGA_CAND_BLOCK 128
+
+struct CandCursor {
+    long long base;   // first slot of the warp's open block (warp-uniform)
+    int fill;         // slots used in it; GENGA_CAND_BLOCK: no block open
+};
+
+__device__ __forceinline__ void close_block(const KickParams& p, CandCursor& c)
 {
     const int lane = threadIdx.x & 31;
-    double s = 0.0, dx = 0.0, dy = 0.0, dz = 0.0;
-    int info = -1;                                         // enc << 8 | k << 5 | owner lane; -1: nothing to add
-    bool hit = false;
-    int lo = 0, hi = 0;
-    own[lane] = 0;
-    if (lane < n) {
-        const int2 e = q[(head + lane) & (GENGA_QCAP - 1)];
-        const int ir = e.x, jr = e.y;
-        const int bi = p.ridx[ir], bj = p.ridx[jr];
-        if (ir != jr && bi >= 0 && bj >= 0) {
-            const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
-            dx = __dsub_rn(jxy.x, ixy.x); dy = __dsub_rn(jxy.y, ixy.y); dz = __dsub_rn(jzm.x, izm.x);
-            const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
-            s = r.s;
-            info = (r.enc << 8) | (((ir >> 5) % IPT) << 5) | (ir & 31);
-            if (r.enc) {
-                if (bi >= p.n_massive) {                   // test particle i, massive j
-                    atomicAdd(p.out_npairs + bj, 1);
-                    hit = true; lo = bj; hi = bi;
-                } else if (bi < bj) {
-                    hit = true; lo = bi; hi = bj;
+    for (int q = c.fill + lane; q < GENGA_CAND_BLOCK; q += 32)
+        if (c.base + q < p.cand_capacity) p.cand[c.base + q] = make_int2(-1, -1);
+    c.fill = GENGA_CAND_BLOCK;
+}
+
+__device__ __forceinline__ void push_candidates(const KickParams& p, CandCursor& c, bool mine, int irec, int jrec)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, mine);
+    const int lane = threadIdx.x & 31;
+    const int n = __popc(m);
+    if (c.fill + n > GENGA_CAND_BLOCK) {                    // warp-uniform
+        if (c.fill < GENGA_CAND_BLOCK) close_block(p, c);
+        int base = 0;
+        if (lane == 0) {
+            base = atomicAdd(p.ncand, GENGA_CAND_BLOCK);
+            if ((long long)base + GENGA_CAND_BLOCK > p.cand_capacity) atomicOr(p.status, GENGA_STATUS_CAND_OVERFLOW);
+        }
+        c.base = __shfl_sync(0xffffffffu, base, 0);
+        c.fill = 0;
+    }
+    if (mine) {
+        const long long slot = c.base + c.fill + __popc(m & ((1u << lane) - 1u));
+        if (slot < p.cand_capacity) p.cand[slot] = make_int2(irec, jrec);
+    }
+    c.fill += n;
+}
+
+__global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
+{
+    const long long n = min((long long)*p.ncand, p.cand_capacity);
+    const int lane = threadIdx.x & 31;
+    // whole warps walk the list (the emission votes need every lane)
+    for (long long wbase = ((long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31)); wbase < n;
+         wbase += (long long)gridDim.x * blockDim.x) {
+        const long long c = wbase + lane;
+        bool hit = false;
+        int lo = 0, hi = 0;
+        if (c < n) {
+            const int2 e = p.cand[c];
+            const int ir = e.x, jr = e.y;
+            const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;    // (-1, -1): empty slot
+            if (ir != jr && bi >= 0 && bj >= 0) {
+                const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
+                const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
+                const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
+                if (r.s != 0.0) {
+                    unsigned long long* acc = p.fx + (size_t)ir * (3 * GENGA_FX_LIMBS);
+                    fx_add(acc, __dmul_rn(r.s, dx), p.status);
+                    fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
+                    fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+                    p.touched[ir] = 1;
+                }
+                if (r.enc) {
+                    atomicAdd(p.out_npairs + bi, 1);
+                    if (bi >= p.n_massive) {               // test particle i, massive j
+                        atomicAdd(p.out_npairs + bj, 1);
+                        hit = true; lo = bj; hi = bi;
+                    } else if (bi < bj) {
+                        hit = true; lo = bi; hi = bj;
+                    }
                 }
             }
         }
+        emit_pairs(p, hit, lo, hi);
     }
-    emit_pairs(p, hit, lo, hi);
-    // hand the terms to the lanes that own the i-bodies: own[l] = mask of the entries lane l owns;
-    // every lane then adds its entries in ascending queue order (a fixed order)
-    __syncwarp();
-    const int owner = info >= 0 ? (info & 31) : 32 + lane;   // 32 + lane: a group of its own, unused
-    const unsigned peers = __match_any_sync(0xffffffffu, owner);
-    if (info >= 0 && lane == __ffs(peers) - 1) own[owner] = (int)peers;
-    __syncwarp();
-    unsigned mine = (unsigned)own[lane];
-    while (__any_sync(0xffffffffu, mine != 0)) {
-        const bool have = mine != 0;
-        const int e = have ? __ffs(mine) - 1 : lane;
-        mine &= mine - 1;
-        const int inf = __shfl_sync(0xffffffffu, info, e);
-        const double se = __shfl_sync(0xffffffffu, s, e);
-        const double dxe = __shfl_sync(0xffffffffu, dx, e), dye = __shfl_sync(0xffffffffu, dy, e),
-                     dze = __shfl_sync(0xffffffffu, dz, e);
-        if (have) {
-            const int k = (inf >> 5) & 7;
-#pragma unroll
-            for (int kk = 0; kk < IPT; kk++)
-                if (kk == k) {
-                    ax[kk] = fma(se, dxe, ax[kk]);
-                    ay[kk] = fma(se, dye, ay[kk]);
-                    az[kk] = fma(se, dze, az[kk]);
-                    cnt[kk] += inf >> 8;
-                }
-        }
-    }
-    __syncwarp();
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
@@ -420,7 +524,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
 #ifdef GENGA_TRACE
     const long long tr_start = trace_now();
-    int tr_near = 0, tr_cand = 0, tr_drain = 0;
+    int tr_near = 0, tr_cand = 0;
+    const int tr_drain = 0;
 #endif
     constexpr int IB = THREADS * IPT;
     constexpr int WARPS = THREADS / 32;
@@ -430,8 +535,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
     static_assert(NG <= 32 && JT % GENGA_GROUP == 0, "one lane per group");
     static_assert(GENGA_CHUNK * IPT <= 32, "one trigger bit per pair of a chunk");
     __shared__ TileStage<JT> st[STAGES];
-    __shared__ int2 queue[WARPS][GENGA_QCAP];
-    __shared__ int qown[WARPS][32];
     __shared__ __align__(8) uint64_t full[STAGES];
     __shared__ __align__(8) uint64_t empty[STAGES];
 
@@ -469,19 +572,16 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         for (int g = 0; g < STAGES && g < n_it; g++) issue(g);
 
     double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT];
-    int fi[IPT], bi[IPT], cnt[IPT];
+    int fi[IPT];
     float4 wlo, whi;                                        // box of the warp's i-records
     int wfw = -1;
     const int first_ib = (int)(t0 / p.n_j_tiles);
     int cur_ib = -1;
-    int2* const q = queue[warp];
-    int qhead = 0, qtail = 0;                               // warp-uniform; entries [qhead, qtail) wait
+    CandCursor cc;
+    cc.base = 0;
+    cc.fill = GENGA_CAND_BLOCK;
 
     auto flush = [&]() {
-        __syncwarp();
-        if (qtail != qhead) drain_queue<IPT>(p, q, qown[warp], qhead, qtail - qhead, ax, ay, az, cnt);
-        qhead = qtail;
-        __syncwarp();
         const size_t base = ((size_t)blockIdx.x * p.max_segs + (cur_ib - first_ib)) * 3 * IB;
 #pragma unroll
         for (int k = 0; k < IPT; k++) {
@@ -489,7 +589,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
             p.partial[base + off] = ax[k];
             p.partial[base + IB + off] = ay[k];
             p.partial[base + 2 * IB + off] = az[k];
-            if (cnt[k] > 0 && bi[k] >= 0) atomicAdd(p.out_npairs + bi[k], cnt[k]);
         }
     };
 
@@ -510,9 +609,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                 const double2 a = p.rxy[r], b = p.rzm[r];
                 xi[k] = a.x; yi[k] = a.y; zi[k] = b.x;
                 fi[k] = p.rfw[r];
-                bi[k] = p.ridx[r];
                 ax[k] = ay[k] = az[k] = 0.0;
-                cnt[k] = 0;
                 // the groups of GENGA_GROUP records are aligned with the warp's k-slices
                 const float4 glo = p.cblo[r / GENGA_GROUP], ghi = p.cbhi[r / GENGA_GROUP];
                 wlo.x = fminf(wlo.x, glo.x); wlo.y = fminf(wlo.y, glo.y); wlo.z = fminf(wlo.z, glo.z);
@@ -566,22 +663,10 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                     const int b = __ffs(todo) - 1;
                     todo &= todo - 1;
                     const bool mine = (tm >> b) & 1u;
-                    const unsigned m = __ballot_sync(0xffffffffu, mine);
-                    if (mine) {
-                        const int slot = qtail + __popc(m & ((1u << lane) - 1u));
-                        q[slot & (GENGA_QCAP - 1)] = make_int2(ib * IB + woff + (b % IPT) * 32, jt * JT + jj + b / IPT);
-                    }
-                    qtail += __popc(m);
+                    push_candidates(p, cc, mine, ib * IB + woff + (b % IPT) * 32, jt * JT + jj + b / IPT);
 #ifdef GENGA_TRACE
-                    tr_cand += __popc(m);
-                    tr_drain += (qtail - qhead >= 32);
+                    tr_cand += __popc(__ballot_sync(0xffffffffu, mine));
 #endif
-                    if (qtail - qhead >= 32) {
-                        __syncwarp();
-                        drain_queue<IPT>(p, q, qown[warp], qhead, 32, ax, ay, az, cnt);
-                        qhead += 32;
-                        __syncwarp();
-                    }
                 }
             }
         }
@@ -590,6 +675,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         if (tid == 0 && it >= 1 && it - 1 + STAGES < n_it) issue(it - 1 + STAGES);
     }
     flush();
+    if (cc.fill < GENGA_CAND_BLOCK) close_block(p, cc);
 #ifdef GENGA_TRACE
     if (lane == 0) {
         unsigned smid;
@@ -607,6 +693,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 __global__ void __launch_bounds__(256)
 reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, int n_rec, int N, int IB,
               int n_j_tiles, long long n_tiles, int n_ctas, int max_segs, double dt,
+              unsigned long long* __restrict__ fx, int* __restrict__ touched, int* __restrict__ status,
               double* __restrict__ out_acc, double* __restrict__ vel)
 {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
@@ -624,6 +711,13 @@ reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, 
         a0 = __dadd_rn(a0, q[0]);
         a1 = __dadd_rn(a1, q[IB]);
         a2 = __dadd_rn(a2, q[2 * (size_t)IB]);
+    }
+    if (touched[r]) {                                      // the exact path's terms (fixed point, see fx_add)
+        touched[r] = 0;
+        unsigned long long* acc = fx + (size_t)r * (3 * GENGA_FX_LIMBS);
+        a0 = __dadd_rn(a0, fx_take(acc, status));
+        a1 = __dadd_rn(a1, fx_take(acc + GENGA_FX_LIMBS, status));
+        a2 = __dadd_rn(a2, fx_take(acc + 2 * GENGA_FX_LIMBS, status));
     }
     if (out_acc) {
         out_acc[b] = a0;

@@ -47,4 +47,9 @@ static const int GENGA_STAGES = 4;          // depth of the j-tile ring in share
 static const int GENGA_M_ALIGN = 256;      // every j_tile divides it
 static const int GENGA_SORT_MIN_BODIES = 4096;   // GENGA_KICK_ORDER_AUTO sorts from here on
 static const int GENGA_REC_ALIGN = 1024;   // every i_block divides it
+// capacity of the candidate list of the exact path: pairs (ordered) inside the largest critical
+// radius of either body; the mean is ~16 per body at N = 65,536
+static const int64_t GENGA_CAND_PER_BODY = 64;
+static const int64_t GENGA_CAND_MIN = (int64_t)1 << 20;
+static const int64_t GENGA_CAND_MAX = (int64_t)1 << 28;
 static const int64_t GENGA_MAX_BODIES = (int64_t)1 << 30;
