@@ -191,7 +191,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         torch.cuda.synchronize()
 
     # FP64 ALU roofline of this device, measured before the timed region
-    dfma_rate = kick.measure_dfma_rate(iters=8192, reps=5)
+    # (pattern 0: loop-invariant operands; 1: three distinct register operands, the shape of the
+    # accumulation a += s d; 2: two distinct register operands -- include/genga_kick.h)
+    fp64_rate = [kick.measure_fp64_rate(pattern, iters=4096, reps=5) for pattern in (0, 1, 2)]
+    dfma_rate = max(fp64_rate)
     for _ in range(args.warmup):
         step()
         flush.fill_(1)
@@ -301,6 +304,13 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                          "peak_source": f"nominal: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes "
                                         f"x 2 x {sm_max_mhz} MHz (no FP64 figure in MEASURED_PEAKS.json)",
                          "peak_measured_dfma": peak_dfma, "frac_of_measured_dfma": achieved / peak_dfma,
+                         "dfma_per_s_by_operand_pattern": {"invariant_operands": fp64_rate[0],
+                                                           "three_distinct_registers": fp64_rate[1],
+                                                           "two_distinct_registers": fp64_rate[2]},
+                         # ceiling of THIS instruction mix: 13 FP64 instructions with <= 2 distinct register
+                         # operands + 3 accumulating DFMAs with 3, each at its measured rate
+                         "mix_ceiling": FLOPS_PER_PAIR / (13.0 / fp64_rate[2] + 3.0 / fp64_rate[1]) / 1e12,
+                         "frac_of_mix_ceiling": achieved / (FLOPS_PER_PAIR / (13.0 / fp64_rate[2] + 3.0 / fp64_rate[1]) / 1e12),
                          "flops_per_pair": FLOPS_PER_PAIR, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR,
                          "fp64_pipe_issue_frac": FP64_INSTR_PER_PAIR * pairs_per_kick / (k0_ms * 1e-3) /
                                                  (props.multi_processor_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),

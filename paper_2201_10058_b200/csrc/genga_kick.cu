@@ -347,17 +347,29 @@ extern "C" int genga_kick_last_pair_loop_ms(genga_kick_ctx* ctx, int32_t changeo
 namespace genga {
 // Independent DFMA chains: the plain FP64 ALU roofline (include/genga_kick.h).  The operands come
 // from memory so that nothing folds; the result is stored so that nothing is dropped.
-__global__ void __launch_bounds__(1024, 2) dfma_rate_kernel(const double* __restrict__ in, double* __restrict__ out, int iters)
+//   PATTERN 0: a = fma(a, m, c), m and c loop-invariant registers (operand reuse possible)
+//   PATTERN 1: a_k = fma(a_k, b_k, c_k): three distinct register operands, no reuse
+//   PATTERN 2: a_k = fma(a_k, b_k, imm): two distinct register operands
+template <int PATTERN>
+__global__ void __launch_bounds__(256, 2) fp64_rate_kernel(const double* __restrict__ in, double* __restrict__ out, int iters)
 {
     const double m = in[0], c = in[1];
-    double a[8];
+    double a[8], b[8], d[8];
 #pragma unroll
-    for (int k = 0; k < 8; k++) a[k] = in[2] * (double)(threadIdx.x + k);
+    for (int k = 0; k < 8; k++) {
+        a[k] = in[2] * (double)(threadIdx.x + k);
+        b[k] = m - 1.0e-9 * (double)k;
+        d[k] = c + 1.0e-9 * (double)k;
+    }
     for (int it = 0; it < iters; it++) {
 #pragma unroll
         for (int u = 0; u < 8; u++) {
 #pragma unroll
-            for (int k = 0; k < 8; k++) a[k] = fma(a[k], m, c);
+            for (int k = 0; k < 8; k++) {
+                if (PATTERN == 0) a[k] = fma(a[k], m, c);
+                if (PATTERN == 1) a[k] = fma(a[k], b[k], d[k]);
+                if (PATTERN == 2) a[k] = fma(a[k], b[k], 1.0e-6);
+            }
         }
     }
     double s = 0.0;
@@ -367,11 +379,12 @@ __global__ void __launch_bounds__(1024, 2) dfma_rate_kernel(const double* __rest
 }
 }  // namespace genga
 
-extern "C" int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, int32_t reps, double* dfma_per_s)
+extern "C" int genga_kick_measure_fp64_rate(genga_kick_ctx* ctx, int32_t pattern, int32_t iters, int32_t reps,
+                                            double* dfma_per_s)
 {
     if (!ctx || !dfma_per_s) return GENGA_KICK_E_NULL;
-    if (iters < 1 || reps < 1) return GENGA_KICK_E_SIZE;
-    const int blocks = 2 * ctx->num_sms, threads = 1024;
+    if (iters < 1 || reps < 1 || pattern < 0 || pattern > 2) return GENGA_KICK_E_SIZE;
+    const int blocks = 8 * ctx->num_sms, threads = 256;
     double* buf = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     cudaStream_t st = ctx->stream;
@@ -384,7 +397,9 @@ extern "C" int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, 
     if ((e = cudaEventCreate(&e1)) != cudaSuccess) goto done;
     for (int r = 0; r <= reps; r++) {                              // launch 0 is the warm-up
         if ((e = cudaEventRecord(e0, st)) != cudaSuccess) goto done;
-        genga::dfma_rate_kernel<<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
+        if (pattern == 0) genga::fp64_rate_kernel<0><<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
+        if (pattern == 1) genga::fp64_rate_kernel<1><<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
+        if (pattern == 2) genga::fp64_rate_kernel<2><<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
         if ((e = cudaGetLastError()) != cudaSuccess) goto done;
         if ((e = cudaEventRecord(e1, st)) != cudaSuccess) goto done;
         if ((e = cudaEventSynchronize(e1)) != cudaSuccess) goto done;
@@ -400,6 +415,11 @@ done:
     if (buf) cudaFree(buf);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, int32_t reps, double* dfma_per_s)
+{
+    return genga_kick_measure_fp64_rate(ctx, 0, iters, reps, dfma_per_s);
 }
 
 #ifdef GENGA_TRACE

@@ -1,0 +1,100 @@
+"""-m gpu: BASELINE.json's configs at their FULL sizes, in the launch configuration bench.py times
+(internal order AUTO, pair capacity 2^20), against the CPU oracle under north_star's rule.
+
+The oracle is a direct sum, so it finishes every full config on the GPU box's host cores in
+seconds (N = 65,536: 4.3e9 pair evaluations per level): the comparison is element by element over
+ALL bodies, not a sample.  Config 1 runs its 100 kicks with the harness drift between them."""
+import numpy as np
+import pytest
+
+import genga_inputs as gi
+from tests.gpu_harness import run_gpu, compare
+from tests import harness_integrator as hi
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-13
+CAPACITY = 1 << 20
+
+
+def _full(ki, oracle_mod, level):
+    gpu = run_gpu(ki, level=level, capacity=CAPACITY, order_mode=0)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=level, G=ki.G,
+                          enc_factor=ki.enc_factor, maxp=256)
+    assert not orc.coincident and gpu.status == 0
+    d = compare(gpu, orc, ki.n_massive, tol=TOL)
+    assert gpu.total == len(gpu.pairs) <= CAPACITY
+    # momentum (pin P3 on the GPU result): sum over the massive bodies, which only feel each other
+    m = ki.mass[:ki.n_massive]
+    p = (m * gpu.acc[:, :ki.n_massive]).sum(axis=1)
+    scale = (m * orc.S[:, :ki.n_massive]).sum(axis=1)
+    assert np.all(np.abs(p) <= TOL * scale)
+    return gpu, orc, d
+
+
+@pytest.mark.parametrize("level", [0, 1])
+def test_config3_full(oracle_mod, level):
+    """N = 65,536, the headline config; the paper's section 2.1 regime: O(10) partners per body."""
+    ki = gi.make_config(3)
+    assert ki.n == 65536
+    gpu, orc, d = _full(ki, oracle_mod, level)
+    if level == 0:
+        assert 10.0 < gpu.counts.mean() < 25.0
+        assert int(gpu.counts.sum()) == 2 * gpu.total
+
+
+@pytest.mark.parametrize("level", [0, 1])
+def test_config2_full(oracle_mod, level):
+    """32,768 planetesimals + Jupiter + Saturn, higher-level changeover."""
+    ki = gi.make_config(2)
+    assert ki.n == 32770
+    gpu, orc, d = _full(ki, oracle_mod, level)
+    assert gpu.total > 1000
+
+
+def test_config4_full(oracle_mod):
+    """2048 massive + 1,048,576 semi-active test particles (rectangular kick)."""
+    ki = gi.make_config(4)
+    assert ki.n_massive == 2048 and ki.n_test == 1 << 20
+    gpu, orc, d = _full(ki, oracle_mod, 0)
+    pr = gpu.pairs
+    assert (pr[:, 0] < ki.n_massive).all()                # no tp-tp pairs
+    assert (pr[:, 1] >= ki.n_massive).sum() > 1000        # tp-massive pairs exist
+    # a massive body counts its test-particle partners (reading G11)
+    want = np.bincount(pr.ravel(), minlength=ki.n)
+    assert np.array_equal(want, gpu.counts)
+
+
+def test_config1_hundred_kicks(oracle_mod):
+    """N = 8192, 100 kicks separated by an oracle-matched heliocentric drift: both sides see the
+    same state at every step (the harness advances it with the ORACLE's acceleration), the
+    encounter list evolves, momentum is checked at every step."""
+    ki = gi.make_config(1)
+    assert ki.n == 8192
+    from paper_2201_10058_b200 import GengaKick
+    n, dt = ki.n, ki.dt
+    kick = GengaKick(n, 0, max_level=0, pair_capacity=CAPACITY, G=ki.G, enc_factor=ki.enc_factor)
+    q, v, mass = ki.pos.copy(), ki.vel.copy(), ki.mass
+    seen = set()
+    totals = []
+    for step in range(100):
+        a_sma = gi.semi_major_axis(q, v, ki.G)
+        ki.pos, ki.vel = np.ascontiguousarray(q), np.ascontiguousarray(v)
+        ki.rcrit = gi.rcrit_rows(a_sma, v, mass, dt, 2, 1)
+        gpu = run_gpu(ki, level=0, capacity=CAPACITY, kick=kick)
+        orc = oracle_mod.kick(q, mass, ki.rcrit, n, 0, level=0, G=ki.G, enc_factor=ki.enc_factor, maxp=64)
+        assert gpu.status == 0
+        compare(gpu, orc, n, tol=TOL)
+        for acc in (gpu.acc, orc.acc):
+            p = (mass * acc).sum(axis=1)
+            assert np.all(np.abs(p) <= TOL * (mass * orc.S).sum(axis=1)), f"momentum at step {step}"
+        totals.append(gpu.total)
+        seen.add(frozenset(map(tuple, gpu.pairs.tolist())))
+        # between kicks: v += dt a_oracle, then the heliocentric drift
+        # HC(dt/2) FG(dt) HC(dt/2) of App. A
+        v = v + dt * orc.acc
+        q = hi.sun_drift(q, v, mass, 1.0, 0.5 * dt)
+        q, v = hi.kepler_drift(q, v, ki.G * 1.0, dt)
+        q = hi.sun_drift(q, v, mass, 1.0, 0.5 * dt)
+    kick.free()
+    assert len(seen) > 50, "the encounter list did not evolve"
+    assert min(totals) > 1000
