@@ -66,19 +66,19 @@ int cuda_fail(genga_kick_ctx* ctx, cudaError_t e)
 
 bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
-template <int THREADS, int IPT, int JT, int CTAS, bool DENSE>
+template <int THREADS, int IPT, int JT, int CTAS>
 cudaError_t launch_kick(const genga::KickParams& kp, cudaStream_t st)
 {
-    genga::kick_kernel<THREADS, IPT, JT, CTAS, DENSE, GENGA_STAGES><<<kp.n_ctas, THREADS, 0, st>>>(kp);
+    genga::kick_kernel<THREADS, IPT, JT, CTAS, GENGA_STAGES><<<kp.n_ctas, THREADS, 0, st>>>(kp);
     return cudaGetLastError();
 }
 
-// the compiled shapes: must list every entry of GENGA_DENSE_VARIANTS / GENGA_SPARSE_VARIANTS
-cudaError_t dispatch_kick(const genga_kick_plan& pl, bool dense, const genga::KickParams& kp, cudaStream_t st)
+// the compiled shapes: must list every entry of GENGA_VARIANTS
+cudaError_t dispatch_kick(const genga_kick_plan& pl, const genga::KickParams& kp, cudaStream_t st)
 {
 #define GK_SHAPE(T, I, J, C)                                                          \
     if (pl.threads == T && pl.i_per_thread == I && pl.j_tile == J)                    \
-        return dense ? launch_kick<T, I, J, C, true>(kp, st) : launch_kick<T, I, J, C, false>(kp, st);
+        return launch_kick<T, I, J, C>(kp, st);
     GK_SHAPE(256, 2, 256, 2)
     GK_SHAPE(128, 2, 128, 4)
     GK_SHAPE(128, 1, 64, 4)
@@ -229,7 +229,14 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
         kp.cand = ctx->cand; kp.cand_capacity = ctx->cand_capacity; kp.ncand = ctx->ncand;
         kp.fx = ctx->fx; kp.touched = ctx->touched;
         if (ctx->timing) GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level], st));
-        GK_CUDA(ctx, dispatch_kick(pl, changeover_level == 0, kp, st));
+        if (changeover_level == 0) {
+            GK_CUDA(ctx, dispatch_kick(pl, kp, st));
+        } else {
+            // W_L = 0 exactly outside the filter radius: a neighbour search, no tile decomposition
+            const int n_igroups = n_rec / GENGA_GROUP, wpc = GENGA_NEAR_THREADS / 32;
+            genga::near_kernel<<<(n_igroups + wpc - 1) / wpc, GENGA_NEAR_THREADS, 0, st>>>(kp, n_rec, pl.m_pad / GENGA_GROUP);
+            GK_CUDA(ctx, cudaGetLastError());
+        }
         if (ctx->timing) {
             GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level + 1], st));
             ctx->ev_set[changeover_level] = true;
@@ -241,8 +248,10 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
         ctx->launches++;
     }
     {
+        // level >= 1: no partial segments (n_ctas = 0), every term comes from the exact path
         genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(ctx->partial, ctx->ridx, n_rec, N, pl.i_block, pl.n_j_tiles,
-                                                                  pl.n_tiles, pl.n_ctas, pl.max_segs, dt, ctx->fx,
+                                                                  pl.n_tiles, changeover_level == 0 ? pl.n_ctas : 0,
+                                                                  pl.max_segs, dt, ctx->fx,
                                                                   ctx->touched, ctx->status, out_acc, vel);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;

@@ -241,13 +241,13 @@ __device__ __forceinline__ double rsqrt_seed_unless(double x, bool skip)
 // The pair loop's arithmetic for one (i, j) -- ROW a2-a4 of SURVEY.md section 8(a).
 //   d = x_j - x_i, r2 = d.d                         3 DADD, 1 DMUL, 2 DFMA
 //   trig = hi(r2) < thr  (integer pipe)             the pair goes to the exact path instead
-//   DENSE (level 0, W = K = 1 for every pair that passes the filter):
+//   level 0 (W = K = 1 for every pair that passes the filter):
 //     y0 = MUFU.RSQ64H(r2) ~ r^-1 (1 + O(2^-20));  e = 1 - r2 y0^2
 //     G m_j r^-3 = y0^2 (G m_j y0) (1 + e (3/2 + 15/8 e))  + O(e^3)      4 DMUL, 3 DFMA
 //     a += s d                                       3 DFMA
 //   16 FP64-pipe instructions, 24 flops.  Every DFMA but the three accumulations has at most two
 //   distinct register operands (a third costs a register-file cycle on this part).
-//   SPARSE (level >= 1): a pair that passes the filter has W_L = 0 exactly; nothing is added.
+//   (level >= 1: a pair that passes the filter has W_L = 0 exactly -- near_kernel, no arithmetic.)
 // ---------------------------------------------------------------------------------------------
 // The same arithmetic without the filter, for groups the box test has cleared.
 __device__ __forceinline__ void pair_bare(double xj, double yj, double zj, double gmj,
@@ -269,7 +269,6 @@ __device__ __forceinline__ void pair_bare(double xj, double yj, double zj, doubl
     az = fma(s, dz, az);
 }
 
-template <bool DENSE>
 __device__ __forceinline__ void pair_fast(double xj, double yj, double zj, double gmj,
                                           double xi, double yi, double zi, int thr,
                                           double& ax, double& ay, double& az, bool& any)
@@ -278,19 +277,17 @@ __device__ __forceinline__ void pair_fast(double xj, double yj, double zj, doubl
     const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
     const bool trig = __double2hiint(r2) < thr;
     any |= trig;
-    if (DENSE) {
-        const double y0 = rsqrt_seed_unless(r2, trig);
-        const double t = __dmul_rn(y0, y0);
-        const double e = fma(-r2, t, 1.0);
-        const double g = __dmul_rn(gmj, y0);
-        const double u = __dmul_rn(t, g);
-        const double c = fma(1.875, e, 1.5);
-        const double q = fma(e, c, 1.0);
-        const double s = __dmul_rn(u, q);
-        ax = fma(s, dx, ax);
-        ay = fma(s, dy, ay);
-        az = fma(s, dz, az);
-    }
+    const double y0 = rsqrt_seed_unless(r2, trig);
+    const double t = __dmul_rn(y0, y0);
+    const double e = fma(-r2, t, 1.0);
+    const double g = __dmul_rn(gmj, y0);
+    const double u = __dmul_rn(t, g);
+    const double c = fma(1.875, e, 1.5);
+    const double q = fma(e, c, 1.0);
+    const double s = __dmul_rn(u, q);
+    ax = fma(s, dx, ax);
+    ay = fma(s, dy, ay);
+    az = fma(s, dz, az);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -302,11 +299,9 @@ __device__ __forceinline__ void pair_fast(double xj, double yj, double zj, doubl
 //
 // Culling: per tile, lane g tests the box of the warp's i-records against the box of j-group g
 // (GENGA_GROUP records).  If the boxes are further apart than the largest filter radius of either
-// side, no pair of the (warp, group) combination can trip the filter, and the group runs
-//   DENSE : the bare pair loop (no compare, no vote) -- same arithmetic, same order, same bits as
-//           the checked loop would give;
-//   SPARSE: not at all (every W_L is exactly 0, nothing is an encounter).
-// Otherwise the group runs the checked loop: per chunk of GENGA_CHUNK j-records one warp vote
+// side, no pair of the (warp, group) combination can trip the filter, and the group runs the bare
+// pair loop (no compare, no vote) -- same arithmetic, same order, same bits as the checked loop
+// would give.  Otherwise the group runs the checked loop: per chunk of GENGA_CHUNK j-records one warp vote
 // decides whether any pair of the chunk needs the exact path.
 // ---------------------------------------------------------------------------------------------
 template <int JT>
@@ -519,7 +514,7 @@ __device__ __forceinline__ long long trace_now()
 }
 #endif
 
-template <int THREADS, int IPT, int JT, int CTAS, bool DENSE, int STAGES>
+template <int THREADS, int IPT, int JT, int CTAS, int STAGES>
 __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
 #ifdef GENGA_TRACE
@@ -630,14 +625,12 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         for (int g = 0; g < NG; g++) {
             const int j0 = g * GENGA_GROUP;
             if (!((nearmask >> g) & 1u)) {
-                if (DENSE) {
 #pragma unroll 4
-                    for (int u = 0; u < GENGA_GROUP; u++) {
-                        const double2 xy = S.xy[j0 + u], zm = S.zm[j0 + u];
+                for (int u = 0; u < GENGA_GROUP; u++) {
+                    const double2 xy = S.xy[j0 + u], zm = S.zm[j0 + u];
 #pragma unroll
-                        for (int k = 0; k < IPT; k++)
-                            pair_bare(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], ax[k], ay[k], az[k]);
-                    }
+                    for (int k = 0; k < IPT; k++)
+                        pair_bare(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], ax[k], ay[k], az[k]);
                 }
                 continue;
             }
@@ -654,7 +647,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 #pragma unroll
                     for (int k = 0; k < IPT; k++) {
                         bool trig = false;
-                        pair_fast<DENSE>(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], trig);
+                        pair_fast(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], trig);
                         tm |= (trig ? 1u : 0u) << (u * IPT + k);
                     }
                 }
@@ -684,6 +677,78 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         o[0] = tr_start; o[1] = trace_now(); o[2] = smid; o[3] = tr_near; o[4] = tr_cand; o[5] = tr_drain;
     }
 #endif
+}
+
+// ---------------------------------------------------------------------------------------------
+// near_kernel: the pair loop of changeover levels L >= 1.  The factor 1 - K_0 of eq. 63
+// vanishes for r >= rc0_ij, so every pair that passes the filter has W_L = 0
+// EXACTLY and is no encounter pair: the level-L kick is a neighbour search.  A warp owns one group
+// of GENGA_GROUP i-records (one per lane) and tests its box against the box of every j-group
+// (staged through shared memory GENGA_NEAR_BOXES at a time, one box per lane and vote); only for
+// the few near groups it forms r^2 for its 32 x 32 pairs and appends the pairs that trip the
+// filter to the candidate list.  No accelerations are accumulated here: all of them come from
+// exact_kernel's fixed-point sums (reduce_kernel is told there are no partial segments).
+// ---------------------------------------------------------------------------------------------
+#define GENGA_NEAR_THREADS 128
+#define GENGA_NEAR_BOXES 256
+
+__global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickParams p, int n_rec, int n_jgroups)
+{
+    __shared__ float4 blo[GENGA_NEAR_BOXES];
+    __shared__ float4 bhi[GENGA_NEAR_BOXES];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ig = blockIdx.x * (GENGA_NEAR_THREADS / 32) + warp;
+    const int r = ig * GENGA_GROUP + lane;
+    double xi = GENGA_SENTINEL_POS, yi = GENGA_SENTINEL_POS, zi = GENGA_SENTINEL_POS;
+    int fi = -1, wfw = -1;
+    float4 wlo = make_float4(3.0e38f, 3.0e38f, 3.0e38f, 0.0f), whi = make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
+    if (r < n_rec) {
+        const double2 a = p.rxy[r], b = p.rzm[r];
+        xi = a.x; yi = a.y; zi = b.x;
+        fi = p.rfw[r];
+        wlo = p.cblo[ig]; whi = p.cbhi[ig];
+        wfw = __float_as_int(wlo.w);
+    }
+    const bool active = wfw >= 0;                           // the group holds at least one real body
+    CandCursor cc;
+    cc.base = 0;
+    cc.fill = GENGA_CAND_BLOCK;
+
+    for (int g0 = 0; g0 < n_jgroups; g0 += GENGA_NEAR_BOXES) {
+        __syncthreads();
+        for (int q = tid; q < GENGA_NEAR_BOXES; q += GENGA_NEAR_THREADS) {
+            const int g = g0 + q;
+            blo[q] = g < n_jgroups ? p.cblo[g] : make_float4(3.0e38f, 3.0e38f, 3.0e38f, __int_as_float(-1));
+            bhi[q] = g < n_jgroups ? p.cbhi[g] : make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
+        }
+        __syncthreads();
+        if (!active) continue;
+#pragma unroll 1
+        for (int q0 = 0; q0 < GENGA_NEAR_BOXES; q0 += 32) {
+            unsigned nearmask = __ballot_sync(0xffffffffu, boxes_near(wlo, whi, wfw, blo[q0 + lane], bhi[q0 + lane]));
+            while (nearmask) {
+                const int j0 = (g0 + q0 + __ffs(nearmask) - 1) * GENGA_GROUP;
+                nearmask &= nearmask - 1;
+                const int fj_lane = p.rfw[j0 + lane];
+                unsigned tm = 0;                            // bit u: pair (r, j0 + u) tripped the filter
+#pragma unroll 8
+                for (int u = 0; u < GENGA_GROUP; u++) {
+                    const double2 xy = __ldg(p.rxy + j0 + u), zm = __ldg(p.rzm + j0 + u);   // same address in every lane
+                    const int thr = max(fi, __shfl_sync(0xffffffffu, fj_lane, u));
+                    const double dx = __dsub_rn(xy.x, xi), dy = __dsub_rn(xy.y, yi), dz = __dsub_rn(zm.x, zi);
+                    const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
+                    tm |= (__double2hiint(r2) < thr ? 1u : 0u) << u;
+                }
+                unsigned todo = __reduce_or_sync(0xffffffffu, tm);
+                while (todo) {                              // warp-uniform: the j-records some lane tripped on
+                    const int b = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    push_candidates(p, cc, (tm >> b) & 1u, r, j0 + b);
+                }
+            }
+        }
+    }
+    if (cc.fill < GENGA_CAND_BLOCK) close_block(p, cc);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -24,7 +24,7 @@ extern "C" int genga_kick_make_plan(int32_t n_massive, int32_t n_test, int32_t l
     const int64_t N = (int64_t)n_massive + (int64_t)n_test;
     if (n_massive < 0 || n_test < 0 || N <= 0 || N > GENGA_MAX_BODIES || num_sms <= 0) return GENGA_KICK_E_SIZE;
 
-    const genga_variant* vars = level == 0 ? GENGA_DENSE_VARIANTS : GENGA_SPARSE_VARIANTS;
+    const genga_variant* vars = GENGA_VARIANTS;     // level >= 1 only uses m_pad and n_rec of the plan
     genga_kick_plan p;
     for (int v = 0; v < GENGA_N_VARIANTS; v++) {
         p.threads = vars[v].threads;

@@ -2,11 +2,10 @@
 // and the launcher (genga_kick.cu).  A variant fixes threads per CTA, i-bodies per thread, the
 // j-tile length and the CTAs per SM the kernel is bounded for (__launch_bounds__).
 //
-// Two families:
-//   dense  (changeover_level == 0): every pair contributes; ~16 FP64-pipe instructions per pair.
-//   sparse (changeover_level >= 1): W_L = 0 exactly for r >= rc0_ij (factor 1 - K_0 of eq. 63,
-//          PAPER.md:627-632), so a far pair costs r^2 + an integer compare; more i-bodies per
-//          thread to amortise the shared-memory loads.
+// The variants are the shapes of the level-0 pair loop (every pair contributes; 16 FP64-pipe
+// instructions per pair).  changeover_level >= 1 does not use them: there W_L = 0 exactly for
+// r >= rc0_ij (factor 1 - K_0 of eq. 63) and the kick is a neighbour search
+// (near_kernel).
 #pragma once
 #include <stdint.h>
 
@@ -32,12 +31,7 @@ static const int GENGA_N_VARIANTS = 3;
 
 // ordered from the large-N shape to the small-N shape; the planner takes the first one that
 // gives every CTA at least GENGA_MIN_TILES_PER_CTA tiles, else the last
-static const genga_variant GENGA_DENSE_VARIANTS[GENGA_N_VARIANTS] = {
-    {256, 2, 256, 2},
-    {128, 2, 128, 4},
-    {128, 1, 64, 4},
-};
-static const genga_variant GENGA_SPARSE_VARIANTS[GENGA_N_VARIANTS] = {
+static const genga_variant GENGA_VARIANTS[GENGA_N_VARIANTS] = {
     {256, 2, 256, 2},
     {128, 2, 128, 4},
     {128, 1, 64, 4},
