@@ -1,9 +1,12 @@
 """CPU oracle of the GENGA kick + encounter pre-check.  TEST INFRASTRUCTURE ONLY.
 
 Importable only from tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference legs.
-The arithmetic lives in genga_kick_oracle.c (plain C, binary64 per pair, long double sums); this
+The arithmetic lives in genga_kick_oracle.c (plain C, binary64 per pair, long double sums) and
+genga_step_oracle.c (Rcrit / HC / FG, long double); this
 module is argument marshalling via ctypes.  It imports nothing from the CUDA package.
 """
 from .oracle import (OracleResult, K_of_y, K, weight, weight_bs, kick, pair_set, num_threads, lib_path)
 
-__all__ = ["OracleResult", "K_of_y", "K", "weight", "weight_bs", "kick", "pair_set", "num_threads", "lib_path"]
+from . import step
+
+__all__ = ["step", "OracleResult", "K_of_y", "K", "weight", "weight_bs", "kick", "pair_set", "num_threads", "lib_path"]

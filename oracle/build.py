@@ -1,17 +1,17 @@
-"""Builds oracle/libgenga_oracle.so from the plain-C oracle (test infrastructure; gcc only)."""
+"""Builds oracle/libgenga_oracle.so from the plain-C oracles (kick + pre-check; Rcrit / HC / FG) (test infrastructure; gcc only)."""
 import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "genga_kick_oracle.c")
+SRCS = [os.path.join(HERE, "genga_kick_oracle.c"), os.path.join(HERE, "genga_step_oracle.c")]
 LIB = os.path.join(HERE, "libgenga_oracle.so")
 # -ffp-contract=off: every product and sum rounds separately, as the header promises.
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall"]
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
-        subprocess.check_call(["gcc", *CFLAGS, SRC, "-o", LIB, "-lm"])
+    if force or not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(s) for s in SRCS):
+        subprocess.check_call(["gcc", *CFLAGS, *SRCS, "-o", LIB, "-lm"])
     return LIB
 
 

@@ -1,0 +1,134 @@
+/*
+ * CPU ORACLE for the O(N) neighbours of the kick in GENGA's hybrid symplectic step
+ * (Rcrit, HC, FG).            *** TEST INFRASTRUCTURE ONLY ***
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * call this file.  It shares no code, header, table or helper with the CUDA path in
+ * paper_2201_10058_b200/csrc/ and neither includes the other.
+ *
+ * What it computes (each is the plain definition, evaluated in long double and rounded once):
+ *
+ *   Rcrit  r_crit,i^(k) = max(n1 R_H,i , n2 (dt / s^k) v_i),  k = 0..nrows-1      eq. 5 PAPER.md:72-76;
+ *          "the critical radius is defined in the same way on each level ... with the reduced
+ *          time step" PAPER.md:638.  R_H,i = a_i (m_i / (3 m_star))^(1/3) with a_i the osculating
+ *          semi-major axis from the vis-viva equation, v_i = |v_i|               (reading G6)
+ *   HC     q_i += dt * (sum_j m_j v_j) / m_star            eq. 4 PAPER.md:68 (H_C = (sum p)^2 / 2 m_star,
+ *          dq_i/dt = dH_C/dp_i), "the democratic momentum summation" App. A
+ *   FG     every body advances by dt on its two-body orbit about the central mass with
+ *          mu = G m_star (the Kepler part p^2/2m - G m m_star / r of eq. 2; the
+ *          pair term [1 - K] of eq. 2 belongs to the Bulirsch-Stoer phase, off this path).
+ *          The exact solution is written with Gauss' f and g functions in the difference dE of
+ *          the eccentric anomaly ("FG", App. A).  Bound orbits only (a > 0);
+ *          others are left untouched and reported                                 (reading G13)
+ *   step   Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt); HC(dt/2); Kick(dt/2)
+ *          App. A PAPER.md:986-992 without the Bulirsch-Stoer branch -- composed in Python
+ *          (oracle/step.py) from these functions and genga_oracle_kick.
+ *
+ * PINS (tests/test_step_oracle_pins.py, `-m "not gpu"`): n1 = 3, n2 = 0.4 and the closed form of
+ * eq. 5 on a circular orbit; HC on a hand-computed 3-body example and conservation of sum p; FG
+ * against the closed-form rotation of a circular orbit, against the input generator's
+ * elements -> Cartesian map at M0 + n dt (an independent Kepler solver), conservation of energy,
+ * angular momentum and eccentricity vector, a full period, and dt followed by -dt; the whole step:
+ * dt^2 scaling of the energy error of a 3-body system (P8 with the oracle's own HC and FG).
+ */
+#include <math.h>
+#include <stdint.h>
+
+/* eq. 5, rows k = 0..nrows-1 at dt / substeps^k.  out [nrows][N].  Returns the number of bodies
+ * with a non-positive semi-major axis (their Hill term is taken as 0). */
+int64_t genga_oracle_rcrit(int64_t N, const double *pos, const double *vel, const double *mass,
+                           double m_star, double G, double dt, double substeps, int32_t nrows,
+                           double n1, double n2, double *out)
+{
+    int64_t unbound = 0;
+    for (int64_t i = 0; i < N; i++) {
+        const long double x = pos[i], y = pos[N + i], z = pos[2 * N + i];
+        const long double vx = vel[i], vy = vel[N + i], vz = vel[2 * N + i];
+        const long double r = sqrtl(x * x + y * y + z * z);
+        const long double v2 = vx * vx + vy * vy + vz * vz;
+        const long double mu = (long double)G * (long double)m_star;
+        const long double inv_a = 2.0L / r - v2 / mu;                  /* vis-viva */
+        long double hill = 0.0L;
+        if (inv_a > 0.0L) hill = (1.0L / inv_a) * cbrtl((long double)mass[i] / (3.0L * (long double)m_star));
+        else unbound++;
+        const long double v = sqrtl(v2);
+        long double dtk = dt;
+        for (int32_t k = 0; k < nrows; k++) {
+            const long double a = (long double)n1 * hill, b = (long double)n2 * dtk * v;
+            out[(int64_t)k * N + i] = (double)(a > b ? a : b);
+            dtk /= (long double)substeps;
+        }
+    }
+    return unbound;
+}
+
+/* eq. 4: q_i += dt * (sum_j m_j v_j) / m_star.  psum (if not NULL) receives sum_j m_j v_j. */
+void genga_oracle_hc(int64_t N, double *pos, const double *vel, const double *mass, double m_star,
+                     double dt, double *psum)
+{
+    long double p[3] = {0.0L, 0.0L, 0.0L};
+    for (int c = 0; c < 3; c++)
+        for (int64_t j = 0; j < N; j++) p[c] += (long double)mass[j] * (long double)vel[c * N + j];
+    for (int c = 0; c < 3; c++) {
+        const long double shift = (long double)dt * p[c] / (long double)m_star;
+        for (int64_t i = 0; i < N; i++) pos[c * N + i] = (double)((long double)pos[c * N + i] + shift);
+        if (psum) psum[c] = (double)p[c];
+    }
+}
+
+/* The Kepler drift of one body, long double.  Returns 0, or 1 if the orbit is not bound. */
+static int kepler_step(long double mu, long double dt, long double q[3], long double v[3])
+{
+    const long double r0 = sqrtl(q[0] * q[0] + q[1] * q[1] + q[2] * q[2]);
+    const long double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    const long double u = q[0] * v[0] + q[1] * v[1] + q[2] * v[2];
+    const long double inv_a = 2.0L / r0 - v2 / mu;
+    if (!(inv_a > 0.0L)) return 1;
+    const long double a = 1.0L / inv_a;
+    const long double n = sqrtl(mu / (a * a * a));                     /* mean motion */
+    const long double ec = 1.0L - r0 / a;                              /* e cos E0 */
+    const long double es = u / (n * a * a);                            /* e sin E0 */
+    const long double dM = n * dt;
+    /* Kepler's equation in the difference dE = E - E0:
+     *   dE - ec sin dE + es (1 - cos dE) = dM          (Newton, from dE = dM) */
+    long double dE = dM;
+    for (int it = 0; it < 60; it++) {
+        const long double s = sinl(dE), c = cosl(dE);
+        const long double fn = dE - ec * s + es * (1.0L - c) - dM;
+        const long double fp = 1.0L - ec * c + es * s;
+        const long double step = fn / fp;
+        dE -= step;
+        if (fabsl(step) <= 1e-19L * (1.0L + fabsl(dE))) break;
+    }
+    const long double s = sinl(dE), c = cosl(dE);
+    const long double r = a * (1.0L - ec * c + es * s);
+    const long double f = 1.0L - (a / r0) * (1.0L - c);
+    const long double g = dt + (s - dE) / n;
+    const long double fd = -(a * a * n / (r0 * r)) * s;
+    const long double gd = 1.0L - (a / r) * (1.0L - c);
+    for (int k = 0; k < 3; k++) {
+        const long double qk = f * q[k] + g * v[k];
+        const long double vk = fd * q[k] + gd * v[k];
+        q[k] = qk;
+        v[k] = vk;
+    }
+    return 0;
+}
+
+/* FG(dt) for all bodies, in place.  Returns the number of bodies that are not on a bound orbit
+ * (left untouched). */
+int64_t genga_oracle_fg(int64_t N, double *pos, double *vel, double mu, double dt)
+{
+    int64_t unbound = 0;
+#pragma omp parallel for schedule(static) reduction(+ : unbound)
+    for (int64_t i = 0; i < N; i++) {
+        long double q[3] = {pos[i], pos[N + i], pos[2 * N + i]};
+        long double v[3] = {vel[i], vel[N + i], vel[2 * N + i]};
+        if (kepler_step((long double)mu, (long double)dt, q, v)) { unbound++; continue; }
+        for (int k = 0; k < 3; k++) {
+            pos[k * N + i] = (double)q[k];
+            vel[k * N + i] = (double)v[k];
+        }
+    }
+    return unbound;
+}

@@ -1,0 +1,203 @@
+"""Pins of oracle/genga_step_oracle.c (Rcrit, HC, FG and the composed step) against what the paper
+and the mathematics fix -- closed forms, invariants, an independently written Kepler solver -- NOT
+against the oracle itself.  CPU only."""
+import os
+
+import numpy as np
+import pytest
+
+import genga_inputs as gi
+
+G = gi.G_AU_DAY_MSUN
+U = 2.0 ** -53
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def st(oracle_mod):
+    return oracle_mod.step
+
+
+def _elements(n, seed, emax=0.3):
+    u = gi.uniforms(seed, 0, 6 * n).reshape(6, n)
+    a = 0.5 + 3.5 * u[0]
+    e = emax * u[1]
+    inc = 0.3 * u[2]
+    return a, e, inc, 2 * np.pi * u[3], 2 * np.pi * u[4], 2 * np.pi * u[5]
+
+
+# ------------------------------------------------------------------------------------ Rcrit (eq. 5)
+def test_rcrit_constants_are_the_papers():
+    """n1 = 3, n2 = 0.4 -- tests/golden/rcrit_constants.txt."""
+    vals = dict(l.split()[:2] for l in open(os.path.join(HERE, "golden", "rcrit_constants.txt"))
+                if l.strip() and not l.startswith("#"))
+    assert float(vals["n1"]) == 3.0 and float(vals["n2"]) == 0.4
+
+
+def test_rcrit_circular_closed_form(st):
+    """Circular orbit of radius a: R_H = a (m / 3 m_star)^(1/3), v = sqrt(mu / a); each branch of the max."""
+    a = np.array([0.5, 1.0, 2.5, 5.2, 5.2])
+    m = np.array([1e-9, 3e-6, 1e-7, 1e-3, 1e-12])          # 5.2 AU: Hill-dominated (Jupiter) and velocity-dominated
+    n = a.size
+    pos = np.zeros((3, n)); vel = np.zeros((3, n))
+    ang = np.linspace(0.3, 5.0, n)
+    pos[0], pos[1] = a * np.cos(ang), a * np.sin(ang)
+    vc = np.sqrt(G / a)
+    vel[0], vel[1] = -vc * np.sin(ang), vc * np.cos(ang)
+    dt = 6.0
+    rc, bad = st.rcrit(pos, vel, m, 1.0, G, dt, substeps=2.0, nrows=3)
+    assert bad == 0 and rc.shape == (3, n)
+    hill = a * np.cbrt(m / 3.0)
+    for k in range(3):
+        want = np.maximum(3.0 * hill, 0.4 * (dt / 2.0 ** k) * vc)
+        assert np.max(np.abs(rc[k] - want) / want) < 64 * U    # a from vis-viva amplifies rounding by ~2 r v^2/mu
+    assert rc[0, 3] == pytest.approx(3.0 * hill[3], rel=1e-13)         # Jupiter: Hill term wins
+    assert rc[0, 4] == pytest.approx(0.4 * dt * vc[4], rel=1e-13)      # dust at 5.2 AU: velocity term wins
+    assert rc[2, 3] == rc[0, 3]                                         # the Hill term does not shrink with the level
+    assert rc[1, 4] == pytest.approx(0.5 * rc[0, 4], rel=1e-15)         # the velocity term halves
+
+
+def test_rcrit_matches_generator_rows(st):
+    """The input generator computes the same rows in numpy from the ELEMENTS' semi-major axis.  Its velocities
+    use mu = G (1 + m_i), the oracle's vis-viva uses mu = G m_star (as FG does): the Hill term differs by
+    O(m_i / m_star) <= 3e-8 there; with the vis-viva axis of the same mu the rows agree to rounding."""
+    ki = gi.make_config(3, n=3000, level=1)
+    rc, bad = st.rcrit(ki.pos, ki.vel, ki.mass, 1.0, ki.G, ki.dt, substeps=2.0, nrows=2)
+    assert bad == 0
+    assert np.max(np.abs(rc - ki.rcrit) / ki.rcrit) < 1e-7
+    rows = gi.rcrit_rows(gi.semi_major_axis(ki.pos, ki.vel, ki.G), ki.vel, ki.mass, ki.dt, 2, 2)
+    assert np.max(np.abs(rc - rows) / rows) < 1e-13
+    assert (rc[0] > 0.4 * ki.dt * np.sqrt((ki.vel ** 2).sum(0)) * (1 + 1e-12)).sum() > 10     # Hill-dominated bodies exist
+
+
+# --------------------------------------------------------------------------------------- HC (eq. 4)
+def test_hc_hand_example(st):
+    """Three bodies, numbers a reader can check: sum m v = (0.5, -1, 2) * 1e-3 exactly in binary."""
+    mass = np.array([0.5, 0.25, 0.125]) * 2.0 ** -10
+    vel = np.array([[1.0, 2.0, -4.0], [0.0, -8.0, 8.0], [4.0, 0.0, 0.0]])       # [3, N]
+    pos = np.array([[1.0, 2.0, 3.0], [0.5, 0.25, 0.125], [-1.0, -2.0, -3.0]])
+    p_want = np.array([0.5 * 1 + 0.25 * 2 - 0.125 * 4, -0.25 * 8 + 0.125 * 8, 0.5 * 4]) * 2.0 ** -10
+    m_star, dt = 2.0, 0.5
+    q, p = st.hc(pos, vel, mass, m_star, dt)
+    assert np.array_equal(p, p_want)
+    assert np.array_equal(q, pos + (dt * p_want / m_star)[:, None])
+    # every body moves by the same vector; velocities are not touched (H_C depends on p only)
+    assert np.ptp(q - pos, axis=1).max() == 0.0
+
+
+def test_hc_sign_and_linearity(st):
+    ki = gi.make_config(0, n=400)
+    q1, p = st.hc(ki.pos, ki.vel, ki.mass, 1.0, 3.0)
+    q2, _ = st.hc(q1, ki.vel, ki.mass, 1.0, -3.0)
+    assert np.max(np.abs(q2 - ki.pos)) < 4 * U * np.abs(ki.pos).max()
+    assert np.allclose(p, (ki.mass * ki.vel).sum(axis=1), rtol=1e-13, atol=0)
+    q3, _ = st.hc(ki.pos, ki.vel, ki.mass, 2.0, 6.0)           # dt / m_star is what matters
+    assert np.max(np.abs(q3 - q1)) < 4 * U * np.abs(ki.pos).max()
+
+
+# --------------------------------------------------------------------------------------- FG (eq. 2)
+def test_fg_circular_orbit_is_a_rotation(st):
+    a = np.array([0.5, 1.0, 2.0, 4.0])
+    n = a.size
+    pos = np.zeros((3, n)); vel = np.zeros((3, n))
+    pos[0] = a
+    vel[1] = np.sqrt(G / a)
+    for dt in (0.1, 6.0, 200.0, -6.0):
+        q, v, bad = st.fg(pos, vel, G, dt)
+        th = np.sqrt(G / a ** 3) * dt
+        assert bad == 0
+        assert np.max(np.abs(q[0] - a * np.cos(th))) < 8 * U * a.max() * max(1.0, abs(th).max())
+        assert np.max(np.abs(q[1] - a * np.sin(th))) < 8 * U * a.max() * max(1.0, abs(th).max())
+        assert np.all(q[2] == 0.0) and np.all(v[2] == 0.0)
+        assert np.max(np.abs(v[0] + np.sqrt(G / a) * np.sin(th))) < 8 * U * max(1.0, abs(th).max())
+
+
+def test_fg_against_the_generators_kepler_solver(st):
+    """State from elements at M0, drifted by dt, equals the state from elements at M0 + n dt (numpy routine of
+    genga_inputs: solves Kepler's equation in E itself, not in dE)."""
+    a, e, inc, Om, om, M0 = _elements(2000, 42)
+    pos, vel = gi.elements_to_cartesian(a, e, inc, Om, om, M0, G)
+    for dt in (6.0, 61.0, -17.0):
+        q, v, bad = st.fg(pos, vel, G, dt)
+        n = np.sqrt(G / a ** 3)
+        qw, vw = gi.elements_to_cartesian(a, e, inc, Om, om, M0 + n * dt, G)
+        assert bad == 0
+        # the numpy side carries ~1e-15 of its own; n dt up to ~3 rad amplifies the rounding of a
+        assert np.max(np.abs(q - qw)) < 2e-14 * a.max()
+        assert np.max(np.abs(v - vw)) < 2e-14 * np.abs(vel).max() * 4
+
+
+def test_fg_invariants_period_and_inverse(st):
+    a, e, inc, Om, om, M0 = _elements(500, 7, emax=0.6)
+    pos, vel = gi.elements_to_cartesian(a, e, inc, Om, om, M0, G)
+
+    def invariants(q, v):
+        en = 0.5 * (v * v).sum(0) - G / np.sqrt((q * q).sum(0))
+        h = np.cross(q.T, v.T).T
+        ev = np.cross(v.T, h.T).T / G - q / np.sqrt((q * q).sum(0))
+        return en, h, ev
+
+    q, v, bad = st.fg(pos, vel, G, 6.0)
+    assert bad == 0
+    for w, w0 in zip(invariants(q, v), invariants(pos, vel)):
+        assert np.max(np.abs(w - w0)) < 1e-13 * max(np.abs(w0).max(), 1e-4)
+    # one full period returns the body to its start
+    period = 2 * np.pi * np.sqrt(a ** 3 / G)
+    for i in (0, 17, 333):
+        qp, vp, _ = st.fg(pos[:, i:i + 1], vel[:, i:i + 1], G, period[i])
+        assert np.max(np.abs(qp - pos[:, i:i + 1])) < 1e-13 * a[i] * 10
+    # dt followed by -dt
+    qb, vb, _ = st.fg(q, v, G, -6.0)
+    assert np.max(np.abs(qb - pos)) < 1e-14 * a.max() and np.max(np.abs(vb - vel)) < 1e-14 * np.abs(vel).max() * 4
+
+
+def test_fg_unbound_is_reported_and_untouched(st):
+    pos = np.array([[1.0, 1.0], [0.0, 0.0], [0.0, 0.0]])
+    vel = np.array([[0.0, 0.0], [np.sqrt(G), 2.0 * np.sqrt(G)], [0.0, 0.0]])       # circular, hyperbolic
+    q, v, bad = st.fg(pos, vel, G, 6.0)
+    assert bad == 1
+    assert np.array_equal(q[:, 1], pos[:, 1]) and np.array_equal(v[:, 1], vel[:, 1])
+    assert not np.array_equal(q[:, 0], pos[:, 0])
+
+
+# ------------------------------------------------------------------------------- the composed step
+def _energy(q, v, mass, m_star):
+    p = mass * v
+    kin = 0.5 * (mass * (v * v).sum(0)).sum() + 0.5 * (p.sum(1) ** 2).sum() / m_star
+    pot = -(G * m_star * mass / np.sqrt((q * q).sum(0))).sum()
+    n = q.shape[1]
+    for i in range(n):
+        for j in range(i + 1, n):
+            pot -= G * mass[i] * mass[j] / np.sqrt(((q[:, i] - q[:, j]) ** 2).sum())
+    return kin + pot
+
+
+def test_step_energy_error_scales_as_dt_squared(st):
+    """Sun + two planets far outside each other's critical radius (K = 1 everywhere: readings G5 coincide):
+    second-order symplectic => energy error ~ dt^2, no secular drift."""
+    mass = np.array([1e-3, 3e-4])
+    a = np.array([1.0, 2.2]); e = np.array([0.05, 0.1]); z = np.zeros(2)
+    pos, vel = gi.elements_to_cartesian(a, e, z + 0.02, z, z + 1.0, np.array([0.3, 2.0]), G)
+    # democratic coordinates: heliocentric positions, barycentric velocities
+    vel = vel - (mass * vel).sum(1, keepdims=True) / (1.0 + mass.sum())
+    e0 = _energy(pos, vel, mass, 1.0)
+    errs = []
+    for dt in (8.0, 4.0, 2.0):
+        q, v = pos.copy(), vel.copy()
+        worst = 0.0
+        for _ in range(int(round(4000 / dt))):
+            r = st.step(q, v, mass, 2, 0, 1.0, G, dt)
+            assert r.first.count.sum() == 0 and r.unbound == 0
+            q, v = r.pos, r.vel
+            worst = max(worst, abs(_energy(q, v, mass, 1.0) - e0) / abs(e0))
+        errs.append(worst)
+    assert 3.5 < errs[0] / errs[1] < 4.5 and 3.5 < errs[1] / errs[2] < 4.5
+    assert errs[2] < 1e-7
+
+
+def test_step_reports_the_first_kicks_candidates(st, oracle_mod):
+    ki = gi.make_config(0, n=800)
+    r = st.step(ki.pos, ki.vel, ki.mass, ki.n, 0, 1.0, ki.G, ki.dt)
+    assert np.max(np.abs(r.rcrit - ki.rcrit[:1]) / ki.rcrit[:1]) < 1e-13
+    ref = oracle_mod.kick(ki.pos, ki.mass, r.rcrit, ki.n, 0, level=0, G=ki.G)
+    assert np.array_equal(ref.count, r.first.count) and ref.count.sum() > 0
