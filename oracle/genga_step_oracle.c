@@ -90,15 +90,24 @@ static int kepler_step(long double mu, long double dt, long double q[3], long do
     const long double es = u / (n * a * a);                            /* e sin E0 */
     const long double dM = n * dt;
     /* Kepler's equation in the difference dE = E - E0:
-     *   dE - ec sin dE + es (1 - cos dE) = dM          (Newton, from dE = dM) */
-    long double dE = dM;
-    for (int it = 0; it < 60; it++) {
+     *   F(dE) = dE - ec sin dE + es (1 - cos dE) - dM = 0.
+     * F' = 1 - ec cos dE + es sin dE = r/a > 0, so F is increasing, and |F(dE) - (dE - dM)| <= |ec| + 2|es|:
+     * the root is bracketed by dM -+ (|ec| + 2|es|).  Plain bisection to the last bit of the bracket
+     * (slow, cannot fail), then two Newton steps to polish. */
+    long double lo = dM - (fabsl(ec) + 2.0L * fabsl(es)) - 1e-300L, hi = dM + (fabsl(ec) + 2.0L * fabsl(es)) + 1e-300L;
+    long double dE = 0.5L * (lo + hi);
+    for (int it = 0; it < 200; it++) {
+        dE = 0.5L * (lo + hi);
+        if (!(dE > lo && dE < hi)) break;
+        const long double fn = (dE - dM) - ec * sinl(dE) + es * (1.0L - cosl(dE));
+        if (fn > 0.0L) hi = dE; else lo = dE;
+    }
+    for (int it = 0; it < 2; it++) {
         const long double s = sinl(dE), c = cosl(dE);
-        const long double fn = dE - ec * s + es * (1.0L - c) - dM;
+        const long double fn = (dE - dM) - ec * s + es * (1.0L - c);
         const long double fp = 1.0L - ec * c + es * s;
-        const long double step = fn / fp;
-        dE -= step;
-        if (fabsl(step) <= 1e-19L * (1.0L + fabsl(dE))) break;
+        const long double nx = dE - fn / fp;
+        if (nx >= lo && nx <= hi) dE = nx;
     }
     const long double s = sinl(dE), c = cosl(dE);
     const long double r = a * (1.0L - ec * c + es * s);

@@ -1,4 +1,4 @@
-"""Thin ctypes binding of libgenga_kick.so (include/genga_kick.h): argument marshalling only.
+"""Thin ctypes binding of libgenga_kick.so (include/genga_kick.h, include/genga_step.h): argument marshalling only.
 
 PyTorch is used for device memory and streams; every step of the path runs in the library's CUDA
 kernels.  There is no CPU fallback: if the library is missing or no sm_100 device is present the
@@ -19,6 +19,9 @@ EXPORTS = (
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
 )
+# include/genga_step.h: the O(N) neighbours of the kick and the composed step
+STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_step")
+STATUS_UNBOUND = 8
 
 
 class GengaKickConfig(C.Structure):
@@ -74,7 +77,12 @@ def lib():
         L.genga_kick_strerror.restype = C.c_char_p
         L.genga_kick_last_cuda_error.argtypes = [vp]
         L.genga_kick_last_cuda_error.restype = C.c_char_p
-        for name in EXPORTS:
+        L.genga_rcrit.argtypes = [vp, vp, vp, vp, d, d, d, i32, d, d, vp]
+        L.genga_hc.argtypes = [vp, vp, vp, vp, d, d]
+        L.genga_fg.argtypes = [vp, vp, vp, d, d]
+        L.genga_drift.argtypes = [vp, vp, vp, vp, d, d]
+        L.genga_step.argtypes = [vp, vp, vp, vp, d, d, d, d, vp, vp, vp, vp]
+        for name in EXPORTS + STEP_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
                 getattr(L, name).restype = C.c_int
         _lib = L
@@ -145,6 +153,24 @@ class GengaKick:
         self._check(lib().genga_kick_host(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit),
                                           int(changeover_level), float(dt), _ptr(out_acc), _ptr(out_pairs),
                                           _ptr(out_npairs)))
+
+    # include/genga_step.h
+    def rcrit(self, pos, vel, mass, m_star, dt, out_rcrit, substeps=2.0, nrows=1, n1=3.0, n2=0.4):
+        self._check(lib().genga_rcrit(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt),
+                                      float(substeps), int(nrows), float(n1), float(n2), _ptr(out_rcrit)))
+
+    def hc(self, pos, vel, mass, m_star, dt):
+        self._check(lib().genga_hc(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt)))
+
+    def fg(self, pos, vel, m_star, dt):
+        self._check(lib().genga_fg(self._ctx, _ptr(pos), _ptr(vel), float(m_star), float(dt)))
+
+    def drift(self, pos, vel, mass, m_star, dt):
+        self._check(lib().genga_drift(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt)))
+
+    def step(self, pos, vel, mass, m_star, dt, rcrit_row, out_acc, out_pairs, out_npairs, n1=3.0, n2=0.4):
+        self._check(lib().genga_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt), float(n1),
+                                     float(n2), _ptr(rcrit_row), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs)))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

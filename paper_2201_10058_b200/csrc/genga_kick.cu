@@ -1,7 +1,7 @@
 // C ABI of the B200-native GENGA kick + close-encounter pre-check (include/genga_kick.h).
 // Host side only: argument checks, scratch ownership, kernel launches on the caller's stream.
 // Every step of the path runs in the kernels of genga_kick_kernels.cuh; there is no CPU fallback.
-#include "../../include/genga_kick.h"
+#include "genga_kick_ctx.h"
 #include "genga_kick_variants.h"
 #include "genga_kick_kernels.cuh"
 #include "genga_kick_sort.cuh"
@@ -12,59 +12,10 @@
 #include <new>
 #include <string>
 
-struct genga_kick_ctx {
-    genga_kick_config cfg;
-    int64_t N;
-    int num_sms;
-    cudaStream_t stream;
-    genga_kick_plan* plans;        // one per level 0..max_level
-    // scratch (device)
-    double2* rxy;
-    double2* rzm;
-    int* rfw;
-    int* ridx;
-    int* cfw;
-    float4* cblo;
-    float4* cbhi;
-    // internal order (genga_kick_sort.cuh); sorted == false: caller's order
-    bool sorted;
-    int sort_blocks;
-    unsigned* bbox;
-    unsigned* keys_a;
-    unsigned* keys_b;
-    int* vals_a;                   // ends up holding the permutation
-    int* vals_b;
-    int* counts;
-    double* partial;
-    int* status;
-    // exact path: candidate list, fixed-point accumulators (genga_kick_kernels.cuh)
-    int2* cand;
-    int64_t cand_capacity;
-    int* ncand;
-    unsigned long long* fx;
-    int* touched;
-    int64_t n_rec_alloc;
-    // staging for genga_kick_host (device, lazily allocated)
-    double* h_pos; double* h_vel; double* h_mass; double* h_rcrit; double* h_acc;
-    int32_t* h_pairs; int32_t* h_npairs;
-    int64_t launches;
-    // measurement aids (genga_kick_enable_timing)
-    bool timing;
-    cudaEvent_t* ev;               // [max_level + 1][2], created by genga_kick_enable_timing
-    bool* ev_set;                  // [max_level + 1]
-    std::string cuda_err;
-};
-
 namespace {
 
-int cuda_fail(genga_kick_ctx* ctx, cudaError_t e)
-{
-    if (ctx) ctx->cuda_err = cudaGetErrorString(e);
-    return GENGA_KICK_E_CUDA;
-}
-#define GK_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_); } while (0)
-
-bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+int cuda_fail(genga_kick_ctx* ctx, cudaError_t e) { return genga_cuda_fail(ctx, e); }
+bool misaligned(const void* p) { return genga_misaligned(p); }
 
 template <int THREADS, int IPT, int JT, int CTAS>
 cudaError_t launch_kick(const genga::KickParams& kp, cudaStream_t st)
@@ -177,9 +128,16 @@ extern "C" int genga_kick_set_stream(genga_kick_ctx* ctx, void* cuda_stream)
 extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
                           int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs)
 {
-    if (!ctx || !pos || !mass || !rcrit || !out_npairs) return GENGA_KICK_E_NULL;
+    if (!out_npairs) return GENGA_KICK_E_NULL;
+    return genga_kick_impl(ctx, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs);
+}
+
+int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
+                    int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs)
+{
+    if (!ctx || !pos || !mass || !rcrit) return GENGA_KICK_E_NULL;
     if (!out_acc && !vel) return GENGA_KICK_E_NULL;
-    if (!out_pairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
+    if (!out_pairs && out_npairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
     if (misaligned(pos) || misaligned(vel) || misaligned(mass) || misaligned(rcrit) || misaligned(out_acc) ||
         misaligned(out_pairs) || misaligned(out_npairs))
         return GENGA_KICK_E_ALIGN;
@@ -445,7 +403,8 @@ extern "C" int genga_kick_free(genga_kick_ctx* ctx)
     if (!ctx) return GENGA_KICK_OK;
     void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
                     ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
-                    ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs};
+                    ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs,
+                    ctx->psum_partial, ctx->psum_ticket, ctx->step_rcrit};
     for (void* b : bufs)
         if (b) cudaFree(b);
     if (ctx->ev)

@@ -1,0 +1,67 @@
+// The context of the C-ABI library (include/genga_kick.h, include/genga_step.h): private to csrc/.
+#pragma once
+#include "../../include/genga_kick.h"
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+struct genga_kick_ctx {
+    genga_kick_config cfg;
+    int64_t N;
+    int num_sms;
+    cudaStream_t stream;
+    genga_kick_plan* plans;        // one per level 0..max_level
+    // scratch (device)
+    double2* rxy;
+    double2* rzm;
+    int* rfw;
+    int* ridx;
+    int* cfw;
+    float4* cblo;
+    float4* cbhi;
+    // internal order (genga_kick_sort.cuh); sorted == false: caller's order
+    bool sorted;
+    int sort_blocks;
+    unsigned* bbox;
+    unsigned* keys_a;
+    unsigned* keys_b;
+    int* vals_a;                   // ends up holding the permutation
+    int* vals_b;
+    int* counts;
+    double* partial;
+    int* status;
+    // exact path: candidate list, fixed-point accumulators (genga_kick_kernels.cuh)
+    int2* cand;
+    int64_t cand_capacity;
+    int* ncand;
+    unsigned long long* fx;
+    int* touched;
+    int64_t n_rec_alloc;
+    // staging for genga_kick_host (device, lazily allocated)
+    double* h_pos; double* h_vel; double* h_mass; double* h_rcrit; double* h_acc;
+    int32_t* h_pairs; int32_t* h_npairs;
+    int64_t launches;
+    // measurement aids (genga_kick_enable_timing)
+    bool timing;
+    cudaEvent_t* ev;               // [max_level + 1][2], created by genga_kick_enable_timing
+    bool* ev_set;                  // [max_level + 1]
+    // O(N) neighbours of the kick (genga_step.cu), lazily allocated
+    double* psum_partial;          // [GENGA_PSUM_BLOCKS][3] block sums of m v, then the totals at [GENGA_PSUM_BLOCKS][3]
+    unsigned* psum_ticket;         // last-block-done counter, zero between launches
+    double* step_rcrit;            // [N] row Rcrit(dt) of genga_step when the caller keeps none
+    std::string cuda_err;
+};
+
+
+static inline int genga_cuda_fail(genga_kick_ctx* ctx, cudaError_t e)
+{
+    if (ctx) ctx->cuda_err = cudaGetErrorString(e);
+    return GENGA_KICK_E_CUDA;
+}
+#define GK_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return genga_cuda_fail(ctx, e_); } while (0)
+
+static inline bool genga_misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+// genga_kick with out_npairs == nullptr allowed: no pre-check output (the closing kick of genga_step)
+int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
+                    int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs);

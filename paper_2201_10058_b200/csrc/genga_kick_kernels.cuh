@@ -44,7 +44,7 @@ struct KickParams {
     // encounter output
     int* __restrict__ out_pairs;       // [capacity][2]
     long long capacity;
-    int* __restrict__ out_npairs;      // [N + 1]
+    int* __restrict__ out_npairs;      // [N + 1]; nullptr: no pre-check output wanted (closing kick of genga_step)
     int* __restrict__ status;
     // exact path (candidate list, fixed-point accumulators)
     int2* __restrict__ cand;           // [cand_capacity] (i-record, j-record)
@@ -127,7 +127,7 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
             cblo[r / GENGA_GROUP] = make_float4(lx, ly, lz, __int_as_float(m));
             cbhi[r / GENGA_GROUP] = make_float4(hx, hy, hz, 0.0f);
         }
-        if (r <= N) out_npairs[r] = 0;
+        if (out_npairs && r <= N) out_npairs[r] = 0;
     }
 }
 
@@ -482,7 +482,7 @@ __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
                     fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
                     p.touched[ir] = 1;
                 }
-                if (r.enc) {
+                if (r.enc && p.out_npairs) {
                     atomicAdd(p.out_npairs + bi, 1);
                     if (bi >= p.n_massive) {               // test particle i, massive j
                         atomicAdd(p.out_npairs + bj, 1);

@@ -29,6 +29,16 @@ def test_every_declared_symbol_is_exported(built):
     assert declared == set(g.EXPORTS), f"binding and header disagree: {declared ^ set(g.EXPORTS)}"
 
 
+def test_every_declared_step_symbol_is_exported(built):
+    header = open(os.path.join(ROOT, "include", "genga_step.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\bint\s+(genga_\w+)\s*\(", header))
+    assert declared == set(g.STEP_EXPORTS), f"binding and header disagree: {declared ^ set(g.STEP_EXPORTS)}"
+    lib = ctypes.CDLL(built)
+    missing = [name for name in sorted(declared) if not hasattr(lib, name)]
+    assert not missing, f"declared but not exported: {missing}"
+
+
 def test_strerror_texts(built):
     for code in (g.OK, g.E_NULL, g.E_ALIGN, g.E_SIZE, g.E_LEVEL, g.E_CUDA, g.E_NOMEM):
         assert g.strerror(code) and "unknown" not in g.strerror(code)
