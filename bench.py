@@ -246,6 +246,30 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         levels[str(level)] = {"ms_per_kick": ms, "pairs_per_s": pairs_per_kick / (ms * 1e-3),
                               "pair_loop_ms": float(np.mean(loop_ms[level])), "encounter_pairs": enc_pairs[level]}
 
+    # NEXT-1: the whole App. A step without the Bulirsch-Stoer branch on the same disk --
+    # Rcrit, Kick(dt/2) + pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) -- and its O(N) part alone
+    sq, sv = pos.clone(), vel.clone()
+    rrow = torch.empty(n, dtype=torch.float64, device=dev)
+    step_ts, drift_ts = [], []
+    for it in range(8):
+        a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        flush.fill_(5)
+        l0 = kick.launch_count()
+        a.record(stream)
+        kick.step(sq, sv, mass, 1.0, ki.dt, rrow, acc, pairs, npairs)
+        b.record(stream)
+        step_launches = kick.launch_count() - l0
+        kick.drift(sq, sv, mass, 1.0, ki.dt)
+        c.record(stream)
+        c.synchronize()
+        if it >= 3:
+            step_ts.append(a.elapsed_time(b))
+            drift_ts.append(b.elapsed_time(c))
+    step_info = {"what": "Rcrit, Kick(dt/2)+pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) at level 0 (genga_step)",
+                 "ms_per_step": float(np.median(step_ts)), "launches_per_step": int(step_launches),
+                 "drift_ms": float(np.median(drift_ts)), "drift_what": "HC(dt/2) FG(dt) HC(dt/2) alone, 3 launches, "
+                 "184 B/body of HBM traffic", "status": kick.status()}
+
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
@@ -293,6 +317,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                        "l2": "256 MiB buffer written between timed iterations (working set 3 MB is L2-resident)",
                        "parallelism": "replicas" if world > 1 else "single GPU"},
             "levels": levels,
+            "step": step_info,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
