@@ -21,6 +21,9 @@ EXPORTS = (
 )
 # include/genga_step.h: the O(N) neighbours of the kick and the composed step
 STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_step")
+# include/genga_group.h: close-encounter groups
+GROUP_EXPORTS = ("genga_group",)
+STATUS_BAD_PAIR = 16
 STATUS_UNBOUND = 8
 
 
@@ -82,7 +85,8 @@ def lib():
         L.genga_fg.argtypes = [vp, vp, vp, d, d]
         L.genga_drift.argtypes = [vp, vp, vp, vp, d, d]
         L.genga_step.argtypes = [vp, vp, vp, vp, d, d, d, d, vp, vp, vp, vp]
-        for name in EXPORTS + STEP_EXPORTS:
+        L.genga_group.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
+        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
                 getattr(L, name).restype = C.c_int
         _lib = L
@@ -171,6 +175,12 @@ class GengaKick:
     def step(self, pos, vel, mass, m_star, dt, rcrit_row, out_acc, out_pairs, out_npairs, n1=3.0, n2=0.4):
         self._check(lib().genga_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt), float(n1),
                                      float(n2), _ptr(rcrit_row), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs)))
+
+    # include/genga_group.h
+    def group(self, pairs, n_pairs, pair_rows, group_of, members, offsets, summary):
+        """n_pairs: a device int32 tensor VIEW whose first element is the pair count (e.g. out_npairs[N:])."""
+        self._check(lib().genga_group(self._ctx, _ptr(pairs), _ptr(n_pairs), int(pair_rows), _ptr(group_of),
+                                      _ptr(members), _ptr(offsets), _ptr(summary)))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

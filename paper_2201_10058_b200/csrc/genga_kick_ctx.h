@@ -49,6 +49,9 @@ struct genga_kick_ctx {
     double* psum_partial;          // [GENGA_PSUM_BLOCKS][3] block sums of m v, then the totals at [GENGA_PSUM_BLOCKS][3]
     unsigned* psum_ticket;         // last-block-done counter, zero between launches
     double* step_rcrit;            // [N] row Rcrit(dt) of genga_step when the caller keeps none
+    // grouping (genga_group.cu), lazily allocated
+    int* grp_label; int* grp_flag; unsigned* grp_keys_a; unsigned* grp_keys_b; int* grp_vals_a; int* grp_vals_b;
+    int* grp_counts;
     std::string cuda_err;
 };
 

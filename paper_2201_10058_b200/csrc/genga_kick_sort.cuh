@@ -34,13 +34,13 @@ __device__ __forceinline__ float ord2f(unsigned u)
 }
 
 // bbox[0..3] = ord(min x), ord(min y), ord(max x), ord(max y)
-__global__ void sort_init_kernel(unsigned* __restrict__ bbox)
+static __global__ void sort_init_kernel(unsigned* __restrict__ bbox)
 {
     if (threadIdx.x < 2) bbox[threadIdx.x] = 0xffffffffu;
     else if (threadIdx.x < 4) bbox[threadIdx.x] = 0u;
 }
 
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 bbox_kernel(const double* __restrict__ pos, int N, unsigned* __restrict__ bbox)
 {
     float lox = 3.0e38f, loy = 3.0e38f, hix = -3.0e38f, hiy = -3.0e38f;
@@ -80,7 +80,7 @@ __device__ __forceinline__ unsigned hilbert_index(unsigned x, unsigned y)
 }
 
 // key of body b; counts of the first digit per sort block
-__global__ void __launch_bounds__(GENGA_SORT_THREADS)
+static __global__ void __launch_bounds__(GENGA_SORT_THREADS)
 key_hist_kernel(const double* __restrict__ pos, int N, int n_massive, const unsigned* __restrict__ bbox,
                 unsigned* __restrict__ keys, int* __restrict__ vals, int bits, int n_blocks, int* __restrict__ counts)
 {
@@ -109,7 +109,7 @@ key_hist_kernel(const double* __restrict__ pos, int N, int n_massive, const unsi
     for (int d = threadIdx.x; d < nd; d += blockDim.x) counts[(size_t)d * n_blocks + blockIdx.x] = hist[d];
 }
 
-__global__ void __launch_bounds__(GENGA_SORT_THREADS)
+static __global__ void __launch_bounds__(GENGA_SORT_THREADS)
 radix_hist_kernel(const unsigned* __restrict__ keys, int N, int shift, int bits, int n_blocks, int* __restrict__ counts)
 {
     __shared__ int hist[GENGA_SORT_MAXDIGITS];
@@ -124,7 +124,7 @@ radix_hist_kernel(const unsigned* __restrict__ keys, int N, int shift, int bits,
 }
 
 // exclusive prefix sum of counts[0..n) in place, one CTA, fixed order
-__global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ counts, int n)
+static __global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ counts, int n)
 {
     __shared__ int wsum[32];
     __shared__ int carry;
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ counts, in
 // [w * 512, (w + 1) * 512) and walks them in order, 32 at a time; the rank of an item among the
 // items of the same digit is (global offset of digit, block) + (count in lower warps) + (count in
 // earlier rounds of this warp) + (lower lanes of this round): no atomics, input order kept.
-__global__ void __launch_bounds__(GENGA_SORT_THREADS)
+static __global__ void __launch_bounds__(GENGA_SORT_THREADS)
 radix_scatter_kernel(const unsigned* __restrict__ keys_in, const int* __restrict__ vals_in, int N, int shift, int bits,
                      int n_blocks, const int* __restrict__ offsets, unsigned* __restrict__ keys_out,
                      int* __restrict__ vals_out)
