@@ -270,6 +270,29 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                  "drift_ms": float(np.median(drift_ts)), "drift_what": "HC(dt/2) FG(dt) HC(dt/2) alone, 3 launches, "
                  "184 B/body of HBM traffic", "status": kick.status()}
 
+    # NEXT-2: grouping of the level-0 pair list (499,679 pairs at N = 65,536) into close-encounter groups
+    kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
+    group_of = torch.empty(n, dtype=torch.int32, device=dev)
+    members = torch.empty(n, dtype=torch.int32, device=dev)
+    offsets = torch.empty(n + 1, dtype=torch.int32, device=dev)
+    summary = torch.empty(4, dtype=torch.int32, device=dev)
+    group_ts = []
+    for it in range(8):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        flush.fill_(6)
+        l0 = kick.launch_count()
+        a.record(stream)
+        kick.group(pairs, npairs[n:], PAIR_CAPACITY, group_of, members, offsets, summary)
+        b.record(stream)
+        b.synchronize()
+        group_launches = kick.launch_count() - l0
+        if it >= 3:
+            group_ts.append(a.elapsed_time(b))
+    sm = summary.cpu().tolist()
+    group_info = {"what": "genga_group on the level-0 pair list: connected components, members sorted by (group, body)",
+                  "ms": float(np.median(group_ts)), "launches": int(group_launches), "pairs": sm[3], "n_groups": sm[0],
+                  "n_members": sm[1], "largest_group": sm[2]}
+
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
@@ -318,6 +341,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                        "parallelism": "replicas" if world > 1 else "single GPU"},
             "levels": levels,
             "step": step_info,
+            "group": group_info,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,

@@ -8,6 +8,8 @@
 
 namespace {
 
+const int GENGA_GROUP_SAMPLE = 8;      // first hook pass: every 8th pair
+
 int ensure_group_scratch(genga_kick_ctx* ctx)
 {
     if (ctx->grp_label) return GENGA_KICK_OK;
@@ -42,19 +44,23 @@ extern "C" int genga_group(genga_kick_ctx* ctx, const int32_t* pairs, const int3
     cudaStream_t st = ctx->stream;
     genga::group_init_kernel<<<blocks, 256, 0, st>>>(ctx->grp_label, ctx->grp_flag, N, offsets, summary);
     const int hook_blocks = (int)std::min<int64_t>(std::max<int64_t>((pair_rows + 255) / 256, 1), 8 * ctx->num_sms);
-    genga::group_hook_kernel<<<hook_blocks, 256, 0, st>>>(reinterpret_cast<const int2*>(pairs), n_pairs, pair_rows, N,
-                                                          ctx->grp_label, ctx->grp_flag, summary, ctx->status);
+    const int2* pr = reinterpret_cast<const int2*>(pairs);
+    genga::group_hook_kernel<<<hook_blocks, 256, 0, st>>>(pr, n_pairs, pair_rows, N, GENGA_GROUP_SAMPLE, true, ctx->grp_label,
+                                                          ctx->grp_flag, summary, ctx->status);
+    genga::group_compress_kernel<<<blocks, 256, 0, st>>>(ctx->grp_label, N);
+    genga::group_hook_kernel<<<hook_blocks, 256, 0, st>>>(pr, n_pairs, pair_rows, N, GENGA_GROUP_SAMPLE, false, ctx->grp_label,
+                                                          ctx->grp_flag, summary, ctx->status);
     genga::group_flat_kernel<<<blocks, 256, 0, st>>>(ctx->grp_label, ctx->grp_flag, N, group_of, ctx->grp_keys_a,
                                                      ctx->grp_vals_a);
-    ctx->launches += 3;
+    ctx->launches += 5;
 
-    // stable LSD radix sort of (key, body) by key in [0, N]: digits of at most 8 bits
+    // stable LSD radix sort of (key, body) by key in [0, N]: digits of at most 9 bits (GENGA_SORT_MAXDIGITS)
     int key_bits = 1;
     while ((1ll << key_bits) <= (long long)N) key_bits++;
     const int nb = (N + GENGA_SORT_BLOCK - 1) / GENGA_SORT_BLOCK;
     unsigned *ka = ctx->grp_keys_a, *kb = ctx->grp_keys_b;
     int *va = ctx->grp_vals_a, *vb = ctx->grp_vals_b;
-    const int passes = (key_bits + 7) / 8;
+    const int passes = (key_bits + 8) / 9;
     for (int pass = 0, shift = 0; pass < passes; pass++) {
         const int bits = (key_bits - shift + (passes - pass) - 1) / (passes - pass);      // spread the bits evenly
         genga::radix_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ka, N, shift, bits, nb, ctx->grp_counts);

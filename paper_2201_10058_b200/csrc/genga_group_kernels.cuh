@@ -28,12 +28,17 @@ group_init_kernel(int* __restrict__ label, int* __restrict__ flag, int N, int* _
     if (i == 0) offsets[0] = 0;
 }
 
-// root of x; reads bypass L1 (other CTAs re-hook roots while this runs); path halving
+// Root of x, with path halving.  The walk reads through L1 (ld.ca): the top of a large tree is read by
+// every thread of the device, and L2-only reads of that one line serialise (measured on the 33,297-body
+// group of config 3: 0.55 ms with ld.cg, 0.18 ms with ld.ca, one pass over all pairs).  A stale line is harmless: label[.] only ever
+// moves to a proper ancestor, so a stale value is still an ancestor, and a stale "root" is caught by the
+// atomicCAS of the hook, which returns the true parent and continues from there with a strictly smaller
+// vertex.
 __device__ __forceinline__ int group_find(int* label, int x)
 {
-    int p = __ldcg(label + x);
+    int p = __ldca(label + x);
     while (p != x) {
-        const int gp = __ldcg(label + p);
+        const int gp = __ldca(label + p);
         if (gp != p) label[x] = gp;                         // still an ancestor: label[.] only ever decreases along a path
         x = p;
         p = gp;
@@ -43,11 +48,16 @@ __device__ __forceinline__ int group_find(int* label, int x)
 
 __global__ void __launch_bounds__(256)
 group_hook_kernel(const int2* __restrict__ pairs, const int* __restrict__ n_pairs, long long pair_rows, int N,
-                  int* __restrict__ label, int* __restrict__ flag, int* __restrict__ summary, int* __restrict__ status)
+                  int sample, bool sampled, int* __restrict__ label, int* __restrict__ flag, int* __restrict__ summary,
+                  int* __restrict__ status)
 {
+    // Two passes (host): first every `sample`-th pair (sampled = true), which already links most of a large
+    // group; then, after group_compress_kernel has flattened the trees, the other pairs (sampled = false) --
+    // for almost all of them both ends then point at the same root and the pair costs two cached reads.
     const long long total = min((long long)max(*n_pairs, 0), pair_rows);
     if (blockIdx.x == 0 && threadIdx.x == 0) summary[3] = (int)total;
     for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < total; p += (long long)gridDim.x * blockDim.x) {
+        if (((p % sample) == 0) != sampled) continue;
         const int2 e = pairs[p];
         if (e.x < 0 || e.y < 0 || e.x >= N || e.y >= N) { atomicOr(status, GENGA_STATUS_BAD_PAIR); continue; }
         flag[e.x] = 1;
@@ -61,6 +71,16 @@ group_hook_kernel(const int2* __restrict__ pairs, const int* __restrict__ n_pair
             rv = group_find(label, lo);
         }
     }
+}
+
+// label[i] = root of i for every body (between the two hook passes)
+__global__ void __launch_bounds__(256) group_compress_kernel(int* __restrict__ label, int N)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int x = i, p = __ldcg(label + x);
+    while (p != x) { x = p; p = __ldcg(label + x); }
+    label[i] = x;                                           // an ancestor of i: concurrent readers stay correct
 }
 
 __global__ void __launch_bounds__(256)
