@@ -21,8 +21,11 @@
  *                                                                            (f: parity unpinned)
  *   J(i) = massive bodies [0, n_massive) for every i (semi-active test
  *   particles feel the massive bodies, not each other)                       sec. 8.1
- *   A massive body also lists its test-particle partners (encounter check only, no force from
- *   massless/semi-active bodies on this path: readings G10, G11).
+ *   A massive body also lists its test-particle partners (reading G11).  tp_mode selects the force
+ *   terms of Fig. 14: 1 = "TP 1", test particles exert no force (the rectangular
+ *   kick of north_star, reading G10); 2 = "TP 2", semi-active particles with mass also act on the
+ *   massive bodies "the same way as in the fully interactive mode": massive i
+ *   then sums over ALL j.
  *
  * Arithmetic: every per-pair quantity in IEEE binary64 exactly in the order written below
  * (compile with -ffp-contract=off); the sums over j in long double (x87 80-bit, 64-bit
@@ -98,7 +101,7 @@ int genga_oracle_num_threads(void)
  *   border   [bcap][2], *nborder: pairs (i, j) with | r/(f rc_L) - 1 | <= 1e-12 ("borderline", G4)
  * returns 0, or -1 on a coincident distinct pair (r2 == 0: outside the domain, G7).
  */
-int genga_oracle_kick(int32_t n_massive, int32_t n_test, int32_t L, double G, double f,
+int genga_oracle_kick_tp(int32_t n_massive, int32_t n_test, int32_t tp_mode, int32_t L, double G, double f,
                       const double *pos, const double *mass, const double *rcrit,
                       const int32_t *rows, int64_t nrows,
                       double *acc, double *S, int32_t *count,
@@ -140,7 +143,7 @@ int genga_oracle_kick(int32_t n_massive, int32_t n_test, int32_t L, double G, do
                 slot = nb++;
                 if (slot < bcap) { border[2 * slot] = (int32_t)i; border[2 * slot + 1] = (int32_t)j; }
             }
-            if (j >= n_massive) continue;                           /* no force from test particles */
+            if (j >= n_massive && tp_mode != 2) continue;           /* TP 1: no force from test particles */
             /* level weight   (eq. 62-63, G3) */
             double W = 1.0;
             for (int k = 0; k < L; k++) {
@@ -160,4 +163,16 @@ int genga_oracle_kick(int32_t n_massive, int32_t n_test, int32_t L, double G, do
     }
     if (nborder) *nborder = nb;
     return bad ? -1 : 0;
+}
+
+/* TP 1 (the rectangular kick of north_star): the entry point the kick tests use. */
+int genga_oracle_kick(int32_t n_massive, int32_t n_test, int32_t L, double G, double f,
+                      const double *pos, const double *mass, const double *rcrit,
+                      const int32_t *rows, int64_t nrows,
+                      double *acc, double *S, int32_t *count,
+                      int32_t *partners, int32_t maxp,
+                      int32_t *border, int64_t bcap, int64_t *nborder)
+{
+    return genga_oracle_kick_tp(n_massive, n_test, 1, L, G, f, pos, mass, rcrit, rows, nrows, acc, S, count,
+                                partners, maxp, border, bcap, nborder);
 }

@@ -28,6 +28,8 @@ def _L():
         lib.genga_oracle_num_threads.restype = C.c_int
         lib.genga_oracle_kick.restype = C.c_int
         lib.genga_oracle_kick.argtypes = [i32, i32, i32, d, d, p, p, p, p, i64, p, p, p, p, i32, p, i64, p]
+        lib.genga_oracle_kick_tp.restype = C.c_int
+        lib.genga_oracle_kick_tp.argtypes = [i32, i32, i32, i32, d, d, p, p, p, p, i64, p, p, p, p, i32, p, i64, p]
         _lib = lib
     return _lib
 
@@ -67,8 +69,9 @@ class OracleResult:
     coincident: bool        # a distinct pair with r2 == 0 was met (outside the domain)
 
 
-def kick(pos, mass, rcrit, n_massive, n_test=0, level=0, G=1.0, enc_factor=1.0, rows=None, maxp=64):
-    """Evaluate the oracle for ``rows`` (default: every body).  Arrays as in SURVEY.md 8(b)."""
+def kick(pos, mass, rcrit, n_massive, n_test=0, level=0, G=1.0, enc_factor=1.0, rows=None, maxp=64, tp_mode=1):
+    """Evaluate the oracle for ``rows`` (default: every body).  Arrays as in SURVEY.md 8(b).
+    tp_mode 1: test particles exert no force (TP 1); 2: they act on the massive bodies (TP 2)."""
     n = int(n_massive) + int(n_test)
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     mass = np.ascontiguousarray(mass, dtype=np.float64)
@@ -83,7 +86,7 @@ def kick(pos, mass, rcrit, n_massive, n_test=0, level=0, G=1.0, enc_factor=1.0, 
     while True:
         part = np.full((nr, maxp), -1, dtype=np.int32)
         nb.value = 0
-        rc = _L().genga_oracle_kick(int(n_massive), int(n_test), int(level), float(G), float(enc_factor),
+        rc = _L().genga_oracle_kick_tp(int(n_massive), int(n_test), int(tp_mode), int(level), float(G), float(enc_factor),
                                     pos.ctypes.data, mass.ctypes.data, rcrit.ctypes.data,
                                     rows.ctypes.data, nr, acc.ctypes.data, S.ctypes.data, count.ctypes.data,
                                     part.ctypes.data, int(maxp), border.ctypes.data, bcap, C.byref(nb))

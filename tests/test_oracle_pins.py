@@ -348,3 +348,40 @@ def test_semi_active_particles_with_mass_exert_no_force_on_this_path(oracle_mod)
     for q in (2, 3):                                                  # particles feel exactly the two massive bodies
         want = sum(G * m[j] * (pos[:, j] - pos[:, q]) / np.linalg.norm(pos[:, j] - pos[:, q]) ** 3 for j in (0, 1))
         assert np.all(np.abs(tp.acc[:, q] - want) <= 8 * U * tp.S[:, q])
+
+
+# ---------------------------------------------------------------- TP 2 (semi-active particles)
+def _tp2_case(n_m=40, n_t=300, seed=3):
+    ki = gi.make_config(4, n=n_m, n_test=n_t)
+    u = gi.uniforms(seed, 0, n_t)
+    ki.mass = ki.mass.copy()
+    ki.mass[n_m:] = 1e-12 * (1.0 + u)                       # semi-active particles WITH mass
+    return ki
+
+
+def test_TP2_momentum_over_all_bodies(oracle_mod):
+    """Every force term of Fig. 14's right panel has its reaction: sum over ALL bodies of m a = 0 (TP 1: it is not)."""
+    ki = _tp2_case()
+    r2 = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, G=ki.G, tp_mode=2)
+    p = (ki.mass * r2.acc).sum(axis=1)
+    assert np.all(np.abs(p) <= 8 * U * (ki.mass * r2.S).sum(axis=1))
+    r1 = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, G=ki.G, tp_mode=1)
+    p1 = (ki.mass * r1.acc).sum(axis=1)
+    assert np.any(np.abs(p1) > 1e3 * U * (ki.mass * r1.S).sum(axis=1))
+    assert np.array_equal(r1.count, r2.count)                # the encounter list does not depend on the mode
+
+
+def test_TP2_is_the_full_interaction_minus_tp_tp(oracle_mod):
+    """Massive bodies: exactly the fully interactive sum (TP 0) over all N.  Semi-active bodies: the TP 0 sum
+    minus the sum over the other semi-active bodies (computed as a TP 0 run on that subset alone)."""
+    ki = _tp2_case()
+    nm, n = ki.n_massive, ki.n
+    r2 = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, nm, ki.n_test, G=ki.G, tp_mode=2)
+    full = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, n, 0, G=ki.G)
+    assert np.array_equal(r2.acc[:, :nm], full.acc[:, :nm]) and np.array_equal(r2.S[:, :nm], full.S[:, :nm])
+    tt = oracle_mod.kick(ki.pos[:, nm:], ki.mass[nm:], ki.rcrit[:, nm:], n - nm, 0, G=ki.G)
+    want = full.acc[:, nm:] - tt.acc
+    assert np.all(np.abs(r2.acc[:, nm:] - want) <= 4 * U * (full.S[:, nm:] + tt.S))
+    # and TP 1 differs from TP 2 only on the massive bodies
+    r1 = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, nm, ki.n_test, G=ki.G, tp_mode=1)
+    assert np.array_equal(r1.acc[:, nm:], r2.acc[:, nm:]) and not np.array_equal(r1.acc[:, :nm], r2.acc[:, :nm])
