@@ -14,8 +14,9 @@
  *   pre-check: (i, j) is an encounter pair iff r_ij^2 < (enc_factor * rcL_ij)^2   (strict)
  *
  * Bodies [0, n_massive) interact fully; bodies [n_massive, n_massive + n_test) are semi-active
- * test particles: they feel the massive bodies and not each other, and exert no force on this
- * path (sec. 8.1).  Readings of the paper where it is silent: DESIGN.md.
+ * test particles: they feel the massive bodies and not each other (sec. 8.1).
+ * With tp_mode = 2 ("TP 2") those that have mass also act on the massive bodies, in the sum above;
+ * otherwise ("TP 1") they exert no force.  Readings of the paper where it is silent: DESIGN.md.
  *
  * All functions return 0 on success or a negative genga_kick_error.  Nothing throws, aborts or
  * prints.  Nothing falls back to the CPU: without a usable CUDA device genga_kick_init fails.
@@ -60,7 +61,9 @@ typedef struct {
     double  enc_factor;     /* f in r_ij < f * rcL_ij; 1.0                                         */
     int32_t order_mode;     /* GENGA_KICK_ORDER_*: the library's INTERNAL body order (never visible
                                in the outputs; changes speed and summation order, not the contract) */
-    int32_t reserved;       /* 0                                                                   */
+    int32_t tp_mode;        /* force terms of the semi-active particles (Fig. 14):
+                               0 or 1 = "TP 1": they feel the massive bodies and exert no force;
+                               2      = "TP 2": those with mass also act on the massive bodies       */
 } genga_kick_config;
 
 #define GENGA_KICK_ORDER_AUTO    0   /* spatially sorted copy when N >= 4096, caller's order below  */
@@ -93,6 +96,9 @@ typedef struct {
  * with num_sms multiprocessors.  Errors: E_NULL, E_SIZE, E_LEVEL (level < 0). */
 int genga_kick_make_plan(int32_t n_massive, int32_t n_test, int32_t level, int32_t num_sms,
                          genga_kick_plan* plan);
+/* TP 2 only: the plan of the second pass of a level-0 kick, massive bodies (i) x semi-active
+ * particles (j), same tile / CTA / partial-sum scheme.  Errors: E_NULL, E_SIZE. */
+int genga_kick_make_plan_tp2(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan);
 /* Tile range [*t0, *t1) of CTA `cta` under *plan.  Errors: E_NULL, E_SIZE. */
 int genga_kick_plan_cta_range(const genga_kick_plan* plan, int32_t cta, int64_t* t0, int64_t* t1);
 /* First and last CTA whose range meets i-block `ib`.  Errors: E_NULL, E_SIZE. */

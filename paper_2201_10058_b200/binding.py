@@ -14,7 +14,7 @@ STATUS_COINCIDENT = 1
 ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 
 EXPORTS = (
-    "genga_kick_make_plan", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
+    "genga_kick_make_plan", "genga_kick_make_plan_tp2", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
     "genga_kick_set_stream", "genga_kick", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
@@ -30,7 +30,7 @@ STATUS_UNBOUND = 8
 class GengaKickConfig(C.Structure):
     _fields_ = [("n_massive", C.c_int32), ("n_test", C.c_int32), ("max_level", C.c_int32), ("device", C.c_int32),
                 ("pair_capacity", C.c_int64), ("G", C.c_double), ("enc_factor", C.c_double),
-                ("order_mode", C.c_int32), ("reserved", C.c_int32)]
+                ("order_mode", C.c_int32), ("tp_mode", C.c_int32)]
 
 
 class GengaKickPlan(C.Structure):
@@ -61,6 +61,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         vp, i32, i64, d = C.c_void_p, C.c_int32, C.c_int64, C.c_double
         L.genga_kick_make_plan.argtypes = [i32, i32, i32, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_make_plan_tp2.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
         L.genga_kick_plan_cta_range.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i64), C.POINTER(i64)]
         L.genga_kick_plan_iblock_ctas.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i32), C.POINTER(i32)]
         L.genga_kick_init.argtypes = [C.POINTER(GengaKickConfig), C.POINTER(vp)]
@@ -105,6 +106,14 @@ def make_plan(n_massive: int, n_test: int, level: int, num_sms: int) -> GengaKic
     return plan
 
 
+def make_plan_tp2(n_massive: int, n_test: int, num_sms: int) -> GengaKickPlan:
+    plan = GengaKickPlan()
+    rc = lib().genga_kick_make_plan_tp2(n_massive, n_test, num_sms, C.byref(plan))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
+    return plan
+
+
 def plan_cta_range(plan: GengaKickPlan, cta: int):
     t0, t1 = C.c_int64(), C.c_int64()
     rc = lib().genga_kick_plan_cta_range(C.byref(plan), cta, C.byref(t0), C.byref(t1))
@@ -130,9 +139,9 @@ class GengaKick:
     kick_host()), float64 / int32, C-contiguous, laid out as include/genga_kick.h states."""
 
     def __init__(self, n_massive, n_test=0, max_level=0, pair_capacity=1 << 20, G=1.0, enc_factor=1.0, device=0,
-                 order_mode=0):
+                 order_mode=0, tp_mode=1):
         self.cfg = GengaKickConfig(int(n_massive), int(n_test), int(max_level), int(device), int(pair_capacity),
-                                   float(G), float(enc_factor), int(order_mode), 0)
+                                   float(G), float(enc_factor), int(order_mode), int(tp_mode))
         self.n = int(n_massive) + int(n_test)
         self._ctx = C.c_void_p()
         rc = lib().genga_kick_init(C.byref(self.cfg), C.byref(self._ctx))

@@ -47,6 +47,7 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
         return GENGA_KICK_E_SIZE;
     if (cfg->max_level < 0 || cfg->max_level > 62) return GENGA_KICK_E_LEVEL;
     if (cfg->order_mode < GENGA_KICK_ORDER_AUTO || cfg->order_mode > GENGA_KICK_ORDER_SORTED) return GENGA_KICK_E_SIZE;
+    if (cfg->tp_mode < 0 || cfg->tp_mode > 2) return GENGA_KICK_E_SIZE;
 
     genga_kick_ctx* ctx = new (std::nothrow) genga_kick_ctx();
     if (!ctx) return GENGA_KICK_E_NOMEM;
@@ -97,6 +98,13 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
             if ((e = cudaMalloc(&ctx->counts, nc * sizeof(int))) != cudaSuccess) goto cuda_error;
         }
         if ((e = cudaMalloc(&ctx->partial, (size_t)max_partial * sizeof(double))) != cudaSuccess) goto cuda_error;
+        ctx->tp2 = cfg->tp_mode == 2 && cfg->n_test > 0 && cfg->n_massive > 0;
+        if (ctx->tp2) {
+            rc = genga_kick_make_plan_tp2(cfg->n_massive, cfg->n_test, ctx->num_sms, &ctx->plan_tp2);
+            if (rc != GENGA_KICK_OK) goto fail;
+            if ((e = cudaMalloc(&ctx->partial2, (size_t)std::max<int64_t>(ctx->plan_tp2.partial_doubles, 1) * sizeof(double))) != cudaSuccess)
+                goto cuda_error;
+        }
         ctx->cand_capacity = std::min<int64_t>(std::max<int64_t>(GENGA_CAND_PER_BODY * N, GENGA_CAND_MIN), GENGA_CAND_MAX);
         if ((e = cudaMalloc(&ctx->cand, (size_t)ctx->cand_capacity * sizeof(int2))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->ncand, sizeof(int))) != cudaSuccess) goto cuda_error;
@@ -180,6 +188,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         kp.cblo = ctx->cblo; kp.cbhi = ctx->cbhi;
         kp.rcrit = rcrit;
         kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
+        kp.react = ctx->tp2 && changeover_level > 0 ? 1 : 0; kp.j_rec0 = 0; kp.force_only = 0;
         kp.n_j_tiles = pl.n_j_tiles; kp.n_ctas = pl.n_ctas; kp.max_segs = pl.max_segs; kp.n_tiles = pl.n_tiles;
         kp.partial = ctx->partial;
         kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
@@ -200,6 +209,15 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             ctx->ev_set[changeover_level] = true;
         }
         ctx->launches++;
+        if (ctx->tp2 && changeover_level == 0 && ctx->plan_tp2.n_ctas > 0) {
+            // TP 2, far field of the massive bodies' sum over the semi-active particles (at level >= 1 it is 0)
+            const genga_kick_plan& p2 = ctx->plan_tp2;
+            genga::KickParams k2 = kp;
+            k2.n_j_tiles = p2.n_j_tiles; k2.n_ctas = p2.n_ctas; k2.max_segs = p2.max_segs; k2.n_tiles = p2.n_tiles;
+            k2.partial = ctx->partial2; k2.j_rec0 = pl.m_pad; k2.force_only = 1;
+            GK_CUDA(ctx, dispatch_kick(p2, k2, st));
+            ctx->launches++;
+        }
         // exact path: one candidate per thread, grid-stride over the list the pair loop has written
         genga::exact_kernel<<<4 * ctx->num_sms, 256, 0, st>>>(kp);
         GK_CUDA(ctx, cudaGetLastError());
@@ -207,9 +225,14 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
     }
     {
         // level >= 1: no partial segments (n_ctas = 0), every term comes from the exact path
+        const genga_kick_plan& p2 = ctx->plan_tp2;
+        const bool second = ctx->tp2 && changeover_level == 0 && p2.n_ctas > 0;
         genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(ctx->partial, ctx->ridx, n_rec, N, pl.i_block, pl.n_j_tiles,
                                                                   pl.n_tiles, changeover_level == 0 ? pl.n_ctas : 0,
-                                                                  pl.max_segs, dt, ctx->fx,
+                                                                  pl.max_segs, ctx->partial2, pl.m_pad,
+                                                                  second ? p2.i_block : 1, second ? p2.n_j_tiles : 1,
+                                                                  second ? p2.n_tiles : 1, second ? p2.n_ctas : 0,
+                                                                  second ? p2.max_segs : 1, dt, ctx->fx,
                                                                   ctx->touched, ctx->status, out_acc, vel);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
@@ -402,7 +425,7 @@ extern "C" int genga_kick_free(genga_kick_ctx* ctx)
 {
     if (!ctx) return GENGA_KICK_OK;
     void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
-                    ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
+                    ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->partial2, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs,
                     ctx->psum_partial, ctx->psum_ticket, ctx->step_rcrit, ctx->grp_label, ctx->grp_flag,
                     ctx->grp_keys_a, ctx->grp_keys_b, ctx->grp_vals_a, ctx->grp_vals_b, ctx->grp_counts};

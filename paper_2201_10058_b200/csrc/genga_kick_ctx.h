@@ -11,6 +11,9 @@ struct genga_kick_ctx {
     int num_sms;
     cudaStream_t stream;
     genga_kick_plan* plans;        // one per level 0..max_level
+    genga_kick_plan plan_tp2;      // TP 2: second pass of the level-0 kick (massive i x semi-active j)
+    bool tp2;
+    double* partial2;              // its partial sums
     // scratch (device)
     double2* rxy;
     double2* rzm;

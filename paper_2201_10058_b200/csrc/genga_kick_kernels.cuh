@@ -36,6 +36,12 @@ struct KickParams {
     // the caller's arrays (read by the exact per-pair path only)
     const double* __restrict__ rcrit;  // [L+1][N]
     int N, n_massive, L;
+    int react;                         // TP 2 at level >= 1: exact_kernel also adds the reaction of a semi-active
+                                       // particle i on the massive body j (near_kernel's pair filter is symmetric)
+    int j_rec0;                        // record of the first j-tile (0; m_pad in the second pass of TP 2)
+    int force_only;                    // second pass of TP 2 at level 0 (massive i x semi-active j): candidates are
+                                       // queued as (i, ~j): exact_kernel adds the force on i and leaves the encounter
+                                       // bookkeeping to the first pass, which meets the same pair from the particle's side
     double f;                          // enc_factor
     // decomposition (genga_kick_plan)
     int n_j_tiles, n_ctas, max_segs;
@@ -148,6 +154,8 @@ __device__ __forceinline__ double changeover_K(double r, double rc)
 
 struct ExactResult {
     double s;     // G m_j W_L / r^3 (0 if the pair contributes nothing)
+    double W;     // W_L
+    double r3;    // r^2 * r
     int enc;      // 1 if (i, j) is an encounter pair
 };
 
@@ -160,6 +168,8 @@ __device__ __noinline__ ExactResult exact_pair(const double* __restrict__ rcrit,
 {
     ExactResult out;
     out.s = 0.0;
+    out.W = 0.0;
+    out.r3 = 1.0;
     out.enc = 0;
     const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
     if (!(r2 > 0.0)) {                                             // coincident distinct bodies
@@ -177,7 +187,9 @@ __device__ __noinline__ ExactResult exact_pair(const double* __restrict__ rcrit,
         W = __dmul_rn(W, __dsub_rn(1.0, changeover_K(r, rck)));
     }
     W = __dmul_rn(W, changeover_K(r, rcL));
-    if (W != 0.0) out.s = __ddiv_rn(__dmul_rn(gmj, W), __dmul_rn(r2, r));
+    out.W = W;
+    out.r3 = __dmul_rn(r2, r);
+    if (W != 0.0) out.s = __ddiv_rn(__dmul_rn(gmj, W), out.r3);
     return out;
 }
 
@@ -469,7 +481,9 @@ __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
         int lo = 0, hi = 0;
         if (c < n) {
             const int2 e = p.cand[c];
-            const int ir = e.x, jr = e.y;
+            const int ir = e.x;
+            const bool force_only = ir >= 0 && e.y < 0;                                     // (i, ~j): see KickParams
+            const int jr = force_only ? ~e.y : e.y;
             const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;    // (-1, -1): empty slot
             if (ir != jr && bi >= 0 && bj >= 0) {
                 const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
@@ -482,7 +496,17 @@ __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
                     fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
                     p.touched[ir] = 1;
                 }
-                if (r.enc && p.out_npairs) {
+                if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
+                    // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
+                    // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
+                    const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
+                    unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
+                    fx_add(accj, -__dmul_rn(si, dx), p.status);
+                    fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
+                    fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+                    p.touched[jr] = 1;
+                }
+                if (r.enc && p.out_npairs && !force_only) {
                     atomicAdd(p.out_npairs + bi, 1);
                     if (bi >= p.n_massive) {               // test particle i, massive j
                         atomicAdd(p.out_npairs + bj, 1);
@@ -556,11 +580,12 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         if (g >= STAGES) mbar_wait(&empty[s], (uint32_t)((g / STAGES - 1) & 1));
         const int jt = (int)((t0 + g) % p.n_j_tiles);
         mbar_expect_tx(&full[s], TILE_BYTES);
-        bulk_g2s(st[s].xy, p.rxy + (size_t)jt * JT, JT * 16, &full[s]);
-        bulk_g2s(st[s].zm, p.rzm + (size_t)jt * JT, JT * 16, &full[s]);
-        bulk_g2s(st[s].blo, p.cblo + (size_t)jt * NG, NG * 16, &full[s]);
-        bulk_g2s(st[s].bhi, p.cbhi + (size_t)jt * NG, NG * 16, &full[s]);
-        bulk_g2s(st[s].cf, p.cfw + (size_t)jt * NCH, NCH * 4, &full[s]);
+        const size_t j0 = (size_t)p.j_rec0 + (size_t)jt * JT;          // a multiple of 64: every offset 16-byte aligned
+        bulk_g2s(st[s].xy, p.rxy + j0, JT * 16, &full[s]);
+        bulk_g2s(st[s].zm, p.rzm + j0, JT * 16, &full[s]);
+        bulk_g2s(st[s].blo, p.cblo + j0 / GENGA_GROUP, NG * 16, &full[s]);
+        bulk_g2s(st[s].bhi, p.cbhi + j0 / GENGA_GROUP, NG * 16, &full[s]);
+        bulk_g2s(st[s].cf, p.cfw + j0 / GENGA_CHUNK, NCH * 4, &full[s]);
     };
     const int n_it = (int)(t1 - t0);
     if (tid == 0)
@@ -656,7 +681,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                     const int b = __ffs(todo) - 1;
                     todo &= todo - 1;
                     const bool mine = (tm >> b) & 1u;
-                    push_candidates(p, cc, mine, ib * IB + woff + (b % IPT) * 32, jt * JT + jj + b / IPT);
+                    const int jrec = p.j_rec0 + jt * JT + jj + b / IPT;
+                    push_candidates(p, cc, mine, ib * IB + woff + (b % IPT) * 32, p.force_only ? ~jrec : jrec);
 #ifdef GENGA_TRACE
                     tr_cand += __popc(__ballot_sync(0xffffffffu, mine));
 #endif
@@ -757,7 +783,9 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, int n_rec, int N, int IB,
-              int n_j_tiles, long long n_tiles, int n_ctas, int max_segs, double dt,
+              int n_j_tiles, long long n_tiles, int n_ctas, int max_segs,
+              const double* __restrict__ partial2, int m_pad, int IB2, int n_j_tiles2, long long n_tiles2, int n_ctas2,
+              int max_segs2, double dt,
               unsigned long long* __restrict__ fx, int* __restrict__ touched, int* __restrict__ status,
               double* __restrict__ out_acc, double* __restrict__ vel)
 {
@@ -776,6 +804,18 @@ reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, 
         a0 = __dadd_rn(a0, q[0]);
         a1 = __dadd_rn(a1, q[IB]);
         a2 = __dadd_rn(a2, q[2 * (size_t)IB]);
+    }
+    if (n_ctas2 > 0 && r < m_pad) {                        // TP 2: the massive body's sum over the semi-active particles
+        const int ib2 = r / IB2, off2 = r - ib2 * IB2;
+        const long long ta2 = (long long)ib2 * n_j_tiles2, tb2 = ta2 + n_j_tiles2 - 1;
+        const int c_first2 = plan_tile_owner(ta2, n_tiles2, n_ctas2), c_last2 = plan_tile_owner(tb2, n_tiles2, n_ctas2);
+        for (int c = c_first2; c <= c_last2; c++) {
+            const int seg = ib2 - (int)(plan_tile_begin(c, n_tiles2, n_ctas2) / n_j_tiles2);
+            const double* q = partial2 + ((size_t)c * max_segs2 + seg) * 3 * IB2 + off2;
+            a0 = __dadd_rn(a0, q[0]);
+            a1 = __dadd_rn(a1, q[IB2]);
+            a2 = __dadd_rn(a2, q[2 * (size_t)IB2]);
+        }
     }
     if (touched[r]) {                                      // the exact path's terms (fixed point, see fx_add)
         touched[r] = 0;

@@ -16,46 +16,74 @@ static int64_t cta_t0(const genga_kick_plan* p, int64_t c)
     return plan_tile_begin(c, p->n_tiles, p->n_ctas);
 }
 
+// Tile decomposition of an (n_i records) x (n_j records) pair matrix: picks the variant, fills the
+// tile, CTA and partial-sum fields of *p (m_pad and n_rec are the caller's business).
+static void fill_tiles(genga_kick_plan* p, int64_t n_i, int64_t n_j, int32_t num_sms)
+{
+    const genga_variant* vars = GENGA_VARIANTS;
+    for (int v = 0; v < GENGA_N_VARIANTS; v++) {
+        p->threads = vars[v].threads;
+        p->i_per_thread = vars[v].i_per_thread;
+        p->i_block = p->threads * p->i_per_thread;
+        p->j_tile = vars[v].j_tile;
+        p->n_i_blocks = (int32_t)((n_i + p->i_block - 1) / p->i_block);
+        p->n_j_tiles = (int32_t)((n_j + p->j_tile - 1) / p->j_tile);
+        p->n_tiles = (int64_t)p->n_i_blocks * p->n_j_tiles;
+        p->n_ctas = num_sms * vars[v].ctas_per_sm;
+        if (p->n_tiles >= (int64_t)GENGA_MIN_TILES_PER_CTA * p->n_ctas) break;
+    }
+    if (p->n_tiles < p->n_ctas) p->n_ctas = (int32_t)p->n_tiles;      // 0 CTAs when there is nothing to do
+
+    // most i-blocks any CTA touches
+    int32_t max_segs = 1;
+    if (p->n_j_tiles > 0) {
+        for (int64_t c = 0; c < p->n_ctas; c++) {
+            const int64_t t0 = cta_t0(p, c), t1 = cta_t0(p, c + 1);
+            if (t1 <= t0) continue;
+            const int32_t segs = (int32_t)((t1 - 1) / p->n_j_tiles - t0 / p->n_j_tiles + 1);
+            if (segs > max_segs) max_segs = segs;
+        }
+    }
+    p->max_segs = max_segs;
+    p->partial_doubles = (int64_t)p->n_ctas * p->max_segs * 3 * p->i_block;
+}
+
+static int plan_records(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* p, int64_t* n_i)
+{
+    const int64_t N = (int64_t)n_massive + (int64_t)n_test;
+    if (n_massive < 0 || n_test < 0 || N <= 0 || N > GENGA_MAX_BODIES || num_sms <= 0) return GENGA_KICK_E_SIZE;
+    // records: massive bodies padded to a multiple of GENGA_M_ALIGN, then the test particles
+    p->m_pad = (int32_t)(((int64_t)n_massive + GENGA_M_ALIGN - 1) / GENGA_M_ALIGN * GENGA_M_ALIGN);
+    *n_i = n_test > 0 ? (int64_t)p->m_pad + n_test : (int64_t)n_massive;
+    p->n_rec = (*n_i + GENGA_REC_ALIGN - 1) / GENGA_REC_ALIGN * GENGA_REC_ALIGN;
+    if (p->n_rec < p->m_pad) p->n_rec = (p->m_pad + GENGA_REC_ALIGN - 1) / GENGA_REC_ALIGN * GENGA_REC_ALIGN;
+    return GENGA_KICK_OK;
+}
+
 extern "C" int genga_kick_make_plan(int32_t n_massive, int32_t n_test, int32_t level, int32_t num_sms,
                                     genga_kick_plan* plan)
 {
     if (!plan) return GENGA_KICK_E_NULL;
     if (level < 0) return GENGA_KICK_E_LEVEL;
-    const int64_t N = (int64_t)n_massive + (int64_t)n_test;
-    if (n_massive < 0 || n_test < 0 || N <= 0 || N > GENGA_MAX_BODIES || num_sms <= 0) return GENGA_KICK_E_SIZE;
-
-    const genga_variant* vars = GENGA_VARIANTS;     // level >= 1 only uses m_pad and n_rec of the plan
     genga_kick_plan p;
-    for (int v = 0; v < GENGA_N_VARIANTS; v++) {
-        p.threads = vars[v].threads;
-        p.i_per_thread = vars[v].i_per_thread;
-        p.i_block = p.threads * p.i_per_thread;
-        p.j_tile = vars[v].j_tile;
-        // records: massive bodies padded to a multiple of GENGA_M_ALIGN, then the test particles
-        p.m_pad = (int32_t)(((int64_t)n_massive + GENGA_M_ALIGN - 1) / GENGA_M_ALIGN * GENGA_M_ALIGN);
-        const int64_t n_i = n_test > 0 ? (int64_t)p.m_pad + n_test : (int64_t)n_massive;
-        p.n_rec = (n_i + GENGA_REC_ALIGN - 1) / GENGA_REC_ALIGN * GENGA_REC_ALIGN;
-        if (p.n_rec < p.m_pad) p.n_rec = (p.m_pad + GENGA_REC_ALIGN - 1) / GENGA_REC_ALIGN * GENGA_REC_ALIGN;
-        p.n_i_blocks = (int32_t)((n_i + p.i_block - 1) / p.i_block);
-        p.n_j_tiles = (n_massive + p.j_tile - 1) / p.j_tile;
-        p.n_tiles = (int64_t)p.n_i_blocks * p.n_j_tiles;
-        p.n_ctas = num_sms * vars[v].ctas_per_sm;
-        if (p.n_tiles >= (int64_t)GENGA_MIN_TILES_PER_CTA * p.n_ctas) break;
-    }
-    if (p.n_tiles < p.n_ctas) p.n_ctas = (int32_t)p.n_tiles;      // 0 CTAs when there is no massive body
+    int64_t n_i = 0;
+    const int rc = plan_records(n_massive, n_test, num_sms, &p, &n_i);
+    if (rc != GENGA_KICK_OK) return rc;
+    fill_tiles(&p, n_i, n_massive, num_sms);         // level >= 1 only uses m_pad and n_rec of the plan
+    *plan = p;
+    return GENGA_KICK_OK;
+}
 
-    // most i-blocks any CTA touches
-    int32_t max_segs = 1;
-    if (p.n_j_tiles > 0) {
-        for (int64_t c = 0; c < p.n_ctas; c++) {
-            const int64_t t0 = cta_t0(&p, c), t1 = cta_t0(&p, c + 1);
-            if (t1 <= t0) continue;
-            const int32_t segs = (int32_t)((t1 - 1) / p.n_j_tiles - t0 / p.n_j_tiles + 1);
-            if (segs > max_segs) max_segs = segs;
-        }
-    }
-    p.max_segs = max_segs;
-    p.partial_doubles = (int64_t)p.n_ctas * p.max_segs * 3 * p.i_block;
+// TP 2: the second, transposed pass of the level-0 kick -- i over the massive
+// records [0, n_massive), j over the test-particle records [m_pad, m_pad + n_test).
+extern "C" int genga_kick_make_plan_tp2(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan)
+{
+    if (!plan) return GENGA_KICK_E_NULL;
+    genga_kick_plan p;
+    int64_t n_i = 0;
+    const int rc = plan_records(n_massive, n_test, num_sms, &p, &n_i);
+    if (rc != GENGA_KICK_OK) return rc;
+    fill_tiles(&p, n_massive, n_test, num_sms);
     *plan = p;
     return GENGA_KICK_OK;
 }

@@ -15,7 +15,8 @@ class GpuResult:
     launches: int = 0
 
 
-def run_gpu(ki, level=None, capacity=1 << 20, with_vel=False, host=False, kick=None, rcrit=None, order_mode=0):
+def run_gpu(ki, level=None, capacity=1 << 20, with_vel=False, host=False, kick=None, rcrit=None, order_mode=0,
+            tp_mode=1):
     import torch
     from paper_2201_10058_b200 import GengaKick
     level = ki.level if level is None else level
@@ -23,7 +24,7 @@ def run_gpu(ki, level=None, capacity=1 << 20, with_vel=False, host=False, kick=N
     own = kick is None
     if own:
         kick = GengaKick(ki.n_massive, ki.n_test, max_level=level, pair_capacity=capacity, G=ki.G,
-                         enc_factor=ki.enc_factor, order_mode=order_mode)
+                         enc_factor=ki.enc_factor, order_mode=order_mode, tp_mode=tp_mode)
     dev = "cpu" if host else "cuda"
     t = lambda a, dt=torch.float64: torch.from_numpy(np.array(a, copy=True)).to(dt).to(dev).contiguous()
     pos, mass = t(ki.pos), t(ki.mass)

@@ -64,6 +64,21 @@ def test_config4_full(oracle_mod):
     assert np.array_equal(want, gpu.counts)
 
 
+def test_config4_full_tp2(oracle_mod):
+    """Config 4's shape with semi-active particles that HAVE mass (TP 2): the massive bodies also
+    sum over the 1,048,576 particles (the transposed rectangular kick)."""
+    ki = gi.make_config(4)
+    u = gi.uniforms(77, 0, ki.n_test)
+    ki.mass = ki.mass.copy()
+    ki.mass[ki.n_massive:] = 1e-12 * (0.5 + u)
+    gpu = run_gpu(ki, level=0, capacity=CAPACITY, order_mode=0, tp_mode=2)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=0, G=ki.G, maxp=256, tp_mode=2)
+    assert gpu.status == 0
+    compare(gpu, orc, ki.n_massive, tol=TOL)
+    p = (ki.mass * gpu.acc).sum(axis=1)
+    assert np.all(np.abs(p) <= TOL * (ki.mass * orc.S).sum(axis=1))
+
+
 def test_config1_hundred_kicks(oracle_mod):
     """N = 8192, 100 kicks separated by an oracle-matched heliocentric drift: both sides see the
     same state at every step (the harness advances it with the ORACLE's acceleration), the

@@ -198,3 +198,30 @@ def test_internal_order_is_invisible(oracle_mod):
         assert np.array_equal(b.acc, c.acc)                      # auto sorts at this size
         orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, level=level, G=ki.G)
         assert np.all(np.abs(a.acc - b.acc) <= 2e-13 * orc.S)
+
+
+# ------------------------------------------------------------------ TP 2
+def _with_tp_masses(ki, seed=11):
+    u = gi.uniforms(seed, 0, ki.n_test)
+    ki.mass = ki.mass.copy()
+    ki.mass[ki.n_massive:] = 1e-11 * (0.5 + u)
+    ki.mass[ki.n_massive::7] = 0.0                        # some stay massless
+    return ki
+
+
+@pytest.mark.parametrize("nm,nt,level", [(300, 5000, 0), (2048, 20000, 0), (1, 100, 0), (257, 1, 0), (700, 3000, 1),
+                                         (5000, 300, 0)])
+def test_tp2_semi_active_particles_act_on_massive_bodies(oracle_mod, nm, nt, level):
+    import tests.gpu_harness as h
+    ki = _with_tp_masses(gi.make_config(4, n=nm, n_test=nt, level=level))
+    gpu = run_gpu(ki, level=level, tp_mode=2)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, nm, nt, level=level, G=ki.G, tp_mode=2)
+    assert gpu.status == 0
+    compare(gpu, orc, nm, tol=TOL)
+    # momentum over ALL bodies (every term of Fig. 14's right panel has its reaction)
+    p = (ki.mass * gpu.acc).sum(axis=1)
+    assert np.all(np.abs(p) <= TOL * (ki.mass * orc.S).sum(axis=1))
+    # TP 1 on the same input: the particles' accelerations are the same, the massive bodies' differ
+    one = run_gpu(ki, level=level, tp_mode=1)
+    assert np.array_equal(one.acc[:, nm:], gpu.acc[:, nm:])
+    assert np.array_equal(sorted_pairs(one.pairs), sorted_pairs(gpu.pairs))

@@ -111,6 +111,26 @@ def test_plan_covers_every_tile_once(built, nm, nt, level):
         assert meets == list(range(a, b + 1))
 
 
+@pytest.mark.parametrize("nm,nt", [(2048, 1048576), (257, 1), (1, 100), (300, 5000), (16, 65520)])
+def test_tp2_plan_covers_every_tile_once(built, nm, nt):
+    """TP 2's second pass: massive bodies (i) x semi-active particles (j), same tile / CTA scheme."""
+    sms = 148
+    p = g.make_plan_tp2(nm, nt, sms)
+    d, d0 = p.as_dict(), g.make_plan(nm, nt, 0, sms).as_dict()
+    assert d["m_pad"] == d0["m_pad"] and d["n_rec"] == d0["n_rec"]
+    assert d["n_i_blocks"] * d["i_block"] >= nm and d["n_i_blocks"] * d["i_block"] <= d["n_rec"]
+    assert d["n_j_tiles"] * d["j_tile"] >= nt and d["m_pad"] + d["n_j_tiles"] * d["j_tile"] <= d["n_rec"]
+    assert d["n_tiles"] == d["n_i_blocks"] * d["n_j_tiles"] and d["m_pad"] % 64 == 0
+    prev, sizes = 0, []
+    for c in range(d["n_ctas"]):
+        t0, t1 = g.plan_cta_range(p, c)
+        assert t0 == prev and t1 >= t0
+        prev = t1
+        sizes.append(t1 - t0)
+    assert prev == d["n_tiles"] and max(sizes) - min(sizes) <= 1
+    assert d["partial_doubles"] == d["n_ctas"] * d["max_segs"] * 3 * d["i_block"]
+
+
 def test_plan_errors(built):
     with pytest.raises(g.GengaKickError) as e:
         g.make_plan(0, 0, 0, 148)
