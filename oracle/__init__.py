@@ -5,9 +5,10 @@ The arithmetic lives in genga_kick_oracle.c (plain C, binary64 per pair, long do
 genga_step_oracle.c (Rcrit / HC / FG, long double), genga_group_oracle.c (grouping); this
 module is argument marshalling via ctypes.  It imports nothing from the CUDA package.
 """
-from .oracle import (OracleResult, K_of_y, K, weight, weight_bs, kick, pair_set, num_threads, lib_path)
+from .oracle import (OracleResult, ListKickResult, K_of_y, K, weight, weight_bs, kick, kick_list, pair_set, num_threads,
+                     lib_path)
 
 from . import step
 from . import group
 
-__all__ = ["step", "group", "OracleResult", "K_of_y", "K", "weight", "weight_bs", "kick", "pair_set", "num_threads", "lib_path"]
+__all__ = ["step", "group", "OracleResult", "K_of_y", "K", "weight", "weight_bs", "kick", "kick_list", "ListKickResult", "pair_set", "num_threads", "lib_path"]

@@ -176,3 +176,65 @@ int genga_oracle_kick(int32_t n_massive, int32_t n_test, int32_t L, double G, do
     return genga_oracle_kick_tp(n_massive, n_test, 1, L, G, f, pos, mass, rcrit, rows, nrows, acc, S, count,
                                 partners, maxp, border, bcap, nborder);
 }
+
+/*
+ * KickS (App. A: "KickS ... similar to the original functions, but applied only to
+ * the relevant bodies in each symplectic level"; groupS "extracts all relevant close-encounter pairs
+ * from the upper symplectic level"): the sum of eq. 3 with the level weight W_L of eq. 62-63 over the
+ * pairs of a LIST (each unordered pair once, rows (i, j), i != j) instead of over all pairs, both
+ * directions of each pair, and the level-L pre-check of the listed pairs.
+ * Per-pair arithmetic exactly as in genga_oracle_kick_tp, from each body's own side (d = x_other - x_self).
+ * Force rules (sec. 8.1): a test particle feels massive bodies only; it acts on a massive body only
+ * if tp_mode == 2; two test particles do not interact.
+ *   acc, S [3][N] (all bodies; bodies in no pair get 0), count [N], enc [n_pairs] (1 if the pair is a
+ *   level-L encounter pair), border [n_pairs] (1 if within 1e-12 of the threshold).
+ * Since W_L = 0 for r >= rc0_ij (factor 1 - K_0), this equals the all-pairs level-L kick (L >= 1)
+ * whenever the list holds every pair with r < rc0_ij -- the pin of tests/test_oracle_pins.py.
+ * returns 0, or -1 on a coincident pair.
+ */
+int genga_oracle_kick_list(int32_t n_massive, int32_t n_test, int32_t tp_mode, int32_t L, double G, double f,
+                           const double *pos, const double *mass, const double *rcrit,
+                           const int32_t *pairs, int64_t n_pairs,
+                           double *acc, double *S, int32_t *count, int8_t *enc, int8_t *border)
+{
+    const int64_t N = (int64_t)n_massive + (int64_t)n_test;
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    long double *a = (long double *)calloc((size_t)(6 * N > 0 ? 6 * N : 1), sizeof(long double));
+    long double *s_abs = a + 3 * N;
+    int bad = 0;
+    for (int64_t i = 0; i < N; i++) count[i] = 0;
+    for (int64_t p = 0; p < n_pairs; p++) {
+        enc[p] = 0; border[p] = 0;
+        for (int side = 0; side < 2; side++) {
+            const int64_t i = pairs[2 * p + side], j = pairs[2 * p + 1 - side];      /* i feels j */
+            if (i == j) continue;
+            const double dx = x[j] - x[i];
+            const double dy = y[j] - y[i];
+            const double dz = z[j] - z[i];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            if (!(r2 > 0.0)) { bad = 1; continue; }
+            const double r = sqrt(r2);
+            const double rcL = fmax(rcrit[(int64_t)L * N + i], rcrit[(int64_t)L * N + j]);
+            const double thr = f * rcL;
+            const int both_tp = i >= n_massive && j >= n_massive;
+            if (r2 < thr * thr && !both_tp) { count[i]++; enc[p] = 1; }
+            if (fabs(r / thr - 1.0) <= 1e-12) border[p] = 1;
+            if (both_tp) continue;
+            if (j >= n_massive && tp_mode != 2) continue;             /* no force from a test particle (TP 1) */
+            double W = 1.0;
+            for (int k = 0; k < L; k++) {
+                const double rck = fmax(rcrit[(int64_t)k * N + i], rcrit[(int64_t)k * N + j]);
+                W *= (1.0 - genga_oracle_K(r, rck));
+            }
+            W *= genga_oracle_K(r, rcL);
+            if (W == 0.0) continue;
+            const double s = G * mass[j] * W / (r2 * r);
+            const double tx = s * dx, ty = s * dy, tz = s * dz;
+            a[i] += tx; a[N + i] += ty; a[2 * N + i] += tz;
+            s_abs[i] += fabs(tx); s_abs[N + i] += fabs(ty); s_abs[2 * N + i] += fabs(tz);
+        }
+    }
+    for (int64_t q = 0; q < 3 * N; q++) { acc[q] = (double)a[q]; S[q] = (double)s_abs[q]; }
+    free(a);
+    return bad ? -1 : 0;
+}

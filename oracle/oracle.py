@@ -30,6 +30,8 @@ def _L():
         lib.genga_oracle_kick.argtypes = [i32, i32, i32, d, d, p, p, p, p, i64, p, p, p, p, i32, p, i64, p]
         lib.genga_oracle_kick_tp.restype = C.c_int
         lib.genga_oracle_kick_tp.argtypes = [i32, i32, i32, i32, d, d, p, p, p, p, i64, p, p, p, p, i32, p, i64, p]
+        lib.genga_oracle_kick_list.restype = C.c_int
+        lib.genga_oracle_kick_list.argtypes = [i32, i32, i32, i32, d, d, p, p, p, p, i64, p, p, p, p, p]
         _lib = lib
     return _lib
 
@@ -109,3 +111,31 @@ def pair_set(res: OracleResult, n_massive: int) -> np.ndarray:
             out.add((i, j) if i < j else (j, i))
     arr = np.array(sorted(out), dtype=np.int32).reshape(-1, 2)
     return arr
+
+
+@dataclass
+class ListKickResult:
+    acc: np.ndarray         # [3, N]
+    S: np.ndarray           # [3, N]
+    count: np.ndarray       # [N] level-L partners among the listed pairs
+    enc: np.ndarray         # [n_pairs] bool: the pair is a level-L encounter pair
+    border: np.ndarray      # [n_pairs] bool: within 1e-12 of the threshold
+    coincident: bool
+
+
+def kick_list(pos, mass, rcrit, n_massive, n_test, pairs, level=1, G=1.0, enc_factor=1.0, tp_mode=1):
+    """KickS (App. A): the level-`level` kick over the pairs of a list + their level pre-check."""
+    n = int(n_massive) + int(n_test)
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    rcrit = np.ascontiguousarray(rcrit, dtype=np.float64).reshape(-1, n)
+    pr = np.ascontiguousarray(np.asarray(pairs, dtype=np.int32).reshape(-1, 2))
+    assert rcrit.shape[0] >= level + 1 and (pr.size == 0 or (pr.min() >= 0 and pr.max() < n))
+    acc = np.zeros((3, n)); S = np.zeros((3, n)); count = np.zeros(n, dtype=np.int32)
+    enc = np.zeros(max(len(pr), 1), dtype=np.int8); border = np.zeros(max(len(pr), 1), dtype=np.int8)
+    rc = _L().genga_oracle_kick_list(int(n_massive), int(n_test), int(tp_mode), int(level), float(G), float(enc_factor),
+                                     pos.ctypes.data, mass.ctypes.data, rcrit.ctypes.data, pr.ctypes.data, len(pr),
+                                     acc.ctypes.data, S.ctypes.data, count.ctypes.data, enc.ctypes.data,
+                                     border.ctypes.data)
+    return ListKickResult(acc=acc, S=S, count=count, enc=enc[:len(pr)].astype(bool), border=border[:len(pr)].astype(bool),
+                          coincident=(rc != 0))

@@ -385,3 +385,52 @@ def test_TP2_is_the_full_interaction_minus_tp_tp(oracle_mod):
     # and TP 1 differs from TP 2 only on the massive bodies
     r1 = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, nm, ki.n_test, G=ki.G, tp_mode=1)
     assert np.array_equal(r1.acc[:, nm:], r2.acc[:, nm:]) and not np.array_equal(r1.acc[:, :nm], r2.acc[:, :nm])
+
+
+# ---------------------------------------------------------------- KickS: the kick over a pair list (App. A)
+def test_KickS_over_the_level0_list_is_the_all_pairs_level_kick(oracle_mod):
+    """W_L = 0 for r >= rc0_ij (factor 1 - K_0 of eq. 63), so the level-L kick over the level-0 encounter list
+    (every pair with r < rc0_ij) equals the all-pairs level-L kick, and its level-L pre-check gives the same list."""
+    for cfg, n, kw in [(3, 4000, {}), (2, 3000, {}), (4, 300, dict(n_test=4000))]:
+        ki = gi.make_config(cfg, n=n, level=2, **kw)
+        top = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=0, G=ki.G, maxp=128)
+        lst = oracle_mod.pair_set(top, ki.n_massive)
+        assert len(lst) > 10
+        for L in (1, 2):
+            full = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=L, G=ki.G, maxp=128)
+            ks = oracle_mod.kick_list(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, lst, level=L, G=ki.G)
+            assert np.all(np.abs(ks.acc - full.acc) <= 4 * U * full.S) and np.all(np.abs(ks.S - full.S) <= 4 * U * full.S)
+            assert np.array_equal(ks.count, full.count)
+            want = {tuple(p) for p in oracle_mod.pair_set(full, ki.n_massive).tolist()}
+            assert {tuple(p) for p in lst[ks.enc].tolist()} == want
+
+
+def test_KickS_all_pairs_list_at_level0_and_closed_form(oracle_mod):
+    ki = gi.make_config(0, n=60)
+    every = np.array([(i, j) for i in range(60) for j in range(i + 1, 60)], dtype=np.int32)
+    full = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, 60, 0, level=0, G=ki.G)
+    ks = oracle_mod.kick_list(ki.pos, ki.mass, ki.rcrit, 60, 0, every, level=0, G=ki.G)
+    assert np.all(np.abs(ks.acc - full.acc) <= 4 * U * full.S) and np.array_equal(ks.count, full.count)
+    # two bodies in mid-band of K: a = (1/2) G m / r^2 each way, momentum exactly balanced in the terms
+    rc, m = 0.03, np.array([2e-7, 5e-8])
+    pos = np.array([[0.0, 0.55 * rc], [0.0, 0.0], [0.0, 0.0]])
+    ks = oracle_mod.kick_list(pos, m, np.full((1, 2), rc), 2, 0, [[0, 1]], level=0, G=G)
+    r = 0.55 * rc
+    assert abs(ks.acc[0, 0] - 0.5 * G * m[1] / r ** 2) <= 8 * U * ks.S[0, 0]
+    assert abs(ks.acc[0, 1] + 0.5 * G * m[0] / r ** 2) <= 8 * U * ks.S[0, 1]
+    assert ks.enc.tolist() == [True] and ks.count.tolist() == [1, 1]
+
+
+def test_KickS_test_particle_rules(oracle_mod):
+    ki = gi.make_config(4, n=100, n_test=2000)
+    ki.mass = ki.mass.copy(); ki.mass[100:] = 1e-12
+    top = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, 100, 2000, level=0, G=ki.G)
+    lst = oracle_mod.pair_set(top, 100)
+    for mode in (1, 2):
+        full = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, 100, 2000, level=0, G=ki.G, tp_mode=mode)
+        ks = oracle_mod.kick_list(ki.pos, ki.mass, ki.rcrit, 100, 2000, lst, level=0, G=ki.G, tp_mode=mode)
+        # level 0 over a partial list: only the listed pairs' terms -- compare with the all-pairs kick restricted to r < rc
+        assert np.array_equal(ks.count, full.count)
+        if mode == 2:
+            p = (ki.mass * ks.acc).sum(axis=1)
+            assert np.all(np.abs(p) <= 8 * U * (ki.mass * ks.S).sum(axis=1))
