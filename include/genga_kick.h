@@ -150,6 +150,28 @@ int genga_kick_host(genga_kick_ctx* ctx,
                     int32_t changeover_level, double dt,
                     double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
 
+/*
+ * KickS (App. A: "KickS ... similar to the original functions, but applied only to
+ * the relevant bodies in each symplectic level"; groupS "extracts all relevant close-encounter pairs
+ * from the upper symplectic level"): the kick of level `changeover_level` over the pairs of a LIST
+ * instead of over all pairs, plus the level pre-check of the listed pairs:
+ *     a_i = sum over listed pairs {i, j} of  G m_j W_L(r_ij) (x_j - x_i) / r_ij^3      (both members of a pair)
+ *     out_pairs / out_npairs: the listed pairs with r_ij^2 < (f rcL_ij)^2, as genga_kick writes them
+ * Since W_L = 0 for r >= rc0_ij (L >= 1), this equals genga_kick at level L whenever the list holds
+ * every pair with r < rc0_ij -- e.g. the list genga_kick wrote at level 0 with enc_factor >= 1 for the
+ * same positions -- at a cost proportional to the list instead of N^2.
+ *   in_pairs    [in_pair_rows][2] int32 device, each unordered pair once (the caller's indices)
+ *   in_n_pairs  device pointer to ONE int32: number of listed pairs (clipped to in_pair_rows), e.g.
+ *               out_npairs + N of the call that wrote in_pairs
+ *   out_pairs, out_npairs: distinct from in_pairs / in_n_pairs.  Other arguments as genga_kick.
+ * Bodies in no listed pair get a = 0.  Semi-active particles: as genga_kick (tp_mode).
+ * A row with an index outside [0, N) or i == j is ignored and sets GENGA_KICK_STATUS_BAD_PAIR (16).
+ * Errors: E_NULL, E_ALIGN, E_SIZE (in_pair_rows < 0), E_LEVEL, E_CUDA.
+ */
+int genga_kick_list(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
+                    int32_t changeover_level, double dt, const int32_t* in_pairs, const int32_t* in_n_pairs,
+                    int64_t in_pair_rows, double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
+
 /* Plan the context uses at `changeover_level` (what genga_kick will launch). */
 int genga_kick_get_plan(const genga_kick_ctx* ctx, int32_t changeover_level, genga_kick_plan* plan);
 

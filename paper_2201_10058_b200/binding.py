@@ -15,7 +15,7 @@ ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 
 EXPORTS = (
     "genga_kick_make_plan", "genga_kick_make_plan_tp2", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
-    "genga_kick_set_stream", "genga_kick", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
+    "genga_kick_set_stream", "genga_kick", "genga_kick_list", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
 )
@@ -67,6 +67,7 @@ def lib():
         L.genga_kick_init.argtypes = [C.POINTER(GengaKickConfig), C.POINTER(vp)]
         L.genga_kick_set_stream.argtypes = [vp, vp]
         L.genga_kick.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, vp]
+        L.genga_kick_list.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, i64, vp, vp, vp]
         L.genga_kick_host.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, vp]
         L.genga_kick_get_plan.argtypes = [vp, i32, C.POINTER(GengaKickPlan)]
         L.genga_kick_status.argtypes = [vp, C.POINTER(i32)]
@@ -161,6 +162,12 @@ class GengaKick:
     def kick(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
         self._check(lib().genga_kick(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit), int(changeover_level),
                                      float(dt), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs)))
+
+    def kick_list(self, pos, vel, mass, rcrit, changeover_level, dt, in_pairs, in_n_pairs, in_pair_rows, out_acc,
+                  out_pairs, out_npairs):
+        self._check(lib().genga_kick_list(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit), int(changeover_level),
+                                          float(dt), _ptr(in_pairs), _ptr(in_n_pairs), int(in_pair_rows), _ptr(out_acc),
+                                          _ptr(out_pairs), _ptr(out_npairs)))
 
     def kick_host(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
         self._check(lib().genga_kick_host(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit),

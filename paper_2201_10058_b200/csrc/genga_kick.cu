@@ -240,6 +240,37 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
     return GENGA_KICK_OK;
 }
 
+extern "C" int genga_kick_list(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
+                               int32_t changeover_level, double dt, const int32_t* in_pairs, const int32_t* in_n_pairs,
+                               int64_t in_pair_rows, double* out_acc, int32_t* out_pairs, int32_t* out_npairs)
+{
+    if (!ctx || !pos || !mass || !rcrit || !in_n_pairs || !out_npairs) return GENGA_KICK_E_NULL;
+    if (!out_acc && !vel) return GENGA_KICK_E_NULL;
+    if (!out_pairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
+    if (in_pair_rows < 0) return GENGA_KICK_E_SIZE;
+    if (!in_pairs && in_pair_rows > 0) return GENGA_KICK_E_NULL;
+    if (misaligned(pos) || misaligned(vel) || misaligned(mass) || misaligned(rcrit) || misaligned(out_acc) ||
+        misaligned(out_pairs) || misaligned(out_npairs) || misaligned(in_pairs))
+        return GENGA_KICK_E_ALIGN;
+    if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
+    const int N = (int)ctx->N;
+    cudaStream_t st = ctx->stream;
+    genga::KickParams kp = {};
+    kp.rcrit = rcrit;
+    kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
+    kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
+    kp.status = ctx->status;
+    kp.fx = ctx->fx; kp.touched = ctx->touched;
+    GK_CUDA(ctx, cudaMemsetAsync(out_npairs, 0, ((size_t)N + 1) * sizeof(int32_t), st));
+    const int blocks = (int)std::min<int64_t>(std::max<int64_t>((in_pair_rows + 255) / 256, 1), 8 * ctx->num_sms);
+    genga::list_kick_kernel<<<blocks, 256, 0, st>>>(kp, pos, mass, ctx->cfg.G, reinterpret_cast<const int2*>(in_pairs),
+                                                    in_n_pairs, in_pair_rows, ctx->cfg.tp_mode == 2 ? 1 : 0);
+    genga::list_reduce_kernel<<<(N + 255) / 256, 256, 0, st>>>(ctx->fx, ctx->touched, N, dt, ctx->status, out_acc, vel);
+    GK_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 2;
+    return GENGA_KICK_OK;
+}
+
 namespace {
 template <typename T>
 int ensure(genga_kick_ctx* ctx, T** p, size_t count)

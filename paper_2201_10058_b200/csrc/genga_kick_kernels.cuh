@@ -778,6 +778,94 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
 }
 
 // ---------------------------------------------------------------------------------------------
+// KickS (App. A): the level-L kick "applied only to the relevant bodies" -- over the
+// pairs of a LIST (the encounter list of the level above, rows (i, j) in the caller's indices) instead
+// of over all pairs.  One thread per listed pair evaluates it once (exact_pair: unfused IEEE, the
+// definition's order) and adds the two terms, each with the bits its own side would compute
+// (d -> -d, r^2 unchanged), to the bodies' fixed-point accumulators -- here indexed by BODY, the list
+// kick uses no records and no internal order -- so the sums do not depend on the order of the list.
+// The level-L pre-check of the listed pairs gives the level-L list (groupS: a compaction of the
+// upper-level list) and the per-body counts.
+// Force rules of sec. 8.1: a semi-active particle feels massive bodies only and acts on them only in
+// TP 2; two particles do not interact.
+// ---------------------------------------------------------------------------------------------
+#define GENGA_STATUS_BAD_LIST_PAIR 16
+
+__global__ void __launch_bounds__(256)
+list_kick_kernel(const KickParams p, const double* __restrict__ pos, const double* __restrict__ mass, double G,
+                 const int2* __restrict__ in_pairs, const int* __restrict__ in_n, long long in_rows, int tp2)
+{
+    const long long total = min((long long)max(*in_n, 0), in_rows);
+    const int lane = threadIdx.x & 31;
+    const size_t N = (size_t)p.N;
+    for (long long wbase = (long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31); wbase < total;
+         wbase += (long long)gridDim.x * blockDim.x) {
+        const long long c = wbase + lane;
+        bool hit = false;
+        int lo = 0, hi = 0;
+        if (c < total) {
+            const int2 e = in_pairs[c];
+            const int i = e.x, j = e.y;
+            if (i < 0 || j < 0 || i >= p.N || j >= p.N || i == j) {
+                atomicOr(p.status, GENGA_STATUS_BAD_LIST_PAIR);
+            } else if (i < p.n_massive || j < p.n_massive) {
+                const double dx = __dsub_rn(pos[j], pos[i]), dy = __dsub_rn(pos[N + j], pos[N + i]),
+                             dz = __dsub_rn(pos[2 * N + j], pos[2 * N + i]);
+                const double gmi = __dmul_rn(G, mass[i]), gmj = __dmul_rn(G, mass[j]);
+                const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, i, j, dx, dy, dz, gmj);
+                if ((j < p.n_massive || tp2) && r.s != 0.0) {            // i feels j
+                    unsigned long long* acc = p.fx + (size_t)i * (3 * GENGA_FX_LIMBS);
+                    fx_add(acc, __dmul_rn(r.s, dx), p.status);
+                    fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
+                    fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+                    p.touched[i] = 1;
+                }
+                if ((i < p.n_massive || tp2) && r.W != 0.0 && gmi != 0.0) {   // j feels i
+                    const double si = __ddiv_rn(__dmul_rn(gmi, r.W), r.r3);
+                    unsigned long long* acc = p.fx + (size_t)j * (3 * GENGA_FX_LIMBS);
+                    fx_add(acc, -__dmul_rn(si, dx), p.status);
+                    fx_add(acc + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
+                    fx_add(acc + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+                    p.touched[j] = 1;
+                }
+                if (r.enc) {
+                    atomicAdd(p.out_npairs + i, 1);
+                    atomicAdd(p.out_npairs + j, 1);
+                    hit = true; lo = min(i, j); hi = max(i, j);
+                }
+            }
+        }
+        emit_pairs(p, hit, lo, hi);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+list_reduce_kernel(unsigned long long* __restrict__ fx, int* __restrict__ touched, int N, double dt,
+                   int* __restrict__ status, double* __restrict__ out_acc, double* __restrict__ vel)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= N) return;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    if (touched[b]) {
+        touched[b] = 0;
+        unsigned long long* acc = fx + (size_t)b * (3 * GENGA_FX_LIMBS);
+        a0 = fx_take(acc, status);
+        a1 = fx_take(acc + GENGA_FX_LIMBS, status);
+        a2 = fx_take(acc + 2 * GENGA_FX_LIMBS, status);
+    }
+    if (out_acc) {
+        out_acc[b] = a0;
+        out_acc[(size_t)N + b] = a1;
+        out_acc[2 * (size_t)N + b] = a2;
+    }
+    if (vel) {
+        vel[b] = fma(dt, a0, vel[b]);
+        vel[(size_t)N + b] = fma(dt, a1, vel[(size_t)N + b]);
+        vel[2 * (size_t)N + b] = fma(dt, a2, vel[2 * (size_t)N + b]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // reduce_kernel (row a8 + a7): record r sums the partial accelerations of the CTAs whose tile
 // range met its i-block, in ascending CTA order, and writes the caller's arrays.
 // ---------------------------------------------------------------------------------------------
