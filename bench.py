@@ -293,6 +293,24 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                   "ms": float(np.median(group_ts)), "launches": int(group_launches), "pairs": sm[3], "n_groups": sm[0],
                   "n_members": sm[1], "largest_group": sm[2]}
 
+    # NEXT-4: KickS -- the level-1 kick over the level-0 pair list (genga_kick_list) instead of over all pairs
+    pairs1 = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev)
+    npairs1 = torch.empty(n + 1, dtype=torch.int32, device=dev)
+    kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
+    list_ts = []
+    for it in range(8):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        flush.fill_(7)
+        a.record(stream)
+        kick.kick_list(pos, sv, mass, rcrit, 1, 0.5 * ki.dt, pairs, npairs[n:], PAIR_CAPACITY, acc, pairs1, npairs1)
+        b.record(stream)
+        b.synchronize()
+        if it >= 3:
+            list_ts.append(a.elapsed_time(b))
+    list_info = {"what": "genga_kick_list: level-1 kick + pre-check over the level-0 encounter list (same result as the "
+                         "all-pairs level-1 kick, W_1 = 0 beyond rc0)", "ms": float(np.median(list_ts)),
+                 "listed_pairs": int(npairs[n].item()), "level1_pairs": int(npairs1[n].item())}
+
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
@@ -342,6 +360,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             "levels": levels,
             "step": step_info,
             "group": group_info,
+            "kick_list": list_info,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
