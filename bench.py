@@ -99,6 +99,24 @@ class ClockSampler(threading.Thread):
         return d
 
 
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """Timing rule: every multi-GPU number is the MAX over ranks (all_reduce on the job's process group; gloo on
+    CPU tensors in the tests, nccl on device tensors in the bench)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, pairs_per_step: int, steps: int, total_ms_max: float) -> float:
+    """Replicas (weak scaling): every rank does the same number of pair interactions on its own disk; the job's
+    throughput is all of them over the slowest rank's time."""
+    return world * pairs_per_step * steps / (total_ms_max * 1e-3)
+
+
 def physical_gpu_index(local_index: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -220,14 +238,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     clocks = sampler.stop()
     launches = kick.launch_count() - launches0
     step_ms = [a.elapsed_time(b) for a, b in zip(e0, e1)]
-    total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
     pairs_per_kick = ki.n_massive * (ki.n_massive - 1) + ki.n_test * ki.n_massive
     pairs_per_step = len(LEVELS) * pairs_per_kick
-    value = world * pairs_per_step * args.steps / (total_ms * 1e-3)
+    value = whole_job_value(world, pairs_per_step, args.steps, total_ms)
 
     # per-level numbers: one more kick each, timed alone (after the timed region)
     levels = {}
@@ -330,14 +344,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     for _ in range(e2e_steps):
         host_step()
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(time.perf_counter() - t0, world, dev)
     h2d = sum(8 * n * (3 + 3 + 1 + (level + 1)) for level in LEVELS)
     d2h = sum(8 * n * (3 + 3) + 4 * (n + 1) + 8 * min(enc_pairs[level], PAIR_CAPACITY) for level in LEVELS)
-    e2e_value = world * pairs_per_step * e2e_steps / e2e_s
+    e2e_value = whole_job_value(world, pairs_per_step, e2e_steps, 1e3 * e2e_s)
 
     if rank == 0:
         props = torch.cuda.get_device_properties(local_rank)
