@@ -86,7 +86,8 @@ typedef struct {
     int32_t n_i_blocks;     /* ceil(n_i / i_block), n_i = n_test ? m_pad + n_test : n_massive      */
     int32_t n_j_tiles;      /* ceil(n_massive / j_tile)                                            */
     int64_t n_tiles;        /* T = n_i_blocks * n_j_tiles                                          */
-    int32_t n_ctas;         /* CTAs launched (a multiple of the SM count unless T is smaller)      */
+    int32_t n_ctas;         /* CTAs launched (a multiple of the SM count unless T is smaller; up to
+                               four waves of resident CTAs when every CTA keeps >= 16 tiles)      */
     int32_t max_segs;       /* most i-blocks any CTA touches                                       */
     int64_t n_rec;          /* records allocated (n_i rounded up to a multiple of 1024)            */
     int64_t partial_doubles;/* doubles of scratch for the partial sums                             */

@@ -37,6 +37,8 @@ static const genga_variant GENGA_VARIANTS[GENGA_N_VARIANTS] = {
     {128, 1, 64, 4},
 };
 static const int GENGA_MIN_TILES_PER_CTA = 4;
+static const int GENGA_MAX_WAVES = 4;               // CTAs launched = SMs x CTAs per SM x waves (planner)
+static const int GENGA_TILES_PER_CTA_FOR_WAVES = 16; // a further wave only while every CTA keeps this many tiles
 static const int GENGA_STAGES = 4;          // depth of the j-tile ring in shared memory
 static const int GENGA_M_ALIGN = 256;      // every j_tile divides it
 static const int GENGA_SORT_MIN_BODIES = 4096;   // GENGA_KICK_ORDER_AUTO sorts from here on
