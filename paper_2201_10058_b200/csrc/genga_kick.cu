@@ -201,7 +201,10 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         } else {
             // W_L = 0 exactly outside the filter radius: a neighbour search, no tile decomposition
             const int n_igroups = n_rec / GENGA_GROUP, wpc = GENGA_NEAR_THREADS / 32;
-            genga::near_kernel<<<(n_igroups + wpc - 1) / wpc, GENGA_NEAR_THREADS, 0, st>>>(kp, n_rec, pl.m_pad / GENGA_GROUP);
+            const int n_jgroups = pl.m_pad / GENGA_GROUP;
+            const int jsplit = n_jgroups >= 8 * GENGA_NEAR_JSPLIT ? GENGA_NEAR_JSPLIT : 1;
+            const int ichunks = (n_igroups + wpc - 1) / wpc;
+            genga::near_kernel<<<dim3(ichunks, jsplit), GENGA_NEAR_THREADS, 0, st>>>(kp, n_rec, n_jgroups);
             GK_CUDA(ctx, cudaGetLastError());
         }
         if (ctx->timing) {
@@ -218,7 +221,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             GK_CUDA(ctx, dispatch_kick(p2, k2, st));
             ctx->launches++;
         }
-        // exact path: one candidate per thread, grid-stride over the list the pair loop has written
+        // exact path: CTAs walk the list the pair loop has written in rounds of 1024 candidates
         genga::exact_kernel<<<4 * ctx->num_sms, 256, 0, st>>>(kp);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
@@ -262,7 +265,7 @@ extern "C" int genga_kick_list(genga_kick_ctx* ctx, const double* pos, double* v
     kp.status = ctx->status;
     kp.fx = ctx->fx; kp.touched = ctx->touched;
     GK_CUDA(ctx, cudaMemsetAsync(out_npairs, 0, ((size_t)N + 1) * sizeof(int32_t), st));
-    const int blocks = (int)std::min<int64_t>(std::max<int64_t>((in_pair_rows + 255) / 256, 1), 8 * ctx->num_sms);
+    const int blocks = (int)std::min<int64_t>(std::max<int64_t>((in_pair_rows + 1023) / 1024, 1), 8 * ctx->num_sms);
     genga::list_kick_kernel<<<blocks, 256, 0, st>>>(kp, pos, mass, ctx->cfg.G, reinterpret_cast<const int2*>(in_pairs),
                                                     in_n_pairs, in_pair_rows, ctx->cfg.tp_mode == 2 ? 1 : 0);
     genga::list_reduce_kernel<<<(N + 255) / 256, 256, 0, st>>>(ctx->fx, ctx->touched, N, dt, ctx->status, out_acc, vel);

@@ -193,23 +193,6 @@ __device__ __noinline__ ExactResult exact_pair(const double* __restrict__ rcrit,
     return out;
 }
 
-// One warp-wide emission step: lanes with `hit` append (lo, hi) to the pair list with one atomic
-// per warp (ballot + popc); rows beyond capacity are dropped but counted.
-__device__ __forceinline__ void emit_pairs(const KickParams& p, bool hit, int lo, int hi)
-{
-    const unsigned m = __ballot_sync(0xffffffffu, hit);
-    if (m == 0) return;
-    const int lane = threadIdx.x & 31;
-    const int leader = __ffs(m) - 1;
-    int base = 0;
-    if (lane == leader) base = atomicAdd(p.out_npairs + p.N, __popc(m));
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (hit) {
-        const long long slot = (long long)base + __popc(m & ((1u << lane) - 1u));
-        if (slot < p.capacity) reinterpret_cast<int2*>(p.out_pairs)[slot] = make_int2(lo, hi);
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // mbarrier + 1-D TMA bulk copy (cp.async.bulk, SASS UBLKCP) for the j-tile staging
 // ---------------------------------------------------------------------------------------------
@@ -469,55 +452,96 @@ __device__ __forceinline__ void push_candidates(const KickParams& p, CandCursor&
     c.fill += n;
 }
 
+// Emission for a whole CTA of 256 threads with U candidates per thread: ONE atomic on the pair counter
+// per CTA and round (the counter is a single address, and an atomic that returns a value waits for it:
+// one per warp made exact_kernel wait ~30,000 times in a row on that address at N = 65,536).
+#define GENGA_EXACT_U 4
+
+template <int U>
+__device__ __forceinline__ void emit_pairs_cta(const KickParams& p, const bool (&hit)[U], const int (&lo)[U],
+                                               const int (&hi)[U])
+{
+    __shared__ int wsum[8];
+    __shared__ int cta_base;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int mine = 0;
+#pragma unroll
+    for (int u = 0; u < U; u++) mine += hit[u] ? 1 : 0;
+    int s = mine;                                           // inclusive scan over the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, s, o);
+        if (lane >= o) s += t;
+    }
+    if (lane == 31) wsum[warp] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; w++) { const int c = wsum[w]; wsum[w] = tot; tot += c; }
+        cta_base = tot ? atomicAdd(p.out_npairs + p.N, tot) : 0;
+    }
+    __syncthreads();
+    long long slot = (long long)cta_base + wsum[warp] + (s - mine);
+#pragma unroll
+    for (int u = 0; u < U; u++)
+        if (hit[u]) {
+            if (slot < p.capacity) reinterpret_cast<int2*>(p.out_pairs)[slot] = make_int2(lo[u], hi[u]);
+            slot++;
+        }
+    __syncthreads();                                        // wsum / cta_base are reused by the next round
+}
+
 __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
 {
+    constexpr int U = GENGA_EXACT_U;
     const long long n = min((long long)*p.ncand, p.cand_capacity);
-    const int lane = threadIdx.x & 31;
-    // whole warps walk the list (the emission votes need every lane)
-    for (long long wbase = ((long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31)); wbase < n;
-         wbase += (long long)gridDim.x * blockDim.x) {
-        const long long c = wbase + lane;
-        bool hit = false;
-        int lo = 0, hi = 0;
-        if (c < n) {
+    // a CTA walks the list in rounds of 256 * U candidates (CTA-uniform trip count: the emission synchronises)
+    for (long long cbase = (long long)blockIdx.x * (256 * U); cbase < n; cbase += (long long)gridDim.x * (256 * U)) {
+        bool hit[U];
+        int lo[U], hi[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const long long c = cbase + u * 256 + threadIdx.x;
+            hit[u] = false; lo[u] = 0; hi[u] = 0;
+            if (c >= n) continue;
             const int2 e = p.cand[c];
             const int ir = e.x;
             const bool force_only = ir >= 0 && e.y < 0;                                     // (i, ~j): see KickParams
             const int jr = force_only ? ~e.y : e.y;
             const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;    // (-1, -1): empty slot
-            if (ir != jr && bi >= 0 && bj >= 0) {
-                const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
-                const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
-                const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
-                if (r.s != 0.0) {
-                    unsigned long long* acc = p.fx + (size_t)ir * (3 * GENGA_FX_LIMBS);
-                    fx_add(acc, __dmul_rn(r.s, dx), p.status);
-                    fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
-                    fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
-                    p.touched[ir] = 1;
-                }
-                if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
-                    // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
-                    // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
-                    const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
-                    unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
-                    fx_add(accj, -__dmul_rn(si, dx), p.status);
-                    fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
-                    fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
-                    p.touched[jr] = 1;
-                }
-                if (r.enc && p.out_npairs && !force_only) {
-                    atomicAdd(p.out_npairs + bi, 1);
-                    if (bi >= p.n_massive) {               // test particle i, massive j
-                        atomicAdd(p.out_npairs + bj, 1);
-                        hit = true; lo = bj; hi = bi;
-                    } else if (bi < bj) {
-                        hit = true; lo = bi; hi = bj;
-                    }
+            if (ir == jr || bi < 0 || bj < 0) continue;
+            const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
+            const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
+            const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
+            if (r.s != 0.0) {
+                unsigned long long* acc = p.fx + (size_t)ir * (3 * GENGA_FX_LIMBS);
+                fx_add(acc, __dmul_rn(r.s, dx), p.status);
+                fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
+                fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+                p.touched[ir] = 1;
+            }
+            if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
+                // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
+                // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
+                const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
+                unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
+                fx_add(accj, -__dmul_rn(si, dx), p.status);
+                fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
+                fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+                p.touched[jr] = 1;
+            }
+            if (r.enc && p.out_npairs && !force_only) {
+                atomicAdd(p.out_npairs + bi, 1);
+                if (bi >= p.n_massive) {               // test particle i, massive j
+                    atomicAdd(p.out_npairs + bj, 1);
+                    hit[u] = true; lo[u] = bj; hi[u] = bi;
+                } else if (bi < bj) {
+                    hit[u] = true; lo[u] = bi; hi[u] = bj;
                 }
             }
         }
-        emit_pairs(p, hit, lo, hi);
+        emit_pairs_cta<U>(p, hit, lo, hi);
     }
 }
 
@@ -714,6 +738,10 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 // the few near groups it forms r^2 for its 32 x 32 pairs and appends the pairs that trip the
 // filter to the candidate list.  No accelerations are accumulated here: all of them come from
 // exact_kernel's fixed-point sums (reduce_kernel is told there are no partial segments).
+// The near groups of a warp cluster where the disk is dense (a few warps have ten times the mean), and
+// a warp walks its near groups one after the other: the j-groups are therefore dealt round-robin to
+// gridDim.y CTAs per i-chunk (CTA y takes the groups g = y mod gridDim.y), which cuts the longest
+// chain by that factor.
 // ---------------------------------------------------------------------------------------------
 #define GENGA_NEAR_THREADS 128
 #define GENGA_NEAR_BOXES 256
@@ -740,10 +768,12 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
     cc.base = 0;
     cc.fill = GENGA_CAND_BLOCK;
 
-    for (int g0 = 0; g0 < n_jgroups; g0 += GENGA_NEAR_BOXES) {
+    const int js = gridDim.y, jy = blockIdx.y;               // this CTA's j-groups: g = q * js + jy
+    const int n_mine = (n_jgroups - jy + js - 1) / js;
+    for (int g0 = 0; g0 < n_mine; g0 += GENGA_NEAR_BOXES) {
         __syncthreads();
         for (int q = tid; q < GENGA_NEAR_BOXES; q += GENGA_NEAR_THREADS) {
-            const int g = g0 + q;
+            const int g = (g0 + q) * js + jy;
             blo[q] = g < n_jgroups ? p.cblo[g] : make_float4(3.0e38f, 3.0e38f, 3.0e38f, __int_as_float(-1));
             bhi[q] = g < n_jgroups ? p.cbhi[g] : make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
         }
@@ -753,7 +783,7 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
         for (int q0 = 0; q0 < GENGA_NEAR_BOXES; q0 += 32) {
             unsigned nearmask = __ballot_sync(0xffffffffu, boxes_near(wlo, whi, wfw, blo[q0 + lane], bhi[q0 + lane]));
             while (nearmask) {
-                const int j0 = (g0 + q0 + __ffs(nearmask) - 1) * GENGA_GROUP;
+                const int j0 = ((g0 + q0 + __ffs(nearmask) - 1) * js + jy) * GENGA_GROUP;
                 nearmask &= nearmask - 1;
                 const int fj_lane = p.rfw[j0 + lane];
                 unsigned tm = 0;                            // bit u: pair (r, j0 + u) tripped the filter
@@ -795,47 +825,50 @@ __global__ void __launch_bounds__(256)
 list_kick_kernel(const KickParams p, const double* __restrict__ pos, const double* __restrict__ mass, double G,
                  const int2* __restrict__ in_pairs, const int* __restrict__ in_n, long long in_rows, int tp2)
 {
+    constexpr int U = GENGA_EXACT_U;
     const long long total = min((long long)max(*in_n, 0), in_rows);
-    const int lane = threadIdx.x & 31;
     const size_t N = (size_t)p.N;
-    for (long long wbase = (long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31); wbase < total;
-         wbase += (long long)gridDim.x * blockDim.x) {
-        const long long c = wbase + lane;
-        bool hit = false;
-        int lo = 0, hi = 0;
-        if (c < total) {
+    for (long long cbase = (long long)blockIdx.x * (256 * U); cbase < total; cbase += (long long)gridDim.x * (256 * U)) {
+        bool hit[U];
+        int lo[U], hi[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const long long c = cbase + u * 256 + threadIdx.x;
+            hit[u] = false; lo[u] = 0; hi[u] = 0;
+            if (c >= total) continue;
             const int2 e = in_pairs[c];
             const int i = e.x, j = e.y;
             if (i < 0 || j < 0 || i >= p.N || j >= p.N || i == j) {
                 atomicOr(p.status, GENGA_STATUS_BAD_LIST_PAIR);
-            } else if (i < p.n_massive || j < p.n_massive) {
-                const double dx = __dsub_rn(pos[j], pos[i]), dy = __dsub_rn(pos[N + j], pos[N + i]),
-                             dz = __dsub_rn(pos[2 * N + j], pos[2 * N + i]);
-                const double gmi = __dmul_rn(G, mass[i]), gmj = __dmul_rn(G, mass[j]);
-                const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, i, j, dx, dy, dz, gmj);
-                if ((j < p.n_massive || tp2) && r.s != 0.0) {            // i feels j
-                    unsigned long long* acc = p.fx + (size_t)i * (3 * GENGA_FX_LIMBS);
-                    fx_add(acc, __dmul_rn(r.s, dx), p.status);
-                    fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
-                    fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
-                    p.touched[i] = 1;
-                }
-                if ((i < p.n_massive || tp2) && r.W != 0.0 && gmi != 0.0) {   // j feels i
-                    const double si = __ddiv_rn(__dmul_rn(gmi, r.W), r.r3);
-                    unsigned long long* acc = p.fx + (size_t)j * (3 * GENGA_FX_LIMBS);
-                    fx_add(acc, -__dmul_rn(si, dx), p.status);
-                    fx_add(acc + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
-                    fx_add(acc + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
-                    p.touched[j] = 1;
-                }
-                if (r.enc) {
-                    atomicAdd(p.out_npairs + i, 1);
-                    atomicAdd(p.out_npairs + j, 1);
-                    hit = true; lo = min(i, j); hi = max(i, j);
-                }
+                continue;
+            }
+            if (i >= p.n_massive && j >= p.n_massive) continue;          // two particles do not interact
+            const double dx = __dsub_rn(pos[j], pos[i]), dy = __dsub_rn(pos[N + j], pos[N + i]),
+                         dz = __dsub_rn(pos[2 * N + j], pos[2 * N + i]);
+            const double gmi = __dmul_rn(G, mass[i]), gmj = __dmul_rn(G, mass[j]);
+            const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, i, j, dx, dy, dz, gmj);
+            if ((j < p.n_massive || tp2) && r.s != 0.0) {            // i feels j
+                unsigned long long* acc = p.fx + (size_t)i * (3 * GENGA_FX_LIMBS);
+                fx_add(acc, __dmul_rn(r.s, dx), p.status);
+                fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
+                fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+                p.touched[i] = 1;
+            }
+            if ((i < p.n_massive || tp2) && r.W != 0.0 && gmi != 0.0) {   // j feels i
+                const double si = __ddiv_rn(__dmul_rn(gmi, r.W), r.r3);
+                unsigned long long* acc = p.fx + (size_t)j * (3 * GENGA_FX_LIMBS);
+                fx_add(acc, -__dmul_rn(si, dx), p.status);
+                fx_add(acc + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
+                fx_add(acc + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+                p.touched[j] = 1;
+            }
+            if (r.enc) {
+                atomicAdd(p.out_npairs + i, 1);
+                atomicAdd(p.out_npairs + j, 1);
+                hit[u] = true; lo[u] = min(i, j); hi[u] = max(i, j);
             }
         }
-        emit_pairs(p, hit, lo, hi);
+        emit_pairs_cta<U>(p, hit, lo, hi);
     }
 }
 

@@ -37,6 +37,7 @@ static const genga_variant GENGA_VARIANTS[GENGA_N_VARIANTS] = {
     {128, 1, 64, 4},
 };
 static const int GENGA_MIN_TILES_PER_CTA = 4;
+static const int GENGA_NEAR_JSPLIT = 8;            // near_kernel: CTAs per i-chunk, j-groups dealt round-robin
 static const int GENGA_MAX_WAVES = 4;               // CTAs launched = SMs x CTAs per SM x waves (planner)
 static const int GENGA_TILES_PER_CTA_FOR_WAVES = 16; // a further wave only while every CTA keeps this many tiles
 static const int GENGA_STAGES = 4;          // depth of the j-tile ring in shared memory
