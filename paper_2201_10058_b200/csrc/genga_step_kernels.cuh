@@ -84,7 +84,9 @@ __device__ __forceinline__ void block_sum3(double& a, double& b, double& c)
 }
 
 // The CTA's partial sum goes to partial[blockIdx.x][3]; the CTA that finishes last (ticket) adds the
-// partials in ascending CTA order and writes the total to partial[GENGA_PSUM_BLOCKS + slot][3].
+// partials -- thread t takes the CTAs t, t + 256, ... in ascending order, then the same fixed tree as
+// above -- and writes the total to partial[GENGA_PSUM_BLOCKS + slot][3].  (A single thread adding up to
+// 1024 partials one L2 round trip after the other took 20 us of the 22 us of psum_kernel.)
 __device__ __forceinline__ void publish_sum3(double a, double b, double c, double* __restrict__ partial,
                                              unsigned* __restrict__ ticket, int slot)
 {
@@ -95,12 +97,15 @@ __device__ __forceinline__ void publish_sum3(double a, double b, double c, doubl
         last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     }
     __syncthreads();
-    if (last && threadIdx.x == 0) {
-        __threadfence();
-        double ta = 0.0, tb = 0.0, tc = 0.0;
-        for (unsigned q = 0; q < gridDim.x; q++) {
-            ta += __ldcg(partial + 3 * q + 0); tb += __ldcg(partial + 3 * q + 1); tc += __ldcg(partial + 3 * q + 2);
-        }
+    if (!last) return;                                       // CTA-uniform
+    __threadfence();
+    double ta = 0.0, tb = 0.0, tc = 0.0;
+    for (unsigned q = threadIdx.x; q < gridDim.x; q += GENGA_STEP_THREADS) {
+        ta += __ldcg(partial + 3 * q + 0); tb += __ldcg(partial + 3 * q + 1); tc += __ldcg(partial + 3 * q + 2);
+    }
+    __syncthreads();                                         // block_sum3's shared array is reused
+    block_sum3(ta, tb, tc);
+    if (threadIdx.x == 0) {
         double* tot = partial + 3 * (GENGA_PSUM_BLOCKS + slot);
         tot[0] = ta; tot[1] = tb; tot[2] = tc;
         *ticket = 0u;                                        // ready for the next launch on the stream
