@@ -3,7 +3,7 @@ built library (north_star: "a per-pair flop count read off the committed SASS").
 
     python -m paper_2201_10058_b200.sass_report > profiles/sass_pair_loop_r01.md
 
-Dumps `kick_kernel<256, 2, 256, 2, true, STAGES>` with cuobjdump, finds the innermost loops that
+Dumps `kick_kernel<256, 2, 256, 2, STAGES>` (the level-0 pair loop) with cuobjdump, finds the innermost loops that
 issue FP64 arithmetic (a backward branch whose body holds no other loop with FP64 instructions),
 and prints for each the instruction mix, the pairs per trip (MUFU.RSQ64H count: one seed per
 pair) and the listing.  No GPU needed.
@@ -26,9 +26,9 @@ def dense_kernel_sass():
     blocks = re.split(r"\n\s*Function : ", out)
     for b in blocks[1:]:
         name = b.split("\n", 1)[0].strip()
-        if re.search(r"kick_kernelILi256ELi2ELi256ELi2ELb1E", name):
+        if re.search(r"kick_kernelILi256ELi2ELi256ELi2ELi\d+EE", name):
             return name, b
-    raise RuntimeError("dense kick_kernel<256, 2, 256, 2, true> not found in " + LIB)
+    raise RuntimeError("kick_kernel<256, 2, 256, 2, STAGES> not found in " + LIB)
 
 
 def parse(block):
