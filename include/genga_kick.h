@@ -44,8 +44,9 @@ typedef enum {
 #define GENGA_KICK_STATUS_COINCIDENT 1   /* two distinct bodies at the same position were met
                                             (outside the domain; that pair was skipped)          */
 #define GENGA_KICK_STATUS_CAND_OVERFLOW 2 /* more pairs inside a critical radius than the library's
-                                            candidate list holds (64 per body): the excess pairs
-                                            were dropped, out_acc / out_pairs are incomplete      */
+                                            candidate list holds (64 per body, at least 2^20): the
+                                            excess pairs were evaluated on a slow path.  The results
+                                            are COMPLETE; the bit only says why the call was slow  */
 #define GENGA_KICK_STATUS_FX_RANGE 4     /* a changeover-weighted term outside [7e-43, 4.5e15]
                                             (or not finite) was met and left out of out_acc       */
 

@@ -11,6 +11,8 @@ LIB_PATH = os.path.join(HERE, "libgenga_kick.so")
 
 OK, E_NULL, E_ALIGN, E_SIZE, E_LEVEL, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4, -5, -6
 STATUS_COINCIDENT = 1
+STATUS_CAND_OVERFLOW = 2
+STATUS_FX_RANGE = 4
 ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 
 EXPORTS = (

@@ -173,17 +173,8 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches += 8;
     }
+    genga::KickParams kp = {};
     {
-        const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
-        genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
-                                                   ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
-                                                   ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw,
-                                                   ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand);
-        GK_CUDA(ctx, cudaGetLastError());
-        ctx->launches++;
-    }
-    if (pl.n_ctas > 0) {
-        genga::KickParams kp;
         kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx; kp.cfw = ctx->cfw;
         kp.cblo = ctx->cblo; kp.cbhi = ctx->cbhi;
         kp.rcrit = rcrit;
@@ -195,6 +186,17 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         kp.status = ctx->status;
         kp.cand = ctx->cand; kp.cand_capacity = ctx->cand_capacity; kp.ncand = ctx->ncand;
         kp.fx = ctx->fx; kp.touched = ctx->touched;
+    }
+    {
+        const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
+        genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
+                                                   ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
+                                                   ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw,
+                                                   ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand);
+        GK_CUDA(ctx, cudaGetLastError());
+        ctx->launches++;
+    }
+    if (pl.n_ctas > 0) {
         if (ctx->timing) GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level], st));
         if (changeover_level == 0) {
             GK_CUDA(ctx, dispatch_kick(pl, kp, st));
@@ -204,7 +206,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             const int n_jgroups = pl.m_pad / GENGA_GROUP;
             const int jsplit = n_jgroups >= 8 * GENGA_NEAR_JSPLIT ? GENGA_NEAR_JSPLIT : 1;
             const int ichunks = (n_igroups + wpc - 1) / wpc;
-            genga::near_kernel<<<dim3(ichunks, jsplit), GENGA_NEAR_THREADS, 0, st>>>(kp, n_rec, n_jgroups);
+            genga::near_kernel<false><<<dim3(ichunks, jsplit), GENGA_NEAR_THREADS, 0, st>>>(kp, n_rec, 0, n_jgroups, 0);
             GK_CUDA(ctx, cudaGetLastError());
         }
         if (ctx->timing) {
@@ -220,6 +222,16 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             k2.partial = ctx->partial2; k2.j_rec0 = pl.m_pad; k2.force_only = 1;
             GK_CUDA(ctx, dispatch_kick(p2, k2, st));
             ctx->launches++;
+        }
+        {
+            // fallback for an overflowed candidate list: returns at once otherwise (see near_kernel<true>)
+            const int wpc = GENGA_NEAR_THREADS / 32;
+            genga::near_kernel<true><<<(n_rec / GENGA_GROUP + wpc - 1) / wpc, GENGA_NEAR_THREADS, 0, st>>>(
+                kp, n_rec, 0, pl.m_pad / GENGA_GROUP, 0);
+            if (ctx->tp2 && changeover_level == 0)
+                genga::near_kernel<true><<<(pl.m_pad / GENGA_GROUP + wpc - 1) / wpc, GENGA_NEAR_THREADS, 0, st>>>(
+                    kp, pl.m_pad, pl.m_pad / GENGA_GROUP, (n_rec - pl.m_pad) / GENGA_GROUP, 1);
+            ctx->launches += ctx->tp2 && changeover_level == 0 ? 2 : 1;
         }
         // exact path: CTAs walk the list the pair loop has written in rounds of 1024 candidates
         genga::exact_kernel<<<4 * ctx->num_sms, 256, 0, st>>>(kp);

@@ -411,6 +411,46 @@ __device__ __forceinline__ double fx_take(unsigned long long* __restrict__ acc, 
     return neg ? -v : v;
 }
 
+// The work of the exact path for one candidate (i-record, j-record or ~j-record for a force-only
+// candidate, or (-1, -1) for an empty slot): weight, force on i (and the TP 2 reaction on j), pre-check,
+// per-body counts.  Returns the pair to emit, if any.
+__device__ __forceinline__ void apply_candidate(const KickParams& p, int ir, int jr_enc, bool& hit, int& lo, int& hi)
+{
+    const bool force_only = ir >= 0 && jr_enc < 0;                                  // (i, ~j): see KickParams
+    const int jr = force_only ? ~jr_enc : jr_enc;
+    const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;      // (-1, -1): empty slot
+    if (ir == jr || bi < 0 || bj < 0) return;
+    const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
+    const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
+    const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
+    if (r.s != 0.0) {
+        unsigned long long* acc = p.fx + (size_t)ir * (3 * GENGA_FX_LIMBS);
+        fx_add(acc, __dmul_rn(r.s, dx), p.status);
+        fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
+        fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+        p.touched[ir] = 1;
+    }
+    if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
+        // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
+        // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
+        const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
+        unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
+        fx_add(accj, -__dmul_rn(si, dx), p.status);
+        fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
+        fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+        p.touched[jr] = 1;
+    }
+    if (r.enc && p.out_npairs && !force_only) {
+        atomicAdd(p.out_npairs + bi, 1);
+        if (bi >= p.n_massive) {               // test particle i, massive j
+            atomicAdd(p.out_npairs + bj, 1);
+            hit = true; lo = bj; hi = bi;
+        } else if (bi < bj) {
+            hit = true; lo = bi; hi = bj;
+        }
+    }
+}
+
 // Append the warp's tripped pairs (i-record, j-record) to the candidate list.  A warp reserves the
 // list GENGA_CAND_BLOCK slots at a time (one atomic per block, not per push: the counter is a
 // single hot address) and fills its block with a private cursor; the slots of a block it does
@@ -447,7 +487,7 @@ __device__ __forceinline__ void push_candidates(const KickParams& p, CandCursor&
     }
     if (mine) {
         const long long slot = c.base + c.fill + __popc(m & ((1u << lane) - 1u));
-        if (slot < p.cand_capacity) p.cand[slot] = make_int2(irec, jrec);
+        if (slot < p.cand_capacity) p.cand[slot] = make_int2(irec, jrec);     // else: dropped; see near_kernel<true>
     }
     c.fill += n;
 }
@@ -495,7 +535,8 @@ __device__ __forceinline__ void emit_pairs_cta(const KickParams& p, const bool (
 __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
 {
     constexpr int U = GENGA_EXACT_U;
-    const long long n = min((long long)*p.ncand, p.cand_capacity);
+    if ((long long)*p.ncand > p.cand_capacity) return;      // the list overflowed: near_kernel<true> has done all of it
+    const long long n = (long long)*p.ncand;
     // a CTA walks the list in rounds of 256 * U candidates (CTA-uniform trip count: the emission synchronises)
     for (long long cbase = (long long)blockIdx.x * (256 * U); cbase < n; cbase += (long long)gridDim.x * (256 * U)) {
         bool hit[U];
@@ -506,40 +547,7 @@ __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
             hit[u] = false; lo[u] = 0; hi[u] = 0;
             if (c >= n) continue;
             const int2 e = p.cand[c];
-            const int ir = e.x;
-            const bool force_only = ir >= 0 && e.y < 0;                                     // (i, ~j): see KickParams
-            const int jr = force_only ? ~e.y : e.y;
-            const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;    // (-1, -1): empty slot
-            if (ir == jr || bi < 0 || bj < 0) continue;
-            const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
-            const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
-            const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
-            if (r.s != 0.0) {
-                unsigned long long* acc = p.fx + (size_t)ir * (3 * GENGA_FX_LIMBS);
-                fx_add(acc, __dmul_rn(r.s, dx), p.status);
-                fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
-                fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
-                p.touched[ir] = 1;
-            }
-            if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
-                // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
-                // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
-                const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
-                unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
-                fx_add(accj, -__dmul_rn(si, dx), p.status);
-                fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
-                fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
-                p.touched[jr] = 1;
-            }
-            if (r.enc && p.out_npairs && !force_only) {
-                atomicAdd(p.out_npairs + bi, 1);
-                if (bi >= p.n_massive) {               // test particle i, massive j
-                    atomicAdd(p.out_npairs + bj, 1);
-                    hit[u] = true; lo[u] = bj; hi[u] = bi;
-                } else if (bi < bj) {
-                    hit[u] = true; lo[u] = bi; hi[u] = bj;
-                }
-            }
+            apply_candidate(p, e.x, e.y, hit[u], lo[u], hi[u]);
         }
         emit_pairs_cta<U>(p, hit, lo, hi);
     }
@@ -746,8 +754,20 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 #define GENGA_NEAR_THREADS 128
 #define GENGA_NEAR_BOXES 256
 
-__global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickParams p, int n_rec, int n_jgroups)
+// RESCAN = false: the level >= 1 pair loop (queues candidates; a pair trips if hi(r^2) < max(fw_i, fw_j)).
+// RESCAN = true : the fallback for a candidate list that overflowed (more pairs inside critical radii than
+//   the list holds: everything inside everything's radius).  Launched after the pair loop of every kick, it
+//   returns at once unless the list overflowed; then it repeats the search -- with the pair loop's own trip
+//   rule, hi(r^2) < max(fw_i, largest fw of j's chunk), so that it meets exactly the pairs the far-field
+//   pass left out -- and evaluates every tripped pair where it finds it (apply_candidate), while
+//   exact_kernel ignores the truncated list.  Slow (one atomic on the pair counter per pair) but complete:
+//   the capacity of the list bounds the speed of pathological inputs, not the correctness of the result.
+//   i-records [0, i_rec_end) against the j-groups [j_group0, j_group0 + n_jgroups); force_only as in KickParams.
+template <bool RESCAN>
+__global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4)
+near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int force_only)
 {
+    if (RESCAN && (long long)*p.ncand <= p.cand_capacity) return;
     __shared__ float4 blo[GENGA_NEAR_BOXES];
     __shared__ float4 bhi[GENGA_NEAR_BOXES];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -756,7 +776,7 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
     double xi = GENGA_SENTINEL_POS, yi = GENGA_SENTINEL_POS, zi = GENGA_SENTINEL_POS;
     int fi = -1, wfw = -1;
     float4 wlo = make_float4(3.0e38f, 3.0e38f, 3.0e38f, 0.0f), whi = make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
-    if (r < n_rec) {
+    if (r < i_rec_end) {
         const double2 a = p.rxy[r], b = p.rzm[r];
         xi = a.x; yi = a.y; zi = b.x;
         fi = p.rfw[r];
@@ -774,8 +794,8 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
         __syncthreads();
         for (int q = tid; q < GENGA_NEAR_BOXES; q += GENGA_NEAR_THREADS) {
             const int g = (g0 + q) * js + jy;
-            blo[q] = g < n_jgroups ? p.cblo[g] : make_float4(3.0e38f, 3.0e38f, 3.0e38f, __int_as_float(-1));
-            bhi[q] = g < n_jgroups ? p.cbhi[g] : make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
+            blo[q] = g < n_jgroups ? p.cblo[j_group0 + g] : make_float4(3.0e38f, 3.0e38f, 3.0e38f, __int_as_float(-1));
+            bhi[q] = g < n_jgroups ? p.cbhi[j_group0 + g] : make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
         }
         __syncthreads();
         if (!active) continue;
@@ -783,9 +803,10 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
         for (int q0 = 0; q0 < GENGA_NEAR_BOXES; q0 += 32) {
             unsigned nearmask = __ballot_sync(0xffffffffu, boxes_near(wlo, whi, wfw, blo[q0 + lane], bhi[q0 + lane]));
             while (nearmask) {
-                const int j0 = ((g0 + q0 + __ffs(nearmask) - 1) * js + jy) * GENGA_GROUP;
+                const int j0 = (j_group0 + (g0 + q0 + __ffs(nearmask) - 1) * js + jy) * GENGA_GROUP;
                 nearmask &= nearmask - 1;
-                const int fj_lane = p.rfw[j0 + lane];
+                // per j-record threshold: its own filter word, or (RESCAN) the largest of its chunk
+                const int fj_lane = RESCAN ? p.cfw[(j0 + lane) / GENGA_CHUNK] : p.rfw[j0 + lane];
                 unsigned tm = 0;                            // bit u: pair (r, j0 + u) tripped the filter
 #pragma unroll 8
                 for (int u = 0; u < GENGA_GROUP; u++) {
@@ -795,16 +816,30 @@ __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4) near_kernel(const KickP
                     const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
                     tm |= (__double2hiint(r2) < thr ? 1u : 0u) << u;
                 }
-                unsigned todo = __reduce_or_sync(0xffffffffu, tm);
-                while (todo) {                              // warp-uniform: the j-records some lane tripped on
-                    const int b = __ffs(todo) - 1;
-                    todo &= todo - 1;
-                    push_candidates(p, cc, (tm >> b) & 1u, r, j0 + b);
+                if (RESCAN) {
+                    while (tm) {                            // per lane: its own tripped pairs, one after the other
+                        const int jr = j0 + __ffs(tm) - 1;
+                        tm &= tm - 1;
+                        bool hit = false;
+                        int lo = 0, hi = 0;
+                        apply_candidate(p, r, force_only ? ~jr : jr, hit, lo, hi);
+                        if (hit) {
+                            const long long slot = atomicAdd(p.out_npairs + p.N, 1);
+                            if (slot < p.capacity) reinterpret_cast<int2*>(p.out_pairs)[slot] = make_int2(lo, hi);
+                        }
+                    }
+                } else {
+                    unsigned todo = __reduce_or_sync(0xffffffffu, tm);
+                    while (todo) {                          // warp-uniform: the j-records some lane tripped on
+                        const int b = __ffs(todo) - 1;
+                        todo &= todo - 1;
+                        push_candidates(p, cc, (tm >> b) & 1u, r, j0 + b);
+                    }
                 }
             }
         }
     }
-    if (cc.fill < GENGA_CAND_BLOCK) close_block(p, cc);
+    if (!RESCAN && cc.fill < GENGA_CAND_BLOCK) close_block(p, cc);
 }
 
 // ---------------------------------------------------------------------------------------------

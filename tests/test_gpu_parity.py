@@ -225,3 +225,37 @@ def test_tp2_semi_active_particles_act_on_massive_bodies(oracle_mod, nm, nt, lev
     one = run_gpu(ki, level=level, tp_mode=1)
     assert np.array_equal(one.acc[:, nm:], gpu.acc[:, nm:])
     assert np.array_equal(sorted_pairs(one.pairs), sorted_pairs(gpu.pairs))
+
+
+def test_candidate_list_overflow_is_complete(oracle_mod):
+    """Everything inside everything's critical radius: 9e6 ordered candidates against a list of 2^20.  The excess is
+    evaluated where it is found (slow path); the result is complete and the status word says the list overflowed."""
+    import paper_2201_10058_b200 as g
+    ki = gi.make_config(0, n=3000)
+    ki.rcrit = np.full_like(ki.rcrit, 12.0)                  # AU: larger than the disk
+    n = ki.n
+    gpu = run_gpu(ki, capacity=1 << 23)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, n, 0, level=0, G=ki.G, maxp=n)
+    assert gpu.status == g.STATUS_CAND_OVERFLOW
+    assert gpu.total == n * (n - 1) // 2 and (gpu.counts == n - 1).all()
+    gpu.status = 0
+    compare(gpu, orc, n, tol=TOL)
+
+
+def test_candidate_list_overflow_tp2_and_level1(oracle_mod):
+    """The overflow fallback also covers the level >= 1 neighbour search and TP 2's transposed pass."""
+    import paper_2201_10058_b200 as g
+    ki = gi.make_config(3, n=2500, level=1)
+    ki.rcrit = np.stack([np.full(ki.n, 12.0), np.full(ki.n, 6.0)])
+    gpu = run_gpu(ki, level=1, capacity=1 << 22)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n, 0, level=1, G=ki.G, maxp=ki.n)
+    assert gpu.status == g.STATUS_CAND_OVERFLOW
+    gpu.status = 0
+    compare(gpu, orc, ki.n, tol=TOL)
+    kt = _with_tp_masses(gi.make_config(4, n=300, n_test=6000))
+    kt.rcrit = np.full_like(kt.rcrit, 12.0)                   # 300 x 6000 x 2 + 300^2 ordered candidates > 2^20
+    gpu = run_gpu(kt, level=0, capacity=1 << 22, tp_mode=2)
+    orc = oracle_mod.kick(kt.pos, kt.mass, kt.rcrit, 300, 6000, level=0, G=kt.G, maxp=kt.n, tp_mode=2)
+    assert gpu.status == g.STATUS_CAND_OVERFLOW
+    gpu.status = 0
+    compare(gpu, orc, 300, tol=TOL)
