@@ -46,6 +46,22 @@ int genga_rcrit(genga_kick_ctx* ctx, const double* pos, const double* vel, const
                 double dt, double substeps, int32_t nrows, double n1, double n2, double* out_rcrit);
 
 /*
+ * RcritS / FGS (App. A: "The functions RcritS, KickS, and FGS are similar to the original
+ * functions, but are applied only to the relevant bodies in each symplectic level"): genga_rcrit and genga_fg
+ * for the bodies of a list only -- e.g. `members` of genga_group.  Bodies not in the list are not read and
+ * not written (genga_rcrit_list writes out_rcrit[k][i] for listed i only).  KickS is genga_kick_list.
+ *   list      [list_rows] int32 device, 16-byte aligned: body indices, each at most once
+ *   n_list    device pointer to ONE int32: number of entries (clipped to list_rows), e.g. summary + 1 of genga_group
+ * An index outside [0, N) is ignored and sets status bit 16.
+ * Errors: as genga_rcrit / genga_fg, plus E_SIZE for list_rows < 0.
+ */
+int genga_rcrit_list(genga_kick_ctx* ctx, const double* pos, const double* vel, const double* mass, double m_star,
+                     double dt, double substeps, int32_t nrows, double n1, double n2, const int32_t* list,
+                     const int32_t* n_list, int64_t list_rows, double* out_rcrit);
+int genga_fg_list(genga_kick_ctx* ctx, double* pos, double* vel, double m_star, double dt, const int32_t* list,
+                  const int32_t* n_list, int64_t list_rows);
+
+/*
  * HC: the Sun part H_C = (sum_i p_i)^2 / (2 m_star) of eq. 4, "the democratic
  * momentum summation" (App. A): pos_i += dt * (sum_j m_j v_j) / m_star for every
  * body, in place.  The sum runs over all N bodies in a fixed order (bit-reproducible,

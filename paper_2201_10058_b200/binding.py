@@ -22,7 +22,7 @@ EXPORTS = (
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
 )
 # include/genga_step.h: the O(N) neighbours of the kick and the composed step
-STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_step")
+STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_step", "genga_rcrit_list", "genga_fg_list")
 # include/genga_group.h: close-encounter groups
 GROUP_EXPORTS = ("genga_group",)
 STATUS_BAD_PAIR = 16
@@ -88,6 +88,8 @@ def lib():
         L.genga_hc.argtypes = [vp, vp, vp, vp, d, d]
         L.genga_fg.argtypes = [vp, vp, vp, d, d]
         L.genga_drift.argtypes = [vp, vp, vp, vp, d, d]
+        L.genga_rcrit_list.argtypes = [vp, vp, vp, vp, d, d, d, i32, d, d, vp, vp, i64, vp]
+        L.genga_fg_list.argtypes = [vp, vp, vp, d, d, vp, vp, i64]
         L.genga_step.argtypes = [vp, vp, vp, vp, d, d, d, d, vp, vp, vp, vp]
         L.genga_group.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
         for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS:
@@ -186,6 +188,16 @@ class GengaKick:
 
     def fg(self, pos, vel, m_star, dt):
         self._check(lib().genga_fg(self._ctx, _ptr(pos), _ptr(vel), float(m_star), float(dt)))
+
+    def rcrit_list(self, pos, vel, mass, m_star, dt, list_, n_list, list_rows, out_rcrit, substeps=2.0, nrows=1, n1=3.0,
+                   n2=0.4):
+        self._check(lib().genga_rcrit_list(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt),
+                                           float(substeps), int(nrows), float(n1), float(n2), _ptr(list_), _ptr(n_list),
+                                           int(list_rows), _ptr(out_rcrit)))
+
+    def fg_list(self, pos, vel, m_star, dt, list_, n_list, list_rows):
+        self._check(lib().genga_fg_list(self._ctx, _ptr(pos), _ptr(vel), float(m_star), float(dt), _ptr(list_),
+                                        _ptr(n_list), int(list_rows)))
 
     def drift(self, pos, vel, mass, m_star, dt):
         self._check(lib().genga_drift(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt)))

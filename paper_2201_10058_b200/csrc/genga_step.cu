@@ -4,6 +4,8 @@
 #include "genga_kick_ctx.h"
 #include "genga_step_kernels.cuh"
 
+#include <algorithm>
+
 namespace {
 
 int ensure_step_scratch(genga_kick_ctx* ctx)
@@ -30,7 +32,43 @@ extern "C" int genga_rcrit(genga_kick_ctx* ctx, const double* pos, const double*
     if (nrows < 1 || !(substeps > 0.0) || !(m_star > 0.0)) return GENGA_KICK_E_SIZE;
     const long long N = ctx->N;
     genga::rcrit_kernel<<<genga::step_blocks(N), GENGA_STEP_THREADS, 0, ctx->stream>>>(
-        pos, vel, mass, N, ctx->cfg.G * m_star, m_star, dt, substeps, nrows, n1, n2, out_rcrit, ctx->status);
+        pos, vel, mass, N, ctx->cfg.G * m_star, m_star, dt, substeps, nrows, n1, n2, out_rcrit, ctx->status, nullptr,
+        nullptr, 0);
+    GK_CUDA(ctx, cudaGetLastError());
+    ctx->launches++;
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_rcrit_list(genga_kick_ctx* ctx, const double* pos, const double* vel, const double* mass,
+                                double m_star, double dt, double substeps, int32_t nrows, double n1, double n2,
+                                const int32_t* list, const int32_t* n_list, int64_t list_rows, double* out_rcrit)
+{
+    if (!ctx || !pos || !vel || !mass || !out_rcrit || !list || !n_list) return GENGA_KICK_E_NULL;
+    if (genga_misaligned(pos) || genga_misaligned(vel) || genga_misaligned(mass) || genga_misaligned(out_rcrit) ||
+        genga_misaligned(list))
+        return GENGA_KICK_E_ALIGN;
+    if (nrows < 1 || !(substeps > 0.0) || !(m_star > 0.0) || list_rows < 0) return GENGA_KICK_E_SIZE;
+    const long long N = ctx->N;
+    const int blocks = (int)std::min<long long>(std::max<long long>((list_rows + GENGA_STEP_THREADS - 1) / GENGA_STEP_THREADS, 1),
+                                                GENGA_PSUM_BLOCKS);
+    genga::rcrit_kernel<<<blocks, GENGA_STEP_THREADS, 0, ctx->stream>>>(
+        pos, vel, mass, N, ctx->cfg.G * m_star, m_star, dt, substeps, nrows, n1, n2, out_rcrit, ctx->status, list, n_list,
+        list_rows);
+    GK_CUDA(ctx, cudaGetLastError());
+    ctx->launches++;
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_fg_list(genga_kick_ctx* ctx, double* pos, double* vel, double m_star, double dt, const int32_t* list,
+                             const int32_t* n_list, int64_t list_rows)
+{
+    if (!ctx || !pos || !vel || !list || !n_list) return GENGA_KICK_E_NULL;
+    if (genga_misaligned(pos) || genga_misaligned(vel) || genga_misaligned(list)) return GENGA_KICK_E_ALIGN;
+    if (!(m_star > 0.0) || list_rows < 0) return GENGA_KICK_E_SIZE;
+    const int blocks = (int)std::min<long long>(std::max<long long>((list_rows + GENGA_STEP_THREADS - 1) / GENGA_STEP_THREADS, 1),
+                                                GENGA_PSUM_BLOCKS);
+    genga::fg_list_kernel<<<blocks, GENGA_STEP_THREADS, 0, ctx->stream>>>(pos, vel, ctx->N, ctx->cfg.G * m_star, dt, list,
+                                                                         n_list, list_rows, ctx->status);
     GK_CUDA(ctx, cudaGetLastError());
     ctx->launches++;
     return GENGA_KICK_OK;

@@ -18,6 +18,7 @@ namespace genga {
 #define GENGA_STEP_THREADS 256
 #define GENGA_PSUM_BLOCKS 1024          // most CTAs of a step kernel = rows of the partial-sum scratch
 #define GENGA_STATUS_UNBOUND 8
+#define GENGA_STATUS_BAD_INDEX 16       // an index of a body list outside [0, N): entry ignored
 
 __host__ __device__ __forceinline__ int step_blocks(long long N)
 {
@@ -38,10 +39,15 @@ __host__ __device__ __forceinline__ long long step_chunk(long long N)
 __global__ void __launch_bounds__(GENGA_STEP_THREADS)
 rcrit_kernel(const double* __restrict__ pos, const double* __restrict__ vel, const double* __restrict__ mass,
              long long N, double mu, double m_star, double dt, double substeps, int nrows, double n1, double n2,
-             double* __restrict__ out, int* __restrict__ status)
+             double* __restrict__ out, int* __restrict__ status, const int* __restrict__ list,
+             const int* __restrict__ n_list, long long list_rows)
 {
-    const long long chunk = step_chunk(N), base = (long long)blockIdx.x * chunk;
-    for (long long i = base + threadIdx.x; i < base + chunk && i < N; i += GENGA_STEP_THREADS) {
+    // list == nullptr: every body; else the bodies list[0 .. min(*n_list, list_rows)) ("RcritS", App. A)
+    const long long count = list ? min((long long)max(*n_list, 0), list_rows) : N;
+    for (long long q = (long long)blockIdx.x * GENGA_STEP_THREADS + threadIdx.x; q < count;
+         q += (long long)gridDim.x * GENGA_STEP_THREADS) {
+        const long long i = list ? list[q] : q;
+        if (i < 0 || i >= N) { atomicOr(status, GENGA_STATUS_BAD_INDEX); continue; }
         const double x = pos[i], y = pos[N + i], z = pos[2 * N + i];
         const double vx = vel[i], vy = vel[N + i], vz = vel[2 * N + i];
         const double r = sqrt(fma(z, z, fma(y, y, x * x)));
@@ -218,6 +224,24 @@ fg_kernel(double* __restrict__ pos, double* __restrict__ vel, const double* __re
     if (SHIFT) {
         block_sum3(px, py, pz);
         publish_sum3(px, py, pz, partial, ticket, slot_out);
+    }
+}
+
+// "FGS" (App. A): the Kepler drift of the bodies of a list only
+__global__ void __launch_bounds__(GENGA_STEP_THREADS)
+fg_list_kernel(double* __restrict__ pos, double* __restrict__ vel, long long N, double mu, double dt,
+               const int* __restrict__ list, const int* __restrict__ n_list, long long list_rows, int* __restrict__ status)
+{
+    const long long count = min((long long)max(*n_list, 0), list_rows);
+    for (long long q = (long long)blockIdx.x * GENGA_STEP_THREADS + threadIdx.x; q < count;
+         q += (long long)gridDim.x * GENGA_STEP_THREADS) {
+        const long long i = list[q];
+        if (i < 0 || i >= N) { atomicOr(status, GENGA_STATUS_BAD_INDEX); continue; }
+        double x = pos[i], y = pos[N + i], z = pos[2 * N + i];
+        double vx = vel[i], vy = vel[N + i], vz = vel[2 * N + i];
+        if (!kepler_fg(mu, dt, x, y, z, vx, vy, vz)) atomicOr(status, GENGA_STATUS_UNBOUND);
+        pos[i] = x; pos[N + i] = y; pos[2 * N + i] = z;
+        vel[i] = vx; vel[N + i] = vy; vel[2 * N + i] = vz;
     }
 }
 

@@ -226,3 +226,52 @@ def test_step_error_codes():
             call()
         assert e.value.code == code
     k.free()
+
+
+def test_rcritS_fgS_on_the_members_of_the_groups(oracle_mod):
+    """RcritS / FGS (App. A): the device chain kick -> group -> rcrit_list / fg_list on `members`
+    with no host round trip; listed bodies match the oracle's Rcrit / FG, the others are not touched."""
+    import torch
+    import paper_2201_10058_b200 as g
+    ost = oracle_mod.step
+    ki = gi.make_config(3, n=20000, level=1)
+    n = ki.n
+    k = _ctx(ki)
+    pos, vel, mass = _dev(ki.pos), _dev(ki.vel), _dev(ki.mass)
+    acc = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    pairs = torch.empty(1 << 20, 2, dtype=torch.int32, device="cuda")
+    npairs = torch.empty(n + 1, dtype=torch.int32, device="cuda")
+    k.kick(pos, None, mass, _dev(ki.rcrit[:1]), 0, ki.dt, acc, pairs, npairs)
+    i32 = lambda m: torch.empty(m, dtype=torch.int32, device="cuda")
+    group_of, members, offsets, summary = i32(n), i32(n), i32(n + 1), i32(4)
+    k.group(pairs, npairs[n:], 1 << 20, group_of, members, offsets, summary)
+    rc = torch.full((2, n), -1.0, dtype=torch.float64, device="cuda")
+    k.rcrit_list(pos, vel, mass, 1.0, 0.5 * ki.dt, members, summary[1:], n, rc, substeps=2.0, nrows=2)
+    q, v = pos.clone(), vel.clone()
+    k.fg_list(q, v, 1.0, 0.5 * ki.dt, members, summary[1:], n)
+    torch.cuda.synchronize()
+    assert k.status() == 0
+    nm = int(summary[1])
+    mem = members[:nm].cpu().numpy()
+    assert 1000 < nm < n
+    inlist = np.zeros(n, bool); inlist[mem] = True
+    want_rc, _ = ost.rcrit(ki.pos, ki.vel, ki.mass, 1.0, ki.G, 0.5 * ki.dt, 2.0, 2)
+    got_rc = rc.cpu().numpy()
+    assert np.all(np.abs(got_rc[:, inlist] - want_rc[:, inlist]) <= 16 * U * want_rc[:, inlist])
+    assert np.all(got_rc[:, ~inlist] == -1.0)
+    qw, vw, _ = ost.fg(ki.pos, ki.vel, ki.G, 0.5 * ki.dt)
+    sq, sv = _scales(ki.pos, ki.vel, 0.5 * ki.dt)
+    gq, gv = q.cpu().numpy(), v.cpu().numpy()
+    assert np.all(np.abs(gq[:, inlist] - qw[:, inlist]) <= 32 * U * sq[inlist])
+    assert np.all(np.abs(gv[:, inlist] - vw[:, inlist]) <= 32 * U * sv[inlist])
+    assert np.array_equal(gq[:, ~inlist], ki.pos[:, ~inlist]) and np.array_equal(gv[:, ~inlist], ki.vel[:, ~inlist])
+    # the same bits as the all-bodies kernels on the listed bodies
+    q2, v2 = pos.clone(), vel.clone()
+    k.fg(q2, v2, 1.0, 0.5 * ki.dt)
+    assert np.array_equal(q2.cpu().numpy()[:, inlist], gq[:, inlist])
+    # a bad index is ignored and reported
+    bad = torch.tensor([5, n + 3, -2, 7], dtype=torch.int32, device="cuda")
+    cnt = torch.tensor([4, 0, 0, 0], dtype=torch.int32, device="cuda")
+    k.fg_list(q, v, 1.0, 1.0, bad, cnt, 4)
+    assert k.status() & 16
+    k.free()
