@@ -275,3 +275,36 @@ def test_rcritS_fgS_on_the_members_of_the_groups(oracle_mod):
     k.fg_list(q, v, 1.0, 1.0, bad, cnt, 4)
     assert k.status() & 16
     k.free()
+
+
+def test_step_can_be_captured_in_a_cuda_graph():
+    """After one warm-up call (lazy scratch allocation) the library only enqueues kernels and async memsets on its
+    stream: a caller may capture genga_step in a CUDA graph (launch-bound small-N loops) and gets the same bits."""
+    import torch
+    ki = gi.make_config(0, n=2048)
+    n = ki.n
+    k = _ctx(ki, capacity=1 << 16)
+    q, v, mass = _dev(ki.pos), _dev(ki.vel), _dev(ki.mass)
+    acc = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    pairs = torch.empty(1 << 16, 2, dtype=torch.int32, device="cuda")
+    npairs = torch.empty(n + 1, dtype=torch.int32, device="cuda")
+    rrow = torch.empty(n, dtype=torch.float64, device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        k.set_stream(s.cuda_stream)
+        k.step(q, v, mass, 1.0, ki.dt, rrow, acc, pairs, npairs)           # warm-up
+        q.copy_(_dev(ki.pos)); v.copy_(_dev(ki.vel))
+        for _ in range(5):
+            k.step(q, v, mass, 1.0, ki.dt, rrow, acc, pairs, npairs)
+        s.synchronize()
+        qe, ve, ne = q.clone(), v.clone(), npairs.clone()
+        q.copy_(_dev(ki.pos)); v.copy_(_dev(ki.vel))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            k.step(q, v, mass, 1.0, ki.dt, rrow, acc, pairs, npairs)
+        q.copy_(_dev(ki.pos)); v.copy_(_dev(ki.vel))
+        for _ in range(5):
+            g.replay()
+        s.synchronize()
+    assert torch.equal(q, qe) and torch.equal(v, ve) and torch.equal(npairs, ne) and k.status() == 0
+    k.free()
