@@ -1,0 +1,55 @@
+/*
+ * genga_bs.h -- C ABI of the Bulirsch-Stoer integration of close-encounter groups.
+ *
+ * "We also use a Bulirsch-Stoer ... method to resolve the close-encounter part" (arXiv 2201.10058 sec. 2,
+ * PAPER.md:47); "All particles in a given close-encounter group need to be integrated synchronously"
+ * (sec. 6.1); App. A `Bulirsch-Stoer(dt)`.  For every group of genga_group the
+ * part H_A of the Hamiltonian (eq. 2) restricted to the group's bodies is integrated over
+ * dt, starting from the state BEFORE the Kepler drift FG:
+ *
+ *     dq_i/dt = v_i
+ *     dv_i/dt = - G m_star q_i / |q_i|^3 + sum_{j in group, j != i} G m_j W_BS(r_ij) (q_j - q_i) / r_ij^3
+ *     W_BS    = prod_{k < nlevels} [1 - K(r_ij; max(rcrit[k][i], rcrit[k][j]))]          (eq. 62-63)
+ *
+ * (nlevels = 1: the complement of the kick's weight).  The result REPLACES the Kepler-drifted state of
+ * the group's bodies; bodies in no group are not touched.
+ *
+ * Method (the paper names it and refers to Grimm & Stadel 2014; reading G15): Gragg-Bulirsch-
+ * Stoer -- modified midpoint with 2, 4, .., 16 sub-steps, polynomial extrapolation in h^2, relative error
+ * per body in position and velocity <= tol, one step size for the whole group (halved on failure, doubled
+ * after fast convergence).  One thread block per group, one thread per body: the regimes BS-B / BS-A of
+ * Table 2, groups of up to 256 bodies.  Larger groups (BS-M) are NOT
+ * integrated: they keep the state already in pos / vel and GENGA_KICK_STATUS_GROUP_TOO_LARGE is set --
+ * sec. 6.3's higher symplectic levels exist to keep groups below that size.
+ *
+ * Works on the context of genga_kick.h (its N, G, stream); only enqueues; all pointers are DEVICE pointers.
+ */
+#ifndef GENGA_BS_H
+#define GENGA_BS_H
+
+#include "genga_kick.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GENGA_KICK_STATUS_GROUP_TOO_LARGE 32   /* a group of more than 256 bodies was left as it was       */
+#define GENGA_KICK_STATUS_BS_NOT_CONVERGED 64  /* a step did not reach tol after 60 halvings: that group
+                                                  stopped at its last accepted time                        */
+#define GENGA_BS_MAX_GROUP 256
+
+/*
+ *   pos_in, vel_in  [3][N] state before FG (read only)          mass [N]
+ *   rcrit           [nlevels][N], 1 <= nlevels <= 4
+ *   members, offsets, summary   as written by genga_group (summary[0] = number of groups, read on the device)
+ *   pos, vel        [3][N] updated for the bodies of the integrated groups (may NOT alias pos_in / vel_in)
+ * Errors: E_NULL, E_ALIGN, E_SIZE (nlevels outside 1..4, m_star <= 0, tol <= 0), E_CUDA.
+ */
+int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double* vel_in, const double* mass, const double* rcrit,
+             int32_t nlevels, double m_star, double dt, double tol, const int32_t* members, const int32_t* offsets,
+             const int32_t* summary, double* pos, double* vel);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GENGA_BS_H */

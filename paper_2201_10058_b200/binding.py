@@ -26,6 +26,9 @@ STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_ste
 # include/genga_group.h: close-encounter groups
 GROUP_EXPORTS = ("genga_group",)
 STATUS_BAD_PAIR = 16
+# include/genga_bs.h: Bulirsch-Stoer integration of the groups
+BS_EXPORTS = ("genga_bs",)
+STATUS_GROUP_TOO_LARGE, STATUS_BS_NOT_CONVERGED = 32, 64
 STATUS_UNBOUND = 8
 
 
@@ -92,7 +95,8 @@ def lib():
         L.genga_fg_list.argtypes = [vp, vp, vp, d, d, vp, vp, i64]
         L.genga_step.argtypes = [vp, vp, vp, vp, d, d, d, d, vp, vp, vp, vp]
         L.genga_group.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
-        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS:
+        L.genga_bs.argtypes = [vp, vp, vp, vp, vp, i32, d, d, d, vp, vp, vp, vp, vp]
+        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
                 getattr(L, name).restype = C.c_int
         _lib = L
@@ -211,6 +215,12 @@ class GengaKick:
         """n_pairs: a device int32 tensor VIEW whose first element is the pair count (e.g. out_npairs[N:])."""
         self._check(lib().genga_group(self._ctx, _ptr(pairs), _ptr(n_pairs), int(pair_rows), _ptr(group_of),
                                       _ptr(members), _ptr(offsets), _ptr(summary)))
+
+    # include/genga_bs.h
+    def bs(self, pos_in, vel_in, mass, rcrit, nlevels, m_star, dt, tol, members, offsets, summary, pos, vel):
+        self._check(lib().genga_bs(self._ctx, _ptr(pos_in), _ptr(vel_in), _ptr(mass), _ptr(rcrit), int(nlevels),
+                                   float(m_star), float(dt), float(tol), _ptr(members), _ptr(offsets), _ptr(summary),
+                                   _ptr(pos), _ptr(vel)))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

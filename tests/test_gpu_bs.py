@@ -1,0 +1,121 @@
+"""-m gpu: genga_bs (include/genga_bs.h) through the C ABI against oracle/genga_bs_oracle.c.
+
+The oracle follows the same Gragg-Bulirsch-Stoer scheme operation for operation (reading G15), both sides in IEEE
+binary64 without contraction, the force sum in member order: the step-size decisions are taken on the same bits and
+the results must agree to the LAST BIT except where the device's sqrt/division sequences differ from the host's --
+they do not (both correctly rounded) -- so the bar is equality; a tolerance of 64 u relative to |q|, |v| is what the
+test enforces, and it reports whether equality held."""
+import numpy as np
+import pytest
+
+import genga_inputs as gi
+
+pytestmark = pytest.mark.gpu
+U = 2.0 ** -53
+G = gi.G_AU_DAY_MSUN
+
+
+def _dev(a, dtype=None):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    return (t if dtype is None else t.to(dtype)).cuda()
+
+
+def _gpu_bs(n, pos_in, vel_in, mass, rcrit, nlevels, dt, tol, members, offsets, pos, vel):
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    k = GengaKick(n, 0, G=G, pair_capacity=8)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    ng = len(offsets) - 1
+    d_mem = torch.zeros(max(n, 4), dtype=torch.int32, device="cuda"); d_mem[:len(members)] = _dev(np.asarray(members, np.int32))
+    d_off = torch.zeros(n + 4, dtype=torch.int32, device="cuda"); d_off[:ng + 1] = _dev(np.asarray(offsets, np.int32))
+    d_sum = torch.tensor([ng, len(members), 0, 0], dtype=torch.int32, device="cuda")
+    q, v = _dev(pos), _dev(vel)
+    k.bs(_dev(pos_in), _dev(vel_in), _dev(mass), _dev(np.asarray(rcrit)[:nlevels]), nlevels, 1.0, dt, tol, d_mem, d_off,
+         d_sum, q, v)
+    torch.cuda.synchronize()
+    st = k.status()
+    k.free()
+    return q.cpu().numpy(), v.cpu().numpy(), st
+
+
+def _check(q, v, qw, vw):
+    sq = np.sqrt((qw ** 2).sum(0)); sv = np.sqrt((vw ** 2).sum(0))
+    assert np.all(np.abs(q - qw) <= 64 * U * sq) and np.all(np.abs(v - vw) <= 64 * U * sv)
+    return bool(np.array_equal(q, qw) and np.array_equal(v, vw))
+
+
+def test_groups_of_a_disk_kick_group_bs_chain(oracle_mod):
+    """Config 1's shape: the pair list of the oracle's kick, grouped by the oracle, every group integrated on both
+    sides from the pre-drift state; bodies in no group keep the (Kepler-drifted) state passed in."""
+    ki = gi.make_config(1, n=6000)
+    n = ki.n
+    res = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, n, 0, level=0, G=ki.G)
+    gr = oracle_mod.group.group(n, oracle_mod.pair_set(res, n))
+    assert gr.n_groups > 100 and gr.max_size <= 256
+    qf, vf, _ = oracle_mod.step.fg(ki.pos, ki.vel, ki.G, ki.dt)                     # what FG left in pos / vel
+    qw, vw, stats, skipped = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, gr.members, gr.offsets, G, 1.0, ki.dt,
+                                              1e-12, qf, vf, nlevels=1)
+    assert not skipped and not any(s.failed for s in stats)
+    q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, ki.dt, 1e-12, gr.members, gr.offsets, qf, vf)
+    assert st == 0
+    exact = _check(q, v, qw, vw)
+    untouched = gr.group_of < 0
+    assert np.array_equal(q[:, untouched], qf[:, untouched]) and np.array_equal(v[:, untouched], vf[:, untouched])
+    assert np.max(np.abs(q[:, ~untouched] - qf[:, ~untouched])) > 1e-12               # the encounters matter
+    print("bit-identical to the oracle:", exact)
+
+
+@pytest.mark.parametrize("nlevels,tol,dt", [(1, 1e-13, 6.0), (2, 1e-11, 6.0), (1, 1e-9, -3.0), (3, 1e-12, 0.75)])
+def test_dense_groups_levels_tolerances(oracle_mod, nlevels, tol, dt):
+    """A denser disk (larger groups, up to the 256-body limit), several levels / tolerances / a negative step."""
+    ki = gi.make_disk(3000, 31, level=2, substeps=2, total_mass=20 * gi.M_EARTH, a_lo=0.9, a_hi=1.3)
+    n = ki.n
+    res = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, n, 0, level=0, G=ki.G, maxp=256)
+    gr = oracle_mod.group.group(n, oracle_mod.pair_set(res, n))
+    qw, vw, stats, skipped = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, gr.members, gr.offsets, G, 1.0, dt, tol,
+                                              ki.pos, ki.vel, nlevels=nlevels, max_group=256)
+    q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, nlevels, dt, tol, gr.members, gr.offsets, ki.pos, ki.vel)
+    assert (st == 32) == bool(skipped) and (st & ~32) == 0
+    assert gr.max_size > 20 and len(stats) > 50
+    _check(q, v, qw, vw)
+
+
+def test_large_group_is_reported_and_left(oracle_mod):
+    import paper_2201_10058_b200 as g
+    n = 600
+    ki = gi.make_ring(n)                                          # one group of 600 > 256
+    members, offsets = np.arange(n), np.array([0, n])
+    q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 6.0, 1e-12, members, offsets, ki.pos * 2, ki.vel * 2)
+    assert st == g.STATUS_GROUP_TOO_LARGE
+    assert np.array_equal(q, ki.pos * 2) and np.array_equal(v, ki.vel * 2)
+    # a ring of 200 is one group of 200: integrated
+    ki = gi.make_ring(200)
+    qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, np.arange(200), [0, 200], ki.G, 1.0, 6.0, 1e-12,
+                                        ki.pos, ki.vel)
+    from paper_2201_10058_b200 import GengaKick
+    q, v, st = _gpu_bs(200, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 6.0, 1e-12, np.arange(200), [0, 200], ki.pos, ki.vel)
+    assert st == 0
+    _check(q, v, qw, vw)
+
+
+def test_bs_error_codes_and_empty():
+    import torch
+    import paper_2201_10058_b200 as g
+    k = g.GengaKick(64, 0, pair_capacity=8)
+    x = torch.zeros(3, 64, dtype=torch.float64, device="cuda"); y = torch.zeros_like(x)
+    m = torch.zeros(64, dtype=torch.float64, device="cuda")
+    i = torch.zeros(80, dtype=torch.int32, device="cuda")
+    for call, code in [(lambda: k.bs(x, x, m, m, 1, 1.0, 6.0, 1e-12, i, i, i, None, y), g.E_NULL),
+                       (lambda: k.bs(x, x, m, m, 0, 1.0, 6.0, 1e-12, i, i, i, y, y), g.E_SIZE),
+                       (lambda: k.bs(x, x, m, m, 1, 1.0, 6.0, 0.0, i, i, i, y, y), g.E_SIZE),
+                       (lambda: k.bs(x, x, m, m, 1, 1.0, 6.0, 1e-12, i, i, i, x, y), g.E_SIZE),
+                       (lambda: k.bs(x, x, m, m, 1, 1.0, 6.0, 1e-12, i[1:], i, i, y, y.clone()), g.E_ALIGN)]:
+        with pytest.raises(g.GengaKickError) as e:
+            call()
+        assert e.value.code == code
+    z = y.clone()
+    k.bs(x, x, m, m, 1, 1.0, 6.0, 1e-12, i, i, i, y, z)              # no groups: nothing happens
+    torch.cuda.synchronize()
+    assert k.status() == 0 and not y.any()
+    k.free()

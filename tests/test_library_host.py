@@ -48,6 +48,15 @@ def test_every_declared_group_symbol_is_exported(built):
     assert all(hasattr(lib, name) for name in declared)
 
 
+def test_every_declared_bs_symbol_is_exported(built):
+    header = open(os.path.join(ROOT, "include", "genga_bs.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\bint\s+(genga_\w+)\s*\(", header))
+    assert declared == set(g.BS_EXPORTS)
+    lib = ctypes.CDLL(built)
+    assert all(hasattr(lib, name) for name in declared)
+
+
 def test_strerror_texts(built):
     for code in (g.OK, g.E_NULL, g.E_ALIGN, g.E_SIZE, g.E_LEVEL, g.E_CUDA, g.E_NOMEM):
         assert g.strerror(code) and "unknown" not in g.strerror(code)
