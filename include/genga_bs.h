@@ -49,6 +49,22 @@ int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double* vel_in, co
              int32_t nlevels, double m_star, double dt, double tol, const int32_t* members, const int32_t* offsets,
              const int32_t* summary, double* pos, double* vel);
 
+/*
+ * The complete step of App. A on the device, no host round trip:
+ *     Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt); grouping; Bulirsch-Stoer(dt) on the groups, from the
+ *     state before FG; HC(dt/2); Kick(dt/2).
+ * Every candidate pair of the pre-check is treated as an encounter pair (the paper's separate "close-encounter
+ * detection" has no printed criterion; a pair that never enters its critical radius has W_BS = 0, so integrating
+ * it is only extra work).  pos, vel are advanced in place; out_pairs / out_npairs: the candidates of the first
+ * kick; group_of / members / offsets / summary: their groups, as genga_group writes them (all four required);
+ * out_acc: acceleration of the closing kick, or NULL.  Groups above 256 bodies keep their Kepler-drifted state and
+ * set GENGA_KICK_STATUS_GROUP_TOO_LARGE.
+ * Errors: E_NULL, E_ALIGN, E_SIZE, E_CUDA.
+ */
+int genga_hybrid_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
+                      double n1, double n2, double tol, double* out_acc, int32_t* out_pairs, int32_t* out_npairs,
+                      int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary);
+
 #ifdef __cplusplus
 }
 #endif

@@ -77,3 +77,39 @@ def step(pos, vel, mass, n_massive, n_test, m_star, G, dt, enc_factor=1.0, n1=3.
     k2 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor)
     v = v + (0.5 * dt) * k2.acc
     return StepResult(pos=q, vel=v, rcrit=rc, first=k1, second=k2, unbound=bad0 + bad1)
+
+
+@dataclass
+class HybridStepResult:
+    pos: np.ndarray
+    vel: np.ndarray
+    rcrit: np.ndarray
+    first: _kick.OracleResult
+    groups: object           # oracle.group.Groups of the first kick's pair list
+    skipped: list            # groups larger than max_group (left at their Kepler-drifted state)
+    unbound: int
+
+
+def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc_factor=1.0, n1=3.0, n2=0.4,
+                max_group=256):
+    """The complete scheme of App. A, every candidate pair of the pre-check treated as an encounter
+    pair (no separate detection: PAPER.md gives no criterion, and a pair that never enters its critical radius has
+    W_BS = 0, so integrating it is only extra work):
+        Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt); grouping; Bulirsch-Stoer(dt) on the groups, from the
+        state before FG; HC(dt/2); Kick(dt/2)."""
+    from . import group as _group, bs as _bs
+    q, v, mass = _c(pos).copy(), _c(vel).copy(), _c(mass)
+    n = q.shape[1]
+    rc, bad0 = rcrit(q, v, mass, m_star, G, dt, 2.0, 1, n1, n2)
+    k1 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    v = v + (0.5 * dt) * k1.acc
+    q, _ = hc(q, v, mass, m_star, 0.5 * dt)
+    q_in, v_in = q.copy(), v.copy()
+    q, v, bad1 = fg(q, v, G * m_star, dt)
+    gr = _group.group(n, _kick.pair_set(k1, n_massive))
+    q, v, _, skipped = _bs.bs(q_in, v_in, mass, rc, gr.members, gr.offsets, G, m_star, dt, tol, q, v, nlevels=1,
+                              max_group=max_group)
+    q, _ = hc(q, v, mass, m_star, 0.5 * dt)
+    k2 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    v = v + (0.5 * dt) * k2.acc
+    return HybridStepResult(pos=q, vel=v, rcrit=rc, first=k1, groups=gr, skipped=skipped, unbound=bad0 + bad1)

@@ -27,7 +27,7 @@ STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_ste
 GROUP_EXPORTS = ("genga_group",)
 STATUS_BAD_PAIR = 16
 # include/genga_bs.h: Bulirsch-Stoer integration of the groups
-BS_EXPORTS = ("genga_bs",)
+BS_EXPORTS = ("genga_bs", "genga_hybrid_step")
 STATUS_GROUP_TOO_LARGE, STATUS_BS_NOT_CONVERGED = 32, 64
 STATUS_UNBOUND = 8
 
@@ -95,6 +95,7 @@ def lib():
         L.genga_fg_list.argtypes = [vp, vp, vp, d, d, vp, vp, i64]
         L.genga_step.argtypes = [vp, vp, vp, vp, d, d, d, d, vp, vp, vp, vp]
         L.genga_group.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
+        L.genga_hybrid_step.argtypes = [vp, vp, vp, vp, d, d, d, d, d, vp, vp, vp, vp, vp, vp, vp]
         L.genga_bs.argtypes = [vp, vp, vp, vp, vp, i32, d, d, d, vp, vp, vp, vp, vp]
         for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
@@ -221,6 +222,12 @@ class GengaKick:
         self._check(lib().genga_bs(self._ctx, _ptr(pos_in), _ptr(vel_in), _ptr(mass), _ptr(rcrit), int(nlevels),
                                    float(m_star), float(dt), float(tol), _ptr(members), _ptr(offsets), _ptr(summary),
                                    _ptr(pos), _ptr(vel)))
+
+    def hybrid_step(self, pos, vel, mass, m_star, dt, tol, out_acc, out_pairs, out_npairs, group_of, members, offsets,
+                    summary, n1=3.0, n2=0.4):
+        self._check(lib().genga_hybrid_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt), float(n1),
+                                            float(n2), float(tol), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs),
+                                            _ptr(group_of), _ptr(members), _ptr(offsets), _ptr(summary)))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

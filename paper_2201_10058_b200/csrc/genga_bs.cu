@@ -1,5 +1,7 @@
 // C ABI of the Bulirsch-Stoer integration of close-encounter groups (include/genga_bs.h).  Host side only.
 #include "../../include/genga_bs.h"
+#include "../../include/genga_group.h"
+#include "../../include/genga_step.h"
 #include "genga_kick_ctx.h"
 #include "genga_bs_kernels.cuh"
 
@@ -27,4 +29,36 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     GK_CUDA(ctx, cudaGetLastError());
     ctx->launches++;
     return GENGA_KICK_OK;
+}
+
+extern "C" int genga_hybrid_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
+                                 double n1, double n2, double tol, double* out_acc, int32_t* out_pairs, int32_t* out_npairs,
+                                 int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary)
+{
+    if (!ctx || !pos || !vel || !mass || !out_npairs || !group_of || !members || !offsets || !summary)
+        return GENGA_KICK_E_NULL;
+    if (!out_pairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
+    const size_t N = (size_t)ctx->N;
+    if (!ctx->step_rcrit) GK_CUDA(ctx, cudaMalloc(&ctx->step_rcrit, N * sizeof(double)));
+    if (!ctx->hyb_state) GK_CUDA(ctx, cudaMalloc(&ctx->hyb_state, 6 * N * sizeof(double)));
+    double* q_in = ctx->hyb_state;
+    double* v_in = ctx->hyb_state + 3 * N;
+    cudaStream_t st = ctx->stream;
+    int rc = genga_rcrit(ctx, pos, vel, mass, m_star, dt, 2.0, 1, n1, n2, ctx->step_rcrit);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_kick(ctx, pos, vel, mass, ctx->step_rcrit, 0, 0.5 * dt, nullptr, out_pairs, out_npairs);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_hc(ctx, pos, vel, mass, m_star, 0.5 * dt);
+    if (rc != GENGA_KICK_OK) return rc;
+    GK_CUDA(ctx, cudaMemcpyAsync(q_in, pos, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    GK_CUDA(ctx, cudaMemcpyAsync(v_in, vel, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    rc = genga_fg(ctx, pos, vel, m_star, dt);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_group(ctx, out_pairs, out_npairs + N, ctx->cfg.pair_capacity, group_of, members, offsets, summary);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_bs(ctx, q_in, v_in, mass, ctx->step_rcrit, 1, m_star, dt, tol, members, offsets, summary, pos, vel);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_hc(ctx, pos, vel, mass, m_star, 0.5 * dt);
+    if (rc != GENGA_KICK_OK) return rc;
+    return genga_kick_impl(ctx, pos, vel, mass, ctx->step_rcrit, 0, 0.5 * dt, out_acc, nullptr, nullptr);
 }

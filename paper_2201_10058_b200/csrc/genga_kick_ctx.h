@@ -55,6 +55,7 @@ struct genga_kick_ctx {
     // grouping (genga_group.cu), lazily allocated
     int* grp_label; int* grp_flag; unsigned* grp_keys_a; unsigned* grp_keys_b; int* grp_vals_a; int* grp_vals_b;
     int* grp_counts;
+    double* hyb_state;             // [6][N] state before FG (genga_hybrid_step), lazily allocated
     std::string cuda_err;
 };
 

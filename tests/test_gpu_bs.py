@@ -119,3 +119,71 @@ def test_bs_error_codes_and_empty():
     torch.cuda.synchronize()
     assert k.status() == 0 and not y.any()
     k.free()
+
+
+def _hybrid_buffers(n, cap):
+    import torch
+    i32 = lambda m: torch.empty(m, dtype=torch.int32, device="cuda")
+    return (torch.empty(3, n, dtype=torch.float64, device="cuda"), torch.empty(cap, 2, dtype=torch.int32, device="cuda"),
+            i32(n + 1), i32(n), i32(n), i32(n + 1), i32(4))
+
+
+def test_hybrid_step_against_oracle(oracle_mod):
+    """genga_hybrid_step (kick, HC, FG, grouping, Bulirsch-Stoer, HC, kick on the device) against oracle.step.hybrid_step."""
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    ki = gi.make_config(1, n=5000)
+    n = ki.n
+    k = GengaKick(n, 0, G=ki.G, pair_capacity=1 << 18)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, v, mass = _dev(ki.pos), _dev(ki.vel), _dev(ki.mass)
+    acc, pairs, npairs, group_of, members, offsets, summary = _hybrid_buffers(n, 1 << 18)
+    k.hybrid_step(q, v, mass, 1.0, ki.dt, 1e-12, acc, pairs, npairs, group_of, members, offsets, summary)
+    torch.cuda.synchronize()
+    r = oracle_mod.step.hybrid_step(ki.pos, ki.vel, ki.mass, n, 0, 1.0, ki.G, ki.dt, tol=1e-12)
+    assert k.status() == 0 and not r.skipped and r.groups.n_groups > 50
+    s = summary.cpu().numpy()
+    assert s[0] == r.groups.n_groups and s[1] == r.groups.n_members and s[2] == r.groups.max_size
+    assert np.array_equal(group_of.cpu().numpy(), r.groups.group_of)
+    rr = np.sqrt((ki.pos ** 2).sum(0)); sp = np.sqrt((ki.vel ** 2).sum(0))
+    sq, sv = rr + sp * ki.dt, sp + rr * np.sqrt(ki.G / rr ** 3)
+    # the states entering Bulirsch-Stoer differ by the kick's and HC's rounding (<= 32 u); an encounter amplifies that
+    # by the ratio of the step to the encounter time scale: 1e-10 relative is a generous bound for these groups
+    in_group = r.groups.group_of >= 0
+    assert np.all(np.abs(q.cpu().numpy() - r.pos)[:, ~in_group] <= 32 * U * sq[~in_group])
+    assert np.all(np.abs(v.cpu().numpy() - r.vel)[:, ~in_group] <= 32 * U * sv[~in_group])
+    assert np.all(np.abs(q.cpu().numpy() - r.pos)[:, in_group] <= 1e-10 * sq[in_group])
+    assert np.all(np.abs(v.cpu().numpy() - r.vel)[:, in_group] <= 1e-10 * sv[in_group])
+    k.free()
+
+
+def test_hybrid_step_keeps_the_energy_through_an_encounter():
+    """The device integrator through the close encounter of tests/test_step_oracle_pins.py: energy error < 1e-5
+    (the plain step loses 6e-3 there)."""
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    mass = np.array([3e-5, 3e-5])
+    a = np.array([1.0, 1.02]); e = np.array([0.02, 0.03]); z = np.zeros(2)
+    pos, vel = gi.elements_to_cartesian(a, e, z + 0.001, z, np.array([0.0, 0.6]), np.array([0.0, -0.57]), G)
+    vel = vel - (mass * vel).sum(1, keepdims=True) / (1.0 + mass.sum())
+
+    def energy(q, v):
+        p = mass * v
+        return (0.5 * (mass * (v * v).sum(0)).sum() + 0.5 * (p.sum(1) ** 2).sum() - (G * mass / np.sqrt((q * q).sum(0))).sum()
+                - G * mass[0] * mass[1] / np.sqrt(((q[:, 0] - q[:, 1]) ** 2).sum()))
+
+    e0 = energy(pos, vel)
+    k = GengaKick(2, 0, G=G, pair_capacity=16)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, v, m = _dev(pos), _dev(vel), _dev(mass)
+    acc, pairs, npairs, group_of, members, offsets, summary = _hybrid_buffers(2, 16)
+    worst, enc, dmin = 0.0, 0, 1e9
+    for _ in range(400):
+        k.hybrid_step(q, v, m, 1.0, 2.0, 1e-13, acc, pairs, npairs, group_of, members, offsets, summary)
+        enc += int(summary[0])
+        qq, vv = q.cpu().numpy(), v.cpu().numpy()
+        dmin = min(dmin, np.sqrt(((qq[:, 0] - qq[:, 1]) ** 2).sum()))
+        worst = max(worst, abs(energy(qq, vv) - e0) / abs(e0))
+    assert k.status() == 0 and enc > 3 and dmin < 5e-3
+    assert worst < 1e-5
+    k.free()

@@ -201,3 +201,34 @@ def test_step_reports_the_first_kicks_candidates(st, oracle_mod):
     assert np.max(np.abs(r.rcrit - ki.rcrit[:1]) / ki.rcrit[:1]) < 1e-13
     ref = oracle_mod.kick(ki.pos, ki.mass, r.rcrit, ki.n, 0, level=0, G=ki.G)
     assert np.array_equal(ref.count, r.first.count) and ref.count.sum() > 0
+
+
+def test_hybrid_step_carries_a_close_encounter(st):
+    """Sun + two planets on crossing orbits that pass each other inside their critical radius.  The plain step (no
+    Bulirsch-Stoer branch) treats the inner part of the encounter with the kick's K-weighted force only and loses the
+    energy there; the hybrid step integrates it and keeps the energy error orders of magnitude smaller."""
+    mass = np.array([3e-5, 3e-5])
+    a = np.array([1.0, 1.02]); e = np.array([0.02, 0.03]); z = np.zeros(2)
+    pos, vel = gi.elements_to_cartesian(a, e, z + 0.001, z, np.array([0.0, 0.6]), np.array([0.0, -0.57]), G)
+    vel = vel - (mass * vel).sum(1, keepdims=True) / (1.0 + mass.sum())
+    e0 = _energy(pos, vel, mass, 1.0)
+    dt = 2.0
+    out = {}
+    for name in ("plain", "hybrid"):
+        q, v = pos.copy(), vel.copy()
+        worst, dmin, in_enc = 0.0, 1e9, 0
+        for _ in range(400):
+            if name == "plain":
+                r = st.step(q, v, mass, 2, 0, 1.0, G, dt)
+            else:
+                r = st.hybrid_step(q, v, mass, 2, 0, 1.0, G, dt, tol=1e-13)
+                in_enc += r.groups.n_groups
+            q, v = r.pos, r.vel
+            dmin = min(dmin, np.sqrt(((q[:, 0] - q[:, 1]) ** 2).sum()))
+            worst = max(worst, abs(_energy(q, v, mass, 1.0) - e0) / abs(e0))
+        out[name] = (worst, dmin, in_enc)
+    rc = 0.4 * dt * np.sqrt((vel ** 2).sum(0)).max()
+    assert out["hybrid"][1] < 0.5 * rc and out["hybrid"][2] > 3          # there was an encounter, well inside r_crit
+    # (the residual ~1e-6 is the price of reading G5: K weights the force, not the potential, inside the band)
+    assert out["hybrid"][0] < 1e-5
+    assert out["plain"][0] > 300 * out["hybrid"][0]
