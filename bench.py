@@ -325,6 +325,35 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                          "all-pairs level-1 kick, W_1 = 0 beyond rc0)", "ms": float(np.median(list_ts)),
                  "listed_pairs": int(npairs[n].item()), "level1_pairs": int(npairs1[n].item())}
 
+    # NEXT-4: the complete hybrid step with the Bulirsch-Stoer branch, on BASELINE.json configs[1] (N = 8192; at
+    # N = 65,536 the level-0 pairs link into one group of 33,297 bodies, beyond the 256-body regime built here)
+    k1 = gi.make_config(1)
+    n1 = k1.n
+    kick1 = GengaKick(n1, 0, max_level=0, pair_capacity=1 << 18, G=k1.G, device=local_rank)
+    kick1.set_stream(stream.cuda_stream)
+    hq, hv, hm = to_dev(k1.pos), to_dev(k1.vel), to_dev(k1.mass)
+    i32 = lambda m: torch.empty(m, dtype=torch.int32, device=dev)
+    hacc = torch.empty(3, n1, dtype=torch.float64, device=dev)
+    hpairs, hnp, hgo, hmem, hoff, hsum = torch.empty(1 << 18, 2, dtype=torch.int32, device=dev), i32(n1 + 1), i32(n1), \
+        i32(n1), i32(n1 + 1), i32(4)
+    hyb_ts = []
+    for it in range(10):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = kick1.launch_count()
+        a.record(stream)
+        kick1.hybrid_step(hq, hv, hm, 1.0, k1.dt, 1e-12, hacc, hpairs, hnp, hgo, hmem, hoff, hsum)
+        b.record(stream)
+        b.synchronize()
+        hyb_launches = kick1.launch_count() - l0
+        if it >= 3:
+            hyb_ts.append(a.elapsed_time(b))
+    hs = hsum.cpu().tolist()
+    hybrid_info = {"what": "genga_hybrid_step on configs[1] (N = 8192): Rcrit, Kick + pre-check, HC, FG, grouping, "
+                           "Bulirsch-Stoer (tol 1e-12), HC, Kick", "ms_per_step": float(np.median(hyb_ts)),
+                   "launches_per_step": int(hyb_launches), "groups": hs[0], "bodies_in_groups": hs[1],
+                   "largest_group": hs[2], "status": kick1.status()}
+    kick1.free()
+
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
@@ -371,6 +400,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             "step": step_info,
             "group": group_info,
             "kick_list": list_info,
+            "hybrid_step": hybrid_info,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,

@@ -17,8 +17,8 @@
  * Method (the paper names it and refers to Grimm & Stadel 2014; reading G15): Gragg-Bulirsch-
  * Stoer -- modified midpoint with 2, 4, .., 16 sub-steps, polynomial extrapolation in h^2, relative error
  * per body in position and velocity <= tol, one step size for the whole group (halved on failure, doubled
- * after fast convergence).  One thread block per group, one thread per body: the regimes BS-B / BS-A of
- * Table 2, groups of up to 256 bodies.  Larger groups (BS-M) are NOT
+ * after fast convergence).  One thread block per group, up to four bodies per thread: the regimes BS-B /
+ * BS-A of Table 2 and a little beyond, groups of up to 1024 bodies.  Larger groups (BS-M) are NOT
  * integrated: they keep the state already in pos / vel and GENGA_KICK_STATUS_GROUP_TOO_LARGE is set --
  * sec. 6.3's higher symplectic levels exist to keep groups below that size.
  *
@@ -33,10 +33,10 @@
 extern "C" {
 #endif
 
-#define GENGA_KICK_STATUS_GROUP_TOO_LARGE 32   /* a group of more than 256 bodies was left as it was       */
+#define GENGA_KICK_STATUS_GROUP_TOO_LARGE 32   /* a group of more than 1024 bodies was left as it was      */
 #define GENGA_KICK_STATUS_BS_NOT_CONVERGED 64  /* a step did not reach tol after 60 halvings: that group
                                                   stopped at its last accepted time                        */
-#define GENGA_BS_MAX_GROUP 256
+#define GENGA_BS_MAX_GROUP 1024
 
 /*
  *   pos_in, vel_in  [3][N] state before FG (read only)          mass [N]
@@ -57,7 +57,7 @@ int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double* vel_in, co
  * detection" has no printed criterion; a pair that never enters its critical radius has W_BS = 0, so integrating
  * it is only extra work).  pos, vel are advanced in place; out_pairs / out_npairs: the candidates of the first
  * kick; group_of / members / offsets / summary: their groups, as genga_group writes them (all four required);
- * out_acc: acceleration of the closing kick, or NULL.  Groups above 256 bodies keep their Kepler-drifted state and
+ * out_acc: acceleration of the closing kick, or NULL.  Groups above 1024 bodies keep their Kepler-drifted state and
  * set GENGA_KICK_STATUS_GROUP_TOO_LARGE.
  * Errors: E_NULL, E_ALIGN, E_SIZE, E_CUDA.
  */

@@ -23,7 +23,14 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     const long long N = ctx->N;
     // at most N / 2 groups; CTAs stride over them (the number of groups is only known on the device)
     const int blocks = (int)std::min<long long>(std::max<long long>(N / 2, 1), 16LL * ctx->num_sms);
-    genga::bs_kernel<<<blocks, GENGA_BS_THREADS, 0, ctx->stream>>>(pos_in, vel_in, mass, rcrit, N, nlevels, ctx->cfg.G,
+    static bool configured[64] = {};                          // per device: the kernel needs 64 KB of dynamic shared memory
+    const int dev = ctx->cfg.device;
+    if (dev >= 0 && dev < 64 && !configured[dev]) {
+        GK_CUDA(ctx, cudaFuncSetAttribute(genga::bs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)genga::bs_smem_bytes()));
+        configured[dev] = true;
+    }
+    genga::bs_kernel<<<blocks, GENGA_BS_THREADS, genga::bs_smem_bytes(), ctx->stream>>>(pos_in, vel_in, mass, rcrit, N, nlevels, ctx->cfg.G,
                                                                   ctx->cfg.G * m_star, dt, tol, members, offsets, summary,
                                                                   pos, vel, ctx->status);
     GK_CUDA(ctx, cudaGetLastError());
