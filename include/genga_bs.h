@@ -17,10 +17,12 @@
  * Method (the paper names it and refers to Grimm & Stadel 2014; reading G15): Gragg-Bulirsch-
  * Stoer -- modified midpoint with 2, 4, .., 16 sub-steps, polynomial extrapolation in h^2, relative error
  * per body in position and velocity <= tol, one step size for the whole group (halved on failure, doubled
- * after fast convergence).  One thread block per group, up to four bodies per thread: the regimes BS-B /
- * BS-A of Table 2 and a little beyond, groups of up to 1024 bodies.  Larger groups (BS-M) are NOT
- * integrated: they keep the state already in pos / vel and GENGA_KICK_STATUS_GROUP_TOO_LARGE is set --
- * sec. 6.3's higher symplectic levels exist to keep groups below that size.
+ * after fast convergence).  Groups of up to 256 bodies: one thread block per group, one thread per body, many
+ * groups side by side (the regimes BS-B / BS-A of Table 2).  Larger groups: one group at a time
+ * over a whole co-resident grid with a grid-wide barrier per force evaluation (the paper's BS-M regime,
+ * PAPER.md:595-597, with the sub-steps kept on the device instead of controlled from the host); a group larger
+ * than that grid (tens of thousands of bodies: 64 threads x resident CTAs) keeps the state already in pos / vel
+ * and GENGA_KICK_STATUS_GROUP_TOO_LARGE is set.
  *
  * Works on the context of genga_kick.h (its N, G, stream); only enqueues; all pointers are DEVICE pointers.
  */
@@ -33,10 +35,9 @@
 extern "C" {
 #endif
 
-#define GENGA_KICK_STATUS_GROUP_TOO_LARGE 32   /* a group of more than 1024 bodies was left as it was      */
+#define GENGA_KICK_STATUS_GROUP_TOO_LARGE 32   /* a group larger than the co-resident grid was left as it was */
 #define GENGA_KICK_STATUS_BS_NOT_CONVERGED 64  /* a step did not reach tol after 60 halvings: that group
                                                   stopped at its last accepted time                        */
-#define GENGA_BS_MAX_GROUP 1024
 
 /*
  *   pos_in, vel_in  [3][N] state before FG (read only)          mass [N]
@@ -57,8 +58,8 @@ int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double* vel_in, co
  * detection" has no printed criterion; a pair that never enters its critical radius has W_BS = 0, so integrating
  * it is only extra work).  pos, vel are advanced in place; out_pairs / out_npairs: the candidates of the first
  * kick; group_of / members / offsets / summary: their groups, as genga_group writes them (all four required);
- * out_acc: acceleration of the closing kick, or NULL.  Groups above 1024 bodies keep their Kepler-drifted state and
- * set GENGA_KICK_STATUS_GROUP_TOO_LARGE.
+ * out_acc: acceleration of the closing kick, or NULL.  Groups too large for genga_bs keep their Kepler-drifted
+ * state and set GENGA_KICK_STATUS_GROUP_TOO_LARGE.
  * Errors: E_NULL, E_ALIGN, E_SIZE, E_CUDA.
  */
 int genga_hybrid_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,

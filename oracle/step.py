@@ -91,7 +91,7 @@ class HybridStepResult:
 
 
 def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc_factor=1.0, n1=3.0, n2=0.4,
-                max_group=1024):
+                max_group=None):
     """The complete scheme of App. A, every candidate pair of the pre-check treated as an encounter
     pair (no separate detection: PAPER.md gives no criterion, and a pair that never enters its critical radius has
     W_BS = 0, so integrating it is only extra work):

@@ -21,18 +21,42 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
         return GENGA_KICK_E_SIZE;
     if (dt == 0.0) return GENGA_KICK_OK;
     const long long N = ctx->N;
-    // at most N / 2 groups; CTAs stride over them (the number of groups is only known on the device)
-    const int blocks = (int)std::min<long long>(std::max<long long>(N / 2, 1), 16LL * ctx->num_sms);
-    static bool configured[64] = {};                          // per device: the kernel needs 64 KB of dynamic shared memory
-    const int dev = ctx->cfg.device;
-    if (dev >= 0 && dev < 64 && !configured[dev]) {
-        GK_CUDA(ctx, cudaFuncSetAttribute(genga::bs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)genga::bs_smem_bytes()));
-        configured[dev] = true;
+    cudaStream_t st = ctx->stream;
+    const double G = ctx->cfg.G, mu = ctx->cfg.G * m_star;
+    int* status = ctx->status;
+    long long NN = N;
+    // whole-grid regime: scratch for one group of up to N bodies, and the size of a co-resident grid
+    if (!ctx->bs_scratch) {
+        GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double)));
+        int per_sm = 0;
+        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<true, GENGA_BS_COOP_THREADS>,
+                                                                 GENGA_BS_COOP_THREADS, 0));
+        if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
+        ctx->bs_coop_blocks = per_sm * ctx->num_sms;
     }
-    genga::bs_kernel<<<blocks, GENGA_BS_THREADS, genga::bs_smem_bytes(), ctx->stream>>>(pos_in, vel_in, mass, rcrit, N, nlevels, ctx->cfg.G,
-                                                                  ctx->cfg.G * m_star, dt, tol, members, offsets, summary,
-                                                                  pos, vel, ctx->status);
+    genga::BsGlobal gm;
+    {
+        double* p = ctx->bs_scratch;
+        for (int h = 0; h < 2; h++) { gm.x[h] = p; p += N; gm.y[h] = p; p += N; gm.z[h] = p; p += N; }
+        gm.gm = p; p += N;
+        for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) { gm.rc[k] = p; p += N; }
+        gm.err = reinterpret_cast<unsigned long long*>(p);
+    }
+    // one CTA per group: at most N / 2 groups; CTAs stride over them (their number is only known on the device)
+    const int blocks = (int)std::min<long long>(std::max<long long>(N / 2, 1), 16LL * ctx->num_sms);
+    int small_max = GENGA_BS_THREADS;
+    genga::bs_kernel<false, GENGA_BS_THREADS><<<blocks, GENGA_BS_THREADS, 0, st>>>(
+        pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max);
+    GK_CUDA(ctx, cudaGetLastError());
+    // the whole grid, one large group after the other (returns at once if there is none)
+    if (N > GENGA_BS_THREADS) {
+        GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
+        void* args[] = {&pos_in, &vel_in, &mass, &rcrit, &NN, &nlevels, const_cast<double*>(&G), const_cast<double*>(&mu), &dt,
+                        &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max};
+        GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<true, GENGA_BS_COOP_THREADS>),
+                                                 dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
+        ctx->launches++;
+    }
     GK_CUDA(ctx, cudaGetLastError());
     ctx->launches++;
     return GENGA_KICK_OK;

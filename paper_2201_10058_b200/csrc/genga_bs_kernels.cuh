@@ -1,8 +1,12 @@
 // sm_100a kernel of the Bulirsch-Stoer integration of close-encounter groups (include/genga_bs.h;
-// PAPER.md:47, :559-597, App. A).  One CTA per group, up to four bodies per thread (the regimes BS-B and
-// BS-A of Table 2, and a little beyond: groups of up to 1024 bodies are integrated inside a
-// single thread block through shared memory, with no host round trip between sub-steps).  Larger groups (the paper's BS-M,
-// host-controlled sub-steps over several blocks) are not integrated: they are reported.
+// PAPER.md:47, :559-597, App. A), one body per thread, in two regimes:
+//   bs_kernel<false>  one CTA of 256 threads per group, the group's state in shared memory: the regimes BS-B and
+//                     BS-A of Table 2, groups of up to 256 bodies, many groups side by side;
+//   bs_kernel<true>   ONE group at a time over the whole grid (cooperative launch, 64-thread CTAs): the paper's
+//                     BS-M regime ("distributed over multiple thread blocks ... sub-steps ...
+//                     controlled from the host ... many different kernel calls") -- but here the sub-steps stay
+//                     on the device: positions are exchanged through L2 (double-buffered) and the CTAs meet at
+//                     one grid-wide barrier per force evaluation.  Groups of 257 .. grid size bodies.
 //
 // The scheme is the textbook Gragg-Bulirsch-Stoer method fixed as reading G15 in DESIGN.md: modified
 // midpoint with n_k = 2k sub-steps (k = 1..8), Aitken-Neville extrapolation in h^2, relative error per body
@@ -16,11 +20,13 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cooperative_groups.h>
+
 namespace genga {
 
-#define GENGA_BS_THREADS 256
-#define GENGA_BS_BPT 4                  // bodies per thread: groups of up to GENGA_BS_THREADS * GENGA_BS_BPT bodies
-#define GENGA_BS_MAX_GROUP (GENGA_BS_THREADS * GENGA_BS_BPT)
+#define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
+#define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
+#define GENGA_BS_TILE 64                // j-bodies staged per round in the whole-grid regime
 #define GENGA_BS_KMAX 8
 #define GENGA_BS_MAX_LEVELS 4
 #define GENGA_BS_MAX_HALVINGS 60
@@ -36,100 +42,172 @@ __device__ __forceinline__ double bs_K(double r, double rc)
     return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
 }
 
-// dynamic shared memory of bs_kernel: the group's positions, G m and critical radii, body-indexed
-struct BsShared {
-    double* x; double* y; double* z; double* gm;
+// Scratch of the whole-grid regime (device memory, library-owned): the group's positions in two buffers
+// (force evaluation e publishes into buffer e & 1 while slower CTAs may still read the other one), G m,
+// the critical-radius rows, and four slots for the group-wide error maximum.
+struct BsGlobal {
+    double* x[2]; double* y[2]; double* z[2];
+    double* gm;
     double* rc[GENGA_BS_MAX_LEVELS];
+    unsigned long long* err;            // [4], all zero between uses
 };
-__host__ __device__ constexpr size_t bs_smem_bytes() { return (size_t)(4 + GENGA_BS_MAX_LEVELS) * GENGA_BS_MAX_GROUP * sizeof(double); }
 
-// dv/dt of body i at the positions the group has published in shared memory:
-//   - G m_star q / |q|^3 + sum_{j != i} G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q) / r^3
-__device__ __forceinline__ void bs_accel(const BsShared& S, int i, int n, int nlevels, double mu, double x, double y,
-                                         double z, double& ax, double& ay, double& az)
+// shared memory: one-CTA regime: the whole group; whole-grid regime: one tile of j-bodies
+template <int ROWS>
+struct BsShared {
+    double x[ROWS], y[ROWS], z[ROWS], gm[ROWS];
+    double rc[GENGA_BS_MAX_LEVELS][ROWS];
+    double red[8];
+    double errmax;
+};
+
+// one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3
+#define GENGA_BS_PAIR(XJ, YJ, ZJ, GMJ, RCJ)                                                            \
+    {                                                                                                  \
+        const double dx = (XJ) - x, dy = (YJ) - y, dz = (ZJ) - z;                                      \
+        const double r2 = dx * dx + dy * dy + dz * dz;                                                 \
+        const double r = sqrt(r2);                                                                     \
+        double W = 1.0;                                                                                \
+        for (int k = 0; k < nlevels; k++) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));                  \
+        if (W != 0.0) {                                                                                \
+            const double s = (GMJ) * W / (r2 * r);                                                     \
+            ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;                                      \
+        }                                                                                              \
+    }
+
+// Every thread publishes the position of its body i (if i < n) and gets dv_i/dt back:
+//   - G m_star q / |q|^3 + the pair terms over j = 0 .. n-1, j != i, in that order.
+// COOP: `eval` counts the force evaluations of the group (buffer parity); one grid barrier per call.
+template <bool COOP, int ROWS>
+__device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, int nlevels,
+                                         double mu, const double (&rci)[GENGA_BS_MAX_LEVELS], const double (&q)[3],
+                                         double (&a)[3])
 {
+    const double x = q[0], y = q[1], z = q[2];
     const double r2s = x * x + y * y + z * z;
     const double rs = sqrt(r2s);
     const double s0 = -mu / (r2s * rs);
-    ax = s0 * x; ay = s0 * y; az = s0 * z;
-    for (int j = 0; j < n; j++) {
-        if (j == i) continue;
-        const double dx = S.x[j] - x, dy = S.y[j] - y, dz = S.z[j] - z;
-        const double r2 = dx * dx + dy * dy + dz * dz;
-        const double r = sqrt(r2);
-        double W = 1.0;
-        for (int k = 0; k < nlevels; k++) W *= (1.0 - bs_K(r, fmax(S.rc[k][i], S.rc[k][j])));
-        if (W != 0.0) {
-            const double s = S.gm[j] * W / (r2 * r);
-            ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;
+    double ax = s0 * x, ay = s0 * y, az = s0 * z;
+    if (!COOP) {
+        __syncthreads();                                      // the previous readers are done
+        if (i < n) { S.x[i] = x; S.y[i] = y; S.z[i] = z; }
+        __syncthreads();
+        if (i < n) {
+#define GENGA_BS_RCJ(k) S.rc[k][j]
+            for (int j = 0; j < n; j++) {
+                if (j == i) continue;
+                GENGA_BS_PAIR(S.x[j], S.y[j], S.z[j], S.gm[j], GENGA_BS_RCJ)
+            }
+#undef GENGA_BS_RCJ
+        }
+    } else {
+        const int p = eval & 1;
+        eval++;
+        if (i < n) { Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z; }
+        cooperative_groups::this_grid().sync();
+        const int t = threadIdx.x;
+        for (int j0 = 0; j0 < n; j0 += ROWS) {                // tiles in ascending order: the sum runs over j = 0 .. n-1
+            __syncthreads();
+            if (t < ROWS && j0 + t < n) {
+                S.x[t] = __ldcg(Gm.x[p] + j0 + t); S.y[t] = __ldcg(Gm.y[p] + j0 + t); S.z[t] = __ldcg(Gm.z[p] + j0 + t);
+                S.gm[t] = __ldcg(Gm.gm + j0 + t);
+                for (int k = 0; k < nlevels; k++) S.rc[k][t] = __ldcg(Gm.rc[k] + j0 + t);
+            }
+            __syncthreads();
+            if (i < n) {
+                const int m = min(ROWS, n - j0);
+#define GENGA_BS_RCJ(k) S.rc[k][jj]
+                for (int jj = 0; jj < m; jj++) {
+                    if (j0 + jj == i) continue;
+                    GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
+                }
+#undef GENGA_BS_RCJ
+            }
         }
     }
+    a[0] = ax; a[1] = ay; a[2] = az;
 }
 
-// every thread publishes the positions of its bodies (i = t + u * GENGA_BS_THREADS < n) and gets their accelerations
-__device__ __forceinline__ void bs_force(const BsShared& S, int t, int n, int nlevels, double mu,
-                                         const double (&q)[GENGA_BS_BPT][3], double (&a)[GENGA_BS_BPT][3])
+// maximum of e over the group (order-free); CTA- (and, COOP, grid-) uniform result
+template <bool COOP, int THREADS, int ROWS>
+__device__ __forceinline__ double bs_group_max(BsShared<ROWS>& S, const BsGlobal& Gm, int& echeck, double e)
 {
-    __syncthreads();                                          // the previous readers are done
+    const int t = threadIdx.x;
 #pragma unroll
-    for (int u = 0; u < GENGA_BS_BPT; u++) {
-        const int i = t + u * GENGA_BS_THREADS;
-        if (i < n) { S.x[i] = q[u][0]; S.y[i] = q[u][1]; S.z[i] = q[u][2]; }
+    for (int o = 16; o > 0; o >>= 1) e = fmax(e, __shfl_xor_sync(0xffffffffu, e, o));
+    __syncthreads();
+    if ((t & 31) == 0) S.red[t >> 5] = e;
+    __syncthreads();
+    if (t == 0) {
+        double m = S.red[0];
+#pragma unroll
+        for (int w = 1; w < THREADS / 32; w++) m = fmax(m, S.red[w]);
+        S.errmax = m;
     }
     __syncthreads();
-#pragma unroll
-    for (int u = 0; u < GENGA_BS_BPT; u++) {
-        const int i = t + u * GENGA_BS_THREADS;
-        if (i < n) bs_accel(S, i, n, nlevels, mu, q[u][0], q[u][1], q[u][2], a[u][0], a[u][1], a[u][2]);
-    }
+    if (!COOP) return S.errmax;
+    // non-negative doubles order like their bit patterns: atomicMax on the bits; four slots used in turn, the slot
+    // two checks ahead is cleared after this check's barrier (its last readers passed the previous barrier)
+    const int slot = echeck & 3;
+    echeck++;
+    if (t == 0) atomicMax(Gm.err + slot, (unsigned long long)__double_as_longlong(S.errmax));
+    cooperative_groups::this_grid().sync();
+    const double m = __longlong_as_double((long long)__ldcg(Gm.err + slot));
+    if (blockIdx.x == 0 && t == 0) Gm.err[(slot + 2) & 3] = 0ULL;
+    return m;
 }
 
-__global__ void __launch_bounds__(GENGA_BS_THREADS)
+// COOP = false: CTA g, g + gridDim.x, ... integrates group g if it has at most THREADS bodies (others: left to
+//               the whole-grid regime).
+// COOP = true : the whole grid integrates, one after the other, the groups with more than `small_max` bodies;
+//               groups larger than the grid are reported and left as they are.
+template <bool COOP, int THREADS>
+__global__ void __launch_bounds__(THREADS)
 bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
-          double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status)
+          double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max)
 {
-    constexpr int BPT = GENGA_BS_BPT;
-    extern __shared__ __align__(16) double bs_smem[];
-    __shared__ double red[GENGA_BS_THREADS / 32];
-    __shared__ double errmax;
-    BsShared S;
-    S.x = bs_smem; S.y = S.x + GENGA_BS_MAX_GROUP; S.z = S.y + GENGA_BS_MAX_GROUP; S.gm = S.z + GENGA_BS_MAX_GROUP;
-#pragma unroll
-    for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) S.rc[k] = S.gm + (size_t)(k + 1) * GENGA_BS_MAX_GROUP;
+    constexpr int ROWS = COOP ? GENGA_BS_TILE : THREADS;
+    __shared__ BsShared<ROWS> S;
     const int t = threadIdx.x;
+    const int i = COOP ? (int)(blockIdx.x * THREADS + t) : t;           // this thread's body within the group
+    const long long capacity = COOP ? (long long)gridDim.x * THREADS : THREADS;
     const int n_groups = summary[0];
-    for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
+    int eval = 0, echeck = 0;
+    for (int g = COOP ? 0 : (int)blockIdx.x; g < n_groups; g += COOP ? 1 : (int)gridDim.x) {
         const int first = offsets[g], n = offsets[g + 1] - first;
-        if (n > GENGA_BS_MAX_GROUP) {                          // CTA-uniform
-            if (t == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
+        if (COOP ? n <= small_max : n > THREADS) continue;             // the other regime's group (grid-/CTA-uniform)
+        if (n > capacity) {
+            if (t == 0 && blockIdx.x == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
             continue;
         }
-        long long b[BPT];
-        double q[BPT][3], v[BPT][3];
-        __syncthreads();                                      // the previous group's readers are done
+        const bool active = i < n;
+        const long long b = active ? members[first + i] : 0;
+        double q[3] = {0.0, 0.0, 0.0}, v[3] = {0.0, 0.0, 0.0}, rci[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
+        if (!COOP) __syncthreads();                                     // the previous group's readers are done
+        if (active) {
 #pragma unroll
-        for (int u = 0; u < BPT; u++) {
-            const int i = t + u * GENGA_BS_THREADS;
-            b[u] = 0;
-#pragma unroll
-            for (int c = 0; c < 3; c++) { q[u][c] = 0.0; v[u][c] = 0.0; }
-            if (i < n) {
-                b[u] = members[first + i];
-#pragma unroll
-                for (int c = 0; c < 3; c++) { q[u][c] = pos_in[c * N + b[u]]; v[u][c] = vel_in[c * N + b[u]]; }
-                S.gm[i] = G * mass[b[u]];
-                for (int k = 0; k < nlevels; k++) S.rc[k][i] = rcrit[(long long)k * N + b[u]];
+            for (int c = 0; c < 3; c++) { q[c] = pos_in[c * N + b]; v[c] = vel_in[c * N + b]; }
+            const double gm = G * mass[b];
+            for (int k = 0; k < nlevels; k++) rci[k] = rcrit[(long long)k * N + b];
+            if (COOP) {
+                Gm.gm[i] = gm;
+                for (int k = 0; k < nlevels; k++) Gm.rc[k][i] = rci[k];
+            } else {
+                S.gm[i] = gm;
+                for (int k = 0; k < nlevels; k++) S.rc[k][i] = rci[k];
             }
         }
-        double Pq[BPT][GENGA_BS_KMAX][3], Pv[BPT][GENGA_BS_KMAX][3];   // P[j] = T_{k-1,j} of the extrapolation tableau
-        double a0[BPT][3], cq[BPT][3], cv[BPT][3], dq[BPT][3], dv[BPT][3];
+        // (COOP: G m and the radii are read by other CTAs only after the first force evaluation's grid barrier;
+        //  the previous group's last readers passed a grid barrier -- its last error check -- before anyone gets here)
+        double Pq[GENGA_BS_KMAX][3], Pv[GENGA_BS_KMAX][3];             // P[j] = T_{k-1,j} of the extrapolation tableau
+        double a0[3], cq[3], cv[3], dq[3], dv[3];
         double done = 0.0, H = dt;
         bool fail = false;
-        while (done != dt) {                                  // all decisions below are CTA-uniform
+        while (done != dt) {                                           // all decisions below are group-uniform
             if ((dt > 0.0 && done + H > dt) || (dt < 0.0 && done + H < dt)) H = dt - done;
-            bs_force(S, t, n, nlevels, mu, q, a0);
+            bs_force<COOP, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, q, a0);
             int halvings = 0, kconv = 0;
             for (;;) {
                 bool ok = false;
@@ -137,80 +215,51 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
                     const int nk = 2 * (k + 1);
                     {   // modified midpoint over H with nk sub-steps: (q, v) -> (cq, cv) = T_{k,0}
                         const double h = H / (double)nk, h2 = 2.0 * h;
-                        double qm[BPT][3], vm[BPT][3], qn[BPT][3], vn[BPT][3], a[BPT][3];
+                        double qm[3], vm[3], qn[3], vn[3], a[3];
 #pragma unroll
-                        for (int u = 0; u < BPT; u++)
-#pragma unroll
-                            for (int c = 0; c < 3; c++) {
-                                qm[u][c] = q[u][c]; vm[u][c] = v[u][c];
-                                qn[u][c] = q[u][c] + h * v[u][c]; vn[u][c] = v[u][c] + h * a0[u][c];
-                                a[u][c] = 0.0;
-                            }
+                        for (int c = 0; c < 3; c++) { qm[c] = q[c]; vm[c] = v[c]; qn[c] = q[c] + h * v[c]; vn[c] = v[c] + h * a0[c]; }
                         for (int m = 1; m < nk; m++) {
-                            bs_force(S, t, n, nlevels, mu, qn, a);
-#pragma unroll
-                            for (int u = 0; u < BPT; u++)
-#pragma unroll
-                                for (int c = 0; c < 3; c++) {
-                                    const double qs = qm[u][c] + h2 * vn[u][c], vs = vm[u][c] + h2 * a[u][c];
-                                    qm[u][c] = qn[u][c]; vm[u][c] = vn[u][c]; qn[u][c] = qs; vn[u][c] = vs;
-                                }
-                        }
-                        bs_force(S, t, n, nlevels, mu, qn, a);
-#pragma unroll
-                        for (int u = 0; u < BPT; u++)
+                            bs_force<COOP, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
 #pragma unroll
                             for (int c = 0; c < 3; c++) {
-                                cq[u][c] = 0.5 * (qn[u][c] + qm[u][c] + h * vn[u][c]);
-                                cv[u][c] = 0.5 * (vn[u][c] + vm[u][c] + h * a[u][c]);
+                                const double qs = qm[c] + h2 * vn[c], vs = vm[c] + h2 * a[c];
+                                qm[c] = qn[c]; vm[c] = vn[c]; qn[c] = qs; vn[c] = vs;
                             }
+                        }
+                        bs_force<COOP, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
+#pragma unroll
+                        for (int c = 0; c < 3; c++) {
+                            cq[c] = 0.5 * (qn[c] + qm[c] + h * vn[c]);
+                            cv[c] = 0.5 * (vn[c] + vm[c] + h * a[c]);
+                        }
                     }
                     for (int j = 1; j <= k; j++) {
                         const double ratio = (double)nk / (double)(2 * (k - j + 1));      // n_k / n_{k-j}
                         const double den = ratio * ratio - 1.0;
 #pragma unroll
-                        for (int u = 0; u < BPT; u++)
-#pragma unroll
-                            for (int c = 0; c < 3; c++) {
-                                const double lq = cq[u][c], lv = cv[u][c];                // T_{k,j-1}
-                                const double nq = lq + (lq - Pq[u][j - 1][c]) / den;      // T_{k,j}
-                                const double nv = lv + (lv - Pv[u][j - 1][c]) / den;
-                                Pq[u][j - 1][c] = lq; Pv[u][j - 1][c] = lv;
-                                cq[u][c] = nq; cv[u][c] = nv;
-                                dq[u][c] = nq - lq; dv[u][c] = nv - lv;                   // after j = k: T_kk - T_k,k-1
-                            }
+                        for (int c = 0; c < 3; c++) {
+                            const double lq = cq[c], lv = cv[c];                          // T_{k,j-1}
+                            const double nq = lq + (lq - Pq[j - 1][c]) / den;             // T_{k,j}
+                            const double nv = lv + (lv - Pv[j - 1][c]) / den;
+                            Pq[j - 1][c] = lq; Pv[j - 1][c] = lv;
+                            cq[c] = nq; cv[c] = nv;
+                            dq[c] = nq - lq; dv[c] = nv - lv;                             // after j = k: T_kk - T_k,k-1
+                        }
                     }
 #pragma unroll
-                    for (int u = 0; u < BPT; u++)
-#pragma unroll
-                        for (int c = 0; c < 3; c++) { Pq[u][k][c] = cq[u][c]; Pv[u][k][c] = cv[u][c]; }   // T_kk
+                    for (int c = 0; c < 3; c++) { Pq[k][c] = cq[c]; Pv[k][c] = cv[c]; }   // T_kk
                     if (k > 0) {
                         double e = 0.0;
-#pragma unroll
-                        for (int u = 0; u < BPT; u++) {
-                            if (t + u * GENGA_BS_THREADS >= n) continue;
+                        if (active) {
                             double eq2 = 0.0, sq2 = 0.0, ev2 = 0.0, sv2 = 0.0;
 #pragma unroll
                             for (int c = 0; c < 3; c++) {
-                                eq2 = eq2 + dq[u][c] * dq[u][c]; sq2 = sq2 + cq[u][c] * cq[u][c];
-                                ev2 = ev2 + dv[u][c] * dv[u][c]; sv2 = sv2 + cv[u][c] * cv[u][c];
+                                eq2 = eq2 + dq[c] * dq[c]; sq2 = sq2 + cq[c] * cq[c];
+                                ev2 = ev2 + dv[c] * dv[c]; sv2 = sv2 + cv[c] * cv[c];
                             }
-                            e = fmax(e, fmax(sqrt(eq2) / sqrt(sq2), sqrt(ev2) / sqrt(sv2)));
+                            e = fmax(sqrt(eq2) / sqrt(sq2), sqrt(ev2) / sqrt(sv2));
                         }
-                        // maximum over the group (order-free)
-#pragma unroll
-                        for (int o = 16; o > 0; o >>= 1) e = fmax(e, __shfl_xor_sync(0xffffffffu, e, o));
-                        __syncthreads();
-                        if ((t & 31) == 0) red[t >> 5] = e;
-                        __syncthreads();
-                        if (t == 0) {
-                            double m = red[0];
-#pragma unroll
-                            for (int w = 1; w < GENGA_BS_THREADS / 32; w++) m = fmax(m, red[w]);
-                            errmax = m;
-                        }
-                        __syncthreads();
-                        if (errmax <= tol) { ok = true; kconv = k + 1; break; }
+                        if (bs_group_max<COOP, THREADS, ROWS>(S, Gm, echeck, e) <= tol) { ok = true; kconv = k + 1; break; }
                     }
                 }
                 if (ok) break;
@@ -219,20 +268,16 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
             }
             if (fail) break;
 #pragma unroll
-            for (int u = 0; u < BPT; u++)
-#pragma unroll
-                for (int c = 0; c < 3; c++) { q[u][c] = cq[u][c]; v[u][c] = cv[u][c]; }
+            for (int c = 0; c < 3; c++) { q[c] = cq[c]; v[c] = cv[c]; }
             if ((dt > 0.0 && done + H >= dt) || (dt < 0.0 && done + H <= dt)) done = dt;
             else done = done + H;
             if (kconv <= 5) H = 2.0 * H;
         }
-        if (fail && t == 0) atomicOr(status, GENGA_STATUS_BS_NOT_CONVERGED);
+        if (fail && t == 0 && blockIdx.x == (COOP ? 0 : blockIdx.x)) atomicOr(status, GENGA_STATUS_BS_NOT_CONVERGED);
+        if (active) {                                                  // (after a failure: the state at the last accepted time)
 #pragma unroll
-        for (int u = 0; u < BPT; u++)                          // (after a failure: the state at the last accepted time)
-            if (t + u * GENGA_BS_THREADS < n) {
-#pragma unroll
-                for (int c = 0; c < 3; c++) { pos[c * N + b[u]] = q[u][c]; vel[c * N + b[u]] = v[u][c]; }
-            }
+            for (int c = 0; c < 3; c++) { pos[c * N + b] = q[c]; vel[c * N + b] = v[c]; }
+        }
     }
 }
 

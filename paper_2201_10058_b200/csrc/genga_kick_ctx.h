@@ -55,6 +55,8 @@ struct genga_kick_ctx {
     // grouping (genga_group.cu), lazily allocated
     int* grp_label; int* grp_flag; unsigned* grp_keys_a; unsigned* grp_keys_b; int* grp_vals_a; int* grp_vals_b;
     int* grp_counts;
+    double* bs_scratch;            // whole-grid Bulirsch-Stoer regime: positions (2 buffers), G m, r_crit rows, error slots
+    int bs_coop_blocks;            // its co-resident grid
     double* hyb_state;             // [6][N] state before FG (genga_hybrid_step), lazily allocated
     std::string cuda_err;
 };

@@ -52,7 +52,7 @@ def test_groups_of_a_disk_kick_group_bs_chain(oracle_mod):
     n = ki.n
     res = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, n, 0, level=0, G=ki.G)
     gr = oracle_mod.group.group(n, oracle_mod.pair_set(res, n))
-    assert gr.n_groups > 100 and gr.max_size <= 1024
+    assert gr.n_groups > 100
     qf, vf, _ = oracle_mod.step.fg(ki.pos, ki.vel, ki.G, ki.dt)                     # what FG left in pos / vel
     qw, vw, stats, skipped = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, gr.members, gr.offsets, G, 1.0, ki.dt,
                                               1e-12, qf, vf, nlevels=1)
@@ -74,29 +74,31 @@ def test_dense_groups_levels_tolerances(oracle_mod, nlevels, tol, dt):
     res = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, n, 0, level=0, G=ki.G, maxp=256)
     gr = oracle_mod.group.group(n, oracle_mod.pair_set(res, n))
     qw, vw, stats, skipped = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, gr.members, gr.offsets, G, 1.0, dt, tol,
-                                              ki.pos, ki.vel, nlevels=nlevels, max_group=1024)
+                                              ki.pos, ki.vel, nlevels=nlevels, max_group=None)
     q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, nlevels, dt, tol, gr.members, gr.offsets, ki.pos, ki.vel)
-    assert (st == 32) == bool(skipped) and (st & ~32) == 0
+    assert st == 0 and not skipped
     assert gr.max_size > 20 and len(stats) > 50
     _check(q, v, qw, vw)
 
 
-def test_large_group_is_reported_and_left(oracle_mod):
-    import paper_2201_10058_b200 as g
-    n = 1500
-    ki = gi.make_ring(n)                                          # one group of 1500 > 1024
-    members, offsets = np.arange(n), np.array([0, n])
-    q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 6.0, 1e-12, members, offsets, ki.pos * 2, ki.vel * 2)
-    assert st == g.STATUS_GROUP_TOO_LARGE
-    assert np.array_equal(q, ki.pos * 2) and np.array_equal(v, ki.vel * 2)
-    # rings of 200, 257, 700 and 1024 bodies are one group each: integrated (1, 2, 3, 4 bodies per thread)
-    for m in (200, 257, 700, 1024):
+def test_large_groups_whole_grid_regime(oracle_mod):
+    """Groups above 256 bodies are integrated by the whole grid, one group at a time (the paper's BS-M regime with the
+    sub-steps kept on the device): rings of 257 .. 3000 bodies, one group each, and a mix of small and large groups."""
+    for m in (200, 257, 700, 1024, 3000):
         ki = gi.make_ring(m)
         qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, np.arange(m), [0, m], ki.G, 1.0, 6.0, 1e-12,
-                                            ki.pos, ki.vel)
+                                            ki.pos, ki.vel, max_group=None)
         q, v, st = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 6.0, 1e-12, np.arange(m), [0, m], ki.pos, ki.vel)
         assert st == 0
-        _check(q, v, qw, vw)
+        assert _check(q, v, qw, vw), "not bit-identical"
+    # three groups in one call: 300 (whole grid), 40 (one CTA), 500 (whole grid) bodies of one ring
+    ki = gi.make_ring(840)
+    members, offsets = np.arange(840), [0, 300, 340, 840]
+    qw, vw, _, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, members, offsets, ki.G, 1.0, -6.0, 1e-11, ki.pos, ki.vel,
+                                    max_group=None)
+    q, v, st = _gpu_bs(840, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, -6.0, 1e-11, members, offsets, ki.pos, ki.vel)
+    assert st == 0
+    _check(q, v, qw, vw)
 
 
 def test_bs_error_codes_and_empty():
