@@ -458,12 +458,6 @@ extern "C" int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, 
     return genga_kick_measure_fp64_rate(ctx, 0, iters, reps, dfma_per_s);
 }
 
-#ifdef GENGA_TRACE
-extern "C" int genga_kick_debug_trace(long long* host, long long n)
-{
-    return (int)cudaMemcpyFromSymbol(host, genga::g_trace, (size_t)n * sizeof(long long));
-}
-#endif
 
 extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return ctx ? ctx->launches : 0; }
 

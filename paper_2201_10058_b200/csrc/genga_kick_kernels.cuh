@@ -558,26 +558,10 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-#ifdef GENGA_TRACE
-// Working aid (never compiled into the product library): per-warp start / end times, SM id and
-// counters of the last kick_kernel launch.
-__device__ long long g_trace[1 << 18];
-__device__ __forceinline__ long long trace_now()
-{
-    long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#endif
 
 template <int THREADS, int IPT, int JT, int CTAS, int STAGES>
 __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
-#ifdef GENGA_TRACE
-    const long long tr_start = trace_now();
-    int tr_near = 0, tr_cand = 0;
-    const int tr_drain = 0;
-#endif
     constexpr int IB = THREADS * IPT;
     constexpr int WARPS = THREADS / 32;
     constexpr int NCH = JT / GENGA_CHUNK;
@@ -674,9 +658,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 
         const bool mine_near = lane < NG ? boxes_near(wlo, whi, wfw, S.blo[lane], S.bhi[lane]) : false;
         const unsigned nearmask = __ballot_sync(0xffffffffu, mine_near);
-#ifdef GENGA_TRACE
-        tr_near += __popc(nearmask);
-#endif
 
 #pragma unroll 1
         for (int g = 0; g < NG; g++) {
@@ -715,9 +696,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                     const bool mine = (tm >> b) & 1u;
                     const int jrec = p.j_rec0 + jt * JT + jj + b / IPT;
                     push_candidates(p, cc, mine, ib * IB + woff + (b % IPT) * 32, p.force_only ? ~jrec : jrec);
-#ifdef GENGA_TRACE
-                    tr_cand += __popc(__ballot_sync(0xffffffffu, mine));
-#endif
                 }
             }
         }
@@ -727,14 +705,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
     }
     flush();
     if (cc.fill < GENGA_CAND_BLOCK) close_block(p, cc);
-#ifdef GENGA_TRACE
-    if (lane == 0) {
-        unsigned smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        long long* o = g_trace + ((size_t)blockIdx.x * WARPS + warp) * 8;
-        o[0] = tr_start; o[1] = trace_now(); o[2] = smid; o[3] = tr_near; o[4] = tr_cand; o[5] = tr_drain;
-    }
-#endif
 }
 
 // ---------------------------------------------------------------------------------------------
