@@ -1,10 +1,11 @@
-"""Builds oracle/libgenga_oracle.so from the plain-C oracles (kick + pre-check; Rcrit / HC / FG; grouping; Bulirsch-Stoer) (test infrastructure; gcc only)."""
+"""Builds oracle/libgenga_oracle.so from the plain-C oracles (kick + pre-check; Rcrit / HC / FG; detection; grouping; Bulirsch-Stoer) (test infrastructure; gcc only)."""
 import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRCS = [os.path.join(HERE, "genga_kick_oracle.c"), os.path.join(HERE, "genga_step_oracle.c"),
-        os.path.join(HERE, "genga_group_oracle.c"), os.path.join(HERE, "genga_bs_oracle.c")]
+        os.path.join(HERE, "genga_group_oracle.c"), os.path.join(HERE, "genga_bs_oracle.c"),
+        os.path.join(HERE, "genga_detect_oracle.c")]
 LIB = os.path.join(HERE, "libgenga_oracle.so")
 # -ffp-contract=off: every product and sum rounds separately, as the header promises.
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall"]
