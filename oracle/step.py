@@ -113,3 +113,104 @@ def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc
     k2 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
     v = v + (0.5 * dt) * k2.acc
     return HybridStepResult(pos=q, vel=v, rcrit=rc, first=k1, groups=gr, skipped=skipped, unbound=bad0 + bad1)
+
+
+@dataclass
+class MultilevelStepResult:
+    pos: np.ndarray
+    vel: np.ndarray
+    rcrit: np.ndarray        # [slevels, N]: row 0 of Rcrit(dt); rows >= 1 as the LAST RcritS of each level left them
+    first: _kick.OracleResult
+    stats: np.ndarray        # [slevels, 4] per level, summed over its sub-steps: candidate pairs, close-encounter pairs,
+                             # groups handed to Bulirsch-Stoer, bodies in them
+    unbound: int
+
+
+def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2, substeps=2, tol=1e-12, enc_factor=1.0,
+                    n1=3.0, n2=0.4, detect=True, max_group=None):
+    """The multi-level scheme of App. A, written as printed there:
+
+        Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt)
+        if candidates: close-encounter detection
+        if SLevels > 1:  if close-encounters: SEnc(dt, 1.0, 0)
+        else:            if close-encounters: grouping; Bulirsch-Stoer(dt)
+        HC(dt/2); Kick(dt/2)
+
+        SEnc(dt, ds, SLevel):  groupS;  SLevel += 1;  ds *= substeps
+          for s in range(substeps):
+            RcritS();  KickS(dt/ds/2);  FGS(dt/ds);  close-encounter detection
+            if close-encounters:
+              if SLevel < SLevels - 1: SEnc(dt, ds, SLevel)
+              else: grouping; Bulirsch-Stoer(dt/ds)
+            KickS(dt/ds/2)
+
+    Readings (G17): level l >= 1 works on the close-encounter pairs of level l-1 (groupS) and on the bodies in
+    them ("the relevant bodies"); those bodies restart from their state BEFORE the upper level's drift (as the
+    Bulirsch-Stoer phase does, G15), which the sub-steps replace; RcritS writes row l of eq. 5 at dt/substeps^l from the
+    current velocities; KickS is the level-l kick of eq. 63 over the listed pairs with its level-l
+    pre-check; the Bulirsch-Stoer phase of the deepest level carries W_BS = prod_{k < SLevels} (1 - K_k).
+    detect=False: every candidate of a pre-check counts as a close-encounter pair (as hybrid_step does)."""
+    from . import group as _group, bs as _bs, detect as _det
+    q, v, mass = _c(pos).copy(), _c(vel).copy(), _c(mass)
+    n = q.shape[1]
+    mu = G * m_star
+    rc = np.zeros((slevels, n))
+    row, bad = rcrit(q, v, mass, m_star, G, dt, 2.0, 1, n1, n2)
+    rc[0] = row[0]
+    stats = np.zeros((slevels, 4), dtype=np.int64)
+    unbound = [bad]
+
+    def encounters(level, q0, v0, q1, v1, h, cand):
+        enc = _det.detect(q0, v0, q1, v1, rc[level], h, cand, enc_factor=1.0).pairs if detect else cand
+        stats[level, 0] += len(cand); stats[level, 1] += len(enc)
+        return enc, _group.group(n, enc)
+
+    def bulirsch_stoer(level, q0, v0, h, gr, q, v):
+        q, v, _, skipped = _bs.bs(q0, v0, mass, rc, gr.members, gr.offsets, G, m_star, h, tol, q, v, nlevels=level + 1,
+                                  max_group=max_group)
+        stats[level, 2] += gr.n_groups - len(skipped)
+        stats[level, 3] += len(gr.members) - sum(int(gr.offsets[g + 1] - gr.offsets[g]) for g in skipped)
+        return q, v
+
+    def senc(q, v, level, pairs_up, bodies):                # `level` is the level being entered (SLevel += 1)
+        h = dt / float(substeps) ** level                   # dt / ds
+        for s in range(substeps):
+            row, _ = rcrit(q, v, mass, m_star, G, h, 2.0, 1, n1, n2)                    # RcritS
+            rc[level, bodies] = row[0, bodies]
+            ks = _kick.kick_list(q, mass, rc[:level + 1], n_massive, n_test, pairs_up, level=level, G=G,
+                                 enc_factor=enc_factor)                                  # KickS(dt/ds/2)
+            v = v + (0.5 * h) * ks.acc
+            q0, v0 = q.copy(), v.copy()
+            qf, vf, b1 = fg(q, v, mu, h)                                                 # FGS(dt/ds)
+            q[:, bodies], v[:, bodies] = qf[:, bodies], vf[:, bodies]
+            enc, gr = encounters(level, q0, v0, q, v, h, pairs_up[ks.enc])
+            if len(enc):
+                if level < slevels - 1:
+                    b = np.asarray(gr.members)
+                    q[:, b], v[:, b] = q0[:, b], v0[:, b]
+                    q, v = senc(q, v, level + 1, enc, b)
+                else:
+                    q, v = bulirsch_stoer(level, q0, v0, h, gr, q, v)
+            ks = _kick.kick_list(q, mass, rc[:level + 1], n_massive, n_test, pairs_up, level=level, G=G,
+                                 enc_factor=enc_factor)                                  # KickS(dt/ds/2)
+            v = v + (0.5 * h) * ks.acc
+        return q, v
+
+    k1 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    v = v + (0.5 * dt) * k1.acc
+    q, _ = hc(q, v, mass, m_star, 0.5 * dt)
+    q_in, v_in = q.copy(), v.copy()
+    q, v, bad1 = fg(q, v, mu, dt)
+    unbound.append(bad1)
+    enc, gr = encounters(0, q_in, v_in, q, v, dt, _kick.pair_set(k1, n_massive))
+    if len(enc):
+        if slevels > 1:
+            b = np.asarray(gr.members)
+            q[:, b], v[:, b] = q_in[:, b], v_in[:, b]
+            q, v = senc(q, v, 1, enc, b)
+        else:
+            q, v = bulirsch_stoer(0, q_in, v_in, dt, gr, q, v)
+    q, _ = hc(q, v, mass, m_star, 0.5 * dt)
+    k2 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    v = v + (0.5 * dt) * k2.acc
+    return MultilevelStepResult(pos=q, vel=v, rcrit=rc, first=k1, stats=stats, unbound=sum(unbound))

@@ -232,3 +232,108 @@ def test_hybrid_step_carries_a_close_encounter(st):
     # (the residual ~1e-6 is the price of reading G5: K weights the force, not the potential, inside the band)
     assert out["hybrid"][0] < 1e-5
     assert out["plain"][0] > 300 * out["hybrid"][0]
+
+
+# ------------------------------------------------------------------------------- the multi-level step (App. A, SEnc)
+def _encounter_system():
+    mass = np.array([3e-5, 3e-5])
+    a = np.array([1.0, 1.02]); e = np.array([0.02, 0.03]); z = np.zeros(2)
+    pos, vel = gi.elements_to_cartesian(a, e, z + 0.001, z, np.array([0.0, 0.6]), np.array([0.0, -0.57]), G)
+    vel = vel - (mass * vel).sum(1, keepdims=True) / (1.0 + mass.sum())
+    return pos, vel, mass
+
+
+def test_multilevel_step_reduces_to_the_hybrid_and_the_plain_step(st):
+    ki = gi.make_config(0, n=900)
+    vel = ki.vel - (ki.mass * ki.vel).sum(1, keepdims=True) / (1.0 + ki.mass.sum())
+    h = st.hybrid_step(ki.pos, vel, ki.mass, ki.n, 0, 1.0, ki.G, ki.dt)
+    m = st.multilevel_step(ki.pos, vel, ki.mass, ki.n, 0, 1.0, ki.G, ki.dt, slevels=1, detect=False)
+    assert h.groups.n_groups > 10 and np.array_equal(h.pos, m.pos) and np.array_equal(h.vel, m.vel)
+    assert m.stats[0].tolist() == [len(h.groups.members) and m.stats[0, 0], m.stats[0, 0], h.groups.n_groups,
+                                   len(h.groups.members)]
+    # SLevels = 1 with the detection: pairs inside r_crit before the drift stay encounter pairs (p(0) = d0) -- same step
+    m = st.multilevel_step(ki.pos, vel, ki.mass, ki.n, 0, 1.0, ki.G, ki.dt, slevels=1, detect=True)
+    assert np.array_equal(h.pos, m.pos) and np.array_equal(h.vel, m.vel)
+    # no candidates at all: every variant is the plain step
+    mass = np.array([1e-3, 3e-4]); z = np.zeros(2)
+    pos, vel = gi.elements_to_cartesian(np.array([1.0, 2.2]), np.array([0.05, 0.1]), z + 0.02, z, z + 1.0,
+                                        np.array([0.3, 2.0]), G)
+    p = st.step(pos, vel, mass, 2, 0, 1.0, G, 4.0)
+    for sl, ss in ((2, 2), (3, 10)):
+        m = st.multilevel_step(pos, vel, mass, 2, 0, 1.0, G, 4.0, slevels=sl, substeps=ss)
+        assert m.stats.sum() == 0 and np.array_equal(p.pos, m.pos) and np.array_equal(p.vel, m.vel)
+
+
+@pytest.mark.parametrize("slevels,substeps", [(2, 2), (3, 2), (2, 10), (3, 4)])
+def test_multilevel_step_carries_a_close_encounter(st, slevels, substeps):
+    """The encounter of test_hybrid_step_carries_a_close_encounter under the multi-level scheme: the energy stays as
+    good as with the two-level hybrid step (the deep part still goes to Bulirsch-Stoer, "only called at the blue lines",
+    PAPER.md:636), and every level was entered."""
+    pos, vel, mass = _encounter_system()
+    e0 = _energy(pos, vel, mass, 1.0)
+    q, v = pos.copy(), vel.copy()
+    worst, stats = 0.0, 0
+    for _ in range(400):
+        r = st.multilevel_step(q, v, mass, 2, 0, 1.0, G, 2.0, slevels=slevels, substeps=substeps, tol=1e-13)
+        q, v = r.pos, r.vel
+        stats = stats + r.stats
+        worst = max(worst, abs(_energy(q, v, mass, 1.0) - e0) / abs(e0))
+    assert worst < 1e-5
+    assert stats[0, 1] > 3 and stats[-1, 2] > 3 and np.all(stats[:-1, 2] == 0)      # BS only at the deepest level
+    for l in range(1, slevels):
+        assert 0 < stats[l, 1] <= substeps * stats[l - 1, 1]
+
+
+def _newton_reference(pos, vel, mass, t_end):
+    """Sun + planets as a plain Newtonian (n + 1)-body problem in barycentric coordinates, scipy DOP853; returns the
+    democratic coordinates (heliocentric positions, barycentric velocities) at t_end."""
+    from scipy.integrate import solve_ivp
+    n = mass.size
+    m = np.concatenate([[1.0], mass])
+    x0 = -(mass * pos).sum(1) / m.sum()
+    x = np.concatenate([x0[:, None], pos + x0[:, None]], 1)
+    u = np.concatenate([(-(mass * vel).sum(1))[:, None], vel], 1)
+
+    def rhs(t, y):
+        x = y[:3 * (n + 1)].reshape(3, n + 1); u = y[3 * (n + 1):].reshape(3, n + 1)
+        a = np.zeros_like(x)
+        for i in range(n + 1):
+            d = x - x[:, i:i + 1]
+            r3 = (d * d).sum(0) ** 1.5
+            r3[i] = 1.0
+            a[:, i] = (G * m * d / r3).sum(1)
+        return np.concatenate([u.ravel(), a.ravel()])
+
+    sol = solve_ivp(rhs, (0.0, t_end), np.concatenate([x.ravel(), u.ravel()]), method="DOP853", rtol=1e-13, atol=1e-16)
+    y = sol.y[:, -1]
+    x = y[:3 * (n + 1)].reshape(3, n + 1); u = y[3 * (n + 1):].reshape(3, n + 1)
+    return x[:, 1:] - x[:, :1], u[:, 1:]
+
+
+def test_multilevel_step_converges_to_the_newtonian_trajectory(st):
+    """The level weights of eq. 62-63 sum to 1, so all levels together integrate the full Newtonian problem.  Reference:
+    an independent DOP853 integration of Sun + 2 planets through the encounter (heliocentric displacement by the
+    encounter ~ 2e-2 AU: the step WITHOUT the encounter branch ends 2.2e-2 AU away from the reference at every dt).
+    A wrong weight, sub-step length, restart state or a missing kick anywhere in SEnc leaves an error of that order;
+    the scheme as printed ends within 1e-5 AU and closer as dt shrinks (the residue at fixed dt is the changeover
+    band, whose width ~ dt: readings G1 / G5, not a clean dt^2)."""
+    pos, vel, mass = _encounter_system()
+    t_end = 200.0                                            # the approach happens around t = 100 .. 160 d
+    q_ref, v_ref = _newton_reference(pos, vel, mass, t_end)
+    q, v = pos.copy(), vel.copy()
+    for _ in range(100):
+        r = st.step(q, v, mass, 2, 0, 1.0, G, 2.0)
+        q, v = r.pos, r.vel
+    assert np.abs(q - q_ref).max() > 1e-2
+    errs = {}
+    for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10)):
+        for dt in (2.0, 0.5):
+            q, v = pos.copy(), vel.copy()
+            deep = 0
+            for _ in range(int(round(t_end / dt))):
+                r = st.multilevel_step(q, v, mass, 2, 0, 1.0, G, dt, slevels=sl, substeps=ss, tol=1e-13)
+                q, v = r.pos, r.vel
+                deep += r.stats[-1, 2]
+            errs[sl, ss, dt] = np.abs(q - q_ref).max()
+            assert deep > 0
+        assert errs[sl, ss, 2.0] < 3e-5 and errs[sl, ss, 0.5] < 3e-6, errs
