@@ -30,12 +30,19 @@ STATUS_BAD_PAIR = 16
 BS_EXPORTS = ("genga_bs", "genga_hybrid_step")
 STATUS_GROUP_TOO_LARGE, STATUS_BS_NOT_CONVERGED = 32, 64
 STATUS_UNBOUND = 8
+# include/genga_senc.h: close-encounter detection and the multi-level step (SEnc)
+SENC_EXPORTS = ("genga_detect", "genga_multilevel_step")
 
 
 class GengaKickConfig(C.Structure):
     _fields_ = [("n_massive", C.c_int32), ("n_test", C.c_int32), ("max_level", C.c_int32), ("device", C.c_int32),
                 ("pair_capacity", C.c_int64), ("G", C.c_double), ("enc_factor", C.c_double),
                 ("order_mode", C.c_int32), ("tp_mode", C.c_int32)]
+
+
+class GengaSencConfig(C.Structure):
+    _fields_ = [("slevels", C.c_int32), ("substeps", C.c_int32), ("detect", C.c_int32), ("reserved", C.c_int32),
+                ("n1", C.c_double), ("n2", C.c_double), ("tol", C.c_double)]
 
 
 class GengaKickPlan(C.Structure):
@@ -97,7 +104,9 @@ def lib():
         L.genga_group.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
         L.genga_hybrid_step.argtypes = [vp, vp, vp, vp, d, d, d, d, d, vp, vp, vp, vp, vp, vp, vp]
         L.genga_bs.argtypes = [vp, vp, vp, vp, vp, i32, d, d, d, vp, vp, vp, vp, vp]
-        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS:
+        L.genga_detect.argtypes = [vp, vp, vp, vp, vp, vp, d, d, vp, vp, i64, vp, vp]
+        L.genga_multilevel_step.argtypes = [vp, vp, vp, vp, d, d, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
+        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS + SENC_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
                 getattr(L, name).restype = C.c_int
         _lib = L
@@ -228,6 +237,20 @@ class GengaKick:
         self._check(lib().genga_hybrid_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt), float(n1),
                                             float(n2), float(tol), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs),
                                             _ptr(group_of), _ptr(members), _ptr(offsets), _ptr(summary)))
+
+    # include/genga_senc.h
+    def detect(self, pos0, vel0, pos1, vel1, rcrit_row, h, in_pairs, in_n_pairs, in_pair_rows, out_pairs, out_npairs,
+               enc_factor=1.0):
+        self._check(lib().genga_detect(self._ctx, _ptr(pos0), _ptr(vel0), _ptr(pos1), _ptr(vel1), _ptr(rcrit_row),
+                                       float(enc_factor), float(h), _ptr(in_pairs), _ptr(in_n_pairs), int(in_pair_rows),
+                                       _ptr(out_pairs), _ptr(out_npairs)))
+
+    def multilevel_step(self, pos, vel, mass, m_star, dt, slevels, substeps, tol, out_acc, out_pairs, out_npairs,
+                        out_stats, detect=True, n1=3.0, n2=0.4):
+        cfg = GengaSencConfig(int(slevels), int(substeps), int(bool(detect)), 0, float(n1), float(n2), float(tol))
+        self._check(lib().genga_multilevel_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt),
+                                                C.byref(cfg), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs),
+                                                _ptr(out_stats)))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

@@ -6,11 +6,12 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgenga_kick.so")
-SOURCES = [os.path.join(CSRC, "genga_kick.cu"), os.path.join(CSRC, "genga_step.cu"), os.path.join(CSRC, "genga_group.cu"), os.path.join(CSRC, "genga_bs.cu"),
+SOURCES = [os.path.join(CSRC, "genga_kick.cu"), os.path.join(CSRC, "genga_step.cu"), os.path.join(CSRC, "genga_group.cu"), os.path.join(CSRC, "genga_bs.cu"), os.path.join(CSRC, "genga_senc.cu"),
            os.path.join(CSRC, "genga_kick_plan.cpp")]
 DEPENDS = SOURCES + [os.path.join(CSRC, "genga_kick_kernels.cuh"), os.path.join(CSRC, "genga_kick_variants.h"),
                      os.path.join(CSRC, "genga_kick_sort.cuh"), os.path.join(CSRC, "genga_kick_ctx.h"),
-                     os.path.join(CSRC, "genga_step_kernels.cuh"), os.path.join(CSRC, "genga_group_kernels.cuh"), os.path.join(CSRC, "genga_bs_kernels.cuh"),
+                     os.path.join(CSRC, "genga_step_kernels.cuh"), os.path.join(CSRC, "genga_group_kernels.cuh"), os.path.join(CSRC, "genga_bs_kernels.cuh"), os.path.join(CSRC, "genga_senc_kernels.cuh"),
+                     os.path.join(os.path.dirname(HERE), "include", "genga_senc.h"),
                      os.path.join(os.path.dirname(HERE), "include", "genga_bs.h"),
                      os.path.join(os.path.dirname(HERE), "include", "genga_group.h"),
                      os.path.join(os.path.dirname(HERE), "include", "genga_step.h"),

@@ -58,6 +58,8 @@ struct genga_kick_ctx {
     double* bs_scratch;            // whole-grid Bulirsch-Stoer regime: positions (2 buffers), G m, r_crit rows, error slots
     int bs_coop_blocks;            // its co-resident grid
     double* hyb_state;             // [6][N] state before FG (genga_hybrid_step), lazily allocated
+    void* senc_slab;               // scratch of genga_multilevel_step (genga_senc.cu), lazily allocated
+    int senc_levels;               // levels it was cut for
     std::string cuda_err;
 };
 

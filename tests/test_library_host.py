@@ -57,6 +57,17 @@ def test_every_declared_bs_symbol_is_exported(built):
     assert all(hasattr(lib, name) for name in declared)
 
 
+def test_every_declared_senc_symbol_is_exported(built):
+    header = open(os.path.join(ROOT, "include", "genga_senc.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\bint\s+(genga_\w+)\s*\(", header))
+    assert declared == set(g.SENC_EXPORTS)
+    lib = ctypes.CDLL(built)
+    assert all(hasattr(lib, name) for name in declared)
+    import ctypes as C
+    assert C.sizeof(g.GengaSencConfig) == 40          # the struct of include/genga_senc.h: 4 x int32 + 3 x double
+
+
 def test_strerror_texts(built):
     for code in (g.OK, g.E_NULL, g.E_ALIGN, g.E_SIZE, g.E_LEVEL, g.E_CUDA, g.E_NOMEM):
         assert g.strerror(code) and "unknown" not in g.strerror(code)
