@@ -354,6 +354,42 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                    "largest_group": hs[2], "status": kick1.status()}
     kick1.free()
 
+    # NEXT-4: the multi-level step (SEnc recursion, App. A) -- the experiment of Fig. 10
+    # (PAPER.md:640): the same disks, the hybrid step against 2-4 symplectic levels
+    def time_multilevel(kin, slevels, substeps, reps):
+        nn = kin.n
+        km = GengaKick(nn, 0, max_level=slevels - 1, pair_capacity=PAIR_CAPACITY, G=kin.G, device=local_rank)
+        km.set_stream(stream.cuda_stream)
+        q0, v0, mm = to_dev(kin.pos), to_dev(kin.vel), to_dev(kin.mass)
+        q, v = q0.clone(), v0.clone()
+        macc = torch.empty(3, nn, dtype=torch.float64, device=dev)
+        mp, mnp = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev), i32(nn + 1)
+        mst = torch.zeros(slevels, 4, dtype=torch.int32, device=dev)
+        ts = []
+        for it in range(reps + 2):
+            q.copy_(q0); v.copy_(v0)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = km.launch_count()
+            a.record(stream)
+            km.multilevel_step(q, v, mm, 1.0, kin.dt, slevels, substeps, 1e-12, macc, mp, mnp, mst, detect=True)
+            b.record(stream)
+            b.synchronize()
+            nl = km.launch_count() - l0
+            if it >= 2:
+                ts.append(a.elapsed_time(b))
+        st = mst.cpu().tolist()
+        out = {"slevels": slevels, "substeps": substeps, "ms_per_step": float(np.median(ts)), "launches_per_step": int(nl),
+               "encounter_pairs_per_level": [r[1] for r in st], "bs_groups": st[-1][2], "bs_bodies": st[-1][3],
+               "status": km.status()}
+        km.free()
+        return out
+
+    multilevel_info = {"what": "genga_multilevel_step (Rcrit, Kick + pre-check, HC, FG, detection, SEnc over KickS / RcritS / "
+                               "FGS / detection / grouping / Bulirsch-Stoer tol 1e-12, HC, Kick), one step from the "
+                               "generated state; 1 level = the hybrid step",
+                       "configs[1] N=8192": [time_multilevel(k1, sl, ss, 5) for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10))],
+                       "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3) for sl, ss in ((2, 10), (4, 2), (3, 4))]}
+
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
@@ -401,6 +437,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             "group": group_info,
             "kick_list": list_info,
             "hybrid_step": hybrid_info,
+            "multilevel_step": multilevel_info,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
