@@ -17,8 +17,9 @@
  * Method (the paper names it and refers to Grimm & Stadel 2014; reading G15): Gragg-Bulirsch-
  * Stoer -- modified midpoint with 2, 4, .., 16 sub-steps, polynomial extrapolation in h^2, relative error
  * per body in position and velocity <= tol, one step size for the whole group (halved on failure, doubled
- * after fast convergence).  Groups of up to 256 bodies: one thread block per group, one thread per body, many
- * groups side by side (the regimes BS-B / BS-A of Table 2).  Larger groups: one group at a time
+ * after fast convergence).  One thread per body.  Groups of up to 32 bodies: one warp per group, eight groups per
+ * thread block (BS-B of Table 2); 33 .. 256 bodies: one thread block per group (BS-A); many
+ * groups side by side.  Larger groups: one group at a time
  * over a whole co-resident grid with a grid-wide barrier per force evaluation (the paper's BS-M regime,
  * PAPER.md:595-597, with the sub-steps kept on the device instead of controlled from the host); a group larger
  * than that grid (tens of thousands of bodies: 64 threads x resident CTAs) keeps the state already in pos / vel
@@ -42,7 +43,8 @@ extern "C" {
 /*
  *   pos_in, vel_in  [3][N] state before FG (read only)          mass [N]
  *   rcrit           [nlevels][N], 1 <= nlevels <= 4
- *   members, offsets, summary   as written by genga_group (summary[0] = number of groups, read on the device)
+ *   members, offsets, summary   as written by genga_group (summary[0] = number of groups and summary[2] = size of the
+ *                   largest group are read on the device; groups above 256 bodies are only looked for if summary[2] says so)
  *   pos, vel        [3][N] updated for the bodies of the integrated groups (may NOT alias pos_in / vel_in)
  * Errors: E_NULL, E_ALIGN, E_SIZE (nlevels outside 1..4, m_star <= 0, tol <= 0), E_CUDA.
  */

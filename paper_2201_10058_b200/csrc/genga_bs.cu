@@ -29,7 +29,7 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     if (!ctx->bs_scratch) {
         GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double)));
         int per_sm = 0;
-        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<true, GENGA_BS_COOP_THREADS>,
+        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>,
                                                                  GENGA_BS_COOP_THREADS, 0));
         if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
         ctx->bs_coop_blocks = per_sm * ctx->num_sms;
@@ -42,18 +42,26 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
         for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) { gm.rc[k] = p; p += N; }
         gm.err = reinterpret_cast<unsigned long long*>(p);
     }
-    // one CTA per group: at most N / 2 groups; CTAs stride over them (their number is only known on the device)
-    const int blocks = (int)std::min<long long>(std::max<long long>(N / 2, 1), 16LL * ctx->num_sms);
+    // at most N / 2 groups; warps / CTAs stride over them (their number is only known on the device)
     int small_max = GENGA_BS_THREADS;
-    genga::bs_kernel<false, GENGA_BS_THREADS><<<blocks, GENGA_BS_THREADS, 0, st>>>(
+    // one warp per group of up to 32 bodies (nearly all groups), eight groups per CTA
+    const int wblocks = (int)std::min<long long>(std::max<long long>((N / 2 + 7) / 8, 1), 8LL * ctx->num_sms);
+    genga::bs_kernel<GENGA_BS_MODE_WARP, GENGA_BS_THREADS><<<wblocks, GENGA_BS_THREADS, 0, st>>>(
         pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max);
+    // one CTA per group of 33 .. 256 bodies
+    if (N > GENGA_BS_WARP_MAX) {
+        const int blocks = (int)std::min<long long>(std::max<long long>(N / (GENGA_BS_WARP_MAX + 1), 1), 16LL * ctx->num_sms);
+        genga::bs_kernel<GENGA_BS_MODE_CTA, GENGA_BS_THREADS><<<blocks, GENGA_BS_THREADS, 0, st>>>(
+            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max);
+        ctx->launches++;
+    }
     GK_CUDA(ctx, cudaGetLastError());
     // the whole grid, one large group after the other (returns at once if there is none)
     if (N > GENGA_BS_THREADS) {
         GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
         void* args[] = {&pos_in, &vel_in, &mass, &rcrit, &NN, &nlevels, const_cast<double*>(&G), const_cast<double*>(&mu), &dt,
                         &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max};
-        GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<true, GENGA_BS_COOP_THREADS>),
+        GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>),
                                                  dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
         ctx->launches++;
     }

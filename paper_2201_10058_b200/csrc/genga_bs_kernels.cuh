@@ -1,8 +1,11 @@
 // sm_100a kernel of the Bulirsch-Stoer integration of close-encounter groups (include/genga_bs.h;
-// PAPER.md:47, :559-597, App. A), one body per thread, in two regimes:
-//   bs_kernel<false>  one CTA of 256 threads per group, the group's state in shared memory: the regimes BS-B and
-//                     BS-A of Table 2, groups of up to 256 bodies, many groups side by side;
-//   bs_kernel<true>   ONE group at a time over the whole grid (cooperative launch, 64-thread CTAs): the paper's
+// PAPER.md:47, :559-597, App. A), one body per thread, in three regimes of one template:
+//   bs_kernel<WARP>   one WARP per group of up to 32 bodies, eight groups side by side in a CTA, the group's state
+//                     in the warp's slice of shared memory, no CTA-wide barrier: the regime BS-B of Table 2
+//                     (sec. 6.1.1: n <= 32) -- nearly all groups are pairs;
+//   bs_kernel<CTA>    one CTA of 256 threads per group of 33 .. 256 bodies, the group's state in shared memory: the
+//                     regime BS-A of Table 2, many groups side by side;
+//   bs_kernel<COOP>   ONE group at a time over the whole grid (cooperative launch, 64-thread CTAs): the paper's
 //                     BS-M regime ("distributed over multiple thread blocks ... sub-steps ...
 //                     controlled from the host ... many different kernel calls") -- but here the sub-steps stay
 //                     on the device: positions are exchanged through L2 (double-buffered) and the CTAs meet at
@@ -24,6 +27,10 @@
 
 namespace genga {
 
+#define GENGA_BS_MODE_CTA 0
+#define GENGA_BS_MODE_COOP 1
+#define GENGA_BS_MODE_WARP 2
+#define GENGA_BS_WARP_MAX 32            // largest group of the warp-per-group regime
 #define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
 #define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
 #define GENGA_BS_TILE 64                // j-bodies staged per round in the whole-grid regime
@@ -78,7 +85,13 @@ struct BsShared {
 // Every thread publishes the position of its body i (if i < n) and gets dv_i/dt back:
 //   - G m_star q / |q|^3 + the pair terms over j = 0 .. n-1, j != i, in that order.
 // COOP: `eval` counts the force evaluations of the group (buffer parity); one grid barrier per call.
-template <bool COOP, int ROWS>
+template <int MODE>
+__device__ __forceinline__ void bs_sync()
+{
+    if (MODE == GENGA_BS_MODE_WARP) __syncwarp(); else __syncthreads();
+}
+
+template <int MODE, int ROWS>
 __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, int nlevels,
                                          double mu, const double (&rci)[GENGA_BS_MAX_LEVELS], const double (&q)[3],
                                          double (&a)[3])
@@ -88,10 +101,11 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
     const double rs = sqrt(r2s);
     const double s0 = -mu / (r2s * rs);
     double ax = s0 * x, ay = s0 * y, az = s0 * z;
+    constexpr bool COOP = MODE == GENGA_BS_MODE_COOP;
     if (!COOP) {
-        __syncthreads();                                      // the previous readers are done
+        bs_sync<MODE>();                                      // the previous readers are done
         if (i < n) { S.x[i] = x; S.y[i] = y; S.z[i] = z; }
-        __syncthreads();
+        bs_sync<MODE>();
         if (i < n) {
 #define GENGA_BS_RCJ(k) S.rc[k][j]
             for (int j = 0; j < n; j++) {
@@ -129,12 +143,14 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 }
 
 // maximum of e over the group (order-free); CTA- (and, COOP, grid-) uniform result
-template <bool COOP, int THREADS, int ROWS>
+template <int MODE, int THREADS, int ROWS>
 __device__ __forceinline__ double bs_group_max(BsShared<ROWS>& S, const BsGlobal& Gm, int& echeck, double e)
 {
+    constexpr bool COOP = MODE == GENGA_BS_MODE_COOP;
     const int t = threadIdx.x;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e = fmax(e, __shfl_xor_sync(0xffffffffu, e, o));
+    if (MODE == GENGA_BS_MODE_WARP) return e;                 // the group is the warp
     __syncthreads();
     if ((t & 31) == 0) S.red[t >> 5] = e;
     __syncthreads();
@@ -157,27 +173,77 @@ __device__ __forceinline__ double bs_group_max(BsShared<ROWS>& S, const BsGlobal
     return m;
 }
 
-// COOP = false: CTA g, g + gridDim.x, ... integrates group g if it has at most THREADS bodies (others: left to
-//               the whole-grid regime).
-// COOP = true : the whole grid integrates, one after the other, the groups with more than `small_max` bodies;
-//               groups larger than the grid are reported and left as they are.
-template <bool COOP, int THREADS>
+// Whole-grid regime: every CTA builds the same list of the next (up to GENGA_BS_BIG_LIST) groups with more than
+// `small_max` bodies, in ascending order, scanning the offsets from group `scan_from` on, THREADS groups per round
+// (a serial walk over tens of thousands of two-body groups cost 0.6 ms per call).  CTA-uniform results.
+#define GENGA_BS_BIG_LIST 256
+template <int THREADS>
+__device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, int n_groups, int small_max, int& scan_from,
+                                              int* big, unsigned* wm, int& nbig)
+{
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    int count = 0;
+    while (scan_from < n_groups && count + THREADS <= GENGA_BS_BIG_LIST) {
+        const int g = scan_from + t;
+        const bool is_big = g < n_groups && offsets[g + 1] - offsets[g] > small_max;
+        const unsigned m = __ballot_sync(0xffffffffu, is_big);
+        __syncthreads();                                               // wm's previous readers are done
+        if (lane == 0) wm[warp] = m;
+        __syncthreads();
+        int before = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < THREADS / 32; w++) {
+            const int c = __popc(wm[w]);
+            if (w < warp) before += c;
+            total += c;
+        }
+        if (is_big) big[count + before + __popc(m & ((1u << lane) - 1u))] = g;
+        count += total;
+        scan_from += THREADS;
+    }
+    __syncthreads();
+    nbig = count;
+}
+
+// WARP: warp w, w + (warps of the grid), ... integrates group w if it has at most 32 bodies.
+// CTA : CTA g, g + gridDim.x, ... integrates group g if it has 33 .. THREADS bodies.
+// COOP: the whole grid integrates, one after the other, the groups with more than `small_max` bodies;
+//       groups larger than the grid are reported and left as they are.
+template <int MODE, int THREADS>
 __global__ void __launch_bounds__(THREADS)
 bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
           double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max)
 {
-    constexpr int ROWS = COOP ? GENGA_BS_TILE : THREADS;
-    __shared__ BsShared<ROWS> S;
-    const int t = threadIdx.x;
+    constexpr bool COOP = MODE == GENGA_BS_MODE_COOP, WARP = MODE == GENGA_BS_MODE_WARP;
+    constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : THREADS);
+    constexpr int UNITS = WARP ? THREADS / 32 : 1;                      // groups in flight per CTA
+    __shared__ BsShared<ROWS> Sall[UNITS];
+    BsShared<ROWS>& S = Sall[WARP ? threadIdx.x >> 5 : 0];
+    const int t = WARP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
     const int i = COOP ? (int)(blockIdx.x * THREADS + t) : t;           // this thread's body within the group
-    const long long capacity = COOP ? (long long)gridDim.x * THREADS : THREADS;
+    const long long capacity = COOP ? (long long)gridDim.x * THREADS : ROWS;
     const int n_groups = summary[0];
     int eval = 0, echeck = 0;
-    for (int g = COOP ? 0 : (int)blockIdx.x; g < n_groups; g += COOP ? 1 : (int)gridDim.x) {
+    const int g0 = COOP ? 0 : (WARP ? (int)(blockIdx.x * UNITS + (threadIdx.x >> 5)) : (int)blockIdx.x);
+    const int gstep = COOP ? 1 : (int)gridDim.x * UNITS;
+    __shared__ int big[COOP ? GENGA_BS_BIG_LIST : 1];
+    __shared__ unsigned wm[THREADS / 32];
+    int scan_from = 0, nbig = 0, ib = 0;
+    if (COOP && summary[2] <= small_max) return;                        // no group for this regime (grid-uniform)
+    for (int g = g0;; g += gstep) {
+        if (COOP) {
+            while (ib == nbig && scan_from < n_groups) {
+                bs_scan_large<THREADS>(offsets, n_groups, small_max, scan_from, big, wm, nbig);
+                ib = 0;
+            }
+            if (ib == nbig) break;
+            g = big[ib++];
+        } else if (g >= n_groups) break;
         const int first = offsets[g], n = offsets[g + 1] - first;
-        if (COOP ? n <= small_max : n > THREADS) continue;             // the other regime's group (grid-/CTA-uniform)
+        // the other regimes' groups (grid- / CTA- / warp-uniform)
+        if (COOP ? n <= small_max : (WARP ? n > GENGA_BS_WARP_MAX : (n > THREADS || n <= GENGA_BS_WARP_MAX))) continue;
         if (n > capacity) {
             if (t == 0 && blockIdx.x == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
             continue;
@@ -185,7 +251,7 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
         const bool active = i < n;
         const long long b = active ? members[first + i] : 0;
         double q[3] = {0.0, 0.0, 0.0}, v[3] = {0.0, 0.0, 0.0}, rci[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
-        if (!COOP) __syncthreads();                                     // the previous group's readers are done
+        if (!COOP) bs_sync<MODE>();                                     // the previous group's readers are done
         if (active) {
 #pragma unroll
             for (int c = 0; c < 3; c++) { q[c] = pos_in[c * N + b]; v[c] = vel_in[c * N + b]; }
@@ -207,7 +273,7 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
         bool fail = false;
         while (done != dt) {                                           // all decisions below are group-uniform
             if ((dt > 0.0 && done + H > dt) || (dt < 0.0 && done + H < dt)) H = dt - done;
-            bs_force<COOP, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, q, a0);
+            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, q, a0);
             int halvings = 0, kconv = 0;
             for (;;) {
                 bool ok = false;
@@ -219,14 +285,14 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
 #pragma unroll
                         for (int c = 0; c < 3; c++) { qm[c] = q[c]; vm[c] = v[c]; qn[c] = q[c] + h * v[c]; vn[c] = v[c] + h * a0[c]; }
                         for (int m = 1; m < nk; m++) {
-                            bs_force<COOP, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
+                            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
 #pragma unroll
                             for (int c = 0; c < 3; c++) {
                                 const double qs = qm[c] + h2 * vn[c], vs = vm[c] + h2 * a[c];
                                 qm[c] = qn[c]; vm[c] = vn[c]; qn[c] = qs; vn[c] = vs;
                             }
                         }
-                        bs_force<COOP, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
+                        bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
 #pragma unroll
                         for (int c = 0; c < 3; c++) {
                             cq[c] = 0.5 * (qn[c] + qm[c] + h * vn[c]);
@@ -259,7 +325,7 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
                             }
                             e = fmax(sqrt(eq2) / sqrt(sq2), sqrt(ev2) / sqrt(sv2));
                         }
-                        if (bs_group_max<COOP, THREADS, ROWS>(S, Gm, echeck, e) <= tol) { ok = true; kconv = k + 1; break; }
+                        if (bs_group_max<MODE, THREADS, ROWS>(S, Gm, echeck, e) <= tol) { ok = true; kconv = k + 1; break; }
                     }
                 }
                 if (ok) break;

@@ -29,7 +29,8 @@ def _gpu_bs(n, pos_in, vel_in, mass, rcrit, nlevels, dt, tol, members, offsets, 
     ng = len(offsets) - 1
     d_mem = torch.zeros(max(n, 4), dtype=torch.int32, device="cuda"); d_mem[:len(members)] = _dev(np.asarray(members, np.int32))
     d_off = torch.zeros(n + 4, dtype=torch.int32, device="cuda"); d_off[:ng + 1] = _dev(np.asarray(offsets, np.int32))
-    d_sum = torch.tensor([ng, len(members), 0, 0], dtype=torch.int32, device="cuda")
+    largest = int(np.diff(np.asarray(offsets)).max()) if ng else 0
+    d_sum = torch.tensor([ng, len(members), largest, 0], dtype=torch.int32, device="cuda")
     q, v = _dev(pos), _dev(vel)
     k.bs(_dev(pos_in), _dev(vel_in), _dev(mass), _dev(np.asarray(rcrit)[:nlevels]), nlevels, 1.0, dt, tol, d_mem, d_off,
          d_sum, q, v)
