@@ -255,3 +255,30 @@ def test_multilevel_step_error_codes():
     assert call(2, 2, m_star=0.0) == g.E_SIZE and call(3, 2) == g.E_LEVEL and call(2, 2, pos=None) == g.E_NULL
     assert call(2, 2, pos=p(x) + 8) == g.E_ALIGN
     k.free()
+
+
+def test_multilevel_step_full_size_config3(oracle_mod):
+    """configs[3] at its full size (N = 65,536) in the configuration bench.py times: 2 levels x 10 sub-steps with
+    detection, capacity 2^20 -- the regime of PAPER.md:78-82 where the level-0 pairs link half the disk into one group
+    and the higher level dissolves it into ~4000 small groups per sub-step."""
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    ki = gi.make_config(3)
+    n, cap = ki.n, 1 << 20
+    assert n == 65536
+    k = GengaKick(n, 0, max_level=1, G=ki.G, pair_capacity=cap)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, v, mass = _dev(ki.pos), _dev(ki.vel), _dev(ki.mass)
+    acc, pairs, npairs, stats = _ml_buffers(n, cap, 2)
+    k.multilevel_step(q, v, mass, 1.0, ki.dt, 2, 10, 1e-12, acc, pairs, npairs, stats)
+    torch.cuda.synchronize()
+    assert k.status() == 0
+    r = oracle_mod.step.multilevel_step(ki.pos, ki.vel, ki.mass, n, 0, 1.0, ki.G, ki.dt, slevels=2, substeps=10, tol=1e-12)
+    gs = stats.cpu().numpy()
+    assert r.stats[0, 1] > 400000 and r.stats[1, 2] > 30000
+    # the per-level decisions (integers from floating point) may differ for a pair within rounding of a threshold: the
+    # critical radii of the two sides differ by <= 7 u (tests/test_gpu_step.py); allow 2 in 1e5, report exact equality
+    assert np.all(np.abs(gs - r.stats) <= np.maximum(2, 2e-5 * r.stats)), (gs.tolist(), r.stats.tolist())
+    print("per-level statistics identical:", bool(np.array_equal(gs, r.stats)), gs.tolist())
+    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0)
+    k.free()
