@@ -14,7 +14,9 @@
  *     W_BS    = prod_{k < nlevels} [1 - K(r_ij; rck_ij)]      K_Bulirsch-Stoer of eq. 62-63;
  *               nlevels = 1: the complement 1 - K of the kick's weight, so that kick + this = Newton
  * (force-weighted like the kick, reading G5; rck_ij = max of the two bodies' rows, reading G2;
- * test particles -- mass 0 -- feel the others and act on nobody by themselves.)
+ * Test-particle modes, sec. 8.1 PAPER.md:791-808 and Fig. 14: with is_tp given, the term of j on i is summed iff j is a
+ * massive body, or j is a semi-active particle, the mode is TP 2 and i is a massive body -- particles feel the massive
+ * bodies "the same way as in the fully interactive mode", act on them only in TP 2, and never feel each other.)
  *
  * How.  PAPER.md names the method and gives no algorithmic detail (it refers to Grimm & Stadel 2014 and
  * to textbooks); the scheme below is the textbook Gragg-Bulirsch-Stoer method, fixed here as reading G15
@@ -52,6 +54,8 @@ typedef struct {
     double G, mu;
     const double *m;        /* [n] */
     const double *rc;       /* [nlevels][n] */
+    const int8_t *is_tp;    /* [n] 1 = semi-active test particle, or NULL (fully interactive, TP 0) */
+    int tp_mode;            /* 2: particles act on the massive bodies; otherwise on nobody */
 } bs_group;
 
 /* f: accelerations of all bodies of the group at positions q [n][3] */
@@ -66,6 +70,7 @@ static void bs_accel(const bs_group *g, const double *q, double *a)
         double ax = s0 * x, ay = s0 * y, az = s0 * z;
         for (int j = 0; j < n; j++) {
             if (j == i) continue;
+            if (g->is_tp && g->is_tp[j] && (g->tp_mode != 2 || g->is_tp[i])) continue;      /* Fig. 14 */
             const double dx = q[3 * j] - x, dy = q[3 * j + 1] - y, dz = q[3 * j + 2] - z;
             const double r2 = dx * dx + dy * dy + dz * dz;
             const double r = sqrt(r2);
@@ -111,10 +116,11 @@ static void bs_midpoint(const bs_group *g, const double *q0, const double *v0, c
  * returns 0, or 1 if a macro step did not converge after BS_MAX_HALVINGS halvings (state left at the last
  * accepted time).
  */
-int genga_oracle_bs_group(int32_t n, int32_t nlevels, double G, double m_star, double dt, double tol,
-                          const double *m, const double *rc, double *q, double *v, int64_t *stats)
+int genga_oracle_bs_group_tp(int32_t n, int32_t nlevels, double G, double m_star, double dt, double tol,
+                             const double *m, const double *rc, double *q, double *v, int64_t *stats,
+                             const int8_t *is_tp, int32_t tp_mode)
 {
-    bs_group g = {n, nlevels, G, G * m_star, m, rc};
+    bs_group g = {n, nlevels, G, G * m_star, m, rc, is_tp, tp_mode};
     const int n3 = 3 * n;
     /* P[j] holds T_{k-1,j} of the previous row, component-wise: Pq[j][n3], Pv[j][n3] */
     double *buf = (double *)malloc((size_t)(2 * BS_KMAX * n3 + 5 * n3 + 5 * n3) * sizeof(double));
@@ -175,4 +181,11 @@ int genga_oracle_bs_group(int32_t n, int32_t nlevels, double G, double m_star, d
     if (stats) { stats[0] = acc; stats[1] = rej; stats[2] = fev; }
     free(buf);
     return fail;
+}
+
+/* fully interactive group (TP 0) */
+int genga_oracle_bs_group(int32_t n, int32_t nlevels, double G, double m_star, double dt, double tol,
+                          const double *m, const double *rc, double *q, double *v, int64_t *stats)
+{
+    return genga_oracle_bs_group_tp(n, nlevels, G, m_star, dt, tol, m, rc, q, v, stats, 0, 0);
 }

@@ -91,7 +91,7 @@ class HybridStepResult:
 
 
 def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc_factor=1.0, n1=3.0, n2=0.4,
-                max_group=None):
+                max_group=None, tp_mode=1):
     """The complete scheme of App. A, every candidate pair of the pre-check treated as an encounter
     pair (no separate detection: PAPER.md gives no criterion, and a pair that never enters its critical radius has
     W_BS = 0, so integrating it is only extra work):
@@ -101,16 +101,17 @@ def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc
     q, v, mass = _c(pos).copy(), _c(vel).copy(), _c(mass)
     n = q.shape[1]
     rc, bad0 = rcrit(q, v, mass, m_star, G, dt, 2.0, 1, n1, n2)
-    k1 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    tpn = n_massive if n_test > 0 else None                # bodies from here on are semi-active particles
+    k1 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256, tp_mode=tp_mode)
     v = v + (0.5 * dt) * k1.acc
     q, _ = hc(q, v, mass, m_star, 0.5 * dt)
     q_in, v_in = q.copy(), v.copy()
     q, v, bad1 = fg(q, v, G * m_star, dt)
     gr = _group.group(n, _kick.pair_set(k1, n_massive))
     q, v, _, skipped = _bs.bs(q_in, v_in, mass, rc, gr.members, gr.offsets, G, m_star, dt, tol, q, v, nlevels=1,
-                              max_group=max_group)
+                              max_group=max_group, n_massive=tpn, tp_mode=tp_mode)
     q, _ = hc(q, v, mass, m_star, 0.5 * dt)
-    k2 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    k2 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256, tp_mode=tp_mode)
     v = v + (0.5 * dt) * k2.acc
     return HybridStepResult(pos=q, vel=v, rcrit=rc, first=k1, groups=gr, skipped=skipped, unbound=bad0 + bad1)
 
@@ -127,7 +128,7 @@ class MultilevelStepResult:
 
 
 def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2, substeps=2, tol=1e-12, enc_factor=1.0,
-                    n1=3.0, n2=0.4, detect=True, max_group=None):
+                    n1=3.0, n2=0.4, detect=True, max_group=None, tp_mode=1):
     """The multi-level scheme of App. A, written as printed there:
 
         Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt)
@@ -149,7 +150,8 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
     Bulirsch-Stoer phase does, G15), which the sub-steps replace; RcritS writes row l of eq. 5 at dt/substeps^l from the
     current velocities; KickS is the level-l kick of eq. 63 over the listed pairs with its level-l
     pre-check; the Bulirsch-Stoer phase of the deepest level carries W_BS = prod_{k < SLevels} (1 - K_k).
-    detect=False: every candidate of a pre-check counts as a close-encounter pair (as hybrid_step does)."""
+    detect=False: every candidate of a pre-check counts as a close-encounter pair (as hybrid_step does).
+    tp_mode: the test-particle mode of every kick and of the Bulirsch-Stoer phase (sec. 8.1)."""
     from . import group as _group, bs as _bs, detect as _det
     q, v, mass = _c(pos).copy(), _c(vel).copy(), _c(mass)
     n = q.shape[1]
@@ -167,7 +169,7 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
 
     def bulirsch_stoer(level, q0, v0, h, gr, q, v):
         q, v, _, skipped = _bs.bs(q0, v0, mass, rc, gr.members, gr.offsets, G, m_star, h, tol, q, v, nlevels=level + 1,
-                                  max_group=max_group)
+                                  max_group=max_group, n_massive=n_massive if n_test > 0 else None, tp_mode=tp_mode)
         stats[level, 2] += gr.n_groups - len(skipped)
         stats[level, 3] += len(gr.members) - sum(int(gr.offsets[g + 1] - gr.offsets[g]) for g in skipped)
         return q, v
@@ -178,7 +180,7 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
             row, _ = rcrit(q, v, mass, m_star, G, h, 2.0, 1, n1, n2)                    # RcritS
             rc[level, bodies] = row[0, bodies]
             ks = _kick.kick_list(q, mass, rc[:level + 1], n_massive, n_test, pairs_up, level=level, G=G,
-                                 enc_factor=enc_factor)                                  # KickS(dt/ds/2)
+                                 enc_factor=enc_factor, tp_mode=tp_mode)                 # KickS(dt/ds/2)
             v = v + (0.5 * h) * ks.acc
             q0, v0 = q.copy(), v.copy()
             qf, vf, b1 = fg(q, v, mu, h)                                                 # FGS(dt/ds)
@@ -192,11 +194,11 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
                 else:
                     q, v = bulirsch_stoer(level, q0, v0, h, gr, q, v)
             ks = _kick.kick_list(q, mass, rc[:level + 1], n_massive, n_test, pairs_up, level=level, G=G,
-                                 enc_factor=enc_factor)                                  # KickS(dt/ds/2)
+                                 enc_factor=enc_factor, tp_mode=tp_mode)                 # KickS(dt/ds/2)
             v = v + (0.5 * h) * ks.acc
         return q, v
 
-    k1 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    k1 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256, tp_mode=tp_mode)
     v = v + (0.5 * dt) * k1.acc
     q, _ = hc(q, v, mass, m_star, 0.5 * dt)
     q_in, v_in = q.copy(), v.copy()
@@ -211,6 +213,6 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
         else:
             q, v = bulirsch_stoer(0, q_in, v_in, dt, gr, q, v)
     q, _ = hc(q, v, mass, m_star, 0.5 * dt)
-    k2 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256)
+    k2 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256, tp_mode=tp_mode)
     v = v + (0.5 * dt) * k2.acc
     return MultilevelStepResult(pos=q, vel=v, rcrit=rc, first=k1, stats=stats, unbound=sum(unbound))

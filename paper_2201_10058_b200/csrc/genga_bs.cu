@@ -25,6 +25,9 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     const double G = ctx->cfg.G, mu = ctx->cfg.G * m_star;
     int* status = ctx->status;
     long long NN = N;
+    // test-particle modes (sec. 8.1): bodies from n_massive on are semi-active particles; TP 0 has none
+    long long n_massive = ctx->cfg.n_test > 0 ? (long long)ctx->cfg.n_massive : N;
+    int tp_mode = ctx->cfg.tp_mode;
     // whole-grid regime: scratch for one group of up to N bodies, and the size of a co-resident grid
     if (!ctx->bs_scratch) {
         GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double)));
@@ -47,12 +50,12 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     // one warp per group of up to 32 bodies (nearly all groups), eight groups per CTA
     const int wblocks = (int)std::min<long long>(std::max<long long>((N / 2 + 7) / 8, 1), 8LL * ctx->num_sms);
     genga::bs_kernel<GENGA_BS_MODE_WARP, GENGA_BS_THREADS><<<wblocks, GENGA_BS_THREADS, 0, st>>>(
-        pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max);
+        pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode);
     // one CTA per group of 33 .. 256 bodies
     if (N > GENGA_BS_WARP_MAX) {
         const int blocks = (int)std::min<long long>(std::max<long long>(N / (GENGA_BS_WARP_MAX + 1), 1), 16LL * ctx->num_sms);
         genga::bs_kernel<GENGA_BS_MODE_CTA, GENGA_BS_THREADS><<<blocks, GENGA_BS_THREADS, 0, st>>>(
-            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max);
+            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode);
         ctx->launches++;
     }
     GK_CUDA(ctx, cudaGetLastError());
@@ -60,7 +63,7 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     if (N > GENGA_BS_THREADS) {
         GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
         void* args[] = {&pos_in, &vel_in, &mass, &rcrit, &NN, &nlevels, const_cast<double*>(&G), const_cast<double*>(&mu), &dt,
-                        &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max};
+                        &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max, &n_massive, &tp_mode};
         GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>),
                                                  dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
         ctx->launches++;

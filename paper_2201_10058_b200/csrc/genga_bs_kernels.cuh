@@ -68,17 +68,24 @@ struct BsShared {
     double errmax;
 };
 
-// one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3
+// one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3.
+// Test-particle modes (sec. 8.1, Fig. 14): a semi-active particle j is staged with the SIGN BIT of
+// G m_j set; it acts on nobody in TP 1 and on the massive bodies only in TP 2 (particles never feel each other).
 #define GENGA_BS_PAIR(XJ, YJ, ZJ, GMJ, RCJ)                                                            \
     {                                                                                                  \
-        const double dx = (XJ) - x, dy = (YJ) - y, dz = (ZJ) - z;                                      \
-        const double r2 = dx * dx + dy * dy + dz * dz;                                                 \
-        const double r = sqrt(r2);                                                                     \
-        double W = 1.0;                                                                                \
-        for (int k = 0; k < nlevels; k++) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));                  \
-        if (W != 0.0) {                                                                                \
-            const double s = (GMJ) * W / (r2 * r);                                                     \
-            ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;                                      \
+        double gmj = (GMJ);                                                                            \
+        bool skip = false;                                                                             \
+        if (__double2hiint(gmj) < 0) { skip = i_tp || tp_mode != 2; gmj = -gmj; }                      \
+        if (!skip) {                                                                                   \
+            const double dx = (XJ) - x, dy = (YJ) - y, dz = (ZJ) - z;                                  \
+            const double r2 = dx * dx + dy * dy + dz * dz;                                             \
+            const double r = sqrt(r2);                                                                 \
+            double W = 1.0;                                                                            \
+            for (int k = 0; k < nlevels; k++) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));              \
+            if (W != 0.0) {                                                                            \
+                const double s = gmj * W / (r2 * r);                                                   \
+                ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;                                  \
+            }                                                                                          \
         }                                                                                              \
     }
 
@@ -93,7 +100,7 @@ __device__ __forceinline__ void bs_sync()
 
 template <int MODE, int ROWS>
 __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, int nlevels,
-                                         double mu, const double (&rci)[GENGA_BS_MAX_LEVELS], const double (&q)[3],
+                                         bool i_tp, int tp_mode, double mu, const double (&rci)[GENGA_BS_MAX_LEVELS], const double (&q)[3],
                                          double (&a)[3])
 {
     const double x = q[0], y = q[1], z = q[2];
@@ -214,7 +221,8 @@ __global__ void __launch_bounds__(THREADS)
 bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
-          double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max)
+          double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max,
+          long long n_massive, int tp_mode)
 {
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP, WARP = MODE == GENGA_BS_MODE_WARP;
     constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : THREADS);
@@ -250,12 +258,14 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
         }
         const bool active = i < n;
         const long long b = active ? members[first + i] : 0;
+        const bool i_tp = b >= n_massive;
         double q[3] = {0.0, 0.0, 0.0}, v[3] = {0.0, 0.0, 0.0}, rci[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
         if (!COOP) bs_sync<MODE>();                                     // the previous group's readers are done
         if (active) {
 #pragma unroll
             for (int c = 0; c < 3; c++) { q[c] = pos_in[c * N + b]; v[c] = vel_in[c * N + b]; }
-            const double gm = G * mass[b];
+            // semi-active particles (b >= n_massive; n_massive = N in TP 0) carry the sign bit: see GENGA_BS_PAIR
+            const double gm = b >= n_massive ? -(G * mass[b]) : G * mass[b];
             for (int k = 0; k < nlevels; k++) rci[k] = rcrit[(long long)k * N + b];
             if (COOP) {
                 Gm.gm[i] = gm;
@@ -273,7 +283,7 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
         bool fail = false;
         while (done != dt) {                                           // all decisions below are group-uniform
             if ((dt > 0.0 && done + H > dt) || (dt < 0.0 && done + H < dt)) H = dt - done;
-            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, q, a0);
+            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, q, a0);
             int halvings = 0, kconv = 0;
             for (;;) {
                 bool ok = false;
@@ -285,14 +295,14 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
 #pragma unroll
                         for (int c = 0; c < 3; c++) { qm[c] = q[c]; vm[c] = v[c]; qn[c] = q[c] + h * v[c]; vn[c] = v[c] + h * a0[c]; }
                         for (int m = 1; m < nk; m++) {
-                            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
+                            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
 #pragma unroll
                             for (int c = 0; c < 3; c++) {
                                 const double qs = qm[c] + h2 * vn[c], vs = vm[c] + h2 * a[c];
                                 qm[c] = qn[c]; vm[c] = vn[c]; qn[c] = qs; vn[c] = vs;
                             }
                         }
-                        bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, mu, rci, qn, a);
+                        bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
 #pragma unroll
                         for (int c = 0; c < 3; c++) {
                             cq[c] = 0.5 * (qn[c] + qm[c] + h * vn[c]);

@@ -112,3 +112,53 @@ def test_reversibility_and_tolerance_scaling(bs):
     q0, v0, _ = bs.bs_group(pos, vel, m0, rc, G, 1.0, 6.0, 1e-13)
     qk, vk, _ = bs.bs_group(pos[:, :1], vel[:, :1], m0[:1], rc[:, :1], G, 1.0, 6.0, 1e-13)
     assert np.max(np.abs(q0[:, 0] - qk[:, 0])) < 1e-13
+
+
+# ------------------------------------------------------------------------------- test-particle modes in a group (sec. 8.1)
+def _tp_group(m_a=1e-9, m_b=1e-9, sep=1e-4):
+    """A massive body M on a Kepler orbit and two semi-active particles a, b next to it, `sep` apart from each other."""
+    pos, vel = gi.elements_to_cartesian(np.array([1.0]), np.array([0.05]), np.array([0.01]), np.zeros(1), np.zeros(1),
+                                        np.array([0.4]), G)
+    q = np.repeat(pos, 3, axis=1); v = np.repeat(vel, 3, axis=1)
+    q[:, 1] += (0.010, 0.002, 0.0005); q[:, 2] = q[:, 1] + (sep, 0.0, 0.0)
+    v[:, 1] += (0.0, 2e-5, 0.0); v[:, 2] += (0.0, 2e-5, 1e-6)
+    mass = np.array([1e-5, m_a, m_b])
+    rc = np.full((1, 3), 0.05)
+    return q, v, mass, rc
+
+
+def test_semi_active_particles_in_a_group(bs, oracle_mod):
+    """Fig. 14 inside the Bulirsch-Stoer phase.  TP 1: nobody feels a particle -- the massive body
+    stays on its Kepler orbit and each particle moves as in its own two-body group with it.  TP 2: a particle acts on
+    the massive body exactly as a fully interactive body does, and particles still do not feel each other."""
+    dt, tol = 1.0, 1e-13
+    q, v, mass, rc = _tp_group()
+    tp = np.array([False, True, True])
+    # --- TP 1
+    q1, v1, st = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol, is_tp=tp, tp_mode=1)
+    assert not st.failed
+    qk, vk, _ = oracle_mod.step.fg(q[:, :1], v[:, :1], G, dt)
+    assert np.abs(q1[:, 0] - qk[:, 0]).max() < 1e-13 and np.abs(v1[:, 0] - vk[:, 0]).max() < 1e-14
+    for p in (1, 2):
+        qs, vs, _ = bs.bs_group(q[:, [0, p]], v[:, [0, p]], mass[[0, p]], rc[:, [0, p]], G, 1.0, dt, tol,
+                                is_tp=np.array([False, True]), tp_mode=1)
+        assert np.abs(q1[:, p] - qs[:, 1]).max() < 1e-12 and np.abs(v1[:, p] - vs[:, 1]).max() < 1e-13
+    # the massive body does act on the particles: they leave their own Kepler orbits
+    qa, va, _ = oracle_mod.step.fg(q[:, 1:], v[:, 1:], G, dt)
+    assert np.abs(q1[:, 1:] - qa).max() > 1e-8
+    # --- TP 2 on a pair (massive, particle) = the fully interactive pair
+    q2, v2, _ = bs.bs_group(q[:, :2], v[:, :2], mass[:2], rc[:, :2], G, 1.0, dt, tol, is_tp=tp[:2], tp_mode=2)
+    qf, vf, _ = bs.bs_group(q[:, :2], v[:, :2], mass[:2], rc[:, :2], G, 1.0, dt, tol)
+    assert np.array_equal(q2, qf) and np.array_equal(v2, vf)
+    qh, vh, _ = bs.bs_group(q[:, :2], v[:, :2], np.array([1e-5, 1e-6]), rc[:, :2], G, 1.0, dt, tol, is_tp=tp[:2], tp_mode=2)
+    assert np.abs(qh[:, 0] - qk[:, 0]).max() > 1e-10                          # the particle moves the massive body
+    # --- particles never feel each other: what b does to a, fully interactive vs TP 2 (heavy particles, 1e-4 AU apart)
+    q, v, mass, rc = _tp_group(m_a=1e-7, m_b=1e-7)
+    alone, _, _ = bs.bs_group(q[:, :2], v[:, :2], mass[:2], rc[:, :2], G, 1.0, dt, tol)
+    full, _, _ = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol)
+    semi, _, _ = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol, is_tp=tp, tp_mode=2)
+    d_full = np.abs(full[:, 1] - alone[:, 1]).max(); d_semi = np.abs(semi[:, 1] - alone[:, 1]).max()
+    assert d_full > 1e-6 and d_semi < 1e-4 * d_full
+    # is_tp all False = fully interactive, bit for bit
+    same, _, _ = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol, is_tp=np.zeros(3, bool), tp_mode=2)
+    assert np.array_equal(same, full)

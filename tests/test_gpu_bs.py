@@ -190,3 +190,42 @@ def test_hybrid_step_keeps_the_energy_through_an_encounter():
     assert k.status() == 0 and enc > 3 and dmin < 5e-3
     assert worst < 1e-5
     k.free()
+
+
+@pytest.mark.parametrize("tp_mode", [1, 2])
+def test_semi_active_particles_in_groups(oracle_mod, tp_mode):
+    """Groups that mix massive bodies and semi-active particles WITH mass (sec. 8.1): particles feel
+    the massive bodies, act on them only in TP 2 and never feel each other -- bit for bit against the oracle's rule."""
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    rng = np.random.default_rng(17)
+    n_m, n_t = 40, 360
+    n = n_m + n_t
+    ki = gi.make_config(0, n=n)
+    pos, vel = ki.pos.copy(), ki.vel.copy()
+    # ten particles in a tight cloud around each of the first 36 massive bodies; one group per cloud
+    members, offsets = [], [0]
+    for g in range(36):
+        idx = np.arange(n_m + 10 * g, n_m + 10 * g + 10)
+        pos[:, idx] = pos[:, [g]] + rng.normal(scale=4e-3, size=(3, 10))
+        vel[:, idx] = vel[:, [g]] + rng.normal(scale=3e-5, size=(3, 10))
+        members += [g] + idx.tolist(); offsets.append(len(members))
+    mass = np.full(n, 2e-6); mass[n_m:] = rng.uniform(1e-8, 1e-7, n_t)
+    rc = np.full((2, n), 0.03); rc[1] = 0.012
+    k = GengaKick(n_m, n_t, G=G, pair_capacity=8, tp_mode=tp_mode)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    d_mem = _dev(np.asarray(members + [0] * (n - len(members)), np.int32))
+    d_off = torch.zeros(n + 4, dtype=torch.int32, device="cuda"); d_off[:len(offsets)] = _dev(np.asarray(offsets, np.int32))
+    d_sum = torch.tensor([36, len(members), 11, 0], dtype=torch.int32, device="cuda")
+    q, v = _dev(pos), _dev(vel)
+    k.bs(_dev(pos), _dev(vel), _dev(mass), _dev(rc), 2, 1.0, 3.0, 1e-12, d_mem, d_off, d_sum, q, v)
+    torch.cuda.synchronize()
+    assert k.status() == 0
+    k.free()
+    qw, vw, stats, _ = oracle_mod.bs.bs(pos, vel, mass, rc, np.asarray(members), np.asarray(offsets), G, 1.0, 3.0, 1e-12,
+                                        pos, vel, nlevels=2, n_massive=n_m, tp_mode=tp_mode)
+    print("identical:", _check(q.cpu().numpy(), v.cpu().numpy(), qw, vw))
+    # and the rule matters here: the fully interactive result is far away
+    qf, vf, _, _ = oracle_mod.bs.bs(pos, vel, mass, rc, np.asarray(members), np.asarray(offsets), G, 1.0, 3.0, 1e-12,
+                                    pos, vel, nlevels=2)
+    assert np.abs(qf - qw).max() > 1e-9

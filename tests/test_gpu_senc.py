@@ -282,3 +282,36 @@ def test_multilevel_step_full_size_config3(oracle_mod):
     print("per-level statistics identical:", bool(np.array_equal(gs, r.stats)), gs.tolist())
     _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0)
     k.free()
+
+
+@pytest.mark.parametrize("tp_mode,slevels", [(1, 2), (2, 3)])
+def test_multilevel_step_with_semi_active_particles(oracle_mod, tp_mode, slevels):
+    """A reduced config 4 (massive bodies + semi-active particles, sec. 8.1) through the multi-level
+    step: particles feel the massive bodies (TP 2: and act on them), never each other -- in the kicks of every level."""
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    ki = gi.make_config(4, n=400, n_test=6000)
+    mass = ki.mass.copy()
+    if tp_mode == 2:
+        mass[ki.n_massive:] = 1e-12
+    n, cap = ki.n, 1 << 16
+    k = GengaKick(ki.n_massive, ki.n_test, max_level=slevels - 1, G=ki.G, pair_capacity=cap, tp_mode=tp_mode)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, v, m = _dev(ki.pos), _dev(ki.vel), _dev(mass)
+    acc, pairs, npairs, stats = _ml_buffers(n, cap, slevels)
+    k.multilevel_step(q, v, m, 1.0, ki.dt, slevels, 2, 1e-12, acc, pairs, npairs, stats)
+    torch.cuda.synchronize()
+    assert k.status() == 0
+    r = _oracle_ml_tp(oracle_mod, ki, mass, slevels, tp_mode)
+    assert np.array_equal(stats.cpu().numpy(), r.stats), (stats.cpu().numpy().tolist(), r.stats.tolist())
+    assert r.stats[0, 1] > 20 and r.stats[-1, 2] > 5
+    c = npairs.cpu().numpy()
+    pr = pairs.cpu().numpy()[:c[n]]
+    assert (pr[:, 0] < ki.n_massive).all()                              # no particle-particle pairs
+    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0)
+    k.free()
+
+
+def _oracle_ml_tp(oracle_mod, ki, mass, slevels, tp_mode):
+    return oracle_mod.step.multilevel_step(ki.pos, ki.vel, mass, ki.n_massive, ki.n_test, 1.0, ki.G, ki.dt,
+                                           slevels=slevels, substeps=2, tol=1e-12, tp_mode=tp_mode)
