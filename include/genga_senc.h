@@ -39,6 +39,10 @@ int genga_detect(genga_kick_ctx* ctx, const double* pos0, const double* vel0, co
                  const double* rcrit_row, double enc_factor, double h, const int32_t* in_pairs,
                  const int32_t* in_n_pairs, int64_t in_pair_rows, int32_t* out_pairs, int32_t* out_npairs);
 
+#define GENGA_KICK_STATUS_LIST_CLIPPED 128   /* genga_multilevel_step: a candidate or close-encounter list was longer than
+                                               the context's pair_capacity; the rows beyond it were not seen by the
+                                               levels below -- repeat the step with a larger capacity               */
+
 typedef struct {
     int32_t slevels;    /* number of symplectic levels, 1 .. 4 (1: the original hybrid scheme; the context needs
                            max_level >= slevels - 1)                                                              */
@@ -72,6 +76,7 @@ typedef struct {
  *
  *   pos, vel     [3][N] advanced in place               mass [N]
  *   out_pairs / out_npairs   the candidates of the first kick, as genga_kick writes them
+ *   A list longer than pair_capacity is clipped (as genga_kick does) and GENGA_KICK_STATUS_LIST_CLIPPED is set.
  *   out_stats    [slevels][4] int32 or NULL: per level, summed over its sub-steps: candidate pairs,
  *                close-encounter pairs, groups handed to Bulirsch-Stoer, bodies in them
  *   out_acc      [3][N] acceleration of the closing kick, or NULL

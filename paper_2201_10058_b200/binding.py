@@ -32,6 +32,7 @@ STATUS_GROUP_TOO_LARGE, STATUS_BS_NOT_CONVERGED = 32, 64
 STATUS_UNBOUND = 8
 # include/genga_senc.h: close-encounter detection and the multi-level step (SEnc)
 SENC_EXPORTS = ("genga_detect", "genga_multilevel_step")
+STATUS_LIST_CLIPPED = 128
 
 
 class GengaKickConfig(C.Structure):

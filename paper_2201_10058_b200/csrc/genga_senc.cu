@@ -85,12 +85,11 @@ int encounters(Senc& s, int level, double h, const int32_t** enc, const int32_t*
     }
     rc = genga_group(s.ctx, *enc, *n_enc, s.cap, L.group_of, L.members, L.offsets, L.summary);
     if (rc != GENGA_KICK_OK) return rc;
-    if (s.stats) {
-        genga::senc_stats_kernel<<<1, 32, 0, s.ctx->stream>>>(s.stats + 4 * level, L.cand_np + s.N, *n_enc, L.summary,
-                                                             level == s.cfg->slevels - 1 ? 1 : 0);
-        GK_CUDA(s.ctx, cudaGetLastError());
-        s.ctx->launches++;
-    }
+    genga::senc_stats_kernel<<<1, 32, 0, s.ctx->stream>>>(s.stats ? s.stats + 4 * level : nullptr, L.cand_np + s.N, *n_enc,
+                                                         L.summary, level == s.cfg->slevels - 1 ? 1 : 0, s.cap,
+                                                         s.ctx->status);
+    GK_CUDA(s.ctx, cudaGetLastError());
+    s.ctx->launches++;
     return GENGA_KICK_OK;
 }
 

@@ -8,6 +8,7 @@
 
 #define GENGA_SENC_THREADS 256
 #define GENGA_STATUS_BAD_DETECT_PAIR 16      // = GENGA_KICK_STATUS_BAD_PAIR
+#define GENGA_STATUS_LIST_CLIPPED 128        // = GENGA_KICK_STATUS_LIST_CLIPPED
 
 namespace genga {
 
@@ -107,12 +108,16 @@ copy_list_kernel(double* __restrict__ dst_pos, double* __restrict__ dst_vel, con
 // per-level statistics of one sub-step: candidates, close-encounter pairs, and (deepest level) groups / bodies of the
 // Bulirsch-Stoer phase
 __global__ void senc_stats_kernel(int* __restrict__ stats, const int* __restrict__ n_cand, const int* __restrict__ n_enc,
-                                  const int* __restrict__ summary, int bs_level)
+                                  const int* __restrict__ summary, int bs_level, long long cap, int* __restrict__ status)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
-        stats[0] += *n_cand;
-        stats[1] += *n_enc;
-        if (bs_level) { stats[2] += summary[0]; stats[3] += summary[1]; }
+        // a list longer than the pair capacity was clipped: the levels below saw only part of the encounters
+        if (*n_cand > cap || *n_enc > cap) atomicOr(status, GENGA_STATUS_LIST_CLIPPED);
+        if (stats) {
+            stats[0] += *n_cand;
+            stats[1] += *n_enc;
+            if (bs_level) { stats[2] += summary[0]; stats[3] += summary[1]; }
+        }
     }
 }
 

@@ -237,6 +237,22 @@ def test_multilevel_step_keeps_the_energy_through_an_encounter():
     k.free()
 
 
+def test_multilevel_step_reports_a_clipped_list():
+    import torch
+    from paper_2201_10058_b200 import GengaKick, binding as g
+    ki = gi.make_config(0, n=3000)
+    n, cap = ki.n, 64                                                # the disk has ~500 level-0 encounter pairs
+    k = GengaKick(n, 0, max_level=1, G=ki.G, pair_capacity=cap)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, v, mass = _dev(ki.pos), _dev(ki.vel), _dev(ki.mass)
+    acc, pairs, npairs, stats = _ml_buffers(n, cap, 2)
+    k.multilevel_step(q, v, mass, 1.0, ki.dt, 2, 2, 1e-12, acc, pairs, npairs, stats)
+    torch.cuda.synchronize()
+    assert int(npairs[n]) > cap and k.status() == g.STATUS_LIST_CLIPPED
+    assert torch.isfinite(q).all() and torch.isfinite(v).all()
+    k.free()
+
+
 def test_multilevel_step_error_codes():
     import torch
     from paper_2201_10058_b200 import GengaKick, binding as g
