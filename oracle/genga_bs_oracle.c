@@ -30,8 +30,12 @@
  *     accept T_kk as soon as err <= tol; if k = 8 is not enough, halve H and start the macro step again
  *   - after an accepted macro step: H <- 2 H if it converged with k <= 5, else H; never beyond the end of dt.
  *     The first macro step tries the whole dt.
- * All arithmetic in IEEE binary64 in the order written (compile with -ffp-contract=off); the force sum runs
- * over the group's members in list order.
+ * All arithmetic in IEEE binary64 in the order written (compile with -ffp-contract=off).  Order of the force sum
+ * ("parallel reductions have a well-defined order"), part of reading G15:
+ *   groups of up to 256 bodies: Sun term, then the pair terms added one by one in member order j = 0 .. n-1;
+ *   larger groups (the paper's multi-block regime BS-M, where the sum is spread over threads):
+ *   eight partial sums p_s = sum of the terms with j = s (mod 8), each in ascending j from 0, combined as
+ *   ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) and added to the Sun term.
  *
  * PINS (tests/test_bs_oracle_pins.py): two bodies far outside each other's critical radius (W_BS = 0):
  * each follows its Kepler orbit -- against the closed-form FG oracle; two bodies deep inside (K = 0): the
@@ -46,6 +50,7 @@
 
 #define BS_KMAX 8
 #define BS_MAX_HALVINGS 60
+#define BS_SEQ_MAX 256      /* largest group whose force sum is sequential */
 
 extern double genga_oracle_K(double r, double rc);
 
@@ -68,6 +73,8 @@ static void bs_accel(const bs_group *g, const double *q, double *a)
         const double rs = sqrt(r2s);
         const double s0 = -g->mu / (r2s * rs);
         double ax = s0 * x, ay = s0 * y, az = s0 * z;
+        double p[8][3] = {{0.0}};
+        const int tree = n > BS_SEQ_MAX;
         for (int j = 0; j < n; j++) {
             if (j == i) continue;
             if (g->is_tp && g->is_tp[j] && (g->tp_mode != 2 || g->is_tp[i])) continue;      /* Fig. 14 */
@@ -81,8 +88,15 @@ static void bs_accel(const bs_group *g, const double *q, double *a)
             }
             if (W != 0.0) {
                 const double s = g->G * g->m[j] * W / (r2 * r);
-                ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;
+                if (tree) { double *ps = p[j & 7]; ps[0] = ps[0] + s * dx; ps[1] = ps[1] + s * dy; ps[2] = ps[2] + s * dz; }
+                else { ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz; }
             }
+        }
+        if (tree) {
+            double t[3];
+            for (int c = 0; c < 3; c++)
+                t[c] = ((p[0][c] + p[1][c]) + (p[2][c] + p[3][c])) + ((p[4][c] + p[5][c]) + (p[6][c] + p[7][c]));
+            ax = ax + t[0]; ay = ay + t[1]; az = az + t[2];
         }
         a[3 * i] = ax; a[3 * i + 1] = ay; a[3 * i + 2] = az;
     }

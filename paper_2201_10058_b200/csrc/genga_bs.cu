@@ -50,23 +50,37 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     // one warp per group of up to 32 bodies (nearly all groups), eight groups per CTA
     const int wblocks = (int)std::min<long long>(std::max<long long>((N / 2 + 7) / 8, 1), 8LL * ctx->num_sms);
     genga::bs_kernel<GENGA_BS_MODE_WARP, GENGA_BS_THREADS><<<wblocks, GENGA_BS_THREADS, 0, st>>>(
-        pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode);
+        pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode, -1);
     // one CTA per group of 33 .. 256 bodies
     if (N > GENGA_BS_WARP_MAX) {
         const int blocks = (int)std::min<long long>(std::max<long long>(N / (GENGA_BS_WARP_MAX + 1), 1), 16LL * ctx->num_sms);
         genga::bs_kernel<GENGA_BS_MODE_CTA, GENGA_BS_THREADS><<<blocks, GENGA_BS_THREADS, 0, st>>>(
-            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode);
+            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode, -1);
         ctx->launches++;
     }
     GK_CUDA(ctx, cudaGetLastError());
-    // the whole grid, one large group after the other (returns at once if there is none)
+    // the whole-grid regime, one large group after the other (returns at once if there is none): first a grid of one
+    // CTA per SM for the groups it can hold (its grid barrier costs a fraction of the full grid's), then the full
+    // co-resident grid for the larger ones
     if (N > GENGA_BS_THREADS) {
         GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
+        const int cap1 = ctx->num_sms * GENGA_BS_COOP_THREADS / GENGA_BS_SUB;
+        const bool two = N > cap1 && ctx->bs_coop_blocks > ctx->num_sms;
+        int big_max = two ? cap1 : -1;
         void* args[] = {&pos_in, &vel_in, &mass, &rcrit, &NN, &nlevels, const_cast<double*>(&G), const_cast<double*>(&mu), &dt,
-                        &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max, &n_massive, &tp_mode};
+                        &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max, &n_massive, &tp_mode, &big_max};
         GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>),
-                                                 dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
+                                                 dim3(two ? ctx->num_sms : ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0,
+                                                 st));
         ctx->launches++;
+        if (two) {
+            small_max = cap1;
+            big_max = -1;
+            GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
+            GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>),
+                                                     dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
+            ctx->launches++;
+        }
     }
     GK_CUDA(ctx, cudaGetLastError());
     ctx->launches++;

@@ -33,6 +33,7 @@ namespace genga {
 #define GENGA_BS_WARP_MAX 32            // largest group of the warp-per-group regime
 #define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
 #define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
+#define GENGA_BS_SUB 8                  // whole-grid regime: lanes per body, each summing the terms with j = lane (mod 8)
 #define GENGA_BS_TILE 64                // j-bodies staged per round in the whole-grid regime
 #define GENGA_BS_KMAX 8
 #define GENGA_BS_MAX_LEVELS 4
@@ -122,12 +123,17 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 #undef GENGA_BS_RCJ
         }
     } else {
+        // GENGA_BS_SUB lanes per body: lane `sub` sums the terms with j = sub (mod 8) in ascending j from 0, the eight
+        // partial sums are combined as ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) (xor butterfly: IEEE addition
+        // commutes, so every lane of the octet gets the same bits) and added to the Sun term
         const int p = eval & 1;
         eval++;
-        if (i < n) { Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z; }
+        const int t = threadIdx.x, sub = t & (GENGA_BS_SUB - 1);
+        if (i < n && sub == 0) { Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z; }
         cooperative_groups::this_grid().sync();
-        const int t = threadIdx.x;
-        for (int j0 = 0; j0 < n; j0 += ROWS) {                // tiles in ascending order: the sum runs over j = 0 .. n-1
+        const double sx = ax, sy = ay, sz = az;
+        ax = 0.0; ay = 0.0; az = 0.0;
+        for (int j0 = 0; j0 < n; j0 += ROWS) {                // ROWS is a multiple of 8: (j0 + jj) mod 8 = jj mod 8
             __syncthreads();
             if (t < ROWS && j0 + t < n) {
                 S.x[t] = __ldcg(Gm.x[p] + j0 + t); S.y[t] = __ldcg(Gm.y[p] + j0 + t); S.z[t] = __ldcg(Gm.z[p] + j0 + t);
@@ -138,13 +144,20 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             if (i < n) {
                 const int m = min(ROWS, n - j0);
 #define GENGA_BS_RCJ(k) S.rc[k][jj]
-                for (int jj = 0; jj < m; jj++) {
+                for (int jj = sub; jj < m; jj += GENGA_BS_SUB) {
                     if (j0 + jj == i) continue;
                     GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
                 }
 #undef GENGA_BS_RCJ
             }
         }
+#pragma unroll
+        for (int o = 1; o < GENGA_BS_SUB; o <<= 1) {
+            ax = ax + __shfl_xor_sync(0xffffffffu, ax, o);
+            ay = ay + __shfl_xor_sync(0xffffffffu, ay, o);
+            az = az + __shfl_xor_sync(0xffffffffu, az, o);
+        }
+        ax = sx + ax; ay = sy + ay; az = sz + az;
     }
     a[0] = ax; a[1] = ay; a[2] = az;
 }
@@ -214,15 +227,17 @@ __device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, i
 
 // WARP: warp w, w + (warps of the grid), ... integrates group w if it has at most 32 bodies.
 // CTA : CTA g, g + gridDim.x, ... integrates group g if it has 33 .. THREADS bodies.
-// COOP: the whole grid integrates, one after the other, the groups with more than `small_max` bodies;
-//       groups larger than the grid are reported and left as they are.
+// COOP: the whole grid integrates, one after the other, the groups with more than `small_max` and at most `big_max`
+//       bodies (two launches: a grid of one CTA per SM, whose barrier is cheap, for groups it can hold, and the full
+//       co-resident grid for the rest); groups larger than the grid of a launch with big_max < 0 are reported and
+//       left as they are.
 template <int MODE, int THREADS>
 __global__ void __launch_bounds__(THREADS)
 bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
           double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max,
-          long long n_massive, int tp_mode)
+          long long n_massive, int tp_mode, int big_max)
 {
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP, WARP = MODE == GENGA_BS_MODE_WARP;
     constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : THREADS);
@@ -230,8 +245,11 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
     __shared__ BsShared<ROWS> Sall[UNITS];
     BsShared<ROWS>& S = Sall[WARP ? threadIdx.x >> 5 : 0];
     const int t = WARP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
-    const int i = COOP ? (int)(blockIdx.x * THREADS + t) : t;           // this thread's body within the group
-    const long long capacity = COOP ? (long long)gridDim.x * THREADS : ROWS;
+    // this thread's body within the group (whole-grid regime: GENGA_BS_SUB consecutive lanes share a body and carry
+    // identical copies of its state; they differ only in the part of the force sum they evaluate)
+    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / GENGA_BS_SUB) : t;
+    const bool writer = !COOP || (t & (GENGA_BS_SUB - 1)) == 0;
+    const long long capacity = COOP ? (long long)gridDim.x * THREADS / GENGA_BS_SUB : ROWS;
     const int n_groups = summary[0];
     int eval = 0, echeck = 0;
     const int g0 = COOP ? 0 : (WARP ? (int)(blockIdx.x * UNITS + (threadIdx.x >> 5)) : (int)blockIdx.x);
@@ -251,7 +269,8 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
         } else if (g >= n_groups) break;
         const int first = offsets[g], n = offsets[g + 1] - first;
         // the other regimes' groups (grid- / CTA- / warp-uniform)
-        if (COOP ? n <= small_max : (WARP ? n > GENGA_BS_WARP_MAX : (n > THREADS || n <= GENGA_BS_WARP_MAX))) continue;
+        if (COOP ? (n <= small_max || (big_max >= 0 && n > big_max))
+                 : (WARP ? n > GENGA_BS_WARP_MAX : (n > THREADS || n <= GENGA_BS_WARP_MAX))) continue;
         if (n > capacity) {
             if (t == 0 && blockIdx.x == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
             continue;
@@ -268,8 +287,10 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
             const double gm = b >= n_massive ? -(G * mass[b]) : G * mass[b];
             for (int k = 0; k < nlevels; k++) rci[k] = rcrit[(long long)k * N + b];
             if (COOP) {
-                Gm.gm[i] = gm;
-                for (int k = 0; k < nlevels; k++) Gm.rc[k][i] = rci[k];
+                if (writer) {
+                    Gm.gm[i] = gm;
+                    for (int k = 0; k < nlevels; k++) Gm.rc[k][i] = rci[k];
+                }
             } else {
                 S.gm[i] = gm;
                 for (int k = 0; k < nlevels; k++) S.rc[k][i] = rci[k];
@@ -350,7 +371,7 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
             if (kconv <= 5) H = 2.0 * H;
         }
         if (fail && t == 0 && blockIdx.x == (COOP ? 0 : blockIdx.x)) atomicOr(status, GENGA_STATUS_BS_NOT_CONVERGED);
-        if (active) {                                                  // (after a failure: the state at the last accepted time)
+        if (active && writer) {                                        // (after a failure: the state at the last accepted time)
 #pragma unroll
             for (int c = 0; c < 3; c++) { pos[c * N + b] = q[c]; vel[c * N + b] = v[c]; }
         }

@@ -162,3 +162,35 @@ def test_semi_active_particles_in_a_group(bs, oracle_mod):
     # is_tp all False = fully interactive, bit for bit
     same, _, _ = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol, is_tp=np.zeros(3, bool), tp_mode=2)
     assert np.array_equal(same, full)
+
+
+def test_large_group_tree_ordered_force_sum(bs):
+    """Groups above 256 bodies sum the pair terms in eight interleaved partial sums (the order fixed in the oracle's
+    header).  What the mathematics fixes: the result does not depend on the order beyond rounding (a permutation of
+    the members changes every partial sum), and a group deep inside every critical radius (K = 0, W_BS = 1) conserves
+    the Newtonian energy of Sun (fixed) + bodies to the tolerance."""
+    n = 320
+    rng = np.random.default_rng(23)
+    ang = 2 * np.pi * np.arange(n) / n
+    pos = np.stack([np.cos(ang), np.sin(ang), 1e-3 * rng.normal(size=n)])
+    vk = np.sqrt(G)
+    vel = np.stack([-vk * np.sin(ang), vk * np.cos(ang), np.zeros(n)]) * (1 + 1e-3 * rng.normal(size=n))
+    mass = np.full(n, 1e-7)
+    rc = np.full((1, n), 50.0)                    # every pair is inside 0.1 r_crit: K = 0
+
+    def energy(q, v):
+        e = 0.5 * (mass * (v * v).sum(0)).sum() - (G * mass / np.sqrt((q * q).sum(0))).sum()
+        for i in range(n):
+            d = np.sqrt(((q[:, i + 1:] - q[:, i:i + 1]) ** 2).sum(0))
+            e -= (G * mass[i] * mass[i + 1:] / d).sum()
+        return e
+
+    q1, v1, st = bs.bs_group(pos, vel, mass, rc, G, 1.0, 20.0, 1e-12)
+    assert not st.failed and abs(energy(q1, v1) / energy(pos, vel) - 1) < 1e-11
+    perm = rng.permutation(n)
+    q2, v2, _ = bs.bs_group(pos[:, perm], vel[:, perm], mass[perm], rc[:, perm], G, 1.0, 20.0, 1e-12)
+    assert np.abs(q2 - q1[:, perm]).max() < 1e-11 and np.abs(v2 - v1[:, perm]).max() < 1e-12
+    assert not np.array_equal(q2, q1[:, perm])                    # (the order does enter the rounding)
+    # the bodies do feel each other: without the pair terms (W_BS = 0) the result differs visibly
+    q3, _, _ = bs.bs_group(pos, vel, mass, np.full((1, n), 1e-9), G, 1.0, 20.0, 1e-12)
+    assert np.abs(q3 - q1).max() > 1e-8
