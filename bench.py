@@ -326,7 +326,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                  "listed_pairs": int(npairs[n].item()), "level1_pairs": int(npairs1[n].item())}
 
     # NEXT-4: the complete hybrid step with the Bulirsch-Stoer branch, on BASELINE.json configs[1] (N = 8192; at
-    # N = 65,536 the level-0 pairs link into one group of 33,297 bodies, beyond the 256-body regime built here)
+    # N = 65,536 the level-0 pairs link into one group of 33,297 bodies -- the case the multi-level step below exists for)
     k1 = gi.make_config(1)
     n1 = k1.n
     kick1 = GengaKick(n1, 0, max_level=0, pair_capacity=1 << 18, G=k1.G, device=local_rank)
@@ -356,7 +356,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
 
     # NEXT-4: the multi-level step (SEnc recursion, App. A) -- the experiment of Fig. 10
     # (PAPER.md:640): the same disks, the hybrid step against 2-4 symplectic levels
-    def time_multilevel(kin, slevels, substeps, reps):
+    def time_multilevel(kin, slevels, substeps, reps, graph=False):
         nn = kin.n
         km = GengaKick(nn, 0, max_level=slevels - 1, pair_capacity=PAIR_CAPACITY, G=kin.G, device=local_rank)
         km.set_stream(stream.cuda_stream)
@@ -378,7 +378,34 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             if it >= 2:
                 ts.append(a.elapsed_time(b))
         st = mst.cpu().tolist()
+        # the same launch sequence captured once in a CUDA graph and replayed (no host launch cost, fixed sequence)
+        graph_ms = None
+        if graph:
+            gs = torch.cuda.Stream()                       # capture needs a non-default stream
+            q.copy_(q0); v.copy_(v0)
+            torch.cuda.synchronize()
+            km.set_stream(gs.cuda_stream)
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=gs):
+                km.multilevel_step(q, v, mm, 1.0, kin.dt, slevels, substeps, 1e-12, macc, mp, mnp, mst, detect=True)
+            gts = []
+            with torch.cuda.stream(gs):
+                for it in range(reps + 2):
+                    q.copy_(q0); v.copy_(v0)
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(gs)
+                    g.replay()
+                    b.record(gs)
+                    b.synchronize()
+                    if it >= 2:
+                        gts.append(a.elapsed_time(b))
+            torch.cuda.synchronize()
+            km.set_stream(stream.cuda_stream)
+            graph_ms = float(np.median(gts))
+            assert mst.cpu().tolist() == st, "the replayed graph took other decisions than the plain launches"
+            del g
         out = {"slevels": slevels, "substeps": substeps, "ms_per_step": float(np.median(ts)), "launches_per_step": int(nl),
+               "ms_per_step_cuda_graph": graph_ms,
                "encounter_pairs_per_level": [r[1] for r in st], "bs_groups": st[-1][2], "bs_bodies": st[-1][3],
                "status": km.status()}
         km.free()
@@ -387,8 +414,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     multilevel_info = {"what": "genga_multilevel_step (Rcrit, Kick + pre-check, HC, FG, detection, SEnc over KickS / RcritS / "
                                "FGS / detection / grouping / Bulirsch-Stoer tol 1e-12, HC, Kick), one step from the "
                                "generated state; 1 level = the hybrid step",
-                       "configs[1] N=8192": [time_multilevel(k1, sl, ss, 5) for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10))],
-                       "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3) for sl, ss in ((2, 10), (4, 2), (3, 4))]}
+                       "configs[1] N=8192": [time_multilevel(k1, sl, ss, 5, graph=(sl, ss) == (2, 2))
+                                             for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10))],
+                       "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3, graph=(sl, ss) == (2, 10))
+                                              for sl, ss in ((2, 10), (4, 2), (3, 4))]}
 
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
