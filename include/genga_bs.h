@@ -22,8 +22,9 @@
  * groups side by side.  Larger groups: one group at a time
  * over a whole co-resident grid with a grid-wide barrier per force evaluation (the paper's BS-M regime,
  * PAPER.md:595-597, with the sub-steps kept on the device instead of controlled from the host); a group larger
- * than that grid (8 lanes per body, each summing an eighth of the pair terms: 64 threads x resident CTAs / 8, about
- * 11,800 bodies on a B200) keeps the state already in pos / vel
+ * than that grid keeps the state already in pos / vel (8 lanes per body, each summing an eighth of the pair terms, up
+ * to 64 threads x resident CTAs / 8 = about 11,800 bodies on a B200; beyond that one lane per body evaluating the same
+ * eight partial sums, up to about 75,000 bodies)
  * and GENGA_KICK_STATUS_GROUP_TOO_LARGE is set.
  *
  * Works on the context of genga_kick.h (its N, G, stream); only enqueues; all pointers are DEVICE pointers.

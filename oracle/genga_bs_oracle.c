@@ -64,17 +64,18 @@ typedef struct {
 } bs_group;
 
 /* f: accelerations of all bodies of the group at positions q [n][3] */
-static void bs_accel(const bs_group *g, const double *q, double *a)
+static inline void bs_accel_body(const bs_group *g, const double *q, double *a, int i)
 {
     const int n = g->n;
-    for (int i = 0; i < n; i++) {
+    {
         const double x = q[3 * i], y = q[3 * i + 1], z = q[3 * i + 2];
         const double r2s = x * x + y * y + z * z;
         const double rs = sqrt(r2s);
         const double s0 = -g->mu / (r2s * rs);
         double ax = s0 * x, ay = s0 * y, az = s0 * z;
-        double p[8][3] = {{0.0}};
         const int tree = n > BS_SEQ_MAX;
+        double p[8][3];
+        if (tree) for (int s8 = 0; s8 < 8; s8++) p[s8][0] = p[s8][1] = p[s8][2] = 0.0;
         for (int j = 0; j < n; j++) {
             if (j == i) continue;
             if (g->is_tp && g->is_tp[j] && (g->tp_mode != 2 || g->is_tp[i])) continue;      /* Fig. 14 */
@@ -99,6 +100,17 @@ static void bs_accel(const bs_group *g, const double *q, double *a)
             ax = ax + t[0]; ay = ay + t[1]; az = az + t[2];
         }
         a[3 * i] = ax; a[3 * i + 1] = ay; a[3 * i + 2] = az;
+    }
+}
+
+static void bs_accel(const bs_group *g, const double *q, double *a)
+{
+    const int n = g->n;
+    if (n > 2048) {         /* bodies are independent of each other here: the threads only share read-only data */
+#pragma omp parallel for schedule(static)
+        for (int i = 0; i < n; i++) bs_accel_body(g, q, a, i);
+    } else {
+        for (int i = 0; i < n; i++) bs_accel_body(g, q, a, i);
     }
 }
 

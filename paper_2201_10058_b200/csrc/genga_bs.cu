@@ -32,10 +32,14 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     if (!ctx->bs_scratch) {
         GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double)));
         int per_sm = 0;
-        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>,
+        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>,
                                                                  GENGA_BS_COOP_THREADS, 0));
         if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
         ctx->bs_coop_blocks = per_sm * ctx->num_sms;
+        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                         &per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 1>, GENGA_BS_COOP_THREADS, 0));
+        if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
+        ctx->bs_coop_blocks1 = per_sm * ctx->num_sms;
     }
     genga::BsGlobal gm;
     {
@@ -69,17 +73,29 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
         int big_max = two ? cap1 : -1;
         void* args[] = {&pos_in, &vel_in, &mass, &rcrit, &NN, &nlevels, const_cast<double*>(&G), const_cast<double*>(&mu), &dt,
                         &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max, &n_massive, &tp_mode, &big_max};
-        GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>),
+        GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>),
                                                  dim3(two ? ctx->num_sms : ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0,
                                                  st));
         ctx->launches++;
         if (two) {
+            // ... the full grid with eight lanes per body, and with one lane per body for the groups beyond that
+            const int cap2 = (int)std::min<long long>((long long)ctx->bs_coop_blocks * GENGA_BS_COOP_THREADS / GENGA_BS_SUB, N);
+            const bool three = N > cap2;
             small_max = cap1;
-            big_max = -1;
+            big_max = three ? cap2 : -1;
             GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
-            GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS>),
+            GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>),
                                                      dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
             ctx->launches++;
+            if (three) {
+                small_max = cap2;
+                big_max = -1;
+                GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
+                GK_CUDA(ctx, cudaLaunchCooperativeKernel(
+                                 reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 1>),
+                                 dim3(ctx->bs_coop_blocks1), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
+                ctx->launches++;
+            }
         }
     }
     GK_CUDA(ctx, cudaGetLastError());

@@ -34,6 +34,7 @@ namespace genga {
 #define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
 #define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
 #define GENGA_BS_SUB 8                  // whole-grid regime: lanes per body, each summing the terms with j = lane (mod 8)
+                                        // (groups too large for that: one lane per body, the same eight partial sums)
 #define GENGA_BS_TILE 64                // j-bodies staged per round in the whole-grid regime
 #define GENGA_BS_KMAX 8
 #define GENGA_BS_MAX_LEVELS 4
@@ -72,7 +73,8 @@ struct BsShared {
 // one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3.
 // Test-particle modes (sec. 8.1, Fig. 14): a semi-active particle j is staged with the SIGN BIT of
 // G m_j set; it acts on nobody in TP 1 and on the massive bodies only in TP 2 (particles never feel each other).
-#define GENGA_BS_PAIR(XJ, YJ, ZJ, GMJ, RCJ)                                                            \
+#define GENGA_BS_PAIR(XJ, YJ, ZJ, GMJ, RCJ) GENGA_BS_PAIR_ACC(XJ, YJ, ZJ, GMJ, RCJ, ax, ay, az)
+#define GENGA_BS_PAIR_ACC(XJ, YJ, ZJ, GMJ, RCJ, AX, AY, AZ)                                            \
     {                                                                                                  \
         double gmj = (GMJ);                                                                            \
         bool skip = false;                                                                             \
@@ -85,7 +87,7 @@ struct BsShared {
             for (int k = 0; k < nlevels; k++) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));              \
             if (W != 0.0) {                                                                            \
                 const double s = gmj * W / (r2 * r);                                                   \
-                ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;                                  \
+                AX = AX + s * dx; AY = AY + s * dy; AZ = AZ + s * dz;                                  \
             }                                                                                          \
         }                                                                                              \
     }
@@ -99,7 +101,7 @@ __device__ __forceinline__ void bs_sync()
     if (MODE == GENGA_BS_MODE_WARP) __syncwarp(); else __syncthreads();
 }
 
-template <int MODE, int ROWS>
+template <int MODE, int ROWS, int SUB>
 __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, int nlevels,
                                          bool i_tp, int tp_mode, double mu, const double (&rci)[GENGA_BS_MAX_LEVELS], const double (&q)[3],
                                          double (&a)[3])
@@ -123,16 +125,20 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 #undef GENGA_BS_RCJ
         }
     } else {
-        // GENGA_BS_SUB lanes per body: lane `sub` sums the terms with j = sub (mod 8) in ascending j from 0, the eight
-        // partial sums are combined as ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) (xor butterfly: IEEE addition
-        // commutes, so every lane of the octet gets the same bits) and added to the Sun term
+        // The pair terms with j = s (mod 8) are summed in ascending j from 0 into p_s, s = 0 .. 7; the eight partial
+        // sums are combined as ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) and added to the Sun term.
+        //   SUB = 8: eight lanes per body, lane `sub` holds p_sub, xor butterfly (IEEE addition commutes, so every
+        //            lane of the octet gets the same bits);
+        //   SUB = 1: one lane per body holds all eight (groups too large for eight lanes each) -- same arithmetic.
         const int p = eval & 1;
         eval++;
-        const int t = threadIdx.x, sub = t & (GENGA_BS_SUB - 1);
+        const int t = threadIdx.x, sub = t & (SUB - 1);
         if (i < n && sub == 0) { Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z; }
         cooperative_groups::this_grid().sync();
         const double sx = ax, sy = ay, sz = az;
-        ax = 0.0; ay = 0.0; az = 0.0;
+        double px[8 / SUB], py[8 / SUB], pz[8 / SUB];
+#pragma unroll
+        for (int u = 0; u < 8 / SUB; u++) { px[u] = 0.0; py[u] = 0.0; pz[u] = 0.0; }
         for (int j0 = 0; j0 < n; j0 += ROWS) {                // ROWS is a multiple of 8: (j0 + jj) mod 8 = jj mod 8
             __syncthreads();
             if (t < ROWS && j0 + t < n) {
@@ -144,18 +150,33 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             if (i < n) {
                 const int m = min(ROWS, n - j0);
 #define GENGA_BS_RCJ(k) S.rc[k][jj]
-                for (int jj = sub; jj < m; jj += GENGA_BS_SUB) {
-                    if (j0 + jj == i) continue;
-                    GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
+                for (int j8 = 0; j8 < m; j8 += 8) {
+#pragma unroll
+                    for (int u = 0; u < 8 / SUB; u++) {
+                        const int jj = j8 + sub + u;          // SUB = 8: u = 0, jj = j8 + sub;  SUB = 1: jj = j8 + u
+                        if (jj < m && j0 + jj != i) {
+                            GENGA_BS_PAIR_ACC(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ, px[u], py[u], pz[u])
+                        }
+                    }
                 }
 #undef GENGA_BS_RCJ
             }
         }
+        if (SUB == 8) {
+            ax = px[0]; ay = py[0]; az = pz[0];
 #pragma unroll
-        for (int o = 1; o < GENGA_BS_SUB; o <<= 1) {
-            ax = ax + __shfl_xor_sync(0xffffffffu, ax, o);
-            ay = ay + __shfl_xor_sync(0xffffffffu, ay, o);
-            az = az + __shfl_xor_sync(0xffffffffu, az, o);
+            for (int o = 1; o < 8; o <<= 1) {
+                ax = ax + __shfl_xor_sync(0xffffffffu, ax, o);
+                ay = ay + __shfl_xor_sync(0xffffffffu, ay, o);
+                az = az + __shfl_xor_sync(0xffffffffu, az, o);
+            }
+        } else {
+            ax = ((px[0] + px[1 % (8 / SUB)]) + (px[2 % (8 / SUB)] + px[3 % (8 / SUB)])) +
+                 ((px[4 % (8 / SUB)] + px[5 % (8 / SUB)]) + (px[6 % (8 / SUB)] + px[7 % (8 / SUB)]));
+            ay = ((py[0] + py[1 % (8 / SUB)]) + (py[2 % (8 / SUB)] + py[3 % (8 / SUB)])) +
+                 ((py[4 % (8 / SUB)] + py[5 % (8 / SUB)]) + (py[6 % (8 / SUB)] + py[7 % (8 / SUB)]));
+            az = ((pz[0] + pz[1 % (8 / SUB)]) + (pz[2 % (8 / SUB)] + pz[3 % (8 / SUB)])) +
+                 ((pz[4 % (8 / SUB)] + pz[5 % (8 / SUB)]) + (pz[6 % (8 / SUB)] + pz[7 % (8 / SUB)]));
         }
         ax = sx + ax; ay = sy + ay; az = sz + az;
     }
@@ -231,7 +252,7 @@ __device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, i
 //       bodies (two launches: a grid of one CTA per SM, whose barrier is cheap, for groups it can hold, and the full
 //       co-resident grid for the rest); groups larger than the grid of a launch with big_max < 0 are reported and
 //       left as they are.
-template <int MODE, int THREADS>
+template <int MODE, int THREADS, int SUB = 1>
 __global__ void __launch_bounds__(THREADS)
 bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
@@ -247,9 +268,9 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
     const int t = WARP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
     // this thread's body within the group (whole-grid regime: GENGA_BS_SUB consecutive lanes share a body and carry
     // identical copies of its state; they differ only in the part of the force sum they evaluate)
-    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / GENGA_BS_SUB) : t;
-    const bool writer = !COOP || (t & (GENGA_BS_SUB - 1)) == 0;
-    const long long capacity = COOP ? (long long)gridDim.x * THREADS / GENGA_BS_SUB : ROWS;
+    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / SUB) : t;
+    const bool writer = !COOP || (t & (SUB - 1)) == 0;
+    const long long capacity = COOP ? (long long)gridDim.x * THREADS / SUB : ROWS;
     const int n_groups = summary[0];
     int eval = 0, echeck = 0;
     const int g0 = COOP ? 0 : (WARP ? (int)(blockIdx.x * UNITS + (threadIdx.x >> 5)) : (int)blockIdx.x);
@@ -304,7 +325,7 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
         bool fail = false;
         while (done != dt) {                                           // all decisions below are group-uniform
             if ((dt > 0.0 && done + H > dt) || (dt < 0.0 && done + H < dt)) H = dt - done;
-            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, q, a0);
+            bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, q, a0);
             int halvings = 0, kconv = 0;
             for (;;) {
                 bool ok = false;
@@ -316,14 +337,14 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
 #pragma unroll
                         for (int c = 0; c < 3; c++) { qm[c] = q[c]; vm[c] = v[c]; qn[c] = q[c] + h * v[c]; vn[c] = v[c] + h * a0[c]; }
                         for (int m = 1; m < nk; m++) {
-                            bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
+                            bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
 #pragma unroll
                             for (int c = 0; c < 3; c++) {
                                 const double qs = qm[c] + h2 * vn[c], vs = vm[c] + h2 * a[c];
                                 qm[c] = qn[c]; vm[c] = vn[c]; qn[c] = qs; vn[c] = vs;
                             }
                         }
-                        bs_force<MODE, ROWS>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
+                        bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
 #pragma unroll
                         for (int c = 0; c < 3; c++) {
                             cq[c] = 0.5 * (qn[c] + qm[c] + h * vn[c]);

@@ -56,7 +56,8 @@ struct genga_kick_ctx {
     int* grp_label; int* grp_flag; unsigned* grp_keys_a; unsigned* grp_keys_b; int* grp_vals_a; int* grp_vals_b;
     int* grp_counts;
     double* bs_scratch;            // whole-grid Bulirsch-Stoer regime: positions (2 buffers), G m, r_crit rows, error slots
-    int bs_coop_blocks;            // its co-resident grid
+    int bs_coop_blocks;            // its co-resident grid (eight lanes per body)
+    int bs_coop_blocks1;           // ... of the one-lane-per-body variant
     double* hyb_state;             // [6][N] state before FG (genga_hybrid_step), lazily allocated
     void* senc_slab;               // scratch of genga_multilevel_step (genga_senc.cu), lazily allocated
     int senc_levels;               // levels it was cut for

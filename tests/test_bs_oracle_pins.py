@@ -152,8 +152,8 @@ def test_semi_active_particles_in_a_group(bs, oracle_mod):
     assert np.array_equal(q2, qf) and np.array_equal(v2, vf)
     qh, vh, _ = bs.bs_group(q[:, :2], v[:, :2], np.array([1e-5, 1e-6]), rc[:, :2], G, 1.0, dt, tol, is_tp=tp[:2], tp_mode=2)
     assert np.abs(qh[:, 0] - qk[:, 0]).max() > 1e-10                          # the particle moves the massive body
-    # --- particles never feel each other: what b does to a, fully interactive vs TP 2 (heavy particles, 1e-4 AU apart)
-    q, v, mass, rc = _tp_group(m_a=1e-7, m_b=1e-7)
+    # --- particles never feel each other: what b does to a, fully interactive vs TP 2 (heavy particles, 1e-3 AU apart)
+    q, v, mass, rc = _tp_group(m_a=1e-7, m_b=1e-7, sep=1e-3)
     alone, _, _ = bs.bs_group(q[:, :2], v[:, :2], mass[:2], rc[:, :2], G, 1.0, dt, tol)
     full, _, _ = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol)
     semi, _, _ = bs.bs_group(q, v, mass, rc, G, 1.0, dt, tol, is_tp=tp, tp_mode=2)

@@ -229,3 +229,16 @@ def test_semi_active_particles_in_groups(oracle_mod, tp_mode):
     qf, vf, _, _ = oracle_mod.bs.bs(pos, vel, mass, rc, np.asarray(members), np.asarray(offsets), G, 1.0, 3.0, 1e-12,
                                     pos, vel, nlevels=2)
     assert np.abs(qf - qw).max() > 1e-9
+
+
+def test_giant_group_one_lane_per_body(oracle_mod):
+    """A group too large for eight lanes per body on the full grid (above ~11,800 bodies on a B200) is integrated with
+    one lane per body, which evaluates the same eight partial sums and the same tree: bit-identical to the oracle."""
+    m = 12500
+    ki = gi.make_ring(m)
+    qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, np.arange(m), [0, m], ki.G, 1.0, 2.0, 1e-9,
+                                        ki.pos, ki.vel, max_group=None)
+    q, v, st = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 2.0, 1e-9, np.arange(m), [0, m], ki.pos, ki.vel)
+    assert st == 0 and not stats[0].failed
+    assert _check(q, v, qw, vw), "not bit-identical"
+    assert np.abs(q - ki.pos).max() > 1e-3
