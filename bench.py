@@ -419,6 +419,34 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                        "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3, graph=(sl, ss) == (2, 10))
                                               for sl, ss in ((2, 10), (4, 2), (3, 4))]}
 
+    # NEXT-4: the Bulirsch-Stoer kernels alone on the ring of Fig. 7 (the experiment of Fig. 8): n bodies
+    # on a ring, 8 close-encounter partners each, one group, integrated over dt = 6 d at tol 1e-12
+    def time_bs_ring(nr, reps=3):
+        kr = gi.make_ring(nr)
+        kb = GengaKick(nr, 0, max_level=0, pair_capacity=8, G=kr.G, device=local_rank)
+        kb.set_stream(stream.cuda_stream)
+        q_in, v_in, mb, rcb = to_dev(kr.pos), to_dev(kr.vel), to_dev(kr.mass), to_dev(kr.rcrit)
+        mem = torch.arange(max(nr, 4), dtype=torch.int32, device=dev)
+        off = torch.zeros(nr + 4, dtype=torch.int32, device=dev); off[1] = nr
+        summ = torch.tensor([1, nr, nr, 0], dtype=torch.int32, device=dev)
+        q, v = q_in.clone(), v_in.clone()
+        ts = []
+        for it in range(reps + 1):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            kb.bs(q_in, v_in, mb, rcb, 1, 1.0, kr.dt, 1e-12, mem, off, summ, q, v)
+            b.record(stream)
+            b.synchronize()
+            if it >= 1:
+                ts.append(a.elapsed_time(b))
+        st = kb.status()
+        kb.free()
+        return {"n": nr, "ms": float(np.median(ts)), "status": st}
+
+    bs_ring_info = {"what": "genga_bs on one ring group of n bodies with 8 partners each (Fig. 7 / Fig. 8), dt = 6 d, tol 1e-12: "
+                            "n <= 32 one warp, <= 256 one CTA, above the whole grid with 8 lanes per body",
+                    "rings": [time_bs_ring(nr) for nr in (2, 8, 32, 64, 256, 512, 1024, 2048, 4096)]}
+
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_pos, h_mass, h_rc, h_vel = pin(ki.pos), pin(ki.mass), pin(ki.rcrit), pin(ki.vel)
@@ -467,6 +495,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             "kick_list": list_info,
             "hybrid_step": hybrid_info,
             "multilevel_step": multilevel_info,
+            "bs_ring": bs_ring_info,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
