@@ -55,11 +55,14 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     const int wblocks = (int)std::min<long long>(std::max<long long>((N / 2 + 7) / 8, 1), 8LL * ctx->num_sms);
     genga::bs_kernel<GENGA_BS_MODE_WARP, GENGA_BS_THREADS><<<wblocks, GENGA_BS_THREADS, 0, st>>>(
         pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode, -1);
-    // one CTA per group of 33 .. 256 bodies
+    // one cluster of 8 CTAs per group of 33 .. 256 bodies, eight lanes per body
     if (N > GENGA_BS_WARP_MAX) {
-        const int blocks = (int)std::min<long long>(std::max<long long>(N / (GENGA_BS_WARP_MAX + 1), 1), 16LL * ctx->num_sms);
-        genga::bs_kernel<GENGA_BS_MODE_CTA, GENGA_BS_THREADS><<<blocks, GENGA_BS_THREADS, 0, st>>>(
-            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode, -1);
+        const long long clusters = std::min<long long>(std::max<long long>(N / (GENGA_BS_WARP_MAX + 1), 1),
+                                                       2LL * ctx->num_sms / GENGA_BS_CLUSTER);
+        int lo = GENGA_BS_WARP_MAX;
+        genga::bs_cluster_kernel<<<(unsigned)(clusters * GENGA_BS_CLUSTER), GENGA_BS_THREADS, 0, st>>>(
+            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, lo,
+            n_massive, tp_mode, -1);
         ctx->launches++;
     }
     GK_CUDA(ctx, cudaGetLastError());

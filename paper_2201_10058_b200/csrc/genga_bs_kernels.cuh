@@ -1,10 +1,12 @@
-// sm_100a kernel of the Bulirsch-Stoer integration of close-encounter groups (include/genga_bs.h;
-// PAPER.md:47, :559-597, App. A), one body per thread, in three regimes of one template:
+// sm_100a kernels of the Bulirsch-Stoer integration of close-encounter groups (include/genga_bs.h;
+// PAPER.md:47, :559-597, App. A), in three regimes of one template:
 //   bs_kernel<WARP>   one WARP per group of up to 32 bodies, eight groups side by side in a CTA, the group's state
 //                     in the warp's slice of shared memory, no CTA-wide barrier: the regime BS-B of Table 2
 //                     (sec. 6.1.1: n <= 32) -- nearly all groups are pairs;
-//   bs_kernel<CTA>    one CTA of 256 threads per group of 33 .. 256 bodies, the group's state in shared memory: the
-//                     regime BS-A of Table 2, many groups side by side;
+//   bs_cluster_kernel one thread-block CLUSTER of 8 CTAs x 256 threads per group of 33 .. 256 bodies, eight lanes per
+//                     body: the CTAs publish their 32 bodies' positions in their own shared memory, gather the others'
+//                     through distributed shared memory and meet at one cluster barrier per force evaluation; many
+//                     clusters side by side: the regime BS-A of Table 2;
 //   bs_kernel<COOP>   ONE group at a time over the whole grid (cooperative launch, 64-thread CTAs): the paper's
 //                     BS-M regime ("distributed over multiple thread blocks ... sub-steps ...
 //                     controlled from the host ... many different kernel calls") -- but here the sub-steps stay
@@ -27,9 +29,12 @@
 
 namespace genga {
 
-#define GENGA_BS_MODE_CTA 0
+#define GENGA_BS_MODE_CTA 0              // (one CTA per group, one lane per body: the warp regime's code path; not launched)
 #define GENGA_BS_MODE_COOP 1
 #define GENGA_BS_MODE_WARP 2
+#define GENGA_BS_MODE_CLUSTER 3
+#define GENGA_BS_CLUSTER 8              // CTAs of a cluster (the portable maximum)
+#define GENGA_BS_CLUSTER_BODIES 32      // bodies per CTA of a cluster = GENGA_BS_THREADS / GENGA_BS_SUB
 #define GENGA_BS_WARP_MAX 32            // largest group of the warp-per-group regime
 #define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
 #define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
@@ -68,6 +73,10 @@ struct BsShared {
     double rc[GENGA_BS_MAX_LEVELS][ROWS];
     double red[8];
     double errmax;
+    // cluster regime: this CTA's bodies, published for the other CTAs of the cluster (two buffers: force evaluation e
+    // publishes into buffer e & 1 while slower CTAs may still gather from the other one), and its error maxima
+    double pubx[2][GENGA_BS_CLUSTER_BODIES], puby[2][GENGA_BS_CLUSTER_BODIES], pubz[2][GENGA_BS_CLUSTER_BODIES];
+    double emax[2];
 };
 
 // one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3.
@@ -112,7 +121,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
     const double s0 = -mu / (r2s * rs);
     double ax = s0 * x, ay = s0 * y, az = s0 * z;
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP;
-    if (!COOP) {
+    if (MODE == GENGA_BS_MODE_WARP || MODE == GENGA_BS_MODE_CTA) {
         bs_sync<MODE>();                                      // the previous readers are done
         if (i < n) { S.x[i] = x; S.y[i] = y; S.z[i] = z; }
         bs_sync<MODE>();
@@ -124,6 +133,39 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             }
 #undef GENGA_BS_RCJ
         }
+    } else if (MODE == GENGA_BS_MODE_CLUSTER) {
+        // Eight lanes per body (as below), the group spread over the CTAs of a cluster: publish, one cluster barrier,
+        // gather everybody's positions through distributed shared memory, then sum from the local copy.
+        cooperative_groups::cluster_group cl = cooperative_groups::this_cluster();
+        const int p = eval & 1;
+        eval++;
+        const int t = threadIdx.x, sub = t & (SUB - 1);
+        if (i < n && sub == 0) { S.pubx[p][t / SUB] = x; S.puby[p][t / SUB] = y; S.pubz[p][t / SUB] = z; }
+        cl.sync();
+        for (int idx = t; idx < n; idx += ROWS) {
+            const unsigned r = idx / GENGA_BS_CLUSTER_BODIES, o = idx % GENGA_BS_CLUSTER_BODIES;
+            S.x[idx] = cl.map_shared_rank(&S.pubx[p][0], r)[o];
+            S.y[idx] = cl.map_shared_rank(&S.puby[p][0], r)[o];
+            S.z[idx] = cl.map_shared_rank(&S.pubz[p][0], r)[o];
+        }
+        __syncthreads();
+        const double sx = ax, sy = ay, sz = az;
+        ax = 0.0; ay = 0.0; az = 0.0;
+        if (i < n) {
+#define GENGA_BS_RCJ(k) S.rc[k][jj]
+            for (int jj = sub; jj < n; jj += SUB) {
+                if (jj == i) continue;
+                GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
+            }
+#undef GENGA_BS_RCJ
+        }
+#pragma unroll
+        for (int o = 1; o < SUB; o <<= 1) {
+            ax = ax + __shfl_xor_sync(0xffffffffu, ax, o);
+            ay = ay + __shfl_xor_sync(0xffffffffu, ay, o);
+            az = az + __shfl_xor_sync(0xffffffffu, az, o);
+        }
+        ax = sx + ax; ay = sy + ay; az = sz + az;
     } else {
         // The pair terms with j = s (mod 8) are summed in ascending j from 0 into p_s, s = 0 .. 7; the eight partial
         // sums are combined as ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) and added to the Sun term.
@@ -202,6 +244,18 @@ __device__ __forceinline__ double bs_group_max(BsShared<ROWS>& S, const BsGlobal
         S.errmax = m;
     }
     __syncthreads();
+    if (MODE == GENGA_BS_MODE_CLUSTER) {
+        // each CTA publishes its maximum (two slots used in turn), one cluster barrier, everybody reads all of them
+        cooperative_groups::cluster_group cl = cooperative_groups::this_cluster();
+        const int slot = echeck & 1;
+        echeck++;
+        if (t == 0) S.emax[slot] = S.errmax;
+        cl.sync();
+        double m = 0.0;
+#pragma unroll
+        for (unsigned r = 0; r < GENGA_BS_CLUSTER; r++) m = fmax(m, *cl.map_shared_rank(&S.emax[slot], r));
+        return m;
+    }
     if (!COOP) return S.errmax;
     // non-negative doubles order like their bit patterns: atomicMax on the bits; four slots used in turn, the slot
     // two checks ahead is cleared after this check's barrier (its last readers passed the previous barrier)
@@ -219,14 +273,15 @@ __device__ __forceinline__ double bs_group_max(BsShared<ROWS>& S, const BsGlobal
 // (a serial walk over tens of thousands of two-body groups cost 0.6 ms per call).  CTA-uniform results.
 #define GENGA_BS_BIG_LIST 256
 template <int THREADS>
-__device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, int n_groups, int small_max, int& scan_from,
-                                              int* big, unsigned* wm, int& nbig)
+__device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, int n_groups, int small_max, int hi_max,
+                                              int& scan_from, int* big, unsigned* wm, int& nbig)
 {
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     int count = 0;
     while (scan_from < n_groups && count + THREADS <= GENGA_BS_BIG_LIST) {
         const int g = scan_from + t;
-        const bool is_big = g < n_groups && offsets[g + 1] - offsets[g] > small_max;
+        const int sz = g < n_groups ? offsets[g + 1] - offsets[g] : 0;
+        const bool is_big = sz > small_max && (hi_max < 0 || sz <= hi_max);
         const unsigned m = __ballot_sync(0xffffffffu, is_big);
         __syncthreads();                                               // wm's previous readers are done
         if (lane == 0) wm[warp] = m;
@@ -247,20 +302,21 @@ __device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, i
 }
 
 // WARP: warp w, w + (warps of the grid), ... integrates group w if it has at most 32 bodies.
-// CTA : CTA g, g + gridDim.x, ... integrates group g if it has 33 .. THREADS bodies.
+// CLUSTER: cluster c, c + (clusters of the grid), ... of the groups with 33 .. 256 bodies (found by the same scan as below).
 // COOP: the whole grid integrates, one after the other, the groups with more than `small_max` and at most `big_max`
 //       bodies (two launches: a grid of one CTA per SM, whose barrier is cheap, for groups it can hold, and the full
 //       co-resident grid for the rest); groups larger than the grid of a launch with big_max < 0 are reported and
 //       left as they are.
-template <int MODE, int THREADS, int SUB = 1>
-__global__ void __launch_bounds__(THREADS)
-bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
+template <int MODE, int THREADS, int SUB>
+__device__ __forceinline__ void
+bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
           double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max,
           long long n_massive, int tp_mode, int big_max)
 {
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP, WARP = MODE == GENGA_BS_MODE_WARP;
+    constexpr bool CLUSTER = MODE == GENGA_BS_MODE_CLUSTER, LISTED = COOP || CLUSTER;
     constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : THREADS);
     constexpr int UNITS = WARP ? THREADS / 32 : 1;                      // groups in flight per CTA
     __shared__ BsShared<ROWS> Sall[UNITS];
@@ -268,30 +324,37 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
     const int t = WARP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
     // this thread's body within the group (whole-grid regime: GENGA_BS_SUB consecutive lanes share a body and carry
     // identical copies of its state; they differ only in the part of the force sum they evaluate)
-    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / SUB) : t;
-    const bool writer = !COOP || (t & (SUB - 1)) == 0;
+    // (cluster regime: the same, over the CTAs of the cluster: CTA r holds the bodies 32 r .. 32 r + 31)
+    const int crank = CLUSTER ? (int)(blockIdx.x % GENGA_BS_CLUSTER) : 0;
+    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / SUB) : (CLUSTER ? (crank * THREADS + t) / SUB : t);
+    const bool writer = !LISTED || (t & (SUB - 1)) == 0;
     const long long capacity = COOP ? (long long)gridDim.x * THREADS / SUB : ROWS;
     const int n_groups = summary[0];
     int eval = 0, echeck = 0;
     const int g0 = COOP ? 0 : (WARP ? (int)(blockIdx.x * UNITS + (threadIdx.x >> 5)) : (int)blockIdx.x);
     const int gstep = COOP ? 1 : (int)gridDim.x * UNITS;
-    __shared__ int big[COOP ? GENGA_BS_BIG_LIST : 1];
+    __shared__ int big[LISTED ? GENGA_BS_BIG_LIST : 1];
     __shared__ unsigned wm[THREADS / 32];
+    // whole-grid regime: every CTA walks the whole list; cluster regime: cluster c takes the entries c, c + clusters, ..
+    const int lfirst = CLUSTER ? (int)(blockIdx.x / GENGA_BS_CLUSTER) : 0;
+    const int lstep = CLUSTER ? (int)(gridDim.x / GENGA_BS_CLUSTER) : 1;
     int scan_from = 0, nbig = 0, ib = 0;
-    if (COOP && summary[2] <= small_max) return;                        // no group for this regime (grid-uniform)
+    if (LISTED && summary[2] <= small_max) return;                      // no group for this regime (grid-uniform)
     for (int g = g0;; g += gstep) {
-        if (COOP) {
-            while (ib == nbig && scan_from < n_groups) {
-                bs_scan_large<THREADS>(offsets, n_groups, small_max, scan_from, big, wm, nbig);
-                ib = 0;
+        if (LISTED) {
+            while (ib >= nbig && scan_from < n_groups) {
+                ib = ib - nbig + (nbig == 0 && scan_from == 0 ? lfirst : 0);      // position within the next batch
+                bs_scan_large<THREADS>(offsets, n_groups, small_max, CLUSTER ? THREADS : big_max, scan_from, big, wm, nbig);
             }
-            if (ib == nbig) break;
-            g = big[ib++];
+            if (ib >= nbig) break;
+            g = big[ib];
+            ib += lstep;
         } else if (g >= n_groups) break;
         const int first = offsets[g], n = offsets[g + 1] - first;
         // the other regimes' groups (grid- / CTA- / warp-uniform)
         if (COOP ? (n <= small_max || (big_max >= 0 && n > big_max))
                  : (WARP ? n > GENGA_BS_WARP_MAX : (n > THREADS || n <= GENGA_BS_WARP_MAX))) continue;
+        // (listed regimes: the scan has already applied these bounds)
         if (n > capacity) {
             if (t == 0 && blockIdx.x == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
             continue;
@@ -312,9 +375,16 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
                     Gm.gm[i] = gm;
                     for (int k = 0; k < nlevels; k++) Gm.rc[k][i] = rci[k];
                 }
-            } else {
+            } else if (!CLUSTER) {
                 S.gm[i] = gm;
                 for (int k = 0; k < nlevels; k++) S.rc[k][i] = rci[k];
+            }
+        }
+        if (CLUSTER) {                                                  // every CTA stages the whole group's G m and radii
+            for (int idx = t; idx < n; idx += THREADS) {
+                const long long bj = members[first + idx];
+                S.gm[idx] = bj >= n_massive ? -(G * mass[bj]) : G * mass[bj];
+                for (int k = 0; k < nlevels; k++) S.rc[k][idx] = rcrit[(long long)k * N + bj];
             }
         }
         // (COOP: G m and the radii are read by other CTAs only after the first force evaluation's grid barrier;
@@ -397,6 +467,30 @@ bs_kernel(const double* __restrict__ pos_in, const double* __restrict__ vel_in, 
             for (int c = 0; c < 3; c++) { pos[c * N + b] = q[c]; vel[c * N + b] = v[c]; }
         }
     }
+    // no CTA of a cluster leaves while another may still read its shared memory
+    if (CLUSTER) cooperative_groups::this_cluster().sync();
+}
+
+#define GENGA_BS_ARGS                                                                                                   \
+    const double *__restrict__ pos_in, const double *__restrict__ vel_in, const double *__restrict__ mass,              \
+        const double *__restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,         \
+        const int *__restrict__ members, const int *__restrict__ offsets, const int *__restrict__ summary,              \
+        double *__restrict__ pos, double *__restrict__ vel, int *__restrict__ status, const BsGlobal Gm, int small_max, \
+        long long n_massive, int tp_mode, int big_max
+#define GENGA_BS_PASS                                                                                                    \
+    pos_in, vel_in, mass, rcrit, N, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, Gm, small_max, \
+        n_massive, tp_mode, big_max
+
+template <int MODE, int THREADS, int SUB = 1>
+__global__ void __launch_bounds__(THREADS) bs_kernel(GENGA_BS_ARGS)
+{
+    bs_run<MODE, THREADS, SUB>(GENGA_BS_PASS);
+}
+
+// the cluster regime: GENGA_BS_CLUSTER CTAs per cluster (the grid is a multiple of it)
+__global__ void __cluster_dims__(GENGA_BS_CLUSTER, 1, 1) __launch_bounds__(GENGA_BS_THREADS) bs_cluster_kernel(GENGA_BS_ARGS)
+{
+    bs_run<GENGA_BS_MODE_CLUSTER, GENGA_BS_THREADS, GENGA_BS_SUB>(GENGA_BS_PASS);
 }
 
 }  // namespace genga
