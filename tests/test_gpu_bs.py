@@ -242,3 +242,23 @@ def test_giant_group_one_lane_per_body(oracle_mod):
     assert st == 0 and not stats[0].failed
     assert _check(q, v, qw, vw), "not bit-identical"
     assert np.abs(q - ki.pos).max() > 1e-3
+
+
+@pytest.mark.parametrize("size,count,dt,tol", [(40, 700, 3.0, 1e-10), (257, 258, 0.01, 1e-6)])
+def test_many_mid_size_groups_are_all_found(oracle_mod, size, count, dt, tol):
+    """More groups of one regime than one batch of the device-side group scan holds (256): 700 groups of 40 bodies for
+    the cluster regime (dealt round-robin to the clusters across batches), 258 groups of 257 bodies for the whole-grid
+    regime (a short step at a loose tolerance: the oracle walks these groups one by one) -- arcs of one large ring,
+    every group integrated, bit-identical to the oracle."""
+    m = size * count
+    ki = gi.make_ring(m, partners=4)
+    members = np.arange(m)
+    offsets = np.arange(0, m + 1, size)
+    qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, members, offsets, ki.G, 1.0, dt, tol,
+                                        ki.pos, ki.vel, max_group=None)
+    q, v, st = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, dt, tol, members, offsets, ki.pos, ki.vel)
+    assert st == 0 and len(stats) == count
+    assert _check(q, v, qw, vw), "not bit-identical"
+    # every group moved away from the state the arrays held before the call
+    moved = np.abs(q - ki.pos).max(axis=0).reshape(count, size).max(axis=1)
+    assert np.all(moved > 1e-6)
