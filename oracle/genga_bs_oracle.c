@@ -32,9 +32,9 @@
  *     The first macro step tries the whole dt.
  * All arithmetic in IEEE binary64 in the order written (compile with -ffp-contract=off).  Order of the force sum
  * ("parallel reductions have a well-defined order"), part of reading G15:
- *   groups of up to 32 bodies (BS-B of Table 2): Sun term, then the pair terms added one by one in
- *   member order j = 0 .. n-1;
- *   larger groups (BS-A and the multi-block regime BS-M, where the sum is spread over threads):
+ *   groups of up to 8 bodies: Sun term, then the pair terms added one by one in member order j = 0 .. n-1;
+ *   larger groups (where the sum of a body is spread over several threads, as in the paper's regimes BS-A and BS-M,
+ *   PAPER.md:589-597):
  *   eight partial sums p_s = sum of the terms with j = s (mod 8), each in ascending j from 0, combined as
  *   ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) and added to the Sun term.
  *
@@ -51,7 +51,7 @@
 
 #define BS_KMAX 8
 #define BS_MAX_HALVINGS 60
-#define BS_SEQ_MAX 32       /* largest group whose force sum is sequential */
+#define BS_SEQ_MAX 8        /* largest group whose force sum is sequential */
 
 extern double genga_oracle_K(double r, double rc);
 

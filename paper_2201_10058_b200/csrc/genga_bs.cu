@@ -51,10 +51,17 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     }
     // at most N / 2 groups; warps / CTAs stride over them (their number is only known on the device)
     int small_max = GENGA_BS_THREADS;
-    // one warp per group of up to 32 bodies (nearly all groups), eight groups per CTA
-    const int wblocks = (int)std::min<long long>(std::max<long long>((N / 2 + 7) / 8, 1), 8LL * ctx->num_sms);
-    genga::bs_kernel<GENGA_BS_MODE_WARP, GENGA_BS_THREADS><<<wblocks, GENGA_BS_THREADS, 0, st>>>(
-        pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max, n_massive, tp_mode, -1);
+    // one launch: one warp per group of up to 8 bodies (nearly all groups), eight groups per CTA, in the first `wblocks`
+    // CTAs; one CTA per group of 9 .. 32 bodies, eight lanes per body, in the rest
+    {
+        const int wblocks = (int)std::min<long long>(std::max<long long>((N / 2 + 7) / 8, 1), 8LL * ctx->num_sms);
+        const int cblocks = N > GENGA_BS_SEQ_MAX
+                                ? (int)std::min<long long>(std::max<long long>(N / (GENGA_BS_SEQ_MAX + 1), 1), 4LL * ctx->num_sms)
+                                : 0;
+        genga::bs_small_kernel<<<wblocks + cblocks, GENGA_BS_THREADS, 0, st>>>(
+            pos_in, vel_in, mass, rcrit, NN, nlevels, G, mu, dt, tol, members, offsets, summary, pos, vel, status, gm, small_max,
+            n_massive, tp_mode, -1, wblocks);
+    }
     // one cluster of 8 CTAs per group of 33 .. 256 bodies, eight lanes per body
     if (N > GENGA_BS_WARP_MAX) {
         const long long clusters = std::min<long long>(std::max<long long>(N / (GENGA_BS_WARP_MAX + 1), 1),

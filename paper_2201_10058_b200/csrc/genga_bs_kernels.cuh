@@ -1,8 +1,10 @@
 // sm_100a kernels of the Bulirsch-Stoer integration of close-encounter groups (include/genga_bs.h;
 // PAPER.md:47, :559-597, App. A), in three regimes of one template:
-//   bs_kernel<WARP>   one WARP per group of up to 32 bodies, eight groups side by side in a CTA, the group's state
-//                     in the warp's slice of shared memory, no CTA-wide barrier: the regime BS-B of Table 2
-//                     (sec. 6.1.1: n <= 32) -- nearly all groups are pairs;
+//   bs_kernel<WARP>   one WARP per group of up to 8 bodies, one lane per body, eight groups side by side in a CTA, the
+//                     group's state in the warp's slice of shared memory, no CTA-wide barrier -- nearly all groups are
+//                     pairs;
+//   bs_kernel<CTA>    one CTA per group of 9 .. 32 bodies, eight lanes per body; with the warp regime the regime BS-B
+//                     of Table 2 (sec. 6.1.1: n <= 32);
 //   bs_cluster_kernel one thread-block CLUSTER of 8 CTAs x 256 threads per group of 33 .. 256 bodies, eight lanes per
 //                     body: the CTAs publish their 32 bodies' positions in their own shared memory, gather the others'
 //                     through distributed shared memory and meet at one cluster barrier per force evaluation; many
@@ -29,13 +31,15 @@
 
 namespace genga {
 
-#define GENGA_BS_MODE_CTA 0              // (one CTA per group, one lane per body: the warp regime's code path; not launched)
+#define GENGA_BS_MODE_CTA 0
 #define GENGA_BS_MODE_COOP 1
 #define GENGA_BS_MODE_WARP 2
 #define GENGA_BS_MODE_CLUSTER 3
 #define GENGA_BS_CLUSTER 8              // CTAs of a cluster (the portable maximum)
 #define GENGA_BS_CLUSTER_BODIES 32      // bodies per CTA of a cluster = GENGA_BS_THREADS / GENGA_BS_SUB
-#define GENGA_BS_WARP_MAX 32            // largest group of the warp-per-group regime
+#define GENGA_BS_WARP_MAX 32            // rows of a warp's shared-memory slice
+#define GENGA_BS_SEQ_MAX 8              // largest group of the warp-per-group regime (force sum in member order)
+#define GENGA_BS_CTA_MAX 32             // largest group of the one-CTA regime = GENGA_BS_THREADS / GENGA_BS_SUB
 #define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
 #define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
 #define GENGA_BS_SUB 8                  // whole-grid regime: lanes per body, each summing the terms with j = lane (mod 8)
@@ -121,7 +125,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
     const double s0 = -mu / (r2s * rs);
     double ax = s0 * x, ay = s0 * y, az = s0 * z;
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP;
-    if (MODE == GENGA_BS_MODE_WARP || MODE == GENGA_BS_MODE_CTA) {
+    if (MODE == GENGA_BS_MODE_WARP) {
         bs_sync<MODE>();                                      // the previous readers are done
         if (i < n) { S.x[i] = x; S.y[i] = y; S.z[i] = z; }
         bs_sync<MODE>();
@@ -133,6 +137,29 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             }
 #undef GENGA_BS_RCJ
         }
+    } else if (MODE == GENGA_BS_MODE_CTA) {
+        // Eight lanes per body inside one CTA (groups of up to 32 bodies): the eight partial sums and the tree as below.
+        const int sub = threadIdx.x & (SUB - 1);
+        __syncthreads();                                      // the previous readers are done
+        if (i < n && sub == 0) { S.x[i] = x; S.y[i] = y; S.z[i] = z; }
+        __syncthreads();
+        const double sx = ax, sy = ay, sz = az;
+        ax = 0.0; ay = 0.0; az = 0.0;
+        if (i < n) {
+#define GENGA_BS_RCJ(k) S.rc[k][jj]
+            for (int jj = sub; jj < n; jj += SUB) {
+                if (jj == i) continue;
+                GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
+            }
+#undef GENGA_BS_RCJ
+        }
+#pragma unroll
+        for (int o = 1; o < SUB; o <<= 1) {
+            ax = ax + __shfl_xor_sync(0xffffffffu, ax, o);
+            ay = ay + __shfl_xor_sync(0xffffffffu, ay, o);
+            az = az + __shfl_xor_sync(0xffffffffu, az, o);
+        }
+        ax = sx + ax; ay = sy + ay; az = sz + az;
     } else if (MODE == GENGA_BS_MODE_CLUSTER) {
         // Eight lanes per body (as below), the group spread over the CTAs of a cluster: publish, one cluster barrier,
         // gather everybody's positions through distributed shared memory, then sum from the local copy.
@@ -301,7 +328,8 @@ __device__ __forceinline__ void bs_scan_large(const int* __restrict__ offsets, i
     nbig = count;
 }
 
-// WARP: warp w, w + (warps of the grid), ... integrates group w if it has at most 32 bodies.
+// WARP: warp w, w + (warps of the grid), ... integrates group w if it has at most 8 bodies.
+// CTA : CTA g, g + gridDim.x, ... integrates group g if it has 9 .. 32 bodies.
 // CLUSTER: cluster c, c + (clusters of the grid), ... of the groups with 33 .. 256 bodies (found by the same scan as below).
 // COOP: the whole grid integrates, one after the other, the groups with more than `small_max` and at most `big_max`
 //       bodies (two launches: a grid of one CTA per SM, whose barrier is cheap, for groups it can hold, and the full
@@ -313,8 +341,9 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
           double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max,
-          long long n_massive, int tp_mode, int big_max)
+          long long n_massive, int tp_mode, int big_max, int vblock, int vgrid)
 {
+    // vblock / vgrid: this CTA's index and the number of CTAs of its regime (the warp and one-CTA regimes share a launch)
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP, WARP = MODE == GENGA_BS_MODE_WARP;
     constexpr bool CLUSTER = MODE == GENGA_BS_MODE_CLUSTER, LISTED = COOP || CLUSTER;
     constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : THREADS);
@@ -326,13 +355,14 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
     // identical copies of its state; they differ only in the part of the force sum they evaluate)
     // (cluster regime: the same, over the CTAs of the cluster: CTA r holds the bodies 32 r .. 32 r + 31)
     const int crank = CLUSTER ? (int)(blockIdx.x % GENGA_BS_CLUSTER) : 0;
-    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / SUB) : (CLUSTER ? (crank * THREADS + t) / SUB : t);
-    const bool writer = !LISTED || (t & (SUB - 1)) == 0;
+    constexpr bool CTA = MODE == GENGA_BS_MODE_CTA;
+    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / SUB) : (CLUSTER ? (crank * THREADS + t) / SUB : (CTA ? t / SUB : t));
+    const bool writer = WARP || (t & (SUB - 1)) == 0;
     const long long capacity = COOP ? (long long)gridDim.x * THREADS / SUB : ROWS;
     const int n_groups = summary[0];
     int eval = 0, echeck = 0;
-    const int g0 = COOP ? 0 : (WARP ? (int)(blockIdx.x * UNITS + (threadIdx.x >> 5)) : (int)blockIdx.x);
-    const int gstep = COOP ? 1 : (int)gridDim.x * UNITS;
+    const int g0 = COOP ? 0 : (WARP ? (int)(vblock * UNITS + (threadIdx.x >> 5)) : vblock);
+    const int gstep = COOP ? 1 : vgrid * UNITS;
     __shared__ int big[LISTED ? GENGA_BS_BIG_LIST : 1];
     __shared__ unsigned wm[THREADS / 32];
     // whole-grid regime: every CTA walks the whole list; cluster regime: cluster c takes the entries c, c + clusters, ..
@@ -353,7 +383,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         const int first = offsets[g], n = offsets[g + 1] - first;
         // the other regimes' groups (grid- / CTA- / warp-uniform)
         if (COOP ? (n <= small_max || (big_max >= 0 && n > big_max))
-                 : (WARP ? n > GENGA_BS_WARP_MAX : (n > THREADS || n <= GENGA_BS_WARP_MAX))) continue;
+                 : (WARP ? n > GENGA_BS_SEQ_MAX : (CTA ? (n <= GENGA_BS_SEQ_MAX || n > GENGA_BS_CTA_MAX) : false))) continue;
         // (listed regimes: the scan has already applied these bounds)
         if (n > capacity) {
             if (t == 0 && blockIdx.x == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
@@ -375,12 +405,12 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
                     Gm.gm[i] = gm;
                     for (int k = 0; k < nlevels; k++) Gm.rc[k][i] = rci[k];
                 }
-            } else if (!CLUSTER) {
+            } else if (WARP) {
                 S.gm[i] = gm;
                 for (int k = 0; k < nlevels; k++) S.rc[k][i] = rci[k];
             }
         }
-        if (CLUSTER) {                                                  // every CTA stages the whole group's G m and radii
+        if (CLUSTER || CTA) {                                           // every CTA stages the whole group's G m and radii
             for (int idx = t; idx < n; idx += THREADS) {
                 const long long bj = members[first + idx];
                 S.gm[idx] = bj >= n_massive ? -(G * mass[bj]) : G * mass[bj];
@@ -484,13 +514,24 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
 template <int MODE, int THREADS, int SUB = 1>
 __global__ void __launch_bounds__(THREADS) bs_kernel(GENGA_BS_ARGS)
 {
-    bs_run<MODE, THREADS, SUB>(GENGA_BS_PASS);
+    bs_run<MODE, THREADS, SUB>(GENGA_BS_PASS, (int)blockIdx.x, (int)gridDim.x);
+}
+
+// the warp regime (CTAs below `split`) and the one-CTA regime (the rest) in ONE launch: their groups are independent, and
+// a launch of its own for the few 9 .. 32-body groups would only add their duration to the step
+__global__ void __launch_bounds__(GENGA_BS_THREADS) bs_small_kernel(GENGA_BS_ARGS, int split)
+{
+    if ((int)blockIdx.x < split)
+        bs_run<GENGA_BS_MODE_WARP, GENGA_BS_THREADS, 1>(GENGA_BS_PASS, (int)blockIdx.x, split);
+    else
+        bs_run<GENGA_BS_MODE_CTA, GENGA_BS_THREADS, GENGA_BS_SUB>(GENGA_BS_PASS, (int)blockIdx.x - split,
+                                                                  (int)gridDim.x - split);
 }
 
 // the cluster regime: GENGA_BS_CLUSTER CTAs per cluster (the grid is a multiple of it)
 __global__ void __cluster_dims__(GENGA_BS_CLUSTER, 1, 1) __launch_bounds__(GENGA_BS_THREADS) bs_cluster_kernel(GENGA_BS_ARGS)
 {
-    bs_run<GENGA_BS_MODE_CLUSTER, GENGA_BS_THREADS, GENGA_BS_SUB>(GENGA_BS_PASS);
+    bs_run<GENGA_BS_MODE_CLUSTER, GENGA_BS_THREADS, GENGA_BS_SUB>(GENGA_BS_PASS, (int)blockIdx.x, (int)gridDim.x);
 }
 
 }  // namespace genga
