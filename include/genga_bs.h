@@ -17,11 +17,12 @@
  * Method (the paper names it and refers to Grimm & Stadel 2014; reading G15): Gragg-Bulirsch-
  * Stoer -- modified midpoint with 2, 4, .., 16 sub-steps, polynomial extrapolation in h^2, relative error
  * per body in position and velocity <= tol, one step size for the whole group (halved on failure, doubled
- * after fast convergence).  Groups of up to 32 bodies: one warp per group, one lane per body, eight groups per
- * thread block, the force sum in member order (BS-B of Table 2); 33 .. 256 bodies: one thread-block
- * cluster (8 x 256 threads) per group, eight lanes per body, positions exchanged through distributed shared memory
- * (BS-A); many groups side by side.  From 33 bodies on the force sum of a body is taken in eight interleaved partial
- * sums combined in a fixed tree (the oracle states the order).  Larger groups: one group at a time
+ * after fast convergence).  Groups of up to 8 bodies: one warp per group, one lane per body, eight groups per thread
+ * block, the force sum in member order; 9 .. 32 bodies: one thread block per group, eight lanes per body (together
+ * BS-B of Table 2); 33 .. 256 bodies: one thread-block cluster (8 x 256 threads) per group, eight
+ * lanes per body, positions exchanged through distributed shared memory (BS-A); many groups side by side.  From 9
+ * bodies on the force sum of a body is taken in eight interleaved partial sums combined in a fixed tree (the oracle
+ * states the order).  Larger groups: one group at a time
  * over a whole co-resident grid with a grid-wide barrier per force evaluation (the paper's BS-M regime,
  * PAPER.md:595-597, with the sub-steps kept on the device instead of controlled from the host); a group larger
  * than that grid keeps the state already in pos / vel (8 lanes per body, each summing an eighth of the pair terms, up
