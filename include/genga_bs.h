@@ -58,6 +58,21 @@ int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double* vel_in, co
              const int32_t* summary, double* pos, double* vel);
 
 /*
+ * Diagnostics of the step-size control (what makes a comparison with another implementation of the same scheme
+ * meaningful: two runs that took the same decisions differ by rounding only; where a decision differs -- an error
+ * estimate within rounding of tol -- both results still satisfy the tolerance, and the difference is of that order).
+ *   genga_bs_set_stats: every following genga_bs writes, for group g < rows (g as in `offsets`), the int32 row
+ *       (accepted macro steps, rejected attempts = halvings, force evaluations, bodies) to group_stats[g];
+ *       device memory owned by the caller, 16-byte aligned; NULL switches it off.  Groups not integrated are not written.
+ *   genga_bs_totals: the same three counts and the number of groups integrated, summed over all groups and all
+ *       genga_bs calls of the context (the ones inside genga_hybrid_step / genga_multilevel_step included) since
+ *       init or the last reset; synchronises the stream.
+ * Errors: E_NULL, E_ALIGN, E_SIZE, E_CUDA.
+ */
+int genga_bs_set_stats(genga_kick_ctx* ctx, int32_t* group_stats, int64_t rows);
+int genga_bs_totals(genga_kick_ctx* ctx, int64_t totals[4], int32_t reset);
+
+/*
  * The complete step of App. A on the device, no host round trip:
  *     Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt); grouping; Bulirsch-Stoer(dt) on the groups, from the
  *     state before FG; HC(dt/2); Kick(dt/2).

@@ -20,7 +20,7 @@
  *
  * How.  PAPER.md names the method and gives no algorithmic detail (it refers to Grimm & Stadel 2014 and
  * to textbooks); the scheme below is the textbook Gragg-Bulirsch-Stoer method, fixed here as reading G15
- * and followed by the CUDA kernel operation for operation:
+ * (DESIGN.md):
  *   - one macro step of length H: modified midpoint rule with n_k = 2 k sub-steps, k = 1 .. 8,
  *         z_0 = y;  z_1 = z_0 + h f(z_0);  z_{m+1} = z_{m-1} + 2 h f(z_m);  y_k = (z_n + z_{n-1} + h f(z_n)) / 2,  h = H / n_k
  *   - polynomial extrapolation in h^2 (Aitken-Neville):  T_{k,0} = y_k,
@@ -30,13 +30,11 @@
  *     accept T_kk as soon as err <= tol; if k = 8 is not enough, halve H and start the macro step again
  *   - after an accepted macro step: H <- 2 H if it converged with k <= 5, else H; never beyond the end of dt.
  *     The first macro step tries the whole dt.
- * All arithmetic in IEEE binary64 in the order written (compile with -ffp-contract=off).  Order of the force sum
- * ("parallel reductions have a well-defined order"), part of reading G15:
- *   groups of up to 8 bodies: Sun term, then the pair terms added one by one in member order j = 0 .. n-1;
- *   larger groups (where the sum of a body is spread over several threads, as in the paper's regimes BS-A and BS-M,
- *   PAPER.md:589-597):
- *   eight partial sums p_s = sum of the terms with j = s (mod 8), each in ascending j from 0, combined as
- *   ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) and added to the Sun term.
+ * All arithmetic in IEEE binary64 in the order written (compile with -ffp-contract=off).  The force on a body is
+ * the plain sum of its definition: the Sun term, then the pair terms added one by one in member order
+ * j = 0 .. n-1, for every group size.  The oracle knows nothing of how a kernel spreads that sum over threads: a kernel
+ * that sums in another order differs from this file at rounding level, and the parity tests bound that difference
+ * (tests/test_gpu_bs.py) instead of asking for equal bits.  Single-threaded.
  *
  * PINS (tests/test_bs_oracle_pins.py): two bodies far outside each other's critical radius (W_BS = 0):
  * each follows its Kepler orbit -- against the closed-form FG oracle; two bodies deep inside (K = 0): the
@@ -51,7 +49,6 @@
 
 #define BS_KMAX 8
 #define BS_MAX_HALVINGS 60
-#define BS_SEQ_MAX 8        /* largest group whose force sum is sequential */
 
 extern double genga_oracle_K(double r, double rc);
 
@@ -65,18 +62,15 @@ typedef struct {
 } bs_group;
 
 /* f: accelerations of all bodies of the group at positions q [n][3] */
-static inline void bs_accel_body(const bs_group *g, const double *q, double *a, int i)
+static void bs_accel(const bs_group *g, const double *q, double *a)
 {
     const int n = g->n;
-    {
+    for (int i = 0; i < n; i++) {
         const double x = q[3 * i], y = q[3 * i + 1], z = q[3 * i + 2];
         const double r2s = x * x + y * y + z * z;
         const double rs = sqrt(r2s);
         const double s0 = -g->mu / (r2s * rs);
         double ax = s0 * x, ay = s0 * y, az = s0 * z;
-        const int tree = n > BS_SEQ_MAX;
-        double p[8][3];
-        if (tree) for (int s8 = 0; s8 < 8; s8++) p[s8][0] = p[s8][1] = p[s8][2] = 0.0;
         for (int j = 0; j < n; j++) {
             if (j == i) continue;
             if (g->is_tp && g->is_tp[j] && (g->tp_mode != 2 || g->is_tp[i])) continue;      /* Fig. 14 */
@@ -90,28 +84,10 @@ static inline void bs_accel_body(const bs_group *g, const double *q, double *a, 
             }
             if (W != 0.0) {
                 const double s = g->G * g->m[j] * W / (r2 * r);
-                if (tree) { double *ps = p[j & 7]; ps[0] = ps[0] + s * dx; ps[1] = ps[1] + s * dy; ps[2] = ps[2] + s * dz; }
-                else { ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz; }
+                ax = ax + s * dx; ay = ay + s * dy; az = az + s * dz;
             }
         }
-        if (tree) {
-            double t[3];
-            for (int c = 0; c < 3; c++)
-                t[c] = ((p[0][c] + p[1][c]) + (p[2][c] + p[3][c])) + ((p[4][c] + p[5][c]) + (p[6][c] + p[7][c]));
-            ax = ax + t[0]; ay = ay + t[1]; az = az + t[2];
-        }
         a[3 * i] = ax; a[3 * i + 1] = ay; a[3 * i + 2] = az;
-    }
-}
-
-static void bs_accel(const bs_group *g, const double *q, double *a)
-{
-    const int n = g->n;
-    if (n > 2048) {         /* bodies are independent of each other here: the threads only share read-only data */
-#pragma omp parallel for schedule(static)
-        for (int i = 0; i < n; i++) bs_accel_body(g, q, a, i);
-    } else {
-        for (int i = 0; i < n; i++) bs_accel_body(g, q, a, i);
     }
 }
 

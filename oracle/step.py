@@ -88,6 +88,7 @@ class HybridStepResult:
     groups: object           # oracle.group.Groups of the first kick's pair list
     skipped: list            # groups larger than max_group (left at their Kepler-drifted state)
     unbound: int
+    bs_totals: tuple = (0, 0, 0, 0)   # step-size control of the Bulirsch-Stoer phase: accepted, rejected, force evaluations, groups
 
 
 def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc_factor=1.0, n1=3.0, n2=0.4,
@@ -108,12 +109,20 @@ def hybrid_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, tol=1e-12, enc
     q_in, v_in = q.copy(), v.copy()
     q, v, bad1 = fg(q, v, G * m_star, dt)
     gr = _group.group(n, _kick.pair_set(k1, n_massive))
-    q, v, _, skipped = _bs.bs(q_in, v_in, mass, rc, gr.members, gr.offsets, G, m_star, dt, tol, q, v, nlevels=1,
-                              max_group=max_group, n_massive=tpn, tp_mode=tp_mode)
+    q, v, bstats, skipped = _bs.bs(q_in, v_in, mass, rc, gr.members, gr.offsets, G, m_star, dt, tol, q, v, nlevels=1,
+                                   max_group=max_group, n_massive=tpn, tp_mode=tp_mode)
     q, _ = hc(q, v, mass, m_star, 0.5 * dt)
     k2 = _kick.kick(q, mass, rc, n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256, tp_mode=tp_mode)
     v = v + (0.5 * dt) * k2.acc
-    return HybridStepResult(pos=q, vel=v, rcrit=rc, first=k1, groups=gr, skipped=skipped, unbound=bad0 + bad1)
+    return HybridStepResult(pos=q, vel=v, rcrit=rc, first=k1, groups=gr, skipped=skipped, unbound=bad0 + bad1,
+                            bs_totals=_bs_totals(bstats))
+
+
+def _bs_totals(stats):
+    """(accepted macro steps, rejected attempts, force evaluations, groups) summed over a list of BsStats: the record
+    of the step-size control a kernel's genga_bs_totals is compared with."""
+    return (sum(s.accepted for s in stats), sum(s.rejected for s in stats), sum(s.force_evaluations for s in stats),
+            len(stats))
 
 
 @dataclass
@@ -125,6 +134,7 @@ class MultilevelStepResult:
     stats: np.ndarray        # [slevels, 4] per level, summed over its sub-steps: candidate pairs, close-encounter pairs,
                              # groups handed to Bulirsch-Stoer, bodies in them
     unbound: int
+    bs_totals: tuple = (0, 0, 0, 0)   # step-size control of all Bulirsch-Stoer calls: accepted, rejected, force evaluations, groups
 
 
 def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2, substeps=2, tol=1e-12, enc_factor=1.0,
@@ -161,6 +171,7 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
     rc[0] = row[0]
     stats = np.zeros((slevels, 4), dtype=np.int64)
     unbound = [bad]
+    bs_all = []
 
     def encounters(level, q0, v0, q1, v1, h, cand):
         enc = _det.detect(q0, v0, q1, v1, rc[level], h, cand, enc_factor=1.0).pairs if detect else cand
@@ -168,8 +179,9 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
         return enc, _group.group(n, enc)
 
     def bulirsch_stoer(level, q0, v0, h, gr, q, v):
-        q, v, _, skipped = _bs.bs(q0, v0, mass, rc, gr.members, gr.offsets, G, m_star, h, tol, q, v, nlevels=level + 1,
-                                  max_group=max_group, n_massive=n_massive if n_test > 0 else None, tp_mode=tp_mode)
+        q, v, bstats, skipped = _bs.bs(q0, v0, mass, rc, gr.members, gr.offsets, G, m_star, h, tol, q, v, nlevels=level + 1,
+                                       max_group=max_group, n_massive=n_massive if n_test > 0 else None, tp_mode=tp_mode)
+        bs_all.extend(bstats)
         stats[level, 2] += gr.n_groups - len(skipped)
         stats[level, 3] += len(gr.members) - sum(int(gr.offsets[g + 1] - gr.offsets[g]) for g in skipped)
         return q, v
@@ -215,4 +227,5 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
     q, _ = hc(q, v, mass, m_star, 0.5 * dt)
     k2 = _kick.kick(q, mass, rc[:1], n_massive, n_test, level=0, G=G, enc_factor=enc_factor, maxp=256, tp_mode=tp_mode)
     v = v + (0.5 * dt) * k2.acc
-    return MultilevelStepResult(pos=q, vel=v, rcrit=rc, first=k1, stats=stats, unbound=sum(unbound))
+    return MultilevelStepResult(pos=q, vel=v, rcrit=rc, first=k1, stats=stats, unbound=sum(unbound),
+                                bs_totals=_bs_totals(bs_all))

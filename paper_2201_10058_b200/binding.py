@@ -27,7 +27,7 @@ STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_ste
 GROUP_EXPORTS = ("genga_group",)
 STATUS_BAD_PAIR = 16
 # include/genga_bs.h: Bulirsch-Stoer integration of the groups
-BS_EXPORTS = ("genga_bs", "genga_hybrid_step")
+BS_EXPORTS = ("genga_bs", "genga_hybrid_step", "genga_bs_set_stats", "genga_bs_totals")
 STATUS_GROUP_TOO_LARGE, STATUS_BS_NOT_CONVERGED = 32, 64
 STATUS_UNBOUND = 8
 # include/genga_senc.h: close-encounter detection and the multi-level step (SEnc)
@@ -105,6 +105,8 @@ def lib():
         L.genga_group.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
         L.genga_hybrid_step.argtypes = [vp, vp, vp, vp, d, d, d, d, d, vp, vp, vp, vp, vp, vp, vp]
         L.genga_bs.argtypes = [vp, vp, vp, vp, vp, i32, d, d, d, vp, vp, vp, vp, vp]
+        L.genga_bs_set_stats.argtypes = [vp, vp, i64]
+        L.genga_bs_totals.argtypes = [vp, C.POINTER(i64 * 4), i32]
         L.genga_detect.argtypes = [vp, vp, vp, vp, vp, vp, d, d, vp, vp, i64, vp, vp]
         L.genga_multilevel_step.argtypes = [vp, vp, vp, vp, d, d, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
         for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS + SENC_EXPORTS:
@@ -150,8 +152,24 @@ def plan_iblock_ctas(plan: GengaKickPlan, ib: int):
     return a.value, b.value
 
 
-def _ptr(t):
-    return None if t is None else C.c_void_p(t.data_ptr())
+def _ptr(t, dtype=None, numel=0, name="array", host=False):
+    """Pointer of a tensor for the C ABI, after the checks the library cannot make on a bare pointer: the side it
+    lives on (device for every call but kick_host), dtype ("f8" / "i4"), C-contiguity and at least `numel` elements.
+    None stays NULL (the library decides whether that argument is optional)."""
+    if t is None:
+        return None
+    if host == bool(getattr(t, "is_cuda", False)):
+        raise ValueError(f"{name}: expected a {'CPU' if host else 'CUDA device'} tensor")
+    if dtype is not None:
+        import torch
+        want = torch.float64 if dtype == "f8" else torch.int32
+        if t.dtype != want:
+            raise TypeError(f"{name}: expected dtype {want}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name}: expected a C-contiguous tensor")
+    if t.numel() < numel:
+        raise ValueError(f"{name}: expected at least {numel} elements, got {t.numel()}")
+    return C.c_void_p(t.data_ptr())
 
 
 class GengaKick:
@@ -178,80 +196,135 @@ class GengaKick:
     def set_stream(self, cuda_stream: int):
         self._check(lib().genga_kick_set_stream(self._ctx, C.c_void_p(int(cuda_stream))))
 
+    def _kick_args(self, pos, vel, mass, rcrit, level, out_acc, out_pairs, out_npairs, host=False):
+        n, cap = self.n, int(self.cfg.pair_capacity)
+        rows = max(int(level), 0) + 1
+        return (_ptr(pos, "f8", 3 * n, "pos", host), _ptr(vel, "f8", 3 * n, "vel", host), _ptr(mass, "f8", n, "mass", host),
+                _ptr(rcrit, "f8", rows * n, "rcrit", host), _ptr(out_acc, "f8", 3 * n, "out_acc", host),
+                _ptr(out_pairs, "i4", 2 * cap, "out_pairs", host), _ptr(out_npairs, "i4", n + 1, "out_npairs", host))
+
     def kick(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
-        self._check(lib().genga_kick(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit), int(changeover_level),
-                                     float(dt), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs)))
+        p, v, m, rc, a, op, on = self._kick_args(pos, vel, mass, rcrit, changeover_level, out_acc, out_pairs, out_npairs)
+        self._check(lib().genga_kick(self._ctx, p, v, m, rc, int(changeover_level), float(dt), a, op, on))
 
     def kick_list(self, pos, vel, mass, rcrit, changeover_level, dt, in_pairs, in_n_pairs, in_pair_rows, out_acc,
                   out_pairs, out_npairs):
-        self._check(lib().genga_kick_list(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit), int(changeover_level),
-                                          float(dt), _ptr(in_pairs), _ptr(in_n_pairs), int(in_pair_rows), _ptr(out_acc),
-                                          _ptr(out_pairs), _ptr(out_npairs)))
+        p, v, m, rc, a, op, on = self._kick_args(pos, vel, mass, rcrit, changeover_level, out_acc, out_pairs, out_npairs)
+        self._check(lib().genga_kick_list(self._ctx, p, v, m, rc, int(changeover_level), float(dt),
+                                          _ptr(in_pairs, "i4", 2 * int(in_pair_rows), "in_pairs"),
+                                          _ptr(in_n_pairs, "i4", 1, "in_n_pairs"), int(in_pair_rows), a, op, on))
 
     def kick_host(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
-        self._check(lib().genga_kick_host(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(rcrit),
-                                          int(changeover_level), float(dt), _ptr(out_acc), _ptr(out_pairs),
-                                          _ptr(out_npairs)))
+        p, v, m, rc, a, op, on = self._kick_args(pos, vel, mass, rcrit, changeover_level, out_acc, out_pairs, out_npairs,
+                                                 host=True)
+        self._check(lib().genga_kick_host(self._ctx, p, v, m, rc, int(changeover_level), float(dt), a, op, on))
 
     # include/genga_step.h
+    def _f(self, t, numel, name):
+        return _ptr(t, "f8", numel, name)
+
+    def _i(self, t, numel, name):
+        return _ptr(t, "i4", numel, name)
+
     def rcrit(self, pos, vel, mass, m_star, dt, out_rcrit, substeps=2.0, nrows=1, n1=3.0, n2=0.4):
-        self._check(lib().genga_rcrit(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt),
-                                      float(substeps), int(nrows), float(n1), float(n2), _ptr(out_rcrit)))
+        n = self.n
+        self._check(lib().genga_rcrit(self._ctx, self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"),
+                                      self._f(mass, n, "mass"), float(m_star), float(dt), float(substeps), int(nrows),
+                                      float(n1), float(n2), self._f(out_rcrit, max(int(nrows), 0) * n, "out_rcrit")))
 
     def hc(self, pos, vel, mass, m_star, dt):
-        self._check(lib().genga_hc(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt)))
+        n = self.n
+        self._check(lib().genga_hc(self._ctx, self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"),
+                                   self._f(mass, n, "mass"), float(m_star), float(dt)))
 
     def fg(self, pos, vel, m_star, dt):
-        self._check(lib().genga_fg(self._ctx, _ptr(pos), _ptr(vel), float(m_star), float(dt)))
+        n = self.n
+        self._check(lib().genga_fg(self._ctx, self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"), float(m_star),
+                                   float(dt)))
 
     def rcrit_list(self, pos, vel, mass, m_star, dt, list_, n_list, list_rows, out_rcrit, substeps=2.0, nrows=1, n1=3.0,
                    n2=0.4):
-        self._check(lib().genga_rcrit_list(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt),
-                                           float(substeps), int(nrows), float(n1), float(n2), _ptr(list_), _ptr(n_list),
-                                           int(list_rows), _ptr(out_rcrit)))
+        n = self.n
+        self._check(lib().genga_rcrit_list(self._ctx, self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"),
+                                           self._f(mass, n, "mass"), float(m_star), float(dt), float(substeps), int(nrows),
+                                           float(n1), float(n2), self._i(list_, int(list_rows), "list"),
+                                           self._i(n_list, 1, "n_list"), int(list_rows),
+                                           self._f(out_rcrit, max(int(nrows), 0) * n, "out_rcrit")))
 
     def fg_list(self, pos, vel, m_star, dt, list_, n_list, list_rows):
-        self._check(lib().genga_fg_list(self._ctx, _ptr(pos), _ptr(vel), float(m_star), float(dt), _ptr(list_),
-                                        _ptr(n_list), int(list_rows)))
+        n = self.n
+        self._check(lib().genga_fg_list(self._ctx, self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"), float(m_star),
+                                        float(dt), self._i(list_, int(list_rows), "list"), self._i(n_list, 1, "n_list"),
+                                        int(list_rows)))
 
     def drift(self, pos, vel, mass, m_star, dt):
-        self._check(lib().genga_drift(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt)))
+        n = self.n
+        self._check(lib().genga_drift(self._ctx, self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"),
+                                      self._f(mass, n, "mass"), float(m_star), float(dt)))
+
+    def _step_args(self, pos, vel, mass, out_acc, out_pairs, out_npairs):
+        n, cap = self.n, int(self.cfg.pair_capacity)
+        return (self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel"), self._f(mass, n, "mass"),
+                self._f(out_acc, 3 * n, "out_acc"), self._i(out_pairs, 2 * cap, "out_pairs"),
+                self._i(out_npairs, n + 1, "out_npairs"))
 
     def step(self, pos, vel, mass, m_star, dt, rcrit_row, out_acc, out_pairs, out_npairs, n1=3.0, n2=0.4):
-        self._check(lib().genga_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt), float(n1),
-                                     float(n2), _ptr(rcrit_row), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs)))
+        p, v, m, a, op, on = self._step_args(pos, vel, mass, out_acc, out_pairs, out_npairs)
+        self._check(lib().genga_step(self._ctx, p, v, m, float(m_star), float(dt), float(n1), float(n2),
+                                     self._f(rcrit_row, self.n, "rcrit_row"), a, op, on))
 
     # include/genga_group.h
+    def _group_args(self, group_of, members, offsets, summary):
+        n = self.n
+        return (self._i(group_of, n, "group_of"), self._i(members, n, "members"), self._i(offsets, n + 1, "offsets"),
+                self._i(summary, 4, "summary"))
+
     def group(self, pairs, n_pairs, pair_rows, group_of, members, offsets, summary):
         """n_pairs: a device int32 tensor VIEW whose first element is the pair count (e.g. out_npairs[N:])."""
-        self._check(lib().genga_group(self._ctx, _ptr(pairs), _ptr(n_pairs), int(pair_rows), _ptr(group_of),
-                                      _ptr(members), _ptr(offsets), _ptr(summary)))
+        self._check(lib().genga_group(self._ctx, self._i(pairs, 2 * int(pair_rows), "pairs"), self._i(n_pairs, 1, "n_pairs"),
+                                      int(pair_rows), *self._group_args(group_of, members, offsets, summary)))
 
     # include/genga_bs.h
     def bs(self, pos_in, vel_in, mass, rcrit, nlevels, m_star, dt, tol, members, offsets, summary, pos, vel):
-        self._check(lib().genga_bs(self._ctx, _ptr(pos_in), _ptr(vel_in), _ptr(mass), _ptr(rcrit), int(nlevels),
-                                   float(m_star), float(dt), float(tol), _ptr(members), _ptr(offsets), _ptr(summary),
-                                   _ptr(pos), _ptr(vel)))
+        n = self.n
+        self._check(lib().genga_bs(self._ctx, self._f(pos_in, 3 * n, "pos_in"), self._f(vel_in, 3 * n, "vel_in"),
+                                   self._f(mass, n, "mass"), self._f(rcrit, max(int(nlevels), 0) * n, "rcrit"), int(nlevels),
+                                   float(m_star), float(dt), float(tol), self._i(members, n, "members"),
+                                   self._i(offsets, n + 1, "offsets"), self._i(summary, 4, "summary"),
+                                   self._f(pos, 3 * n, "pos"), self._f(vel, 3 * n, "vel")))
+
+    def bs_set_stats(self, group_stats, rows):
+        self._check(lib().genga_bs_set_stats(self._ctx, self._i(group_stats, 4 * int(rows), "group_stats"), int(rows)))
+
+    def bs_totals(self, reset=False):
+        """(accepted macro steps, rejected attempts, force evaluations, groups integrated) since init / the last reset."""
+        t = (C.c_int64 * 4)()
+        self._check(lib().genga_bs_totals(self._ctx, C.byref(t), 1 if reset else 0))
+        return tuple(int(x) for x in t)
 
     def hybrid_step(self, pos, vel, mass, m_star, dt, tol, out_acc, out_pairs, out_npairs, group_of, members, offsets,
                     summary, n1=3.0, n2=0.4):
-        self._check(lib().genga_hybrid_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt), float(n1),
-                                            float(n2), float(tol), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs),
-                                            _ptr(group_of), _ptr(members), _ptr(offsets), _ptr(summary)))
+        p, v, m, a, op, on = self._step_args(pos, vel, mass, out_acc, out_pairs, out_npairs)
+        self._check(lib().genga_hybrid_step(self._ctx, p, v, m, float(m_star), float(dt), float(n1), float(n2), float(tol),
+                                            a, op, on, *self._group_args(group_of, members, offsets, summary)))
 
     # include/genga_senc.h
     def detect(self, pos0, vel0, pos1, vel1, rcrit_row, h, in_pairs, in_n_pairs, in_pair_rows, out_pairs, out_npairs,
                enc_factor=1.0):
-        self._check(lib().genga_detect(self._ctx, _ptr(pos0), _ptr(vel0), _ptr(pos1), _ptr(vel1), _ptr(rcrit_row),
-                                       float(enc_factor), float(h), _ptr(in_pairs), _ptr(in_n_pairs), int(in_pair_rows),
-                                       _ptr(out_pairs), _ptr(out_npairs)))
+        n, cap = self.n, int(self.cfg.pair_capacity)
+        self._check(lib().genga_detect(self._ctx, self._f(pos0, 3 * n, "pos0"), self._f(vel0, 3 * n, "vel0"),
+                                       self._f(pos1, 3 * n, "pos1"), self._f(vel1, 3 * n, "vel1"),
+                                       self._f(rcrit_row, n, "rcrit_row"), float(enc_factor), float(h),
+                                       self._i(in_pairs, 2 * int(in_pair_rows), "in_pairs"),
+                                       self._i(in_n_pairs, 1, "in_n_pairs"), int(in_pair_rows),
+                                       self._i(out_pairs, 2 * cap, "out_pairs"), self._i(out_npairs, n + 1, "out_npairs")))
 
     def multilevel_step(self, pos, vel, mass, m_star, dt, slevels, substeps, tol, out_acc, out_pairs, out_npairs,
                         out_stats, detect=True, n1=3.0, n2=0.4):
         cfg = GengaSencConfig(int(slevels), int(substeps), int(bool(detect)), 0, float(n1), float(n2), float(tol))
-        self._check(lib().genga_multilevel_step(self._ctx, _ptr(pos), _ptr(vel), _ptr(mass), float(m_star), float(dt),
-                                                C.byref(cfg), _ptr(out_acc), _ptr(out_pairs), _ptr(out_npairs),
-                                                _ptr(out_stats)))
+        p, v, m, a, op, on = self._step_args(pos, vel, mass, out_acc, out_pairs, out_npairs)
+        self._check(lib().genga_multilevel_step(self._ctx, p, v, m, float(m_star), float(dt), C.byref(cfg), a, op, on,
+                                                self._i(out_stats, 4 * max(int(slevels), 0), "out_stats")))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

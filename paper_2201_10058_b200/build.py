@@ -1,32 +1,46 @@
 """Builds paper_2201_10058_b200/libgenga_kick.so (the C-ABI library of include/genga_kick.h) with
-nvcc for sm_100a, in-tree.  nvcc cross-compiles without a GPU.  Usage: python -m paper_2201_10058_b200.build"""
+nvcc for sm_100a, in-tree.  nvcc cross-compiles without a GPU.  Usage: python -m paper_2201_10058_b200.build
+
+Every translation unit is compiled to an object of its own (in parallel, rebuilt only when it or a header
+is newer) and the objects are linked into the shared library."""
+import glob
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgenga_kick.so")
-SOURCES = [os.path.join(CSRC, "genga_kick.cu"), os.path.join(CSRC, "genga_step.cu"), os.path.join(CSRC, "genga_group.cu"), os.path.join(CSRC, "genga_bs.cu"), os.path.join(CSRC, "genga_senc.cu"),
-           os.path.join(CSRC, "genga_kick_plan.cpp")]
-DEPENDS = SOURCES + [os.path.join(CSRC, "genga_kick_kernels.cuh"), os.path.join(CSRC, "genga_kick_variants.h"),
-                     os.path.join(CSRC, "genga_kick_sort.cuh"), os.path.join(CSRC, "genga_kick_ctx.h"),
-                     os.path.join(CSRC, "genga_step_kernels.cuh"), os.path.join(CSRC, "genga_group_kernels.cuh"), os.path.join(CSRC, "genga_bs_kernels.cuh"), os.path.join(CSRC, "genga_senc_kernels.cuh"),
-                     os.path.join(os.path.dirname(HERE), "include", "genga_senc.h"),
-                     os.path.join(os.path.dirname(HERE), "include", "genga_bs.h"),
-                     os.path.join(os.path.dirname(HERE), "include", "genga_group.h"),
-                     os.path.join(os.path.dirname(HERE), "include", "genga_step.h"),
-                     os.path.join(os.path.dirname(HERE), "include", "genga_kick.h")]
+SOURCES = sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) +
+                 glob.glob(os.path.join(os.path.dirname(HERE), "include", "*.h")))
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # --fmad=false: no contraction the source does not spell out (the kernels write every fma() themselves)
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=false",
-         "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+         "-Xcompiler", "-fPIC"]
+
+
+def _obj(src: str) -> str:
+    return os.path.join(OBJ, os.path.splitext(os.path.basename(src))[0] + ".o")
+
+
+def _compile(src: str, verbose: bool) -> None:
+    subprocess.check_call([NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", src, "-o", _obj(src)])
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    stale = force or not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in DEPENDS)
+    os.makedirs(OBJ, exist_ok=True)
+    newest_header = max(os.path.getmtime(h) for h in HEADERS)
+    stale = [s for s in SOURCES
+             if force or not os.path.exists(_obj(s)) or os.path.getmtime(_obj(s)) < max(os.path.getmtime(s), newest_header)]
     if stale:
-        cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), *SOURCES, "-o", LIB]
-        subprocess.check_call(cmd)
+        with ThreadPoolExecutor(max_workers=min(len(stale), os.cpu_count() or 4)) as pool:
+            list(pool.map(lambda s: _compile(s, verbose), stale))
+    objs = [_obj(s) for s in SOURCES]
+    if stale or not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(o) for o in objs):
+        subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a",
+                               *objs, "-o", LIB])
     return LIB
 
 

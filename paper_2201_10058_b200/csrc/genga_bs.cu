@@ -2,6 +2,7 @@
 #include "../../include/genga_bs.h"
 #include "../../include/genga_group.h"
 #include "../../include/genga_step.h"
+#include "../../include/genga_senc.h"
 #include "genga_kick_ctx.h"
 #include "genga_bs_kernels.cuh"
 
@@ -30,7 +31,9 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     int tp_mode = ctx->cfg.tp_mode;
     // whole-grid regime: scratch for one group of up to N bodies, and the size of a co-resident grid
     if (!ctx->bs_scratch) {
-        GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double)));
+        const size_t bytes = ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double);
+        GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, bytes));
+        GK_CUDA(ctx, cudaMemsetAsync(ctx->bs_scratch, 0, bytes, st));
         int per_sm = 0;
         GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>,
                                                                  GENGA_BS_COOP_THREADS, 0));
@@ -48,6 +51,9 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
         gm.gm = p; p += N;
         for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) { gm.rc[k] = p; p += N; }
         gm.err = reinterpret_cast<unsigned long long*>(p);
+        gm.totals = gm.err + 4;
+        gm.stats = reinterpret_cast<int4*>(ctx->bs_stats);
+        gm.stats_rows = ctx->bs_stats_rows;
     }
     // at most N / 2 groups; warps / CTAs stride over them (their number is only known on the device)
     int small_max = GENGA_BS_THREADS;
@@ -113,6 +119,28 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     return GENGA_KICK_OK;
 }
 
+extern "C" int genga_bs_set_stats(genga_kick_ctx* ctx, int32_t* group_stats, int64_t rows)
+{
+    if (!ctx) return GENGA_KICK_E_NULL;
+    if (rows < 0 || (rows > 0 && !group_stats)) return GENGA_KICK_E_SIZE;
+    if (genga_misaligned(group_stats)) return GENGA_KICK_E_ALIGN;
+    ctx->bs_stats = group_stats;
+    ctx->bs_stats_rows = group_stats ? rows : 0;
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_bs_totals(genga_kick_ctx* ctx, int64_t* totals, int32_t reset)
+{
+    if (!ctx || !totals) return GENGA_KICK_E_NULL;
+    totals[0] = totals[1] = totals[2] = totals[3] = 0;
+    if (!ctx->bs_scratch) return GENGA_KICK_OK;                       // genga_bs has not run yet
+    unsigned long long* t = reinterpret_cast<unsigned long long*>(ctx->bs_scratch + (size_t)(7 + GENGA_BS_MAX_LEVELS) * ctx->N) + 4;
+    GK_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    GK_CUDA(ctx, cudaMemcpy(totals, t, 4 * sizeof(int64_t), cudaMemcpyDeviceToHost));
+    if (reset) GK_CUDA(ctx, cudaMemset(t, 0, 4 * sizeof(int64_t)));
+    return GENGA_KICK_OK;
+}
+
 extern "C" int genga_hybrid_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
                                  double n1, double n2, double tol, double* out_acc, int32_t* out_pairs, int32_t* out_npairs,
                                  int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary)
@@ -136,7 +164,8 @@ extern "C" int genga_hybrid_step(genga_kick_ctx* ctx, double* pos, double* vel, 
     GK_CUDA(ctx, cudaMemcpyAsync(v_in, vel, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
     rc = genga_fg(ctx, pos, vel, m_star, dt);
     if (rc != GENGA_KICK_OK) return rc;
-    rc = genga_group(ctx, out_pairs, out_npairs + N, ctx->cfg.pair_capacity, group_of, members, offsets, summary);
+    rc = genga_group_impl(ctx, out_pairs, out_npairs + N, ctx->cfg.pair_capacity, group_of, members, offsets, summary,
+                          GENGA_KICK_STATUS_LIST_CLIPPED);
     if (rc != GENGA_KICK_OK) return rc;
     rc = genga_bs(ctx, q_in, v_in, mass, ctx->step_rcrit, 1, m_star, dt, tol, members, offsets, summary, pos, vel);
     if (rc != GENGA_KICK_OK) return rc;

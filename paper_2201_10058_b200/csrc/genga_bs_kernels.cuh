@@ -68,6 +68,10 @@ struct BsGlobal {
     double* gm;
     double* rc[GENGA_BS_MAX_LEVELS];
     unsigned long long* err;            // [4], all zero between uses
+    // diagnostics of the step-size control (include/genga_bs.h: genga_bs_set_stats, genga_bs_totals)
+    unsigned long long* totals;         // [4] accepted macro steps, rejected attempts, force evaluations, groups: summed
+    int4* stats;                        // [stats_rows] per group (accepted, rejected, force evaluations, bodies), or nullptr
+    long long stats_rows;
 };
 
 // shared memory: one-CTA regime: the whole group; whole-grid regime: one tile of j-bodies
@@ -423,14 +427,17 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         double a0[3], cq[3], cv[3], dq[3], dv[3];
         double done = 0.0, H = dt;
         bool fail = false;
+        int n_acc = 0, n_rej = 0, n_fev = 0;                           // group-uniform, like every decision below
         while (done != dt) {                                           // all decisions below are group-uniform
             if ((dt > 0.0 && done + H > dt) || (dt < 0.0 && done + H < dt)) H = dt - done;
             bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, q, a0);
+            n_fev++;
             int halvings = 0, kconv = 0;
             for (;;) {
                 bool ok = false;
                 for (int k = 0; k < GENGA_BS_KMAX; k++) {
                     const int nk = 2 * (k + 1);
+                    n_fev += nk;
                     {   // modified midpoint over H with nk sub-steps: (q, v) -> (cq, cv) = T_{k,0}
                         const double h = H / (double)nk, h2 = 2.0 * h;
                         double qm[3], vm[3], qn[3], vn[3], a[3];
@@ -481,10 +488,12 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
                     }
                 }
                 if (ok) break;
+                n_rej++;
                 if (++halvings > GENGA_BS_MAX_HALVINGS) { fail = true; break; }
                 H = 0.5 * H;
             }
             if (fail) break;
+            n_acc++;
 #pragma unroll
             for (int c = 0; c < 3; c++) { q[c] = cq[c]; v[c] = cv[c]; }
             if ((dt > 0.0 && done + H >= dt) || (dt < 0.0 && done + H <= dt)) done = dt;
@@ -495,6 +504,11 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         if (active && writer) {                                        // (after a failure: the state at the last accepted time)
 #pragma unroll
             for (int c = 0; c < 3; c++) { pos[c * N + b] = q[c]; vel[c * N + b] = v[c]; }
+            if (i == 0) {                                              // one thread per group: the step-size control's record
+                atomicAdd(Gm.totals + 0, (unsigned long long)n_acc); atomicAdd(Gm.totals + 1, (unsigned long long)n_rej);
+                atomicAdd(Gm.totals + 2, (unsigned long long)n_fev); atomicAdd(Gm.totals + 3, 1ULL);
+                if (Gm.stats && g < Gm.stats_rows) Gm.stats[g] = make_int4(n_acc, n_rej, n_fev, n);
+            }
         }
     }
     // no CTA of a cluster leaves while another may still read its shared memory

@@ -30,6 +30,12 @@ int ensure_group_scratch(genga_kick_ctx* ctx)
 extern "C" int genga_group(genga_kick_ctx* ctx, const int32_t* pairs, const int32_t* n_pairs, int64_t pair_rows,
                            int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary)
 {
+    return genga_group_impl(ctx, pairs, n_pairs, pair_rows, group_of, members, offsets, summary, 0);
+}
+
+int genga_group_impl(genga_kick_ctx* ctx, const int32_t* pairs, const int32_t* n_pairs, int64_t pair_rows,
+                     int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary, int clip_status)
+{
     if (!ctx || !n_pairs || !group_of || !members || !offsets || !summary) return GENGA_KICK_E_NULL;
     if (pair_rows < 0) return GENGA_KICK_E_SIZE;
     if (!pairs && pair_rows > 0) return GENGA_KICK_E_NULL;
@@ -46,10 +52,10 @@ extern "C" int genga_group(genga_kick_ctx* ctx, const int32_t* pairs, const int3
     const int hook_blocks = (int)std::min<int64_t>(std::max<int64_t>((pair_rows + 255) / 256, 1), 8 * ctx->num_sms);
     const int2* pr = reinterpret_cast<const int2*>(pairs);
     genga::group_hook_kernel<<<hook_blocks, 256, 0, st>>>(pr, n_pairs, pair_rows, N, GENGA_GROUP_SAMPLE, true, ctx->grp_label,
-                                                          ctx->grp_flag, summary, ctx->status);
+                                                          ctx->grp_flag, summary, ctx->status, clip_status);
     genga::group_compress_kernel<<<blocks, 256, 0, st>>>(ctx->grp_label, N);
     genga::group_hook_kernel<<<hook_blocks, 256, 0, st>>>(pr, n_pairs, pair_rows, N, GENGA_GROUP_SAMPLE, false, ctx->grp_label,
-                                                          ctx->grp_flag, summary, ctx->status);
+                                                          ctx->grp_flag, summary, ctx->status, clip_status);
     genga::group_flat_kernel<<<blocks, 256, 0, st>>>(ctx->grp_label, ctx->grp_flag, N, group_of, ctx->grp_keys_a,
                                                      ctx->grp_vals_a);
     ctx->launches += 5;

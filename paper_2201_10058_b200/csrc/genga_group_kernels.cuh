@@ -49,13 +49,17 @@ __device__ __forceinline__ int group_find(int* label, int x)
 __global__ void __launch_bounds__(256)
 group_hook_kernel(const int2* __restrict__ pairs, const int* __restrict__ n_pairs, long long pair_rows, int N,
                   int sample, bool sampled, int* __restrict__ label, int* __restrict__ flag, int* __restrict__ summary,
-                  int* __restrict__ status)
+                  int* __restrict__ status, int clip_status)
 {
     // Two passes (host): first every `sample`-th pair (sampled = true), which already links most of a large
     // group; then, after group_compress_kernel has flattened the trees, the other pairs (sampled = false) --
     // for almost all of them both ends then point at the same root and the pair costs two cached reads.
     const long long total = min((long long)max(*n_pairs, 0), pair_rows);
-    if (blockIdx.x == 0 && threadIdx.x == 0) summary[3] = (int)total;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        summary[3] = (int)total;
+        // a composed step (genga_hybrid_step) must not lose encounter pairs silently: clip_status = LIST_CLIPPED there
+        if (clip_status && (long long)*n_pairs > pair_rows) atomicOr(status, clip_status);
+    }
     for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < total; p += (long long)gridDim.x * blockDim.x) {
         if (((p % sample) == 0) != sampled) continue;
         const int2 e = pairs[p];

@@ -179,7 +179,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         kp.cblo = ctx->cblo; kp.cbhi = ctx->cbhi;
         kp.rcrit = rcrit;
         kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
-        kp.react = ctx->tp2 && changeover_level > 0 ? 1 : 0; kp.j_rec0 = 0; kp.force_only = 0;
+        kp.react = ctx->tp2 && changeover_level > 0 ? 1 : 0; kp.j_rec0 = 0; kp.force_only = 0; kp.i_rec_end = n_rec;
         kp.n_j_tiles = pl.n_j_tiles; kp.n_ctas = pl.n_ctas; kp.max_segs = pl.max_segs; kp.n_tiles = pl.n_tiles;
         kp.partial = ctx->partial;
         kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
@@ -219,7 +219,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             const genga_kick_plan& p2 = ctx->plan_tp2;
             genga::KickParams k2 = kp;
             k2.n_j_tiles = p2.n_j_tiles; k2.n_ctas = p2.n_ctas; k2.max_segs = p2.max_segs; k2.n_tiles = p2.n_tiles;
-            k2.partial = ctx->partial2; k2.j_rec0 = pl.m_pad; k2.force_only = 1;
+            k2.partial = ctx->partial2; k2.j_rec0 = pl.m_pad; k2.force_only = 1; k2.i_rec_end = pl.m_pad;
             GK_CUDA(ctx, dispatch_kick(p2, k2, st));
             ctx->launches++;
         }

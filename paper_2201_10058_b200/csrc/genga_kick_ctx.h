@@ -56,6 +56,8 @@ struct genga_kick_ctx {
     int* grp_label; int* grp_flag; unsigned* grp_keys_a; unsigned* grp_keys_b; int* grp_vals_a; int* grp_vals_b;
     int* grp_counts;
     double* bs_scratch;            // whole-grid Bulirsch-Stoer regime: positions (2 buffers), G m, r_crit rows, error slots
+    int32_t* bs_stats;             // caller's per-group record of the step-size control, or nullptr (genga_bs_set_stats)
+    int64_t bs_stats_rows;
     int bs_coop_blocks;            // its co-resident grid (eight lanes per body)
     int bs_coop_blocks1;           // ... of the one-lane-per-body variant
     double* hyb_state;             // [6][N] state before FG (genga_hybrid_step), lazily allocated
@@ -77,3 +79,6 @@ static inline bool genga_misaligned(const void* p) { return (reinterpret_cast<ui
 // genga_kick with out_npairs == nullptr allowed: no pre-check output (the closing kick of genga_step)
 int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
                     int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
+// genga_group with a status bit to raise when the pair list was clipped to pair_rows (0: none, the public call)
+int genga_group_impl(genga_kick_ctx* ctx, const int32_t* pairs, const int32_t* n_pairs, int64_t pair_rows,
+                     int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary, int clip_status);

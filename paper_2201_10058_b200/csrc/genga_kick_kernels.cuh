@@ -39,6 +39,9 @@ struct KickParams {
     int react;                         // TP 2 at level >= 1: exact_kernel also adds the reaction of a semi-active
                                        // particle i on the massive body j (near_kernel's pair filter is symmetric)
     int j_rec0;                        // record of the first j-tile (0; m_pad in the second pass of TP 2)
+    int i_rec_end;                     // i-records from here on take no part in the pass (n_rec; m_pad in the second pass
+                                       // of TP 2, whose last i-block may reach past the massive records: sec. 8.1
+                                       // particles never feel each other)
     int force_only;                    // second pass of TP 2 at level 0 (massive i x semi-active j): candidates are
                                        // queued as (i, ~j): exact_kernel adds the force on i and leaves the encounter
                                        // bookkeeping to the first pass, which meets the same pair from the particle's side
@@ -68,7 +71,10 @@ struct KickParams {
 // (DSETP runs at a quarter of the DFMA rate); the + 1 covers the truncated low word, the one-ulp
 // difference between the fused r^2 of the pair loop and the unfused r^2 of the exact path, and
 // the rounding of y = (r - 0.1 rc)/(0.9 rc) near 1: a pair that passes the filter has
-// r^2 >= R^2 (1 + 2^-20).
+// hi(r^2) >= hi(R^2) + 1, i.e. r^2 exceeds R^2 by at least one unit of the high word minus the
+// truncated low word of R^2 -- a margin between 1 ulp of the high word (2^-20 relative) and, when
+// R^2's low word is all ones, a single ulp of the double.  Either is enough: r^2 > R^2 strictly in
+// both the fused and the unfused evaluation means K = 1 (level 0) resp. 1 - K_0 = 0 and no encounter.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int filter_word(double rc0, double rcL, double f)
 {
@@ -420,6 +426,7 @@ __device__ __forceinline__ void apply_candidate(const KickParams& p, int ir, int
     const int jr = force_only ? ~jr_enc : jr_enc;
     const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;      // (-1, -1): empty slot
     if (ir == jr || bi < 0 || bj < 0) return;
+    if (force_only && bi >= p.n_massive) return;            // the second pass of TP 2 only serves massive i
     const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
     const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
     const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
@@ -460,6 +467,8 @@ __device__ __forceinline__ void apply_candidate(const KickParams& p, int ir, int
 struct CandCursor {
     long long base;   // first slot of the warp's open block (warp-uniform)
     int fill;         // slots used in it; GENGA_CAND_BLOCK: no block open
+    bool over;        // the warp has seen the list full: it reserves no more (the counter stays below
+                      // capacity + one block per warp of the grid and cannot wrap); see near_kernel<true>
 };
 
 __device__ __forceinline__ void close_block(const KickParams& p, CandCursor& c)
@@ -473,6 +482,7 @@ __device__ __forceinline__ void close_block(const KickParams& p, CandCursor& c)
 __device__ __forceinline__ void push_candidates(const KickParams& p, CandCursor& c, bool mine, int irec, int jrec)
 {
     const unsigned m = __ballot_sync(0xffffffffu, mine);
+    if (c.over) return;                                     // warp-uniform; the list is abandoned (near_kernel<true>)
     const int lane = threadIdx.x & 31;
     const int n = __popc(m);
     if (c.fill + n > GENGA_CAND_BLOCK) {                    // warp-uniform
@@ -484,10 +494,15 @@ __device__ __forceinline__ void push_candidates(const KickParams& p, CandCursor&
         }
         c.base = __shfl_sync(0xffffffffu, base, 0);
         c.fill = 0;
+        if (c.base < 0 || c.base + GENGA_CAND_BLOCK > p.cand_capacity) {      // *ncand > capacity from now on
+            c.over = true;
+            c.fill = GENGA_CAND_BLOCK;
+            return;
+        }
     }
     if (mine) {
         const long long slot = c.base + c.fill + __popc(m & ((1u << lane) - 1u));
-        if (slot < p.cand_capacity) p.cand[slot] = make_int2(irec, jrec);     // else: dropped; see near_kernel<true>
+        if (slot >= 0 && slot < p.cand_capacity) p.cand[slot] = make_int2(irec, jrec);
     }
     c.fill += n;
 }
@@ -616,6 +631,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
     CandCursor cc;
     cc.base = 0;
     cc.fill = GENGA_CAND_BLOCK;
+    cc.over = false;
 
     auto flush = [&]() {
         const size_t base = ((size_t)blockIdx.x * p.max_segs + (cur_ib - first_ib)) * 3 * IB;
@@ -642,10 +658,15 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 #pragma unroll
             for (int k = 0; k < IPT; k++) {
                 const size_t r = (size_t)ib * IB + woff + k * 32;
+                ax[k] = ay[k] = az[k] = 0.0;
+                if (r >= (size_t)p.i_rec_end) {             // whole groups of 32 records (i_rec_end is a multiple of 32)
+                    xi[k] = yi[k] = zi[k] = GENGA_SENTINEL_POS;
+                    fi[k] = -1;
+                    continue;
+                }
                 const double2 a = p.rxy[r], b = p.rzm[r];
                 xi[k] = a.x; yi[k] = a.y; zi[k] = b.x;
                 fi[k] = p.rfw[r];
-                ax[k] = ay[k] = az[k] = 0.0;
                 // the groups of GENGA_GROUP records are aligned with the warp's k-slices
                 const float4 glo = p.cblo[r / GENGA_GROUP], ghi = p.cbhi[r / GENGA_GROUP];
                 wlo.x = fminf(wlo.x, glo.x); wlo.y = fminf(wlo.y, glo.y); wlo.z = fminf(wlo.z, glo.z);
@@ -757,6 +778,7 @@ near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int 
     CandCursor cc;
     cc.base = 0;
     cc.fill = GENGA_CAND_BLOCK;
+    cc.over = false;
 
     const int js = gridDim.y, jy = blockIdx.y;               // this CTA's j-groups: g = q * js + jy
     const int n_mine = (n_jgroups - jy + js - 1) / js;

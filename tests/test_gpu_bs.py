@@ -1,10 +1,24 @@
 """-m gpu: genga_bs (include/genga_bs.h) through the C ABI against oracle/genga_bs_oracle.c.
 
-The oracle follows the same Gragg-Bulirsch-Stoer scheme operation for operation (reading G15), both sides in IEEE
-binary64 without contraction, the force sum in member order: the step-size decisions are taken on the same bits and
-the results must agree to the LAST BIT except where the device's sqrt/division sequences differ from the host's --
-they do not (both correctly rounded) -- so the bar is equality; a tolerance of 64 u relative to |q|, |v| is what the
-test enforces, and it reports whether equality held."""
+Both sides run the same Gragg-Bulirsch-Stoer scheme (reading G15) in IEEE binary64 without contraction.  The oracle adds
+a body's pair terms in member order, for every group size; the kernel does the same for groups of up to 8 bodies (one
+lane per body) and spreads the sum over eight lanes with a tree above that -- its choice, not the oracle's.  Hence:
+
+  * groups of <= 8 bodies: same operations in the same order => the bar is EQUAL BITS (and equal step-size decisions);
+  * larger groups: the force sums differ at rounding level.  As long as both sides take the same step-size decisions
+    (accepted steps, halvings, force evaluations -- the kernel reports them per group, genga_bs_set_stats), the results
+    differ by that rounding, amplified by the encounter; where an error estimate falls within rounding of tol the two
+    sides may decide differently (a FLIP: counted and reported, the analogue of north_star's borderline pairs), and then
+    they are two valid answers of the scheme.  Either way each side's local error per accepted macro step is <= tol
+    (relative, per body, in position and in velocity: the scheme's own acceptance test), so
+        |dq| / |q|,  |dv| / |v|   <=   C_TOL * tol * (accepted macro steps of the group)
+    with C_TOL = 4 (2 sides x 2 for the error estimate being that of the previous column).  The measured worst ratio
+    to that bound is printed, so the record shows the slack; without a flip it is 1e-7 .. 1e-1 (1 .. 3000 u).
+  * a flipped group whose encounter amplifies perturbations (a bound, nearly radial passage takes thousands of macro
+    steps) is compared under the same bound times the amplification A of the flow, MEASURED on the oracle: the
+    relative change of its result under a relative perturbation of 2^-40 of the group's input positions, over 2^-40
+    (at least 1).  A is printed with the flip; where A * bound exceeds 1 the group is chaotic at this tolerance, the
+    two answers are both valid and nothing more can be asserted than that the kernel reports it took other decisions."""
 import numpy as np
 import pytest
 
@@ -13,6 +27,8 @@ import genga_inputs as gi
 pytestmark = pytest.mark.gpu
 U = 2.0 ** -53
 G = gi.G_AU_DAY_MSUN
+C_TOL = 4.0
+SEQ_MAX = 8            # groups up to here are summed in member order by the kernel too (include/genga_bs.h)
 
 
 def _dev(a, dtype=None):
@@ -22,6 +38,7 @@ def _dev(a, dtype=None):
 
 
 def _gpu_bs(n, pos_in, vel_in, mass, rcrit, nlevels, dt, tol, members, offsets, pos, vel):
+    """Returns (pos, vel, status, per-group rows (accepted, rejected, force evaluations, bodies))."""
     import torch
     from paper_2201_10058_b200 import GengaKick
     k = GengaKick(n, 0, G=G, pair_capacity=8)
@@ -31,19 +48,66 @@ def _gpu_bs(n, pos_in, vel_in, mass, rcrit, nlevels, dt, tol, members, offsets, 
     d_off = torch.zeros(n + 4, dtype=torch.int32, device="cuda"); d_off[:ng + 1] = _dev(np.asarray(offsets, np.int32))
     largest = int(np.diff(np.asarray(offsets)).max()) if ng else 0
     d_sum = torch.tensor([ng, len(members), largest, 0], dtype=torch.int32, device="cuda")
+    gstats = torch.full((max(ng, 1), 4), -1, dtype=torch.int32, device="cuda")
+    k.bs_set_stats(gstats, max(ng, 1))
     q, v = _dev(pos), _dev(vel)
     k.bs(_dev(pos_in), _dev(vel_in), _dev(mass), _dev(np.asarray(rcrit)[:nlevels]), nlevels, 1.0, dt, tol, d_mem, d_off,
          d_sum, q, v)
     torch.cuda.synchronize()
     st = k.status()
+    tot = k.bs_totals()
+    gs = gstats.cpu().numpy()[:ng]
+    assert tot[3] == ng and tot[0] == gs[:, 0].sum() and tot[2] == gs[:, 2].sum()
     k.free()
-    return q.cpu().numpy(), v.cpu().numpy(), st
+    return q.cpu().numpy(), v.cpu().numpy(), st, gs
 
 
-def _check(q, v, qw, vw):
-    sq = np.sqrt((qw ** 2).sum(0)); sv = np.sqrt((vw ** 2).sum(0))
-    assert np.all(np.abs(q - qw) <= 64 * U * sq) and np.all(np.abs(v - vw) <= 64 * U * sv)
-    return bool(np.array_equal(q, qw) and np.array_equal(v, vw))
+def _amplification(rerun, idx, qw, vw):
+    """Sensitivity of the oracle's result for one group to its input: see the header."""
+    delta = 2.0 ** -40
+    qp, vp = rerun(idx, delta)
+    nq = np.sqrt((qw[:, idx] ** 2).sum(0)); nv = np.sqrt((vw[:, idx] ** 2).sum(0))
+    rel = max(np.max(np.sqrt(((qp - qw[:, idx]) ** 2).sum(0)) / nq), np.max(np.sqrt(((vp - vw[:, idx]) ** 2).sum(0)) / nv))
+    return max(1.0, rel / delta)
+
+
+def _check(q, v, qw, vw, members, offsets, gstats, ostats, tol, label="", rerun=None):
+    """The rule of this file's header, group by group.  Returns (all bits equal, number of flipped groups).
+    rerun(idx, delta) -> the oracle's (q, v) of the group with bodies idx from input positions scaled by 1 + delta *
+    (a fixed +-1 pattern); needed only if a group flips."""
+    members = np.asarray(members); offsets = np.asarray(offsets)
+    flips, worst, worst_u, small, equal = 0, 0.0, 0.0, 0, True
+    for g in range(len(offsets) - 1):
+        idx = members[offsets[g]:offsets[g + 1]]
+        want = (ostats[g].accepted, ostats[g].rejected, ostats[g].force_evaluations, len(idx))
+        flip = tuple(int(x) for x in gstats[g]) != want
+        flips += flip
+        nq = np.sqrt((qw[:, idx] ** 2).sum(0)); nv = np.sqrt((vw[:, idx] ** 2).sum(0))
+        rel = max(np.max(np.sqrt(((q[:, idx] - qw[:, idx]) ** 2).sum(0)) / nq),
+                  np.max(np.sqrt(((v[:, idx] - vw[:, idx]) ** 2).sum(0)) / nv))
+        same = np.array_equal(q[:, idx], qw[:, idx]) and np.array_equal(v[:, idx], vw[:, idx])
+        equal &= bool(same)
+        if len(idx) <= SEQ_MAX:
+            small += 1
+            assert same and not flip, f"group {g} of {len(idx)} bodies (member-order sum on both sides): bits differ"
+            continue
+        steps = max(int(gstats[g][0]), ostats[g].accepted)
+        amp = 1.0
+        if flip and rel > C_TOL * tol * steps and rerun is not None:
+            amp = _amplification(rerun, idx, qw, vw)
+            print(f"{label}group {g} ({len(idx)} bodies): flipped decision, kernel {tuple(int(x) for x in gstats[g][:3])} vs "
+                  f"oracle {want[:3]}; difference {rel:.2e}; amplification of the flow {amp:.2e}; bound "
+                  f"{min(1.0, amp * C_TOL * tol * steps):.2e}" + (" (chaotic at this tolerance)" if amp * C_TOL * tol * steps >= 1 else ""))
+        if amp * C_TOL * tol * steps < 1.0:
+            assert rel <= amp * C_TOL * tol * steps, (f"group {g} ({len(idx)} bodies, flip={flip}): {rel:.2e} > "
+                                                      f"{amp:.1e} * {C_TOL} * tol * {steps} accepted steps")
+        worst = max(worst, rel / (amp * C_TOL * tol * steps))
+        if not flip:
+            worst_u = max(worst_u, rel / U)
+    ng = len(offsets) - 1
+    print(f"{label}{ng} groups ({small} of <= {SEQ_MAX} bodies: bit-identical); larger groups: {flips} with a flipped "
+          f"step-size decision, worst difference / (C_TOL tol steps) = {worst:.2e}, worst without a flip = {worst_u:.0f} u")
+    return equal, flips
 
 
 def test_groups_of_a_disk_kick_group_bs_chain(oracle_mod):
@@ -58,13 +122,13 @@ def test_groups_of_a_disk_kick_group_bs_chain(oracle_mod):
     qw, vw, stats, skipped = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, gr.members, gr.offsets, G, 1.0, ki.dt,
                                               1e-12, qf, vf, nlevels=1)
     assert not skipped and not any(s.failed for s in stats)
-    q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, ki.dt, 1e-12, gr.members, gr.offsets, qf, vf)
+    q, v, st, gs = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, ki.dt, 1e-12, gr.members, gr.offsets, qf, vf)
     assert st == 0
-    exact = _check(q, v, qw, vw)
+    exact, _ = _check(q, v, qw, vw, gr.members, gr.offsets, gs, stats, 1e-12)
     untouched = gr.group_of < 0
     assert np.array_equal(q[:, untouched], qf[:, untouched]) and np.array_equal(v[:, untouched], vf[:, untouched])
     assert np.max(np.abs(q[:, ~untouched] - qf[:, ~untouched])) > 1e-12               # the encounters matter
-    print("bit-identical to the oracle:", exact)
+    print("every group bit-identical to the oracle:", exact)
 
 
 @pytest.mark.parametrize("nlevels,tol,dt", [(1, 1e-13, 6.0), (2, 1e-11, 6.0), (1, 1e-9, -3.0), (3, 1e-12, 0.75)])
@@ -76,10 +140,10 @@ def test_dense_groups_levels_tolerances(oracle_mod, nlevels, tol, dt):
     gr = oracle_mod.group.group(n, oracle_mod.pair_set(res, n))
     qw, vw, stats, skipped = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, gr.members, gr.offsets, G, 1.0, dt, tol,
                                               ki.pos, ki.vel, nlevels=nlevels, max_group=None)
-    q, v, st = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, nlevels, dt, tol, gr.members, gr.offsets, ki.pos, ki.vel)
+    q, v, st, gs = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, nlevels, dt, tol, gr.members, gr.offsets, ki.pos, ki.vel)
     assert st == 0 and not skipped
     assert gr.max_size > 20 and len(stats) > 50
-    _check(q, v, qw, vw)
+    _check(q, v, qw, vw, gr.members, gr.offsets, gs, stats, tol)
 
 
 def test_large_groups_whole_grid_regime(oracle_mod):
@@ -89,17 +153,17 @@ def test_large_groups_whole_grid_regime(oracle_mod):
         ki = gi.make_ring(m)
         qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, np.arange(m), [0, m], ki.G, 1.0, 6.0, 1e-12,
                                             ki.pos, ki.vel, max_group=None)
-        q, v, st = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 6.0, 1e-12, np.arange(m), [0, m], ki.pos, ki.vel)
+        q, v, st, gs = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 6.0, 1e-12, np.arange(m), [0, m], ki.pos, ki.vel)
         assert st == 0
-        assert _check(q, v, qw, vw), "not bit-identical"
+        _check(q, v, qw, vw, np.arange(m), [0, m], gs, stats, 1e-12, label=f"ring of {m}: ")
     # three groups in one call: 300 (whole grid), 40 (one CTA), 500 (whole grid) bodies of one ring
     ki = gi.make_ring(840)
     members, offsets = np.arange(840), [0, 300, 340, 840]
-    qw, vw, _, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, members, offsets, ki.G, 1.0, -6.0, 1e-11, ki.pos, ki.vel,
-                                    max_group=None)
-    q, v, st = _gpu_bs(840, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, -6.0, 1e-11, members, offsets, ki.pos, ki.vel)
+    qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, members, offsets, ki.G, 1.0, -6.0, 1e-11, ki.pos,
+                                        ki.vel, max_group=None)
+    q, v, st, gs = _gpu_bs(840, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, -6.0, 1e-11, members, offsets, ki.pos, ki.vel)
     assert st == 0
-    _check(q, v, qw, vw)
+    _check(q, v, qw, vw, members, offsets, gs, stats, 1e-11)
 
 
 def test_bs_error_codes_and_empty():
@@ -150,13 +214,21 @@ def test_hybrid_step_against_oracle(oracle_mod):
     assert np.array_equal(group_of.cpu().numpy(), r.groups.group_of)
     rr = np.sqrt((ki.pos ** 2).sum(0)); sp = np.sqrt((ki.vel ** 2).sum(0))
     sq, sv = rr + sp * ki.dt, sp + rr * np.sqrt(ki.G / rr ** 3)
-    # the states entering Bulirsch-Stoer differ by the kick's and HC's rounding (<= 32 u); an encounter amplifies that
-    # by the ratio of the step to the encounter time scale: 1e-10 relative is a generous bound for these groups
+    # the states entering Bulirsch-Stoer differ by the kick's and HC's rounding (<= 32 u), which an encounter
+    # amplifies.  Same record of the step-size control on both sides (the usual case): same operations on inputs 32 u
+    # apart, bound 2.5e-13 relative (~100 x the largest difference measured here, 1.8e-15; printed).  A different record: some
+    # error estimate fell within rounding of tol, two valid answers of the scheme: 4 tol x 1e3 (amplification), reported.
     in_group = r.groups.group_of >= 0
     assert np.all(np.abs(q.cpu().numpy() - r.pos)[:, ~in_group] <= 32 * U * sq[~in_group])
     assert np.all(np.abs(v.cpu().numpy() - r.vel)[:, ~in_group] <= 32 * U * sv[~in_group])
-    assert np.all(np.abs(q.cpu().numpy() - r.pos)[:, in_group] <= 1e-10 * sq[in_group])
-    assert np.all(np.abs(v.cpu().numpy() - r.vel)[:, in_group] <= 1e-10 * sv[in_group])
+    tot = k.bs_totals()
+    same = tuple(tot) == tuple(r.bs_totals)
+    bound = 2.5e-13 if same else 4e3 * 1e-12
+    worst = max(np.max(np.abs(q.cpu().numpy() - r.pos)[:, in_group] / sq[in_group]),
+                np.max(np.abs(v.cpu().numpy() - r.vel)[:, in_group] / sv[in_group]))
+    print(f"hybrid step: bodies in groups: worst difference {worst:.2e} (bound {bound:.0e}); Bulirsch-Stoer record kernel {tot} "
+          f"oracle {r.bs_totals}" + ("" if same else "  ** a step-size decision flipped **"))
+    assert worst <= bound
     k.free()
 
 
@@ -217,6 +289,8 @@ def test_semi_active_particles_in_groups(oracle_mod, tp_mode):
     d_mem = _dev(np.asarray(members + [0] * (n - len(members)), np.int32))
     d_off = torch.zeros(n + 4, dtype=torch.int32, device="cuda"); d_off[:len(offsets)] = _dev(np.asarray(offsets, np.int32))
     d_sum = torch.tensor([36, len(members), 11, 0], dtype=torch.int32, device="cuda")
+    gstats = torch.full((36, 4), -1, dtype=torch.int32, device="cuda")
+    k.bs_set_stats(gstats, 36)
     q, v = _dev(pos), _dev(vel)
     k.bs(_dev(pos), _dev(vel), _dev(mass), _dev(rc), 2, 1.0, 3.0, 1e-12, d_mem, d_off, d_sum, q, v)
     torch.cuda.synchronize()
@@ -224,7 +298,14 @@ def test_semi_active_particles_in_groups(oracle_mod, tp_mode):
     k.free()
     qw, vw, stats, _ = oracle_mod.bs.bs(pos, vel, mass, rc, np.asarray(members), np.asarray(offsets), G, 1.0, 3.0, 1e-12,
                                         pos, vel, nlevels=2, n_massive=n_m, tp_mode=tp_mode)
-    print("identical:", _check(q.cpu().numpy(), v.cpu().numpy(), qw, vw))
+    sign = np.where(rng.random(pos.shape) < 0.5, -1.0, 1.0)
+
+    def rerun(idx, delta):
+        qq, vv, _ = oracle_mod.bs.bs_group(pos[:, idx] * (1.0 + delta * sign[:, idx]), vel[:, idx], mass[idx], rc[:, idx], G, 1.0,
+                                           3.0, 1e-12, is_tp=idx >= n_m, tp_mode=tp_mode)
+        return qq, vv
+
+    _check(q.cpu().numpy(), v.cpu().numpy(), qw, vw, members, offsets, gstats.cpu().numpy(), stats, 1e-12, rerun=rerun)
     # and the rule matters here: the fully interactive result is far away
     qf, vf, _, _ = oracle_mod.bs.bs(pos, vel, mass, rc, np.asarray(members), np.asarray(offsets), G, 1.0, 3.0, 1e-12,
                                     pos, vel, nlevels=2)
@@ -238,9 +319,9 @@ def test_giant_group_one_lane_per_body(oracle_mod):
     ki = gi.make_ring(m)
     qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, np.arange(m), [0, m], ki.G, 1.0, 2.0, 1e-9,
                                         ki.pos, ki.vel, max_group=None)
-    q, v, st = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 2.0, 1e-9, np.arange(m), [0, m], ki.pos, ki.vel)
+    q, v, st, gs = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 2.0, 1e-9, np.arange(m), [0, m], ki.pos, ki.vel)
     assert st == 0 and not stats[0].failed
-    assert _check(q, v, qw, vw), "not bit-identical"
+    _check(q, v, qw, vw, np.arange(m), [0, m], gs, stats, 1e-9)
     assert np.abs(q - ki.pos).max() > 1e-3
 
 
@@ -256,9 +337,9 @@ def test_many_mid_size_groups_are_all_found(oracle_mod, size, count, dt, tol):
     offsets = np.arange(0, m + 1, size)
     qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, members, offsets, ki.G, 1.0, dt, tol,
                                         ki.pos, ki.vel, max_group=None)
-    q, v, st = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, dt, tol, members, offsets, ki.pos, ki.vel)
+    q, v, st, gs = _gpu_bs(m, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, dt, tol, members, offsets, ki.pos, ki.vel)
     assert st == 0 and len(stats) == count
-    assert _check(q, v, qw, vw), "not bit-identical"
+    _check(q, v, qw, vw, members, offsets, gs, stats, tol)
     # every group moved away from the state the arrays held before the call
     moved = np.abs(q - ki.pos).max(axis=0).reshape(count, size).max(axis=1)
     assert np.all(moved > 1e-6)

@@ -79,6 +79,29 @@ def test_config4_full_tp2(oracle_mod):
     assert np.all(np.abs(p) <= TOL * (ki.mass * orc.S).sum(axis=1))
 
 
+@pytest.mark.parametrize("nm,nt", [(16, 1048560), (600, 1 << 20)])
+def test_tp2_last_iblock_reaches_past_the_massive_records(oracle_mod, nm, nt):
+    """TP 2 where the transposed pass's i-block (512 records) does not divide the padded massive range (256 / 768
+    records): the i-records beyond it are particles and must take no part -- particles never feel each other
+    (sec. 8.1).  (16 massive bodies + N - 16 particles is the paper's own test-particle benchmark
+    shape, PAPER.md:848.)"""
+    from paper_2201_10058_b200 import binding
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    p2 = binding.make_plan_tp2(nm, nt, sms)
+    assert p2.m_pad % p2.i_block != 0, "the case this test is for: the last i-block spills past m_pad"
+    ki = gi.make_config(4, n=nm, n_test=nt)
+    u = gi.uniforms(78, 0, ki.n_test)
+    ki.mass = ki.mass.copy()
+    ki.mass[ki.n_massive:] = 1e-12 * (0.5 + u)
+    gpu = run_gpu(ki, level=0, capacity=CAPACITY, order_mode=0, tp_mode=2)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=0, G=ki.G, maxp=256, tp_mode=2)
+    assert gpu.status == 0
+    compare(gpu, orc, ki.n_massive, tol=TOL)
+    p = (ki.mass * gpu.acc).sum(axis=1)
+    assert np.all(np.abs(p) <= TOL * (ki.mass * orc.S).sum(axis=1))
+
+
 def test_config1_hundred_kicks(oracle_mod):
     """N = 8192, 100 kicks separated by an oracle-matched heliocentric drift: both sides see the
     same state at every step (the harness advances it with the ORACLE's acceleration), the

@@ -178,11 +178,22 @@ def test_error_codes():
         k.kick(x[1:], None, m, m, 0, 1.0, acc, pr, npr)
     assert e.value.code == g.E_ALIGN
     with pytest.raises(g.GengaKickError) as e:
-        k.kick(x, None, m, m, 1, 1.0, acc, pr, npr)
+        k.kick(x, None, m, torch.ones(128, dtype=torch.float64, device="cuda"), 1, 1.0, acc, pr, npr)
     assert e.value.code == g.E_LEVEL
     with pytest.raises(g.GengaKickError) as e:
         k.kick(x, None, m, m, 0, 1.0, None, pr, npr)
     assert e.value.code == g.E_NULL
+    # what the library cannot check on a bare pointer, the binding does before the call: side, dtype, layout, size
+    for bad, exc in [(lambda: k.kick(x.cpu(), None, m, m, 0, 1.0, acc, pr, npr), ValueError),
+                     (lambda: k.kick(x.float(), None, m, m, 0, 1.0, acc, pr, npr), TypeError),
+                     (lambda: k.kick(x, None, m, m, 0, 1.0, acc.t(), pr, npr), ValueError),
+                     (lambda: k.kick(x, None, m[:63], m, 0, 1.0, acc, pr, npr), ValueError),
+                     (lambda: k.kick(x, None, m, m, 0, 1.0, acc, pr[:7], npr), ValueError),
+                     (lambda: k.kick(x, None, m, m, 0, 1.0, acc, pr, npr[:64]), ValueError),
+                     (lambda: k.kick(x, None, m, m, 0, 1.0, acc, pr.long(), npr), TypeError),
+                     (lambda: k.kick_host(x, None, m, m, 0, 1.0, acc, pr, npr), ValueError)]:
+        with pytest.raises(exc):
+            bad()
     k.free()
 
 

@@ -129,13 +129,30 @@ def _ml_buffers(n, cap, slevels):
             torch.empty(n + 1, dtype=torch.int32, device="cuda"), torch.full((slevels, 4), -1, dtype=torch.int32, device="cuda"))
 
 
-def _ml_check(ki, q, v, r, in_enc):
+IN_ENC_SAME = 2.5e-13    # bodies inside encounters, both sides took the same Bulirsch-Stoer decisions (see _ml_check)
+
+
+def _ml_check(ki, q, v, r, in_enc, gpu_totals=None, tol=1e-12, label=""):
+    """Bodies outside every encounter: <= 32 u (the step's rounding).  Bodies inside: their Bulirsch-Stoer start states
+    differ by the kicks' rounding (<= 32 u), which the encounter amplifies.  If the kernel's record of the step-size
+    control (genga_bs_totals: accepted steps, halvings, force evaluations, groups) equals the oracle's, both sides did
+    the same operations on inputs 32 u apart: bound IN_ENC_SAME = 2.5e-13 relative, ~100 x the largest difference measured
+    on these disks (printed).  If the records differ, some error estimate fell within rounding of tol and the two sides
+    are two valid answers of the scheme: bound 4 tol (accepted macro steps of the largest group ~ 1) x 1e3 for the
+    amplification, and the flip is reported."""
     rr = np.sqrt((ki.pos ** 2).sum(0)); sp = np.sqrt((ki.vel ** 2).sum(0))
     sq, sv = rr + sp * ki.dt, sp + rr * np.sqrt(ki.G / rr ** 3)
     assert np.all(np.abs(q - r.pos)[:, ~in_enc] <= 32 * U * sq[~in_enc])
     assert np.all(np.abs(v - r.vel)[:, ~in_enc] <= 32 * U * sv[~in_enc])
-    assert np.all(np.abs(q - r.pos)[:, in_enc] <= 1e-10 * sq[in_enc])
-    assert np.all(np.abs(v - r.vel)[:, in_enc] <= 1e-10 * sv[in_enc])
+    same = gpu_totals is None or tuple(gpu_totals) == tuple(r.bs_totals)
+    bound = IN_ENC_SAME if same else 4e3 * tol
+    worst = 0.0
+    if in_enc.any():
+        worst = max(np.max(np.abs(q - r.pos)[:, in_enc] / sq[in_enc]), np.max(np.abs(v - r.vel)[:, in_enc] / sv[in_enc]))
+    print(f"{label}bodies in encounters: worst difference {worst:.2e} (bound {bound:.0e}); Bulirsch-Stoer record "
+          f"(accepted, rejected, force evaluations, groups) kernel {gpu_totals} oracle {r.bs_totals}"
+          + ("" if same else "  ** a step-size decision flipped **"))
+    assert worst <= bound
 
 
 @pytest.mark.parametrize("slevels,substeps,detect,f", [(1, 2, False, 1.0), (1, 2, True, 2.0), (2, 2, True, 1.0),
@@ -162,7 +179,7 @@ def test_multilevel_step_against_oracle(oracle_mod, slevels, substeps, detect, f
     want = oracle_mod.pair_set(r.first, n)
     assert np.array_equal(sorted_pairs(pairs.cpu().numpy()[:c[n]]), want)
     in_enc = r.first.count > 0
-    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, in_enc)
+    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, in_enc, gpu_totals=k.bs_totals())
     if slevels == 1 and not detect:
         # the same launch sequence as genga_hybrid_step: identical bits
         q2, v2 = _dev(ki.pos), _dev(ki.vel)
@@ -296,7 +313,7 @@ def test_multilevel_step_full_size_config3(oracle_mod):
     # critical radii of the two sides differ by <= 7 u (tests/test_gpu_step.py); allow 2 in 1e5, report exact equality
     assert np.all(np.abs(gs - r.stats) <= np.maximum(2, 2e-5 * r.stats)), (gs.tolist(), r.stats.tolist())
     print("per-level statistics identical:", bool(np.array_equal(gs, r.stats)), gs.tolist())
-    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0)
+    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0, gpu_totals=k.bs_totals())
     k.free()
 
 
@@ -324,7 +341,7 @@ def test_multilevel_step_with_semi_active_particles(oracle_mod, tp_mode, slevels
     c = npairs.cpu().numpy()
     pr = pairs.cpu().numpy()[:c[n]]
     assert (pr[:, 0] < ki.n_massive).all()                              # no particle-particle pairs
-    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0)
+    _ml_check(ki, q.cpu().numpy(), v.cpu().numpy(), r, r.first.count > 0, gpu_totals=k.bs_totals())
     k.free()
 
 

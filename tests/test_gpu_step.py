@@ -175,10 +175,14 @@ def test_step_against_oracle(oracle_mod, name, make):
     assert (got ^ want) <= border and len(want) > 0
     if not (got ^ want):
         assert np.array_equal(counts, r.first.count)
-    # the closing kick's acceleration, under the kick's own rule relaxed by the state's rounding: the state
-    # the GPU kicked differs from the oracle's by <= 32 u, which moves a pair term by <= 32 u (r / d) relative
-    err = np.abs(acc.cpu().numpy() - r.second.acc)
-    assert np.all(err <= 1e-10 * r.second.S + 1e-30)
+    # the closing kick's acceleration under the kick's own rule (north_star: 1e-13 * sum|term|), like for like: the
+    # oracle's kick of the positions and critical radii the DEVICE kicked (positions do not change in a kick, so
+    # these are the step's final positions) -- no allowance for the <= 32 u by which the two states differ
+    like = oracle_mod.kick(q.cpu().numpy(), ki.mass, rrow.cpu().numpy()[None, :], ki.n_massive, ki.n_test, level=0, G=ki.G,
+                           enc_factor=ki.enc_factor, maxp=256)
+    err = np.abs(acc.cpu().numpy() - like.acc)
+    assert np.all(err <= 1e-13 * like.S)
+    print(f"closing kick: max |da| / sum|term| = {np.max(err / np.maximum(like.S, 1e-300)):.2e} (bound 1e-13)")
     k.free()
 
 
@@ -187,21 +191,33 @@ def test_twenty_steps_track_the_oracle(oracle_mod):
     import torch
     ki = gi.make_config(1, n=1500)
     n = ki.n
-    k = _ctx(ki)
+    k = _ctx(ki, capacity=1 << 16)
     q, v, mass = _dev(ki.pos), _dev(ki.vel), _dev(ki.mass)
     acc = torch.empty(3, n, dtype=torch.float64, device="cuda")
     pairs = torch.empty(1 << 16, 2, dtype=torch.int32, device="cuda")
     npairs = torch.empty(n + 1, dtype=torch.int32, device="cuda")
     oq, ov = ki.pos.copy(), ki.vel.copy()
+    worst = 0.0
     for _ in range(20):
+        gq, gv = q.cpu().numpy(), v.cpu().numpy()                  # the device's state before this step
         k.step(q, v, mass, 1.0, ki.dt, None, acc, pairs, npairs)
         r = oracle_mod.step.step(oq, ov, ki.mass, n, 0, 1.0, ki.G, ki.dt)
         oq, ov = r.pos, r.vel
+        # every single step like for like: the oracle's step from the device's own state, at the one-step bound (32 u)
+        one = oracle_mod.step.step(gq, gv, ki.mass, n, 0, 1.0, ki.G, ki.dt)
+        sq, sv = _scales(gq, gv, ki.dt)
+        eq = np.max(np.abs(q.cpu().numpy() - one.pos) / sq) / U; ev = np.max(np.abs(v.cpu().numpy() - one.vel) / sv) / U
+        assert eq <= 32 and ev <= 32
+        worst = max(worst, eq, ev)
     torch.cuda.synchronize()
     sq, sv = _scales(oq, ov, ki.dt)
-    # 20 steps of <= 32 u each, amplified by the Kepler shear (d(n t)/da ~ 1.5 n t / a over t = 120 d)
-    assert np.all(np.abs(q.cpu().numpy() - oq) <= 20 * 32 * U * sq * 8)
-    assert np.all(np.abs(v.cpu().numpy() - ov) <= 20 * 32 * U * sv * 8)
+    # ... and the two free-running trajectories: 20 steps of <= 32 u each, amplified by the Kepler shear: a relative
+    # error e in the semi-major axis turns into a phase error 1.5 n t e, n t <= 2 pi 120 d / (0.5^1.5 x 365.25 d) = 5.8
+    # at the disk's inner edge (a = 0.5 AU): amplification <= 1.5 x 5.8 = 8.8
+    dq = np.max(np.abs(q.cpu().numpy() - oq) / sq) / U; dv = np.max(np.abs(v.cpu().numpy() - ov) / sv) / U
+    print(f"20 steps: worst single step {worst:.1f} u (bound 32 u); free-running difference {dq:.0f} u (pos), {dv:.0f} u (vel) "
+          f"(bound 20 x 32 x 8.8 = 5632 u)")
+    assert dq <= 20 * 32 * 8.8 and dv <= 20 * 32 * 8.8
     assert k.status() == 0
     k.free()
 
@@ -219,7 +235,7 @@ def test_step_error_codes():
                        (lambda: k.hc(q, v, None, 1.0, 6.0), g.E_NULL),
                        (lambda: k.hc(q, v, m, -1.0, 6.0), g.E_SIZE),
                        (lambda: k.fg(q, None, 1.0, 6.0), g.E_NULL),
-                       (lambda: k.fg(q.view(-1)[1:], v, 1.0, 6.0), g.E_ALIGN),
+                       (lambda: k.fg(torch.zeros(3 * 64 + 1, dtype=torch.float64, device="cuda")[1:], v, 1.0, 6.0), g.E_ALIGN),
                        (lambda: k.drift(q, v, None, 1.0, 6.0), g.E_NULL),
                        (lambda: k.step(q, v, m, 1.0, 6.0, None, None, None, None), g.E_NULL)]:
         with pytest.raises(g.GengaKickError) as e:
