@@ -92,6 +92,12 @@ typedef struct {
     int32_t max_segs;       /* most i-blocks any CTA touches                                       */
     int64_t n_rec;          /* records allocated (n_i rounded up to a multiple of 1024)            */
     int64_t partial_doubles;/* doubles of scratch for the partial sums                             */
+    /* symmetric plans only (genga_kick_make_plan_sym; 0 otherwise) */
+    int32_t symmetric;      /* 1: massive x massive with every unordered pair evaluated once: row I (i-block I)
+                               holds only the j-tiles jt >= I * tiles_per_iblock; tiles numbered row-major  */
+    int32_t tiles_per_iblock;/* i_block / j_tile: the first that many tiles of a row overlap the i-block
+                               (diagonal tiles, one-sided); the rest give force and reaction           */
+    int64_t react_doubles;  /* doubles of scratch for the reaction partial sums: n_tiles * 3 * j_tile */
 } genga_kick_plan;
 
 /* Fill *plan for a problem of n_massive + n_test bodies at changeover level `level` on a device
@@ -101,6 +107,19 @@ int genga_kick_make_plan(int32_t n_massive, int32_t n_test, int32_t level, int32
 /* TP 2 only: the plan of the second pass of a level-0 kick, massive bodies (i) x semi-active
  * particles (j), same tile / CTA / partial-sum scheme.  Errors: E_NULL, E_SIZE. */
 int genga_kick_make_plan_tp2(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan);
+/* Level 0, massive x massive, Newton's third law: each unordered pair is evaluated once (eq. 3 is symmetric in i, j:
+ * PAPER.md:63-64), the j-side sums are written per tile and added in ascending row order by the reduction pass.
+ * plan->n_ctas == 0 if the library does not use it for this size (n_massive below 24,576, or the reaction scratch
+ * above 2 GiB).  Test particles are not part of it (they take the one-sided rows of genga_kick_make_plan_tprows).
+ * Errors: E_NULL, E_SIZE. */
+int genga_kick_make_plan_sym(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan);
+/* The one-sided rows of the semi-active particles (i = particles, j = massive bodies) when the massive bodies take the
+ * symmetric plan: same tile / CTA / partial-sum scheme as genga_kick_make_plan, i-blocks counted from record m_pad.
+ * Errors: E_NULL, E_SIZE. */
+int genga_kick_make_plan_tprows(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan);
+/* Symmetric plans: first tile of row `row` (row = n_i_blocks gives n_tiles) and the row of tile t. */
+int64_t genga_kick_plan_sym_row_begin(const genga_kick_plan* plan, int32_t row);
+int32_t genga_kick_plan_sym_row_of(const genga_kick_plan* plan, int64_t t);
 /* Tile range [*t0, *t1) of CTA `cta` under *plan.  Errors: E_NULL, E_SIZE. */
 int genga_kick_plan_cta_range(const genga_kick_plan* plan, int32_t cta, int64_t* t0, int64_t* t1);
 /* First and last CTA whose range meets i-block `ib`.  Errors: E_NULL, E_SIZE. */

@@ -16,7 +16,8 @@ STATUS_FX_RANGE = 4
 ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 
 EXPORTS = (
-    "genga_kick_make_plan", "genga_kick_make_plan_tp2", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
+    "genga_kick_make_plan", "genga_kick_make_plan_tp2", "genga_kick_make_plan_sym", "genga_kick_make_plan_tprows",
+    "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
     "genga_kick_set_stream", "genga_kick", "genga_kick_list", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
@@ -49,7 +50,8 @@ class GengaSencConfig(C.Structure):
 class GengaKickPlan(C.Structure):
     _fields_ = [("threads", C.c_int32), ("i_per_thread", C.c_int32), ("i_block", C.c_int32), ("j_tile", C.c_int32),
                 ("m_pad", C.c_int32), ("n_i_blocks", C.c_int32), ("n_j_tiles", C.c_int32), ("n_tiles", C.c_int64),
-                ("n_ctas", C.c_int32), ("max_segs", C.c_int32), ("n_rec", C.c_int64), ("partial_doubles", C.c_int64)]
+                ("n_ctas", C.c_int32), ("max_segs", C.c_int32), ("n_rec", C.c_int64), ("partial_doubles", C.c_int64),
+                ("symmetric", C.c_int32), ("tiles_per_iblock", C.c_int32), ("react_doubles", C.c_int64)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -75,6 +77,12 @@ def lib():
         vp, i32, i64, d = C.c_void_p, C.c_int32, C.c_int64, C.c_double
         L.genga_kick_make_plan.argtypes = [i32, i32, i32, i32, C.POINTER(GengaKickPlan)]
         L.genga_kick_make_plan_tp2.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_make_plan_sym.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_make_plan_tprows.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_plan_sym_row_begin.argtypes = [C.POINTER(GengaKickPlan), i32]
+        L.genga_kick_plan_sym_row_begin.restype = i64
+        L.genga_kick_plan_sym_row_of.argtypes = [C.POINTER(GengaKickPlan), i64]
+        L.genga_kick_plan_sym_row_of.restype = i32
         L.genga_kick_plan_cta_range.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i64), C.POINTER(i64)]
         L.genga_kick_plan_iblock_ctas.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i32), C.POINTER(i32)]
         L.genga_kick_init.argtypes = [C.POINTER(GengaKickConfig), C.POINTER(vp)]
@@ -110,7 +118,8 @@ def lib():
         L.genga_detect.argtypes = [vp, vp, vp, vp, vp, vp, d, d, vp, vp, i64, vp, vp]
         L.genga_multilevel_step.argtypes = [vp, vp, vp, vp, d, d, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
         for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS + SENC_EXPORTS:
-            if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error"):
+            if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error",
+                            "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -134,6 +143,30 @@ def make_plan_tp2(n_massive: int, n_test: int, num_sms: int) -> GengaKickPlan:
     if rc != OK:
         raise GengaKickError(rc, strerror(rc))
     return plan
+
+
+def make_plan_sym(n_massive: int, n_test: int, num_sms: int) -> GengaKickPlan:
+    plan = GengaKickPlan()
+    rc = lib().genga_kick_make_plan_sym(n_massive, n_test, num_sms, C.byref(plan))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
+    return plan
+
+
+def make_plan_tprows(n_massive: int, n_test: int, num_sms: int) -> GengaKickPlan:
+    plan = GengaKickPlan()
+    rc = lib().genga_kick_make_plan_tprows(n_massive, n_test, num_sms, C.byref(plan))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
+    return plan
+
+
+def plan_sym_row_begin(plan: GengaKickPlan, row: int) -> int:
+    return int(lib().genga_kick_plan_sym_row_begin(C.byref(plan), int(row)))
+
+
+def plan_sym_row_of(plan: GengaKickPlan, t: int) -> int:
+    return int(lib().genga_kick_plan_sym_row_of(C.byref(plan), int(t)))
 
 
 def plan_cta_range(plan: GengaKickPlan, cta: int):

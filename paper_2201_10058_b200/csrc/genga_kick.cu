@@ -4,6 +4,7 @@
 #include "genga_kick_ctx.h"
 #include "genga_kick_variants.h"
 #include "genga_kick_kernels.cuh"
+#include "genga_kick_sym.cuh"
 #include "genga_kick_sort.cuh"
 
 #include <algorithm>
@@ -82,7 +83,6 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
         if ((e = cudaMalloc(&ctx->rzm, (size_t)nr * sizeof(double2))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->rfw, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->ridx, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
-        if ((e = cudaMalloc(&ctx->cfw, (size_t)(nr / GENGA_CHUNK) * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->cblo, (size_t)(nr / GENGA_GROUP) * sizeof(float4))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->cbhi, (size_t)(nr / GENGA_GROUP) * sizeof(float4))) != cudaSuccess) goto cuda_error;
         ctx->sorted = cfg->order_mode == GENGA_KICK_ORDER_SORTED ||
@@ -96,6 +96,17 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
             if ((e = cudaMalloc(&ctx->vals_a, (size_t)N * sizeof(int))) != cudaSuccess) goto cuda_error;
             if ((e = cudaMalloc(&ctx->vals_b, (size_t)N * sizeof(int))) != cudaSuccess) goto cuda_error;
             if ((e = cudaMalloc(&ctx->counts, nc * sizeof(int))) != cudaSuccess) goto cuda_error;
+        }
+        rc = genga_kick_make_plan_sym(cfg->n_massive, cfg->n_test, ctx->num_sms, &ctx->plan_sym);
+        if (rc != GENGA_KICK_OK) goto fail;
+        if (ctx->plan_sym.n_ctas > 0) {
+            if ((e = cudaMalloc(&ctx->partial_sym, (size_t)ctx->plan_sym.partial_doubles * sizeof(double))) != cudaSuccess) goto cuda_error;
+            if ((e = cudaMalloc(&ctx->react, (size_t)ctx->plan_sym.react_doubles * sizeof(double))) != cudaSuccess) goto cuda_error;
+            if (cfg->n_test > 0) {
+                rc = genga_kick_make_plan_tprows(cfg->n_massive, cfg->n_test, ctx->num_sms, &ctx->plan_tprows);
+                if (rc != GENGA_KICK_OK) goto fail;
+                if (ctx->plan_tprows.partial_doubles > max_partial) max_partial = ctx->plan_tprows.partial_doubles;
+            }
         }
         if ((e = cudaMalloc(&ctx->partial, (size_t)max_partial * sizeof(double))) != cudaSuccess) goto cuda_error;
         ctx->tp2 = cfg->tp_mode == 2 && cfg->n_test > 0 && cfg->n_massive > 0;
@@ -175,11 +186,11 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
     }
     genga::KickParams kp = {};
     {
-        kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx; kp.cfw = ctx->cfw;
+        kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx;
         kp.cblo = ctx->cblo; kp.cbhi = ctx->cbhi;
         kp.rcrit = rcrit;
         kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
-        kp.react = ctx->tp2 && changeover_level > 0 ? 1 : 0; kp.j_rec0 = 0; kp.force_only = 0; kp.i_rec_end = n_rec;
+        kp.react = ctx->tp2 && changeover_level > 0 ? 1 : 0; kp.j_rec0 = 0; kp.i_rec0 = 0; kp.force_only = 0; kp.i_rec_end = n_rec;
         kp.n_j_tiles = pl.n_j_tiles; kp.n_ctas = pl.n_ctas; kp.max_segs = pl.max_segs; kp.n_tiles = pl.n_tiles;
         kp.partial = ctx->partial;
         kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
@@ -191,14 +202,33 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
         genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
                                                    ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
-                                                   ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw,
+                                                   ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx,
                                                    ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
     }
+    const bool use_sym = changeover_level == 0 && ctx->plan_sym.n_ctas > 0;
     if (pl.n_ctas > 0) {
         if (ctx->timing) GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level], st));
-        if (changeover_level == 0) {
+        if (changeover_level == 0 && use_sym) {
+            // massive x massive: every unordered pair once (kick_sym_kernel); the particles' rows one-sided beside it
+            const genga_kick_plan& ps = ctx->plan_sym;
+            genga::KickParams ks = kp;
+            ks.n_j_tiles = ps.n_j_tiles; ks.n_ctas = ps.n_ctas; ks.max_segs = ps.max_segs; ks.n_tiles = ps.n_tiles;
+            ks.partial = ctx->partial_sym;
+            ks.i_rec_end = (ctx->cfg.n_massive + 31) / 32 * 32;
+            genga::SymParams sp = {ps.n_i_blocks, ps.tiles_per_iblock, ctx->react};
+            genga::kick_sym_kernel<GENGA_SYM_THREADS, GENGA_SYM_IPT, GENGA_STAGES><<<ps.n_ctas, GENGA_SYM_THREADS, 0, st>>>(ks, sp);
+            GK_CUDA(ctx, cudaGetLastError());
+            if (ctx->plan_tprows.n_ctas > 0) {
+                const genga_kick_plan& pt = ctx->plan_tprows;
+                genga::KickParams kt = kp;
+                kt.n_j_tiles = pt.n_j_tiles; kt.n_ctas = pt.n_ctas; kt.max_segs = pt.max_segs; kt.n_tiles = pt.n_tiles;
+                kt.i_rec0 = pl.m_pad;
+                GK_CUDA(ctx, dispatch_kick(pt, kt, st));
+                ctx->launches++;
+            }
+        } else if (changeover_level == 0) {
             GK_CUDA(ctx, dispatch_kick(pl, kp, st));
         } else {
             // W_L = 0 exactly outside the filter radius: a neighbour search, no tile decomposition
@@ -240,15 +270,28 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
     }
     {
         // level >= 1: no partial segments (n_ctas = 0), every term comes from the exact path
+        auto seg_of = [](const genga_kick_plan& q, const double* partial, int rec0, int rec_end, bool on) {
+            genga::SegPlan sg = {};
+            sg.partial = partial; sg.IB = q.i_block > 0 ? q.i_block : 1; sg.n_j_tiles = q.n_j_tiles > 0 ? q.n_j_tiles : 1;
+            sg.n_ctas = on ? q.n_ctas : 0; sg.max_segs = q.max_segs; sg.n_tiles = q.n_tiles > 0 ? q.n_tiles : 1;
+            sg.rec0 = rec0; sg.rec_end = rec_end;
+            sg.symmetric = q.symmetric; sg.r = q.tiles_per_iblock; sg.n_rows = q.n_i_blocks;
+            return sg;
+        };
         const genga_kick_plan& p2 = ctx->plan_tp2;
         const bool second = ctx->tp2 && changeover_level == 0 && p2.n_ctas > 0;
-        genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(ctx->partial, ctx->ridx, n_rec, N, pl.i_block, pl.n_j_tiles,
-                                                                  pl.n_tiles, changeover_level == 0 ? pl.n_ctas : 0,
-                                                                  pl.max_segs, ctx->partial2, pl.m_pad,
-                                                                  second ? p2.i_block : 1, second ? p2.n_j_tiles : 1,
-                                                                  second ? p2.n_tiles : 1, second ? p2.n_ctas : 0,
-                                                                  second ? p2.max_segs : 1, dt, ctx->fx,
-                                                                  ctx->touched, ctx->status, out_acc, vel);
+        genga::ReduceParams rp = {};
+        if (use_sym) {
+            rp.seg[0] = seg_of(ctx->plan_sym, ctx->partial_sym, 0, pl.m_pad, true);
+            rp.react = ctx->react; rp.react_jt = ctx->plan_sym.j_tile;
+            rp.seg[2] = seg_of(ctx->plan_tprows, ctx->partial, pl.m_pad, n_rec, ctx->plan_tprows.n_ctas > 0);
+        } else {
+            rp.seg[0] = seg_of(pl, ctx->partial, 0, n_rec, changeover_level == 0);
+            rp.seg[2] = seg_of(pl, ctx->partial, 0, 0, false);
+        }
+        rp.seg[1] = seg_of(p2, ctx->partial2, 0, pl.m_pad, second);
+        genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(rp, ctx->ridx, n_rec, N, dt, ctx->fx, ctx->touched,
+                                                                  ctx->status, out_acc, vel);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
     }
@@ -343,7 +386,7 @@ extern "C" int genga_kick_get_plan(const genga_kick_ctx* ctx, int32_t changeover
 {
     if (!ctx || !plan) return GENGA_KICK_E_NULL;
     if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
-    *plan = ctx->plans[changeover_level];
+    *plan = changeover_level == 0 && ctx->plan_sym.n_ctas > 0 ? ctx->plan_sym : ctx->plans[changeover_level];
     return GENGA_KICK_OK;
 }
 
@@ -464,7 +507,7 @@ extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return c
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)
 {
     if (!ctx) return GENGA_KICK_OK;
-    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->cfw, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
+    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->partial_sym, ctx->react, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
                     ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->partial2, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs,
                     ctx->psum_partial, ctx->psum_ticket, ctx->step_rcrit, ctx->grp_label, ctx->grp_flag,

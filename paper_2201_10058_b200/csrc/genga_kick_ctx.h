@@ -14,12 +14,15 @@ struct genga_kick_ctx {
     genga_kick_plan plan_tp2;      // TP 2: second pass of the level-0 kick (massive i x semi-active j)
     bool tp2;
     double* partial2;              // its partial sums
+    genga_kick_plan plan_sym;      // level 0, massive x massive, every unordered pair once (n_ctas == 0: not used)
+    genga_kick_plan plan_tprows;   // ... and the one-sided rows of the semi-active particles beside it
+    double* partial_sym;           // i-side partial sums of the symmetric pass
+    double* react;                 // its reaction sums, one slot per tile
     // scratch (device)
     double2* rxy;
     double2* rzm;
     int* rfw;
     int* ridx;
-    int* cfw;
     float4* cblo;
     float4* cbhi;
     // internal order (genga_kick_sort.cuh); sorted == false: caller's order

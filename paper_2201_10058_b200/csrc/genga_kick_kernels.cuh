@@ -30,7 +30,6 @@ struct KickParams {
     const double2* __restrict__ rzm;   // (z, G m)
     const int* __restrict__ rfw;       // filter word (see filter_word)
     const int* __restrict__ ridx;      // caller's body index, -1 for padding
-    const int* __restrict__ cfw;       // max filter word of each chunk of GENGA_CHUNK records
     const float4* __restrict__ cblo;   // box of each group of GENGA_GROUP records: (lo x, lo y, lo z, max filter word)
     const float4* __restrict__ cbhi;   //                                            (hi x, hi y, hi z, -)
     // the caller's arrays (read by the exact per-pair path only)
@@ -39,6 +38,7 @@ struct KickParams {
     int react;                         // TP 2 at level >= 1: exact_kernel also adds the reaction of a semi-active
                                        // particle i on the massive body j (near_kernel's pair filter is symmetric)
     int j_rec0;                        // record of the first j-tile (0; m_pad in the second pass of TP 2)
+    int i_rec0;                        // record of the first i-block (0; m_pad for the particles' rows beside kick_sym_kernel)
     int i_rec_end;                     // i-records from here on take no part in the pass (n_rec; m_pad in the second pass
                                        // of TP 2, whose last i-block may reach past the massive records: sec. 8.1
                                        // particles never feel each other)
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(256)
 pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, const double* __restrict__ rcrit,
             const int* __restrict__ perm, int N, int n_massive, int m_pad, int n_rec, int L, double G, double f,
             double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
-            int* __restrict__ cfw, float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs,
+            float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs,
             int* __restrict__ ncand)
 {
     if (blockIdx.x == 0 && threadIdx.x == 0) *ncand = 0;
@@ -113,12 +113,7 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
             rfw[r] = fw;
             ridx[r] = b;
         }
-        // chunk maximum over GENGA_CHUNK consecutive records (= consecutive lanes)
         int m = fw;
-        m = max(m, __shfl_xor_sync(0xffffffffu, m, 1));
-        m = max(m, __shfl_xor_sync(0xffffffffu, m, 2));
-        m = max(m, __shfl_xor_sync(0xffffffffu, m, 4));
-        if (r < n_rec && (r % GENGA_CHUNK) == 0) cfw[r / GENGA_CHUNK] = m;
         // group box
         // ... over the real bodies of the group only: a padding record (fw = -1) cannot trip the
         // filter, and a group without real bodies gets an empty box that is near to nothing
@@ -128,7 +123,7 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
         float hx = real ? __double2float_ru(x) : -3.0e38f, hy = real ? __double2float_ru(y) : -3.0e38f,
               hz = real ? __double2float_ru(z) : -3.0e38f;
 #pragma unroll
-        for (int o = 8; o < 32; o <<= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+        for (int o = 1; o < 32; o <<= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             lx = fminf(lx, __shfl_xor_sync(0xffffffffu, lx, o)); hx = fmaxf(hx, __shfl_xor_sync(0xffffffffu, hx, o));
@@ -311,7 +306,7 @@ struct alignas(128) TileStage {
     double2 zm[JT];
     float4 blo[JT / GENGA_GROUP];
     float4 bhi[JT / GENGA_GROUP];
-    int cf[JT / GENGA_CHUNK];
+    int fw[JT];
 };
 
 // lower bound of the squared distance between two boxes against the upper bound of the squared
@@ -420,9 +415,14 @@ __device__ __forceinline__ double fx_take(unsigned long long* __restrict__ acc, 
 // The work of the exact path for one candidate (i-record, j-record or ~j-record for a force-only
 // candidate, or (-1, -1) for an empty slot): weight, force on i (and the TP 2 reaction on j), pre-check,
 // per-body counts.  Returns the pair to emit, if any.
-__device__ __forceinline__ void apply_candidate(const KickParams& p, int ir, int jr_enc, bool& hit, int& lo, int& hi)
+__device__ __forceinline__ void apply_candidate(const KickParams& p, int ir_enc, int jr_enc, bool& hit, int& lo, int& hi)
 {
-    const bool force_only = ir >= 0 && jr_enc < 0;                                  // (i, ~j): see KickParams
+    // (i, j) one-sided: the force on i and i's side of the bookkeeping (the mirror (j, i) is queued too);
+    // (i, ~j) force-only: see KickParams;  (~i, j) symmetric (kick_sym_kernel): both forces, the pair's bookkeeping once;
+    // (-1, -1) an empty slot
+    const bool sym = ir_enc < 0 && jr_enc >= 0;
+    const int ir = sym ? ~ir_enc : ir_enc;
+    const bool force_only = ir >= 0 && jr_enc < 0;
     const int jr = force_only ? ~jr_enc : jr_enc;
     const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;      // (-1, -1): empty slot
     if (ir == jr || bi < 0 || bj < 0) return;
@@ -437,6 +437,15 @@ __device__ __forceinline__ void apply_candidate(const KickParams& p, int ir, int
         fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
         p.touched[ir] = 1;
     }
+    if (sym && r.W != 0.0 && izm.y != 0.0) {
+        // the force of i on j with the bits the definition gives from j's side (d -> -d, r^2 and W unchanged)
+        const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
+        unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
+        fx_add(accj, -__dmul_rn(si, dx), p.status);
+        fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
+        fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+        p.touched[jr] = 1;
+    }
     if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
         // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
         // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
@@ -449,7 +458,10 @@ __device__ __forceinline__ void apply_candidate(const KickParams& p, int ir, int
     }
     if (r.enc && p.out_npairs && !force_only) {
         atomicAdd(p.out_npairs + bi, 1);
-        if (bi >= p.n_massive) {               // test particle i, massive j
+        if (sym) {                             // both massive, queued once
+            atomicAdd(p.out_npairs + bj, 1);
+            hit = true; lo = min(bi, bj); hi = max(bi, bj);
+        } else if (bi >= p.n_massive) {        // test particle i, massive j
             atomicAdd(p.out_npairs + bj, 1);
             hit = true; lo = bj; hi = bi;
         } else if (bi < bj) {
@@ -579,9 +591,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 {
     constexpr int IB = THREADS * IPT;
     constexpr int WARPS = THREADS / 32;
-    constexpr int NCH = JT / GENGA_CHUNK;
     constexpr int NG = JT / GENGA_GROUP;
-    constexpr uint32_t TILE_BYTES = JT * 32 + NG * 32 + NCH * 4;
+    constexpr uint32_t TILE_BYTES = JT * 32 + NG * 32 + JT * 4;
     static_assert(NG <= 32 && JT % GENGA_GROUP == 0, "one lane per group");
     static_assert(GENGA_CHUNK * IPT <= 32, "one trigger bit per pair of a chunk");
     __shared__ TileStage<JT> st[STAGES];
@@ -616,7 +627,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
         bulk_g2s(st[s].zm, p.rzm + j0, JT * 16, &full[s]);
         bulk_g2s(st[s].blo, p.cblo + j0 / GENGA_GROUP, NG * 16, &full[s]);
         bulk_g2s(st[s].bhi, p.cbhi + j0 / GENGA_GROUP, NG * 16, &full[s]);
-        bulk_g2s(st[s].cf, p.cfw + j0 / GENGA_CHUNK, NCH * 4, &full[s]);
+        bulk_g2s(st[s].fw, p.rfw + j0, JT * 4, &full[s]);
     };
     const int n_it = (int)(t1 - t0);
     if (tid == 0)
@@ -657,7 +668,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
             wfw = -1;
 #pragma unroll
             for (int k = 0; k < IPT; k++) {
-                const size_t r = (size_t)ib * IB + woff + k * 32;
+                const size_t r = (size_t)p.i_rec0 + (size_t)ib * IB + woff + k * 32;
                 ax[k] = ay[k] = az[k] = 0.0;
                 if (r >= (size_t)p.i_rec_end) {             // whole groups of 32 records (i_rec_end is a multiple of 32)
                     xi[k] = yi[k] = zi[k] = GENGA_SENTINEL_POS;
@@ -695,18 +706,15 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
             }
 #pragma unroll 1
             for (int jj = j0; jj < j0 + GENGA_GROUP; jj += GENGA_CHUNK) {
-                const int cm = S.cf[jj / GENGA_CHUNK];
-                int thr[IPT];
-#pragma unroll
-                for (int k = 0; k < IPT; k++) thr[k] = max(fi[k], cm);
                 unsigned tm = 0;                            // bit u * IPT + k: pair (k, jj + u) tripped the filter
 #pragma unroll
                 for (int u = 0; u < GENGA_CHUNK; u++) {
                     const double2 xy = S.xy[jj + u], zm = S.zm[jj + u];
+                    const int fj = S.fw[jj + u];            // the exact per-pair rule: hi(r^2) < max(fw_i, fw_j)
 #pragma unroll
                     for (int k = 0; k < IPT; k++) {
                         bool trig = false;
-                        pair_fast(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], thr[k], ax[k], ay[k], az[k], trig);
+                        pair_fast(xy.x, xy.y, zm.x, zm.y, xi[k], yi[k], zi[k], max(fi[k], fj), ax[k], ay[k], az[k], trig);
                         tm |= (trig ? 1u : 0u) << (u * IPT + k);
                     }
                 }
@@ -716,7 +724,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
                     todo &= todo - 1;
                     const bool mine = (tm >> b) & 1u;
                     const int jrec = p.j_rec0 + jt * JT + jj + b / IPT;
-                    push_candidates(p, cc, mine, ib * IB + woff + (b % IPT) * 32, p.force_only ? ~jrec : jrec);
+                    push_candidates(p, cc, mine, p.i_rec0 + ib * IB + woff + (b % IPT) * 32, p.force_only ? ~jrec : jrec);
                 }
             }
         }
@@ -748,9 +756,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) kick_kernel(const KickParams p)
 // RESCAN = false: the level >= 1 pair loop (queues candidates; a pair trips if hi(r^2) < max(fw_i, fw_j)).
 // RESCAN = true : the fallback for a candidate list that overflowed (more pairs inside critical radii than
 //   the list holds: everything inside everything's radius).  Launched after the pair loop of every kick, it
-//   returns at once unless the list overflowed; then it repeats the search -- with the pair loop's own trip
-//   rule, hi(r^2) < max(fw_i, largest fw of j's chunk), so that it meets exactly the pairs the far-field
-//   pass left out -- and evaluates every tripped pair where it finds it (apply_candidate), while
+//   returns at once unless the list overflowed; then it repeats the search -- with the pair loops' own trip
+//   rule on the same bits (r^2 of (i, j) and of (j, i) are the same double), so that it meets exactly the ordered
+//   pairs the far-field pass left out -- and evaluates every tripped pair where it finds it (apply_candidate), while
 //   exact_kernel ignores the truncated list.  Slow (one atomic on the pair counter per pair) but complete:
 //   the capacity of the list bounds the speed of pathological inputs, not the correctness of the result.
 //   i-records [0, i_rec_end) against the j-groups [j_group0, j_group0 + n_jgroups); force_only as in KickParams.
@@ -797,8 +805,7 @@ near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int 
             while (nearmask) {
                 const int j0 = (j_group0 + (g0 + q0 + __ffs(nearmask) - 1) * js + jy) * GENGA_GROUP;
                 nearmask &= nearmask - 1;
-                // per j-record threshold: its own filter word, or (RESCAN) the largest of its chunk
-                const int fj_lane = RESCAN ? p.cfw[(j0 + lane) / GENGA_CHUNK] : p.rfw[j0 + lane];
+                const int fj_lane = p.rfw[j0 + lane];          // the pair rule of every pair loop: hi(r^2) < max(fw_i, fw_j)
                 unsigned tm = 0;                            // bit u: pair (r, j0 + u) tripped the filter
 #pragma unroll 8
                 for (int u = 0; u < GENGA_GROUP; u++) {
@@ -926,14 +933,45 @@ list_reduce_kernel(unsigned long long* __restrict__ fx, int* __restrict__ touche
 }
 
 // ---------------------------------------------------------------------------------------------
-// reduce_kernel (row a8 + a7): record r sums the partial accelerations of the CTAs whose tile
-// range met its i-block, in ascending CTA order, and writes the caller's arrays.
+// reduce_kernel (row a8 + a7): record r adds, in a FIXED order, what the pair loops
+// left for it: the partial segments of its i-block in ascending CTA order (up to three pair-loop
+// passes, each with its own plan), the reaction sums of the symmetric pass in ascending row order,
+// and the exact path's fixed-point sum; then writes the caller's arrays.
 // ---------------------------------------------------------------------------------------------
+struct SegPlan {                       // the partial segments one pair-loop pass has written
+    const double* __restrict__ partial;   // [n_ctas][max_segs][3][IB]
+    int IB, n_j_tiles, n_ctas, max_segs;  // n_ctas == 0: the pass did not run
+    long long n_tiles;
+    int rec0, rec_end;                 // the pass served the i-records [rec0, rec_end), i-block 0 at rec0
+    int symmetric, r, n_rows;          // kick_sym_kernel's row-major triangular tile numbering (genga_kick_variants.h)
+};
+
+struct ReduceParams {
+    SegPlan seg[3];                    // added in this order
+    const double* __restrict__ react;  // symmetric pass: [n_tiles][3][JT] reaction sums (nullptr: none); plan = seg[0]
+    int react_jt;                      // its j-tile
+};
+
+__device__ __forceinline__ void add_segments(const SegPlan& q, int r, double& a0, double& a1, double& a2)
+{
+    if (q.n_ctas <= 0 || r < q.rec0 || r >= q.rec_end) return;
+    const int ib = (r - q.rec0) / q.IB, off = (r - q.rec0) - ib * q.IB;
+    const long long ta = q.symmetric ? sym_row_begin(ib, q.n_j_tiles, q.r) : (long long)ib * q.n_j_tiles;
+    const long long tb = (q.symmetric ? sym_row_begin(ib + 1, q.n_j_tiles, q.r) : ta + q.n_j_tiles) - 1;
+    if (tb < ta) return;
+    const int c_first = plan_tile_owner(ta, q.n_tiles, q.n_ctas), c_last = plan_tile_owner(tb, q.n_tiles, q.n_ctas);
+    for (int c = c_first; c <= c_last; c++) {
+        const long long tc = plan_tile_begin(c, q.n_tiles, q.n_ctas);
+        const int seg = ib - (q.symmetric ? sym_row_of(tc, q.n_j_tiles, q.r, q.n_rows) : (int)(tc / q.n_j_tiles));
+        const double* v = q.partial + ((size_t)c * q.max_segs + seg) * 3 * q.IB + off;
+        a0 = __dadd_rn(a0, v[0]);
+        a1 = __dadd_rn(a1, v[q.IB]);
+        a2 = __dadd_rn(a2, v[2 * (size_t)q.IB]);
+    }
+}
+
 __global__ void __launch_bounds__(256)
-reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, int n_rec, int N, int IB,
-              int n_j_tiles, long long n_tiles, int n_ctas, int max_segs,
-              const double* __restrict__ partial2, int m_pad, int IB2, int n_j_tiles2, long long n_tiles2, int n_ctas2,
-              int max_segs2, double dt,
+reduce_kernel(const ReduceParams rp, const int* __restrict__ ridx, int n_rec, int N, double dt,
               unsigned long long* __restrict__ fx, int* __restrict__ touched, int* __restrict__ status,
               double* __restrict__ out_acc, double* __restrict__ vel)
 {
@@ -941,30 +979,22 @@ reduce_kernel(const double* __restrict__ partial, const int* __restrict__ ridx, 
     if (r >= n_rec) return;
     const int b = ridx[r];
     if (b < 0) return;
-    const int ib = r / IB, off = r - ib * IB;
-    const long long ta = (long long)ib * n_j_tiles, tb = ta + n_j_tiles - 1;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-    const int c_first = n_ctas > 0 ? plan_tile_owner(ta, n_tiles, n_ctas) : 0;
-    const int c_last = n_ctas > 0 ? plan_tile_owner(tb, n_tiles, n_ctas) : -1;    // no massive body: a = 0
-    for (int c = c_first; c <= c_last; c++) {
-        const int seg = ib - (int)(plan_tile_begin(c, n_tiles, n_ctas) / n_j_tiles);
-        const double* q = partial + ((size_t)c * max_segs + seg) * 3 * IB + off;
-        a0 = __dadd_rn(a0, q[0]);
-        a1 = __dadd_rn(a1, q[IB]);
-        a2 = __dadd_rn(a2, q[2 * (size_t)IB]);
-    }
-    if (n_ctas2 > 0 && r < m_pad) {                        // TP 2: the massive body's sum over the semi-active particles
-        const int ib2 = r / IB2, off2 = r - ib2 * IB2;
-        const long long ta2 = (long long)ib2 * n_j_tiles2, tb2 = ta2 + n_j_tiles2 - 1;
-        const int c_first2 = plan_tile_owner(ta2, n_tiles2, n_ctas2), c_last2 = plan_tile_owner(tb2, n_tiles2, n_ctas2);
-        for (int c = c_first2; c <= c_last2; c++) {
-            const int seg = ib2 - (int)(plan_tile_begin(c, n_tiles2, n_ctas2) / n_j_tiles2);
-            const double* q = partial2 + ((size_t)c * max_segs2 + seg) * 3 * IB2 + off2;
-            a0 = __dadd_rn(a0, q[0]);
-            a1 = __dadd_rn(a1, q[IB2]);
-            a2 = __dadd_rn(a2, q[2 * (size_t)IB2]);
+    add_segments(rp.seg[0], r, a0, a1, a2);
+    if (rp.react && r < rp.seg[0].rec_end) {
+        // the reaction sums of the symmetric tiles that hold record r as a j-record: rows 0 .. (row of r) - 1
+        const SegPlan& q = rp.seg[0];
+        const int JT = rp.react_jt, jt = r / JT, off = r - jt * JT, rows = r / q.IB;
+        for (int I = 0; I < rows; I++) {
+            const long long t = sym_row_begin(I, q.n_j_tiles, q.r) + (jt - I * q.r);
+            const double* v = rp.react + (size_t)t * (3 * JT) + off;
+            a0 = __dadd_rn(a0, v[0]);
+            a1 = __dadd_rn(a1, v[JT]);
+            a2 = __dadd_rn(a2, v[2 * JT]);
         }
     }
+    add_segments(rp.seg[1], r, a0, a1, a2);
+    add_segments(rp.seg[2], r, a0, a1, a2);
     if (touched[r]) {                                      // the exact path's terms (fixed point, see fx_add)
         touched[r] = 0;
         unsigned long long* acc = fx + (size_t)r * (3 * GENGA_FX_LIMBS);

@@ -20,6 +20,7 @@ static int64_t cta_t0(const genga_kick_plan* p, int64_t c)
 // tile, CTA and partial-sum fields of *p (m_pad and n_rec are the caller's business).
 static void fill_tiles(genga_kick_plan* p, int64_t n_i, int64_t n_j, int32_t num_sms)
 {
+    p->symmetric = 0; p->tiles_per_iblock = 0; p->react_doubles = 0;
     const genga_variant* vars = GENGA_VARIANTS;
     for (int v = 0; v < GENGA_N_VARIANTS; v++) {
         p->threads = vars[v].threads;
@@ -97,6 +98,62 @@ extern "C" int genga_kick_make_plan_tp2(int32_t n_massive, int32_t n_test, int32
     return GENGA_KICK_OK;
 }
 
+extern "C" int genga_kick_make_plan_tprows(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan)
+{
+    if (!plan) return GENGA_KICK_E_NULL;
+    genga_kick_plan p;
+    int64_t n_i = 0;
+    const int rc = plan_records(n_massive, n_test, num_sms, &p, &n_i);
+    if (rc != GENGA_KICK_OK) return rc;
+    fill_tiles(&p, n_test, n_massive, num_sms);
+    *plan = p;
+    return GENGA_KICK_OK;
+}
+
+extern "C" int genga_kick_make_plan_sym(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan)
+{
+    if (!plan) return GENGA_KICK_E_NULL;
+    genga_kick_plan p;
+    int64_t n_i = 0;
+    const int rc = plan_records(n_massive, n_test, num_sms, &p, &n_i);
+    if (rc != GENGA_KICK_OK) return rc;
+    p.threads = GENGA_SYM_THREADS; p.i_per_thread = GENGA_SYM_IPT; p.i_block = GENGA_SYM_IBLOCK; p.j_tile = GENGA_SYM_JT;
+    p.symmetric = 1;
+    p.tiles_per_iblock = p.i_block / p.j_tile;
+    p.n_i_blocks = (int32_t)(((int64_t)n_massive + p.i_block - 1) / p.i_block);
+    p.n_j_tiles = (int32_t)(((int64_t)n_massive + p.j_tile - 1) / p.j_tile);
+    p.n_tiles = sym_row_begin(p.n_i_blocks, p.n_j_tiles, p.tiles_per_iblock);
+    p.react_doubles = p.n_tiles * 3 * p.j_tile;
+    p.n_ctas = num_sms;                                                // one CTA of 256 threads x 8 i-bodies per SM
+    const bool use = n_massive >= GENGA_SYM_MIN_BODIES && p.react_doubles * (int64_t)sizeof(double) <= GENGA_SYM_MAX_REACT_BYTES;
+    if (!use) p.n_ctas = 0;
+    if (p.n_tiles < p.n_ctas) p.n_ctas = (int32_t)p.n_tiles;
+    int32_t max_segs = 1;
+    for (int64_t c = 0; c < p.n_ctas; c++) {
+        const int64_t t0 = cta_t0(&p, c), t1 = cta_t0(&p, c + 1);
+        if (t1 <= t0) continue;
+        const int32_t segs = sym_row_of(t1 - 1, p.n_j_tiles, p.tiles_per_iblock, p.n_i_blocks) -
+                             sym_row_of(t0, p.n_j_tiles, p.tiles_per_iblock, p.n_i_blocks) + 1;
+        if (segs > max_segs) max_segs = segs;
+    }
+    p.max_segs = max_segs;
+    p.partial_doubles = (int64_t)p.n_ctas * p.max_segs * 3 * p.i_block;
+    *plan = p;
+    return GENGA_KICK_OK;
+}
+
+extern "C" int64_t genga_kick_plan_sym_row_begin(const genga_kick_plan* plan, int32_t row)
+{
+    if (!plan || !plan->symmetric || row < 0 || row > plan->n_i_blocks) return -1;
+    return sym_row_begin(row, plan->n_j_tiles, plan->tiles_per_iblock);
+}
+
+extern "C" int32_t genga_kick_plan_sym_row_of(const genga_kick_plan* plan, int64_t t)
+{
+    if (!plan || !plan->symmetric || t < 0 || t >= plan->n_tiles) return -1;
+    return sym_row_of(t, plan->n_j_tiles, plan->tiles_per_iblock, plan->n_i_blocks);
+}
+
 extern "C" int genga_kick_plan_cta_range(const genga_kick_plan* plan, int32_t cta, int64_t* t0, int64_t* t1)
 {
     if (!plan || !t0 || !t1) return GENGA_KICK_E_NULL;
@@ -113,7 +170,9 @@ extern "C" int genga_kick_plan_iblock_ctas(const genga_kick_plan* plan, int32_t 
     // the CTA that owns tile t is the largest c with floor(c T / C) <= t,
     // i.e. c = floor(((t + 1) C - 1) / T)
     const int64_t T = plan->n_tiles, C = plan->n_ctas;
-    const int64_t ta = (int64_t)ib * plan->n_j_tiles, tb = ta + plan->n_j_tiles - 1;
+    if (C <= 0) return GENGA_KICK_E_SIZE;
+    const int64_t ta = plan->symmetric ? sym_row_begin(ib, plan->n_j_tiles, plan->tiles_per_iblock) : (int64_t)ib * plan->n_j_tiles;
+    const int64_t tb = plan->symmetric ? sym_row_begin(ib + 1, plan->n_j_tiles, plan->tiles_per_iblock) - 1 : ta + plan->n_j_tiles - 1;
     *c_first = plan_tile_owner(ta, T, C);
     *c_last = plan_tile_owner(tb, T, C);
     return GENGA_KICK_OK;

@@ -20,6 +20,29 @@ GENGA_HD long long plan_tile_begin(long long c, long long T, long long C) { retu
 // The CTA that owns tile t: the largest c with floor(c T / C) <= t.
 GENGA_HD int plan_tile_owner(long long t, long long T, long long C) { return (int)(((t + 1) * C - 1) / T); }
 
+// ---- the symmetric level-0 pair loop (kick_sym_kernel): massive x massive, every unordered pair once ----
+// Rows = i-blocks of GENGA_SYM_IBLOCK records; row I holds the j-tiles jt = I r .. n_jt - 1 (r = i_block / j_tile): the
+// first r of them overlap the i-block itself (the DIAGONAL tiles, evaluated one-sidedly), the others lie beyond it (the
+// SYMMETRIC tiles: the force on i and the reaction on j from one evaluation).  Tiles are numbered row-major.
+static const int GENGA_SYM_THREADS = 256;
+static const int GENGA_SYM_IPT = 8;
+static const int GENGA_SYM_JT = 256;               // = 32 x warps of the CTA (one j-group per warp and phase)
+static const int GENGA_SYM_IBLOCK = GENGA_SYM_THREADS * GENGA_SYM_IPT;
+static const int GENGA_SYM_MIN_BODIES = 24576;     // below this the one-sided kernel's finer tiles balance better
+static const int64_t GENGA_SYM_MAX_REACT_BYTES = (int64_t)2 << 30;   // reaction partial sums: T x 3 x JT doubles
+// first tile of row I
+GENGA_HD long long sym_row_begin(long long I, long long n_jt, long long r) { return I * n_jt - r * (I * (I - 1) / 2); }
+// the row that holds tile t (rows 0 .. n_rows - 1, t < sym_row_begin(n_rows))
+GENGA_HD int sym_row_of(long long t, long long n_jt, long long r, int n_rows)
+{
+    int lo = 0, hi = n_rows - 1;                   // largest I with sym_row_begin(I) <= t
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (sym_row_begin(mid, n_jt, r) <= t) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
 struct genga_variant {
     int32_t threads;
     int32_t i_per_thread;

@@ -102,6 +102,57 @@ def test_tp2_last_iblock_reaches_past_the_massive_records(oracle_mod, nm, nt):
     assert np.all(np.abs(p) <= TOL * (ki.mass * orc.S).sum(axis=1))
 
 
+def _tp_masses(ki, seed):
+    u = gi.uniforms(seed, 0, ki.n_test)
+    ki.mass = ki.mass.copy()
+    ki.mass[ki.n_massive:] = 1e-12 * (0.5 + u)
+    return ki
+
+
+@pytest.mark.parametrize("nm,nt,tp_mode,order_mode", [(24577, 0, 1, 0), (30001, 20000, 1, 0), (30001, 20000, 2, 0),
+                                                      (26000, 0, 1, 1), (40000, 300, 2, 2)])
+def test_symmetric_pass_ragged_sizes_and_particles(oracle_mod, nm, nt, tp_mode, order_mode):
+    """The symmetric level-0 pass (every unordered massive pair once, from 24,576 massive bodies on) at sizes that are
+    multiples of neither its 2048-record i-blocks nor its 256-record j-tiles, alone, beside the particles' one-sided
+    rows (TP 1) and beside TP 2's transposed pass; caller's order, sorted order and auto."""
+    from paper_2201_10058_b200 import binding
+    import torch
+    assert binding.make_plan_sym(nm, nt, torch.cuda.get_device_properties(0).multi_processor_count).n_ctas > 0
+    ki = gi.make_config(3 if nt == 0 else 4, n=nm, n_test=nt if nt else None, level=0)
+    if tp_mode == 2:
+        ki = _tp_masses(ki, 79)
+    gpu = run_gpu(ki, level=0, capacity=CAPACITY, order_mode=order_mode, tp_mode=tp_mode)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n_massive, ki.n_test, level=0, G=ki.G, maxp=256, tp_mode=tp_mode)
+    assert gpu.status == 0 and not orc.coincident
+    d = compare(gpu, orc, ki.n_massive, tol=TOL)
+    assert gpu.total == len(gpu.pairs) and gpu.total > 1000
+    nmom = ki.n if tp_mode == 2 else ki.n_massive           # TP 2: every term has its reaction
+    p = (ki.mass[:nmom] * gpu.acc[:, :nmom]).sum(axis=1)
+    assert np.all(np.abs(p) <= TOL * (ki.mass[:nmom] * orc.S[:, :nmom]).sum(axis=1))
+    print(f"nm={nm} nt={nt} tp={tp_mode} order={order_mode}: {gpu.total} pairs, max |da|/S = {d['max_err_over_S']:.2e}")
+
+
+def test_symmetric_pass_candidate_list_overflow(oracle_mod):
+    """More pairs inside critical radii than the candidate list holds (64 per body), with the symmetric pass as the
+    far field: the fallback search repeats the pair loop's trip rule on the same bits, so the result is complete."""
+    import paper_2201_10058_b200 as g
+    ki = gi.make_config(3, n=24576, level=0)
+    ki.rcrit = ki.rcrit * 4.0
+    gpu = run_gpu(ki, level=0, capacity=1 << 23, order_mode=0)
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n, 0, level=0, G=ki.G, maxp=4096)
+    assert gpu.status == g.STATUS_CAND_OVERFLOW and gpu.total > 64 * ki.n // 2
+    gpu.status = 0
+    compare(gpu, orc, ki.n, tol=TOL)
+
+
+def test_symmetric_pass_is_bit_reproducible():
+    ki = gi.make_config(3, n=33000, level=0)
+    a = run_gpu(ki, level=0, capacity=CAPACITY, with_vel=True)
+    b = run_gpu(ki, level=0, capacity=CAPACITY, with_vel=True)
+    assert np.array_equal(a.acc, b.acc) and np.array_equal(a.counts, b.counts) and np.array_equal(a.vel, b.vel)
+    assert np.array_equal(sorted(map(tuple, a.pairs.tolist())), sorted(map(tuple, b.pairs.tolist())))
+
+
 def test_config1_hundred_kicks(oracle_mod):
     """N = 8192, 100 kicks separated by an oracle-matched heliocentric drift: both sides see the
     same state at every step (the harness advances it with the ORACLE's acceleration), the

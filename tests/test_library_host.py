@@ -151,6 +151,49 @@ def test_tp2_plan_covers_every_tile_once(built, nm, nt):
     assert d["partial_doubles"] == d["n_ctas"] * d["max_segs"] * 3 * d["i_block"]
 
 
+@pytest.mark.parametrize("nm,nt", [(65536, 0), (32770, 0), (24576, 0), (30001, 7), (65536, 1048576), (24575, 0), (100, 0)])
+def test_symmetric_plan_covers_every_unordered_tile_once(built, nm, nt):
+    """Level 0, massive x massive, every unordered pair once: rows of 2048-record i-blocks, row I holding the 256-record
+    j-tiles jt >= 8 I, numbered row-major; CTA ranges contiguous and balanced; the particles' rows one-sided beside it."""
+    sms = 148
+    p = g.make_plan_sym(nm, nt, sms)
+    d = p.as_dict()
+    assert d["symmetric"] == 1 and d["i_block"] == 2048 and d["j_tile"] == 256 and d["tiles_per_iblock"] == 8
+    if nm < 24576:
+        assert d["n_ctas"] == 0                       # the library keeps the one-sided kernel for small N
+        return
+    rows, njt, r = d["n_i_blocks"], d["n_j_tiles"], d["tiles_per_iblock"]
+    assert rows * 2048 >= nm > (rows - 1) * 2048 and njt * 256 >= nm > (njt - 1) * 256
+    # every (i-block, j-tile) with the j-tile at or beyond the i-block's first tile appears exactly once
+    want = [(I, jt) for I in range(rows) for jt in range(I * r, njt)]
+    assert d["n_tiles"] == len(want) and d["react_doubles"] == len(want) * 3 * 256
+    for t in sorted({0, 1, len(want) // 3, len(want) // 2, len(want) - 2, len(want) - 1} | set(range(njt - 2, njt + 3))):
+        I = g.plan_sym_row_of(p, t)
+        assert (I, I * r + t - g.plan_sym_row_begin(p, I)) == want[t]
+    assert g.plan_sym_row_begin(p, rows) == d["n_tiles"]
+    # the unordered massive pairs are covered: tiles beyond the diagonal blocks + the diagonal blocks (one-sided there)
+    assert d["n_ctas"] == sms
+    prev, sizes, segs = 0, [], 1
+    for c in range(d["n_ctas"]):
+        t0, t1 = g.plan_cta_range(p, c)
+        assert t0 == prev and t1 > t0
+        prev = t1
+        sizes.append(t1 - t0)
+        segs = max(segs, g.plan_sym_row_of(p, t1 - 1) - g.plan_sym_row_of(p, t0) + 1)
+    assert prev == d["n_tiles"] and max(sizes) - min(sizes) <= 1
+    assert d["max_segs"] == segs and d["partial_doubles"] == sms * segs * 3 * 2048
+    for ib in sorted({0, rows // 2, rows - 1}):
+        a, b = g.plan_iblock_ctas(p, ib)
+        ta, tb = g.plan_sym_row_begin(p, ib), g.plan_sym_row_begin(p, ib + 1)
+        meets = [c for c in range(d["n_ctas"]) if (lambda q: q[0] < tb and q[1] > ta)(g.plan_cta_range(p, c))]
+        assert meets == list(range(a, b + 1))
+    if nt:
+        q = g.make_plan_tprows(nm, nt, sms).as_dict()
+        assert q["symmetric"] == 0 and q["m_pad"] == d["m_pad"] and q["n_i_blocks"] * q["i_block"] >= nt
+        assert q["n_j_tiles"] * q["j_tile"] >= nm and q["n_tiles"] == q["n_i_blocks"] * q["n_j_tiles"]
+        assert q["m_pad"] + q["n_i_blocks"] * q["i_block"] <= q["n_rec"]
+
+
 def test_plan_errors(built):
     with pytest.raises(g.GengaKickError) as e:
         g.make_plan(0, 0, 0, 148)
