@@ -117,6 +117,10 @@ int genga_kick_make_plan_sym(int32_t n_massive, int32_t n_test, int32_t num_sms,
  * symmetric plan: same tile / CTA / partial-sum scheme as genga_kick_make_plan, i-blocks counted from record m_pad.
  * Errors: E_NULL, E_SIZE. */
 int genga_kick_make_plan_tprows(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan);
+/* Symmetric plans: the first tile of every CTA, cta_first_tile[0 .. n_ctas] (the last entry is n_tiles).  The ranges
+ * are contiguous and ascending but not equally long: they balance a cost model in which a diagonal tile (ordered
+ * pairs, mostly inside filter radii) weighs 1.4 symmetric tiles.  Errors: E_NULL, E_SIZE (not a symmetric plan in use). */
+int genga_kick_plan_sym_table(const genga_kick_plan* plan, int64_t* cta_first_tile);
 /* Symmetric plans: first tile of row `row` (row = n_i_blocks gives n_tiles) and the row of tile t. */
 int64_t genga_kick_plan_sym_row_begin(const genga_kick_plan* plan, int32_t row);
 int32_t genga_kick_plan_sym_row_of(const genga_kick_plan* plan, int64_t t);

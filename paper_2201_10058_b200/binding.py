@@ -17,7 +17,7 @@ ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 
 EXPORTS = (
     "genga_kick_make_plan", "genga_kick_make_plan_tp2", "genga_kick_make_plan_sym", "genga_kick_make_plan_tprows",
-    "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
+    "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of", "genga_kick_plan_sym_table", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
     "genga_kick_set_stream", "genga_kick", "genga_kick_list", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
@@ -79,6 +79,7 @@ def lib():
         L.genga_kick_make_plan_tp2.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
         L.genga_kick_make_plan_sym.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
         L.genga_kick_make_plan_tprows.argtypes = [i32, i32, i32, C.POINTER(GengaKickPlan)]
+        L.genga_kick_plan_sym_table.argtypes = [C.POINTER(GengaKickPlan), vp]
         L.genga_kick_plan_sym_row_begin.argtypes = [C.POINTER(GengaKickPlan), i32]
         L.genga_kick_plan_sym_row_begin.restype = i64
         L.genga_kick_plan_sym_row_of.argtypes = [C.POINTER(GengaKickPlan), i64]

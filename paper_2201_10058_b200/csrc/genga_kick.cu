@@ -12,6 +12,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 namespace {
 
@@ -102,6 +103,13 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
         if (ctx->plan_sym.n_ctas > 0) {
             if ((e = cudaMalloc(&ctx->partial_sym, (size_t)ctx->plan_sym.partial_doubles * sizeof(double))) != cudaSuccess) goto cuda_error;
             if ((e = cudaMalloc(&ctx->react, (size_t)ctx->plan_sym.react_doubles * sizeof(double))) != cudaSuccess) goto cuda_error;
+            {
+                std::vector<int64_t> tab((size_t)ctx->plan_sym.n_ctas + 1, 0);
+                rc = genga_kick_plan_sym_table(&ctx->plan_sym, tab.data());
+                if (rc != GENGA_KICK_OK) goto fail;
+                if ((e = cudaMalloc(&ctx->sym_t0, tab.size() * sizeof(long long))) != cudaSuccess) goto cuda_error;
+                if ((e = cudaMemcpy(ctx->sym_t0, tab.data(), tab.size() * sizeof(long long), cudaMemcpyHostToDevice)) != cudaSuccess) goto cuda_error;
+            }
             if (cfg->n_test > 0) {
                 rc = genga_kick_make_plan_tprows(cfg->n_massive, cfg->n_test, ctx->num_sms, &ctx->plan_tprows);
                 if (rc != GENGA_KICK_OK) goto fail;
@@ -217,7 +225,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             ks.n_j_tiles = ps.n_j_tiles; ks.n_ctas = ps.n_ctas; ks.max_segs = ps.max_segs; ks.n_tiles = ps.n_tiles;
             ks.partial = ctx->partial_sym;
             ks.i_rec_end = (ctx->cfg.n_massive + 31) / 32 * 32;
-            genga::SymParams sp = {ps.n_i_blocks, ps.tiles_per_iblock, ctx->react};
+            genga::SymParams sp = {ps.n_i_blocks, ps.tiles_per_iblock, ctx->react, ctx->sym_t0};
             genga::kick_sym_kernel<GENGA_SYM_THREADS, GENGA_SYM_IPT, GENGA_STAGES><<<ps.n_ctas, GENGA_SYM_THREADS, 0, st>>>(ks, sp);
             GK_CUDA(ctx, cudaGetLastError());
             if (ctx->plan_tprows.n_ctas > 0) {
@@ -283,6 +291,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         genga::ReduceParams rp = {};
         if (use_sym) {
             rp.seg[0] = seg_of(ctx->plan_sym, ctx->partial_sym, 0, pl.m_pad, true);
+            rp.seg[0].tbegin = ctx->sym_t0;
             rp.react = ctx->react; rp.react_jt = ctx->plan_sym.j_tile;
             rp.seg[2] = seg_of(ctx->plan_tprows, ctx->partial, pl.m_pad, n_rec, ctx->plan_tprows.n_ctas > 0);
         } else {
@@ -507,7 +516,7 @@ extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return c
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)
 {
     if (!ctx) return GENGA_KICK_OK;
-    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->partial_sym, ctx->react, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
+    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->partial_sym, ctx->react, ctx->sym_t0, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
                     ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->partial2, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs,
                     ctx->psum_partial, ctx->psum_ticket, ctx->step_rcrit, ctx->grp_label, ctx->grp_flag,

@@ -18,6 +18,7 @@ struct genga_kick_ctx {
     genga_kick_plan plan_tprows;   // ... and the one-sided rows of the semi-active particles beside it
     double* partial_sym;           // i-side partial sums of the symmetric pass
     double* react;                 // its reaction sums, one slot per tile
+    long long* sym_t0;             // [n_ctas + 1] first tile of every CTA of the symmetric pass (device)
     // scratch (device)
     double2* rxy;
     double2* rzm;

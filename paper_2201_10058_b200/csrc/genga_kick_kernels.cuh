@@ -944,6 +944,7 @@ struct SegPlan {                       // the partial segments one pair-loop pas
     long long n_tiles;
     int rec0, rec_end;                 // the pass served the i-records [rec0, rec_end), i-block 0 at rec0
     int symmetric, r, n_rows;          // kick_sym_kernel's row-major triangular tile numbering (genga_kick_variants.h)
+    const long long* __restrict__ tbegin;  // symmetric: [n_ctas + 1] first tile of every CTA; else nullptr (c T / C)
 };
 
 struct ReduceParams {
@@ -959,9 +960,23 @@ __device__ __forceinline__ void add_segments(const SegPlan& q, int r, double& a0
     const long long ta = q.symmetric ? sym_row_begin(ib, q.n_j_tiles, q.r) : (long long)ib * q.n_j_tiles;
     const long long tb = (q.symmetric ? sym_row_begin(ib + 1, q.n_j_tiles, q.r) : ta + q.n_j_tiles) - 1;
     if (tb < ta) return;
-    const int c_first = plan_tile_owner(ta, q.n_tiles, q.n_ctas), c_last = plan_tile_owner(tb, q.n_tiles, q.n_ctas);
+    int c_first, c_last;
+    if (q.tbegin) {                                        // the largest c with tbegin[c] <= t (empty ranges repeat a value)
+        auto owner = [&](long long t) {
+            int lo = 0, hi = q.n_ctas - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (q.tbegin[mid] <= t) lo = mid; else hi = mid - 1;
+            }
+            return lo;
+        };
+        c_first = owner(ta); c_last = owner(tb);
+    } else {
+        c_first = plan_tile_owner(ta, q.n_tiles, q.n_ctas); c_last = plan_tile_owner(tb, q.n_tiles, q.n_ctas);
+    }
     for (int c = c_first; c <= c_last; c++) {
-        const long long tc = plan_tile_begin(c, q.n_tiles, q.n_ctas);
+        const long long tc = q.tbegin ? q.tbegin[c] : plan_tile_begin(c, q.n_tiles, q.n_ctas);
+        if (q.tbegin && q.tbegin[c + 1] <= tc) continue;   // a CTA without tiles wrote nothing
         const int seg = ib - (q.symmetric ? sym_row_of(tc, q.n_j_tiles, q.r, q.n_rows) : (int)(tc / q.n_j_tiles));
         const double* v = q.partial + ((size_t)c * q.max_segs + seg) * 3 * q.IB + off;
         a0 = __dadd_rn(a0, v[0]);

@@ -11,6 +11,8 @@
 #include "../../include/genga_kick.h"
 #include "genga_kick_variants.h"
 
+#include <vector>
+
 static int64_t cta_t0(const genga_kick_plan* p, int64_t c)
 {
     return plan_tile_begin(c, p->n_tiles, p->n_ctas);
@@ -110,6 +112,38 @@ extern "C" int genga_kick_make_plan_tprows(int32_t n_massive, int32_t n_test, in
     return GENGA_KICK_OK;
 }
 
+// Symmetric plans: first tile of every CTA under the cost model of genga_kick_variants.h; out[n_ctas] = n_tiles.
+// Tile t (row-major) belongs to CTA floor(W(t) C / W_total), W(t) = cost of the tiles before t: ranges are contiguous,
+// ascending and a fixed function of the plan.
+static void sym_cta_table(const genga_kick_plan* p, int64_t* out)
+{
+    const int64_t C = p->n_ctas;
+    int64_t Wtot = 0;
+    for (int64_t I = 0; I < p->n_i_blocks; I++) {
+        const int64_t count = p->n_j_tiles - I * p->tiles_per_iblock;
+        const int64_t nd = count < p->tiles_per_iblock ? count : p->tiles_per_iblock;
+        Wtot += nd * GENGA_SYM_COST_DIAG + (count - nd) * GENGA_SYM_COST_SYM;
+    }
+    int64_t t = 0, W = 0, next = 0;                       // next: the CTA whose first tile is looked for
+    for (int64_t I = 0; I < p->n_i_blocks; I++) {
+        const int64_t count = p->n_j_tiles - I * p->tiles_per_iblock;
+        for (int64_t q = 0; q < count; q++, t++) {
+            const int64_t owner = W * C / Wtot;
+            while (next <= owner && next < C) out[next++] = t;
+            W += q < p->tiles_per_iblock ? GENGA_SYM_COST_DIAG : GENGA_SYM_COST_SYM;
+        }
+    }
+    while (next <= C) out[next++] = t;
+}
+
+extern "C" int genga_kick_plan_sym_table(const genga_kick_plan* plan, int64_t* cta_first_tile)
+{
+    if (!plan || !cta_first_tile) return GENGA_KICK_E_NULL;
+    if (!plan->symmetric || plan->n_ctas <= 0) return GENGA_KICK_E_SIZE;
+    sym_cta_table(plan, cta_first_tile);
+    return GENGA_KICK_OK;
+}
+
 extern "C" int genga_kick_make_plan_sym(int32_t n_massive, int32_t n_test, int32_t num_sms, genga_kick_plan* plan)
 {
     if (!plan) return GENGA_KICK_E_NULL;
@@ -129,8 +163,10 @@ extern "C" int genga_kick_make_plan_sym(int32_t n_massive, int32_t n_test, int32
     if (!use) p.n_ctas = 0;
     if (p.n_tiles < p.n_ctas) p.n_ctas = (int32_t)p.n_tiles;
     int32_t max_segs = 1;
+    std::vector<int64_t> tab((size_t)p.n_ctas + 1, 0);
+    if (p.n_ctas > 0) sym_cta_table(&p, tab.data());
     for (int64_t c = 0; c < p.n_ctas; c++) {
-        const int64_t t0 = cta_t0(&p, c), t1 = cta_t0(&p, c + 1);
+        const int64_t t0 = tab[(size_t)c], t1 = tab[(size_t)c + 1];
         if (t1 <= t0) continue;
         const int32_t segs = sym_row_of(t1 - 1, p.n_j_tiles, p.tiles_per_iblock, p.n_i_blocks) -
                              sym_row_of(t0, p.n_j_tiles, p.tiles_per_iblock, p.n_i_blocks) + 1;
@@ -158,6 +194,13 @@ extern "C" int genga_kick_plan_cta_range(const genga_kick_plan* plan, int32_t ct
 {
     if (!plan || !t0 || !t1) return GENGA_KICK_E_NULL;
     if (cta < 0 || cta >= plan->n_ctas) return GENGA_KICK_E_SIZE;
+    if (plan->symmetric) {
+        std::vector<int64_t> tab((size_t)plan->n_ctas + 1, 0);
+        sym_cta_table(plan, tab.data());
+        *t0 = tab[(size_t)cta];
+        *t1 = tab[(size_t)cta + 1];
+        return GENGA_KICK_OK;
+    }
     *t0 = cta_t0(plan, cta);
     *t1 = cta_t0(plan, (int64_t)cta + 1);
     return GENGA_KICK_OK;
@@ -171,6 +214,21 @@ extern "C" int genga_kick_plan_iblock_ctas(const genga_kick_plan* plan, int32_t 
     // i.e. c = floor(((t + 1) C - 1) / T)
     const int64_t T = plan->n_tiles, C = plan->n_ctas;
     if (C <= 0) return GENGA_KICK_E_SIZE;
+    if (plan->symmetric) {
+        std::vector<int64_t> tab((size_t)C + 1, 0);
+        sym_cta_table(plan, tab.data());
+        const int64_t a = sym_row_begin(ib, plan->n_j_tiles, plan->tiles_per_iblock);
+        const int64_t b = sym_row_begin(ib + 1, plan->n_j_tiles, plan->tiles_per_iblock) - 1;
+        int32_t first = -1, last = -1;
+        for (int64_t c = 0; c < C; c++) {
+            if (tab[(size_t)c + 1] <= tab[(size_t)c]) continue;
+            if (first < 0 && tab[(size_t)c + 1] > a) first = (int32_t)c;
+            if (tab[(size_t)c] <= b) last = (int32_t)c;
+        }
+        *c_first = first;
+        *c_last = last;
+        return GENGA_KICK_OK;
+    }
     const int64_t ta = plan->symmetric ? sym_row_begin(ib, plan->n_j_tiles, plan->tiles_per_iblock) : (int64_t)ib * plan->n_j_tiles;
     const int64_t tb = plan->symmetric ? sym_row_begin(ib + 1, plan->n_j_tiles, plan->tiles_per_iblock) - 1 : ta + plan->n_j_tiles - 1;
     *c_first = plan_tile_owner(ta, T, C);

@@ -4,13 +4,13 @@
 // Why: an ordered pair costs 16 FP64-pipe instructions, an unordered pair 20 (3 DADD + 3 for r^2 + 6 for r^-3 + 2
 // products with G m_j, G m_i + 6 accumulating DFMAs) instead of 32 -- measured 46.7 issue cycles per warp and unordered
 // pair against 2 x 36 (profiles/ncu_r02*.md).  The FP64 pipe's dispatch port is the bottleneck (2 cycles per FP64
-// instruction, 1 per anything else), so the loop is built to issue as little else as possible: 8 i-bodies per thread.
+// instruction, 1 per anything else), so the loop is built to issue as little else as possible: 6 i-bodies per thread.
 //
-// How.  The pair matrix of the massive records is cut into rows (i-blocks of 2048 records) x j-tiles of 256 records;
-// row I only holds the tiles jt >= 8 I (genga_kick_variants.h).  The 8 tiles that overlap the i-block itself (DIAGONAL)
+// How.  The pair matrix of the massive records is cut into rows (i-blocks of 1536 records) x j-tiles of 256 records;
+// row I only holds the tiles jt >= 6 I (genga_kick_variants.h).  The 6 tiles that overlap the i-block itself (DIAGONAL)
 // are evaluated one-sidedly exactly as kick_kernel does.  In every other tile (SYMMETRIC) a warp walks the tile's
 // eight 32-record groups; lane l starts a group at its record l and moves on by one record per step (32 steps):
-// at step s it evaluates its 8 i-bodies against j-record (l + s) mod 32, read from shared memory (every lane another
+// at step s it evaluates its 6 i-bodies against j-record (l + s) mod 32, read from shared memory (every lane another
 // record: conflict-free), adds s_i d to its own sums and -s_j d to the j-record's running reaction sum, which travels
 // round the warp by shuffle (3 doubles per step) and is back at lane l after 32 steps.  The eight warps of the CTA
 // visit the groups in rotated order (warp w starts at group w), and hand a group's reaction sum on through shared
@@ -94,6 +94,7 @@ struct SymParams {
     int n_rows;                        // i-blocks
     int r;                             // tiles_per_iblock
     double* __restrict__ react;        // [n_tiles][3][JT]
+    const long long* __restrict__ cta_t0;   // [n_ctas + 1] first tile of every CTA (genga_kick_plan_sym_table)
 };
 
 template <int THREADS, int IPT, int STAGES>
@@ -112,12 +113,12 @@ __global__ void __launch_bounds__(THREADS, 1) kick_sym_kernel(const KickParams p
     __shared__ double rs[3][JT];                            // a group's reaction sum on its way through the warps
     __shared__ volatile int cnt[NG];                        // contributions a group's sum has taken so far
     __shared__ float4 wblo[WARPS], wbhi[WARPS];             // box of each warp's i-records (.w of lo: largest filter word)
+    __shared__ float4 wslo[WARPS][IPT], wshi[WARPS][IPT];   // ... and of each of its IPT slices of 32 records
     __shared__ CandCursor ccs[WARPS];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int woff = warp * (32 * IPT) + lane;
-    const long long t0 = plan_tile_begin(blockIdx.x, p.n_tiles, p.n_ctas);
-    const long long t1 = plan_tile_begin(blockIdx.x + 1, p.n_tiles, p.n_ctas);
+    const long long t0 = sp.cta_t0[blockIdx.x], t1 = sp.cta_t0[blockIdx.x + 1];
     if (t0 >= t1) return;
 
     if (tid == 0) {
@@ -192,11 +193,16 @@ __global__ void __launch_bounds__(THREADS, 1) kick_sym_kernel(const KickParams p
                 if (r >= (size_t)p.i_rec_end) {             // whole groups of 32 records (i_rec_end is a multiple of 32)
                     xi[k] = yi[k] = zi[k] = GENGA_SENTINEL_POS;
                     gi[k] = 0.0;
+                    if (lane == 0) {                        // an empty box, near to nothing
+                        wslo[warp][k] = make_float4(3.0e38f, 3.0e38f, 3.0e38f, __int_as_float(-1));
+                        wshi[warp][k] = make_float4(-3.0e38f, -3.0e38f, -3.0e38f, 0.0f);
+                    }
                     continue;
                 }
                 const double2 a = p.rxy[r], b = p.rzm[r];
                 xi[k] = a.x; yi[k] = a.y; zi[k] = b.x; gi[k] = b.y;
                 const float4 glo = p.cblo[r / GENGA_GROUP], ghi = p.cbhi[r / GENGA_GROUP];
+                if (lane == 0) { wslo[warp][k] = glo; wshi[warp][k] = ghi; }
                 lo.x = fminf(lo.x, glo.x); lo.y = fminf(lo.y, glo.y); lo.z = fminf(lo.z, glo.z);
                 hi.x = fmaxf(hi.x, ghi.x); hi.y = fmaxf(hi.y, ghi.y); hi.z = fmaxf(hi.z, ghi.z);
                 wfw = max(wfw, __float_as_int(glo.w));
@@ -263,7 +269,14 @@ __global__ void __launch_bounds__(THREADS, 1) kick_sym_kernel(const KickParams p
             for (int ph = 0; ph < WARPS; ph++) {
                 const int g = (warp + ph) % NG, j0 = g * GENGA_GROUP;
                 double rx = 0.0, ry = 0.0, rz = 0.0;
-                if (!((nearmask >> g) & 1u)) {
+                // the warp's box (256 records) is near the group: look again slice by slice (32 records each)
+                bool checked = (nearmask >> g) & 1u;
+                if (checked) {
+                    const bool kn = lane < IPT ? boxes_near(wslo[warp][lane], wshi[warp][lane], __float_as_int(wslo[warp][lane].w),
+                                                            S.blo[g], S.bhi[g]) : false;
+                    checked = __ballot_sync(0xffffffffu, kn) != 0u;
+                }
+                if (!checked) {
 #pragma unroll 2
                     for (int q = 0; q < 32; q++) {
                         const int jj = j0 + ((lane + q) & 31);

@@ -21,15 +21,23 @@ GENGA_HD long long plan_tile_begin(long long c, long long T, long long C) { retu
 GENGA_HD int plan_tile_owner(long long t, long long T, long long C) { return (int)(((t + 1) * C - 1) / T); }
 
 // ---- the symmetric level-0 pair loop (kick_sym_kernel): massive x massive, every unordered pair once ----
+// (6 i-bodies per thread: 254 registers without spills; 8 would issue 4 % fewer instructions per pair but leaves the
+// register allocator no room, and the smaller tiles balance better.)
 // Rows = i-blocks of GENGA_SYM_IBLOCK records; row I holds the j-tiles jt = I r .. n_jt - 1 (r = i_block / j_tile): the
 // first r of them overlap the i-block itself (the DIAGONAL tiles, evaluated one-sidedly), the others lie beyond it (the
 // SYMMETRIC tiles: the force on i and the reaction on j from one evaluation).  Tiles are numbered row-major.
 static const int GENGA_SYM_THREADS = 256;
-static const int GENGA_SYM_IPT = 8;
+static const int GENGA_SYM_IPT = 6;
 static const int GENGA_SYM_JT = 256;               // = 32 x warps of the CTA (one j-group per warp and phase)
 static const int GENGA_SYM_IBLOCK = GENGA_SYM_THREADS * GENGA_SYM_IPT;
 static const int GENGA_SYM_MIN_BODIES = 24576;     // below this the one-sided kernel's finer tiles balance better
 static const int64_t GENGA_SYM_MAX_REACT_BYTES = (int64_t)2 << 30;   // reaction partial sums: T x 3 x JT doubles
+// Cost model of the static partition (CTA c owns the tiles whose cumulative cost starts in [c W / C, (c + 1) W / C)):
+// a diagonal tile evaluates i_block x j_tile ORDERED pairs, most of them in the checked loop (the block's own bodies
+// and their neighbours are inside each other's filter radius), a symmetric tile as many UNORDERED pairs in the bare
+// loop; measured on the disks of BASELINE.json (profiles/ncu_r02*.md).
+static const int GENGA_SYM_COST_SYM = 10;
+static const int GENGA_SYM_COST_DIAG = 14;
 // first tile of row I
 GENGA_HD long long sym_row_begin(long long I, long long n_jt, long long r) { return I * n_jt - r * (I * (I - 1) / 2); }
 // the row that holds tile t (rows 0 .. n_rows - 1, t < sym_row_begin(n_rows))

@@ -113,7 +113,7 @@ def _tp_masses(ki, seed):
                                                       (26000, 0, 1, 1), (40000, 300, 2, 2)])
 def test_symmetric_pass_ragged_sizes_and_particles(oracle_mod, nm, nt, tp_mode, order_mode):
     """The symmetric level-0 pass (every unordered massive pair once, from 24,576 massive bodies on) at sizes that are
-    multiples of neither its 2048-record i-blocks nor its 256-record j-tiles, alone, beside the particles' one-sided
+    multiples of neither its 1536-record i-blocks nor its 256-record j-tiles, alone, beside the particles' one-sided
     rows (TP 1) and beside TP 2's transposed pass; caller's order, sorted order and auto."""
     from paper_2201_10058_b200 import binding
     import torch

@@ -153,17 +153,19 @@ def test_tp2_plan_covers_every_tile_once(built, nm, nt):
 
 @pytest.mark.parametrize("nm,nt", [(65536, 0), (32770, 0), (24576, 0), (30001, 7), (65536, 1048576), (24575, 0), (100, 0)])
 def test_symmetric_plan_covers_every_unordered_tile_once(built, nm, nt):
-    """Level 0, massive x massive, every unordered pair once: rows of 2048-record i-blocks, row I holding the 256-record
-    j-tiles jt >= 8 I, numbered row-major; CTA ranges contiguous and balanced; the particles' rows one-sided beside it."""
+    """Level 0, massive x massive, every unordered pair once: rows of 1536-record i-blocks, row I holding the 256-record
+    j-tiles jt >= 6 I, numbered row-major; CTA ranges contiguous, balanced under the cost model (a diagonal tile weighs
+    1.4 symmetric tiles); the particles' rows one-sided beside it."""
     sms = 148
     p = g.make_plan_sym(nm, nt, sms)
     d = p.as_dict()
-    assert d["symmetric"] == 1 and d["i_block"] == 2048 and d["j_tile"] == 256 and d["tiles_per_iblock"] == 8
+    IB = 1536
+    assert d["symmetric"] == 1 and d["i_block"] == IB and d["j_tile"] == 256 and d["tiles_per_iblock"] == 6
     if nm < 24576:
         assert d["n_ctas"] == 0                       # the library keeps the one-sided kernel for small N
         return
     rows, njt, r = d["n_i_blocks"], d["n_j_tiles"], d["tiles_per_iblock"]
-    assert rows * 2048 >= nm > (rows - 1) * 2048 and njt * 256 >= nm > (njt - 1) * 256
+    assert rows * IB >= nm > (rows - 1) * IB and njt * 256 >= nm > (njt - 1) * 256
     # every (i-block, j-tile) with the j-tile at or beyond the i-block's first tile appears exactly once
     want = [(I, jt) for I in range(rows) for jt in range(I * r, njt)]
     assert d["n_tiles"] == len(want) and d["react_doubles"] == len(want) * 3 * 256
@@ -173,19 +175,24 @@ def test_symmetric_plan_covers_every_unordered_tile_once(built, nm, nt):
     assert g.plan_sym_row_begin(p, rows) == d["n_tiles"]
     # the unordered massive pairs are covered: tiles beyond the diagonal blocks + the diagonal blocks (one-sided there)
     assert d["n_ctas"] == sms
-    prev, sizes, segs = 0, [], 1
+    import ctypes as C
+    tab = (C.c_int64 * (sms + 1))()
+    assert g.lib().genga_kick_plan_sym_table(C.byref(p), tab) == 0 and tab[0] == 0 and tab[sms] == d["n_tiles"]
+    cost = lambda t: 14 if want[t][1] < (want[t][0] + 1) * r else 10          # diagonal : symmetric
+    prev, costs, segs = 0, [], 1
     for c in range(d["n_ctas"]):
         t0, t1 = g.plan_cta_range(p, c)
-        assert t0 == prev and t1 > t0
+        assert t0 == prev == tab[c] and t1 >= t0
         prev = t1
-        sizes.append(t1 - t0)
-        segs = max(segs, g.plan_sym_row_of(p, t1 - 1) - g.plan_sym_row_of(p, t0) + 1)
-    assert prev == d["n_tiles"] and max(sizes) - min(sizes) <= 1
-    assert d["max_segs"] == segs and d["partial_doubles"] == sms * segs * 3 * 2048
+        costs.append(sum(cost(t) for t in range(t0, t1)))
+        if t1 > t0:
+            segs = max(segs, g.plan_sym_row_of(p, t1 - 1) - g.plan_sym_row_of(p, t0) + 1)
+    assert prev == d["n_tiles"] and max(costs) - min(costs) <= 2 * 14             # balanced to a tile or two
+    assert d["max_segs"] == segs and d["partial_doubles"] == sms * segs * 3 * IB
     for ib in sorted({0, rows // 2, rows - 1}):
         a, b = g.plan_iblock_ctas(p, ib)
         ta, tb = g.plan_sym_row_begin(p, ib), g.plan_sym_row_begin(p, ib + 1)
-        meets = [c for c in range(d["n_ctas"]) if (lambda q: q[0] < tb and q[1] > ta)(g.plan_cta_range(p, c))]
+        meets = [c for c in range(d["n_ctas"]) if tab[c] < tb and tab[c + 1] > ta and tab[c + 1] > tab[c]]
         assert meets == list(range(a, b + 1))
     if nt:
         q = g.make_plan_tprows(nm, nt, sms).as_dict()
