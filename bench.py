@@ -11,9 +11,14 @@ One STEP = one pass of the whole hot path over that disk with the paper's two-le
 weights of eq. 63: the all-pairs kick with W_0 = K(r, dt) and the all-pairs kick
 with W_1 = (1 - K(r, dt)) K(r, dt/2), each fused with its encounter pre-check, pair list, per-body
 counts and the velocity update v += dt a (rows a1-a8 of SURVEY.md 8(a)).
-A step is 2 N (N - 1) ordered pair interactions.  The per-level numbers are reported beside the
-aggregate (`levels`): the level-0 kick is the dense one (every pair contributes) and is the kernel
-the `roofline` object describes.
+
+What `value` counts: the ordered pair interactions whose force is actually EVALUATED, per second of
+the whole step.  The level-0 kick evaluates all N (N - 1) of them (the symmetric pair loop forms one
+r^-3 per unordered pair and applies both forces).  The level-1 kick is a neighbour search: W_1 = 0
+exactly outside the level-0 critical radius, so all but ~1e6 of its 4.3e9 pairs are dismissed by box
+tests and are NOT counted.  `value_nominal_two_level` is the same step counted as 2 N (N - 1) (the
+convention of round 1), `value_dense_level0` the level-0 call alone; `levels` has each level, and
+`configs` the other BASELINE.json configs (0, 2, 4) timed the same way.
 
 N > 1 GPUs (torchrun, one rank per GPU): the path runs on one GPU (north_star); ranks are
 independent replicas on independently seeded disks, no data-path collective ("scaling": "weak").
@@ -41,14 +46,19 @@ UNIT = "pair interactions/s"
 N_BODIES = 65536
 LEVELS = (0, 1)
 PAIR_CAPACITY = 1 << 20
-# FP64-pipe instructions and flops of one far pair in the dense (level-0) pair loop, read off the
-# committed SASS (profiles/sass_pair_loop_r01.md): 3 DADD + 5 DMUL + 8 DFMA; kept in ONE place.
+# ALGORITHMIC work of one ordered pair ("~17 FP64-pipe instructions, ~25 flops"; the one-sided loop's
+# SASS has 3 DADD + 5 DMUL + 8 DFMA = 16 instructions, 24 flops: profiles/sass_pair_loop_r01.md) -- the per-unit figure
+# of roofline.achieved.  EXECUTED work of the symmetric loop (profiles/sass_sym_loop_r02.md): one UNORDERED pair costs
+# 3 DADD + 6 DMUL + 11 DFMA = 20 instructions, 31 flops, i.e. 10 instructions / 15.5 flops per ordered pair.
 FP64_INSTR_PER_PAIR = 16
 FLOPS_PER_PAIR = 24
+SYM_FP64_INSTR_PER_UNORDERED_PAIR = 20
+SYM_FLOPS_PER_UNORDERED_PAIR = 31
 FP64_LANES_PER_SM = 64           # 148 SMs x 64 lanes x 2 flops x clocks.max.sm
-# dram__bytes_read.sum + dram__bytes_write.sum of one level-0 kick_kernel launch, from the ncu
-# --set full capture summarised in profiles/ncu_r01c.md
-NCU_DRAM_BYTES_PER_LAUNCH = 2501120        # profiles/ncu_r01c.md: 2.49 MB read + 9 KB written
+# From the ncu captures of round 2 (profiles/ncu_r02a.md), per launch / per two-level step at N = 65,536; constants
+# read off those captures, not measured in this run:
+NCU_DRAM_BYTES_PER_LAUNCH = None           # filled from profiles/ncu_r02a.md once captured
+NCU_EXECUTED_FLOPS_PER_STEP = None         # DADD + DMUL + 2 DFMA thread instructions of every kernel of one step
 
 
 def workload(rank: int):
@@ -211,7 +221,8 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     # FP64 ALU roofline of this device, measured before the timed region
     # (pattern 0: loop-invariant operands; 1: three distinct register operands, the shape of the
     # accumulation a += s d; 2: two distinct register operands -- include/genga_kick.h)
-    fp64_rate = [kick.measure_fp64_rate(pattern, iters=4096, reps=5) for pattern in (0, 1, 2)]
+    import bench_aids                                   # bench-side helper library, not the product
+    fp64_rate = [bench_aids.fp64_rate(pattern, iters=4096, reps=5, stream=stream.cuda_stream) for pattern in (0, 1, 2)]
     dfma_rate = max(fp64_rate)
     for _ in range(args.warmup):
         step()
@@ -240,8 +251,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     step_ms = [a.elapsed_time(b) for a, b in zip(e0, e1)]
     total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
     pairs_per_kick = ki.n_massive * (ki.n_massive - 1) + ki.n_test * ki.n_massive
-    pairs_per_step = len(LEVELS) * pairs_per_kick
+    pairs_per_step = pairs_per_kick                    # EVALUATED: all of level 0; level 1's are culled, not counted
+    nominal_pairs_per_step = len(LEVELS) * pairs_per_kick
     value = whole_job_value(world, pairs_per_step, args.steps, total_ms)
+    value_nominal = whole_job_value(world, nominal_pairs_per_step, args.steps, total_ms)
 
     # per-level numbers: one more kick each, timed alone (after the timed region)
     levels = {}
@@ -257,8 +270,90 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             ts.append(a.elapsed_time(b))
         enc_pairs[level] = int(npairs[n].item())
         ms = float(np.median(ts))
-        levels[str(level)] = {"ms_per_kick": ms, "pairs_per_s": pairs_per_kick / (ms * 1e-3),
-                              "pair_loop_ms": float(np.mean(loop_ms[level])), "encounter_pairs": enc_pairs[level]}
+        levels[str(level)] = {"ms_per_kick": ms, "pair_loop_ms": float(np.mean(loop_ms[level])),
+                              "encounter_pairs": enc_pairs[level]}
+        if level == 0:
+            levels["0"]["pairs_per_s"] = pairs_per_kick / (ms * 1e-3)
+            levels["0"]["what"] = "dense: every ordered pair's force evaluated (one r^-3 per unordered pair)"
+        else:
+            levels[str(level)]["nominal_pairs_per_s"] = pairs_per_kick / (ms * 1e-3)
+            levels[str(level)]["what"] = ("neighbour search: W_L = 0 exactly beyond the level-0 critical radius, the pairs "
+                                          "are culled by box tests, not evaluated (nominal figure, not work done)")
+
+    # the other BASELINE.json configs, each timed like the headline (L2 flushed before every kick, median of 7 after 3
+    # warm-ups): configs[0] (launch-bound: plain launches and a CUDA-graph replay), configs[1], configs[2] at both
+    # levels, configs[4] in both test-particle modes
+    def time_config(kin, level, tp_mode=1, mass_override=None, graph=False, reps=7):
+        nn = kin.n
+        kc = GengaKick(kin.n_massive, kin.n_test, max_level=level, pair_capacity=PAIR_CAPACITY, G=kin.G,
+                       enc_factor=kin.enc_factor, device=local_rank, tp_mode=tp_mode)
+        kc.set_stream(stream.cuda_stream)
+        kc.enable_timing(True)
+        cp, cm = to_dev(kin.pos), to_dev(kin.mass if mass_override is None else mass_override)
+        crc, cv = to_dev(kin.rcrit[:level + 1]), to_dev(kin.vel)
+        ca = torch.empty(3, nn, dtype=torch.float64, device=dev)
+        cnp = torch.empty(nn + 1, dtype=torch.int32, device=dev)
+        ts, loops = [], []
+        for it in range(reps + 3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            flush.fill_(9)
+            l0 = kc.launch_count()
+            a.record(stream)
+            kc.kick(cp, cv, cm, crc, level, 0.5 * kin.dt, ca, pairs, cnp)
+            b.record(stream)
+            b.synchronize()
+            nl = kc.launch_count() - l0
+            if it >= 3:
+                ts.append(a.elapsed_time(b))
+                loops.append(kc.last_pair_loop_ms(level))
+        ms = float(np.median(ts))
+        ordered = kin.n_massive * (kin.n_massive - 1) + kin.n_test * kin.n_massive * (2 if tp_mode == 2 else 1)
+        out = {"n_massive": kin.n_massive, "n_test": kin.n_test, "level": level, "ms_per_kick": ms,
+               "pair_loop_ms": float(np.median(loops)), "launches": int(nl), "encounter_pairs": int(cnp[nn].item()),
+               "symmetric_pass": bool(kc.plan(0).symmetric) if level == 0 else False, "status": kc.status()}
+        if level == 0:
+            out["pairs_per_s"] = ordered / (ms * 1e-3)
+        else:
+            out["nominal_pairs_per_s"] = ordered / (ms * 1e-3)
+        if tp_mode == 2:
+            out["tp_mode"] = 2
+        if graph:
+            gs = torch.cuda.Stream()
+            torch.cuda.synchronize()
+            kc.set_stream(gs.cuda_stream)
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=gs):
+                kc.kick(cp, cv, cm, crc, level, 0.5 * kin.dt, ca, pairs, cnp)
+            gts = []
+            with torch.cuda.stream(gs):
+                for it in range(reps + 3):
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(gs)
+                    g.replay()
+                    b.record(gs)
+                    b.synchronize()
+                    if it >= 3:
+                        gts.append(a.elapsed_time(b))
+            torch.cuda.synchronize()
+            out["ms_per_kick_cuda_graph"] = float(np.median(gts))
+            del g
+        kc.free()
+        return out
+
+    k4 = gi.make_config(4)
+    m4 = k4.mass.copy()
+    m4[k4.n_massive:] = 1e-12 * (0.5 + gi.uniforms(77, 0, k4.n_test))       # TP 2: particles with mass
+    k2 = gi.make_config(2)
+    configs_info = {
+        "what": "one kick + pre-check (v += dt a, pair list, counts) per BASELINE.json config, L2 flushed before each; "
+                "pairs_per_s counts evaluated ordered pairs (level 0); level >= 1 kicks are neighbour searches (nominal)",
+        "configs[0] N=2048 L=0": time_config(gi.make_config(0), 0, graph=True),
+        "configs[1] N=8192 L=0": time_config(gi.make_config(1), 0),
+        "configs[2] N=32770 L=0": time_config(k2, 0),
+        "configs[2] N=32770 L=1": time_config(k2, 1),
+        "configs[4] 2048+1048576 tp, TP 1": time_config(k4, 0),
+        "configs[4] 2048+1048576 tp, TP 2": time_config(k4, 0, tp_mode=2, mass_override=m4),
+    }
 
     # NEXT-1: the whole App. A step without the Bulirsch-Stoer branch on the same disk --
     # Rcrit, Kick(dt/2) + pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) -- and its O(N) part alone
@@ -443,8 +538,8 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         kb.free()
         return {"n": nr, "ms": float(np.median(ts)), "status": st}
 
-    bs_ring_info = {"what": "genga_bs on one ring group of n bodies with 8 partners each (Fig. 7 / Fig. 8), dt = 6 d, tol 1e-12: "
-                            "n <= 32 one warp, <= 256 one CTA, above the whole grid with 8 lanes per body",
+    bs_ring_info = {"what": "genga_bs on one ring group of n bodies with 8 partners each (Fig. 7 / Fig. 8), dt = 6 d, tol 1e-12 "
+                            "(regimes by group size: include/genga_bs.h)",
                     "rings": [time_bs_ring(nr) for nr in (2, 8, 32, 64, 256, 512, 1024, 2048, 4096)]}
 
     # end to end through the host entry point: pinned host arrays in, results back, every step
@@ -477,19 +572,44 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
         peak_dfma = 2.0 * dfma_rate / 1e12
         k0_ms = float(np.mean(loop_ms[0]))
+        sym = bool(kick.plan(0).symmetric)
+        # roofline.achieved (the contract's definition): ALGORITHMIC flops per unit x units per launch / kernel time,
+        # the per-unit figure being SURVEY.md 8(d)'s one ordered pair = 24 flops (its "~25"), counted over all
+        # N (N - 1) ordered pairs.  The symmetric loop EXECUTES fewer: 31 flops per unordered pair = 15.5 per ordered
+        # pair -- it reaches the same result with 35 % less arithmetic, so its executed-flop fraction
+        # (frac_executed_flops) is LOWER than the one-sided loop's 0.64 while its throughput is 40 % higher.
         achieved = FLOPS_PER_PAIR * pairs_per_kick / (k0_ms * 1e-3) / 1e12
+        n_m = ki.n_massive
+        if sym:
+            pl = kick.plan(0)
+            ib, r = pl.i_block, pl.tiles_per_iblock
+            diag_ordered = sum(min(ib, n_m - I * ib) * min(n_m - I * ib, ib) for I in range(pl.n_i_blocks))
+            unordered_sym = (n_m * n_m - diag_ordered) // 2
+            exec_flops = SYM_FLOPS_PER_UNORDERED_PAIR * unordered_sym + FLOPS_PER_PAIR * diag_ordered
+            exec_instr = SYM_FP64_INSTR_PER_UNORDERED_PAIR * unordered_sym + FP64_INSTR_PER_PAIR * diag_ordered
+        else:
+            exec_flops, exec_instr = FLOPS_PER_PAIR * pairs_per_kick, FP64_INSTR_PER_PAIR * pairs_per_kick
+        executed = exec_flops / (k0_ms * 1e-3) / 1e12
+        pipe_rate = props.multi_processor_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6
+        step_ms = total_ms / args.steps
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "value_what": "ordered pair interactions whose force is evaluated, per second of the two-level step (all "
+                          "N (N - 1) of level 0; the level-1 kick's pairs are culled by a neighbour search and not counted)",
+            "value_dense_level0": levels["0"]["pairs_per_s"],
+            "value_nominal_two_level": value_nominal,
             "config": {"workload": "configs[3]: N=65536 planetesimal disk (sigma ~ a^-1.5, log-uniform masses), "
                                    "step = level-0 kick + level-1 kick (two-level changeover, eq. 63), each "
                                    "with encounter pre-check, pair list, counts and v += dt a",
                        "n_massive": ki.n_massive, "n_test": ki.n_test, "levels": list(LEVELS),
-                       "pairs_per_step": pairs_per_step, "pair_capacity": PAIR_CAPACITY,
+                       "pairs_per_step": pairs_per_step, "nominal_pairs_per_step": nominal_pairs_per_step,
+                       "pair_capacity": PAIR_CAPACITY,
                        "l2": "256 MiB buffer written between timed iterations (working set 3 MB is L2-resident)",
                        "parallelism": "replicas" if world > 1 else "single GPU"},
             "levels": levels,
+            "configs": configs_info,
             "step": step_info,
             "group": group_info,
             "kick_list": list_info,
@@ -501,8 +621,11 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
                     "api": "genga_kick_host (pinned host arrays, copies and synchronisation inside the call)"},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "alu", "kernel": "kick_kernel<dense> (level 0)", "achieved": achieved,
-                         "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
+            "roofline": {"bound": "alu",
+                         "kernel": "kick_sym_kernel (level 0, every unordered pair once)" if sym else "kick_kernel (level 0)",
+                         "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
+                         "achieved_what": "algorithmic: 24 flops per ordered pair (SURVEY.md 8(d); the one-sided loop's SASS "
+                                          "count) x N (N - 1) ordered pairs / kernel time",
                          "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
                          "peak_source": f"nominal: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes "
                                         f"x 2 x {sm_max_mhz} MHz (no FP64 figure in MEASURED_PEAKS.json)",
@@ -510,14 +633,23 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                          "dfma_per_s_by_operand_pattern": {"invariant_operands": fp64_rate[0],
                                                            "three_distinct_registers": fp64_rate[1],
                                                            "two_distinct_registers": fp64_rate[2]},
-                         # ceiling of THIS instruction mix: 13 FP64 instructions with <= 2 distinct register
-                         # operands + 3 accumulating DFMAs with 3, each at its measured rate
-                         "mix_ceiling": FLOPS_PER_PAIR / (13.0 / fp64_rate[2] + 3.0 / fp64_rate[1]) / 1e12,
-                         "frac_of_mix_ceiling": achieved / (FLOPS_PER_PAIR / (13.0 / fp64_rate[2] + 3.0 / fp64_rate[1]) / 1e12),
-                         "flops_per_pair": FLOPS_PER_PAIR, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR,
-                         "fp64_pipe_issue_frac": FP64_INSTR_PER_PAIR * pairs_per_kick / (k0_ms * 1e-3) /
-                                                 (props.multi_processor_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
-                         "kernel_ms": k0_ms, "pairs_per_launch": pairs_per_kick},
+                         "executed": executed, "frac_executed_flops": executed / peak_nominal,
+                         "executed_what": "flops the kernel executes (SASS count x pairs of each path: 31 per unordered pair "
+                                          "in the symmetric tiles, 24 per ordered pair in the diagonal tiles) / kernel time: "
+                                          "fewer flops per pair than the one-sided loop, hence a lower fraction at a higher "
+                                          "throughput",
+                         "executed_flops_per_launch": exec_flops,
+                         "fp64_pipe_issue_frac": exec_instr / (k0_ms * 1e-3) / pipe_rate,
+                         "whole_step_frac_executed_flops": (exec_flops if NCU_EXECUTED_FLOPS_PER_STEP is None
+                                                            else NCU_EXECUTED_FLOPS_PER_STEP) / (step_ms * 1e-3) / 1e12 / peak_nominal,
+                         "whole_step_what": "executed FP64 flops of every kernel of one two-level step (ncu's executed "
+                                            "DADD / DMUL / DFMA counters, profiles/ncu_r02a.md; the pair loop's static count "
+                                            "if no capture is recorded) / step time / peak",
+                         "algorithmic_flops_per_ordered_pair": FLOPS_PER_PAIR,
+                         "executed_flops_per_unordered_pair": SYM_FLOPS_PER_UNORDERED_PAIR if sym else 2 * FLOPS_PER_PAIR,
+                         "executed_fp64_instr_per_unordered_pair": SYM_FP64_INSTR_PER_UNORDERED_PAIR if sym else 2 * FP64_INSTR_PER_PAIR,
+                         "kernel_ms": k0_ms, "pairs_per_launch": pairs_per_kick,
+                         "ordered_pair_equivalents_per_s": pairs_per_kick / (k0_ms * 1e-3)},
         }
         import oracle                                   # cpu_baseline leg: rank 0, N=1 only
         if world == 1 and not args.no_cpu_baseline:

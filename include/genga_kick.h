@@ -216,21 +216,6 @@ int64_t genga_kick_launch_count(const genga_kick_ctx* ctx);
 int genga_kick_enable_timing(genga_kick_ctx* ctx, int32_t on);
 int genga_kick_last_pair_loop_ms(genga_kick_ctx* ctx, int32_t changeover_level, float* ms);
 
-/* Measurement aid: the plain FP64 ALU roofline of the device.  Runs `reps` launches of a kernel
- * of independent DFMA chains (8 chains per thread, `iters` x 8 DFMAs each, 256 threads x 8 CTAs
- * per SM) on the context's stream and returns the best launch's rate in *dfma_per_s (one DFMA =
- * 2 flops).  `pattern` selects the register-operand pattern of the DFMAs, which decides the rate
- * this part sustains:
- *   0  a = fma(a, m, c) with loop-invariant m, c (operand reuse possible);
- *   1  a_k = fma(a_k, b_k, c_k): three distinct register operands, the shape of the pair loop's
- *      accumulation a += s * d;
- *   2  a_k = fma(a_k, b_k, constant): two distinct register operands.
- * genga_kick_measure_dfma_rate is pattern 0.
- * Synchronises.  Errors: E_NULL, E_SIZE (iters or reps < 1, pattern outside 0..2), E_CUDA. */
-int genga_kick_measure_fp64_rate(genga_kick_ctx* ctx, int32_t pattern, int32_t iters, int32_t reps,
-                                 double* dfma_per_s);
-int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, int32_t reps, double* dfma_per_s);
-
 /* Free the context and its scratch.  NULL is allowed. */
 int genga_kick_free(genga_kick_ctx* ctx);
 

@@ -20,7 +20,7 @@ EXPORTS = (
     "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of", "genga_kick_plan_sym_table", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
     "genga_kick_set_stream", "genga_kick", "genga_kick_list", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
-    "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms", "genga_kick_measure_dfma_rate", "genga_kick_measure_fp64_rate",
+    "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms",
 )
 # include/genga_step.h: the O(N) neighbours of the kick and the composed step
 STEP_EXPORTS = ("genga_rcrit", "genga_hc", "genga_fg", "genga_drift", "genga_step", "genga_rcrit_list", "genga_fg_list")
@@ -96,8 +96,6 @@ def lib():
         L.genga_kick_launch_count.argtypes = [vp]
         L.genga_kick_enable_timing.argtypes = [vp, i32]
         L.genga_kick_last_pair_loop_ms.argtypes = [vp, i32, C.POINTER(C.c_float)]
-        L.genga_kick_measure_dfma_rate.argtypes = [vp, i32, i32, C.POINTER(d)]
-        L.genga_kick_measure_fp64_rate.argtypes = [vp, i32, i32, i32, C.POINTER(d)]
         L.genga_kick_launch_count.restype = i64
         L.genga_kick_free.argtypes = [vp]
         L.genga_kick_strerror.argtypes = [C.c_int]
@@ -380,16 +378,6 @@ class GengaKick:
         ms = C.c_float()
         self._check(lib().genga_kick_last_pair_loop_ms(self._ctx, int(changeover_level), C.byref(ms)))
         return float(ms.value)
-
-    def measure_dfma_rate(self, iters=4096, reps=5) -> float:
-        r = C.c_double()
-        self._check(lib().genga_kick_measure_dfma_rate(self._ctx, int(iters), int(reps), C.byref(r)))
-        return float(r.value)
-
-    def measure_fp64_rate(self, pattern=0, iters=4096, reps=5) -> float:
-        r = C.c_double()
-        self._check(lib().genga_kick_measure_fp64_rate(self._ctx, int(pattern), int(iters), int(reps), C.byref(r)))
-        return float(r.value)
 
     def free(self):
         if self._ctx:

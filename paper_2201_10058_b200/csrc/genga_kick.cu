@@ -432,85 +432,6 @@ extern "C" int genga_kick_last_pair_loop_ms(genga_kick_ctx* ctx, int32_t changeo
     return GENGA_KICK_OK;
 }
 
-namespace genga {
-// Independent DFMA chains: the plain FP64 ALU roofline (include/genga_kick.h).  The operands come
-// from memory so that nothing folds; the result is stored so that nothing is dropped.
-//   PATTERN 0: a = fma(a, m, c), m and c loop-invariant registers (operand reuse possible)
-//   PATTERN 1: a_k = fma(a_k, b_k, c_k): three distinct register operands, no reuse
-//   PATTERN 2: a_k = fma(a_k, b_k, imm): two distinct register operands
-template <int PATTERN>
-__global__ void __launch_bounds__(256, 2) fp64_rate_kernel(const double* __restrict__ in, double* __restrict__ out, int iters)
-{
-    const double m = in[0], c = in[1];
-    double a[8], b[8], d[8];
-#pragma unroll
-    for (int k = 0; k < 8; k++) {
-        a[k] = in[2] * (double)(threadIdx.x + k);
-        b[k] = m - 1.0e-9 * (double)k;
-        d[k] = c + 1.0e-9 * (double)k;
-    }
-    for (int it = 0; it < iters; it++) {
-#pragma unroll
-        for (int u = 0; u < 8; u++) {
-#pragma unroll
-            for (int k = 0; k < 8; k++) {
-                if (PATTERN == 0) a[k] = fma(a[k], m, c);
-                if (PATTERN == 1) a[k] = fma(a[k], b[k], d[k]);
-                if (PATTERN == 2) a[k] = fma(a[k], b[k], 1.0e-6);
-            }
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int k = 0; k < 8; k++) s += a[k];
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-}  // namespace genga
-
-extern "C" int genga_kick_measure_fp64_rate(genga_kick_ctx* ctx, int32_t pattern, int32_t iters, int32_t reps,
-                                            double* dfma_per_s)
-{
-    if (!ctx || !dfma_per_s) return GENGA_KICK_E_NULL;
-    if (iters < 1 || reps < 1 || pattern < 0 || pattern > 2) return GENGA_KICK_E_SIZE;
-    const int blocks = 8 * ctx->num_sms, threads = 256;
-    double* buf = nullptr;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    cudaStream_t st = ctx->stream;
-    const double host_in[3] = {0.999999, 1.0e-6, 1.0e-3};
-    cudaError_t e;
-    float best = 0.0f;
-    if ((e = cudaMalloc(&buf, ((size_t)blocks * threads + 4) * sizeof(double))) != cudaSuccess) goto done;
-    if ((e = cudaMemcpyAsync(buf, host_in, sizeof(host_in), cudaMemcpyHostToDevice, st)) != cudaSuccess) goto done;
-    if ((e = cudaEventCreate(&e0)) != cudaSuccess) goto done;
-    if ((e = cudaEventCreate(&e1)) != cudaSuccess) goto done;
-    for (int r = 0; r <= reps; r++) {                              // launch 0 is the warm-up
-        if ((e = cudaEventRecord(e0, st)) != cudaSuccess) goto done;
-        if (pattern == 0) genga::fp64_rate_kernel<0><<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
-        if (pattern == 1) genga::fp64_rate_kernel<1><<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
-        if (pattern == 2) genga::fp64_rate_kernel<2><<<blocks, threads, 0, st>>>(buf, buf + 4, iters);
-        if ((e = cudaGetLastError()) != cudaSuccess) goto done;
-        if ((e = cudaEventRecord(e1, st)) != cudaSuccess) goto done;
-        if ((e = cudaEventSynchronize(e1)) != cudaSuccess) goto done;
-        float ms = 0.0f;
-        if ((e = cudaEventElapsedTime(&ms, e0, e1)) != cudaSuccess) goto done;
-        if (r > 0 && (best == 0.0f || ms < best)) best = ms;
-        ctx->launches++;
-    }
-    *dfma_per_s = (double)blocks * threads * 64.0 * (double)iters / ((double)best * 1.0e-3);
-done:
-    if (e0) cudaEventDestroy(e0);
-    if (e1) cudaEventDestroy(e1);
-    if (buf) cudaFree(buf);
-    if (e != cudaSuccess) return cuda_fail(ctx, e);
-    return GENGA_KICK_OK;
-}
-
-extern "C" int genga_kick_measure_dfma_rate(genga_kick_ctx* ctx, int32_t iters, int32_t reps, double* dfma_per_s)
-{
-    return genga_kick_measure_fp64_rate(ctx, 0, iters, reps, dfma_per_s);
-}
-
-
 extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)
