@@ -379,6 +379,32 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                  "drift_ms": float(np.median(drift_ts)), "drift_what": "HC(dt/2) FG(dt) HC(dt/2) alone, 3 launches, "
                  "184 B/body of HBM traffic", "status": kick.status()}
 
+    # genga_steps: consecutive steps with the closing kick of a step and the opening kick of the next merged into one
+    # pass over the pairs (one all-pairs pass per step instead of two): 100 steps without the encounter branch, and
+    # 10 steps of the multi-level scheme (2 levels x 10 sub-steps), from the generated state
+    def time_steps(n_steps, slevels, substeps, reps=2):
+        kk = kick if slevels <= 1 + max(LEVELS) else None
+        st_buf = torch.zeros(max(slevels, 1), 4, dtype=torch.int32, device=dev)
+        ts = []
+        for it in range(reps + 1):
+            sq2, sv2 = pos.clone(), vel.clone()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            flush.fill_(4)
+            l0 = kk.launch_count()
+            a.record(stream)
+            kk.steps(sq2, sv2, mass, 1.0, ki.dt, n_steps, slevels, substeps, 1e-12, acc, pairs, npairs, st_buf)
+            b.record(stream)
+            b.synchronize()
+            nl = kk.launch_count() - l0
+            if it >= 1:
+                ts.append(a.elapsed_time(b))
+        return {"n_steps": n_steps, "slevels": slevels, "substeps": substeps if slevels > 1 else None,
+                "ms_per_step": float(np.median(ts)) / n_steps, "launches_per_step": nl / n_steps, "status": kk.status()}
+
+    steps_info = {"what": "genga_steps: n consecutive steps, merged kicks (slevels 0: Rcrit, Kick, HC, FG, HC, Kick without "
+                          "the encounter branch; 2 x 10: the multi-level step), ms per step",
+                  "runs": [time_steps(100, 0, 2), time_steps(10, 2, 10)]}
+
     # NEXT-2: grouping of the level-0 pair list (499,679 pairs at N = 65,536) into close-encounter groups
     kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
     group_of = torch.empty(n, dtype=torch.int32, device=dev)
@@ -611,6 +637,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             "levels": levels,
             "configs": configs_info,
             "step": step_info,
+            "steps_merged": steps_info,
             "group": group_info,
             "kick_list": list_info,
             "hybrid_step": hybrid_info,

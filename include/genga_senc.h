@@ -45,7 +45,7 @@ int genga_detect(genga_kick_ctx* ctx, const double* pos0, const double* vel0, co
 
 typedef struct {
     int32_t slevels;    /* number of symplectic levels, 1 .. 4 (1: the original hybrid scheme; the context needs
-                           max_level >= slevels - 1)                                                              */
+                           max_level >= slevels - 1); genga_steps also takes 0: no encounter branch                                                              */
     int32_t substeps;   /* sub-steps per level >= 1 ("two, four, or 10, but any other number is also possible",
                            PAPER.md:619); ignored for slevels == 1                                                */
     int32_t detect;     /* 1: close-encounter detection as genga_detect (threshold: the critical radius itself);
@@ -86,6 +86,29 @@ typedef struct {
 int genga_multilevel_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
                           const genga_senc_config* cfg, double* out_acc, int32_t* out_pairs, int32_t* out_npairs,
                           int32_t* out_stats);
+
+#define GENGA_KICK_STATUS_RCRIT_JUMP 256   /* genga_steps: a body's critical radius grew by more than 1/64 from one step
+                                             to the next, more than the merged kick's candidate list allows for:
+                                             repeat from the state before the call with single steps               */
+
+/*
+ * n_steps consecutive steps of the scheme above in one call, with the closing Kick(dt/2) of every step but the last
+ * and the opening Kick(dt/2) + pre-check of the next MERGED into one pass over the pairs: both act on the same
+ * positions (App. A, repeated) and differ only in the critical radii -- the next step's Rcrit(dt) is
+ * taken from the velocities after the closing kick -- i.e. only in the pairs inside a critical radius.  The far field
+ * is summed once and the listed pairs are evaluated twice (rc of the step that ends, then rc of the step that begins,
+ * with its pre-check).  The result equals n_steps calls of genga_multilevel_step (cfg->slevels >= 1; 1 = the hybrid
+ * step of genga_bs.h when cfg->detect == 0) or of genga_step (cfg->slevels == 0: no encounter branch, cfg->n1 / n2
+ * used, cfg->tol / substeps / detect ignored) up to the rounding of the far-field sums; a step costs one all-pairs
+ * pass instead of two.
+ *   out_pairs / out_npairs   the candidates of the LAST step's opening kick
+ *   out_stats                [slevels][4] summed over all steps, or NULL
+ *   out_acc                  acceleration of the final closing kick, or NULL
+ * Errors: as genga_multilevel_step; E_SIZE also for n_steps < 1.
+ */
+int genga_steps(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
+                int32_t n_steps, const genga_senc_config* cfg, double* out_acc, int32_t* out_pairs, int32_t* out_npairs,
+                int32_t* out_stats);
 
 #ifdef __cplusplus
 }

@@ -229,3 +229,20 @@ def multilevel_step(pos, vel, mass, n_massive, n_test, m_star, G, dt, slevels=2,
     v = v + (0.5 * dt) * k2.acc
     return MultilevelStepResult(pos=q, vel=v, rcrit=rc, first=k1, stats=stats, unbound=sum(unbound),
                                 bs_totals=_bs_totals(bs_all))
+
+
+def steps(pos, vel, mass, n_massive, n_test, m_star, G, dt, n_steps, slevels=0, **kw):
+    """n_steps consecutive steps: the definition of what genga_steps computes IS the repetition of the single step
+    (App. A, `n_steps` times) -- merging the closing kick of a step with the opening kick of the next
+    is a device-side economy that must not change the result beyond rounding.  slevels = 0: `step` (no encounter
+    branch); slevels >= 1: `multilevel_step` (kw: substeps, tol, detect, ...).  Returns the list of per-step results."""
+    q, v = _c(pos).copy(), _c(vel).copy()
+    out = []
+    for _ in range(n_steps):
+        if slevels == 0:
+            r = step(q, v, mass, n_massive, n_test, m_star, G, dt, **{k: w for k, w in kw.items() if k in ("enc_factor", "n1", "n2")})
+        else:
+            r = multilevel_step(q, v, mass, n_massive, n_test, m_star, G, dt, slevels=slevels, **kw)
+        q, v = r.pos, r.vel
+        out.append(r)
+    return out

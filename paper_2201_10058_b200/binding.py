@@ -32,7 +32,8 @@ BS_EXPORTS = ("genga_bs", "genga_hybrid_step", "genga_bs_set_stats", "genga_bs_t
 STATUS_GROUP_TOO_LARGE, STATUS_BS_NOT_CONVERGED = 32, 64
 STATUS_UNBOUND = 8
 # include/genga_senc.h: close-encounter detection and the multi-level step (SEnc)
-SENC_EXPORTS = ("genga_detect", "genga_multilevel_step")
+SENC_EXPORTS = ("genga_detect", "genga_multilevel_step", "genga_steps")
+STATUS_RCRIT_JUMP = 256
 STATUS_LIST_CLIPPED = 128
 
 
@@ -116,6 +117,7 @@ def lib():
         L.genga_bs_totals.argtypes = [vp, C.POINTER(i64 * 4), i32]
         L.genga_detect.argtypes = [vp, vp, vp, vp, vp, vp, d, d, vp, vp, i64, vp, vp]
         L.genga_multilevel_step.argtypes = [vp, vp, vp, vp, d, d, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
+        L.genga_steps.argtypes = [vp, vp, vp, vp, d, d, i32, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
         for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS + SENC_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error",
                             "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of"):
@@ -357,6 +359,14 @@ class GengaKick:
         p, v, m, a, op, on = self._step_args(pos, vel, mass, out_acc, out_pairs, out_npairs)
         self._check(lib().genga_multilevel_step(self._ctx, p, v, m, float(m_star), float(dt), C.byref(cfg), a, op, on,
                                                 self._i(out_stats, 4 * max(int(slevels), 0), "out_stats")))
+
+    def steps(self, pos, vel, mass, m_star, dt, n_steps, slevels, substeps, tol, out_acc, out_pairs, out_npairs, out_stats,
+              detect=True, n1=3.0, n2=0.4):
+        """n_steps consecutive steps with merged kicks (include/genga_senc.h); slevels = 0: no encounter branch."""
+        cfg = GengaSencConfig(int(slevels), int(substeps), int(bool(detect)), 0, float(n1), float(n2), float(tol))
+        p, v, m, a, op, on = self._step_args(pos, vel, mass, out_acc, out_pairs, out_npairs)
+        self._check(lib().genga_steps(self._ctx, p, v, m, float(m_star), float(dt), int(n_steps), C.byref(cfg), a, op, on,
+                                      self._i(out_stats, 4 * max(int(slevels), 0), "out_stats")))
 
     def plan(self, changeover_level=0) -> GengaKickPlan:
         plan = GengaKickPlan()

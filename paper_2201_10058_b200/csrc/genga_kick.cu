@@ -2,6 +2,7 @@
 // Host side only: argument checks, scratch ownership, kernel launches on the caller's stream.
 // Every step of the path runs in the kernels of genga_kick_kernels.cuh; there is no CPU fallback.
 #include "genga_kick_ctx.h"
+#include "../../include/genga_step.h"
 #include "genga_kick_variants.h"
 #include "genga_kick_kernels.cuh"
 #include "genga_kick_sym.cuh"
@@ -159,6 +160,19 @@ extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, c
     return genga_kick_impl(ctx, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs);
 }
 
+namespace {
+
+// A kick in two halves.  kick_front: internal order, records, and the pair loop(s) -- the far-field partial sums and
+// the candidate list of the pairs that tripped the filter (built from the rows of `rcrit`, the filter radius scaled
+// by fw_scale).  kick_back: the exact path over that list with the rows of kp.rcrit (weights, pre-check, pair list)
+// and the fixed-order sum -> out_acc, v += dt a.  One front can serve several backs (genga_kick_merged).
+int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const double* rcrit, int32_t changeover_level,
+               double fw_scale, int32_t* out_pairs, int32_t* out_npairs, genga::KickParams& kp);
+int kick_back(genga_kick_ctx* ctx, const genga::KickParams& kp, int32_t changeover_level, double dt, double* out_acc,
+              double* vel);
+
+}  // namespace
+
 int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
                     int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs)
 {
@@ -169,7 +183,17 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         misaligned(out_pairs) || misaligned(out_npairs))
         return GENGA_KICK_E_ALIGN;
     if (changeover_level < 0 || changeover_level > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
+    genga::KickParams kp = {};
+    int rc = kick_front(ctx, pos, mass, rcrit, changeover_level, 1.0, out_pairs, out_npairs, kp);
+    if (rc != GENGA_KICK_OK) return rc;
+    return kick_back(ctx, kp, changeover_level, dt, out_acc, vel);
+}
 
+namespace {
+
+int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const double* rcrit, int32_t changeover_level,
+               double fw_scale, int32_t* out_pairs, int32_t* out_npairs, genga::KickParams& kp)
+{
     const genga_kick_plan& pl = ctx->plans[changeover_level];
     const int N = (int)ctx->N;
     const int n_rec = (int)pl.n_rec;
@@ -192,7 +216,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches += 8;
     }
-    genga::KickParams kp = {};
+    kp = genga::KickParams{};
     {
         kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx;
         kp.cblo = ctx->cblo; kp.cbhi = ctx->cbhi;
@@ -210,7 +234,7 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
         genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
                                                    ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
-                                                   ctx->cfg.enc_factor, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx,
+                                                   ctx->cfg.enc_factor, fw_scale, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx,
                                                    ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
@@ -261,6 +285,19 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
             GK_CUDA(ctx, dispatch_kick(p2, k2, st));
             ctx->launches++;
         }
+    }
+    return GENGA_KICK_OK;
+}
+
+int kick_back(genga_kick_ctx* ctx, const genga::KickParams& kp, int32_t changeover_level, double dt, double* out_acc,
+              double* vel)
+{
+    const genga_kick_plan& pl = ctx->plans[changeover_level];
+    const int N = (int)ctx->N;
+    const int n_rec = (int)pl.n_rec;
+    cudaStream_t st = ctx->stream;
+    const bool use_sym = changeover_level == 0 && ctx->plan_sym.n_ctas > 0;
+    if (pl.n_ctas > 0) {
         {
             // fallback for an overflowed candidate list: returns at once otherwise (see near_kernel<true>)
             const int wpc = GENGA_NEAR_THREADS / 32;
@@ -305,6 +342,45 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
         ctx->launches++;
     }
     return GENGA_KICK_OK;
+}
+
+}  // namespace
+
+// The closing Kick(dt/2) of a step and the opening Kick(dt/2) + pre-check of the next act on the same positions
+// (App. A PAPER.md:986-992 repeated): one pass over the pairs serves both.  They differ only in the critical radii --
+// the next step's Rcrit(dt) is taken from the velocities AFTER the closing kick -- hence only in the pairs inside a
+// critical radius, i.e. in the candidate list: far field once, exact path twice.
+//     a_A = far + exact(rc_old);  v += (dt/2) a_A;  rc_new = Rcrit(pos, v);  a_B = far + exact(rc_new), pre-check;
+//     v += (dt/2) a_B
+// Equal to the two separate kicks up to the rounding of the far-field sum (whose filter radius is that of rc_old
+// times 1 + GENGA_MERGE_MARGIN, so that the list also holds the pairs inside the new radii; a body whose critical
+// radius grew by more raises GENGA_KICK_STATUS_RCRIT_JUMP: repeat those steps with genga_step).
+int genga_kick_merged_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rc_old,
+                           double* rc_new, double m_star, double dt_step, double n1, double n2, double* out_acc,
+                           int32_t* out_pairs, int32_t* out_npairs)
+{
+    if (!ctx || !pos || !vel || !mass || !rc_old || !rc_new || !out_npairs) return GENGA_KICK_E_NULL;
+    if (!out_pairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
+    if (misaligned(pos) || misaligned(vel) || misaligned(mass) || misaligned(rc_old) || misaligned(rc_new) ||
+        misaligned(out_acc) || misaligned(out_pairs) || misaligned(out_npairs))
+        return GENGA_KICK_E_ALIGN;
+    genga::KickParams kp = {};
+    int rc = kick_front(ctx, pos, mass, rc_old, 0, 1.0 + GENGA_MERGE_MARGIN, out_pairs, out_npairs, kp);
+    if (rc != GENGA_KICK_OK) return rc;
+    genga::KickParams ka = kp;                             // the closing kick: no pre-check output
+    ka.out_pairs = nullptr; ka.out_npairs = nullptr;
+    rc = kick_back(ctx, ka, 0, 0.5 * dt_step, nullptr, vel);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_rcrit(ctx, pos, vel, mass, m_star, dt_step, 2.0, 1, n1, n2, rc_new);
+    if (rc != GENGA_KICK_OK) return rc;
+    const int N = (int)ctx->N;
+    genga::rcrit_jump_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(rc_old, rc_new, N, 1.0 + GENGA_MERGE_MARGIN,
+                                                                     ctx->status);
+    GK_CUDA(ctx, cudaGetLastError());
+    ctx->launches++;
+    genga::KickParams kb = kp;                             // the opening kick of the next step
+    kb.rcrit = rc_new;
+    return kick_back(ctx, kb, 0, 0.5 * dt_step, out_acc, vel);
 }
 
 extern "C" int genga_kick_list(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,

@@ -86,3 +86,8 @@ int genga_kick_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const d
 // genga_group with a status bit to raise when the pair list was clipped to pair_rows (0: none, the public call)
 int genga_group_impl(genga_kick_ctx* ctx, const int32_t* pairs, const int32_t* n_pairs, int64_t pair_rows,
                      int32_t* group_of, int32_t* members, int32_t* offsets, int32_t* summary, int clip_status);
+// closing Kick(dt_step / 2) of a step + Rcrit(dt_step) + opening Kick(dt_step / 2) with pre-check of the next, in one
+// pass over the pairs (genga_kick.cu); rc_old: the row of the step that ends, rc_new: [N] receives the next step's row
+int genga_kick_merged_impl(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rc_old,
+                           double* rc_new, double m_star, double dt_step, double n1, double n2, double* out_acc,
+                           int32_t* out_pairs, int32_t* out_npairs);

@@ -76,9 +76,11 @@ struct KickParams {
 // R^2's low word is all ones, a single ulp of the double.  Either is enough: r^2 > R^2 strictly in
 // both the fused and the unfused evaluation means K = 1 (level 0) resp. 1 - K_0 = 0 and no encounter.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int filter_word(double rc0, double rcL, double f)
+__device__ __forceinline__ int filter_word(double rc0, double rcL, double f, double scale)
 {
-    const double m = fmax(rc0, __dmul_rn(f, rcL));
+    // scale = 1 but for the merged kick of consecutive steps (genga_kick_merged), whose candidate list must also
+    // hold the pairs inside the critical radii of the NEXT step, not known yet: they may be larger by that factor
+    const double m = __dmul_rn(fmax(rc0, __dmul_rn(f, rcL)), scale);
     return __double2hiint(__dmul_rn(m, m)) + 1;
 }
 
@@ -88,7 +90,7 @@ __device__ __forceinline__ int filter_word(double rc0, double rcL, double f)
 __global__ void __launch_bounds__(256)
 pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, const double* __restrict__ rcrit,
             const int* __restrict__ perm, int N, int n_massive, int m_pad, int n_rec, int L, double G, double f,
-            double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
+            double fw_scale, double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
             float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs,
             int* __restrict__ ncand)
 {
@@ -106,7 +108,7 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
             if (b >= 0) {
                 x = pos[b]; y = pos[(size_t)N + b]; z = pos[2 * (size_t)N + b];
                 gm = __dmul_rn(G, mass[b]);
-                fw = filter_word(rcrit[b], rcrit[(size_t)L * N + b], f);
+                fw = filter_word(rcrit[b], rcrit[(size_t)L * N + b], f, fw_scale);
             }
             rxy[r] = make_double2(x, y);
             rzm[r] = make_double2(z, gm);
@@ -930,6 +932,16 @@ list_reduce_kernel(unsigned long long* __restrict__ fx, int* __restrict__ touche
         vel[(size_t)N + b] = fma(dt, a1, vel[(size_t)N + b]);
         vel[2 * (size_t)N + b] = fma(dt, a2, vel[2 * (size_t)N + b]);
     }
+}
+
+// genga_kick_merged: the candidate list was built for critical radii up to `scale` times the old ones
+#define GENGA_STATUS_RCRIT_JUMP 256
+__global__ void __launch_bounds__(256)
+rcrit_jump_kernel(const double* __restrict__ rc_old, const double* __restrict__ rc_new, int N, double scale,
+                  int* __restrict__ status)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < N && rc_new[b] > __dmul_rn(rc_old[b], scale)) atomicOr(status, GENGA_STATUS_RCRIT_JUMP);
 }
 
 // ---------------------------------------------------------------------------------------------

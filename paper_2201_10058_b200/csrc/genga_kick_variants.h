@@ -80,4 +80,6 @@ static const int GENGA_REC_ALIGN = 1024;   // every i_block divides it
 static const int64_t GENGA_CAND_PER_BODY = 64;
 static const int64_t GENGA_CAND_MIN = (int64_t)1 << 20;
 static const int64_t GENGA_CAND_MAX = (int64_t)1 << 28;
+// genga_kick_merged: the filter radius of the shared far-field pass is that of the old critical radii times 1 + this
+static const double GENGA_MERGE_MARGIN = 1.0 / 64.0;
 static const int64_t GENGA_MAX_BODIES = (int64_t)1 << 30;

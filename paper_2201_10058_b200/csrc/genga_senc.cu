@@ -140,36 +140,46 @@ int senc(Senc& s, int level, const int32_t* pairs_up, const int32_t* n_up, const
 
 }  // namespace
 
-extern "C" int genga_multilevel_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star,
-                                     double dt, const genga_senc_config* cfg, double* out_acc, int32_t* out_pairs,
-                                     int32_t* out_npairs, int32_t* out_stats)
+namespace {
+
+int check_ml_args(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star,
+                  const genga_senc_config* cfg, double* out_acc, int32_t* out_pairs, int32_t* out_npairs,
+                  int32_t* out_stats, int min_levels)
 {
     if (!ctx || !pos || !vel || !mass || !cfg || !out_npairs) return GENGA_KICK_E_NULL;
     if (!out_pairs && ctx->cfg.pair_capacity > 0) return GENGA_KICK_E_NULL;
     if (genga_misaligned(pos) || genga_misaligned(vel) || genga_misaligned(mass) || genga_misaligned(out_acc) ||
         genga_misaligned(out_pairs) || genga_misaligned(out_npairs) || genga_misaligned(out_stats))
         return GENGA_KICK_E_ALIGN;
-    if (cfg->slevels < 1 || cfg->slevels > GENGA_SENC_MAX_LEVELS || (cfg->slevels > 1 && cfg->substeps < 1) ||
-        !(cfg->tol > 0.0) || !(m_star > 0.0))
+    if (cfg->slevels < min_levels || cfg->slevels > GENGA_SENC_MAX_LEVELS || (cfg->slevels > 1 && cfg->substeps < 1) ||
+        (cfg->slevels >= 1 && !(cfg->tol > 0.0)) || !(m_star > 0.0))
         return GENGA_KICK_E_SIZE;
     if (cfg->slevels - 1 > ctx->cfg.max_level) return GENGA_KICK_E_LEVEL;
-    const size_t N = (size_t)ctx->N, cap = (size_t)ctx->cfg.pair_capacity;
-    const int SL = cfg->slevels;
-    cudaStream_t st = ctx->stream;
+    return GENGA_KICK_OK;
+}
 
+// cuts the library's slab for cfg->slevels levels (at least one r_crit row) plus one spare r_crit row (*rc_spare)
+int setup_senc(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
+               const genga_senc_config* cfg, int32_t* out_pairs, int32_t* out_npairs, int32_t* out_stats, Senc& s,
+               double** rc_spare)
+{
+    const size_t N = (size_t)ctx->N, cap = (size_t)ctx->cfg.pair_capacity;
+    const int SL = std::max(cfg->slevels, 1);
+    cudaStream_t st = ctx->stream;
     // scratch: one slab, cut per level (kept for the next call with as many or fewer levels)
     const size_t b_pairs = up16(std::max<size_t>(cap, 1) * 2 * sizeof(int32_t)), b_np = up16((N + 1) * sizeof(int32_t));
     const size_t b_n = up16(N * sizeof(int32_t)), b_state = up16(3 * N * sizeof(double)), b_row = up16(N * sizeof(double));
     const size_t per_level = 2 * b_pairs + 2 * b_np + 2 * b_n + b_np + 16 + 2 * b_state;
     if (!ctx->senc_slab || ctx->senc_levels < SL) {
         if (ctx->senc_slab) { GK_CUDA(ctx, cudaStreamSynchronize(st)); cudaFree(ctx->senc_slab); ctx->senc_slab = nullptr; }
-        GK_CUDA(ctx, cudaMalloc(&ctx->senc_slab, SL * (per_level + b_row)));
+        GK_CUDA(ctx, cudaMalloc(&ctx->senc_slab, SL * (per_level + b_row) + b_row));
         ctx->senc_levels = SL;
     }
-    Senc s = {};
+    s = Senc{};
     s.ctx = ctx; s.cfg = cfg; s.pos = pos; s.vel = vel; s.mass = mass; s.m_star = m_star; s.dt = dt;
     s.N = (long long)N; s.cap = (long long)cap; s.stats = out_stats;
     char* p = static_cast<char*>(ctx->senc_slab);
+    *rc_spare = reinterpret_cast<double*>(p); p += b_row;
     s.rc = reinterpret_cast<double*>(p); p += SL * b_row;
     for (int l = 0; l < SL; l++) {
         Level& L = s.lv[l];
@@ -186,24 +196,78 @@ extern "C" int genga_multilevel_step(genga_kick_ctx* ctx, double* pos, double* v
     }
     // level 0 writes its candidates where the caller reads them
     s.lv[0].cand = out_pairs; s.lv[0].cand_np = out_npairs;
-    if (out_stats) GK_CUDA(ctx, cudaMemsetAsync(out_stats, 0, (size_t)SL * 4 * sizeof(int32_t), st));
+    if (out_stats && cfg->slevels >= 1)
+        GK_CUDA(ctx, cudaMemsetAsync(out_stats, 0, (size_t)cfg->slevels * 4 * sizeof(int32_t), st));
+    return GENGA_KICK_OK;
+}
 
-    int rc = genga_rcrit(ctx, pos, vel, mass, m_star, dt, 2.0, 1, cfg->n1, cfg->n2, s.rc);
+// what lies between the two kicks of a step: HC(dt/2); FG(dt); detection, SEnc or grouping + Bulirsch-Stoer; HC(dt/2)
+// (slevels == 0: no encounter branch -- genga_drift)
+int middle(Senc& s)
+{
+    genga_kick_ctx* ctx = s.ctx;
+    const size_t N = (size_t)s.N;
+    if (s.cfg->slevels == 0) return genga_drift(ctx, s.pos, s.vel, s.mass, s.m_star, s.dt);
+    int rc = genga_hc(ctx, s.pos, s.vel, s.mass, s.m_star, 0.5 * s.dt);
+    if (rc != GENGA_KICK_OK) return rc;
+    GK_CUDA(ctx, cudaMemcpyAsync(s.lv[0].q0, s.pos, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    GK_CUDA(ctx, cudaMemcpyAsync(s.lv[0].v0, s.vel, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    rc = genga_fg(ctx, s.pos, s.vel, s.m_star, s.dt);
+    if (rc != GENGA_KICK_OK) return rc;
+    const int32_t *enc, *n_enc;
+    rc = encounters(s, 0, s.dt, &enc, &n_enc);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = descend(s, 0, s.dt, enc, n_enc);
+    if (rc != GENGA_KICK_OK) return rc;
+    return genga_hc(ctx, s.pos, s.vel, s.mass, s.m_star, 0.5 * s.dt);
+}
+
+}  // namespace
+
+extern "C" int genga_multilevel_step(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star,
+                                     double dt, const genga_senc_config* cfg, double* out_acc, int32_t* out_pairs,
+                                     int32_t* out_npairs, int32_t* out_stats)
+{
+    int rc = check_ml_args(ctx, pos, vel, mass, m_star, cfg, out_acc, out_pairs, out_npairs, out_stats, 1);
+    if (rc != GENGA_KICK_OK) return rc;
+    Senc s;
+    double* spare;
+    rc = setup_senc(ctx, pos, vel, mass, m_star, dt, cfg, out_pairs, out_npairs, out_stats, s, &spare);
+    if (rc != GENGA_KICK_OK) return rc;
+    rc = genga_rcrit(ctx, pos, vel, mass, m_star, dt, 2.0, 1, cfg->n1, cfg->n2, s.rc);
     if (rc != GENGA_KICK_OK) return rc;
     rc = genga_kick(ctx, pos, vel, mass, s.rc, 0, 0.5 * dt, nullptr, out_pairs, out_npairs);
     if (rc != GENGA_KICK_OK) return rc;
-    rc = genga_hc(ctx, pos, vel, mass, m_star, 0.5 * dt);
+    rc = middle(s);
     if (rc != GENGA_KICK_OK) return rc;
-    GK_CUDA(ctx, cudaMemcpyAsync(s.lv[0].q0, pos, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
-    GK_CUDA(ctx, cudaMemcpyAsync(s.lv[0].v0, vel, 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, st));
-    rc = genga_fg(ctx, pos, vel, m_star, dt);
+    return genga_kick_impl(ctx, pos, vel, mass, s.rc, 0, 0.5 * dt, out_acc, nullptr, nullptr);
+}
+
+extern "C" int genga_steps(genga_kick_ctx* ctx, double* pos, double* vel, const double* mass, double m_star, double dt,
+                           int32_t n_steps, const genga_senc_config* cfg, double* out_acc, int32_t* out_pairs,
+                           int32_t* out_npairs, int32_t* out_stats)
+{
+    int rc = check_ml_args(ctx, pos, vel, mass, m_star, cfg, out_acc, out_pairs, out_npairs, out_stats, 0);
     if (rc != GENGA_KICK_OK) return rc;
-    const int32_t *enc, *n_enc;
-    rc = encounters(s, 0, dt, &enc, &n_enc);
+    if (n_steps < 1) return GENGA_KICK_E_SIZE;
+    Senc s;
+    double* spare;
+    rc = setup_senc(ctx, pos, vel, mass, m_star, dt, cfg, out_pairs, out_npairs, out_stats, s, &spare);
     if (rc != GENGA_KICK_OK) return rc;
-    rc = descend(s, 0, dt, enc, n_enc);
+    const size_t N = (size_t)ctx->N;
+    rc = genga_rcrit(ctx, pos, vel, mass, m_star, dt, 2.0, 1, cfg->n1, cfg->n2, s.rc);
     if (rc != GENGA_KICK_OK) return rc;
-    rc = genga_hc(ctx, pos, vel, mass, m_star, 0.5 * dt);
+    rc = genga_kick(ctx, pos, vel, mass, s.rc, 0, 0.5 * dt, nullptr, out_pairs, out_npairs);
     if (rc != GENGA_KICK_OK) return rc;
+    for (int step = 0; step < n_steps; step++) {
+        rc = middle(s);
+        if (rc != GENGA_KICK_OK) return rc;
+        if (step == n_steps - 1) break;
+        // closing kick of this step + Rcrit + opening kick and pre-check of the next: one pass over the pairs
+        rc = genga_kick_merged_impl(ctx, pos, vel, mass, s.rc, spare, m_star, dt, cfg->n1, cfg->n2, nullptr, out_pairs,
+                                    out_npairs);
+        if (rc != GENGA_KICK_OK) return rc;
+        GK_CUDA(ctx, cudaMemcpyAsync(s.rc, spare, N * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    }
     return genga_kick_impl(ctx, pos, vel, mass, s.rc, 0, 0.5 * dt, out_acc, nullptr, nullptr);
 }
