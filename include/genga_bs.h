@@ -22,13 +22,16 @@
  * BS-B of Table 2); 33 .. 256 bodies: one thread-block cluster (8 x 256 threads) per group, eight
  * lanes per body, positions exchanged through distributed shared memory (BS-A); many groups side by side.  From 9
  * bodies on the force sum of a body is taken in eight interleaved partial sums combined in a fixed tree (the oracle
- * states the order).  Larger groups: one group at a time
- * over a whole co-resident grid with a grid-wide barrier per force evaluation (the paper's BS-M regime,
- * PAPER.md:595-597, with the sub-steps kept on the device instead of controlled from the host); a group larger
- * than that grid keeps the state already in pos / vel (8 lanes per body, each summing an eighth of the pair terms, up
- * to 64 threads x resident CTAs / 8 = about 11,800 bodies on a B200; beyond that one lane per body evaluating the same
- * eight partial sums, up to about 75,000 bodies)
- * and GENGA_KICK_STATUS_GROUP_TOO_LARGE is set.
+ * states the order).  Larger groups: cooperative launches of co-resident thread blocks, eight lanes per body, positions
+ * exchanged through L2 with one barrier per force evaluation (the paper's BS-M regime, with the
+ * sub-steps kept on the device instead of controlled from the host): groups of up to 512 and of up to 2048 bodies
+ * several at a time (the grid cut into teams of 64 / 256 blocks, a team per group with a barrier of its own), larger
+ * ones one after the other over the whole grid -- with 8, 4, 2 or 1 lanes per body as the grid holds them (9472 /
+ * 18,944 / 37,888 / 75,776 bodies on 148 SMs); beyond that GENGA_KICK_STATUS_GROUP_TOO_LARGE is set and the group keeps
+ * the state already in pos / vel.  In these regimes a body only evaluates the partners on its NEIGHBOUR LIST (built at
+ * the start of the group from the straight-line relative motion over dt; a pair outside the lists stays outside every
+ * critical radius and contributes exactly 0, as in the all-pairs sum: same bits, n x a few terms instead of n^2 per
+ * force evaluation), and a pair with r^2 >= rc0^2 (1 + 2^-20) is dismissed after 8 FP64 instructions in every regime.
  *
  * Works on the context of genga_kick.h (its N, G, stream); only enqueues; all pointers are DEVICE pointers.
  */
@@ -44,6 +47,10 @@ extern "C" {
 #define GENGA_KICK_STATUS_GROUP_TOO_LARGE 32   /* a group larger than the co-resident grid was left as it was */
 #define GENGA_KICK_STATUS_BS_NOT_CONVERGED 64  /* a step did not reach tol after 60 halvings: that group
                                                   stopped at its last accepted time                        */
+#define GENGA_KICK_STATUS_BS_LIST_ESCAPE 512   /* a body of a group above 256 bodies strayed further than
+                                                  G m_star dt^2 / |q|^2 from the straight line through its initial
+                                                  state: a pair outside that group's neighbour lists may have been
+                                                  missed (twice what the Sun's pull allows: never seen on a disk)    */
 
 /*
  *   pos_in, vel_in  [3][N] state before FG (read only)          mass [N]

@@ -29,11 +29,9 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
     // test-particle modes (sec. 8.1): bodies from n_massive on are semi-active particles; TP 0 has none
     long long n_massive = ctx->cfg.n_test > 0 ? (long long)ctx->cfg.n_massive : N;
     int tp_mode = ctx->cfg.tp_mode;
-    // whole-grid regime: scratch for one group of up to N bodies, and the size of a co-resident grid
+    // whole-grid regime: the size of a co-resident grid, and scratch for one group of up to N bodies or for one group
+    // of up to GENGA_BS_TEAM_BODIES bodies per team
     if (!ctx->bs_scratch) {
-        const size_t bytes = ((size_t)(7 + GENGA_BS_MAX_LEVELS) * N + 8) * sizeof(double);
-        GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, bytes));
-        GK_CUDA(ctx, cudaMemsetAsync(ctx->bs_scratch, 0, bytes, st));
         int per_sm = 0;
         GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>,
                                                                  GENGA_BS_COOP_THREADS, 0));
@@ -43,17 +41,52 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
                          &per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 1>, GENGA_BS_COOP_THREADS, 0));
         if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
         ctx->bs_coop_blocks1 = per_sm * ctx->num_sms;
+        ctx->bs_coop_blocks_by_lanes[0] = ctx->bs_coop_blocks;
+        ctx->bs_coop_blocks_by_lanes[3] = ctx->bs_coop_blocks1;
+        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                         &per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 4>, GENGA_BS_COOP_THREADS, 0));
+        if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
+        ctx->bs_coop_blocks_by_lanes[1] = per_sm * ctx->num_sms;
+        GK_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                         &per_sm, genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 2>, GENGA_BS_COOP_THREADS, 0));
+        if (per_sm < 1) return genga_cuda_fail(ctx, cudaErrorLaunchOutOfResources);
+        ctx->bs_coop_blocks_by_lanes[2] = per_sm * ctx->num_sms;
+        ctx->bs_teams = ctx->bs_coop_blocks / GENGA_BS_TEAM_CTAS;           // most teams any launch forms
+        ctx->bs_rows = std::max<long long>(N, (long long)ctx->bs_coop_blocks * GENGA_BS_COOP_THREADS / GENGA_BS_SUB);
+        for (int v = 1, lanes = GENGA_BS_SUB / 2; v < 4; v++, lanes /= 2)
+            ctx->bs_rows = std::max<long long>(ctx->bs_rows, lanes > 1 ? (long long)ctx->bs_coop_blocks_by_lanes[v] * GENGA_BS_COOP_THREADS / lanes : N);
+        const size_t bytes = ((size_t)(28 + GENGA_BS_MAX_LEVELS) * ctx->bs_rows + 16 * (size_t)std::max(ctx->bs_teams, 1) + 8) * sizeof(double);
+        GK_CUDA(ctx, cudaMalloc(&ctx->bs_scratch, bytes));
+        GK_CUDA(ctx, cudaMemsetAsync(ctx->bs_scratch, 0, bytes, st));
+        if (N > GENGA_BS_THREADS) {
+            // neighbour lists of the whole-grid regime: room for 1024 partners per body of the context (at least 2^24
+            // entries, at most 2^28), shared out among the teams; a group whose lists need more falls back to all pairs
+            ctx->bs_nbr_capacity = std::min<long long>(std::max<long long>(1024LL * N, 1LL << 24), 1LL << 28);
+            GK_CUDA(ctx, cudaMalloc(&ctx->bs_nbr, (size_t)ctx->bs_nbr_capacity * sizeof(int)));
+        }
     }
-    genga::BsGlobal gm;
+    genga::BsGlobal gm = {};
+    const size_t ctrl_words = 16 * (size_t)std::max(ctx->bs_teams, 1);
     {
+        const long long R = ctx->bs_rows;
         double* p = ctx->bs_scratch;
-        for (int h = 0; h < 2; h++) { gm.x[h] = p; p += N; gm.y[h] = p; p += N; gm.z[h] = p; p += N; }
-        gm.gm = p; p += N;
-        for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) { gm.rc[k] = p; p += N; }
-        gm.err = reinterpret_cast<unsigned long long*>(p);
-        gm.totals = gm.err + 4;
+        for (int h = 0; h < 2; h++) { gm.pk[h] = reinterpret_cast<double2*>(p); p += 4 * R; }     // (16-byte aligned: first)
+        gm.sr = reinterpret_cast<double2*>(p); p += 6 * R;
+        for (int h = 0; h < 2; h++) { gm.x[h] = p; p += R; gm.y[h] = p; p += R; gm.z[h] = p; p += R; }
+        gm.gm = p; p += R;
+        gm.rcsq = p; p += R;
+        gm.lr = p; p += R;
+        gm.la = p; p += R;
+        gm.ld = p; p += R;
+        gm.vx = p; p += R; gm.vy = p; p += R; gm.vz = p; p += R;
+        for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) { gm.rc[k] = p; p += R; }
+        gm.err = reinterpret_cast<unsigned long long*>(p);               // [teams][16] control words, then totals[4]
+        gm.totals = gm.err + ctrl_words;
+        gm.nbr = ctx->bs_nbr;
+        gm.nbr_capacity = ctx->bs_nbr_capacity;
         gm.stats = reinterpret_cast<int4*>(ctx->bs_stats);
         gm.stats_rows = ctx->bs_stats_rows;
+        gm.team_ctas = 0;
     }
     // at most N / 2 groups; warps / CTAs stride over them (their number is only known on the device)
     int small_max = GENGA_BS_THREADS;
@@ -79,39 +112,43 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
         ctx->launches++;
     }
     GK_CUDA(ctx, cudaGetLastError());
-    // the whole-grid regime, one large group after the other (returns at once if there is none): first a grid of one
-    // CTA per SM for the groups it can hold (its grid barrier costs a fraction of the full grid's), then the full
-    // co-resident grid for the larger ones
+    // groups above 256 bodies: cooperative launches (co-resident CTAs), eight lanes per body.  First the groups of up
+    // to 512 and then of up to 2048 bodies, several at a time: the grid cut into teams of 64 resp. 256 CTAs, a team per
+    // group with a barrier of its own.  Then the larger ones, one after the other over the whole grid, while the grid
+    // holds them at eight lanes per body (~11,800 bodies); one lane per body beyond.  Every launch returns at once if
+    // summary[2] shows no group for it.
     if (N > GENGA_BS_THREADS) {
-        GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
-        const int cap1 = ctx->num_sms * GENGA_BS_COOP_THREADS / GENGA_BS_SUB;
-        const bool two = N > cap1 && ctx->bs_coop_blocks > ctx->num_sms;
-        int big_max = two ? cap1 : -1;
+        int big_max = 0;
         void* args[] = {&pos_in, &vel_in, &mass, &rcrit, &NN, &nlevels, const_cast<double*>(&G), const_cast<double*>(&mu), &dt,
                         &tol, &members, &offsets, &summary, &pos, &vel, &status, &gm, &small_max, &n_massive, &tp_mode, &big_max};
-        GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>),
-                                                 dim3(two ? ctx->num_sms : ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0,
-                                                 st));
-        ctx->launches++;
-        if (two) {
-            // ... the full grid with eight lanes per body, and with one lane per body for the groups beyond that
-            const int cap2 = (int)std::min<long long>((long long)ctx->bs_coop_blocks * GENGA_BS_COOP_THREADS / GENGA_BS_SUB, N);
-            const bool three = N > cap2;
-            small_max = cap1;
-            big_max = three ? cap2 : -1;
-            GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
-            GK_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>),
-                                                     dim3(ctx->bs_coop_blocks), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
+        void* k8 = reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>);
+        void* k1 = reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 1>);
+        small_max = GENGA_BS_THREADS;
+        for (int mult = 1; mult <= 4; mult *= 4) {                          // teams of 64 and of 256 CTAs
+            const int tctas = GENGA_BS_TEAM_CTAS * mult, teams = ctx->bs_coop_blocks / tctas;
+            const int cap = tctas * GENGA_BS_COOP_THREADS / GENGA_BS_SUB;
+            if (teams < 2 || N <= small_max) continue;
+            big_max = N > cap ? cap : -1;
+            gm.team_ctas = tctas;
+            GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, ctrl_words * sizeof(unsigned long long), st));
+            GK_CUDA(ctx, cudaLaunchCooperativeKernel(k8, dim3(teams * tctas), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
             ctx->launches++;
-            if (three) {
-                small_max = cap2;
-                big_max = -1;
-                GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, 4 * sizeof(unsigned long long), st));
-                GK_CUDA(ctx, cudaLaunchCooperativeKernel(
-                                 reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 1>),
-                                 dim3(ctx->bs_coop_blocks1), dim3(GENGA_BS_COOP_THREADS), args, 0, st));
-                ctx->launches++;
-            }
+            small_max = cap;
+        }
+        gm.team_ctas = 0;
+        // the whole grid on one group at a time: as many lanes per body as the grid has for the group's size
+        void* kern[4] = {k8,
+                         reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 4>),
+                         reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 2>), k1};
+        for (int v = 0, lanes = GENGA_BS_SUB; v < 4 && N > small_max; v++, lanes /= 2) {
+            const long long cap = lanes > 1 ? (long long)ctx->bs_coop_blocks_by_lanes[v] * GENGA_BS_COOP_THREADS / lanes : N;
+            if (cap <= small_max) continue;
+            big_max = N > cap ? (int)cap : -1;
+            GK_CUDA(ctx, cudaMemsetAsync(gm.err, 0, ctrl_words * sizeof(unsigned long long), st));
+            GK_CUDA(ctx, cudaLaunchCooperativeKernel(kern[v], dim3(ctx->bs_coop_blocks_by_lanes[v]), dim3(GENGA_BS_COOP_THREADS),
+                                                     args, 0, st));
+            ctx->launches++;
+            small_max = (int)std::min<long long>(cap, N);
         }
     }
     GK_CUDA(ctx, cudaGetLastError());
@@ -134,7 +171,8 @@ extern "C" int genga_bs_totals(genga_kick_ctx* ctx, int64_t* totals, int32_t res
     if (!ctx || !totals) return GENGA_KICK_E_NULL;
     totals[0] = totals[1] = totals[2] = totals[3] = 0;
     if (!ctx->bs_scratch) return GENGA_KICK_OK;                       // genga_bs has not run yet
-    unsigned long long* t = reinterpret_cast<unsigned long long*>(ctx->bs_scratch + (size_t)(7 + GENGA_BS_MAX_LEVELS) * ctx->N) + 4;
+    unsigned long long* t = reinterpret_cast<unsigned long long*>(ctx->bs_scratch + (size_t)(28 + GENGA_BS_MAX_LEVELS) * ctx->bs_rows) +
+                            16 * (size_t)std::max(ctx->bs_teams, 1);
     GK_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     GK_CUDA(ctx, cudaMemcpy(totals, t, 4 * sizeof(int64_t), cudaMemcpyDeviceToHost));
     if (reset) GK_CUDA(ctx, cudaMemset(t, 0, 4 * sizeof(int64_t)));

@@ -45,11 +45,13 @@ namespace genga {
 #define GENGA_BS_SUB 8                  // whole-grid regime: lanes per body, each summing the terms with j = lane (mod 8)
                                         // (groups too large for that: one lane per body, the same eight partial sums)
 #define GENGA_BS_TILE 64                // j-bodies staged per round in the whole-grid regime
+#define GENGA_BS_TEAM_CTAS 64            // whole-grid regime in teams: CTAs of the small teams (512 bodies at eight lanes each)
 #define GENGA_BS_KMAX 8
 #define GENGA_BS_MAX_LEVELS 4
 #define GENGA_BS_MAX_HALVINGS 60
 #define GENGA_STATUS_GROUP_TOO_LARGE 32
 #define GENGA_STATUS_BS_NOT_CONVERGED 64
+#define GENGA_STATUS_BS_LIST_ESCAPE 512
 
 // the changeover function K (reading G1), IEEE operations in a fixed order
 __device__ __forceinline__ double bs_K(double r, double rc)
@@ -65,9 +67,27 @@ __device__ __forceinline__ double bs_K(double r, double rc)
 // the critical-radius rows, and four slots for the group-wide error maximum.
 struct BsGlobal {
     double* x[2]; double* y[2]; double* z[2];
+    double2* pk[2];                     // the same positions packed with the far-pair bound: (x, y), (z, bound) per body,
+                                        // one 32-byte sector per list entry
+    double2* sr;                        // what a NEAR list entry needs besides: (G m, rc0), (rc1, rc2), (rc3, -) per body
     double* gm;
+    double* rcsq;                       // far-pair bound of each body (bs_far_bound)
     double* rc[GENGA_BS_MAX_LEVELS];
+    // neighbour lists of the whole-grid regime (bs_build_lists)
+    double* lr;                         // [n] sqrt(far-pair bound) of each body
+    double* la;                         // [n] A_b: bound on its deviation from straight-line motion during the call
+    double* ld;                         // [n] |v_b| |dt| + A_b: bound on its displacement (cheap first test)
+    double* vx; double* vy; double* vz; // [n] velocities at the start of the call
+    int* nbr;                           // [nbr_capacity] list entries (member positions within the group)
+    long long nbr_capacity;
+    unsigned long long* cursor;         // entries reserved so far (zero between groups)
     unsigned long long* err;            // [4], all zero between uses
+    // teams: the co-resident grid cut into teams of team_ctas CTAs, each integrating its own groups with a barrier
+    // of its own (0: one team = the whole grid, cooperative-groups barrier).  bs_run points the arrays above at the
+    // team's slice of the scratch; ctrl = [teams][16] words: err[4], cursor, barrier counter.
+    int team_ctas;
+    int tb;                             // this CTA's index within its team (set by bs_run)
+    unsigned long long* bar;            // the team's barrier counter (only ever incremented within a launch)
     // diagnostics of the step-size control (include/genga_bs.h: genga_bs_set_stats, genga_bs_totals)
     unsigned long long* totals;         // [4] accepted macro steps, rejected attempts, force evaluations, groups: summed
     int4* stats;                        // [stats_rows] per group (accepted, rejected, force evaluations, bodies), or nullptr
@@ -78,6 +98,7 @@ struct BsGlobal {
 template <int ROWS>
 struct BsShared {
     double x[ROWS], y[ROWS], z[ROWS], gm[ROWS];
+    double rcsq[ROWS];                  // far-pair bound of each body (bs_far_bound)
     double rc[GENGA_BS_MAX_LEVELS][ROWS];
     double red[8];
     double errmax;
@@ -85,29 +106,86 @@ struct BsShared {
     // publishes into buffer e & 1 while slower CTAs may still gather from the other one), and its error maxima
     double pubx[2][GENGA_BS_CLUSTER_BODIES], puby[2][GENGA_BS_CLUSTER_BODIES], pubz[2][GENGA_BS_CLUSTER_BODIES];
     double emax[2];
+    unsigned long long bar_target;      // whole-grid regime in teams: the count the team's barrier has to reach next
 };
+
+// Barrier over the CTAs that integrate a group together: the whole grid (cooperative groups), or one team of it -- the
+// CTAs of a cooperative launch are co-resident, so a team may wait on a counter of its own: every CTA adds one and
+// waits until all team_ctas have (the counter is never reset within a launch; each CTA keeps the next target).
+template <int ROWS>
+__device__ __forceinline__ void bs_gsync(BsShared<ROWS>& S, const BsGlobal& Gm)
+{
+    if (Gm.team_ctas == 0) {
+        cooperative_groups::this_grid().sync();
+        return;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        S.bar_target += (unsigned long long)Gm.team_ctas;
+        __threadfence();
+        atomicAdd(Gm.bar, 1ULL);
+        unsigned long long seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(Gm.bar) : "memory");
+        } while (seen < S.bar_target);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// A pair with r^2 >= max(bound_i, bound_j), bound_b = rc0_b^2 (1 + 2^-20), has r > rc0_ij by more than 2^-22 relative:
+// y = (r - 0.1 rc)/(0.9 rc) > 1 whatever its rounding, K_0 = 1 and W_BS = prod (1 - K_k) = 0 EXACTLY -- the pair adds
+// nothing, as in the definition, and costs 8 FP64 instructions instead of ~100 (sqrt, a divide per level and one for
+// the term).  In the large groups of a disk almost all pairs are of this kind: a group is a chain of neighbours.
+__device__ __forceinline__ double bs_far_bound(double rc0) { return (rc0 * rc0) * (1.0 + 9.5367431640625e-07); }
 
 // one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3.
 // Test-particle modes (sec. 8.1, Fig. 14): a semi-active particle j is staged with the SIGN BIT of
 // G m_j set; it acts on nobody in TP 1 and on the massive bodies only in TP 2 (particles never feel each other).
-#define GENGA_BS_PAIR(XJ, YJ, ZJ, GMJ, RCJ) GENGA_BS_PAIR_ACC(XJ, YJ, ZJ, GMJ, RCJ, ax, ay, az)
-#define GENGA_BS_PAIR_ACC(XJ, YJ, ZJ, GMJ, RCJ, AX, AY, AZ)                                            \
+#define GENGA_BS_PAIR(XJ, YJ, ZJ, GMJ, RCJ, BNDJ) GENGA_BS_PAIR_ACC(XJ, YJ, ZJ, GMJ, RCJ, BNDJ, ax, ay, az)
+#define GENGA_BS_PAIR_ACC(XJ, YJ, ZJ, GMJ, RCJ, BNDJ, AX, AY, AZ)                                      \
     {                                                                                                  \
         double gmj = (GMJ);                                                                            \
         bool skip = false;                                                                             \
         if (__double2hiint(gmj) < 0) { skip = i_tp || tp_mode != 2; gmj = -gmj; }                      \
-        if (!skip) {                                                                                   \
-            const double dx = (XJ) - x, dy = (YJ) - y, dz = (ZJ) - z;                                  \
-            const double r2 = dx * dx + dy * dy + dz * dz;                                             \
+        const double dx = (XJ) - x, dy = (YJ) - y, dz = (ZJ) - z;                                      \
+        const double r2 = dx * dx + dy * dy + dz * dz;                                                 \
+        if (!skip && r2 < fmax(bnd_i, (BNDJ))) {                                                       \
             const double r = sqrt(r2);                                                                 \
             double W = 1.0;                                                                            \
-            for (int k = 0; k < nlevels; k++) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));              \
+            _Pragma("unroll")                                                                          \
+            for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++)                                              \
+                if (k < nlevels) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));                           \
             if (W != 0.0) {                                                                            \
                 const double s = gmj * W / (r2 * r);                                                   \
                 AX = AX + s * dx; AY = AY + s * dy; AZ = AZ + s * dz;                                  \
             }                                                                                          \
         }                                                                                              \
     }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Neighbour lists of the whole-grid regime.  A large group of a disk is a chain of neighbours: of its n^2 pairs all but
+// a few per body lie far outside every critical radius for the whole call and add exactly nothing (bs_far_bound).  At
+// the start of a group every lane lists the partners it may ever have to evaluate: those whose STRAIGHT-LINE relative
+// motion over the call comes closer than the far-pair radius plus the two bodies' allowances,
+//     min over tau in [0, dt] of |dq_ij(t0) + dv_ij(t0) tau|  <  max(R_i, R_j) + A_i + A_j,
+//     R_b = sqrt(far-pair bound of b),    A_b = G m_star dt^2 / |q_b(t0)|^2   (twice the Sun's a dt^2 / 2)
+// A_b bounds the body's deviation from q_b(t0) + v_b(t0) tau during the call; every force evaluation CHECKS it (it
+// knows its time tau) and raises GENGA_STATUS_BS_LIST_ESCAPE if a body strayed further -- then, and only then, a pair
+// outside the lists may have come inside a critical radius unseen.  A pair outside the lists therefore has
+// r > max(R_i, R_j) at every force evaluation and contributes exactly 0, as in the all-pairs sum: the lists change the
+// cost (n x a few partners instead of n^2 pairs per force evaluation), not one bit of the result.  A lane keeps the sub-list of ITS share of the
+// partners (j = lane (mod 8), ascending j), so the partial sums and their tree are those of the all-pairs loop.
+// Lists that do not fit the scratch (nbr_capacity entries) are not used: that group falls back to all pairs.
+// ---------------------------------------------------------------------------------------------------------------------
+template <int NL>
+struct BsList {
+    bool on;                            // lists in use for this group (grid-uniform)
+    long long base[NL];                 // this lane's sub-lists: u-th holds the partners j = sub + u (mod 8)
+    int count[NL];
+    double q0[3], v0[3];                // the body's state at the start of the call
+    double a2;                          // A_b^2
+};
 
 // Every thread publishes the position of its body i (if i < n) and gets dv_i/dt back:
 //   - G m_star q / |q|^3 + the pair terms over j = 0 .. n-1, j != i, in that order.
@@ -121,8 +199,9 @@ __device__ __forceinline__ void bs_sync()
 template <int MODE, int ROWS, int SUB>
 __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, int nlevels,
                                          bool i_tp, int tp_mode, double mu, const double (&rci)[GENGA_BS_MAX_LEVELS], const double (&q)[3],
-                                         double (&a)[3])
+                                         double (&a)[3], const BsList<8 / SUB>& L, double tau, int* __restrict__ status)
 {
+    const double bnd_i = bs_far_bound(rci[0]);
     const double x = q[0], y = q[1], z = q[2];
     const double r2s = x * x + y * y + z * z;
     const double rs = sqrt(r2s);
@@ -137,7 +216,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 #define GENGA_BS_RCJ(k) S.rc[k][j]
             for (int j = 0; j < n; j++) {
                 if (j == i) continue;
-                GENGA_BS_PAIR(S.x[j], S.y[j], S.z[j], S.gm[j], GENGA_BS_RCJ)
+                GENGA_BS_PAIR(S.x[j], S.y[j], S.z[j], S.gm[j], GENGA_BS_RCJ, S.rcsq[j])
             }
 #undef GENGA_BS_RCJ
         }
@@ -153,7 +232,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 #define GENGA_BS_RCJ(k) S.rc[k][jj]
             for (int jj = sub; jj < n; jj += SUB) {
                 if (jj == i) continue;
-                GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
+                GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ, S.rcsq[jj])
             }
 #undef GENGA_BS_RCJ
         }
@@ -186,7 +265,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 #define GENGA_BS_RCJ(k) S.rc[k][jj]
             for (int jj = sub; jj < n; jj += SUB) {
                 if (jj == i) continue;
-                GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ)
+                GENGA_BS_PAIR(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ, S.rcsq[jj])
             }
 #undef GENGA_BS_RCJ
         }
@@ -206,17 +285,53 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
         const int p = eval & 1;
         eval++;
         const int t = threadIdx.x, sub = t & (SUB - 1);
-        if (i < n && sub == 0) { Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z; }
-        cooperative_groups::this_grid().sync();
+        if (i < n && sub == 0) {
+            Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z;
+            if (L.on) { Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bnd_i); }
+        }
+        bs_gsync(S, Gm);
         const double sx = ax, sy = ay, sz = az;
         double px[8 / SUB], py[8 / SUB], pz[8 / SUB];
 #pragma unroll
         for (int u = 0; u < 8 / SUB; u++) { px[u] = 0.0; py[u] = 0.0; pz[u] = 0.0; }
-        for (int j0 = 0; j0 < n; j0 += ROWS) {                // ROWS is a multiple of 8: (j0 + jj) mod 8 = jj mod 8
+        if (L.on && i < n) {
+            // the body must still be where the lists allow it to be
+            const double ex = x - (L.q0[0] + L.v0[0] * tau), ey = y - (L.q0[1] + L.v0[1] * tau), ez = z - (L.q0[2] + L.v0[2] * tau);
+            if (ex * ex + ey * ey + ez * ez > L.a2) atomicOr(status, GENGA_STATUS_BS_LIST_ESCAPE);
+#pragma unroll
+            for (int u = 0; u < 8 / SUB; u++) {
+                const long long end = L.base[u] + L.count[u];
+                for (long long e = L.base[u]; e < end; e += 4) {          // four entries' loads in flight at a time
+                    int jn[4];
+                    double2 pa[4], pb[4];
+#pragma unroll
+                    for (int k = 0; k < 4; k++) jn[k] = e + k < end ? Gm.nbr[e + k] : -1;
+#pragma unroll
+                    for (int k = 0; k < 4; k++)
+                        if (jn[k] >= 0) { pa[k] = __ldcg(Gm.pk[p] + 2 * jn[k]); pb[k] = __ldcg(Gm.pk[p] + 2 * jn[k] + 1); }
+#pragma unroll
+                    for (int k = 0; k < 4; k++) {
+                        if (jn[k] < 0) continue;
+                        const int jj = jn[k];
+                        // the far test on the packed record alone; G m_j and the radii are fetched for near pairs only
+                        const double fx = pa[k].x - x, fy = pa[k].y - y, fz = pb[k].x - z;
+                        if (fx * fx + fy * fy + fz * fz < fmax(bnd_i, pb[k].y)) {
+                            const double2 s0 = __ldcg(Gm.sr + 3 * jj), s1 = __ldcg(Gm.sr + 3 * jj + 1), s2 = __ldcg(Gm.sr + 3 * jj + 2);
+                            const double rcj[GENGA_BS_MAX_LEVELS] = {s0.y, s1.x, s1.y, s2.x};
+#define GENGA_BS_RCL(k) rcj[k]
+                            GENGA_BS_PAIR_ACC(pa[k].x, pa[k].y, pb[k].x, s0.x, GENGA_BS_RCL, pb[k].y, px[u], py[u], pz[u])
+#undef GENGA_BS_RCL
+                        }
+                    }
+                }
+            }
+        }
+        for (int j0 = 0; j0 < (L.on ? 0 : n); j0 += ROWS) {   // ROWS is a multiple of 8: (j0 + jj) mod 8 = jj mod 8
             __syncthreads();
             if (t < ROWS && j0 + t < n) {
                 S.x[t] = __ldcg(Gm.x[p] + j0 + t); S.y[t] = __ldcg(Gm.y[p] + j0 + t); S.z[t] = __ldcg(Gm.z[p] + j0 + t);
                 S.gm[t] = __ldcg(Gm.gm + j0 + t);
+                S.rcsq[t] = __ldcg(Gm.rcsq + j0 + t);
                 for (int k = 0; k < nlevels; k++) S.rc[k][t] = __ldcg(Gm.rc[k] + j0 + t);
             }
             __syncthreads();
@@ -226,34 +341,128 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
                 for (int j8 = 0; j8 < m; j8 += 8) {
 #pragma unroll
                     for (int u = 0; u < 8 / SUB; u++) {
-                        const int jj = j8 + sub + u;          // SUB = 8: u = 0, jj = j8 + sub;  SUB = 1: jj = j8 + u
+                        const int jj = j8 + sub + SUB * u;    // this lane's residues j mod 8: sub, sub + SUB, ..
                         if (jj < m && j0 + jj != i) {
-                            GENGA_BS_PAIR_ACC(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ, px[u], py[u], pz[u])
+                            GENGA_BS_PAIR_ACC(S.x[jj], S.y[jj], S.z[jj], S.gm[jj], GENGA_BS_RCJ, S.rcsq[jj], px[u], py[u], pz[u])
                         }
                     }
                 }
 #undef GENGA_BS_RCJ
             }
         }
-        if (SUB == 8) {
-            ax = px[0]; ay = py[0]; az = pz[0];
+        // p_r = the terms with j = r (mod 8); lane `sub` holds p_sub, p_sub+SUB, ..: first the pairs of the tree that lie
+        // in different lanes (xor butterfly: IEEE addition commutes, so every lane of the body gets the same bits),
+        // then those within the lane: ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) whatever SUB is
 #pragma unroll
-            for (int o = 1; o < 8; o <<= 1) {
-                ax = ax + __shfl_xor_sync(0xffffffffu, ax, o);
-                ay = ay + __shfl_xor_sync(0xffffffffu, ay, o);
-                az = az + __shfl_xor_sync(0xffffffffu, az, o);
+        for (int o = 1; o < SUB; o <<= 1) {
+#pragma unroll
+            for (int u = 0; u < 8 / SUB; u++) {
+                px[u] = px[u] + __shfl_xor_sync(0xffffffffu, px[u], o);
+                py[u] = py[u] + __shfl_xor_sync(0xffffffffu, py[u], o);
+                pz[u] = pz[u] + __shfl_xor_sync(0xffffffffu, pz[u], o);
             }
-        } else {
-            ax = ((px[0] + px[1 % (8 / SUB)]) + (px[2 % (8 / SUB)] + px[3 % (8 / SUB)])) +
-                 ((px[4 % (8 / SUB)] + px[5 % (8 / SUB)]) + (px[6 % (8 / SUB)] + px[7 % (8 / SUB)]));
-            ay = ((py[0] + py[1 % (8 / SUB)]) + (py[2 % (8 / SUB)] + py[3 % (8 / SUB)])) +
-                 ((py[4 % (8 / SUB)] + py[5 % (8 / SUB)]) + (py[6 % (8 / SUB)] + py[7 % (8 / SUB)]));
-            az = ((pz[0] + pz[1 % (8 / SUB)]) + (pz[2 % (8 / SUB)] + pz[3 % (8 / SUB)])) +
-                 ((pz[4 % (8 / SUB)] + pz[5 % (8 / SUB)]) + (pz[6 % (8 / SUB)] + pz[7 % (8 / SUB)]));
         }
+#pragma unroll
+        for (int w = 1; w < 8 / SUB; w <<= 1) {
+#pragma unroll
+            for (int u = 0; u + w < 8 / SUB; u += 2 * w) {
+                px[u] = px[u] + px[u + w]; py[u] = py[u] + py[u + w]; pz[u] = pz[u] + pz[u + w];
+            }
+        }
+        ax = px[0]; ay = py[0]; az = pz[0];
         ax = sx + ax; ay = sy + ay; az = sz + az;
     }
     a[0] = ax; a[1] = ay; a[2] = az;
+}
+
+// Whole-grid regime, start of a group: publishes the bodies' starting positions, R_b and D_b, counts and fills the
+// lanes' sub-lists (two scans of the group, tile by tile through shared memory; a lane reserves the room of its
+// sub-lists with one atomic on a cursor -- where a sub-list lies is irrelevant, its entries are in ascending j).
+// Two grid barriers; the positions go to buffer eval & 1 like a force evaluation's.
+template <int ROWS, int SUB>
+__device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, bool i_tp,
+                                               int tp_mode, const double (&q)[3], const double (&v)[3], double rc0, double dt,
+                                               double mu, BsList<8 / SUB>& L)
+{
+    constexpr int NL = 8 / SUB;
+    const int t = threadIdx.x, sub = t & (SUB - 1);
+    const int p = eval & 1;
+    eval++;
+    const double x = q[0], y = q[1], z = q[2];
+    const double lr_i = sqrt(bs_far_bound(rc0));
+    const double la_i = i < n ? mu * (dt * dt) / (x * x + y * y + z * z) : 0.0;
+    const double ld_i = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) * fabs(dt) + la_i;
+    L.q0[0] = x; L.q0[1] = y; L.q0[2] = z;
+    L.v0[0] = v[0]; L.v0[1] = v[1]; L.v0[2] = v[2];
+    L.a2 = la_i * la_i;
+    if (i < n && sub == 0) {
+        Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z;
+        Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bs_far_bound(rc0));
+        Gm.vx[i] = v[0]; Gm.vy[i] = v[1]; Gm.vz[i] = v[2];
+        Gm.lr[i] = lr_i; Gm.la[i] = la_i; Gm.ld[i] = ld_i;
+    }
+    if (Gm.tb == 0 && t == 0) *Gm.cursor = 0ULL;            // (its last readers passed several barriers ago)
+    bs_gsync(S, Gm);
+#pragma unroll
+    for (int u = 0; u < NL; u++) { L.base[u] = 0; L.count[u] = 0; }
+    L.on = false;
+    for (int pass = 0; pass < 2; pass++) {                    // 0: count, 1: fill
+        int c[NL];
+#pragma unroll
+        for (int u = 0; u < NL; u++) c[u] = 0;
+        for (int j0 = 0; j0 < n; j0 += ROWS) {
+            __syncthreads();
+            if (t < ROWS && j0 + t < n) {
+                S.x[t] = __ldcg(Gm.x[p] + j0 + t); S.y[t] = __ldcg(Gm.y[p] + j0 + t); S.z[t] = __ldcg(Gm.z[p] + j0 + t);
+                S.gm[t] = __ldcg(Gm.gm + j0 + t);
+                S.rcsq[t] = __ldcg(Gm.lr + j0 + t);
+                S.rc[0][t] = __ldcg(Gm.ld + j0 + t);
+                S.rc[1][t] = __ldcg(Gm.la + j0 + t);
+            }
+            __syncthreads();
+            if (i < n) {
+                const int m = min(ROWS, n - j0);
+                for (int j8 = 0; j8 < m; j8 += 8) {
+#pragma unroll
+                    for (int u = 0; u < NL; u++) {
+                        const int jj = j8 + sub + SUB * u;
+                        if (jj < m && j0 + jj != i) {
+                            const bool never = __double2hiint(S.gm[jj]) < 0 && (i_tp || tp_mode != 2);   // sec. 8.1
+                            const double dx = S.x[jj] - x, dy = S.y[jj] - y, dz = S.z[jj] - z;
+                            const double Rm = fmax(lr_i, S.rcsq[jj]);
+                            const double R = Rm + (ld_i + S.rc[0][jj]);
+                            // first the cheap test on the displacement bounds (implied by the one below), then the
+                            // closest approach of the straight-line relative motion over [0, dt]
+                            if (!never && dx * dx + dy * dy + dz * dz < R * R) {
+                                const double wx = __ldcg(Gm.vx + j0 + jj) - v[0], wy = __ldcg(Gm.vy + j0 + jj) - v[1],
+                                             wz = __ldcg(Gm.vz + j0 + jj) - v[2];
+                                const double w2 = wx * wx + wy * wy + wz * wz, dw = dx * wx + dy * wy + dz * wz;
+                                double ts = w2 > 0.0 ? -dw / w2 : 0.0;            // unconstrained closest approach
+                                ts = dt > 0.0 ? fmin(fmax(ts, 0.0), dt) : fmax(fmin(ts, 0.0), dt);
+                                const double cx = dx + wx * ts, cy = dy + wy * ts, cz = dz + wz * ts;
+                                const double Ra = Rm + (la_i + S.rc[1][jj]);
+                                // (1 + 2^-30: the roundings of this test must not drop a pair the exact test keeps)
+                                if (cx * cx + cy * cy + cz * cz < (Ra * Ra) * (1.0 + 9.313225746154785e-10)) {
+                                    if (pass) Gm.nbr[L.base[u] + c[u]] = j0 + jj;
+                                    c[u]++;
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        if (pass) break;
+        unsigned long long total = 0;
+#pragma unroll
+        for (int u = 0; u < NL; u++) { L.count[u] = c[u]; total += (unsigned long long)c[u]; }
+        unsigned long long base = total ? atomicAdd(Gm.cursor, total) : 0ULL;
+#pragma unroll
+        for (int u = 0; u < NL; u++) { L.base[u] = (long long)base; base += (unsigned long long)c[u]; }
+        bs_gsync(S, Gm);
+        if (__ldcg(Gm.cursor) > (unsigned long long)Gm.nbr_capacity) return;    // team-uniform: all pairs instead
+    }
+    L.on = true;
 }
 
 // maximum of e over the group (order-free); CTA- (and, COOP, grid-) uniform result
@@ -293,9 +502,9 @@ __device__ __forceinline__ double bs_group_max(BsShared<ROWS>& S, const BsGlobal
     const int slot = echeck & 3;
     echeck++;
     if (t == 0) atomicMax(Gm.err + slot, (unsigned long long)__double_as_longlong(S.errmax));
-    cooperative_groups::this_grid().sync();
+    bs_gsync(S, Gm);
     const double m = __longlong_as_double((long long)__ldcg(Gm.err + slot));
-    if (blockIdx.x == 0 && t == 0) Gm.err[(slot + 2) & 3] = 0ULL;
+    if (Gm.tb == 0 && t == 0) Gm.err[(slot + 2) & 3] = 0ULL;
     return m;
 }
 
@@ -344,13 +553,14 @@ __device__ __forceinline__ void
 bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, const double* __restrict__ mass,
           const double* __restrict__ rcrit, long long N, int nlevels, double G, double mu, double dt, double tol,
           const int* __restrict__ members, const int* __restrict__ offsets, const int* __restrict__ summary,
-          double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm, int small_max,
+          double* __restrict__ pos, double* __restrict__ vel, int* __restrict__ status, const BsGlobal Gm_in, int small_max,
           long long n_massive, int tp_mode, int big_max, int vblock, int vgrid)
 {
+    BsGlobal Gm = Gm_in;
     // vblock / vgrid: this CTA's index and the number of CTAs of its regime (the warp and one-CTA regimes share a launch)
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP, WARP = MODE == GENGA_BS_MODE_WARP;
     constexpr bool CLUSTER = MODE == GENGA_BS_MODE_CLUSTER, LISTED = COOP || CLUSTER;
-    constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : THREADS);
+    constexpr int ROWS = COOP ? GENGA_BS_TILE : (WARP ? GENGA_BS_WARP_MAX : (MODE == GENGA_BS_MODE_CTA ? GENGA_BS_CTA_MAX : THREADS));
     constexpr int UNITS = WARP ? THREADS / 32 : 1;                      // groups in flight per CTA
     __shared__ BsShared<ROWS> Sall[UNITS];
     BsShared<ROWS>& S = Sall[WARP ? threadIdx.x >> 5 : 0];
@@ -360,9 +570,27 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
     // (cluster regime: the same, over the CTAs of the cluster: CTA r holds the bodies 32 r .. 32 r + 31)
     const int crank = CLUSTER ? (int)(blockIdx.x % GENGA_BS_CLUSTER) : 0;
     constexpr bool CTA = MODE == GENGA_BS_MODE_CTA;
-    const int i = COOP ? (int)((blockIdx.x * THREADS + t) / SUB) : (CLUSTER ? (crank * THREADS + t) / SUB : (CTA ? t / SUB : t));
+    // whole-grid regime: this CTA's team (the whole grid, or team_ctas consecutive CTAs), and the team's slice of the scratch
+    const int tctas = COOP ? (Gm.team_ctas ? Gm.team_ctas : (int)gridDim.x) : 1;
+    const int team = COOP ? (int)blockIdx.x / tctas : 0, n_teams = COOP ? (int)gridDim.x / tctas : 1;
+    if (COOP) {
+        if (team >= n_teams) return;                                    // CTAs beyond the last whole team
+        Gm.tb = (int)blockIdx.x - team * tctas;
+        const long long off = (long long)team * tctas * THREADS / SUB;
+#pragma unroll
+        for (int h = 0; h < 2; h++) { Gm.x[h] += off; Gm.y[h] += off; Gm.z[h] += off; Gm.pk[h] += 2 * off; }
+        Gm.sr += 3 * off;
+        Gm.gm += off; Gm.rcsq += off; Gm.lr += off; Gm.la += off; Gm.ld += off; Gm.vx += off; Gm.vy += off; Gm.vz += off;
+#pragma unroll
+        for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) Gm.rc[k] += off;
+        Gm.err += 16 * team; Gm.cursor = Gm.err + 4; Gm.bar = Gm.err + 5;
+        Gm.nbr_capacity = Gm.nbr_capacity / n_teams;
+        Gm.nbr += (long long)team * Gm.nbr_capacity;
+        if (threadIdx.x == 0) S.bar_target = 0ULL;
+    }
+    const int i = COOP ? (int)((Gm.tb * THREADS + t) / SUB) : (CLUSTER ? (crank * THREADS + t) / SUB : (CTA ? t / SUB : t));
     const bool writer = WARP || (t & (SUB - 1)) == 0;
-    const long long capacity = COOP ? (long long)gridDim.x * THREADS / SUB : ROWS;
+    const long long capacity = COOP ? (long long)tctas * THREADS / SUB : ROWS;
     const int n_groups = summary[0];
     int eval = 0, echeck = 0;
     const int g0 = COOP ? 0 : (WARP ? (int)(vblock * UNITS + (threadIdx.x >> 5)) : vblock);
@@ -370,8 +598,8 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
     __shared__ int big[LISTED ? GENGA_BS_BIG_LIST : 1];
     __shared__ unsigned wm[THREADS / 32];
     // whole-grid regime: every CTA walks the whole list; cluster regime: cluster c takes the entries c, c + clusters, ..
-    const int lfirst = CLUSTER ? (int)(blockIdx.x / GENGA_BS_CLUSTER) : 0;
-    const int lstep = CLUSTER ? (int)(gridDim.x / GENGA_BS_CLUSTER) : 1;
+    const int lfirst = CLUSTER ? (int)(blockIdx.x / GENGA_BS_CLUSTER) : team;
+    const int lstep = CLUSTER ? (int)(gridDim.x / GENGA_BS_CLUSTER) : n_teams;
     int scan_from = 0, nbig = 0, ib = 0;
     if (LISTED && summary[2] <= small_max) return;                      // no group for this regime (grid-uniform)
     for (int g = g0;; g += gstep) {
@@ -390,7 +618,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
                  : (WARP ? n > GENGA_BS_SEQ_MAX : (CTA ? (n <= GENGA_BS_SEQ_MAX || n > GENGA_BS_CTA_MAX) : false))) continue;
         // (listed regimes: the scan has already applied these bounds)
         if (n > capacity) {
-            if (t == 0 && blockIdx.x == 0) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
+            if (t == 0 && (COOP ? Gm.tb == 0 : blockIdx.x == 0)) atomicOr(status, GENGA_STATUS_GROUP_TOO_LARGE);
             continue;
         }
         const bool active = i < n;
@@ -407,10 +635,14 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
             if (COOP) {
                 if (writer) {
                     Gm.gm[i] = gm;
+                    Gm.sr[3 * i] = make_double2(gm, rci[0]); Gm.sr[3 * i + 1] = make_double2(rci[1], rci[2]);
+                    Gm.sr[3 * i + 2] = make_double2(rci[3], 0.0);
+                    Gm.rcsq[i] = bs_far_bound(rci[0]);
                     for (int k = 0; k < nlevels; k++) Gm.rc[k][i] = rci[k];
                 }
             } else if (WARP) {
                 S.gm[i] = gm;
+                S.rcsq[i] = bs_far_bound(rci[0]);
                 for (int k = 0; k < nlevels; k++) S.rc[k][i] = rci[k];
             }
         }
@@ -418,11 +650,15 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
             for (int idx = t; idx < n; idx += THREADS) {
                 const long long bj = members[first + idx];
                 S.gm[idx] = bj >= n_massive ? -(G * mass[bj]) : G * mass[bj];
+                S.rcsq[idx] = bs_far_bound(rcrit[bj]);
                 for (int k = 0; k < nlevels; k++) S.rc[k][idx] = rcrit[(long long)k * N + bj];
             }
         }
         // (COOP: G m and the radii are read by other CTAs only after the first force evaluation's grid barrier;
         //  the previous group's last readers passed a grid barrier -- its last error check -- before anyone gets here)
+        BsList<8 / SUB> L;
+        L.on = false;
+        if (COOP) bs_build_lists<ROWS, SUB>(S, Gm, eval, i, n, i_tp, tp_mode, q, v, rci[0], dt, mu, L);
         double Pq[GENGA_BS_KMAX][3], Pv[GENGA_BS_KMAX][3];             // P[j] = T_{k-1,j} of the extrapolation tableau
         double a0[3], cq[3], cv[3], dq[3], dv[3];
         double done = 0.0, H = dt;
@@ -430,7 +666,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         int n_acc = 0, n_rej = 0, n_fev = 0;                           // group-uniform, like every decision below
         while (done != dt) {                                           // all decisions below are group-uniform
             if ((dt > 0.0 && done + H > dt) || (dt < 0.0 && done + H < dt)) H = dt - done;
-            bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, q, a0);
+            bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, q, a0, L, done, status);
             n_fev++;
             int halvings = 0, kconv = 0;
             for (;;) {
@@ -444,14 +680,15 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
 #pragma unroll
                         for (int c = 0; c < 3; c++) { qm[c] = q[c]; vm[c] = v[c]; qn[c] = q[c] + h * v[c]; vn[c] = v[c] + h * a0[c]; }
                         for (int m = 1; m < nk; m++) {
-                            bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
+                            bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a, L,
+                                                      done + (double)m * h, status);
 #pragma unroll
                             for (int c = 0; c < 3; c++) {
                                 const double qs = qm[c] + h2 * vn[c], vs = vm[c] + h2 * a[c];
                                 qm[c] = qn[c]; vm[c] = vn[c]; qn[c] = qs; vn[c] = vs;
                             }
                         }
-                        bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a);
+                        bs_force<MODE, ROWS, SUB>(S, Gm, eval, i, n, nlevels, i_tp, tp_mode, mu, rci, qn, a, L, done + H, status);
 #pragma unroll
                         for (int c = 0; c < 3; c++) {
                             cq[c] = 0.5 * (qn[c] + qm[c] + h * vn[c]);
@@ -500,7 +737,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
             else done = done + H;
             if (kconv <= 5) H = 2.0 * H;
         }
-        if (fail && t == 0 && blockIdx.x == (COOP ? 0 : blockIdx.x)) atomicOr(status, GENGA_STATUS_BS_NOT_CONVERGED);
+        if (fail && t == 0 && (!COOP || Gm.tb == 0)) atomicOr(status, GENGA_STATUS_BS_NOT_CONVERGED);
         if (active && writer) {                                        // (after a failure: the state at the last accepted time)
 #pragma unroll
             for (int c = 0; c < 3; c++) { pos[c * N + b] = q[c]; vel[c * N + b] = v[c]; }
@@ -526,7 +763,9 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         n_massive, tp_mode, big_max
 
 template <int MODE, int THREADS, int SUB = 1>
-__global__ void __launch_bounds__(THREADS) bs_kernel(GENGA_BS_ARGS)
+// (8 CTAs of 64 threads per SM whatever the variant: the capacities of the whole-grid regime -- 9472 bodies at eight
+// lanes each on 148 SMs, twice that at four, .. -- must not move with the register allocator's mood)
+__global__ void __launch_bounds__(THREADS, 8) bs_kernel(GENGA_BS_ARGS)
 {
     bs_run<MODE, THREADS, SUB>(GENGA_BS_PASS, (int)blockIdx.x, (int)gridDim.x);
 }

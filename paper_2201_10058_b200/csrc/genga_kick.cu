@@ -517,7 +517,7 @@ extern "C" int genga_kick_free(genga_kick_ctx* ctx)
                     ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->partial2, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs,
                     ctx->psum_partial, ctx->psum_ticket, ctx->step_rcrit, ctx->grp_label, ctx->grp_flag,
-                    ctx->grp_keys_a, ctx->grp_keys_b, ctx->grp_vals_a, ctx->grp_vals_b, ctx->grp_counts, ctx->hyb_state, ctx->bs_scratch, ctx->senc_slab};
+                    ctx->grp_keys_a, ctx->grp_keys_b, ctx->grp_vals_a, ctx->grp_vals_b, ctx->grp_counts, ctx->hyb_state, ctx->bs_scratch, ctx->bs_nbr, ctx->senc_slab};
     for (void* b : bufs)
         if (b) cudaFree(b);
     if (ctx->ev)

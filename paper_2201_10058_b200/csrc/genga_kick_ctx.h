@@ -62,8 +62,13 @@ struct genga_kick_ctx {
     double* bs_scratch;            // whole-grid Bulirsch-Stoer regime: positions (2 buffers), G m, r_crit rows, error slots
     int32_t* bs_stats;             // caller's per-group record of the step-size control, or nullptr (genga_bs_set_stats)
     int64_t bs_stats_rows;
+    int* bs_nbr;                   // ... neighbour lists of the group being integrated
+    long long bs_nbr_capacity;
     int bs_coop_blocks;            // its co-resident grid (eight lanes per body)
     int bs_coop_blocks1;           // ... of the one-lane-per-body variant
+    int bs_coop_blocks_by_lanes[4];// co-resident grids of the variants with 8, 4, 2, 1 lanes per body
+    int bs_teams;                  // teams of GENGA_BS_TEAM_CTAS CTAs that grid is cut into
+    long long bs_rows;             // rows of every array of bs_scratch
     double* hyb_state;             // [6][N] state before FG (genga_hybrid_step), lazily allocated
     void* senc_slab;               // scratch of genga_multilevel_step (genga_senc.cu), lazily allocated
     int senc_levels;               // levels it was cut for

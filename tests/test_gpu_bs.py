@@ -312,9 +312,23 @@ def test_semi_active_particles_in_groups(oracle_mod, tp_mode):
     assert np.abs(qf - qw).max() > 1e-9
 
 
-def test_giant_group_one_lane_per_body(oracle_mod):
-    """A group too large for eight lanes per body on the full grid (above ~11,800 bodies on a B200) is integrated with
-    one lane per body, which evaluates the same eight partial sums and the same tree: bit-identical to the oracle."""
+def test_dense_large_group_falls_back_to_all_pairs(oracle_mod):
+    """A large group in which every body is inside every other's critical radius: its neighbour lists (n^2 entries) do
+    not fit the team's share of the list scratch, the group is integrated over all pairs instead -- same result."""
+    m = 2000
+    ki = gi.make_ring(m)
+    rc = np.full((1, m), 10.0)                                    # AU: K = 0, W_BS = 1 for every pair
+    mass = np.full(m, 1e-10)
+    qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, mass, rc, np.arange(m), [0, m], ki.G, 1.0, 1.0, 1e-10, ki.pos, ki.vel,
+                                        max_group=None)
+    q, v, st, gs = _gpu_bs(m, ki.pos, ki.vel, mass, rc, 1, 1.0, 1e-10, np.arange(m), [0, m], ki.pos, ki.vel)
+    assert st == 0 and not stats[0].failed
+    _check(q, v, qw, vw, np.arange(m), [0, m], gs, stats, 1e-10)
+
+
+def test_giant_group_fewer_lanes_per_body(oracle_mod):
+    """A group too large for eight lanes per body on the full grid (above 9472 bodies on a B200) is integrated with four
+    lanes per body (two, one beyond 18,944 / 37,888), each lane holding more of the eight partial sums: the same tree."""
     m = 12500
     ki = gi.make_ring(m)
     qw, vw, stats, _ = oracle_mod.bs.bs(ki.pos, ki.vel, ki.mass, ki.rcrit, np.arange(m), [0, m], ki.G, 1.0, 2.0, 1e-9,
@@ -325,12 +339,12 @@ def test_giant_group_one_lane_per_body(oracle_mod):
     assert np.abs(q - ki.pos).max() > 1e-3
 
 
-@pytest.mark.parametrize("size,count,dt,tol", [(40, 700, 3.0, 1e-10), (257, 258, 0.01, 1e-6)])
+@pytest.mark.parametrize("size,count,dt,tol", [(40, 700, 3.0, 1e-10), (257, 258, 0.01, 1e-6), (600, 41, 0.5, 1e-8)])
 def test_many_mid_size_groups_are_all_found(oracle_mod, size, count, dt, tol):
     """More groups of one regime than one batch of the device-side group scan holds (256): 700 groups of 40 bodies for
-    the cluster regime (dealt round-robin to the clusters across batches), 258 groups of 257 bodies for the whole-grid
-    regime (a short step at a loose tolerance: the oracle walks these groups one by one) -- arcs of one large ring,
-    every group integrated, bit-identical to the oracle."""
+    the cluster regime (dealt round-robin to the clusters across batches), 258 groups of 257 bodies for the teams of 64
+    CTAs of the whole-grid regime and 41 groups of 600 bodies for its teams of 256 CTAs (several groups at a time, each
+    team with its own barrier and neighbour lists) -- arcs of one large ring, every group integrated."""
     m = size * count
     ki = gi.make_ring(m, partners=4)
     members = np.arange(m)
