@@ -210,8 +210,11 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 256 MiB > 126 MB of L2
 
     def step():
+        # (the level-1 kick acts on the positions the level-0 kick has just sorted: it keeps that internal order)
         for level in LEVELS:
+            kick.set_order_reuse(level > 0)
             kick.kick(pos, vel, mass, rcrit, level, 0.5 * ki.dt, acc, pairs, npairs)
+        kick.set_order_reuse(False)
 
     def barrier():
         if world > 1:
@@ -577,7 +580,9 @@ def run_b200(args, rank: int, world: int, local_rank: int):
 
     def host_step():
         for level in LEVELS:
+            kick.set_order_reuse(level > 0)
             kick.kick_host(h_pos, h_vel, h_mass, h_rc, level, 0.5 * ki.dt, h_acc, h_pairs, h_np)
+        kick.set_order_reuse(False)
 
     for _ in range(max(args.warmup, 3)):
         host_step()

@@ -165,6 +165,15 @@ int genga_kick(genga_kick_ctx* ctx,
                double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
 
 /*
+ * While `on` is non-zero, genga_kick keeps the internal body order of the last call that sorted instead of sorting
+ * again: for consecutive calls on unchanged or little-changed positions, e.g. the kicks of several changeover levels
+ * of one step.  The internal order is never visible and never changes a result beyond the order of its sums; it
+ * only decides how many tiles the culling can clear (speed).  Off by default (every call sorts: its outputs are a fixed
+ * function of its inputs alone).  Errors: E_NULL.
+ */
+int genga_kick_set_order_reuse(genga_kick_ctx* ctx, int32_t on);
+
+/*
  * The same call with HOST arrays (same shapes; any alignment; vel and out_acc may be NULL as
  * above, out_pairs may be NULL): copies the inputs to library-owned device buffers, runs
  * genga_kick, copies the results back and synchronises the stream before returning.  At most

@@ -18,7 +18,7 @@ ORDER_AUTO, ORDER_CALLER, ORDER_SORTED = 0, 1, 2
 EXPORTS = (
     "genga_kick_make_plan", "genga_kick_make_plan_tp2", "genga_kick_make_plan_sym", "genga_kick_make_plan_tprows",
     "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of", "genga_kick_plan_sym_table", "genga_kick_plan_cta_range", "genga_kick_plan_iblock_ctas", "genga_kick_init",
-    "genga_kick_set_stream", "genga_kick", "genga_kick_list", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
+    "genga_kick_set_stream", "genga_kick", "genga_kick_set_order_reuse", "genga_kick_list", "genga_kick_host", "genga_kick_get_plan", "genga_kick_status",
     "genga_kick_launch_count", "genga_kick_free", "genga_kick_strerror", "genga_kick_last_cuda_error",
     "genga_kick_enable_timing", "genga_kick_last_pair_loop_ms",
 )
@@ -89,6 +89,7 @@ def lib():
         L.genga_kick_plan_iblock_ctas.argtypes = [C.POINTER(GengaKickPlan), i32, C.POINTER(i32), C.POINTER(i32)]
         L.genga_kick_init.argtypes = [C.POINTER(GengaKickConfig), C.POINTER(vp)]
         L.genga_kick_set_stream.argtypes = [vp, vp]
+        L.genga_kick_set_order_reuse.argtypes = [vp, i32]
         L.genga_kick.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, vp]
         L.genga_kick_list.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, i64, vp, vp, vp]
         L.genga_kick_host.argtypes = [vp, vp, vp, vp, vp, i32, d, vp, vp, vp]
@@ -236,6 +237,9 @@ class GengaKick:
         return (_ptr(pos, "f8", 3 * n, "pos", host), _ptr(vel, "f8", 3 * n, "vel", host), _ptr(mass, "f8", n, "mass", host),
                 _ptr(rcrit, "f8", rows * n, "rcrit", host), _ptr(out_acc, "f8", 3 * n, "out_acc", host),
                 _ptr(out_pairs, "i4", 2 * cap, "out_pairs", host), _ptr(out_npairs, "i4", n + 1, "out_npairs", host))
+
+    def set_order_reuse(self, on: bool):
+        self._check(lib().genga_kick_set_order_reuse(self._ctx, 1 if on else 0))
 
     def kick(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
         p, v, m, rc, a, op, on = self._kick_args(pos, vel, mass, rcrit, changeover_level, out_acc, out_pairs, out_npairs)

@@ -153,6 +153,13 @@ extern "C" int genga_kick_set_stream(genga_kick_ctx* ctx, void* cuda_stream)
     return GENGA_KICK_OK;
 }
 
+extern "C" int genga_kick_set_order_reuse(genga_kick_ctx* ctx, int32_t on)
+{
+    if (!ctx) return GENGA_KICK_E_NULL;
+    ctx->reuse_order = on != 0;
+    return GENGA_KICK_OK;
+}
+
 extern "C" int genga_kick(genga_kick_ctx* ctx, const double* pos, double* vel, const double* mass, const double* rcrit,
                           int32_t changeover_level, double dt, double* out_acc, int32_t* out_pairs, int32_t* out_npairs)
 {
@@ -199,7 +206,7 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
     const int n_rec = (int)pl.n_rec;
     cudaStream_t st = ctx->stream;
 
-    if (ctx->sorted) {
+    if (ctx->sorted && !(ctx->reuse_order && ctx->order_valid)) {
         // stable LSD radix sort of the 17-bit keys: digits of 8 and 9 bits
         const int nb = ctx->sort_blocks;
         genga::sort_init_kernel<<<1, 32, 0, st>>>(ctx->bbox);
@@ -215,6 +222,7 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
                                                                        nullptr, ctx->vals_a);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches += 8;
+        ctx->order_valid = true;
     }
     kp = genga::KickParams{};
     {

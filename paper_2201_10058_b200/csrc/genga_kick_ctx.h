@@ -28,6 +28,8 @@ struct genga_kick_ctx {
     float4* cbhi;
     // internal order (genga_kick_sort.cuh); sorted == false: caller's order
     bool sorted;
+    bool reuse_order;              // genga_kick_set_order_reuse: keep the permutation of the last sort
+    bool order_valid;              // ... there is one
     int sort_blocks;
     unsigned* bbox;
     unsigned* keys_a;

@@ -197,6 +197,28 @@ def test_error_codes():
     k.free()
 
 
+def test_order_reuse_across_levels(oracle_mod):
+    """genga_kick_set_order_reuse: the level-1 kick of a step keeps the internal order the level-0 kick sorted -- the
+    same positions, so the same order as a fresh sort and the same bits; on MOVED positions a kept order is still
+    correct (it only decides what the culling can clear)."""
+    from paper_2201_10058_b200 import GengaKick
+    ki = gi.make_config(3, n=9000, level=1)
+    fresh = run_gpu(ki, level=1, order_mode=2)
+    k = GengaKick(ki.n, 0, max_level=1, pair_capacity=1 << 20, G=ki.G, order_mode=2)
+    run_gpu(ki, level=0, kick=k)
+    k.set_order_reuse(True)
+    kept = run_gpu(ki, level=1, kick=k)
+    assert np.array_equal(kept.acc, fresh.acc) and np.array_equal(kept.counts, fresh.counts)
+    assert np.array_equal(sorted_pairs(kept.pairs), sorted_pairs(fresh.pairs)) and kept.launches < 2 * fresh.launches
+    moved = gi.make_config(3, n=9000, level=1)
+    moved.pos = moved.pos + 0.05 * np.sin(7.0 * moved.pos[::-1])            # ~0.05 AU away from where the order was taken
+    stale = run_gpu(moved, level=0, kick=k)
+    orc = oracle_mod.kick(moved.pos, moved.mass, moved.rcrit, moved.n, 0, level=0, G=moved.G)
+    assert stale.status == 0
+    compare(stale, orc, moved.n, tol=TOL)
+    k.free()
+
+
 def test_internal_order_is_invisible(oracle_mod):
     """Caller's order, sorted order and auto give the same pair set and counts; accelerations agree
     to the rounding of a different summation order."""
