@@ -283,293 +283,295 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             levels[str(level)]["what"] = ("neighbour search: W_L = 0 exactly beyond the level-0 critical radius, the pairs "
                                           "are culled by box tests, not evaluated (nominal figure, not work done)")
 
-    # the other BASELINE.json configs, each timed like the headline (L2 flushed before every kick, median of 7 after 3
-    # warm-ups): configs[0] (launch-bound: plain launches and a CUDA-graph replay), configs[1], configs[2] at both
-    # levels, configs[4] in both test-particle modes
-    def time_config(kin, level, tp_mode=1, mass_override=None, graph=False, reps=7):
-        nn = kin.n
-        kc = GengaKick(kin.n_massive, kin.n_test, max_level=level, pair_capacity=PAIR_CAPACITY, G=kin.G,
-                       enc_factor=kin.enc_factor, device=local_rank, tp_mode=tp_mode)
-        kc.set_stream(stream.cuda_stream)
-        kc.enable_timing(True)
-        cp, cm = to_dev(kin.pos), to_dev(kin.mass if mass_override is None else mass_override)
-        crc, cv = to_dev(kin.rcrit[:level + 1]), to_dev(kin.vel)
-        ca = torch.empty(3, nn, dtype=torch.float64, device=dev)
-        cnp = torch.empty(nn + 1, dtype=torch.int32, device=dev)
-        ts, loops = [], []
-        for it in range(reps + 3):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            flush.fill_(9)
-            l0 = kc.launch_count()
-            a.record(stream)
-            kc.kick(cp, cv, cm, crc, level, 0.5 * kin.dt, ca, pairs, cnp)
-            b.record(stream)
-            b.synchronize()
-            nl = kc.launch_count() - l0
-            if it >= 3:
-                ts.append(a.elapsed_time(b))
-                loops.append(kc.last_pair_loop_ms(level))
-        ms = float(np.median(ts))
-        ordered = kin.n_massive * (kin.n_massive - 1) + kin.n_test * kin.n_massive * (2 if tp_mode == 2 else 1)
-        out = {"n_massive": kin.n_massive, "n_test": kin.n_test, "level": level, "ms_per_kick": ms,
-               "pair_loop_ms": float(np.median(loops)), "launches": int(nl), "encounter_pairs": int(cnp[nn].item()),
-               "symmetric_pass": bool(kc.plan(0).symmetric) if level == 0 else False, "status": kc.status()}
-        if level == 0:
-            out["pairs_per_s"] = ordered / (ms * 1e-3)
-        else:
-            out["nominal_pairs_per_s"] = ordered / (ms * 1e-3)
-        if tp_mode == 2:
-            out["tp_mode"] = 2
-        if graph:
-            gs = torch.cuda.Stream()
-            torch.cuda.synchronize()
-            kc.set_stream(gs.cuda_stream)
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=gs):
+    configs_info = step_info = steps_info = group_info = list_info = hybrid_info = multilevel_info = bs_ring_info = None
+    if not args.headline_only:          # (--headline-only: the timed step alone, e.g. under ncu)
+        # the other BASELINE.json configs, each timed like the headline (L2 flushed before every kick, median of 7 after 3
+        # warm-ups): configs[0] (launch-bound: plain launches and a CUDA-graph replay), configs[1], configs[2] at both
+        # levels, configs[4] in both test-particle modes
+        def time_config(kin, level, tp_mode=1, mass_override=None, graph=False, reps=7):
+            nn = kin.n
+            kc = GengaKick(kin.n_massive, kin.n_test, max_level=level, pair_capacity=PAIR_CAPACITY, G=kin.G,
+                           enc_factor=kin.enc_factor, device=local_rank, tp_mode=tp_mode)
+            kc.set_stream(stream.cuda_stream)
+            kc.enable_timing(True)
+            cp, cm = to_dev(kin.pos), to_dev(kin.mass if mass_override is None else mass_override)
+            crc, cv = to_dev(kin.rcrit[:level + 1]), to_dev(kin.vel)
+            ca = torch.empty(3, nn, dtype=torch.float64, device=dev)
+            cnp = torch.empty(nn + 1, dtype=torch.int32, device=dev)
+            ts, loops = [], []
+            for it in range(reps + 3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                flush.fill_(9)
+                l0 = kc.launch_count()
+                a.record(stream)
                 kc.kick(cp, cv, cm, crc, level, 0.5 * kin.dt, ca, pairs, cnp)
-            gts = []
-            with torch.cuda.stream(gs):
-                for it in range(reps + 3):
-                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record(gs)
-                    g.replay()
-                    b.record(gs)
-                    b.synchronize()
-                    if it >= 3:
-                        gts.append(a.elapsed_time(b))
-            torch.cuda.synchronize()
-            out["ms_per_kick_cuda_graph"] = float(np.median(gts))
-            del g
-        kc.free()
-        return out
+                b.record(stream)
+                b.synchronize()
+                nl = kc.launch_count() - l0
+                if it >= 3:
+                    ts.append(a.elapsed_time(b))
+                    loops.append(kc.last_pair_loop_ms(level))
+            ms = float(np.median(ts))
+            ordered = kin.n_massive * (kin.n_massive - 1) + kin.n_test * kin.n_massive * (2 if tp_mode == 2 else 1)
+            out = {"n_massive": kin.n_massive, "n_test": kin.n_test, "level": level, "ms_per_kick": ms,
+                   "pair_loop_ms": float(np.median(loops)), "launches": int(nl), "encounter_pairs": int(cnp[nn].item()),
+                   "symmetric_pass": bool(kc.plan(0).symmetric) if level == 0 else False, "status": kc.status()}
+            if level == 0:
+                out["pairs_per_s"] = ordered / (ms * 1e-3)
+            else:
+                out["nominal_pairs_per_s"] = ordered / (ms * 1e-3)
+            if tp_mode == 2:
+                out["tp_mode"] = 2
+            if graph:
+                gs = torch.cuda.Stream()
+                torch.cuda.synchronize()
+                kc.set_stream(gs.cuda_stream)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=gs):
+                    kc.kick(cp, cv, cm, crc, level, 0.5 * kin.dt, ca, pairs, cnp)
+                gts = []
+                with torch.cuda.stream(gs):
+                    for it in range(reps + 3):
+                        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        a.record(gs)
+                        g.replay()
+                        b.record(gs)
+                        b.synchronize()
+                        if it >= 3:
+                            gts.append(a.elapsed_time(b))
+                torch.cuda.synchronize()
+                out["ms_per_kick_cuda_graph"] = float(np.median(gts))
+                del g
+            kc.free()
+            return out
 
-    k4 = gi.make_config(4)
-    m4 = k4.mass.copy()
-    m4[k4.n_massive:] = 1e-12 * (0.5 + gi.uniforms(77, 0, k4.n_test))       # TP 2: particles with mass
-    k2 = gi.make_config(2)
-    configs_info = {
-        "what": "one kick + pre-check (v += dt a, pair list, counts) per BASELINE.json config, L2 flushed before each; "
-                "pairs_per_s counts evaluated ordered pairs (level 0); level >= 1 kicks are neighbour searches (nominal)",
-        "configs[0] N=2048 L=0": time_config(gi.make_config(0), 0, graph=True),
-        "configs[1] N=8192 L=0": time_config(gi.make_config(1), 0),
-        "configs[2] N=32770 L=0": time_config(k2, 0),
-        "configs[2] N=32770 L=1": time_config(k2, 1),
-        "configs[4] 2048+1048576 tp, TP 1": time_config(k4, 0),
-        "configs[4] 2048+1048576 tp, TP 2": time_config(k4, 0, tp_mode=2, mass_override=m4),
-    }
+        k4 = gi.make_config(4)
+        m4 = k4.mass.copy()
+        m4[k4.n_massive:] = 1e-12 * (0.5 + gi.uniforms(77, 0, k4.n_test))       # TP 2: particles with mass
+        k2 = gi.make_config(2)
+        configs_info = {
+            "what": "one kick + pre-check (v += dt a, pair list, counts) per BASELINE.json config, L2 flushed before each; "
+                    "pairs_per_s counts evaluated ordered pairs (level 0); level >= 1 kicks are neighbour searches (nominal)",
+            "configs[0] N=2048 L=0": time_config(gi.make_config(0), 0, graph=True),
+            "configs[1] N=8192 L=0": time_config(gi.make_config(1), 0),
+            "configs[2] N=32770 L=0": time_config(k2, 0),
+            "configs[2] N=32770 L=1": time_config(k2, 1),
+            "configs[4] 2048+1048576 tp, TP 1": time_config(k4, 0),
+            "configs[4] 2048+1048576 tp, TP 2": time_config(k4, 0, tp_mode=2, mass_override=m4),
+        }
 
-    # NEXT-1: the whole App. A step without the Bulirsch-Stoer branch on the same disk --
-    # Rcrit, Kick(dt/2) + pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) -- and its O(N) part alone
-    sq, sv = pos.clone(), vel.clone()
-    rrow = torch.empty(n, dtype=torch.float64, device=dev)
-    step_ts, drift_ts = [], []
-    for it in range(8):
-        a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-        flush.fill_(5)
-        l0 = kick.launch_count()
-        a.record(stream)
-        kick.step(sq, sv, mass, 1.0, ki.dt, rrow, acc, pairs, npairs)
-        b.record(stream)
-        step_launches = kick.launch_count() - l0
-        kick.drift(sq, sv, mass, 1.0, ki.dt)
-        c.record(stream)
-        c.synchronize()
-        if it >= 3:
-            step_ts.append(a.elapsed_time(b))
-            drift_ts.append(b.elapsed_time(c))
-    step_info = {"what": "Rcrit, Kick(dt/2)+pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) at level 0 (genga_step)",
-                 "ms_per_step": float(np.median(step_ts)), "launches_per_step": int(step_launches),
-                 "drift_ms": float(np.median(drift_ts)), "drift_what": "HC(dt/2) FG(dt) HC(dt/2) alone, 3 launches, "
-                 "184 B/body of HBM traffic", "status": kick.status()}
-
-    # genga_steps: consecutive steps with the closing kick of a step and the opening kick of the next merged into one
-    # pass over the pairs (one all-pairs pass per step instead of two): 100 steps without the encounter branch, and
-    # 10 steps of the multi-level scheme (2 levels x 10 sub-steps), from the generated state
-    def time_steps(n_steps, slevels, substeps, reps=2):
-        kk = kick if slevels <= 1 + max(LEVELS) else None
-        st_buf = torch.zeros(max(slevels, 1), 4, dtype=torch.int32, device=dev)
-        ts = []
-        for it in range(reps + 1):
-            sq2, sv2 = pos.clone(), vel.clone()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            flush.fill_(4)
-            l0 = kk.launch_count()
+        # NEXT-1: the whole App. A step without the Bulirsch-Stoer branch on the same disk --
+        # Rcrit, Kick(dt/2) + pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) -- and its O(N) part alone
+        sq, sv = pos.clone(), vel.clone()
+        rrow = torch.empty(n, dtype=torch.float64, device=dev)
+        step_ts, drift_ts = [], []
+        for it in range(8):
+            a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            flush.fill_(5)
+            l0 = kick.launch_count()
             a.record(stream)
-            kk.steps(sq2, sv2, mass, 1.0, ki.dt, n_steps, slevels, substeps, 1e-12, acc, pairs, npairs, st_buf)
+            kick.step(sq, sv, mass, 1.0, ki.dt, rrow, acc, pairs, npairs)
+            b.record(stream)
+            step_launches = kick.launch_count() - l0
+            kick.drift(sq, sv, mass, 1.0, ki.dt)
+            c.record(stream)
+            c.synchronize()
+            if it >= 3:
+                step_ts.append(a.elapsed_time(b))
+                drift_ts.append(b.elapsed_time(c))
+        step_info = {"what": "Rcrit, Kick(dt/2)+pre-check, HC(dt/2), FG(dt), HC(dt/2), Kick(dt/2) at level 0 (genga_step)",
+                     "ms_per_step": float(np.median(step_ts)), "launches_per_step": int(step_launches),
+                     "drift_ms": float(np.median(drift_ts)), "drift_what": "HC(dt/2) FG(dt) HC(dt/2) alone, 3 launches, "
+                     "184 B/body of HBM traffic", "status": kick.status()}
+
+        # genga_steps: consecutive steps with the closing kick of a step and the opening kick of the next merged into one
+        # pass over the pairs (one all-pairs pass per step instead of two): 100 steps without the encounter branch, and
+        # 10 steps of the multi-level scheme (2 levels x 10 sub-steps), from the generated state
+        def time_steps(n_steps, slevels, substeps, reps=2):
+            kk = kick if slevels <= 1 + max(LEVELS) else None
+            st_buf = torch.zeros(max(slevels, 1), 4, dtype=torch.int32, device=dev)
+            ts = []
+            for it in range(reps + 1):
+                sq2, sv2 = pos.clone(), vel.clone()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                flush.fill_(4)
+                l0 = kk.launch_count()
+                a.record(stream)
+                kk.steps(sq2, sv2, mass, 1.0, ki.dt, n_steps, slevels, substeps, 1e-12, acc, pairs, npairs, st_buf)
+                b.record(stream)
+                b.synchronize()
+                nl = kk.launch_count() - l0
+                if it >= 1:
+                    ts.append(a.elapsed_time(b))
+            return {"n_steps": n_steps, "slevels": slevels, "substeps": substeps if slevels > 1 else None,
+                    "ms_per_step": float(np.median(ts)) / n_steps, "launches_per_step": nl / n_steps, "status": kk.status()}
+
+        steps_info = {"what": "genga_steps: n consecutive steps, merged kicks (slevels 0: Rcrit, Kick, HC, FG, HC, Kick without "
+                              "the encounter branch; 2 x 10: the multi-level step), ms per step",
+                      "runs": [time_steps(100, 0, 2), time_steps(10, 2, 10)]}
+
+        # NEXT-2: grouping of the level-0 pair list (499,679 pairs at N = 65,536) into close-encounter groups
+        kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
+        group_of = torch.empty(n, dtype=torch.int32, device=dev)
+        members = torch.empty(n, dtype=torch.int32, device=dev)
+        offsets = torch.empty(n + 1, dtype=torch.int32, device=dev)
+        summary = torch.empty(4, dtype=torch.int32, device=dev)
+        group_ts = []
+        for it in range(8):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            flush.fill_(6)
+            l0 = kick.launch_count()
+            a.record(stream)
+            kick.group(pairs, npairs[n:], PAIR_CAPACITY, group_of, members, offsets, summary)
             b.record(stream)
             b.synchronize()
-            nl = kk.launch_count() - l0
-            if it >= 1:
-                ts.append(a.elapsed_time(b))
-        return {"n_steps": n_steps, "slevels": slevels, "substeps": substeps if slevels > 1 else None,
-                "ms_per_step": float(np.median(ts)) / n_steps, "launches_per_step": nl / n_steps, "status": kk.status()}
+            group_launches = kick.launch_count() - l0
+            if it >= 3:
+                group_ts.append(a.elapsed_time(b))
+        sm = summary.cpu().tolist()
+        group_info = {"what": "genga_group on the level-0 pair list: connected components, members sorted by (group, body)",
+                      "ms": float(np.median(group_ts)), "launches": int(group_launches), "pairs": sm[3], "n_groups": sm[0],
+                      "n_members": sm[1], "largest_group": sm[2]}
 
-    steps_info = {"what": "genga_steps: n consecutive steps, merged kicks (slevels 0: Rcrit, Kick, HC, FG, HC, Kick without "
-                          "the encounter branch; 2 x 10: the multi-level step), ms per step",
-                  "runs": [time_steps(100, 0, 2), time_steps(10, 2, 10)]}
-
-    # NEXT-2: grouping of the level-0 pair list (499,679 pairs at N = 65,536) into close-encounter groups
-    kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
-    group_of = torch.empty(n, dtype=torch.int32, device=dev)
-    members = torch.empty(n, dtype=torch.int32, device=dev)
-    offsets = torch.empty(n + 1, dtype=torch.int32, device=dev)
-    summary = torch.empty(4, dtype=torch.int32, device=dev)
-    group_ts = []
-    for it in range(8):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        flush.fill_(6)
-        l0 = kick.launch_count()
-        a.record(stream)
-        kick.group(pairs, npairs[n:], PAIR_CAPACITY, group_of, members, offsets, summary)
-        b.record(stream)
-        b.synchronize()
-        group_launches = kick.launch_count() - l0
-        if it >= 3:
-            group_ts.append(a.elapsed_time(b))
-    sm = summary.cpu().tolist()
-    group_info = {"what": "genga_group on the level-0 pair list: connected components, members sorted by (group, body)",
-                  "ms": float(np.median(group_ts)), "launches": int(group_launches), "pairs": sm[3], "n_groups": sm[0],
-                  "n_members": sm[1], "largest_group": sm[2]}
-
-    # NEXT-4: KickS -- the level-1 kick over the level-0 pair list (genga_kick_list) instead of over all pairs
-    pairs1 = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev)
-    npairs1 = torch.empty(n + 1, dtype=torch.int32, device=dev)
-    kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
-    list_ts = []
-    for it in range(8):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        flush.fill_(7)
-        a.record(stream)
-        kick.kick_list(pos, sv, mass, rcrit, 1, 0.5 * ki.dt, pairs, npairs[n:], PAIR_CAPACITY, acc, pairs1, npairs1)
-        b.record(stream)
-        b.synchronize()
-        if it >= 3:
-            list_ts.append(a.elapsed_time(b))
-    list_info = {"what": "genga_kick_list: level-1 kick + pre-check over the level-0 encounter list (same result as the "
-                         "all-pairs level-1 kick, W_1 = 0 beyond rc0)", "ms": float(np.median(list_ts)),
-                 "listed_pairs": int(npairs[n].item()), "level1_pairs": int(npairs1[n].item())}
-
-    # NEXT-4: the complete hybrid step with the Bulirsch-Stoer branch, on BASELINE.json configs[1] (N = 8192; at
-    # N = 65,536 the level-0 pairs link into one group of 33,297 bodies -- the case the multi-level step below exists for)
-    k1 = gi.make_config(1)
-    n1 = k1.n
-    kick1 = GengaKick(n1, 0, max_level=0, pair_capacity=1 << 18, G=k1.G, device=local_rank)
-    kick1.set_stream(stream.cuda_stream)
-    hq, hv, hm = to_dev(k1.pos), to_dev(k1.vel), to_dev(k1.mass)
-    i32 = lambda m: torch.empty(m, dtype=torch.int32, device=dev)
-    hacc = torch.empty(3, n1, dtype=torch.float64, device=dev)
-    hpairs, hnp, hgo, hmem, hoff, hsum = torch.empty(1 << 18, 2, dtype=torch.int32, device=dev), i32(n1 + 1), i32(n1), \
-        i32(n1), i32(n1 + 1), i32(4)
-    hyb_ts = []
-    for it in range(10):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        l0 = kick1.launch_count()
-        a.record(stream)
-        kick1.hybrid_step(hq, hv, hm, 1.0, k1.dt, 1e-12, hacc, hpairs, hnp, hgo, hmem, hoff, hsum)
-        b.record(stream)
-        b.synchronize()
-        hyb_launches = kick1.launch_count() - l0
-        if it >= 3:
-            hyb_ts.append(a.elapsed_time(b))
-    hs = hsum.cpu().tolist()
-    hybrid_info = {"what": "genga_hybrid_step on configs[1] (N = 8192): Rcrit, Kick + pre-check, HC, FG, grouping, "
-                           "Bulirsch-Stoer (tol 1e-12), HC, Kick", "ms_per_step": float(np.median(hyb_ts)),
-                   "launches_per_step": int(hyb_launches), "groups": hs[0], "bodies_in_groups": hs[1],
-                   "largest_group": hs[2], "status": kick1.status()}
-    kick1.free()
-
-    # NEXT-4: the multi-level step (SEnc recursion, App. A) -- the experiment of Fig. 10
-    # (PAPER.md:640): the same disks, the hybrid step against 2-4 symplectic levels
-    def time_multilevel(kin, slevels, substeps, reps, graph=False):
-        nn = kin.n
-        km = GengaKick(nn, 0, max_level=slevels - 1, pair_capacity=PAIR_CAPACITY, G=kin.G, device=local_rank)
-        km.set_stream(stream.cuda_stream)
-        q0, v0, mm = to_dev(kin.pos), to_dev(kin.vel), to_dev(kin.mass)
-        q, v = q0.clone(), v0.clone()
-        macc = torch.empty(3, nn, dtype=torch.float64, device=dev)
-        mp, mnp = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev), i32(nn + 1)
-        mst = torch.zeros(slevels, 4, dtype=torch.int32, device=dev)
-        ts = []
-        for it in range(reps + 2):
-            q.copy_(q0); v.copy_(v0)
+        # NEXT-4: KickS -- the level-1 kick over the level-0 pair list (genga_kick_list) instead of over all pairs
+        pairs1 = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev)
+        npairs1 = torch.empty(n + 1, dtype=torch.int32, device=dev)
+        kick.kick(pos, None, mass, rcrit, 0, 0.5 * ki.dt, acc, pairs, npairs)
+        list_ts = []
+        for it in range(8):
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            l0 = km.launch_count()
+            flush.fill_(7)
             a.record(stream)
-            km.multilevel_step(q, v, mm, 1.0, kin.dt, slevels, substeps, 1e-12, macc, mp, mnp, mst, detect=True)
+            kick.kick_list(pos, sv, mass, rcrit, 1, 0.5 * ki.dt, pairs, npairs[n:], PAIR_CAPACITY, acc, pairs1, npairs1)
             b.record(stream)
             b.synchronize()
-            nl = km.launch_count() - l0
-            if it >= 2:
-                ts.append(a.elapsed_time(b))
-        st = mst.cpu().tolist()
-        # the same launch sequence captured once in a CUDA graph and replayed (no host launch cost, fixed sequence)
-        graph_ms = None
-        if graph:
-            gs = torch.cuda.Stream()                       # capture needs a non-default stream
-            q.copy_(q0); v.copy_(v0)
-            torch.cuda.synchronize()
-            km.set_stream(gs.cuda_stream)
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=gs):
-                km.multilevel_step(q, v, mm, 1.0, kin.dt, slevels, substeps, 1e-12, macc, mp, mnp, mst, detect=True)
-            gts = []
-            with torch.cuda.stream(gs):
-                for it in range(reps + 2):
-                    q.copy_(q0); v.copy_(v0)
-                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record(gs)
-                    g.replay()
-                    b.record(gs)
-                    b.synchronize()
-                    if it >= 2:
-                        gts.append(a.elapsed_time(b))
-            torch.cuda.synchronize()
+            if it >= 3:
+                list_ts.append(a.elapsed_time(b))
+        list_info = {"what": "genga_kick_list: level-1 kick + pre-check over the level-0 encounter list (same result as the "
+                             "all-pairs level-1 kick, W_1 = 0 beyond rc0)", "ms": float(np.median(list_ts)),
+                     "listed_pairs": int(npairs[n].item()), "level1_pairs": int(npairs1[n].item())}
+
+        # NEXT-4: the complete hybrid step with the Bulirsch-Stoer branch, on BASELINE.json configs[1] (N = 8192; at
+        # N = 65,536 the level-0 pairs link into one group of 33,297 bodies -- the case the multi-level step below exists for)
+        k1 = gi.make_config(1)
+        n1 = k1.n
+        kick1 = GengaKick(n1, 0, max_level=0, pair_capacity=1 << 18, G=k1.G, device=local_rank)
+        kick1.set_stream(stream.cuda_stream)
+        hq, hv, hm = to_dev(k1.pos), to_dev(k1.vel), to_dev(k1.mass)
+        i32 = lambda m: torch.empty(m, dtype=torch.int32, device=dev)
+        hacc = torch.empty(3, n1, dtype=torch.float64, device=dev)
+        hpairs, hnp, hgo, hmem, hoff, hsum = torch.empty(1 << 18, 2, dtype=torch.int32, device=dev), i32(n1 + 1), i32(n1), \
+            i32(n1), i32(n1 + 1), i32(4)
+        hyb_ts = []
+        for it in range(10):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = kick1.launch_count()
+            a.record(stream)
+            kick1.hybrid_step(hq, hv, hm, 1.0, k1.dt, 1e-12, hacc, hpairs, hnp, hgo, hmem, hoff, hsum)
+            b.record(stream)
+            b.synchronize()
+            hyb_launches = kick1.launch_count() - l0
+            if it >= 3:
+                hyb_ts.append(a.elapsed_time(b))
+        hs = hsum.cpu().tolist()
+        hybrid_info = {"what": "genga_hybrid_step on configs[1] (N = 8192): Rcrit, Kick + pre-check, HC, FG, grouping, "
+                               "Bulirsch-Stoer (tol 1e-12), HC, Kick", "ms_per_step": float(np.median(hyb_ts)),
+                       "launches_per_step": int(hyb_launches), "groups": hs[0], "bodies_in_groups": hs[1],
+                       "largest_group": hs[2], "status": kick1.status()}
+        kick1.free()
+
+        # NEXT-4: the multi-level step (SEnc recursion, App. A) -- the experiment of Fig. 10
+        # (PAPER.md:640): the same disks, the hybrid step against 2-4 symplectic levels
+        def time_multilevel(kin, slevels, substeps, reps, graph=False):
+            nn = kin.n
+            km = GengaKick(nn, 0, max_level=slevels - 1, pair_capacity=PAIR_CAPACITY, G=kin.G, device=local_rank)
             km.set_stream(stream.cuda_stream)
-            graph_ms = float(np.median(gts))
-            assert mst.cpu().tolist() == st, "the replayed graph took other decisions than the plain launches"
-            del g
-        out = {"slevels": slevels, "substeps": substeps, "ms_per_step": float(np.median(ts)), "launches_per_step": int(nl),
-               "ms_per_step_cuda_graph": graph_ms,
-               "encounter_pairs_per_level": [r[1] for r in st], "bs_groups": st[-1][2], "bs_bodies": st[-1][3],
-               "status": km.status()}
-        km.free()
-        return out
+            q0, v0, mm = to_dev(kin.pos), to_dev(kin.vel), to_dev(kin.mass)
+            q, v = q0.clone(), v0.clone()
+            macc = torch.empty(3, nn, dtype=torch.float64, device=dev)
+            mp, mnp = torch.empty(PAIR_CAPACITY, 2, dtype=torch.int32, device=dev), i32(nn + 1)
+            mst = torch.zeros(slevels, 4, dtype=torch.int32, device=dev)
+            ts = []
+            for it in range(reps + 2):
+                q.copy_(q0); v.copy_(v0)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                l0 = km.launch_count()
+                a.record(stream)
+                km.multilevel_step(q, v, mm, 1.0, kin.dt, slevels, substeps, 1e-12, macc, mp, mnp, mst, detect=True)
+                b.record(stream)
+                b.synchronize()
+                nl = km.launch_count() - l0
+                if it >= 2:
+                    ts.append(a.elapsed_time(b))
+            st = mst.cpu().tolist()
+            # the same launch sequence captured once in a CUDA graph and replayed (no host launch cost, fixed sequence)
+            graph_ms = None
+            if graph:
+                gs = torch.cuda.Stream()                       # capture needs a non-default stream
+                q.copy_(q0); v.copy_(v0)
+                torch.cuda.synchronize()
+                km.set_stream(gs.cuda_stream)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=gs):
+                    km.multilevel_step(q, v, mm, 1.0, kin.dt, slevels, substeps, 1e-12, macc, mp, mnp, mst, detect=True)
+                gts = []
+                with torch.cuda.stream(gs):
+                    for it in range(reps + 2):
+                        q.copy_(q0); v.copy_(v0)
+                        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        a.record(gs)
+                        g.replay()
+                        b.record(gs)
+                        b.synchronize()
+                        if it >= 2:
+                            gts.append(a.elapsed_time(b))
+                torch.cuda.synchronize()
+                km.set_stream(stream.cuda_stream)
+                graph_ms = float(np.median(gts))
+                assert mst.cpu().tolist() == st, "the replayed graph took other decisions than the plain launches"
+                del g
+            out = {"slevels": slevels, "substeps": substeps, "ms_per_step": float(np.median(ts)), "launches_per_step": int(nl),
+                   "ms_per_step_cuda_graph": graph_ms,
+                   "encounter_pairs_per_level": [r[1] for r in st], "bs_groups": st[-1][2], "bs_bodies": st[-1][3],
+                   "status": km.status()}
+            km.free()
+            return out
 
-    multilevel_info = {"what": "genga_multilevel_step (Rcrit, Kick + pre-check, HC, FG, detection, SEnc over KickS / RcritS / "
-                               "FGS / detection / grouping / Bulirsch-Stoer tol 1e-12, HC, Kick), one step from the "
-                               "generated state; 1 level = the hybrid step",
-                       "configs[1] N=8192": [time_multilevel(k1, sl, ss, 5, graph=(sl, ss) == (2, 2))
-                                             for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10))],
-                       "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3, graph=(sl, ss) == (2, 10))
-                                              for sl, ss in ((2, 10), (4, 2), (3, 4))]}
+        multilevel_info = {"what": "genga_multilevel_step (Rcrit, Kick + pre-check, HC, FG, detection, SEnc over KickS / RcritS / "
+                                   "FGS / detection / grouping / Bulirsch-Stoer tol 1e-12, HC, Kick), one step from the "
+                                   "generated state; 1 level = the hybrid step",
+                           "configs[1] N=8192": [time_multilevel(k1, sl, ss, 5, graph=(sl, ss) == (2, 2))
+                                                 for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10))],
+                           "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3, graph=(sl, ss) == (2, 10))
+                                                  for sl, ss in ((2, 10), (4, 2), (3, 4))]}
 
-    # NEXT-4: the Bulirsch-Stoer kernels alone on the ring of Fig. 7 (the experiment of Fig. 8): n bodies
-    # on a ring, 8 close-encounter partners each, one group, integrated over dt = 6 d at tol 1e-12
-    def time_bs_ring(nr, reps=3):
-        kr = gi.make_ring(nr)
-        kb = GengaKick(nr, 0, max_level=0, pair_capacity=8, G=kr.G, device=local_rank)
-        kb.set_stream(stream.cuda_stream)
-        q_in, v_in, mb, rcb = to_dev(kr.pos), to_dev(kr.vel), to_dev(kr.mass), to_dev(kr.rcrit)
-        mem = torch.arange(max(nr, 4), dtype=torch.int32, device=dev)
-        off = torch.zeros(nr + 4, dtype=torch.int32, device=dev); off[1] = nr
-        summ = torch.tensor([1, nr, nr, 0], dtype=torch.int32, device=dev)
-        q, v = q_in.clone(), v_in.clone()
-        ts = []
-        for it in range(reps + 1):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            kb.bs(q_in, v_in, mb, rcb, 1, 1.0, kr.dt, 1e-12, mem, off, summ, q, v)
-            b.record(stream)
-            b.synchronize()
-            if it >= 1:
-                ts.append(a.elapsed_time(b))
-        st = kb.status()
-        kb.free()
-        return {"n": nr, "ms": float(np.median(ts)), "status": st}
+        # NEXT-4: the Bulirsch-Stoer kernels alone on the ring of Fig. 7 (the experiment of Fig. 8): n bodies
+        # on a ring, 8 close-encounter partners each, one group, integrated over dt = 6 d at tol 1e-12
+        def time_bs_ring(nr, reps=3):
+            kr = gi.make_ring(nr)
+            kb = GengaKick(nr, 0, max_level=0, pair_capacity=8, G=kr.G, device=local_rank)
+            kb.set_stream(stream.cuda_stream)
+            q_in, v_in, mb, rcb = to_dev(kr.pos), to_dev(kr.vel), to_dev(kr.mass), to_dev(kr.rcrit)
+            mem = torch.arange(max(nr, 4), dtype=torch.int32, device=dev)
+            off = torch.zeros(nr + 4, dtype=torch.int32, device=dev); off[1] = nr
+            summ = torch.tensor([1, nr, nr, 0], dtype=torch.int32, device=dev)
+            q, v = q_in.clone(), v_in.clone()
+            ts = []
+            for it in range(reps + 1):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                kb.bs(q_in, v_in, mb, rcb, 1, 1.0, kr.dt, 1e-12, mem, off, summ, q, v)
+                b.record(stream)
+                b.synchronize()
+                if it >= 1:
+                    ts.append(a.elapsed_time(b))
+            st = kb.status()
+            kb.free()
+            return {"n": nr, "ms": float(np.median(ts)), "status": st}
 
-    bs_ring_info = {"what": "genga_bs on one ring group of n bodies with 8 partners each (Fig. 7 / Fig. 8), dt = 6 d, tol 1e-12 "
-                            "(regimes by group size: include/genga_bs.h)",
-                    "rings": [time_bs_ring(nr) for nr in (2, 8, 32, 64, 256, 512, 1024, 2048, 4096)]}
+        bs_ring_info = {"what": "genga_bs on one ring group of n bodies with 8 partners each (Fig. 7 / Fig. 8), dt = 6 d, tol 1e-12 "
+                                "(regimes by group size: include/genga_bs.h)",
+                        "rings": [time_bs_ring(nr) for nr in (2, 8, 32, 64, 256, 512, 1024, 2048, 4096)]}
 
     # end to end through the host entry point: pinned host arrays in, results back, every step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -703,6 +705,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--headline-only", action="store_true",
+                    help="time the headline step only (skip the per-config and NEXT-row timings): for profiler runs")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3                                  # timing rule: W >= 3
