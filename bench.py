@@ -55,10 +55,10 @@ FLOPS_PER_PAIR = 24
 SYM_FP64_INSTR_PER_UNORDERED_PAIR = 20
 SYM_FLOPS_PER_UNORDERED_PAIR = 31
 FP64_LANES_PER_SM = 64           # 148 SMs x 64 lanes x 2 flops x clocks.max.sm
-# From the ncu captures of round 2 (profiles/ncu_r02a.md), per launch / per two-level step at N = 65,536; constants
-# read off those captures, not measured in this run:
-NCU_DRAM_BYTES_PER_LAUNCH = None           # filled from profiles/ncu_r02a.md once captured
-NCU_EXECUTED_FLOPS_PER_STEP = None         # DADD + DMUL + 2 DFMA thread instructions of every kernel of one step
+# From the ncu captures of round 2 (profiles/ncu_r02a.md), per launch / per two-level step at N = 65,536 (rank 0's disk);
+# constants read off those captures, not measured in this run:
+NCU_DRAM_BYTES_PER_LAUNCH = 4204288        # kick_sym_kernel: dram__bytes_read.sum 2,497,536 + dram__bytes_write.sum 1,706,752
+NCU_EXECUTED_FLOPS_PER_STEP = 67817100000  # DADD + DMUL + 2 DFMA thread instructions of every kernel of one step (flops_r02a.csv)
 
 
 def workload(rank: int):

@@ -785,6 +785,10 @@ near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int 
         wfw = __float_as_int(wlo.w);
     }
     const bool active = wfw >= 0;                           // the group holds at least one real body
+    // Level >= 1 search, massive i-group against the massive j-groups: the trip rule is symmetric, so each unordered
+    // pair is queued ONCE, as a symmetric candidate (half the search, half the exact path's atomics).  The particles'
+    // groups and the fallback after an overflow keep ordered pairs.
+    const bool sym_i = !RESCAN && !force_only && j_group0 == 0 && ig < n_jgroups;
     CandCursor cc;
     cc.base = 0;
     cc.fill = GENGA_CAND_BLOCK;
@@ -803,7 +807,9 @@ near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int 
         if (!active) continue;
 #pragma unroll 1
         for (int q0 = 0; q0 < GENGA_NEAR_BOXES; q0 += 32) {
-            unsigned nearmask = __ballot_sync(0xffffffffu, boxes_near(wlo, whi, wfw, blo[q0 + lane], bhi[q0 + lane]));
+            // (massive i-group in the level >= 1 search: every unordered massive pair once -- only the j-groups from its own on)
+            const bool ahead = !sym_i || (g0 + q0 + lane) * js + jy >= ig;
+            unsigned nearmask = __ballot_sync(0xffffffffu, ahead && boxes_near(wlo, whi, wfw, blo[q0 + lane], bhi[q0 + lane]));
             while (nearmask) {
                 const int j0 = (j_group0 + (g0 + q0 + __ffs(nearmask) - 1) * js + jy) * GENGA_GROUP;
                 nearmask &= nearmask - 1;
@@ -817,6 +823,7 @@ near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int 
                     const double r2 = fma(dz, dz, fma(dy, dy, __dmul_rn(dx, dx)));
                     tm |= (__double2hiint(r2) < thr ? 1u : 0u) << u;
                 }
+                if (sym_i && j0 == ig * GENGA_GROUP) tm &= lane < 31 ? ~0u << (lane + 1) : 0u;   // own group: j-record > i-record
                 if (RESCAN) {
                     while (tm) {                            // per lane: its own tripped pairs, one after the other
                         const int jr = j0 + __ffs(tm) - 1;
@@ -834,7 +841,7 @@ near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int 
                     while (todo) {                          // warp-uniform: the j-records some lane tripped on
                         const int b = __ffs(todo) - 1;
                         todo &= todo - 1;
-                        push_candidates(p, cc, (tm >> b) & 1u, r, j0 + b);
+                        push_candidates(p, cc, (tm >> b) & 1u, sym_i ? ~r : r, j0 + b);      // (~i, j): both forces, once
                     }
                 }
             }
