@@ -18,8 +18,10 @@
  *          mu = G m_star (the Kepler part p^2/2m - G m m_star / r of eq. 2; the
  *          pair term [1 - K] of eq. 2 belongs to the Bulirsch-Stoer phase, off this path).
  *          The exact solution is written with Gauss' f and g functions in the difference dE of
- *          the eccentric anomaly ("FG", App. A).  Bound orbits only (a > 0);
- *          others are left untouched and reported                                 (reading G13)
+ *          the eccentric anomaly ("FG", App. A); a body on a hyperbolic orbit
+ *          (1/a < 0: ejected, or above the escape speed inside a deep passage) follows the same
+ *          two-body solution in the difference dH of the hyperbolic anomaly; only the parabolic
+ *          case 1/a = 0 exactly is left untouched and reported                    (reading G13)
  *   step   Rcrit(dt); Kick(dt/2) + pre-check; HC(dt/2); FG(dt); HC(dt/2); Kick(dt/2)
  *          App. A PAPER.md:986-992 without the Bulirsch-Stoer branch -- composed in Python
  *          (oracle/step.py) from these functions and genga_oracle_kick.
@@ -76,14 +78,57 @@ void genga_oracle_hc(int64_t N, double *pos, const double *vel, const double *ma
     }
 }
 
-/* The Kepler drift of one body, long double.  Returns 0, or 1 if the orbit is not bound. */
+/* The Kepler drift of one body, long double.  Returns 0, or 1 if the orbit is parabolic (left untouched). */
 static int kepler_step(long double mu, long double dt, long double q[3], long double v[3])
 {
     const long double r0 = sqrtl(q[0] * q[0] + q[1] * q[1] + q[2] * q[2]);
     const long double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
     const long double u = q[0] * v[0] + q[1] * v[1] + q[2] * v[2];
     const long double inv_a = 2.0L / r0 - v2 / mu;
-    if (!(inv_a > 0.0L)) return 1;
+    if (inv_a < 0.0L) {
+        /* hyperbolic: a' = -a > 0, n' = sqrt(mu / a'^3); Kepler's equation in the difference dH = H - H0:
+         *   F(dH) = ec sinh dH + es (cosh dH - 1) - dH - n' dt = 0,   ec = e cosh H0 = 1 + r0/a',  es = e sinh H0 = u / (n' a'^2)
+         * F' = ec cosh dH + es sinh dH - 1 = r/a' > 0: increasing.  Bracket by doubling, bisection, two Newton steps.
+         *   r = a' (ec cosh dH + es sinh dH - 1),  f = 1 - (a'/r0)(cosh dH - 1),  g = dt - (sinh dH - dH)/n',
+         *   f' = -(a'^2 n' / (r0 r)) sinh dH,      g' = 1 - (a'/r)(cosh dH - 1) */
+        const long double ap = -1.0L / inv_a;
+        const long double np_ = sqrtl(mu / (ap * ap * ap));
+        const long double ec = 1.0L + r0 / ap, es = u / (np_ * ap * ap), dN = np_ * dt;
+        long double lo = 0.0L, hi = 0.0L, w = 1.0L;
+        for (int it = 0; it < 64; it++) {
+            const long double x = dN > 0.0L ? w : -w;
+            const long double fn = ec * sinhl(x) + es * (coshl(x) - 1.0L) - x - dN;
+            if (dN > 0.0L ? fn >= 0.0L : fn <= 0.0L) { if (dN > 0.0L) hi = x; else lo = x; break; }
+            if (dN > 0.0L) lo = x; else hi = x;
+            w *= 2.0L;
+        }
+        long double dH = 0.5L * (lo + hi);
+        for (int it = 0; it < 200; it++) {
+            dH = 0.5L * (lo + hi);
+            if (!(dH > lo && dH < hi)) break;
+            const long double fn = ec * sinhl(dH) + es * (coshl(dH) - 1.0L) - dH - dN;
+            if (fn > 0.0L) hi = dH; else lo = dH;
+        }
+        for (int it = 0; it < 2; it++) {
+            const long double sh = sinhl(dH), ch = coshl(dH);
+            const long double nx = dH - (ec * sh + es * (ch - 1.0L) - dH - dN) / (ec * ch + es * sh - 1.0L);
+            if (nx >= lo && nx <= hi) dH = nx;
+        }
+        const long double sh = sinhl(dH), ch = coshl(dH);
+        const long double r = ap * (ec * ch + es * sh - 1.0L);
+        const long double f = 1.0L - (ap / r0) * (ch - 1.0L);
+        const long double g = dt - (sh - dH) / np_;
+        const long double fd = -(ap * ap * np_ / (r0 * r)) * sh;
+        const long double gd = 1.0L - (ap / r) * (ch - 1.0L);
+        for (int k = 0; k < 3; k++) {
+            const long double qk = f * q[k] + g * v[k];
+            const long double vk = fd * q[k] + gd * v[k];
+            q[k] = qk;
+            v[k] = vk;
+        }
+        return 0;
+    }
+    if (!(inv_a > 0.0L)) return 1;                                     /* parabolic (or not a number) */
     const long double a = 1.0L / inv_a;
     const long double n = sqrtl(mu / (a * a * a));                     /* mean motion */
     const long double ec = 1.0L - r0 / a;                              /* e cos E0 */
@@ -124,8 +169,8 @@ static int kepler_step(long double mu, long double dt, long double q[3], long do
     return 0;
 }
 
-/* FG(dt) for all bodies, in place.  Returns the number of bodies that are not on a bound orbit
- * (left untouched). */
+/* FG(dt) for all bodies, in place.  Returns the number of bodies on a parabolic orbit (1/a = 0
+ * exactly: left untouched). */
 int64_t genga_oracle_fg(int64_t N, double *pos, double *vel, double mu, double dt)
 {
     int64_t unbound = 0;

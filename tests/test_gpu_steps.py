@@ -142,6 +142,26 @@ def test_merged_steps_with_encounters(oracle_mod, slevels, substeps, detect, n_s
     k.free()
 
 
+def test_rcrit_jump_is_reported():
+    """The merged kick builds its candidate list for critical radii up to 1 + 1/64 times those of the step that ends.
+    Two heavy bodies (1e-2 solar masses, Hill-dominated critical radii) 0.7 AU apart and a 60-day step: the closing
+    kick changes a semi-major axis, hence a Hill radius, by 2 % -- the next step's radius is outside that allowance and
+    the status word says so (the caller repeats those steps with genga_step).  The disks above never raise it."""
+    import torch
+    import paper_2201_10058_b200 as g
+    pos = np.array([[1.0, 1.0], [0.0, 0.7], [0.0, 0.0]])
+    r = np.sqrt((pos ** 2).sum(0)); vc = np.sqrt(G / r)
+    vel = np.stack([-pos[1] / r * vc, pos[0] / r * vc, np.zeros(2)])
+    k = g.GengaKick(2, 0, max_level=0, pair_capacity=16, G=G)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, v = _dev(pos), _dev(vel)
+    k.steps(q, v, _dev(np.array([1e-2, 1e-2])), 1.0, 60.0, 2, 0, 2, 1e-12, None, torch.empty(16, 2, dtype=torch.int32, device="cuda"),
+            torch.empty(3, dtype=torch.int32, device="cuda"), None)
+    torch.cuda.synchronize()
+    assert k.status() & g.binding.STATUS_RCRIT_JUMP
+    k.free()
+
+
 def test_steps_error_codes_and_graph_capture():
     import torch
     import paper_2201_10058_b200 as g

@@ -151,10 +151,40 @@ def test_fg_invariants_period_and_inverse(st):
     assert np.max(np.abs(qb - pos)) < 1e-14 * a.max() and np.max(np.abs(vb - vel)) < 1e-14 * np.abs(vel).max() * 4
 
 
-def test_fg_unbound_is_reported_and_untouched(st):
-    pos = np.array([[1.0, 1.0], [0.0, 0.0], [0.0, 0.0]])
-    vel = np.array([[0.0, 0.0], [np.sqrt(G), 2.0 * np.sqrt(G)], [0.0, 0.0]])       # circular, hyperbolic
-    q, v, bad = st.fg(pos, vel, G, 6.0)
+def test_fg_hyperbolic_orbits(st):
+    """A body above the escape speed follows the hyperbolic two-body solution (it used to be left in place): pinned by
+    an independent integration of the two-body problem (scipy DOP853, rtol 1e-13), by the conserved energy, angular
+    momentum and eccentricity vector, and by dt followed by -dt."""
+    from scipy.integrate import solve_ivp
+    rng = np.random.default_rng(5)
+    n = 12
+    pos = rng.normal(size=(3, n)); pos *= rng.uniform(0.3, 3.0, n) / np.sqrt((pos ** 2).sum(0))
+    r = np.sqrt((pos ** 2).sum(0))
+    vdir = rng.normal(size=(3, n)); vdir /= np.sqrt((vdir ** 2).sum(0))
+    vel = vdir * np.sqrt(2.0 * G / r) * rng.uniform(1.05, 4.0, n)              # 1.05 .. 4 escape speeds, any direction
+    for dt in (6.0, -40.0, 300.0):
+        q, v, bad = st.fg(pos, vel, G, dt)
+        assert bad == 0 and np.isfinite(q).all()
+        for i in range(n):
+            sol = solve_ivp(lambda t, y: np.concatenate([y[3:], -G * y[:3] / np.sqrt((y[:3] ** 2).sum()) ** 3]), (0.0, dt),
+                            np.concatenate([pos[:, i], vel[:, i]]), method="DOP853", rtol=1e-13, atol=1e-16)
+            sc_q, sc_v = np.sqrt((sol.y[:3, -1] ** 2).sum()), np.sqrt((sol.y[3:, -1] ** 2).sum())
+            assert np.abs(q[:, i] - sol.y[:3, -1]).max() < 2e-10 * sc_q and np.abs(v[:, i] - sol.y[3:, -1]).max() < 2e-10 * sc_v
+        en0 = 0.5 * (vel ** 2).sum(0) - G / r; en1 = 0.5 * (v ** 2).sum(0) - G / np.sqrt((q ** 2).sum(0))
+        assert np.all(en0 > 0) and np.max(np.abs(en1 / en0 - 1)) < 1e-13
+        h0, h1 = np.cross(pos.T, vel.T), np.cross(q.T, v.T)
+        assert np.max(np.abs(h1 - h0)) < 1e-14 * np.abs(h0).max()
+        e0 = np.cross(vel.T, h0) / G - (pos / r).T; e1 = np.cross(v.T, h1) / G - (q / np.sqrt((q ** 2).sum(0))).T
+        assert np.max(np.abs(e1 - e0)) < 1e-12 * np.abs(e0).max() and np.all(np.sqrt((e0 ** 2).sum(1)) > 1.0)
+        qb, vb, _ = st.fg(q, v, G, -dt)
+        assert np.max(np.abs(qb - pos)) < 1e-12 * np.abs(q).max() and np.max(np.abs(vb - vel)) < 1e-12 * np.abs(vel).max()
+
+
+def test_fg_parabolic_is_reported_and_untouched(st):
+    pos = np.array([[1.0, 2.0], [0.0, 0.0], [0.0, 0.0]])
+    vel = np.array([[0.0, 0.0], [0.25, 0.25], [0.0, 0.0]])
+    mu = 0.0625                                   # body 1: v^2 = 1/16 = 2 mu / r exactly (all dyadic): 1/a = 0; body 0: circular
+    q, v, bad = st.fg(pos, vel, mu, 6.0)
     assert bad == 1
     assert np.array_equal(q[:, 1], pos[:, 1]) and np.array_equal(v[:, 1], vel[:, 1])
     assert not np.array_equal(q[:, 0], pos[:, 0])
