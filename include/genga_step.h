@@ -28,9 +28,10 @@
 extern "C" {
 #endif
 
-#define GENGA_KICK_STATUS_UNBOUND 8   /* Rcrit / FG met a body that is not on a bound orbit about the
-                                         central mass (1/a = 2/r - v^2/mu <= 0): its Hill term is taken
-                                         as 0 and FG leaves it where it is                              */
+#define GENGA_KICK_STATUS_UNBOUND 8   /* Rcrit met a body that is not on a bound orbit about the central mass
+                                         (1/a = 2/r - v^2/mu <= 0): its Hill term is taken as 0.  FG sets the
+                                         bit only for 1/a = 0 exactly (parabolic; the body is left where it is):
+                                         a hyperbolic body follows its two-body orbit like any other          */
 
 /*
  * Rcrit: the critical radii of eq. 5, one row per symplectic level (PAPER.md:638:
@@ -73,7 +74,8 @@ int genga_hc(genga_kick_ctx* ctx, double* pos, const double* vel, const double* 
 /*
  * FG: the Kepler part of eq. 2: every body advances by dt on its two-body orbit
  * about the central mass, mu = G m_star, with Gauss' f and g functions; pos and vel in place.
- * Bound orbits only: a body with 1/a <= 0 is left untouched and GENGA_KICK_STATUS_UNBOUND is set.
+ * Elliptic and hyperbolic orbits alike; only a body with 1/a = 0 exactly (parabolic) is left untouched and
+ * GENGA_KICK_STATUS_UNBOUND is set.
  * (The pair term [1 - K] of eq. 2 belongs to the Bulirsch-Stoer phase and is not applied here.)
  * Errors: E_NULL, E_ALIGN, E_SIZE (m_star <= 0), E_CUDA.
  */

@@ -152,7 +152,11 @@ shift_kernel(double* __restrict__ pos, long long N, const double* __restrict__ p
 // has F' = r/a > 0: F is increasing and |F(dE) - (dE - dM)| <= |ec| + 2 |es|, so the root lies in
 // dM +- (|ec| + 2 |es|); Newton from dE = dM, any step that leaves the bracket replaced by its
 // midpoint (bisection), which converges for every bound orbit.
-// Returns false (state untouched) if the orbit is not bound.
+// A hyperbolic orbit (1/a < 0: an ejected body, or one above the escape speed inside a deep passage) takes the same
+// two-body solution in the difference dH of the hyperbolic anomaly, with a' = -a, n' = sqrt(mu / a'^3):
+//     F(dH) = ec sinh dH + es (cosh dH - 1) - dH - n' dt = 0,   ec = 1 + r0/a',  es = u / (n' a'^2),   F' = r/a' > 0,
+// bracketed by doubling from 0, then the same safeguarded Newton iteration.
+// Returns false (state untouched) only for 1/a = 0 exactly (parabolic) or a state that is not a number.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ bool kepler_fg(double mu, double dt, double& x, double& y, double& z,
                                           double& vx, double& vy, double& vz)
@@ -161,6 +165,41 @@ __device__ __forceinline__ bool kepler_fg(double mu, double dt, double& x, doubl
     const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
     const double u = fma(z, vz, fma(y, vy, x * vx));
     const double inv_a = 2.0 / r0 - v2 / mu;
+    if (inv_a < 0.0) {
+        const double ap = -1.0 / inv_a;
+        const double np_ = sqrt(-mu * inv_a) * -inv_a;       // sqrt(mu / a'^3)
+        const double ec = 1.0 + r0 / ap, es = u / (np_ * ap * ap), dN = np_ * dt;
+        double lo = 0.0, hi = 0.0, w = 1.0;
+        for (int it = 0; it < 64; it++) {                    // F is increasing and F(0) = -dN: the root lies beyond 0 on dN's side
+            const double xw = dN > 0.0 ? w : -w;
+            const double fn = ec * sinh(xw) + es * (cosh(xw) - 1.0) - xw - dN;
+            if (dN > 0.0 ? fn >= 0.0 : fn <= 0.0) { if (dN > 0.0) hi = xw; else lo = xw; break; }
+            if (dN > 0.0) lo = xw; else hi = xw;
+            w *= 2.0;
+        }
+        double dH = 0.5 * (lo + hi), sh, ch;
+        for (int it = 0; it < 80; it++) {
+            sh = sinh(dH); ch = cosh(dH);
+            const double fn = ec * sh + es * (ch - 1.0) - dH - dN;
+            const double fp = ec * ch + es * sh - 1.0;
+            if (fn > 0.0) hi = dH; else lo = dH;
+            double nx = dH - fn / fp;
+            if (!(nx > lo && nx < hi)) nx = 0.5 * (lo + hi);
+            const double step = nx - dH;
+            dH = nx;
+            if (fabs(step) <= 4.0e-16 * (1.0 + fabs(dH))) break;
+        }
+        sh = sinh(dH); ch = cosh(dH);
+        const double r = ap * (ec * ch + es * sh - 1.0);
+        const double f = 1.0 - (ap / r0) * (ch - 1.0);
+        const double g = dt - (sh - dH) / np_;
+        const double fd = -(ap * ap * np_ / (r0 * r)) * sh;
+        const double gd = 1.0 - (ap / r) * (ch - 1.0);
+        const double nx = f * x + g * vx, ny = f * y + g * vy, nz = f * z + g * vz;
+        const double nvx = fd * x + gd * vx, nvy = fd * y + gd * vy, nvz = fd * z + gd * vz;
+        x = nx; y = ny; z = nz; vx = nvx; vy = nvy; vz = nvz;
+        return true;
+    }
     if (!(inv_a > 0.0)) return false;
     const double a = 1.0 / inv_a;
     const double n = sqrt(mu * inv_a) * inv_a;               // mean motion sqrt(mu / a^3)

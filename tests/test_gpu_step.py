@@ -105,24 +105,30 @@ def test_fg_eccentric_orbits_and_long_steps(oracle_mod):
     k.free()
 
 
-def test_unbound_body_is_reported_and_left_in_place(oracle_mod):
+def test_hyperbolic_bodies_drift_and_rcrit_reports_them(oracle_mod):
+    """Bodies above the escape speed follow their hyperbolic two-body orbit in FG (same bound as the elliptic ones);
+    Rcrit has no Hill radius for them and says so."""
     import torch
     import paper_2201_10058_b200 as g
     ki = gi.make_config(0, n=300)
     ki.vel[:, 17] *= 3.0                                     # hyperbolic
+    ki.vel[:, 40] *= -1.6
+    ki.vel[:, 41] = 1.5 * ki.vel[:, 41] + 1.5 * np.sqrt(G / (ki.pos[:, 41] ** 2).sum()) * ki.pos[:, 41]     # outwards at 45 degrees
     k = _ctx(ki)
+    for dt in (ki.dt, -50.0):
+        q, v = _dev(ki.pos), _dev(ki.vel)
+        k.fg(q, v, 1.0, dt)
+        assert k.status() == 0
+        qw, vw, bad = oracle_mod.step.fg(ki.pos, ki.vel, ki.G, dt)
+        assert bad == 0 and np.abs(qw[:, 17] - ki.pos[:, 17]).max() > 0.1
+        sq, sv = _scales(ki.pos, ki.vel, dt)
+        assert np.all(np.abs(q.cpu().numpy() - qw) <= 32 * U * sq) and np.all(np.abs(v.cpu().numpy() - vw) <= 32 * U * sv)
     q, v = _dev(ki.pos), _dev(ki.vel)
-    k.fg(q, v, 1.0, ki.dt)
-    assert k.status() & g.STATUS_UNBOUND
-    qw, vw, bad = oracle_mod.step.fg(ki.pos, ki.vel, ki.G, ki.dt)
-    assert bad == 1
-    assert np.array_equal(q.cpu().numpy()[:, 17], ki.pos[:, 17]) and np.array_equal(v.cpu().numpy()[:, 17], ki.vel[:, 17])
-    sq, sv = _scales(ki.pos, ki.vel, ki.dt)
-    assert np.all(np.abs(q.cpu().numpy() - qw) <= 32 * U * sq)
     rc = torch.empty(1, ki.n, dtype=torch.float64, device="cuda")
     k.rcrit(_dev(ki.pos), _dev(ki.vel), _dev(ki.mass), 1.0, ki.dt, rc)
     want, bad = oracle_mod.step.rcrit(ki.pos, ki.vel, ki.mass, 1.0, ki.G, ki.dt)
-    assert bad == 1 and np.all(np.abs(rc.cpu().numpy() - want) <= 16 * U * want)
+    assert bad == 3 and np.all(np.abs(rc.cpu().numpy() - want) <= 16 * U * want)
+    assert k.status() == g.STATUS_UNBOUND
     k.free()
 
 
