@@ -543,7 +543,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                            "configs[1] N=8192": [time_multilevel(k1, sl, ss, 5, graph=(sl, ss) == (2, 2))
                                                  for sl, ss in ((1, 2), (2, 2), (3, 2), (2, 10))],
                            "configs[3] N=65536": [time_multilevel(ki, sl, ss, 3, graph=(sl, ss) == (2, 10))
-                                                  for sl, ss in ((2, 10), (4, 2), (3, 4))]}
+                                                  for sl, ss in ((2, 10), (4, 2), (3, 4), (3, 2), (2, 2))]}
 
         # NEXT-4: the Bulirsch-Stoer kernels alone on the ring of Fig. 7 (the experiment of Fig. 8): n bodies
         # on a ring, 8 close-encounter partners each, one group, integrated over dt = 6 d at tol 1e-12
