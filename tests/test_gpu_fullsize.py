@@ -145,6 +145,38 @@ def test_symmetric_pass_candidate_list_overflow(oracle_mod):
     compare(gpu, orc, ki.n, tol=TOL)
 
 
+def test_symmetric_pass_edge_cases(oracle_mod):
+    """The symmetric pass with a widened and a narrowed pre-check net (enc_factor), with a pair list too small for the
+    pairs found (true total kept, rows clipped, never out of bounds), with coincident bodies (skipped and flagged, in a
+    symmetric tile and in a diagonal one), with the level-1 kick on top (symmetric candidates of the neighbour search),
+    and through the host entry point."""
+    ki = gi.make_config(3, n=25000, level=1)
+    for f in (1.6, 0.5):
+        ki.enc_factor = f
+        for level in (0, 1):
+            gpu = run_gpu(ki, level=level, capacity=CAPACITY, order_mode=0)
+            orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n, 0, level=level, G=ki.G, enc_factor=f, maxp=512)
+            assert gpu.status == 0
+            compare(gpu, orc, ki.n, tol=TOL)
+    ki.enc_factor = 1.0
+    full = run_gpu(ki, level=0, capacity=CAPACITY, order_mode=0)
+    small = run_gpu(ki, level=0, capacity=100, order_mode=0)
+    assert small.total == full.total > 100 and len(small.pairs) == 100 and np.array_equal(small.counts, full.counts)
+    allp = {tuple(p) for p in full.pairs.tolist()}
+    assert all(tuple(p) in allp for p in small.pairs.tolist()) and np.array_equal(small.acc, full.acc)
+    host = run_gpu(ki, level=0, capacity=CAPACITY, order_mode=0, host=True)
+    assert np.array_equal(host.acc, full.acc) and host.total == full.total
+    ki.pos = ki.pos.copy()
+    ki.pos[:, 20000] = ki.pos[:, 7]                          # far apart in the caller's order: a symmetric tile or a diagonal one,
+    ki.pos[:, 8] = ki.pos[:, 9]                              # wherever the internal order puts them
+    gpu = run_gpu(ki, level=0, capacity=CAPACITY, order_mode=0)
+    assert gpu.status & 1 and np.isfinite(gpu.acc).all()
+    orc = oracle_mod.kick(ki.pos, ki.mass, ki.rcrit, ki.n, 0, level=0, G=ki.G, maxp=512)
+    assert orc.coincident
+    gpu.status = 0
+    compare(gpu, orc, ki.n, tol=TOL)
+
+
 def test_symmetric_pass_is_bit_reproducible():
     ki = gi.make_config(3, n=33000, level=0)
     a = run_gpu(ki, level=0, capacity=CAPACITY, with_vel=True)
