@@ -115,10 +115,9 @@ struct BsShared {
 template <int ROWS>
 __device__ __forceinline__ void bs_gsync(BsShared<ROWS>& S, const BsGlobal& Gm)
 {
-    if (Gm.team_ctas == 0) {
-        cooperative_groups::this_grid().sync();
-        return;
-    }
+    // (the whole grid is one team of gridDim.x CTAs.  The poll is a RELAXED load followed by one fence: an acquire load,
+    // like the one in cooperative groups' grid barrier, invalidates the SM's L1 on every iteration -- and with it the
+    // extrapolation tableaus, in local memory, of the CTAs that are still working)
     __syncthreads();
     if (threadIdx.x == 0) {
         S.bar_target += (unsigned long long)Gm.team_ctas;
@@ -126,7 +125,7 @@ __device__ __forceinline__ void bs_gsync(BsShared<ROWS>& S, const BsGlobal& Gm)
         atomicAdd(Gm.bar, 1ULL);
         unsigned long long seen;
         do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(Gm.bar) : "memory");
+            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(Gm.bar) : "memory");
         } while (seen < S.bar_target);
         __threadfence();
     }
@@ -576,6 +575,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
     if (COOP) {
         if (team >= n_teams) return;                                    // CTAs beyond the last whole team
         Gm.tb = (int)blockIdx.x - team * tctas;
+        Gm.team_ctas = tctas;
         const long long off = (long long)team * tctas * THREADS / SUB;
 #pragma unroll
         for (int h = 0; h < 2; h++) { Gm.x[h] += off; Gm.y[h] += off; Gm.z[h] += off; Gm.pk[h] += 2 * off; }
