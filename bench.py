@@ -215,7 +215,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     def step():
         # (the level-1 kick acts on the positions the level-0 kick has just sorted: it keeps that internal order)
         for level in LEVELS:
-            kick.set_order_reuse(level > 0)
+            kick.set_order_reuse(2 if level > 0 else 0)
             kick.kick(pos, vel, mass, rcrit, level, 0.5 * ki.dt, acc, pairs, npairs)
         kick.set_order_reuse(False)
 
@@ -585,7 +585,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
 
     def host_step():
         for level in LEVELS:
-            kick.set_order_reuse(level > 0)
+            kick.set_order_reuse(2 if level > 0 else 0)
             kick.kick_host(h_pos, h_vel, h_mass, h_rc, level, 0.5 * ki.dt, h_acc, h_pairs, h_np)
         kick.set_order_reuse(False)
 

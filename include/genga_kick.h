@@ -165,12 +165,26 @@ int genga_kick(genga_kick_ctx* ctx,
                double* out_acc, int32_t* out_pairs, int32_t* out_npairs);
 
 /*
- * While `on` is non-zero, genga_kick keeps the internal body order of the last call that sorted instead of sorting
- * again: for consecutive calls on unchanged or little-changed positions, e.g. the kicks of several changeover levels
- * of one step.  The internal order is never visible and never changes a result beyond the order of its sums; it
- * only decides how many tiles the culling can clear (speed).  Off by default (every call sorts: its outputs are a fixed
- * function of its inputs alone).  Errors: E_NULL.
+ * What a call may keep from the calls before it (the kicks of several changeover levels of one step act on the same
+ * positions; sec. 7.1, eq. 62-63):
+ *   on = GENGA_KICK_REUSE_OFF   (default) every call sorts and searches: its outputs are a fixed function of its inputs alone.
+ *   on = GENGA_KICK_REUSE_ORDER genga_kick keeps the internal body order of the last call that sorted instead of sorting
+ *        again: for consecutive calls on unchanged or little-changed positions.  The internal order is never visible
+ *        and never changes a result beyond the order of its sums; it only decides how many tiles the culling can clear.
+ *   on = GENGA_KICK_REUSE_LIST  as GENGA_KICK_REUSE_ORDER, and the caller states that `pos` of every level >= 1 call made
+ *        under this setting is BIT-IDENTICAL to `pos` of the last level-0 call on this context: such a kick also skips
+ *        its neighbour search and evaluates the list of near pairs the level-0 kick has left (the pairs inside
+ *        max(rc0, f rc0) of either body: a superset of the pairs inside max(rc0, f rcL), outside of which W_L = 0 and
+ *        there is no encounter, as long as no body's filter radius at level L exceeds its level-0 one -- checked per
+ *        body on the device; if one does, or if no level-0 list is at hand, that kick searches all pairs itself).
+ *        Results are those of GENGA_KICK_REUSE_ORDER bit for bit (the near terms are summed exactly; the order of the
+ *        rows of out_pairs is arbitrary in every mode).  Changed positions under this setting give wrong results
+ *        without a status bit: the library cannot see it.
+ * Errors: E_NULL, E_SIZE (on outside 0..2).
  */
+#define GENGA_KICK_REUSE_OFF 0
+#define GENGA_KICK_REUSE_ORDER 1
+#define GENGA_KICK_REUSE_LIST 2
 int genga_kick_set_order_reuse(genga_kick_ctx* ctx, int32_t on);
 
 /*

@@ -34,6 +34,7 @@ STATUS_UNBOUND = 8
 # include/genga_senc.h: close-encounter detection and the multi-level step (SEnc)
 SENC_EXPORTS = ("genga_detect", "genga_multilevel_step", "genga_steps")
 STATUS_RCRIT_JUMP = 256
+REUSE_OFF, REUSE_ORDER, REUSE_LIST = 0, 1, 2
 STATUS_LIST_CLIPPED = 128
 
 
@@ -238,8 +239,9 @@ class GengaKick:
                 _ptr(rcrit, "f8", rows * n, "rcrit", host), _ptr(out_acc, "f8", 3 * n, "out_acc", host),
                 _ptr(out_pairs, "i4", 2 * cap, "out_pairs", host), _ptr(out_npairs, "i4", n + 1, "out_npairs", host))
 
-    def set_order_reuse(self, on: bool):
-        self._check(lib().genga_kick_set_order_reuse(self._ctx, 1 if on else 0))
+    def set_order_reuse(self, on):
+        """0 / False: off; 1 / True: keep the internal order (REUSE_ORDER); 2: also the level-0 list of near pairs (REUSE_LIST)"""
+        self._check(lib().genga_kick_set_order_reuse(self._ctx, int(on)))
 
     def kick(self, pos, vel, mass, rcrit, changeover_level, dt, out_acc, out_pairs, out_npairs):
         p, v, m, rc, a, op, on = self._kick_args(pos, vel, mass, rcrit, changeover_level, out_acc, out_pairs, out_npairs)

@@ -84,6 +84,9 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
         if ((e = cudaMalloc(&ctx->rxy, (size_t)nr * sizeof(double2))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->rzm, (size_t)nr * sizeof(double2))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->rfw, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->rfw_ref, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMalloc(&ctx->need_near, ((size_t)cfg->max_level + 1) * sizeof(int))) != cudaSuccess) goto cuda_error;
+        if ((e = cudaMemset(ctx->need_near, 0, ((size_t)cfg->max_level + 1) * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->ridx, (size_t)nr * sizeof(int))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->cblo, (size_t)(nr / GENGA_GROUP) * sizeof(float4))) != cudaSuccess) goto cuda_error;
         if ((e = cudaMalloc(&ctx->cbhi, (size_t)(nr / GENGA_GROUP) * sizeof(float4))) != cudaSuccess) goto cuda_error;
@@ -156,7 +159,9 @@ extern "C" int genga_kick_set_stream(genga_kick_ctx* ctx, void* cuda_stream)
 extern "C" int genga_kick_set_order_reuse(genga_kick_ctx* ctx, int32_t on)
 {
     if (!ctx) return GENGA_KICK_E_NULL;
+    if (on < 0 || on > GENGA_KICK_REUSE_LIST) return GENGA_KICK_E_SIZE;
     ctx->reuse_order = on != 0;
+    ctx->reuse_list = on == GENGA_KICK_REUSE_LIST;
     return GENGA_KICK_OK;
 }
 
@@ -223,7 +228,11 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches += 8;
         ctx->order_valid = true;
+        ctx->list_valid = false;
     }
+    // GENGA_KICK_REUSE_LIST: a level >= 1 kick evaluates the candidate list the level-0 kick has left
+    const bool keep_list = changeover_level > 0 && ctx->reuse_list && ctx->list_valid;
+    if (!keep_list) ctx->list_valid = changeover_level == 0;   // whose list ctx->cand holds after this call
     kp = genga::KickParams{};
     {
         kp.rxy = ctx->rxy; kp.rzm = ctx->rzm; kp.rfw = ctx->rfw; kp.ridx = ctx->ridx;
@@ -236,14 +245,17 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
         kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
         kp.status = ctx->status;
         kp.cand = ctx->cand; kp.cand_capacity = ctx->cand_capacity; kp.ncand = ctx->ncand;
-        kp.fx = ctx->fx; kp.touched = ctx->touched;
+        kp.fx = ctx->fx; kp.fx_stride = ctx->n_rec_alloc; kp.touched = ctx->touched;
+        kp.need_near = keep_list ? ctx->need_near + changeover_level : nullptr;
     }
     {
         const int blocks = (int)((std::max<int64_t>(n_rec, N + 1) + 255) / 256);
         genga::pack_kernel<<<blocks, 256, 0, st>>>(pos, mass, rcrit, ctx->sorted ? ctx->vals_a : nullptr, N,
                                                    ctx->cfg.n_massive, pl.m_pad, n_rec, changeover_level, ctx->cfg.G,
                                                    ctx->cfg.enc_factor, fw_scale, ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx,
-                                                   ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand);
+                                                   ctx->cblo, ctx->cbhi, out_npairs, ctx->ncand,
+                                                   ctx->rfw_ref, ctx->need_near,
+                                                   ctx->cfg.max_level + 1, keep_list ? 1 : 0);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
     }
@@ -270,7 +282,7 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
             }
         } else if (changeover_level == 0) {
             GK_CUDA(ctx, dispatch_kick(pl, kp, st));
-        } else {
+        } else if (!keep_list) {
             // W_L = 0 exactly outside the filter radius: a neighbour search, no tile decomposition
             const int n_igroups = n_rec / GENGA_GROUP, wpc = GENGA_NEAR_THREADS / 32;
             const int n_jgroups = pl.m_pad / GENGA_GROUP;
@@ -283,7 +295,7 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
             GK_CUDA(ctx, cudaEventRecord(ctx->ev[2 * changeover_level + 1], st));
             ctx->ev_set[changeover_level] = true;
         }
-        ctx->launches++;
+        if (!keep_list) ctx->launches++;
         if (ctx->tp2 && changeover_level == 0 && ctx->plan_tp2.n_ctas > 0) {
             // TP 2, far field of the massive bodies' sum over the semi-active particles (at level >= 1 it is 0)
             const genga_kick_plan& p2 = ctx->plan_tp2;
@@ -344,7 +356,8 @@ int kick_back(genga_kick_ctx* ctx, const genga::KickParams& kp, int32_t changeov
             rp.seg[2] = seg_of(pl, ctx->partial, 0, 0, false);
         }
         rp.seg[1] = seg_of(p2, ctx->partial2, 0, pl.m_pad, second);
-        genga::reduce_kernel<<<(n_rec + 255) / 256, 256, 0, st>>>(rp, ctx->ridx, n_rec, N, dt, ctx->fx, ctx->touched,
+        genga::reduce_kernel<<<(n_rec + GENGA_REDUCE_THREADS - 1) / GENGA_REDUCE_THREADS, GENGA_REDUCE_THREADS, 0, st>>>(
+            rp, ctx->ridx, n_rec, N, dt, ctx->fx, ctx->n_rec_alloc, ctx->touched,
                                                                   ctx->status, out_acc, vel);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
@@ -411,12 +424,12 @@ extern "C" int genga_kick_list(genga_kick_ctx* ctx, const double* pos, double* v
     kp.N = N; kp.n_massive = ctx->cfg.n_massive; kp.L = changeover_level; kp.f = ctx->cfg.enc_factor;
     kp.out_pairs = out_pairs; kp.capacity = ctx->cfg.pair_capacity; kp.out_npairs = out_npairs;
     kp.status = ctx->status;
-    kp.fx = ctx->fx; kp.touched = ctx->touched;
+    kp.fx = ctx->fx; kp.fx_stride = ctx->n_rec_alloc; kp.touched = ctx->touched;
     GK_CUDA(ctx, cudaMemsetAsync(out_npairs, 0, ((size_t)N + 1) * sizeof(int32_t), st));
     const int blocks = (int)std::min<int64_t>(std::max<int64_t>((in_pair_rows + 1023) / 1024, 1), 8 * ctx->num_sms);
     genga::list_kick_kernel<<<blocks, 256, 0, st>>>(kp, pos, mass, ctx->cfg.G, reinterpret_cast<const int2*>(in_pairs),
                                                     in_n_pairs, in_pair_rows, ctx->cfg.tp_mode == 2 ? 1 : 0);
-    genga::list_reduce_kernel<<<(N + 255) / 256, 256, 0, st>>>(ctx->fx, ctx->touched, N, dt, ctx->status, out_acc, vel);
+    genga::list_reduce_kernel<<<(N + 255) / 256, 256, 0, st>>>(ctx->fx, ctx->n_rec_alloc, ctx->touched, N, dt, ctx->status, out_acc, vel);
     GK_CUDA(ctx, cudaGetLastError());
     ctx->launches += 2;
     return GENGA_KICK_OK;
@@ -521,7 +534,7 @@ extern "C" int64_t genga_kick_launch_count(const genga_kick_ctx* ctx) { return c
 extern "C" int genga_kick_free(genga_kick_ctx* ctx)
 {
     if (!ctx) return GENGA_KICK_OK;
-    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->ridx, ctx->partial_sym, ctx->react, ctx->sym_t0, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
+    void* bufs[] = {ctx->rxy, ctx->rzm, ctx->rfw, ctx->rfw_ref, ctx->need_near, ctx->ridx, ctx->partial_sym, ctx->react, ctx->sym_t0, ctx->cblo, ctx->cbhi, ctx->bbox, ctx->keys_a,
                     ctx->keys_b, ctx->vals_a, ctx->vals_b, ctx->counts, ctx->partial, ctx->partial2, ctx->status, ctx->cand, ctx->ncand, ctx->fx, ctx->touched, ctx->h_pos,
                     ctx->h_vel, ctx->h_mass, ctx->h_rcrit, ctx->h_acc, ctx->h_pairs, ctx->h_npairs,
                     ctx->psum_partial, ctx->psum_ticket, ctx->step_rcrit, ctx->grp_label, ctx->grp_flag,

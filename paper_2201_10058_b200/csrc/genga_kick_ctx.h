@@ -30,6 +30,11 @@ struct genga_kick_ctx {
     bool sorted;
     bool reuse_order;              // genga_kick_set_order_reuse: keep the permutation of the last sort
     bool order_valid;              // ... there is one
+    bool reuse_list;               // genga_kick_set_order_reuse(2): level >= 1 kicks also take the candidate list of the
+                                   // last level-0 kick (positions unchanged since then)
+    bool list_valid;               // ... ctx->cand holds one (the last kick that wrote a list was a level-0 kick)
+    int* rfw_ref;                  // [n_rec] filter words that list was built with
+    int* need_near;                // [max_level + 1] != 0: some body's filter word at that level exceeds rfw_ref
     int sort_blocks;
     unsigned* bbox;
     unsigned* keys_a;

@@ -59,9 +59,19 @@ struct KickParams {
     int2* __restrict__ cand;           // [cand_capacity] (i-record, j-record)
     long long cand_capacity;
     int* __restrict__ ncand;           // candidates appended (may exceed the capacity: status bit)
-    unsigned long long* __restrict__ fx;   // [n_rec][3][GENGA_FX_LIMBS], all zero between calls
+    unsigned long long* __restrict__ fx;   // [3][GENGA_FX_LIMBS][fx_stride], all zero between calls (a record's limbs lie
+                                           // fx_stride apart: reduce_kernel reads them coalesced)
+    long long fx_stride;
     int* __restrict__ touched;         // [n_rec] != 0: the record's accumulators were added to
+    const int* __restrict__ need_near; // level >= 1 kick on the candidate list of the level-0 kick (GENGA_KICK_REUSE_LIST):
+                                       // != 0 if that list may miss a pair of this level (pack_kernel); nullptr otherwise
 };
+
+// the candidate list cannot serve this kick: near_kernel<true> searches and evaluates all pairs itself
+__device__ __forceinline__ bool list_unusable(const KickParams& p)
+{
+    return (long long)*p.ncand > p.cand_capacity || (p.need_near && *p.need_near != 0);
+}
 
 // ---------------------------------------------------------------------------------------------
 // Filter word of a body.  With R_b = max(rc0_b, f rcL_b), a pair (i, j) can only have W != 1
@@ -92,9 +102,14 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
             const int* __restrict__ perm, int N, int n_massive, int m_pad, int n_rec, int L, double G, double f,
             double fw_scale, double2* __restrict__ rxy, double2* __restrict__ rzm, int* __restrict__ rfw, int* __restrict__ ridx,
             float4* __restrict__ cblo, float4* __restrict__ cbhi, int* __restrict__ out_npairs,
-            int* __restrict__ ncand)
+            int* __restrict__ ncand, int* __restrict__ rfw_ref, int* __restrict__ need_near, int n_levels, int keep_list)
 {
-    if (blockIdx.x == 0 && threadIdx.x == 0) *ncand = 0;
+    // keep_list (GENGA_KICK_REUSE_LIST, level >= 1): the candidate list of the level-0 kick stays; a body whose filter
+    // word now exceeds the one that list was built with (rfw_ref) raises need_near[L].  The level-0 kick writes rfw_ref
+    // and clears the flags of every level.
+    if (blockIdx.x == 0 && threadIdx.x == 0 && !keep_list) *ncand = 0;
+    if (blockIdx.x == 0 && rfw_ref && !keep_list)
+        for (int l = threadIdx.x; l < n_levels; l += blockDim.x) need_near[l] = 0;
     const int stride = gridDim.x * blockDim.x;       // a multiple of 32
     const int top = max(n_rec, ((N + 1 + 31) / 32) * 32);
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < top; r += stride) {
@@ -114,6 +129,10 @@ pack_kernel(const double* __restrict__ pos, const double* __restrict__ mass, con
             rzm[r] = make_double2(z, gm);
             rfw[r] = fw;
             ridx[r] = b;
+            if (rfw_ref) {
+                if (!keep_list) rfw_ref[r] = fw;
+                else if (fw > rfw_ref[r]) need_near[L] = 1;
+            }
         }
         int m = fw;
         // group box
@@ -349,7 +368,7 @@ __device__ __forceinline__ bool boxes_near(float4 alo, float4 ahi, int afw, floa
 #define GENGA_STATUS_CAND_OVERFLOW 2
 #define GENGA_STATUS_FX_RANGE 4
 
-__device__ __forceinline__ void fx_add(unsigned long long* __restrict__ acc, double x, int* status)
+__device__ __forceinline__ void fx_add(unsigned long long* __restrict__ acc, long long stride, double x, int* status)
 {
     const long long bits = __double_as_longlong(x);
     const int ex = (int)((bits >> 52) & 0x7ff);
@@ -372,20 +391,20 @@ __device__ __forceinline__ void fx_add(unsigned long long* __restrict__ acc, dou
         atomicOr(status, GENGA_STATUS_FX_RANGE);
         return;
     }
-    if (q0) atomicAdd(acc + l0, neg ? 0ULL - q0 : q0);
-    if (q1) atomicAdd(acc + l0 + 1, neg ? 0ULL - q1 : q1);
-    if (q2) atomicAdd(acc + l0 + 2, neg ? 0ULL - q2 : q2);
+    if (q0) atomicAdd(acc + l0 * stride, neg ? 0ULL - q0 : q0);
+    if (q1) atomicAdd(acc + (l0 + 1) * stride, neg ? 0ULL - q1 : q1);
+    if (q2) atomicAdd(acc + (l0 + 2) * stride, neg ? 0ULL - q2 : q2);
 }
 
 // value of one accumulator; clears it for the next call
-__device__ __forceinline__ double fx_take(unsigned long long* __restrict__ acc, int* status)
+__device__ __forceinline__ double fx_take(unsigned long long* __restrict__ acc, long long stride, int* status)
 {
     unsigned w[GENGA_FX_LIMBS];
     long long carry = 0;
 #pragma unroll
     for (int l = 0; l < GENGA_FX_LIMBS; l++) {
-        const long long v = (long long)acc[l] + carry;
-        acc[l] = 0ULL;
+        const long long v = (long long)acc[l * stride] + carry;
+        acc[l * stride] = 0ULL;
         w[l] = (unsigned)((unsigned long long)v & 0xffffffffULL);
         carry = v >> 32;                                   // arithmetic: the sign travels upwards
     }
@@ -429,33 +448,34 @@ __device__ __forceinline__ void apply_candidate(const KickParams& p, int ir_enc,
     const int bi = ir >= 0 ? p.ridx[ir] : -1, bj = ir >= 0 ? p.ridx[jr] : -1;      // (-1, -1): empty slot
     if (ir == jr || bi < 0 || bj < 0) return;
     if (force_only && bi >= p.n_massive) return;            // the second pass of TP 2 only serves massive i
+    if (force_only && p.L > 0) return;                      // a level-0 list at level >= 1: `react` covers TP 2 there
     const double2 ixy = p.rxy[ir], izm = p.rzm[ir], jxy = p.rxy[jr], jzm = p.rzm[jr];
     const double dx = __dsub_rn(jxy.x, ixy.x), dy = __dsub_rn(jxy.y, ixy.y), dz = __dsub_rn(jzm.x, izm.x);
     const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, bi, bj, dx, dy, dz, jzm.y);
     if (r.s != 0.0) {
-        unsigned long long* acc = p.fx + (size_t)ir * (3 * GENGA_FX_LIMBS);
-        fx_add(acc, __dmul_rn(r.s, dx), p.status);
-        fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
-        fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+        unsigned long long* acc = p.fx + ir;
+        fx_add(acc, p.fx_stride, __dmul_rn(r.s, dx), p.status);
+        fx_add(acc + GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, __dmul_rn(r.s, dy), p.status);
+        fx_add(acc + 2 * GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, __dmul_rn(r.s, dz), p.status);
         p.touched[ir] = 1;
     }
     if (sym && r.W != 0.0 && izm.y != 0.0) {
         // the force of i on j with the bits the definition gives from j's side (d -> -d, r^2 and W unchanged)
         const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
-        unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
-        fx_add(accj, -__dmul_rn(si, dx), p.status);
-        fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
-        fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+        unsigned long long* accj = p.fx + jr;
+        fx_add(accj, p.fx_stride, -__dmul_rn(si, dx), p.status);
+        fx_add(accj + GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, -__dmul_rn(si, dy), p.status);
+        fx_add(accj + 2 * GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, -__dmul_rn(si, dz), p.status);
         p.touched[jr] = 1;
     }
     if (p.react && bi >= p.n_massive && r.W != 0.0 && izm.y != 0.0) {
         // TP 2: the reaction of the semi-active particle i on the massive body j, G m_i W (x_i - x_j) / r^3,
         // with the bits the definition gives from j's side (d -> -d, r^2 unchanged)
         const double si = __ddiv_rn(__dmul_rn(izm.y, r.W), r.r3);
-        unsigned long long* accj = p.fx + (size_t)jr * (3 * GENGA_FX_LIMBS);
-        fx_add(accj, -__dmul_rn(si, dx), p.status);
-        fx_add(accj + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
-        fx_add(accj + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+        unsigned long long* accj = p.fx + jr;
+        fx_add(accj, p.fx_stride, -__dmul_rn(si, dx), p.status);
+        fx_add(accj + GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, -__dmul_rn(si, dy), p.status);
+        fx_add(accj + 2 * GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, -__dmul_rn(si, dz), p.status);
         p.touched[jr] = 1;
     }
     if (r.enc && p.out_npairs && !force_only) {
@@ -564,7 +584,7 @@ __device__ __forceinline__ void emit_pairs_cta(const KickParams& p, const bool (
 __global__ void __launch_bounds__(256) exact_kernel(const KickParams p)
 {
     constexpr int U = GENGA_EXACT_U;
-    if ((long long)*p.ncand > p.cand_capacity) return;      // the list overflowed: near_kernel<true> has done all of it
+    if (list_unusable(p)) return;                           // the list overflowed: near_kernel<true> has done all of it
     const long long n = (long long)*p.ncand;
     // a CTA walks the list in rounds of 256 * U candidates (CTA-uniform trip count: the emission synchronises)
     for (long long cbase = (long long)blockIdx.x * (256 * U); cbase < n; cbase += (long long)gridDim.x * (256 * U)) {
@@ -768,7 +788,7 @@ template <bool RESCAN>
 __global__ void __launch_bounds__(GENGA_NEAR_THREADS, 4)
 near_kernel(const KickParams p, int i_rec_end, int j_group0, int n_jgroups, int force_only)
 {
-    if (RESCAN && (long long)*p.ncand <= p.cand_capacity) return;
+    if (RESCAN && !list_unusable(p)) return;
     __shared__ float4 blo[GENGA_NEAR_BOXES];
     __shared__ float4 bhi[GENGA_NEAR_BOXES];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -891,18 +911,18 @@ list_kick_kernel(const KickParams p, const double* __restrict__ pos, const doubl
             const double gmi = __dmul_rn(G, mass[i]), gmj = __dmul_rn(G, mass[j]);
             const ExactResult r = exact_pair(p.rcrit, p.N, p.L, p.f, p.status, i, j, dx, dy, dz, gmj);
             if ((j < p.n_massive || tp2) && r.s != 0.0) {            // i feels j
-                unsigned long long* acc = p.fx + (size_t)i * (3 * GENGA_FX_LIMBS);
-                fx_add(acc, __dmul_rn(r.s, dx), p.status);
-                fx_add(acc + GENGA_FX_LIMBS, __dmul_rn(r.s, dy), p.status);
-                fx_add(acc + 2 * GENGA_FX_LIMBS, __dmul_rn(r.s, dz), p.status);
+                unsigned long long* acc = p.fx + i;
+                fx_add(acc, p.fx_stride, __dmul_rn(r.s, dx), p.status);
+                fx_add(acc + GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, __dmul_rn(r.s, dy), p.status);
+                fx_add(acc + 2 * GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, __dmul_rn(r.s, dz), p.status);
                 p.touched[i] = 1;
             }
             if ((i < p.n_massive || tp2) && r.W != 0.0 && gmi != 0.0) {   // j feels i
                 const double si = __ddiv_rn(__dmul_rn(gmi, r.W), r.r3);
-                unsigned long long* acc = p.fx + (size_t)j * (3 * GENGA_FX_LIMBS);
-                fx_add(acc, -__dmul_rn(si, dx), p.status);
-                fx_add(acc + GENGA_FX_LIMBS, -__dmul_rn(si, dy), p.status);
-                fx_add(acc + 2 * GENGA_FX_LIMBS, -__dmul_rn(si, dz), p.status);
+                unsigned long long* acc = p.fx + j;
+                fx_add(acc, p.fx_stride, -__dmul_rn(si, dx), p.status);
+                fx_add(acc + GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, -__dmul_rn(si, dy), p.status);
+                fx_add(acc + 2 * GENGA_FX_LIMBS * p.fx_stride, p.fx_stride, -__dmul_rn(si, dz), p.status);
                 p.touched[j] = 1;
             }
             if (r.enc) {
@@ -916,7 +936,7 @@ list_kick_kernel(const KickParams p, const double* __restrict__ pos, const doubl
 }
 
 __global__ void __launch_bounds__(256)
-list_reduce_kernel(unsigned long long* __restrict__ fx, int* __restrict__ touched, int N, double dt,
+list_reduce_kernel(unsigned long long* __restrict__ fx, long long fx_stride, int* __restrict__ touched, int N, double dt,
                    int* __restrict__ status, double* __restrict__ out_acc, double* __restrict__ vel)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -924,10 +944,10 @@ list_reduce_kernel(unsigned long long* __restrict__ fx, int* __restrict__ touche
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
     if (touched[b]) {
         touched[b] = 0;
-        unsigned long long* acc = fx + (size_t)b * (3 * GENGA_FX_LIMBS);
-        a0 = fx_take(acc, status);
-        a1 = fx_take(acc + GENGA_FX_LIMBS, status);
-        a2 = fx_take(acc + 2 * GENGA_FX_LIMBS, status);
+        unsigned long long* acc = fx + b;
+        a0 = fx_take(acc, fx_stride, status);
+        a1 = fx_take(acc + GENGA_FX_LIMBS * fx_stride, fx_stride, status);
+        a2 = fx_take(acc + 2 * GENGA_FX_LIMBS * fx_stride, fx_stride, status);
     }
     if (out_acc) {
         out_acc[b] = a0;
@@ -1004,9 +1024,10 @@ __device__ __forceinline__ void add_segments(const SegPlan& q, int r, double& a0
     }
 }
 
-__global__ void __launch_bounds__(256)
+#define GENGA_REDUCE_THREADS 64      // small CTAs: 65,536 records spread evenly over 148 SMs
+__global__ void __launch_bounds__(GENGA_REDUCE_THREADS)
 reduce_kernel(const ReduceParams rp, const int* __restrict__ ridx, int n_rec, int N, double dt,
-              unsigned long long* __restrict__ fx, int* __restrict__ touched, int* __restrict__ status,
+              unsigned long long* __restrict__ fx, long long fx_stride, int* __restrict__ touched, int* __restrict__ status,
               double* __restrict__ out_acc, double* __restrict__ vel)
 {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1019,22 +1040,33 @@ reduce_kernel(const ReduceParams rp, const int* __restrict__ ridx, int n_rec, in
         // the reaction sums of the symmetric tiles that hold record r as a j-record: rows 0 .. (row of r) - 1
         const SegPlan& q = rp.seg[0];
         const int JT = rp.react_jt, jt = r / JT, off = r - jt * JT, rows = r / q.IB;
-        for (int I = 0; I < rows; I++) {
-            const long long t = sym_row_begin(I, q.n_j_tiles, q.r) + (jt - I * q.r);
-            const double* v = rp.react + (size_t)t * (3 * JT) + off;
-            a0 = __dadd_rn(a0, v[0]);
-            a1 = __dadd_rn(a1, v[JT]);
-            a2 = __dadd_rn(a2, v[2 * JT]);
+        // (loads of 8 rows in flight, added in row order)
+        for (int I0 = 0; I0 < rows; I0 += 8) {
+            double v0[8], v1[8], v2[8];
+#pragma unroll
+            for (int u = 0; u < 8; u++) {
+                const int I = min(I0 + u, rows - 1);
+                const long long t = sym_row_begin(I, q.n_j_tiles, q.r) + (jt - I * q.r);
+                const double* v = rp.react + (size_t)t * (3 * JT) + off;
+                v0[u] = v[0]; v1[u] = v[JT]; v2[u] = v[2 * JT];
+            }
+#pragma unroll
+            for (int u = 0; u < 8; u++)
+                if (I0 + u < rows) {
+                    a0 = __dadd_rn(a0, v0[u]);
+                    a1 = __dadd_rn(a1, v1[u]);
+                    a2 = __dadd_rn(a2, v2[u]);
+                }
         }
     }
     add_segments(rp.seg[1], r, a0, a1, a2);
     add_segments(rp.seg[2], r, a0, a1, a2);
     if (touched[r]) {                                      // the exact path's terms (fixed point, see fx_add)
         touched[r] = 0;
-        unsigned long long* acc = fx + (size_t)r * (3 * GENGA_FX_LIMBS);
-        a0 = __dadd_rn(a0, fx_take(acc, status));
-        a1 = __dadd_rn(a1, fx_take(acc + GENGA_FX_LIMBS, status));
-        a2 = __dadd_rn(a2, fx_take(acc + 2 * GENGA_FX_LIMBS, status));
+        unsigned long long* acc = fx + r;
+        a0 = __dadd_rn(a0, fx_take(acc, fx_stride, status));
+        a1 = __dadd_rn(a1, fx_take(acc + GENGA_FX_LIMBS * fx_stride, fx_stride, status));
+        a2 = __dadd_rn(a2, fx_take(acc + 2 * GENGA_FX_LIMBS * fx_stride, fx_stride, status));
     }
     if (out_acc) {
         out_acc[b] = a0;

@@ -219,6 +219,44 @@ def test_order_reuse_across_levels(oracle_mod):
     k.free()
 
 
+@pytest.mark.parametrize("tp_mode,n,n_test", [(1, 9000, 0), (1, 30000, 0), (1, 1500, 4500), (2, 1500, 4500)])
+def test_list_reuse_across_levels(oracle_mod, tp_mode, n, n_test):
+    """GENGA_KICK_REUSE_LIST: the level-1 and level-2 kicks of a step evaluate the near pairs the level-0 kick has listed
+    (no neighbour search of their own): the same bits, counts and pair set as their own search, with and without test
+    particles, below and above the size from which level 0 runs the symmetric loop.  If a body's filter radius at the
+    level exceeds its level-0 one (here: row 1 of rcrit scaled up), the device check sends that kick to the all-pairs
+    search; the results are still those of the oracle."""
+    from paper_2201_10058_b200 import GengaKick
+    make = lambda: gi.make_config(4, n=n, n_test=n_test, level=2) if n_test else gi.make_config(3, n=n, level=2)
+    ki = make()
+    if tp_mode == 2:
+        _with_tp_masses(ki)
+    kw = dict(max_level=2, pair_capacity=1 << 20, G=ki.G, enc_factor=ki.enc_factor, tp_mode=tp_mode)
+    k = GengaKick(ki.n_massive, ki.n_test, **kw)
+    run_gpu(ki, level=0, kick=k)
+    k.set_order_reuse(2)
+    for level in (1, 2):
+        before = k.launch_count()
+        kept = run_gpu(ki, level=level, kick=k)
+        kept.launches -= before
+        fresh = run_gpu(ki, level=level, tp_mode=tp_mode)
+        assert kept.status == 0
+        assert np.array_equal(kept.acc, fresh.acc) and np.array_equal(kept.counts, fresh.counts)
+        assert np.array_equal(sorted_pairs(kept.pairs), sorted_pairs(fresh.pairs))
+        assert kept.launches < fresh.launches
+    grown = make()
+    grown.mass = ki.mass
+    grown.rcrit = grown.rcrit.copy()
+    grown.rcrit[1, ::7] = 3.0 * grown.rcrit[0, ::7]                      # f rc1 > f rc0 for every seventh body
+    run_gpu(grown, level=0, kick=k)
+    wide = run_gpu(grown, level=1, kick=k)
+    orc = oracle_mod.kick(grown.pos, grown.mass, grown.rcrit, grown.n_massive, grown.n_test, level=1, G=grown.G,
+                          enc_factor=grown.enc_factor, tp_mode=tp_mode)
+    assert wide.status == 0
+    compare(wide, orc, grown.n_massive, tol=TOL)
+    k.free()
+
+
 def test_internal_order_is_invisible(oracle_mod):
     """Caller's order, sorted order and auto give the same pair set and counts; accelerations agree
     to the rounding of a different summation order."""
