@@ -36,6 +36,10 @@ SENC_EXPORTS = ("genga_detect", "genga_multilevel_step", "genga_steps")
 STATUS_RCRIT_JUMP = 256
 REUSE_OFF, REUSE_ORDER, REUSE_LIST = 0, 1, 2
 STATUS_LIST_CLIPPED = 128
+# include/genga_kick_static.h: the list kick without a context and without any allocation
+STATIC_EXPORTS = ("genga_kick_list_static",)
+STATIC_MAX_BODIES = 65536
+E_STATIC_MAX = -7
 
 
 class GengaKickConfig(C.Structure):
@@ -120,7 +124,8 @@ def lib():
         L.genga_detect.argtypes = [vp, vp, vp, vp, vp, vp, d, d, vp, vp, i64, vp, vp]
         L.genga_multilevel_step.argtypes = [vp, vp, vp, vp, d, d, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
         L.genga_steps.argtypes = [vp, vp, vp, vp, d, d, i32, C.POINTER(GengaSencConfig), vp, vp, vp, vp]
-        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS + SENC_EXPORTS:
+        L.genga_kick_list_static.argtypes = [vp, vp, vp, vp, i64, i64, i32, i32, d, d, d, vp, vp, i64, vp, vp, i64, vp, vp, vp]
+        for name in EXPORTS + STEP_EXPORTS + GROUP_EXPORTS + BS_EXPORTS + SENC_EXPORTS + STATIC_EXPORTS:
             if name not in ("genga_kick_launch_count", "genga_kick_strerror", "genga_kick_last_cuda_error",
                             "genga_kick_plan_sym_row_begin", "genga_kick_plan_sym_row_of"):
                 getattr(L, name).restype = C.c_int
@@ -130,6 +135,25 @@ def lib():
 
 def strerror(code: int) -> str:
     return lib().genga_kick_strerror(int(code)).decode()
+
+
+def kick_list_static(pos, vel, mass, rcrit, n_massive, n_test, changeover_level, dt, in_pairs, in_n_pairs, in_pair_rows,
+                     out_acc, out_pairs, out_npairs, status, G=1.0, enc_factor=1.0, tp_mode=1, cuda_stream=0):
+    """include/genga_kick_static.h: genga_kick_list with the scratch in a static device array of the library -- no
+    context, no allocation, N <= STATIC_MAX_BODIES; calls that overlap on the GPU race on that array.  `status`: one
+    int32 on the device (out).  out_pairs: [capacity, 2] int32 or None."""
+    n = int(n_massive) + int(n_test)
+    cap = 0 if out_pairs is None else int(out_pairs.numel()) // 2
+    rows = max(int(changeover_level), 0) + 1
+    rc = lib().genga_kick_list_static(
+        _ptr(pos, "f8", 3 * n, "pos"), _ptr(vel, "f8", 3 * n, "vel"), _ptr(mass, "f8", n, "mass"),
+        _ptr(rcrit, "f8", rows * n, "rcrit"), int(n_massive), int(n_test), int(changeover_level), int(tp_mode), float(G),
+        float(enc_factor), float(dt), _ptr(in_pairs, "i4", 2 * int(in_pair_rows), "in_pairs"),
+        _ptr(in_n_pairs, "i4", 1, "in_n_pairs"), int(in_pair_rows), _ptr(out_acc, "f8", 3 * n, "out_acc"),
+        _ptr(out_pairs, "i4", 2 * cap, "out_pairs"), cap, _ptr(out_npairs, "i4", n + 1, "out_npairs"),
+        _ptr(status, "i4", 1, "status"), C.c_void_p(int(cuda_stream)))
+    if rc != OK:
+        raise GengaKickError(rc, strerror(rc))
 
 
 def make_plan(n_massive: int, n_test: int, level: int, num_sms: int) -> GengaKickPlan:

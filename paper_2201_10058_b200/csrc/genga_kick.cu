@@ -555,3 +555,98 @@ extern "C" const char* genga_kick_last_cuda_error(const genga_kick_ctx* ctx)
 {
     return ctx ? ctx->cuda_err.c_str() : "";
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// genga_kick_list_static (include/genga_kick_static.h): the list kick without a context and without any allocation.
+// Its scratch -- the fixed-point accumulators fx[3][GENGA_FX_LIMBS][stride] and the flags touched[N] behind them -- is
+// this file-scope array: every device that loads the library holds it until the process exits.  In HOST code the
+// array's name is a host-side stand-in, not a device address: static_scratch_of() asks the runtime for the address
+// (cudaGetSymbolAddress, once per device, with that device current) and the kernels get that pointer.
+// ---------------------------------------------------------------------------------------------------------------------
+#include "../../include/genga_kick_static.h"
+#include <mutex>
+
+static_assert(GENGA_KICK_STATIC_SCRATCH_BYTES == GENGA_KICK_STATIC_MAX_BODIES * (3 * GENGA_FX_LIMBS * 8 + 4),
+              "include/genga_kick_static.h states the size of the accumulators");
+static __device__ __align__(256) unsigned long long genga_static_scratch[GENGA_KICK_STATIC_SCRATCH_BYTES / 8];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+    unsigned long long* scratch;   // device address of genga_static_scratch on this device; nullptr: not asked yet
+    int num_sms;
+};
+StaticDevice g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+// set-up of the current device, once: no allocation (attribute queries and the symbol's address)
+int static_scratch_of(StaticDevice& out)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kStaticMaxDevices) return GENGA_KICK_E_CUDA;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& d = g_static_dev[dev];
+    if (!d.scratch) {
+        int major = 0, sms = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return GENGA_KICK_E_CUDA;
+        if (major != 10) return GENGA_KICK_E_CUDA;                                   // sm_100a only
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return GENGA_KICK_E_CUDA;
+        unsigned long long* ptr = nullptr;
+        if (cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), genga_static_scratch) != cudaSuccess || !ptr)
+            return GENGA_KICK_E_CUDA;
+        d.num_sms = sms;
+        d.scratch = ptr;
+    }
+    out = d;
+    return GENGA_KICK_OK;
+}
+
+}  // namespace
+
+extern "C" int genga_kick_list_static(const double* pos, double* vel, const double* mass, const double* rcrit,
+                                      int64_t n_massive, int64_t n_test, int32_t changeover_level, int32_t tp_mode,
+                                      double G, double enc_factor, double dt, const int32_t* in_pairs,
+                                      const int32_t* in_n_pairs, int64_t in_pair_rows, double* out_acc, int32_t* out_pairs,
+                                      int64_t pair_capacity, int32_t* out_npairs, int32_t* status, void* cuda_stream)
+{
+    if (!pos || !mass || !rcrit || !in_n_pairs || !out_npairs || !status) return GENGA_KICK_E_NULL;
+    if (!out_acc && !vel) return GENGA_KICK_E_NULL;
+    if (n_massive < 0 || n_test < 0 || pair_capacity < 0 || in_pair_rows < 0) return GENGA_KICK_E_SIZE;
+    if (n_massive > GENGA_MAX_BODIES || n_test > GENGA_MAX_BODIES) return GENGA_KICK_E_SIZE;
+    const int64_t N64 = n_massive + n_test;
+    if (N64 <= 0 || N64 > GENGA_MAX_BODIES || tp_mode < 0 || tp_mode > 2) return GENGA_KICK_E_SIZE;
+    if (N64 > GENGA_KICK_STATIC_MAX_BODIES) return GENGA_KICK_E_STATIC_MAX;
+    if (!out_pairs && pair_capacity > 0) return GENGA_KICK_E_NULL;
+    if (!in_pairs && in_pair_rows > 0) return GENGA_KICK_E_NULL;
+    if (changeover_level < 0 || changeover_level > 62) return GENGA_KICK_E_LEVEL;
+    if (misaligned(pos) || misaligned(vel) || misaligned(mass) || misaligned(rcrit) || misaligned(out_acc) ||
+        misaligned(out_pairs) || misaligned(out_npairs) || misaligned(in_pairs))
+        return GENGA_KICK_E_ALIGN;
+    StaticDevice sd = {};
+    int rc = static_scratch_of(sd);
+    if (rc != GENGA_KICK_OK) return rc;
+
+    const int N = (int)N64;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const long long stride = ((long long)N + 31) / 32 * 32;            // rows of the accumulators: 256-byte multiples
+    unsigned long long* fx = sd.scratch;
+    int* touched = reinterpret_cast<int*>(sd.scratch + 3 * GENGA_FX_LIMBS * stride);
+    // the array keeps what the last call (perhaps one that failed half way) left: clear what this one uses
+    const size_t used = (size_t)(3 * GENGA_FX_LIMBS * stride) * sizeof(unsigned long long) + (size_t)N * sizeof(int);
+    if (cudaMemsetAsync(sd.scratch, 0, used, st) != cudaSuccess) return GENGA_KICK_E_CUDA;
+    if (cudaMemsetAsync(status, 0, sizeof(int32_t), st) != cudaSuccess) return GENGA_KICK_E_CUDA;
+    if (cudaMemsetAsync(out_npairs, 0, ((size_t)N + 1) * sizeof(int32_t), st) != cudaSuccess) return GENGA_KICK_E_CUDA;
+
+    genga::KickParams kp = {};
+    kp.rcrit = rcrit;
+    kp.N = N; kp.n_massive = (int)n_massive; kp.L = changeover_level; kp.f = enc_factor;
+    kp.out_pairs = out_pairs; kp.capacity = pair_capacity; kp.out_npairs = out_npairs;
+    kp.status = status;
+    kp.fx = fx; kp.fx_stride = stride; kp.touched = touched;
+    const int blocks = (int)std::min<int64_t>(std::max<int64_t>((in_pair_rows + 1023) / 1024, 1), 8 * sd.num_sms);
+    genga::list_kick_kernel<<<blocks, 256, 0, st>>>(kp, pos, mass, G, reinterpret_cast<const int2*>(in_pairs), in_n_pairs,
+                                                    in_pair_rows, tp_mode == 2 ? 1 : 0);
+    genga::list_reduce_kernel<<<(N + 255) / 256, 256, 0, st>>>(fx, stride, touched, N, dt, status, out_acc, vel);
+    return cudaGetLastError() == cudaSuccess ? GENGA_KICK_OK : GENGA_KICK_E_CUDA;
+}

@@ -246,6 +246,7 @@ extern "C" const char* genga_kick_strerror(int code)
     case GENGA_KICK_E_LEVEL: return "changeover_level is outside [0, max_level]";
     case GENGA_KICK_E_CUDA: return "a CUDA call failed";
     case GENGA_KICK_E_NOMEM: return "host allocation failed";
+    case -7: return "N exceeds GENGA_KICK_STATIC_MAX_BODIES (65536): the static scratch of genga_kick_list_static cannot hold it";   // genga_kick_static.h
     default: return "unknown genga_kick error code";
     }
 }
