@@ -78,8 +78,8 @@ struct BsGlobal {
     double* la;                         // [n] A_b: bound on its deviation from straight-line motion during the call
     double* ld;                         // [n] |v_b| |dt| + A_b: bound on its displacement (cheap first test)
     double* vx; double* vy; double* vz; // [n] velocities at the start of the call
-    int* nbr;                           // [nbr_capacity] list entries (member positions within the group)
-    long long nbr_capacity;
+    int* nbr;                           // the warps' lists: chunks of 32 entries, bs_chunk_words(nlevels) 8-byte words each
+    long long nbr_capacity;             // ... its size in 4-byte units
     unsigned long long* cursor;         // entries reserved so far (zero between groups)
     unsigned long long* err;            // [4], all zero between uses
     // teams: the co-resident grid cut into teams of team_ctas CTAs, each integrating its own groups with a barrier
@@ -138,6 +138,25 @@ __device__ __forceinline__ void bs_gsync(BsShared<ROWS>& S, const BsGlobal& Gm)
 // the term).  In the large groups of a disk almost all pairs are of this kind: a group is a chain of neighbours.
 __device__ __forceinline__ double bs_far_bound(double rc0) { return (rc0 * rc0) * (1.0 + 9.5367431640625e-07); }
 
+// The weight and the factor of a pair inside a far-pair bound: s = G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) / r^3;
+// false: the product is 0 and the pair adds nothing.  OUT OF LINE, one copy per kernel: a square root, a divide for s and
+// two per level are ~400 instructions, and the force loops name a pair in up to a dozen places (lanes' sub-lists x
+// loads in flight, all-pairs fallback) -- inlined, the whole-grid kernels were 13,000 - 61,000 instructions long and
+// their list walk ran out of the instruction cache (12 us per near pair; profiles/ncu_r02c.md).
+__device__ __noinline__ bool bs_pair_factor(double r2, double gmj, int nlevels, double rci0, double rci1, double rci2, double rci3,
+                                            double rcj0, double rcj1, double rcj2, double rcj3, double& s)
+{
+    const double r = sqrt(r2);
+    double W = 1.0;
+    W *= (1.0 - bs_K(r, fmax(rci0, rcj0)));
+    if (1 < nlevels) W *= (1.0 - bs_K(r, fmax(rci1, rcj1)));
+    if (2 < nlevels) W *= (1.0 - bs_K(r, fmax(rci2, rcj2)));
+    if (3 < nlevels) W *= (1.0 - bs_K(r, fmax(rci3, rcj3)));
+    if (W == 0.0) return false;
+    s = gmj * W / (r2 * r);
+    return true;
+}
+
 // one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3.
 // Test-particle modes (sec. 8.1, Fig. 14): a semi-active particle j is staged with the SIGN BIT of
 // G m_j set; it acts on nobody in TP 1 and on the massive bodies only in TP 2 (particles never feel each other).
@@ -150,13 +169,10 @@ __device__ __forceinline__ double bs_far_bound(double rc0) { return (rc0 * rc0) 
         const double dx = (XJ) - x, dy = (YJ) - y, dz = (ZJ) - z;                                      \
         const double r2 = dx * dx + dy * dy + dz * dz;                                                 \
         if (!skip && r2 < fmax(bnd_i, (BNDJ))) {                                                       \
-            const double r = sqrt(r2);                                                                 \
-            double W = 1.0;                                                                            \
-            _Pragma("unroll")                                                                          \
-            for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++)                                              \
-                if (k < nlevels) W *= (1.0 - bs_K(r, fmax(rci[k], RCJ(k))));                           \
-            if (W != 0.0) {                                                                            \
-                const double s = gmj * W / (r2 * r);                                                   \
+            double s;                                                                                  \
+            if (bs_pair_factor(r2, gmj, nlevels, rci[0], rci[1], rci[2], rci[3], RCJ(0),               \
+                               1 < nlevels ? RCJ(1) : 0.0, 2 < nlevels ? RCJ(2) : 0.0,                 \
+                               3 < nlevels ? RCJ(3) : 0.0, s)) {                                       \
                 AX = AX + s * dx; AY = AY + s * dy; AZ = AZ + s * dz;                                  \
             }                                                                                          \
         }                                                                                              \
@@ -173,18 +189,36 @@ __device__ __forceinline__ double bs_far_bound(double rc0) { return (rc0 * rc0) 
 // knows its time tau) and raises GENGA_STATUS_BS_LIST_ESCAPE if a body strayed further -- then, and only then, a pair
 // outside the lists may have come inside a critical radius unseen.  A pair outside the lists therefore has
 // r > max(R_i, R_j) at every force evaluation and contributes exactly 0, as in the all-pairs sum: the lists change the
-// cost (n x a few partners instead of n^2 pairs per force evaluation), not one bit of the result.  A lane keeps the sub-list of ITS share of the
-// partners (j = lane (mod 8), ascending j), so the partial sums and their tree are those of the all-pairs loop.
-// Lists that do not fit the scratch (nbr_capacity entries) are not used: that group falls back to all pairs.
+// cost (n x a few partners instead of n^2 pairs per force evaluation) and the ORDER of the sum (below), nothing else.
+//
+// The lists are kept per WARP, not per lane: the entries of the warp's bodies (32 / SUB of them), sorted by body, in
+// chunks of 32.  A force evaluation walks the chunks with all 32 lanes -- one entry per lane whatever body it belongs
+// to, so that a body with 100 partners and one with 5 cost the warp the same per entry (per-lane lists left a warp
+// waiting for its longest lane, 9 of 32 lanes active on average in the dense group of configs[3] at 2 levels x 2
+// sub-steps: profiles/ncu_r02c.md) -- and adds the terms of a chunk with a segmented scan over the lanes (segments =
+// bodies; IEEE additions in a fixed tree), the segment sums to the bodies' accumulators in chunk order.  The order of a
+// body's sum is thus a fixed function of the list, i.e. of the inputs; it is the kernel's own choice
+// like every force-sum order here (reading G15).
+// Lists that do not fit the scratch (nbr_capacity) are not used: that group falls back to all pairs.
 // ---------------------------------------------------------------------------------------------------------------------
 template <int NL>
 struct BsList {
-    bool on;                            // lists in use for this group (grid-uniform)
-    long long base[NL];                 // this lane's sub-lists: u-th holds the partners j = sub + u (mod 8)
-    int count[NL];
+    bool on;                            // lists in use for this group (team-uniform)
+    long long wbase;                    // this WARP's list: first chunk (warp-uniform) ...
+    int wchunks;                        // ... and number of chunks of 32 entries
     double q0[3], v0[3];                // the body's state at the start of the call
     double a2;                          // A_b^2
 };
+
+// A chunk of a warp's list: 32 entries, field by field (every load of the walk is one coalesced 256-byte row):
+//   row 0       (j, slot) -- the partner's position within the group (-1: padding) and which of the warp's bodies the
+//               entry belongs to (lane / SUB of its lanes); the entries of a warp are sorted by slot
+//   row 1       G m_j
+//   row 2       max(bound_i, bound_j), the far-pair bound of the pair (bs_far_bound)
+//   row 3 + k   max(rc_k,i, rc_k,j), k < nlevels
+// i.e. everything about the pair that does not change during the call: a force evaluation reads the entry and ONE
+// 32-byte record of the partner's current position.
+__device__ __forceinline__ int bs_chunk_words(int nlevels) { return 32 * (3 + nlevels); }
 
 // Every thread publishes the position of its body i (if i < n) and gets dv_i/dt back:
 //   - G m_star q / |q|^3 + the pair terms over j = 0 .. n-1, j != i, in that order.
@@ -207,7 +241,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
     const double s0 = -mu / (r2s * rs);
     double ax = s0 * x, ay = s0 * y, az = s0 * z;
     constexpr bool COOP = MODE == GENGA_BS_MODE_COOP;
-    if (MODE == GENGA_BS_MODE_WARP) {
+    if constexpr (MODE == GENGA_BS_MODE_WARP) {
         bs_sync<MODE>();                                      // the previous readers are done
         if (i < n) { S.x[i] = x; S.y[i] = y; S.z[i] = z; }
         bs_sync<MODE>();
@@ -219,7 +253,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             }
 #undef GENGA_BS_RCJ
         }
-    } else if (MODE == GENGA_BS_MODE_CTA) {
+    } else if constexpr (MODE == GENGA_BS_MODE_CTA) {
         // Eight lanes per body inside one CTA (groups of up to 32 bodies): the eight partial sums and the tree as below.
         const int sub = threadIdx.x & (SUB - 1);
         __syncthreads();                                      // the previous readers are done
@@ -242,7 +276,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             az = az + __shfl_xor_sync(0xffffffffu, az, o);
         }
         ax = sx + ax; ay = sy + ay; az = sz + az;
-    } else if (MODE == GENGA_BS_MODE_CLUSTER) {
+    } else if constexpr (MODE == GENGA_BS_MODE_CLUSTER) {
         // Eight lanes per body (as below), the group spread over the CTAs of a cluster: publish, one cluster barrier,
         // gather everybody's positions through distributed shared memory, then sum from the local copy.
         cooperative_groups::cluster_group cl = cooperative_groups::this_cluster();
@@ -288,42 +322,67 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z;
             if (L.on) { Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bnd_i); }
         }
+        // the warp's bodies, for the lanes that walk their entries: current positions and the accumulators
+        constexpr int WB = 32 / SUB;
+        __shared__ double wpos[GENGA_BS_COOP_THREADS / 32][WB][3];
+        __shared__ double wacc[GENGA_BS_COOP_THREADS / 32][WB][3];
+        const int lane = t & 31, wid = t >> 5;
+        if (L.on && sub == 0) {
+            wpos[wid][lane / SUB][0] = x; wpos[wid][lane / SUB][1] = y; wpos[wid][lane / SUB][2] = z;
+            wacc[wid][lane / SUB][0] = 0.0; wacc[wid][lane / SUB][1] = 0.0; wacc[wid][lane / SUB][2] = 0.0;
+        }
         bs_gsync(S, Gm);
         const double sx = ax, sy = ay, sz = az;
         double px[8 / SUB], py[8 / SUB], pz[8 / SUB];
 #pragma unroll
         for (int u = 0; u < 8 / SUB; u++) { px[u] = 0.0; py[u] = 0.0; pz[u] = 0.0; }
-        if (L.on && i < n) {
-            // the body must still be where the lists allow it to be
-            const double ex = x - (L.q0[0] + L.v0[0] * tau), ey = y - (L.q0[1] + L.v0[1] * tau), ez = z - (L.q0[2] + L.v0[2] * tau);
-            if (ex * ex + ey * ey + ez * ez > L.a2) atomicOr(status, GENGA_STATUS_BS_LIST_ESCAPE);
-#pragma unroll
-            for (int u = 0; u < 8 / SUB; u++) {
-                const long long end = L.base[u] + L.count[u];
-                for (long long e = L.base[u]; e < end; e += 4) {          // four entries' loads in flight at a time
-                    int jn[4];
-                    double2 pa[4], pb[4];
-#pragma unroll
-                    for (int k = 0; k < 4; k++) jn[k] = e + k < end ? Gm.nbr[e + k] : -1;
-#pragma unroll
-                    for (int k = 0; k < 4; k++)
-                        if (jn[k] >= 0) { pa[k] = __ldcg(Gm.pk[p] + 2 * jn[k]); pb[k] = __ldcg(Gm.pk[p] + 2 * jn[k] + 1); }
-#pragma unroll
-                    for (int k = 0; k < 4; k++) {
-                        if (jn[k] < 0) continue;
-                        const int jj = jn[k];
-                        // the far test on the packed record alone; G m_j and the radii are fetched for near pairs only
-                        const double fx = pa[k].x - x, fy = pa[k].y - y, fz = pb[k].x - z;
-                        if (fx * fx + fy * fy + fz * fz < fmax(bnd_i, pb[k].y)) {
-                            const double2 s0 = __ldcg(Gm.sr + 3 * jj), s1 = __ldcg(Gm.sr + 3 * jj + 1), s2 = __ldcg(Gm.sr + 3 * jj + 2);
-                            const double rcj[GENGA_BS_MAX_LEVELS] = {s0.y, s1.x, s1.y, s2.x};
-#define GENGA_BS_RCL(k) rcj[k]
-                            GENGA_BS_PAIR_ACC(pa[k].x, pa[k].y, pb[k].x, s0.x, GENGA_BS_RCL, pb[k].y, px[u], py[u], pz[u])
-#undef GENGA_BS_RCL
+        if (L.on) {
+            if (i < n) {
+                // the body must still be where the lists allow it to be
+                const double ex = x - (L.q0[0] + L.v0[0] * tau), ey = y - (L.q0[1] + L.v0[1] * tau), ez = z - (L.q0[2] + L.v0[2] * tau);
+                if (ex * ex + ey * ey + ez * ez > L.a2) atomicOr(status, GENGA_STATUS_BS_LIST_ESCAPE);
+            }
+            const int cw = bs_chunk_words(nlevels);
+            const unsigned long long* rec = reinterpret_cast<const unsigned long long*>(Gm.nbr) + L.wbase * cw + lane;
+            for (int c = 0; c < L.wchunks; c++, rec += cw) {
+                const unsigned long long js = __ldcg(rec);
+                const int jj = (int)(unsigned)(js & 0xffffffffULL), slot = (int)(js >> 32);
+                double tx = 0.0, ty = 0.0, tz = 0.0;
+                if (jj >= 0) {
+                    const double gmj = __longlong_as_double((long long)__ldcg(rec + 32));
+                    const double bnd = __longlong_as_double((long long)__ldcg(rec + 64));
+                    const double2 pa = __ldcg(Gm.pk[p] + 2 * jj), pb = __ldcg(Gm.pk[p] + 2 * jj + 1);
+                    const double dx = pa.x - wpos[wid][slot][0], dy = pa.y - wpos[wid][slot][1], dz = pb.x - wpos[wid][slot][2];
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 < bnd) {
+                        const double rc0 = __longlong_as_double((long long)__ldcg(rec + 96));
+                        const double rc1 = 1 < nlevels ? __longlong_as_double((long long)__ldcg(rec + 128)) : 0.0;
+                        const double rc2 = 2 < nlevels ? __longlong_as_double((long long)__ldcg(rec + 160)) : 0.0;
+                        const double rc3 = 3 < nlevels ? __longlong_as_double((long long)__ldcg(rec + 192)) : 0.0;
+                        double sfac;
+                        if (bs_pair_factor(r2, gmj, nlevels, rc0, rc1, rc2, rc3, 0.0, 0.0, 0.0, 0.0, sfac)) {
+                            tx = sfac * dx; ty = sfac * dy; tz = sfac * dz;
                         }
                     }
                 }
+                // sum of each body's terms of this chunk: inclusive scan over the lanes within runs of equal slot
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int so = __shfl_up_sync(0xffffffffu, slot, o);
+                    const double ux = __shfl_up_sync(0xffffffffu, tx, o), uy = __shfl_up_sync(0xffffffffu, ty, o),
+                                 uz = __shfl_up_sync(0xffffffffu, tz, o);
+                    if (lane >= o && so == slot) { tx = ux + tx; ty = uy + ty; tz = uz + tz; }
+                }
+                const int snext = __shfl_down_sync(0xffffffffu, slot, 1);
+                if (slot < WB && (lane == 31 || snext != slot)) {      // the last lane of a run holds its sum
+                    wacc[wid][slot][0] = wacc[wid][slot][0] + tx;
+                    wacc[wid][slot][1] = wacc[wid][slot][1] + ty;
+                    wacc[wid][slot][2] = wacc[wid][slot][2] + tz;
+                }
+                __syncwarp();                                           // the next chunk may continue the run in another lane
             }
+            px[0] = wacc[wid][lane / SUB][0]; py[0] = wacc[wid][lane / SUB][1]; pz[0] = wacc[wid][lane / SUB][2];
+            __syncwarp();                                               // (before the next evaluation clears them)
         }
         for (int j0 = 0; j0 < (L.on ? 0 : n); j0 += ROWS) {   // ROWS is a multiple of 8: (j0 + jj) mod 8 = jj mod 8
             __syncthreads();
@@ -352,6 +411,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
         // p_r = the terms with j = r (mod 8); lane `sub` holds p_sub, p_sub+SUB, ..: first the pairs of the tree that lie
         // in different lanes (xor butterfly: IEEE addition commutes, so every lane of the body gets the same bits),
         // then those within the lane: ((p0 + p1) + (p2 + p3)) + ((p4 + p5) + (p6 + p7)) whatever SUB is
+        if (!L.on) {
 #pragma unroll
         for (int o = 1; o < SUB; o <<= 1) {
 #pragma unroll
@@ -368,6 +428,7 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
                 px[u] = px[u] + px[u + w]; py[u] = py[u] + py[u + w]; pz[u] = pz[u] + pz[u + w];
             }
         }
+        }
         ax = px[0]; ay = py[0]; az = pz[0];
         ax = sx + ax; ay = sy + ay; az = sz + az;
     }
@@ -375,20 +436,24 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 }
 
 // Whole-grid regime, start of a group: publishes the bodies' starting positions, R_b and D_b, counts and fills the
-// lanes' sub-lists (two scans of the group, tile by tile through shared memory; a lane reserves the room of its
-// sub-lists with one atomic on a cursor -- where a sub-list lies is irrelevant, its entries are in ascending j).
+// warps' lists (two scans of the group, tile by tile through shared memory: a lane scans for its body the partners
+// j = sub, sub + SUB, .. (mod 8); a warp reserves the chunks of its list with one atomic on a cursor -- where a list
+// lies is irrelevant; within it the entries are in the order lane, residue class of j, ascending j).
 // Two grid barriers; the positions go to buffer eval & 1 like a force evaluation's.
 template <int ROWS, int SUB>
 __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, bool i_tp,
-                                               int tp_mode, const double (&q)[3], const double (&v)[3], double rc0, double dt,
-                                               double mu, BsList<8 / SUB>& L)
+                                               int tp_mode, const double (&q)[3], const double (&v)[3],
+                                               const double (&rci)[GENGA_BS_MAX_LEVELS], int nlevels, double dt, double mu,
+                                               BsList<8 / SUB>& L)
 {
     constexpr int NL = 8 / SUB;
-    const int t = threadIdx.x, sub = t & (SUB - 1);
+    const int t = threadIdx.x, sub = t & (SUB - 1), lane = t & 31;
     const int p = eval & 1;
     eval++;
     const double x = q[0], y = q[1], z = q[2];
-    const double lr_i = sqrt(bs_far_bound(rc0));
+    const double rc0 = rci[0];
+    const double bnd_i = bs_far_bound(rc0);
+    const double lr_i = sqrt(bnd_i);
     const double la_i = i < n ? mu * (dt * dt) / (x * x + y * y + z * z) : 0.0;
     const double ld_i = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) * fabs(dt) + la_i;
     L.q0[0] = x; L.q0[1] = y; L.q0[2] = z;
@@ -396,15 +461,20 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
     L.a2 = la_i * la_i;
     if (i < n && sub == 0) {
         Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z;
-        Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bs_far_bound(rc0));
+        Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bnd_i);
         Gm.vx[i] = v[0]; Gm.vy[i] = v[1]; Gm.vz[i] = v[2];
         Gm.lr[i] = lr_i; Gm.la[i] = la_i; Gm.ld[i] = ld_i;
     }
     if (Gm.tb == 0 && t == 0) *Gm.cursor = 0ULL;            // (its last readers passed several barriers ago)
     bs_gsync(S, Gm);
-#pragma unroll
-    for (int u = 0; u < NL; u++) { L.base[u] = 0; L.count[u] = 0; }
+    L.wbase = 0; L.wchunks = 0;
     L.on = false;
+    const int cw = bs_chunk_words(nlevels);
+    unsigned long long* const words = reinterpret_cast<unsigned long long*>(Gm.nbr);
+    int cnt[NL];                                              // pass 0: entries of each of the lane's residue classes
+    int lane_off = 0, wtotal = 0;                             // the lane's first entry within the warp's list; its length
+#pragma unroll
+    for (int u = 0; u < NL; u++) cnt[u] = 0;
     for (int pass = 0; pass < 2; pass++) {                    // 0: count, 1: fill
         int c[NL];
 #pragma unroll
@@ -442,7 +512,19 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
                                 const double Ra = Rm + (la_i + S.rc[1][jj]);
                                 // (1 + 2^-30: the roundings of this test must not drop a pair the exact test keeps)
                                 if (cx * cx + cy * cy + cz * cz < (Ra * Ra) * (1.0 + 9.313225746154785e-10)) {
-                                    if (pass) Gm.nbr[L.base[u] + c[u]] = j0 + jj;
+                                    if (pass) {
+                                        int e = lane_off + c[u];              // entry within the warp's list
+#pragma unroll
+                                        for (int w = 0; w < NL; w++)
+                                            if (w < u) e += cnt[w];
+                                        const int jg = j0 + jj;
+                                        unsigned long long* rec = words + (L.wbase + (e >> 5)) * cw + (e & 31);
+                                        rec[0] = (unsigned long long)(unsigned)jg | ((unsigned long long)(unsigned)(lane / SUB) << 32);
+                                        rec[32] = (unsigned long long)__double_as_longlong(fabs(S.gm[jj]));
+                                        rec[64] = (unsigned long long)__double_as_longlong(fmax(bnd_i, __ldcg(Gm.rcsq + jg)));
+                                        for (int k = 0; k < nlevels; k++)
+                                            rec[96 + 32 * k] = (unsigned long long)__double_as_longlong(fmax(rci[k], __ldcg(Gm.rc[k] + jg)));
+                                    }
                                     c[u]++;
                                 }
                             }
@@ -452,15 +534,29 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
             }
         }
         if (pass) break;
-        unsigned long long total = 0;
+        int total = 0;
 #pragma unroll
-        for (int u = 0; u < NL; u++) { L.count[u] = c[u]; total += (unsigned long long)c[u]; }
-        unsigned long long base = total ? atomicAdd(Gm.cursor, total) : 0ULL;
+        for (int u = 0; u < NL; u++) { cnt[u] = c[u]; total += c[u]; }
+        int incl = total;                                         // inclusive scan over the warp's lanes
 #pragma unroll
-        for (int u = 0; u < NL; u++) { L.base[u] = (long long)base; base += (unsigned long long)c[u]; }
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += up;
+        }
+        wtotal = __shfl_sync(0xffffffffu, incl, 31);
+        lane_off = incl - total;
+        const int chunks = (wtotal + 31) >> 5;
+        unsigned long long wb = 0ULL;
+        if (lane == 0 && chunks) wb = atomicAdd(Gm.cursor, (unsigned long long)chunks);
+        L.wbase = (long long)__shfl_sync(0xffffffffu, wb, 0);
+        L.wchunks = chunks;
         bs_gsync(S, Gm);
-        if (__ldcg(Gm.cursor) > (unsigned long long)Gm.nbr_capacity) return;    // team-uniform: all pairs instead
+        // team-uniform: all pairs instead if the lists do not fit
+        if (__ldcg(Gm.cursor) * (unsigned long long)cw > (unsigned long long)(Gm.nbr_capacity / 2)) { L.wchunks = 0; return; }
     }
+    // padding at the end of the warp's last chunk: entries that belong to no body
+    for (int e = wtotal + lane; e < 32 * L.wchunks; e += 32)
+        words[(L.wbase + (e >> 5)) * cw + (e & 31)] = 0xffffffffULL | (32ULL << 32);
     L.on = true;
 }
 
@@ -584,7 +680,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
 #pragma unroll
         for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) Gm.rc[k] += off;
         Gm.err += 16 * team; Gm.cursor = Gm.err + 4; Gm.bar = Gm.err + 5;
-        Gm.nbr_capacity = Gm.nbr_capacity / n_teams;
+        Gm.nbr_capacity = (Gm.nbr_capacity / n_teams) & ~3LL;     // (a team's slice starts on a 16-byte boundary)
         Gm.nbr += (long long)team * Gm.nbr_capacity;
         if (threadIdx.x == 0) S.bar_target = 0ULL;
     }
@@ -658,7 +754,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         //  the previous group's last readers passed a grid barrier -- its last error check -- before anyone gets here)
         BsList<8 / SUB> L;
         L.on = false;
-        if (COOP) bs_build_lists<ROWS, SUB>(S, Gm, eval, i, n, i_tp, tp_mode, q, v, rci[0], dt, mu, L);
+        if (COOP) bs_build_lists<ROWS, SUB>(S, Gm, eval, i, n, i_tp, tp_mode, q, v, rci, nlevels, dt, mu, L);
         double Pq[GENGA_BS_KMAX][3], Pv[GENGA_BS_KMAX][3];             // P[j] = T_{k-1,j} of the extrapolation tableau
         double a0[3], cq[3], cv[3], dq[3], dv[3];
         double done = 0.0, H = dt;
