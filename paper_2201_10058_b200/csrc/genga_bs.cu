@@ -124,7 +124,7 @@ extern "C" int genga_bs(genga_kick_ctx* ctx, const double* pos_in, const double*
         void* k8 = reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, GENGA_BS_SUB>);
         void* k1 = reinterpret_cast<void*>(genga::bs_kernel<GENGA_BS_MODE_COOP, GENGA_BS_COOP_THREADS, 1>);
         small_max = GENGA_BS_THREADS;
-        for (int mult = 1; mult <= 4; mult *= 4) {                          // teams of 64 and of 256 CTAs
+        for (int mult = 1; mult <= 4; mult *= 4) {                          // teams of 16 and of 64 CTAs (4096 and 16,384 lanes)
             const int tctas = GENGA_BS_TEAM_CTAS * mult, teams = ctx->bs_coop_blocks / tctas;
             const int cap = tctas * GENGA_BS_COOP_THREADS / GENGA_BS_SUB;
             if (teams < 2 || N <= small_max) continue;

@@ -41,11 +41,11 @@ namespace genga {
 #define GENGA_BS_SEQ_MAX 8              // largest group of the warp-per-group regime (force sum in member order)
 #define GENGA_BS_CTA_MAX 32             // largest group of the one-CTA regime = GENGA_BS_THREADS / GENGA_BS_SUB
 #define GENGA_BS_THREADS 256            // CTA of the one-CTA-per-group regime = largest group it takes
-#define GENGA_BS_COOP_THREADS 64        // CTA of the whole-grid regime
+#define GENGA_BS_COOP_THREADS 256       // CTA of the whole-grid regime (its bodies' lists are pooled: bs_build_lists)
 #define GENGA_BS_SUB 8                  // whole-grid regime: lanes per body, each summing the terms with j = lane (mod 8)
                                         // (groups too large for that: one lane per body, the same eight partial sums)
-#define GENGA_BS_TILE 64                // j-bodies staged per round in the whole-grid regime
-#define GENGA_BS_TEAM_CTAS 64            // whole-grid regime in teams: CTAs of the small teams (512 bodies at eight lanes each)
+#define GENGA_BS_TILE 256               // j-bodies staged per round in the whole-grid regime
+#define GENGA_BS_TEAM_CTAS 16           // whole-grid regime in teams: CTAs of the small teams (512 bodies at eight lanes each)
 #define GENGA_BS_KMAX 8
 #define GENGA_BS_MAX_LEVELS 4
 #define GENGA_BS_MAX_HALVINGS 60
@@ -204,21 +204,58 @@ __device__ __noinline__ bool bs_pair_factor(double r2, double gmj, int nlevels, 
 template <int NL>
 struct BsList {
     bool on;                            // lists in use for this group (team-uniform)
-    long long wbase;                    // this WARP's list: first chunk (warp-uniform) ...
-    int wchunks;                        // ... and number of chunks of 32 entries
+    long long cbase;                    // this CTA's list: first chunk (CTA-uniform) ...
+    int cchunks;                        // ... and number of chunks of 32 entries
     double q0[3], v0[3];                // the body's state at the start of the call
     double a2;                          // A_b^2
+    double gmi;                         // G m_b (published with the position: what a partner's walk needs of this body)
 };
 
-// A chunk of a warp's list: 32 entries, field by field (every load of the walk is one coalesced 256-byte row):
-//   row 0       (j, slot) -- the partner's position within the group (-1: padding) and which of the warp's bodies the
-//               entry belongs to (lane / SUB of its lanes); the entries of a warp are sorted by slot
-//   row 1       G m_j
-//   row 2       max(bound_i, bound_j), the far-pair bound of the pair (bs_far_bound)
-//   row 3 + k   max(rc_k,i, rc_k,j), k < nlevels
+// A chunk of a CTA's list: 32 entries, field by field (every load of the walk is one coalesced 256-byte row):
+//   row 0       (j, slot) -- the partner's position within the group (-1: padding) and which of the CTA's bodies the
+//               entry belongs to (thread / SUB of its lanes); the entries of a CTA are sorted by slot
+//   row 1       max(bound_i, bound_j), the far-pair bound of the pair (bs_far_bound)
+//   row 2 + k   1 / (0.9 max(rc_k,i, rc_k,j)), k < nlevels: y_k = r / (0.9 rc) - 1/9 (bs_pair_factor_listed)
 // i.e. everything about the pair that does not change during the call: a force evaluation reads the entry and ONE
-// 32-byte record of the partner's current position.
-__device__ __forceinline__ int bs_chunk_words(int nlevels) { return 32 * (3 + nlevels); }
+// 32-byte record of the partner, (x, y), (z, G m), at its current position.
+__device__ __forceinline__ int bs_chunk_words(int nlevels) { return 32 * (2 + nlevels); }
+
+// The factor s = G m_j prod_k (1 - K(r; rc_k)) / r^3 of a listed pair inside its far-pair bound, with the quantities
+// the list holds.  1 - K(y) = (1 - y)^2 / (2 y^2 - 2 y + 1) (reading G1), so the product over the
+// levels is one quotient; 1/r comes from the MUFU.RSQ64H seed and a third-order correction (relative error < 2^-58), the
+// reciprocal of the denominator from the MUFU.RCP64H seed and two Newton steps: ~35 FP64 instructions where the
+// literal evaluation (a square root, two divisions per level, one for the term) takes ~450.  The same function of
+// (r, rc_k) as bs_K up to a few units in the last place of each factor -- the whole-grid regime's force sum differs
+// from the oracle's by its order already (reading G15); the parity bound of tests/test_gpu_bs.py has room for 1e-12.
+// false: some level has y_k >= 1, the pair adds nothing.
+__device__ __forceinline__ bool bs_pair_factor_listed(double r2, double gmj, int nlevels, double b0, double b1, double b2,
+                                                      double b3, double& s)
+{
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
+    const double e = fma(-r2, y0 * y0, 1.0);
+    const double rinv = y0 * fma(e, fma(0.375, e, 0.5), 1.0);
+    const double r = r2 * rinv;
+    double num = 1.0, den = 1.0;
+    const double bk[GENGA_BS_MAX_LEVELS] = {b0, b1, b2, b3};
+#pragma unroll
+    for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++)
+        if (k < nlevels) {
+            const double y = fma(r, bk[k], -0.1111111111111111);
+            if (y >= 1.0) return false;
+            if (y > 0.0) {
+                const double omy = 1.0 - y;
+                num = num * (omy * omy);
+                den = den * fma(2.0 * y, y - 1.0, 1.0);
+            }
+        }
+    double x;                                                   // 1 / den, den in (2^-4, 1]
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(den));
+    x = fma(x, fma(-den, x, 1.0), x);
+    x = fma(x, fma(-den, x, 1.0), x);
+    s = ((gmj * num) * x) * ((rinv * rinv) * rinv);
+    return true;
+}
 
 // Every thread publishes the position of its body i (if i < n) and gets dv_i/dt back:
 //   - G m_star q / |q|^3 + the pair terms over j = 0 .. n-1, j != i, in that order.
@@ -320,16 +357,21 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
         const int t = threadIdx.x, sub = t & (SUB - 1);
         if (i < n && sub == 0) {
             Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z;
-            if (L.on) { Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bnd_i); }
+            if (L.on) { Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, L.gmi); }
         }
-        // the warp's bodies, for the lanes that walk their entries: current positions and the accumulators
-        constexpr int WB = 32 / SUB;
-        __shared__ double wpos[GENGA_BS_COOP_THREADS / 32][WB][3];
-        __shared__ double wacc[GENGA_BS_COOP_THREADS / 32][WB][3];
+        // the CTA's bodies, for the lanes that walk their entries: current positions and the accumulators
+        constexpr int WB = GENGA_BS_COOP_THREADS / SUB, NW = GENGA_BS_COOP_THREADS / 32;
+        __shared__ double wpos[WB][3];
+        __shared__ double wacc[WB][3];
+        __shared__ double wcarry[NW][3];                                // a warp's terms of the body its range starts inside
+        __shared__ int wcarry_slot[NW];                                 // ... and which body that is (-1: none)
         const int lane = t & 31, wid = t >> 5;
-        if (L.on && sub == 0) {
-            wpos[wid][lane / SUB][0] = x; wpos[wid][lane / SUB][1] = y; wpos[wid][lane / SUB][2] = z;
-            wacc[wid][lane / SUB][0] = 0.0; wacc[wid][lane / SUB][1] = 0.0; wacc[wid][lane / SUB][2] = 0.0;
+        if (L.on) {
+            if (sub == 0) {
+                wpos[t / SUB][0] = x; wpos[t / SUB][1] = y; wpos[t / SUB][2] = z;
+                wacc[t / SUB][0] = 0.0; wacc[t / SUB][1] = 0.0; wacc[t / SUB][2] = 0.0;
+            }
+            if (lane == 0) { wcarry[wid][0] = 0.0; wcarry[wid][1] = 0.0; wcarry[wid][2] = 0.0; wcarry_slot[wid] = -1; }
         }
         bs_gsync(S, Gm);
         const double sx = ax, sy = ay, sz = az;
@@ -342,27 +384,49 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
                 const double ex = x - (L.q0[0] + L.v0[0] * tau), ey = y - (L.q0[1] + L.v0[1] * tau), ez = z - (L.q0[2] + L.v0[2] * tau);
                 if (ex * ex + ey * ey + ez * ez > L.a2) atomicOr(status, GENGA_STATUS_BS_LIST_ESCAPE);
             }
+            // warp w walks the chunks [w C / 8, (w + 1) C / 8) of the CTA's list (sorted by body): the bodies of its range
+            // are its own but for the first, which may have begun in the range of the warp before
             const int cw = bs_chunk_words(nlevels);
-            const unsigned long long* rec = reinterpret_cast<const unsigned long long*>(Gm.nbr) + L.wbase * cw + lane;
-            for (int c = 0; c < L.wchunks; c++, rec += cw) {
-                const unsigned long long js = __ldcg(rec);
-                const int jj = (int)(unsigned)(js & 0xffffffffULL), slot = (int)(js >> 32);
+            const int c0 = (int)((long long)wid * L.cchunks / NW), c1 = (int)((long long)(wid + 1) * L.cchunks / NW);
+            const unsigned long long* rec = reinterpret_cast<const unsigned long long*>(Gm.nbr) + (L.cbase + c0) * cw + lane;
+            int prev_slot = -1;
+            if (c0 > 0 && c1 > c0) prev_slot = (int)(__ldcg(rec - lane - cw + 31) >> 32);     // (warp-uniform)
+            if (lane == 0) wcarry_slot[wid] = prev_slot;
+            // Three chunks in flight: while chunk c is evaluated, the partners' records of chunk c + 1 are on their way
+            // (their indices arrived during chunk c - 1) and so are the indices of chunk c + 2.
+            constexpr unsigned long long PAD = 0xffffffffULL | (0x7fffULL << 32);
+            unsigned long long jsA = PAD, jsB = PAD, jsC = PAD;             // entries of chunk c + 2, c + 1, c
+            double bndB = 0.0, bB[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
+            double2 paB = make_double2(0.0, 0.0), pbB = make_double2(0.0, 0.0);
+            double bndC = 0.0, bC[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
+            double2 paC = make_double2(0.0, 0.0), pbC = make_double2(0.0, 0.0);
+            for (int c = c0 - 2; c < c1; c++) {
+                // the oldest stage moves on
+                jsC = jsB; bndC = bndB; paC = paB; pbC = pbB;
+#pragma unroll
+                for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) bC[k] = bB[k];
+                jsB = jsA;
+                jsA = c + 2 < c1 ? __ldcg(rec + (long long)(c + 2 - c0) * cw) : PAD;
+                {   // chunk c + 1: its constants and the partners' records
+                    const int jb = (int)(unsigned)(jsB & 0xffffffffULL);
+                    if (jb >= 0) {
+                        const unsigned long long* rb = rec + (long long)(c + 1 - c0) * cw;
+                        bndB = __longlong_as_double((long long)__ldcg(rb + 32));
+#pragma unroll
+                        for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++)
+                            if (k < nlevels) bB[k] = __longlong_as_double((long long)__ldcg(rb + 64 + 32 * k));
+                        paB = __ldcg(Gm.pk[p] + 2 * jb); pbB = __ldcg(Gm.pk[p] + 2 * jb + 1);
+                    }
+                }
+                if (c < c0) continue;                                   // (warp-uniform: the pipeline is filling)
+                const int jj = (int)(unsigned)(jsC & 0xffffffffULL), slot = (int)(jsC >> 32);
                 double tx = 0.0, ty = 0.0, tz = 0.0;
                 if (jj >= 0) {
-                    const double gmj = __longlong_as_double((long long)__ldcg(rec + 32));
-                    const double bnd = __longlong_as_double((long long)__ldcg(rec + 64));
-                    const double2 pa = __ldcg(Gm.pk[p] + 2 * jj), pb = __ldcg(Gm.pk[p] + 2 * jj + 1);
-                    const double dx = pa.x - wpos[wid][slot][0], dy = pa.y - wpos[wid][slot][1], dz = pb.x - wpos[wid][slot][2];
+                    const double dx = paC.x - wpos[slot][0], dy = paC.y - wpos[slot][1], dz = pbC.x - wpos[slot][2];
                     const double r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 < bnd) {
-                        const double rc0 = __longlong_as_double((long long)__ldcg(rec + 96));
-                        const double rc1 = 1 < nlevels ? __longlong_as_double((long long)__ldcg(rec + 128)) : 0.0;
-                        const double rc2 = 2 < nlevels ? __longlong_as_double((long long)__ldcg(rec + 160)) : 0.0;
-                        const double rc3 = 3 < nlevels ? __longlong_as_double((long long)__ldcg(rec + 192)) : 0.0;
-                        double sfac;
-                        if (bs_pair_factor(r2, gmj, nlevels, rc0, rc1, rc2, rc3, 0.0, 0.0, 0.0, 0.0, sfac)) {
-                            tx = sfac * dx; ty = sfac * dy; tz = sfac * dz;
-                        }
+                    double sfac;
+                    if (r2 < bndC && bs_pair_factor_listed(r2, pbC.y, nlevels, bC[0], bC[1], bC[2], bC[3], sfac)) {
+                        tx = sfac * dx; ty = sfac * dy; tz = sfac * dz;
                     }
                 }
                 // sum of each body's terms of this chunk: inclusive scan over the lanes within runs of equal slot
@@ -375,14 +439,18 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
                 }
                 const int snext = __shfl_down_sync(0xffffffffu, slot, 1);
                 if (slot < WB && (lane == 31 || snext != slot)) {      // the last lane of a run holds its sum
-                    wacc[wid][slot][0] = wacc[wid][slot][0] + tx;
-                    wacc[wid][slot][1] = wacc[wid][slot][1] + ty;
-                    wacc[wid][slot][2] = wacc[wid][slot][2] + tz;
+                    double* acc = slot == prev_slot ? wcarry[wid] : wacc[slot];
+                    acc[0] = acc[0] + tx; acc[1] = acc[1] + ty; acc[2] = acc[2] + tz;
                 }
                 __syncwarp();                                           // the next chunk may continue the run in another lane
             }
-            px[0] = wacc[wid][lane / SUB][0]; py[0] = wacc[wid][lane / SUB][1]; pz[0] = wacc[wid][lane / SUB][2];
-            __syncwarp();                                               // (before the next evaluation clears them)
+            __syncthreads();
+            // a body's sum: what the warp that met its first entry gathered, then the carries of the warps after it, in order
+            px[0] = wacc[t / SUB][0]; py[0] = wacc[t / SUB][1]; pz[0] = wacc[t / SUB][2];
+#pragma unroll
+            for (int w = 1; w < NW; w++)
+                if (wcarry_slot[w] == t / SUB) { px[0] = px[0] + wcarry[w][0]; py[0] = py[0] + wcarry[w][1]; pz[0] = pz[0] + wcarry[w][2]; }
+            __syncthreads();                                            // (before the next evaluation clears them)
         }
         for (int j0 = 0; j0 < (L.on ? 0 : n); j0 += ROWS) {   // ROWS is a multiple of 8: (j0 + jj) mod 8 = jj mod 8
             __syncthreads();
@@ -436,9 +504,9 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
 }
 
 // Whole-grid regime, start of a group: publishes the bodies' starting positions, R_b and D_b, counts and fills the
-// warps' lists (two scans of the group, tile by tile through shared memory: a lane scans for its body the partners
-// j = sub, sub + SUB, .. (mod 8); a warp reserves the chunks of its list with one atomic on a cursor -- where a list
-// lies is irrelevant; within it the entries are in the order lane, residue class of j, ascending j).
+// CTAs' lists (two scans of the group, tile by tile through shared memory: a lane scans for its body the partners
+// j = sub, sub + SUB, .. (mod 8); a CTA reserves the chunks of its list with one atomic on a cursor -- where a list
+// lies is irrelevant; within it the entries are in the order thread, residue class of j, ascending j).
 // Two grid barriers; the positions go to buffer eval & 1 like a force evaluation's.
 template <int ROWS, int SUB>
 __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal& Gm, int& eval, int i, int n, bool i_tp,
@@ -459,20 +527,24 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
     L.q0[0] = x; L.q0[1] = y; L.q0[2] = z;
     L.v0[0] = v[0]; L.v0[1] = v[1]; L.v0[2] = v[2];
     L.a2 = la_i * la_i;
+    L.gmi = i < n ? fabs(__ldcg(Gm.gm + i)) : 0.0;               // (written by this body's first lane at the start of the group:
+    L.gmi = __shfl_sync(0xffffffffu, L.gmi, (t & 31) & ~(SUB - 1));  //  the other lanes of the body take it from that lane)
     if (i < n && sub == 0) {
         Gm.x[p][i] = x; Gm.y[p][i] = y; Gm.z[p][i] = z;
-        Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, bnd_i);
+        Gm.pk[p][2 * i] = make_double2(x, y); Gm.pk[p][2 * i + 1] = make_double2(z, L.gmi);
         Gm.vx[i] = v[0]; Gm.vy[i] = v[1]; Gm.vz[i] = v[2];
         Gm.lr[i] = lr_i; Gm.la[i] = la_i; Gm.ld[i] = ld_i;
     }
     if (Gm.tb == 0 && t == 0) *Gm.cursor = 0ULL;            // (its last readers passed several barriers ago)
     bs_gsync(S, Gm);
-    L.wbase = 0; L.wchunks = 0;
+    L.cbase = 0; L.cchunks = 0;
     L.on = false;
+    __shared__ int wtot[GENGA_BS_COOP_THREADS / 32];
+    __shared__ long long cta_base;
     const int cw = bs_chunk_words(nlevels);
     unsigned long long* const words = reinterpret_cast<unsigned long long*>(Gm.nbr);
     int cnt[NL];                                              // pass 0: entries of each of the lane's residue classes
-    int lane_off = 0, wtotal = 0;                             // the lane's first entry within the warp's list; its length
+    int lane_off = 0, ctotal = 0;                             // the lane's first entry within the CTA's list; its length
 #pragma unroll
     for (int u = 0; u < NL; u++) cnt[u] = 0;
     for (int pass = 0; pass < 2; pass++) {                    // 0: count, 1: fill
@@ -513,17 +585,17 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
                                 // (1 + 2^-30: the roundings of this test must not drop a pair the exact test keeps)
                                 if (cx * cx + cy * cy + cz * cz < (Ra * Ra) * (1.0 + 9.313225746154785e-10)) {
                                     if (pass) {
-                                        int e = lane_off + c[u];              // entry within the warp's list
+                                        int e = lane_off + c[u];              // entry within the CTA's list
 #pragma unroll
                                         for (int w = 0; w < NL; w++)
                                             if (w < u) e += cnt[w];
                                         const int jg = j0 + jj;
-                                        unsigned long long* rec = words + (L.wbase + (e >> 5)) * cw + (e & 31);
-                                        rec[0] = (unsigned long long)(unsigned)jg | ((unsigned long long)(unsigned)(lane / SUB) << 32);
-                                        rec[32] = (unsigned long long)__double_as_longlong(fabs(S.gm[jj]));
-                                        rec[64] = (unsigned long long)__double_as_longlong(fmax(bnd_i, __ldcg(Gm.rcsq + jg)));
+                                        unsigned long long* rec = words + (L.cbase + (e >> 5)) * cw + (e & 31);
+                                        rec[0] = (unsigned long long)(unsigned)jg | ((unsigned long long)(unsigned)(t / SUB) << 32);
+                                        rec[32] = (unsigned long long)__double_as_longlong(fmax(bnd_i, __ldcg(Gm.rcsq + jg)));
                                         for (int k = 0; k < nlevels; k++)
-                                            rec[96 + 32 * k] = (unsigned long long)__double_as_longlong(fmax(rci[k], __ldcg(Gm.rc[k] + jg)));
+                                            rec[64 + 32 * k] = (unsigned long long)__double_as_longlong(
+                                                1.0 / (0.9 * fmax(rci[k], __ldcg(Gm.rc[k] + jg))));
                                     }
                                     c[u]++;
                                 }
@@ -537,26 +609,34 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
         int total = 0;
 #pragma unroll
         for (int u = 0; u < NL; u++) { cnt[u] = c[u]; total += c[u]; }
-        int incl = total;                                         // inclusive scan over the warp's lanes
+        int incl = total;                                         // inclusive scan over the CTA's threads
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int up = __shfl_up_sync(0xffffffffu, incl, o);
             if (lane >= o) incl += up;
         }
-        wtotal = __shfl_sync(0xffffffffu, incl, 31);
-        lane_off = incl - total;
-        const int chunks = (wtotal + 31) >> 5;
-        unsigned long long wb = 0ULL;
-        if (lane == 0 && chunks) wb = atomicAdd(Gm.cursor, (unsigned long long)chunks);
-        L.wbase = (long long)__shfl_sync(0xffffffffu, wb, 0);
-        L.wchunks = chunks;
+        __syncthreads();
+        if (lane == 31) wtot[t >> 5] = incl;
+        __syncthreads();
+        int before = 0;
+        ctotal = 0;
+#pragma unroll
+        for (int w = 0; w < GENGA_BS_COOP_THREADS / 32; w++) {
+            if (w < (t >> 5)) before += wtot[w];
+            ctotal += wtot[w];
+        }
+        lane_off = before + incl - total;
+        const int chunks = (ctotal + 31) >> 5;
+        if (t == 0) cta_base = chunks ? (long long)atomicAdd(Gm.cursor, (unsigned long long)chunks) : 0LL;
         bs_gsync(S, Gm);
+        L.cbase = cta_base;
+        L.cchunks = chunks;
         // team-uniform: all pairs instead if the lists do not fit
-        if (__ldcg(Gm.cursor) * (unsigned long long)cw > (unsigned long long)(Gm.nbr_capacity / 2)) { L.wchunks = 0; return; }
+        if (__ldcg(Gm.cursor) * (unsigned long long)cw > (unsigned long long)(Gm.nbr_capacity / 2)) { L.cchunks = 0; return; }
     }
-    // padding at the end of the warp's last chunk: entries that belong to no body
-    for (int e = wtotal + lane; e < 32 * L.wchunks; e += 32)
-        words[(L.wbase + (e >> 5)) * cw + (e & 31)] = 0xffffffffULL | (32ULL << 32);
+    // padding at the end of the CTA's last chunk: entries that belong to no body
+    for (int e = ctotal + t; e < 32 * L.cchunks; e += GENGA_BS_COOP_THREADS)
+        words[(L.cbase + (e >> 5)) * cw + (e & 31)] = 0xffffffffULL | (0x7fffULL << 32);
     L.on = true;
 }
 
@@ -861,7 +941,7 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
 template <int MODE, int THREADS, int SUB = 1>
 // (8 CTAs of 64 threads per SM whatever the variant: the capacities of the whole-grid regime -- 9472 bodies at eight
 // lanes each on 148 SMs, twice that at four, .. -- must not move with the register allocator's mood)
-__global__ void __launch_bounds__(THREADS, 8) bs_kernel(GENGA_BS_ARGS)
+__global__ void __launch_bounds__(THREADS, 512 / THREADS) bs_kernel(GENGA_BS_ARGS)
 {
     bs_run<MODE, THREADS, SUB>(GENGA_BS_PASS, (int)blockIdx.x, (int)gridDim.x);
 }
