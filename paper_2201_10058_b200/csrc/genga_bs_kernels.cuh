@@ -393,39 +393,34 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
             if (c0 > 0 && c1 > c0) prev_slot = (int)(__ldcg(rec - lane - cw + 31) >> 32);     // (warp-uniform)
             if (lane == 0) wcarry_slot[wid] = prev_slot;
             // Three chunks in flight: while chunk c is evaluated, the partners' records of chunk c + 1 are on their way
-            // (their indices arrived during chunk c - 1) and so are the indices of chunk c + 2.
+            // (their indices arrived during chunk c - 1) and so are the indices of chunk c + 2.  Two register sets take
+            // the partners' records in turn (no copies between the stages).
             constexpr unsigned long long PAD = 0xffffffffULL | (0x7fffULL << 32);
-            unsigned long long jsA = PAD, jsB = PAD, jsC = PAD;             // entries of chunk c + 2, c + 1, c
-            double bndB = 0.0, bB[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
-            double2 paB = make_double2(0.0, 0.0), pbB = make_double2(0.0, 0.0);
-            double bndC = 0.0, bC[GENGA_BS_MAX_LEVELS] = {0.0, 0.0, 0.0, 0.0};
-            double2 paC = make_double2(0.0, 0.0), pbC = make_double2(0.0, 0.0);
-            for (int c = c0 - 2; c < c1; c++) {
-                // the oldest stage moves on
-                jsC = jsB; bndC = bndB; paC = paB; pbC = pbB;
+            struct Stage { double bnd, b[GENGA_BS_MAX_LEVELS]; double2 pa, pb; };
+            Stage s0, s1;
+            s0.bnd = 0.0; s0.pa = make_double2(0.0, 0.0); s0.pb = s0.pa;
 #pragma unroll
-                for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) bC[k] = bB[k];
-                jsB = jsA;
-                jsA = c + 2 < c1 ? __ldcg(rec + (long long)(c + 2 - c0) * cw) : PAD;
-                {   // chunk c + 1: its constants and the partners' records
-                    const int jb = (int)(unsigned)(jsB & 0xffffffffULL);
-                    if (jb >= 0) {
-                        const unsigned long long* rb = rec + (long long)(c + 1 - c0) * cw;
-                        bndB = __longlong_as_double((long long)__ldcg(rb + 32));
+            for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++) s0.b[k] = 0.0;
+            s1 = s0;
+            const double2* const pkp = Gm.pk[p];
+            auto gather = [&](Stage& g, unsigned long long js, const unsigned long long* rb) {
+                const int jb = (int)(unsigned)(js & 0xffffffffULL);
+                if (jb >= 0) {
+                    g.bnd = __longlong_as_double((long long)__ldcg(rb + 32));
 #pragma unroll
-                        for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++)
-                            if (k < nlevels) bB[k] = __longlong_as_double((long long)__ldcg(rb + 64 + 32 * k));
-                        paB = __ldcg(Gm.pk[p] + 2 * jb); pbB = __ldcg(Gm.pk[p] + 2 * jb + 1);
-                    }
+                    for (int k = 0; k < GENGA_BS_MAX_LEVELS; k++)
+                        if (k < nlevels) g.b[k] = __longlong_as_double((long long)__ldcg(rb + 64 + 32 * k));
+                    g.pa = __ldcg(pkp + 2 * jb); g.pb = __ldcg(pkp + 2 * jb + 1);
                 }
-                if (c < c0) continue;                                   // (warp-uniform: the pipeline is filling)
-                const int jj = (int)(unsigned)(jsC & 0xffffffffULL), slot = (int)(jsC >> 32);
+            };
+            auto evaluate = [&](const Stage& g, unsigned long long js) {
+                const int jj = (int)(unsigned)(js & 0xffffffffULL), slot = (int)(js >> 32);
                 double tx = 0.0, ty = 0.0, tz = 0.0;
                 if (jj >= 0) {
-                    const double dx = paC.x - wpos[slot][0], dy = paC.y - wpos[slot][1], dz = pbC.x - wpos[slot][2];
+                    const double dx = g.pa.x - wpos[slot][0], dy = g.pa.y - wpos[slot][1], dz = g.pb.x - wpos[slot][2];
                     const double r2 = dx * dx + dy * dy + dz * dz;
                     double sfac;
-                    if (r2 < bndC && bs_pair_factor_listed(r2, pbC.y, nlevels, bC[0], bC[1], bC[2], bC[3], sfac)) {
+                    if (r2 < g.bnd && bs_pair_factor_listed(r2, g.pb.y, nlevels, g.b[0], g.b[1], g.b[2], g.b[3], sfac)) {
                         tx = sfac * dx; ty = sfac * dy; tz = sfac * dz;
                     }
                 }
@@ -435,7 +430,10 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
                     const int so = __shfl_up_sync(0xffffffffu, slot, o);
                     const double ux = __shfl_up_sync(0xffffffffu, tx, o), uy = __shfl_up_sync(0xffffffffu, ty, o),
                                  uz = __shfl_up_sync(0xffffffffu, tz, o);
-                    if (lane >= o && so == slot) { tx = ux + tx; ty = uy + ty; tz = uz + tz; }
+                    const int take = (lane >= o && so == slot) ? 1 : 0;
+                    asm("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %6, 0;\n\t@q add.rn.f64 %0, %3, %0;\n\t@q add.rn.f64 %1, %4, %1;\n\t"
+                        "@q add.rn.f64 %2, %5, %2;\n\t}"
+                        : "+d"(tx), "+d"(ty), "+d"(tz) : "d"(ux), "d"(uy), "d"(uz), "r"(take));
                 }
                 const int snext = __shfl_down_sync(0xffffffffu, slot, 1);
                 if (slot < WB && (lane == 31 || snext != slot)) {      // the last lane of a run holds its sum
@@ -443,6 +441,19 @@ __device__ __forceinline__ void bs_force(BsShared<ROWS>& S, const BsGlobal& Gm, 
                     acc[0] = acc[0] + tx; acc[1] = acc[1] + ty; acc[2] = acc[2] + tz;
                 }
                 __syncwarp();                                           // the next chunk may continue the run in another lane
+            };
+            unsigned long long jsA = PAD, jsB = PAD, jsC = PAD;             // entries of chunk c + 2, c + 1, c
+            const unsigned long long* rA = rec;                             // row 0 of the chunk jsA is loaded from next
+            for (int c = c0 - 2; c < c1; c += 2) {
+                jsC = jsB; jsB = jsA;
+                jsA = c + 2 < c1 ? __ldcg(rA) : PAD;
+                gather(s0, jsB, rA - cw);                                   // chunk c + 1
+                if (c >= c0) evaluate(s1, jsC);                             // chunk c (warp-uniform condition)
+                jsC = jsB; jsB = jsA;
+                jsA = c + 3 < c1 ? __ldcg(rA + cw) : PAD;
+                gather(s1, jsB, rA);                                        // chunk c + 2
+                if (c + 1 >= c0 && c + 1 < c1) evaluate(s0, jsC);           // chunk c + 1
+                rA += 2 * cw;
             }
             __syncthreads();
             // a body's sum: what the warp that met its first entry gathered, then the carries of the warps after it, in order
@@ -541,6 +552,15 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
     L.on = false;
     __shared__ int wtot[GENGA_BS_COOP_THREADS / 32];
     __shared__ long long cta_base;
+    // FP32 copy of the staged tile for a first, conservative test (one 16-byte shared-memory load and ten FP32
+    // instructions per pair instead of six loads and FP64): (x, y, z, h), h_b >= R_b + D_b + the rounding of b's
+    // coordinates to FP32; a pair can only pass the exact tests below if |dq|_FP32 <= h_i + h_j (R = max(R_i, R_j) +
+    // D_i + D_j <= h_i + h_j).  The lists are those of the exact tests alone.
+    __shared__ float4 ftile[ROWS];
+    __shared__ double tvz[ROWS];                                 // the tile's velocities: S.rc[2], S.rc[3] and this
+    const float fxi = (float)x, fyi = (float)y, fzi = (float)z;
+    const float h_i = __fadd_ru(__fadd_ru(__double2float_ru(lr_i), __double2float_ru(ld_i)),
+                                __fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fxi), fabsf(fyi)), fabsf(fzi))));
     const int cw = bs_chunk_words(nlevels);
     unsigned long long* const words = reinterpret_cast<unsigned long long*>(Gm.nbr);
     int cnt[NL];                                              // pass 0: entries of each of the lane's residue classes
@@ -559,6 +579,11 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
                 S.rcsq[t] = __ldcg(Gm.lr + j0 + t);
                 S.rc[0][t] = __ldcg(Gm.ld + j0 + t);
                 S.rc[1][t] = __ldcg(Gm.la + j0 + t);
+                S.rc[2][t] = __ldcg(Gm.vx + j0 + t); S.rc[3][t] = __ldcg(Gm.vy + j0 + t); tvz[t] = __ldcg(Gm.vz + j0 + t);
+                const float fxj = (float)S.x[t], fyj = (float)S.y[t], fzj = (float)S.z[t];
+                ftile[t] = make_float4(fxj, fyj, fzj,
+                                       __fadd_ru(__fadd_ru(__double2float_ru(S.rcsq[t]), __double2float_ru(S.rc[0][t])),
+                                                 __fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fxj), fabsf(fyj)), fabsf(fzj)))));
             }
             __syncthreads();
             if (i < n) {
@@ -567,7 +592,11 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
 #pragma unroll
                     for (int u = 0; u < NL; u++) {
                         const int jj = j8 + sub + SUB * u;
-                        if (jj < m && j0 + jj != i) {
+                        if (jj >= m) continue;
+                        const float4 fj = ftile[jj];
+                        const float ex = fj.x - fxi, ey = fj.y - fyi, ez = fj.z - fzi, hh = __fadd_ru(fj.w, h_i);
+                        if (!(ex * ex + ey * ey + ez * ez <= __fmul_ru(__fmul_ru(hh, hh), 1.000002f))) continue;
+                        if (j0 + jj != i) {
                             const bool never = __double2hiint(S.gm[jj]) < 0 && (i_tp || tp_mode != 2);   // sec. 8.1
                             const double dx = S.x[jj] - x, dy = S.y[jj] - y, dz = S.z[jj] - z;
                             const double Rm = fmax(lr_i, S.rcsq[jj]);
@@ -575,8 +604,7 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
                             // first the cheap test on the displacement bounds (implied by the one below), then the
                             // closest approach of the straight-line relative motion over [0, dt]
                             if (!never && dx * dx + dy * dy + dz * dz < R * R) {
-                                const double wx = __ldcg(Gm.vx + j0 + jj) - v[0], wy = __ldcg(Gm.vy + j0 + jj) - v[1],
-                                             wz = __ldcg(Gm.vz + j0 + jj) - v[2];
+                                const double wx = S.rc[2][jj] - v[0], wy = S.rc[3][jj] - v[1], wz = tvz[jj] - v[2];
                                 const double w2 = wx * wx + wy * wy + wz * wz, dw = dx * wx + dy * wy + dz * wz;
                                 double ts = w2 > 0.0 ? -dw / w2 : 0.0;            // unconstrained closest approach
                                 ts = dt > 0.0 ? fmin(fmax(ts, 0.0), dt) : fmax(fmin(ts, 0.0), dt);
