@@ -792,7 +792,9 @@ bs_run(const double* __restrict__ pos_in, const double* __restrict__ vel_in, con
         Gm.nbr += (long long)team * Gm.nbr_capacity;
         if (threadIdx.x == 0) S.bar_target = 0ULL;
     }
-    const int i = COOP ? (int)((Gm.tb * THREADS + t) / SUB) : (CLUSTER ? (crank * THREADS + t) / SUB : (CTA ? t / SUB : t));
+    // (whole-grid regime: the group's bodies are dealt round the team's CTAs, body i to CTA i mod tctas: every CTA of the
+    // team gets its share whatever the group's size)
+    const int i = COOP ? (t / SUB) * tctas + Gm.tb : (CLUSTER ? (crank * THREADS + t) / SUB : (CTA ? t / SUB : t));
     const bool writer = WARP || (t & (SUB - 1)) == 0;
     const long long capacity = COOP ? (long long)tctas * THREADS / SUB : ROWS;
     const int n_groups = summary[0];
