@@ -22,16 +22,21 @@
  * BS-B of Table 2); 33 .. 256 bodies: one thread-block cluster (8 x 256 threads) per group, eight
  * lanes per body, positions exchanged through distributed shared memory (BS-A); many groups side by side.  From 9
  * bodies on the force sum of a body is taken in eight interleaved partial sums combined in a fixed tree (the oracle
- * states the order).  Larger groups: cooperative launches of co-resident thread blocks, eight lanes per body, positions
- * exchanged through L2 with one barrier per force evaluation (the paper's BS-M regime, with the
- * sub-steps kept on the device instead of controlled from the host): groups of up to 512 and of up to 2048 bodies
- * several at a time (the grid cut into teams of 64 / 256 blocks, a team per group with a barrier of its own), larger
- * ones one after the other over the whole grid -- with 8, 4, 2 or 1 lanes per body as the grid holds them (9472 /
+ * states the order).  Larger groups: cooperative launches of co-resident thread blocks of 256 threads, eight lanes per
+ * body, positions exchanged through L2 with one barrier per force evaluation (the paper's BS-M regime, PAPER.md:595-597,
+ * with the sub-steps kept on the device instead of controlled from the host): groups of up to 512 and of up to 2048
+ * bodies several at a time (the grid cut into teams of 16 / 64 blocks, a team per group with a barrier of its own),
+ * larger ones one after the other over the whole grid -- with 8, 4, 2 or 1 lanes per body as the grid holds them (9472 /
  * 18,944 / 37,888 / 75,776 bodies on 148 SMs); beyond that GENGA_KICK_STATUS_GROUP_TOO_LARGE is set and the group keeps
  * the state already in pos / vel.  In these regimes a body only evaluates the partners on its NEIGHBOUR LIST (built at
  * the start of the group from the straight-line relative motion over dt; a pair outside the lists stays outside every
- * critical radius and contributes exactly 0, as in the all-pairs sum: same bits, n x a few terms instead of n^2 per
- * force evaluation), and a pair with r^2 >= rc0^2 (1 + 2^-20) is dismissed after 8 FP64 instructions in every regime.
+ * critical radius and contributes exactly 0, as in the all-pairs sum: n x a few terms instead of n^2 per force
+ * evaluation).  The lists of a block's bodies are pooled and walked by all its warps, 32 entries at a time; a listed
+ * pair's factor prod_k (1 - K_k) / r^3 is evaluated as one quotient, prod (1 - y_k)^2 / (r^3 prod (2 y_k^2 - 2 y_k + 1)),
+ * from reciprocal seeds refined to < 2^-58 (the same function of r and the radii as the literal form, a few units in the
+ * last place apart; the order of a body's sum is a fixed function of its list).  Groups whose lists do not fit the
+ * scratch take the all-pairs sum with the literal form.  A pair with r^2 >= rc0^2 (1 + 2^-20) is dismissed after 8 FP64
+ * instructions in every regime.
  *
  * Works on the context of genga_kick.h (its N, G, stream); only enqueues; all pointers are DEVICE pointers.
  */

@@ -552,15 +552,25 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
     L.on = false;
     __shared__ int wtot[GENGA_BS_COOP_THREADS / 32];
     __shared__ long long cta_base;
-    // FP32 copy of the staged tile for a first, conservative test (one 16-byte shared-memory load and ten FP32
-    // instructions per pair instead of six loads and FP64): (x, y, z, h), h_b >= R_b + D_b + the rounding of b's
-    // coordinates to FP32; a pair can only pass the exact tests below if |dq|_FP32 <= h_i + h_j (R = max(R_i, R_j) +
-    // D_i + D_j <= h_i + h_j).  The lists are those of the exact tests alone.
+    // FP32 copies of the staged tile for two conservative tests before the exact FP64 ones (which alone decide the
+    // lists): of ~300 bodies within reach of a body's displacement bounds in the dense group of configs[3], ~80 pass the
+    // FP32 closest-approach test, 77 are listed.  ftile = (x, y, z, h), h_b >= R_b + D_b + e_b, e_b >= the rounding of b's
+    // coordinates to FP32: a pair can only pass the exact tests if |dq|_FP32 <= h_i + h_j (R = max(R_i, R_j) + D_i + D_j
+    // <= h_i + h_j).  vtile = (v, A_b + e_b + f_b), f_b >= |dt| x the rounding of b's velocity; ltile = (R_b, f_b).
+    // The FP32 closest approach is taken at the FP32 minimiser ts of |dq + dv tau|: the true distance there exceeds the
+    // true minimum by at most |dv| |ts - tau*| <= sqrt(2 |dq| (f_i + f_j)) (the error of ts is that of dq.dv / dv.dv,
+    // and |dv| |ts| <= |dv| |dt|), which is added to the radius with the e's and f's; 1.001 covers the FP32 roundings.
     __shared__ float4 ftile[ROWS];
-    __shared__ double tvz[ROWS];                                 // the tile's velocities: S.rc[2], S.rc[3] and this
-    const float fxi = (float)x, fyi = (float)y, fzi = (float)z;
-    const float h_i = __fadd_ru(__fadd_ru(__double2float_ru(lr_i), __double2float_ru(ld_i)),
-                                __fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fxi), fabsf(fyi)), fabsf(fzi))));
+    __shared__ float4 vtile[ROWS];
+    __shared__ float2 ltile[ROWS];
+    __shared__ double tvz[ROWS];                                 // the tile's velocities in FP64: S.rc[2], S.rc[3] and this
+    const float fxi = (float)x, fyi = (float)y, fzi = (float)z, fvxi = (float)v[0], fvyi = (float)v[1], fvzi = (float)v[2];
+    const float fdt = (float)dt;
+    const float e_i = __fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fxi), fabsf(fyi)), fabsf(fzi)));
+    const float f_i = __fmul_ru(__fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fvxi), fabsf(fvyi)), fabsf(fvzi))),
+                                __fmul_ru(fabsf(fdt), 1.000001f));
+    const float h_i = __fadd_ru(__fadd_ru(__double2float_ru(lr_i), __double2float_ru(ld_i)), e_i);
+    const float lrf_i = __double2float_ru(lr_i), laf_i = __fadd_ru(__fadd_ru(__double2float_ru(la_i), e_i), f_i);
     const int cw = bs_chunk_words(nlevels);
     unsigned long long* const words = reinterpret_cast<unsigned long long*>(Gm.nbr);
     int cnt[NL];                                              // pass 0: entries of each of the lane's residue classes
@@ -581,21 +591,55 @@ __device__ __forceinline__ void bs_build_lists(BsShared<ROWS>& S, const BsGlobal
                 S.rc[1][t] = __ldcg(Gm.la + j0 + t);
                 S.rc[2][t] = __ldcg(Gm.vx + j0 + t); S.rc[3][t] = __ldcg(Gm.vy + j0 + t); tvz[t] = __ldcg(Gm.vz + j0 + t);
                 const float fxj = (float)S.x[t], fyj = (float)S.y[t], fzj = (float)S.z[t];
+                const float fvxj = (float)S.rc[2][t], fvyj = (float)S.rc[3][t], fvzj = (float)tvz[t];
+                const float e_j = __fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fxj), fabsf(fyj)), fabsf(fzj)));
+                const float f_j = __fmul_ru(__fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fvxj), fabsf(fvyj)), fabsf(fvzj))),
+                                            __fmul_ru(fabsf(fdt), 1.000001f));
                 ftile[t] = make_float4(fxj, fyj, fzj,
-                                       __fadd_ru(__fadd_ru(__double2float_ru(S.rcsq[t]), __double2float_ru(S.rc[0][t])),
-                                                 __fmul_ru(2.4e-7f, __fadd_ru(__fadd_ru(fabsf(fxj), fabsf(fyj)), fabsf(fzj)))));
+                                       __fadd_ru(__fadd_ru(__double2float_ru(S.rcsq[t]), __double2float_ru(S.rc[0][t])), e_j));
+                vtile[t] = make_float4(fvxj, fvyj, fvzj, __fadd_ru(__fadd_ru(__double2float_ru(S.rc[1][t]), e_j), f_j));
+                ltile[t] = make_float2(__double2float_ru(S.rcsq[t]), f_j);
             }
             __syncthreads();
             if (i < n) {
                 const int m = min(ROWS, n - j0);
-                for (int j8 = 0; j8 < m; j8 += 8) {
+                // First the FP32 test of the tile's bodies against this lane's, without a branch: one bit per body that
+                // passes (a lane meets a candidate in 2 % of its tests, a WARP in half of them: taking the tests and the
+                // follow-up of the hits in turn made every other test pay for a hit).  Then each lane's own hits.
+                static_assert(ROWS <= 256, "one bit per j8 round of a tile");
+                unsigned hits[NL];
+#pragma unroll
+                for (int u = 0; u < NL; u++) hits[u] = 0u;
+#pragma unroll 4
+                for (int j8 = 0; j8 < ROWS; j8 += 8) {
 #pragma unroll
                     for (int u = 0; u < NL; u++) {
                         const int jj = j8 + sub + SUB * u;
-                        if (jj >= m) continue;
+                        const float4 fj = ftile[jj];                          // (beyond m: stale, masked below)
+                        const float ex = fj.x - fxi, ey = fj.y - fyi, ez = fj.z - fzi, hh = __fadd_ru(fj.w, h_i);
+                        const bool hit = jj < m && ex * ex + ey * ey + ez * ez <= __fmul_ru(__fmul_ru(hh, hh), 1.000002f);
+                        hits[u] |= (hit ? 1u : 0u) << (j8 >> 3);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < NL; u++) {
+                    while (hits[u]) {
+                        const int jj = 8 * (__ffs(hits[u]) - 1) + sub + SUB * u;
+                        hits[u] &= hits[u] - 1u;
                         const float4 fj = ftile[jj];
                         const float ex = fj.x - fxi, ey = fj.y - fyi, ez = fj.z - fzi, hh = __fadd_ru(fj.w, h_i);
-                        if (!(ex * ex + ey * ey + ez * ez <= __fmul_ru(__fmul_ru(hh, hh), 1.000002f))) continue;
+                        {
+                            const float4 vj = vtile[jj];
+                            const float2 lj = ltile[jj];
+                            const float wxf = vj.x - fvxi, wyf = vj.y - fvyi, wzf = vj.z - fvzi;
+                            const float w2f = wxf * wxf + wyf * wyf + wzf * wzf, dwf = ex * wxf + ey * wyf + ez * wzf;
+                            float tsf = w2f > 0.0f ? __fdividef(-dwf, w2f) : 0.0f;
+                            tsf = fdt > 0.0f ? fminf(fmaxf(tsf, 0.0f), fdt) : fmaxf(fminf(tsf, 0.0f), fdt);
+                            const float cxf = ex + wxf * tsf, cyf = ey + wyf * tsf, czf = ez + wzf * tsf;
+                            const float raf = __fadd_ru(__fadd_ru(fmaxf(lrf_i, lj.x), __fadd_ru(laf_i, vj.w)),
+                                                        __fmul_ru(1.0001f, __fsqrt_ru(__fmul_ru(__fmul_ru(2.0f, hh), __fadd_ru(f_i, lj.y)))));
+                            if (!(cxf * cxf + cyf * cyf + czf * czf <= __fmul_ru(__fmul_ru(raf, raf), 1.001f))) continue;
+                        }
                         if (j0 + jj != i) {
                             const bool never = __double2hiint(S.gm[jj]) < 0 && (i_tp || tp_mode != 2);   // sec. 8.1
                             const double dx = S.x[jj] - x, dy = S.y[jj] - y, dz = S.z[jj] - z;
