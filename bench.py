@@ -58,7 +58,7 @@ FP64_LANES_PER_SM = 64           # 148 SMs x 64 lanes x 2
 # From the ncu captures of round 2 (profiles/ncu_r02a.md), per launch / per two-level step at N = 65,536 (rank 0's disk);
 # constants read off those captures, not measured in this run:
 NCU_DRAM_BYTES_PER_LAUNCH = 4204288        # kick_sym_kernel: dram__bytes_read.sum 2,497,536 + dram__bytes_write.sum 1,706,752
-NCU_EXECUTED_FLOPS_PER_STEP = 67817100000  # DADD + DMUL + 2 DFMA thread instructions of every kernel of one step (flops_r02a.csv)
+NCU_EXECUTED_FLOPS_PER_STEP = 67657959455  # DADD + DMUL + 2 DFMA thread instructions of every kernel of one step (flops_r02c.csv)
 
 
 def workload(rank: int):

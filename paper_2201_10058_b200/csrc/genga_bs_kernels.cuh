@@ -143,8 +143,8 @@ __device__ __forceinline__ double bs_far_bound(double rc0) { return (rc0 * rc0) 
 // two per level are ~400 instructions, and the force loops name a pair in up to a dozen places (lanes' sub-lists x
 // loads in flight, all-pairs fallback) -- inlined, the whole-grid kernels were 13,000 - 61,000 instructions long and
 // their list walk ran out of the instruction cache (12 us per near pair; profiles/ncu_r02c.md).
-__device__ __noinline__ bool bs_pair_factor(double r2, double gmj, int nlevels, double rci0, double rci1, double rci2, double rci3,
-                                            double rcj0, double rcj1, double rcj2, double rcj3, double& s)
+__device__ __forceinline__ bool bs_pair_factor_inline(double r2, double gmj, int nlevels, double rci0, double rci1, double rci2,
+                                                      double rci3, double rcj0, double rcj1, double rcj2, double rcj3, double& s)
 {
     const double r = sqrt(r2);
     double W = 1.0;
@@ -155,6 +155,13 @@ __device__ __noinline__ bool bs_pair_factor(double r2, double gmj, int nlevels, 
     if (W == 0.0) return false;
     s = gmj * W / (r2 * r);
     return true;
+}
+// (the whole-grid kernels, which name a pair in the all-pairs fallback of every lane count, take it out of line; the warp,
+// CTA and cluster regimes, each with one pair loop, inline it)
+__device__ __noinline__ bool bs_pair_factor(double r2, double gmj, int nlevels, double rci0, double rci1, double rci2, double rci3,
+                                            double rcj0, double rcj1, double rcj2, double rcj3, double& s)
+{
+    return bs_pair_factor_inline(r2, gmj, nlevels, rci0, rci1, rci2, rci3, rcj0, rcj1, rcj2, rcj3, s);
 }
 
 // one pair term of dv_i/dt, added in place: G m_j prod_k (1 - K(r; max(rc_k,i, rc_k,j))) (q_j - q_i) / r^3.
@@ -170,9 +177,13 @@ __device__ __noinline__ bool bs_pair_factor(double r2, double gmj, int nlevels, 
         const double r2 = dx * dx + dy * dy + dz * dz;                                                 \
         if (!skip && r2 < fmax(bnd_i, (BNDJ))) {                                                       \
             double s;                                                                                  \
-            if (bs_pair_factor(r2, gmj, nlevels, rci[0], rci[1], rci[2], rci[3], RCJ(0),               \
-                               1 < nlevels ? RCJ(1) : 0.0, 2 < nlevels ? RCJ(2) : 0.0,                 \
-                               3 < nlevels ? RCJ(3) : 0.0, s)) {                                       \
+            if (MODE == GENGA_BS_MODE_COOP                                                             \
+                    ? bs_pair_factor(r2, gmj, nlevels, rci[0], rci[1], rci[2], rci[3], RCJ(0),         \
+                                     1 < nlevels ? RCJ(1) : 0.0, 2 < nlevels ? RCJ(2) : 0.0,           \
+                                     3 < nlevels ? RCJ(3) : 0.0, s)                                    \
+                    : bs_pair_factor_inline(r2, gmj, nlevels, rci[0], rci[1], rci[2], rci[3], RCJ(0),  \
+                                            1 < nlevels ? RCJ(1) : 0.0, 2 < nlevels ? RCJ(2) : 0.0,    \
+                                            3 < nlevels ? RCJ(3) : 0.0, s)) {                          \
                 AX = AX + s * dx; AY = AY + s * dy; AZ = AZ + s * dz;                                  \
             }                                                                                          \
         }                                                                                              \

@@ -10,6 +10,8 @@ Cases: kick_sym   the symmetric level-0 pair loop (mbarrier ring, hand-over coun
        bs_grid    one group of 2500 bodies on the whole grid
        kick_tp_full  configs[4] at full size (2048 + 1,048,576 particles): the one-sided pair loop at its large-N shape (profiler runs)
        steps      three merged steps of the multi-level scheme (2 levels x 2 sub-steps), N = 3000
+       multilevel_2x2  one multi-level step of configs[3] at full size, 2 levels x 2 sub-steps: one Bulirsch-Stoer group of
+                  16,823 bodies on the whole grid, four lanes per body (profiler runs)
 Each case checks its status word and prints one line."""
 import sys
 
@@ -84,6 +86,20 @@ def main(cases):
             torch.cuda.synchronize()
             assert k.status() == 0
             out = stats.cpu().tolist()
+            k.free()
+        elif c == "multilevel_2x2":
+            ki = gi.make_config(3)
+            n = ki.n
+            k = GengaKick(n, 0, max_level=1, pair_capacity=1 << 20, G=ki.G)
+            k.set_stream(torch.cuda.current_stream().cuda_stream)
+            q, v = dev(ki.pos), dev(ki.vel)
+            stats = torch.zeros(2, 4, dtype=torch.int32, device="cuda")
+            k.multilevel_step(q, v, dev(ki.mass), 1.0, ki.dt, 2, 2, 1e-12, torch.empty(3, n, dtype=torch.float64, device="cuda"),
+                              torch.empty(1 << 20, 2, dtype=torch.int32, device="cuda"),
+                              torch.empty(n + 1, dtype=torch.int32, device="cuda"), stats)
+            torch.cuda.synchronize()
+            assert k.status() == 0
+            out = (stats.cpu().tolist(), k.bs_totals())
             k.free()
         else:
             raise SystemExit(f"unknown case {c}")
