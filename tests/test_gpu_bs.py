@@ -339,6 +339,28 @@ def test_giant_group_fewer_lanes_per_body(oracle_mod):
     assert np.abs(q - ki.pos).max() > 1e-3
 
 
+@pytest.mark.parametrize("m", [20000, 40000])
+def test_giant_rings_two_and_one_lanes_per_body(m):
+    """Groups above 18,944 and above 37,888 bodies (two lanes, one lane per body: 128 and 256 bodies' lists pooled per CTA)
+    are beyond what the oracle integrates in a test's time; a ring has a check of its own: its bodies are images of one
+    another under rotation by 2 pi / m, so after the call they must still lie on one circle with one speed and the ring's
+    spacing -- a list that lost or doubled an entry, a carry added to the wrong body or a body left out would break it.
+    (Rounding differs from body to body: 1e-12.)  The same holds at 12,500 bodies, where the oracle agrees as well."""
+    for n in (12500, m):
+        ki = gi.make_ring(n)
+        q, v, st, gs = _gpu_bs(n, ki.pos, ki.vel, ki.mass, ki.rcrit, 1, 2.0, 1e-9, np.arange(n), [0, n], ki.pos, ki.vel)
+        assert st == 0 and gs[0][3] == n and gs[0][0] >= 1
+        r, sp = np.linalg.norm(q, axis=0), np.linalg.norm(v, axis=0)
+        assert np.ptp(r) <= 1e-12 * r.mean() and np.ptp(sp) <= 1e-12 * sp.mean()
+        phi = np.unwrap(np.arctan2(q[1], q[0]))
+        assert np.abs(np.diff(phi) - 2.0 * np.pi / n).max() <= 1e-12
+        assert np.abs(q[2]).max() == 0.0 and np.abs(q - ki.pos).max() > 1e-3      # planar, and it moved
+        if n == 12500:
+            ref = (r.mean(), sp.mean())
+        else:                                                  # rings of equal bodies with 8 partners each: nearly the same motion
+            assert abs(r.mean() - ref[0]) < 1e-6 and abs(sp.mean() - ref[1]) < 1e-7
+
+
 @pytest.mark.parametrize("size,count,dt,tol", [(40, 700, 3.0, 1e-10), (257, 258, 0.01, 1e-6), (600, 41, 0.5, 1e-8)])
 def test_many_mid_size_groups_are_all_found(oracle_mod, size, count, dt, tol):
     """More groups of one regime than one batch of the device-side group scan holds (256): 700 groups of 40 bodies for
