@@ -312,6 +312,39 @@ def test_semi_active_particles_in_groups(oracle_mod, tp_mode):
     assert np.abs(qf - qw).max() > 1e-9
 
 
+@pytest.mark.parametrize("tp_mode,m", [(1, 300), (2, 300), (2, 2600)])
+def test_semi_active_particles_in_a_large_group(oracle_mod, tp_mode, m):
+    """The test-particle rules in the whole-grid regime (teams and the full grid), where they decide what a body's
+    neighbour list holds: a ring in which every third body is massive and the others are semi-active particles with mass,
+    one group; against the oracle's rule, and the rule matters (TP 1, TP 2 and the fully interactive result differ)."""
+    import torch
+    from paper_2201_10058_b200 import GengaKick
+    ring = gi.make_ring(m)
+    n_m = m // 3
+    order = np.concatenate([np.arange(0, 3 * n_m, 3), np.setdiff1d(np.arange(m), np.arange(0, 3 * n_m, 3))])
+    pos, vel = np.ascontiguousarray(ring.pos[:, order]), np.ascontiguousarray(ring.vel[:, order])
+    mass = np.full(m, 3e-7); mass[n_m:] = 1e-7 * (0.5 + gi.uniforms(23, 0, m - n_m))
+    rc = np.ascontiguousarray(ring.rcrit[:1] * 1.5)
+    members, offsets = np.arange(m), [0, m]
+    k = GengaKick(n_m, m - n_m, G=G, pair_capacity=8, tp_mode=tp_mode)
+    k.set_stream(torch.cuda.current_stream().cuda_stream)
+    d_sum = torch.tensor([1, m, m, 0], dtype=torch.int32, device="cuda")
+    d_off = torch.zeros(m + 4, dtype=torch.int32, device="cuda"); d_off[1] = m
+    gstats = torch.full((1, 4), -1, dtype=torch.int32, device="cuda")
+    k.bs_set_stats(gstats, 1)
+    q, v = _dev(pos), _dev(vel)
+    k.bs(_dev(pos), _dev(vel), _dev(mass), _dev(rc), 1, 1.0, 6.0, 1e-11, _dev(members.astype(np.int32)), d_off, d_sum, q, v)
+    torch.cuda.synchronize()
+    assert k.status() == 0
+    k.free()
+    qw, vw, stats, _ = oracle_mod.bs.bs(pos, vel, mass, rc, members, np.asarray(offsets), G, 1.0, 6.0, 1e-11, pos, vel,
+                                        n_massive=n_m, tp_mode=tp_mode, max_group=None)
+    _check(q.cpu().numpy(), v.cpu().numpy(), qw, vw, members, offsets, gstats.cpu().numpy(), stats, 1e-11)
+    qo, vo, _, _ = oracle_mod.bs.bs(pos, vel, mass, rc, members, np.asarray(offsets), G, 1.0, 6.0, 1e-11, pos, vel,
+                                    n_massive=n_m, tp_mode=3 - tp_mode, max_group=None)
+    assert np.abs(qo - qw).max() > 1e-10
+
+
 def test_dense_large_group_falls_back_to_all_pairs(oracle_mod):
     """A large group in which every body is inside every other's critical radius: its neighbour lists (n^2 entries) do
     not fit the team's share of the list scratch, the group is integrated over all pairs instead -- same result."""
