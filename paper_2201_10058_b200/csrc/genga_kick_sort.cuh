@@ -123,7 +123,8 @@ radix_hist_kernel(const unsigned* __restrict__ keys, int N, int shift, int bits,
     for (int d = threadIdx.x; d < nd; d += blockDim.x) counts[(size_t)d * n_blocks + blockIdx.x] = hist[d];
 }
 
-// exclusive prefix sum of counts[0..n) in place, one CTA, fixed order
+// exclusive prefix sum of counts[0..n) in place, one CTA, fixed order (integers: any order gives the same sums);
+// four consecutive elements per thread and round (16-byte loads and stores when the array allows them)
 static __global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ counts, int n)
 {
     __shared__ int wsum[32];
@@ -131,9 +132,18 @@ static __global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ cou
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int base = 0; base < n; base += 1024) {
-        const int q = base + threadIdx.x;
-        const int v = q < n ? counts[q] : 0;
+    const bool vec = (n & 3) == 0 && (reinterpret_cast<uintptr_t>(counts) & 15u) == 0;
+    for (int base = 0; base < n; base += 4096) {
+        const int q = base + 4 * threadIdx.x;
+        int e[4] = {0, 0, 0, 0};
+        if (vec) {
+            if (q < n) { const int4 v4 = *reinterpret_cast<const int4*>(counts + q); e[0] = v4.x; e[1] = v4.y; e[2] = v4.z; e[3] = v4.w; }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; k++)
+                if (q + k < n) e[k] = counts[q + k];
+        }
+        const int v = e[0] + e[1] + e[2] + e[3];
         int s = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -153,7 +163,15 @@ static __global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ cou
         }
         __syncthreads();
         const int before = carry + (w ? wsum[w - 1] : 0) + s - v;
-        if (q < n) counts[q] = before;
+        const int x0 = before, x1 = x0 + e[0], x2 = x1 + e[1], x3 = x2 + e[2];
+        if (vec) {
+            if (q < n) *reinterpret_cast<int4*>(counts + q) = make_int4(x0, x1, x2, x3);
+        } else {
+            if (q < n) counts[q] = x0;
+            if (q + 1 < n) counts[q + 1] = x1;
+            if (q + 2 < n) counts[q + 2] = x2;
+            if (q + 3 < n) counts[q + 3] = x3;
+        }
         __syncthreads();
         if (threadIdx.x == 1023) carry = before + v;
         __syncthreads();
