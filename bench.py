@@ -55,7 +55,8 @@ FLOPS_PER_PAIR = 24
 SYM_FP64_INSTR_PER_UNORDERED_PAIR = 20
 SYM_FLOPS_PER_UNORDERED_PAIR = 31
 FP64_LANES_PER_SM = 64           # 148 SMs x 64 lanes x 2 flops x clocks.max.sm
-# From the ncu captures of round 2 (profiles/ncu_r02a.md), per launch / per two-level step at N = 65,536 (rank 0's disk);
+# From the ncu captures of round 2 (profiles/ncu_r02a.md: kick_sym_kernel; profiles/ncu_r02c.md: the step's flop counters),
+# per launch / per two-level step at N = 65,536 (rank 0's disk);
 # constants read off those captures, not measured in this run:
 NCU_DRAM_BYTES_PER_LAUNCH = 4204288        # kick_sym_kernel: dram__bytes_read.sum 2,497,536 + dram__bytes_write.sum 1,706,752
 NCU_EXECUTED_FLOPS_PER_STEP = 67657959455  # DADD + DMUL + 2 DFMA thread instructions of every kernel of one step (flops_r02c.csv)
@@ -680,7 +681,7 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                          "whole_step_frac_executed_flops": (exec_flops if NCU_EXECUTED_FLOPS_PER_STEP is None
                                                             else NCU_EXECUTED_FLOPS_PER_STEP) / (step_ms * 1e-3) / 1e12 / peak_nominal,
                          "whole_step_what": "executed FP64 flops of every kernel of one two-level step (ncu's executed "
-                                            "DADD / DMUL / DFMA counters, profiles/ncu_r02a.md; the pair loop's static count "
+                                            "DADD / DMUL / DFMA counters, profiles/ncu_r02c.md; the pair loop's static count "
                                             "if no capture is recorded) / step time / peak",
                          "algorithmic_flops_per_ordered_pair": FLOPS_PER_PAIR,
                          "executed_flops_per_unordered_pair": SYM_FLOPS_PER_UNORDERED_PAIR if sym else 2 * FLOPS_PER_PAIR,
