@@ -17,7 +17,7 @@
 namespace genga {
 
 #define GENGA_SORT_THREADS 256
-#define GENGA_SORT_ITEMS 16                                   // per thread
+#define GENGA_SORT_ITEMS 4                                    // per thread (64 sort CTAs at N = 65,536: 16 items left the SMs idle)
 #define GENGA_SORT_BLOCK (GENGA_SORT_THREADS * GENGA_SORT_ITEMS)
 #define GENGA_SORT_MAXDIGITS 512
 #define GENGA_GRID_BITS 8
