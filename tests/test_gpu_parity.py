@@ -257,6 +257,28 @@ def test_list_reuse_across_levels(oracle_mod, tp_mode, n, n_test):
     k.free()
 
 
+def test_reuse_setting_is_validated_and_a_level_without_a_list_searches(oracle_mod):
+    """genga_kick_set_order_reuse takes 0, 1 or 2; with GENGA_KICK_REUSE_LIST a level >= 1 kick that finds no level-0
+    list at hand (the first call on the context; a level-1 kick in between has replaced the list) searches itself."""
+    from paper_2201_10058_b200 import GengaKick, GengaKickError, E_SIZE
+    ki = gi.make_config(3, n=5000, level=1)
+    k = GengaKick(ki.n, 0, max_level=1, pair_capacity=1 << 18, G=ki.G)
+    for bad in (-1, 3):
+        with pytest.raises(GengaKickError) as e:
+            k.set_order_reuse(bad)
+        assert e.value.code == E_SIZE
+    fresh = run_gpu(ki, level=1)
+    k.set_order_reuse(2)
+    first = run_gpu(ki, level=1, kick=k)                     # no level-0 kick yet on this context
+    run_gpu(ki, level=0, kick=k)
+    kept = run_gpu(ki, level=1, kick=k)                      # on the level-0 list
+    again = run_gpu(ki, level=1, kick=k)                     # still on it (a kick on a kept list writes none)
+    for got in (first, kept, again):
+        assert got.status == 0 and np.array_equal(got.acc, fresh.acc) and np.array_equal(got.counts, fresh.counts)
+        assert np.array_equal(sorted_pairs(got.pairs), sorted_pairs(fresh.pairs))
+    k.free()
+
+
 def test_internal_order_is_invisible(oracle_mod):
     """Caller's order, sorted order and auto give the same pair set and counts; accelerations agree
     to the rounding of a different summation order."""
