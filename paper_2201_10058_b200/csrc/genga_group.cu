@@ -14,7 +14,7 @@ int ensure_group_scratch(genga_kick_ctx* ctx)
 {
     if (ctx->grp_label) return GENGA_KICK_OK;
     const size_t N = (size_t)ctx->N;
-    const size_t nb = (N + GENGA_SORT_BLOCK - 1) / GENGA_SORT_BLOCK;
+    const size_t nb = (N + genga::genga_sort_block((long long)N) - 1) / genga::genga_sort_block((long long)N);
     GK_CUDA(ctx, cudaMalloc(&ctx->grp_label, N * sizeof(int)));
     GK_CUDA(ctx, cudaMalloc(&ctx->grp_flag, N * sizeof(int)));
     GK_CUDA(ctx, cudaMalloc(&ctx->grp_keys_a, N * sizeof(unsigned)));
@@ -63,15 +63,15 @@ int genga_group_impl(genga_kick_ctx* ctx, const int32_t* pairs, const int32_t* n
     // stable LSD radix sort of (key, body) by key in [0, N]: digits of at most 9 bits (GENGA_SORT_MAXDIGITS)
     int key_bits = 1;
     while ((1ll << key_bits) <= (long long)N) key_bits++;
-    const int nb = (N + GENGA_SORT_BLOCK - 1) / GENGA_SORT_BLOCK;
+    const int sb = genga::genga_sort_block(N), nb = (N + sb - 1) / sb;
     unsigned *ka = ctx->grp_keys_a, *kb = ctx->grp_keys_b;
     int *va = ctx->grp_vals_a, *vb = ctx->grp_vals_b;
     const int passes = (key_bits + 8) / 9;
     for (int pass = 0, shift = 0; pass < passes; pass++) {
         const int bits = (key_bits - shift + (passes - pass) - 1) / (passes - pass);      // spread the bits evenly
-        genga::radix_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ka, N, shift, bits, nb, ctx->grp_counts);
+        genga::radix_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ka, N, shift, bits, nb, ctx->grp_counts, sb);
         genga::scan_kernel<<<1, 1024, 0, st>>>(ctx->grp_counts, (1 << bits) * nb);
-        genga::radix_scatter_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ka, va, N, shift, bits, nb, ctx->grp_counts, kb, vb);
+        genga::radix_scatter_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ka, va, N, shift, bits, nb, ctx->grp_counts, kb, vb, sb);
         std::swap(ka, kb);
         std::swap(va, vb);
         shift += bits;

@@ -93,7 +93,7 @@ extern "C" int genga_kick_init(const genga_kick_config* cfg, genga_kick_ctx** ou
         ctx->sorted = cfg->order_mode == GENGA_KICK_ORDER_SORTED ||
                       (cfg->order_mode == GENGA_KICK_ORDER_AUTO && N >= GENGA_SORT_MIN_BODIES);
         if (ctx->sorted) {
-            ctx->sort_blocks = (int)((N + GENGA_SORT_BLOCK - 1) / GENGA_SORT_BLOCK);
+            ctx->sort_blocks = (int)((N + genga::genga_sort_block(N) - 1) / genga::genga_sort_block(N));
             const size_t nc = (size_t)GENGA_SORT_MAXDIGITS * ctx->sort_blocks;
             if ((e = cudaMalloc(&ctx->bbox, 4 * sizeof(unsigned))) != cudaSuccess) goto cuda_error;
             if ((e = cudaMalloc(&ctx->keys_a, (size_t)N * sizeof(unsigned))) != cudaSuccess) goto cuda_error;
@@ -213,18 +213,18 @@ int kick_front(genga_kick_ctx* ctx, const double* pos, const double* mass, const
 
     if (ctx->sorted && !(ctx->reuse_order && ctx->order_valid)) {
         // stable LSD radix sort of the 17-bit keys: digits of 8 and 9 bits
-        const int nb = ctx->sort_blocks;
+        const int nb = ctx->sort_blocks, sb = genga::genga_sort_block(N);
         genga::sort_init_kernel<<<1, 32, 0, st>>>(ctx->bbox);
         genga::bbox_kernel<<<std::min((N + 255) / 256, 8 * ctx->num_sms), 256, 0, st>>>(pos, N, ctx->bbox);
         genga::key_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(pos, N, ctx->cfg.n_massive, ctx->bbox, ctx->keys_a,
-                                                                  ctx->vals_a, 8, nb, ctx->counts);
+                                                                  ctx->vals_a, 8, nb, ctx->counts, sb);
         genga::scan_kernel<<<1, 1024, 0, st>>>(ctx->counts, 256 * nb);
         genga::radix_scatter_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_a, ctx->vals_a, N, 0, 8, nb, ctx->counts,
-                                                                       ctx->keys_b, ctx->vals_b);
-        genga::radix_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_b, N, 8, 9, nb, ctx->counts);
+                                                                       ctx->keys_b, ctx->vals_b, sb);
+        genga::radix_hist_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_b, N, 8, 9, nb, ctx->counts, sb);
         genga::scan_kernel<<<1, 1024, 0, st>>>(ctx->counts, 512 * nb);
         genga::radix_scatter_kernel<<<nb, GENGA_SORT_THREADS, 0, st>>>(ctx->keys_b, ctx->vals_b, N, 8, 9, nb, ctx->counts,
-                                                                       nullptr, ctx->vals_a);
+                                                                       nullptr, ctx->vals_a, sb);
         GK_CUDA(ctx, cudaGetLastError());
         ctx->launches += 8;
         ctx->order_valid = true;

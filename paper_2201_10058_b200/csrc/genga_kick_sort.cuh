@@ -17,8 +17,9 @@
 namespace genga {
 
 #define GENGA_SORT_THREADS 256
-#define GENGA_SORT_ITEMS 4                                    // per thread (64 sort CTAs at N = 65,536: 16 items left the SMs idle)
-#define GENGA_SORT_BLOCK (GENGA_SORT_THREADS * GENGA_SORT_ITEMS)
+// keys per sort CTA: 1024 up to 2^18 bodies (64 CTAs per pass at N = 65,536: blocks of 4096 left the SMs idle), 4096
+// beyond (the single-CTA scan of digits x blocks counters is what grows with the number of blocks)
+static inline int genga_sort_block(long long n) { return n > (1LL << 18) ? 4096 : 1024; }
 #define GENGA_SORT_MAXDIGITS 512
 #define GENGA_GRID_BITS 8
 
@@ -82,7 +83,7 @@ __device__ __forceinline__ unsigned hilbert_index(unsigned x, unsigned y)
 // key of body b; counts of the first digit per sort block
 static __global__ void __launch_bounds__(GENGA_SORT_THREADS)
 key_hist_kernel(const double* __restrict__ pos, int N, int n_massive, const unsigned* __restrict__ bbox,
-                unsigned* __restrict__ keys, int* __restrict__ vals, int bits, int n_blocks, int* __restrict__ counts)
+                unsigned* __restrict__ keys, int* __restrict__ vals, int bits, int n_blocks, int* __restrict__ counts, int block)
 {
     __shared__ int hist[GENGA_SORT_MAXDIGITS];
     const int nd = 1 << bits;
@@ -91,8 +92,8 @@ key_hist_kernel(const double* __restrict__ pos, int N, int n_massive, const unsi
     const float x0 = ord2f(bbox[0]), y0 = ord2f(bbox[1]), x1 = ord2f(bbox[2]), y1 = ord2f(bbox[3]);
     const float cells = (float)(1 << GENGA_GRID_BITS);
     const float sx = x1 > x0 ? cells / (x1 - x0) : 0.0f, sy = y1 > y0 ? cells / (y1 - y0) : 0.0f;
-    const int base = blockIdx.x * GENGA_SORT_BLOCK;
-    for (int q = threadIdx.x; q < GENGA_SORT_BLOCK; q += blockDim.x) {
+    const int base = blockIdx.x * block;
+    for (int q = threadIdx.x; q < block; q += blockDim.x) {
         const int b = base + q;
         if (b < N) {
             const float fx = ((float)pos[b] - x0) * sx, fy = ((float)pos[(size_t)N + b] - y0) * sy;
@@ -110,14 +111,15 @@ key_hist_kernel(const double* __restrict__ pos, int N, int n_massive, const unsi
 }
 
 static __global__ void __launch_bounds__(GENGA_SORT_THREADS)
-radix_hist_kernel(const unsigned* __restrict__ keys, int N, int shift, int bits, int n_blocks, int* __restrict__ counts)
+radix_hist_kernel(const unsigned* __restrict__ keys, int N, int shift, int bits, int n_blocks, int* __restrict__ counts,
+                  int block)
 {
     __shared__ int hist[GENGA_SORT_MAXDIGITS];
     const int nd = 1 << bits;
     for (int d = threadIdx.x; d < nd; d += blockDim.x) hist[d] = 0;
     __syncthreads();
-    const int base = blockIdx.x * GENGA_SORT_BLOCK;
-    for (int q = threadIdx.x; q < GENGA_SORT_BLOCK; q += blockDim.x)
+    const int base = blockIdx.x * block;
+    for (int q = threadIdx.x; q < block; q += blockDim.x)
         if (base + q < N) atomicAdd(&hist[(keys[base + q] >> shift) & (nd - 1)], 1);
     __syncthreads();
     for (int d = threadIdx.x; d < nd; d += blockDim.x) counts[(size_t)d * n_blocks + blockIdx.x] = hist[d];
@@ -185,16 +187,16 @@ static __global__ void __launch_bounds__(1024) scan_kernel(int* __restrict__ cou
 static __global__ void __launch_bounds__(GENGA_SORT_THREADS)
 radix_scatter_kernel(const unsigned* __restrict__ keys_in, const int* __restrict__ vals_in, int N, int shift, int bits,
                      int n_blocks, const int* __restrict__ offsets, unsigned* __restrict__ keys_out,
-                     int* __restrict__ vals_out)
+                     int* __restrict__ vals_out, int block)
 {
     constexpr int WARPS = GENGA_SORT_THREADS / 32;
-    constexpr int PER_WARP = GENGA_SORT_BLOCK / WARPS;
+    const int PER_WARP = block / WARPS;
     __shared__ int whist[WARPS][GENGA_SORT_MAXDIGITS];
     const int nd = 1 << bits;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (int d = threadIdx.x; d < WARPS * GENGA_SORT_MAXDIGITS; d += blockDim.x) (&whist[0][0])[d] = 0;
     __syncthreads();
-    const int wbase = blockIdx.x * GENGA_SORT_BLOCK + w * PER_WARP;
+    const int wbase = blockIdx.x * block + w * PER_WARP;
     for (int r = 0; r < PER_WARP; r += 32) {
         const int q = wbase + r + lane;
         if (q < N) atomicAdd(&whist[w][(keys_in[q] >> shift) & (nd - 1)], 1);    // a count: order-free
